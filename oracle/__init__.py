@@ -1,0 +1,146 @@
+"""ORACLE -- TEST INFRASTRUCTURE ONLY (never imported by the product package).
+
+Plain CPU definition of the batched y-direction tridiagonal solve, used by ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs.
+
+  * ``solve_y(a, b, c, d, precision="f64"|"ld")``  -- textbook Thomas per line
+    (problem statement PAPER.md:127-131, 210), implemented in
+    ``thomas_oracle.c`` (gcc, fp-contraction off so no FMA sneaks in).
+  * ``residual_y`` / ``apply_y``                   -- long-double residual and d = A x.
+  * ``thomas_line``                                -- the same recurrence as a pure-Python loop
+    for one small line (brute-force cross-checks).
+
+Parity status: pinned (tests/test_oracle_pins.py): dense LAPACK solve n<=32, banded LAPACK,
+manufactured solutions, Toeplitz closed forms (eigen-form and Green's function), identity /
+diagonal / n=1,2 degenerate cases, long-double vs fp64 agreement.  The paper prints no worked
+numerical example (Figs. 3-4 are images), so there is no paper-value pin.
+
+Nothing here imports or links anything from ``paper_2509_03933_b200``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "thomas_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile thomas_oracle.c -> liboracle.so (gcc -O2 -fopenmp -ffp-contract=off)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    tmp = _LIB + ".tmp.%d" % os.getpid()
+    cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+           "-o", tmp, _SRC, "-lm"]
+    subprocess.run(cmd, check=True, capture_output=True, text=True)
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.oracle_solve_y.argtypes = [ctypes.c_int] * 3 + [dp] * 5 + [ctypes.c_int]
+        lib.oracle_solve_y.restype = ctypes.c_int
+        lib.oracle_residual_y.argtypes = [ctypes.c_int] * 3 + [dp] * 9
+        lib.oracle_residual_y.restype = ctypes.c_int
+        lib.oracle_apply_y.argtypes = [ctypes.c_int] * 3 + [dp] * 5
+        lib.oracle_apply_y.restype = ctypes.c_int
+        lib.oracle_max_threads.restype = ctypes.c_int
+        lib.oracle_set_threads.argtypes = [ctypes.c_int]
+        _lib = lib
+    return _lib
+
+
+def _as3(arr) -> np.ndarray:
+    out = np.ascontiguousarray(np.asarray(arr, dtype=np.float64))
+    if out.ndim != 3:
+        raise ValueError("expected an array of shape (nz, ny, nx)")
+    return out
+
+
+def _ptr(arr: np.ndarray):
+    return arr.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def max_threads() -> int:
+    return int(_load().oracle_max_threads())
+
+
+def set_threads(n: int) -> None:
+    _load().oracle_set_threads(int(n))
+
+
+def solve_y(a, b, c, d, precision: str = "f64") -> np.ndarray:
+    """x with A x = d for every y-line; arrays of shape (nz, ny, nx), x fastest."""
+    a, b, c, d = map(_as3, (a, b, c, d))
+    if not (a.shape == b.shape == c.shape == d.shape):
+        raise ValueError("a, b, c, d must have the same shape")
+    nz, ny, nx = a.shape
+    x = np.empty_like(d)
+    use_ld = {"f64": 0, "ld": 1}[precision]
+    rc = _load().oracle_solve_y(nx, ny, nz, _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(x), use_ld)
+    if rc != 0:
+        raise RuntimeError("oracle_solve_y failed (%d)" % rc)
+    return x
+
+
+def residual_y(a, b, c, d, x) -> Tuple[np.ndarray, np.ndarray, np.ndarray, np.ndarray]:
+    """Per line (shape (nz, nx)): ||Ax-d||_inf, ||d||_inf, ||x||_inf, ||A||_inf; long double."""
+    a, b, c, d, x = map(_as3, (a, b, c, d, x))
+    nz, ny, nx = a.shape
+    outs = [np.empty((nz, nx), dtype=np.float64) for _ in range(4)]
+    rc = _load().oracle_residual_y(nx, ny, nz, _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(x),
+                                   *[_ptr(o) for o in outs])
+    if rc != 0:
+        raise RuntimeError("oracle_residual_y failed (%d)" % rc)
+    return tuple(outs)
+
+
+def apply_y(a, b, c, x) -> np.ndarray:
+    """d = A x per line, accumulated in long double and rounded once."""
+    a, b, c, x = map(_as3, (a, b, c, x))
+    nz, ny, nx = a.shape
+    d = np.empty_like(x)
+    rc = _load().oracle_apply_y(nx, ny, nz, _ptr(a), _ptr(b), _ptr(c), _ptr(x), _ptr(d))
+    if rc != 0:
+        raise RuntimeError("oracle_apply_y failed (%d)" % rc)
+    return d
+
+
+def thomas_line(a: Sequence[float], b: Sequence[float], c: Sequence[float],
+                d: Sequence[float]) -> list:
+    """Thomas algorithm for ONE line as a pure-Python loop; tiny inputs only."""
+    n = len(b)
+    cp = [0.0] * n
+    dp = [0.0] * n
+    cp[0] = (c[0] / b[0]) if n > 1 else 0.0
+    dp[0] = d[0] / b[0]
+    for j in range(1, n):
+        den = b[j] - a[j] * cp[j - 1]
+        cp[j] = (c[j] / den) if j < n - 1 else 0.0
+        dp[j] = (d[j] - a[j] * dp[j - 1]) / den
+    x = [0.0] * n
+    x[n - 1] = dp[n - 1]
+    for j in range(n - 2, -1, -1):
+        x[j] = dp[j] - cp[j] * x[j + 1]
+    return x
+
+
+def normwise_error(x: np.ndarray, x_ref: np.ndarray) -> np.ndarray:
+    """Per-line E = ||x - x_ref||_inf / ||x_ref||_inf, shape (nz, nx).
+    Lines whose reference is identically zero report the absolute error."""
+    x, x_ref = _as3(x), _as3(x_ref)
+    num = np.max(np.abs(x - x_ref), axis=1)
+    den = np.max(np.abs(x_ref), axis=1)
+    return np.where(den > 0, num / np.where(den > 0, den, 1.0), num)

@@ -1,0 +1,323 @@
+"""Pins for the CPU oracle: the oracle is checked against things
+other than itself before any CUDA result is compared with it.
+
+  P1  dense brute force: Gaussian elimination with partial pivoting in long double written out
+      here, and LAPACK dgesv (np.linalg.solve), n <= 32, NON-symmetric matrices (a != c) so a
+      transposed operand fails
+  P1b banded LAPACK (scipy.linalg.solve_banded) on Poisson-type and random lines up to n = 256
+  P2  manufactured solutions: choose x*, form d = A x* with numpy long double, recover x*
+  P3  residual ||Ax-d||_inf (evaluated here independently of the oracle's own evaluator)
+  P4  closed forms of the constant-coefficient Toeplitz system a=c=-alpha, b=1+2alpha:
+      eigen-form (sine modes) and Green's function; plus the exact rational inverse of the
+      second-difference matrix tridiag(-1,2,-1) from tests/golden/second_difference_inverse.txt
+  P7  degenerate cases: identity, diagonal, n = 1, n = 2, nx = 1, nz = 1, ignored a_0 / c_{n-1}
+No paper-printed worked example exists (Figs. 3-4 are images).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import scipy.linalg
+
+import oracle
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LD = np.longdouble
+PI_LD = np.longdouble("3.14159265358979323846264338327950288")
+
+
+# ----------------------------------------------------------------------------------------------
+# helpers written independently of oracle/
+# ----------------------------------------------------------------------------------------------
+def dense_from_line(a, b, c):
+    n = len(b)
+    A = np.zeros((n, n), dtype=LD)
+    for j in range(n):
+        A[j, j] = b[j]
+        if j > 0:
+            A[j, j - 1] = a[j]
+        if j < n - 1:
+            A[j, j + 1] = c[j]
+    return A
+
+
+def gauss_partial_pivot_ld(A, d):
+    """Textbook Gaussian elimination with partial pivoting, long double."""
+    A = np.array(A, dtype=LD)
+    y = np.array(d, dtype=LD)
+    n = len(y)
+    for col in range(n):
+        piv = col + int(np.argmax(np.abs(A[col:, col])))
+        if piv != col:
+            A[[col, piv]] = A[[piv, col]]
+            y[[col, piv]] = y[[piv, col]]
+        for row in range(col + 1, n):
+            f = A[row, col] / A[col, col]
+            if f != 0:
+                A[row, col:] -= f * A[col, col:]
+                y[row] -= f * y[col]
+    x = np.zeros(n, dtype=LD)
+    for row in range(n - 1, -1, -1):
+        x[row] = (y[row] - np.dot(A[row, row + 1:], x[row + 1:])) / A[row, row]
+    return x
+
+
+def random_lines(rng, nz, ny, nx, dominant=True):
+    a = rng.uniform(-1, 1, (nz, ny, nx))
+    c = rng.uniform(-1, 1, (nz, ny, nx))
+    if dominant:
+        b = 2.0 + np.abs(a) + np.abs(c) + rng.uniform(0, 1, (nz, ny, nx))
+        b *= rng.choice([-1.0, 1.0], (nz, 1, nx))          # both signs of the diagonal
+    else:
+        b = rng.uniform(2.5, 4.0, (nz, ny, nx))
+    d = rng.uniform(-1, 1, (nz, ny, nx))
+    return a, b, c, d
+
+
+def apply_ld(a, b, c, x):
+    """d = A x along axis 1 in numpy long double (a_0, c_{n-1} ignored)."""
+    a, b, c, x = (np.asarray(v, dtype=LD) for v in (a, b, c, x))
+    out = b * x
+    out[:, 1:, :] += a[:, 1:, :] * x[:, :-1, :]
+    out[:, :-1, :] += c[:, :-1, :] * x[:, 1:, :]
+    return out
+
+
+def rel_inf(x, ref):
+    ref = np.asarray(ref, dtype=np.float64)
+    return float(np.max(np.abs(np.asarray(x, dtype=np.float64) - ref)) / np.max(np.abs(ref)))
+
+
+# ----------------------------------------------------------------------------------------------
+# P1 dense brute force
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 8, 16, 31, 32])
+@pytest.mark.parametrize("precision", ["f64", "ld"])
+def test_p1_dense_gauss_long_double(n, precision):
+    rng = np.random.default_rng(100 + n)
+    nz, nx = 2, 3
+    a, b, c, d = random_lines(rng, nz, n, nx)
+    x = oracle.solve_y(a, b, c, d, precision)
+    for k in range(nz):
+        for i in range(nx):
+            A = dense_from_line(a[k, :, i], b[k, :, i], c[k, :, i])
+            ref = gauss_partial_pivot_ld(A, d[k, :, i])
+            assert rel_inf(x[k, :, i], ref) <= 1e-14
+
+
+@pytest.mark.parametrize("n", [4, 17, 32])
+def test_p1_dense_lapack(n):
+    rng = np.random.default_rng(7 + n)
+    a, b, c, d = random_lines(rng, 3, n, 4, dominant=False)      # not strictly dominant either
+    x = oracle.solve_y(a, b, c, d)
+    for k in range(3):
+        for i in range(4):
+            A = dense_from_line(a[k, :, i], b[k, :, i], c[k, :, i]).astype(np.float64)
+            ref = np.linalg.solve(A, d[k, :, i])
+            assert rel_inf(x[k, :, i], ref) <= 5e-13
+
+
+def test_p1_pure_python_loop_matches_c():
+    rng = np.random.default_rng(3)
+    a, b, c, d = random_lines(rng, 1, 24, 2)
+    x = oracle.solve_y(a, b, c, d)
+    for i in range(2):
+        ref = oracle.thomas_line(list(a[0, :, i]), list(b[0, :, i]), list(c[0, :, i]), list(d[0, :, i]))
+        # same recurrence, same precision, no FMA contraction on either side: bit-identical
+        assert np.array_equal(x[0, :, i], np.array(ref))
+
+
+def test_p1b_banded_lapack_poisson_lines():
+    """Poisson-type line: stretched-grid weights, b = -(a+c) - k^2 (weakly dominant)."""
+    import tdma_inputs
+    ny = 256
+    a_y, c_y = tdma_inputs.poisson_y_coefficients(ny, 2.0)
+    a_y, c_y = a_y.numpy(), c_y.numpy()
+    rng = np.random.default_rng(11)
+    k2 = np.array([0.5, 3.0, 40.0, 1.0e4])
+    nx = len(k2)
+    a = np.broadcast_to(a_y[None, :, None], (1, ny, nx)).copy()
+    c = np.broadcast_to(c_y[None, :, None], (1, ny, nx)).copy()
+    b = -(a + c) - k2[None, None, :]
+    d = rng.standard_normal((1, ny, nx))
+    x = oracle.solve_y(a, b, c, d)
+    xl = oracle.solve_y(a, b, c, d, "ld")
+    for i in range(nx):
+        ab = np.zeros((3, ny))
+        ab[0, 1:] = c[0, :-1, i]
+        ab[1, :] = b[0, :, i]
+        ab[2, :-1] = a[0, 1:, i]
+        ref = scipy.linalg.solve_banded((1, 1), ab, d[0, :, i])
+        assert rel_inf(x[0, :, i], ref) <= 1e-10 / max(k2[i], 1.0) + 1e-12
+        assert rel_inf(x[0, :, i], xl[0, :, i]) <= 1e-10 / max(k2[i], 1.0) + 1e-12
+
+
+# ----------------------------------------------------------------------------------------------
+# P2 manufactured solutions, P3 residual
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("shape", [(2, 64, 5), (1, 257, 3), (3, 1024, 2)])
+def test_p2_manufactured_solution(shape):
+    rng = np.random.default_rng(sum(shape))
+    nz, ny, nx = shape
+    a, b, c, _ = random_lines(rng, nz, ny, nx)
+    xstar = rng.uniform(-1, 1, shape)
+    d = apply_ld(a, b, c, xstar).astype(np.float64)
+    for precision in ("f64", "ld"):
+        x = oracle.solve_y(a, b, c, d, precision)
+        err = oracle.normwise_error(x, xstar)
+        assert err.max() <= 5e-15                     # cond <= ~3.5 for these lines
+    # the oracle's own A x evaluator agrees with the numpy long double one
+    assert np.array_equal(oracle.apply_y(a, b, c, xstar), d)
+
+
+def test_p3_residual_and_evaluator():
+    rng = np.random.default_rng(5)
+    a, b, c, d = random_lines(rng, 2, 96, 7)
+    x = oracle.solve_y(a, b, c, d)
+    r_here = np.max(np.abs(apply_ld(a, b, c, x) - d.astype(LD)), axis=1).astype(np.float64)
+    res, dinf, xinf, ainf = oracle.residual_y(a, b, c, d, x)
+    assert np.allclose(res, r_here, rtol=1e-6, atol=1e-19)
+    assert np.allclose(dinf, np.max(np.abs(d), axis=1))
+    assert np.allclose(xinf, np.max(np.abs(x), axis=1))
+    a0 = a.copy(); a0[:, 0, :] = 0
+    c0 = c.copy(); c0[:, -1, :] = 0
+    assert np.allclose(ainf, np.max(np.abs(a0) + np.abs(b) + np.abs(c0), axis=1))
+    assert (res <= 1e-15 * np.maximum(dinf, 1e-300) * 10).all()      # literal bound, dominant lines
+    # a deliberately wrong x is seen by the evaluator
+    xb = x.copy(); xb[0, 10, 3] += 1e-6
+    res_b = oracle.residual_y(a, b, c, d, xb)[0]
+    assert res_b[0, 3] > 1e-7
+
+
+# ----------------------------------------------------------------------------------------------
+# P4 Toeplitz closed forms
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("alpha", [0.1, 1.0, 7.3])
+@pytest.mark.parametrize("n", [8, 64, 512])
+def test_p4_toeplitz_eigenform(alpha, n):
+    """d_j = sin(pi q j/(n+1)), j=1..n  =>  x = d / lambda_q,
+    lambda_q = 1 + 2 alpha - 2 alpha cos(pi q/(n+1))."""
+    qs = [1, 2, n // 2, n]
+    nx = len(qs)
+    j = np.arange(1, n + 1, dtype=LD)
+    a = np.full((1, n, nx), -alpha)
+    c = np.full((1, n, nx), -alpha)
+    b = np.full((1, n, nx), 1 + 2 * alpha)
+    d = np.zeros((1, n, nx))
+    ref = np.zeros((1, n, nx))
+    for col, q in enumerate(qs):
+        mode = np.sin(PI_LD * q * j / (n + 1))
+        lam = 1 + 2 * LD(alpha) - 2 * LD(alpha) * np.cos(PI_LD * q / (n + 1))
+        d[0, :, col] = mode.astype(np.float64)
+        ref[0, :, col] = (d[0, :, col].astype(LD) / lam).astype(np.float64)
+    x = oracle.solve_y(a, b, c, d)
+    # d was rounded to fp64 before the solve, so compare against d/lambda of the ROUNDED d
+    # up to the perturbation a 1-ulp change of d produces: cond <= 1 + 4 alpha.
+    tol = (1 + 4 * alpha) * 4e-16 * 8
+    assert oracle.normwise_error(x, ref).max() <= tol
+
+
+@pytest.mark.parametrize("alpha", [0.1, 1.0, 9.9])
+def test_p4_toeplitz_greens_function(alpha):
+    """d = e_q  =>  x_j = (r^-lo - r^lo)(r^-(n+1-hi) - r^(n+1-hi)) /
+                          (alpha (r^-1 - r)(r^-(n+1) - r^(n+1))),  lo/hi = min/max(j,q),
+    r the root < 1 of alpha r^2 - (1+2 alpha) r + alpha = 0  (1-based j, q)."""
+    n = 40
+    qs = [1, 7, 20, 40]
+    al = LD(alpha)
+    r = ((1 + 2 * al) - np.sqrt((1 + 2 * al) ** 2 - 4 * al * al)) / (2 * al)
+    nx = len(qs)
+    a = np.full((1, n, nx), -alpha)
+    c = np.full((1, n, nx), -alpha)
+    b = np.full((1, n, nx), 1 + 2 * alpha)
+    d = np.zeros((1, n, nx))
+    ref = np.zeros((1, n, nx))
+    for col, q in enumerate(qs):
+        d[0, q - 1, col] = 1.0
+        for j in range(1, n + 1):
+            lo, hi = min(j, q), max(j, q)
+            num = (r ** (-lo) - r ** lo) * (r ** (-(n + 1 - hi)) - r ** (n + 1 - hi))
+            den = al * (1 / r - r) * (r ** (-(n + 1)) - r ** (n + 1))
+            ref[0, j - 1, col] = float(num / den)
+    x = oracle.solve_y(a, b, c, d)
+    assert oracle.normwise_error(x, ref).max() <= 2e-14
+
+
+def test_p4_second_difference_inverse_golden():
+    """tests/golden/second_difference_inverse.txt: (tridiag(-1,2,-1))^-1_{ij} =
+    min(i,j)(n+1-max(i,j))/(n+1), stored as exact integers over (n+1)."""
+    path = os.path.join(HERE, "golden", "second_difference_inverse.txt")
+    rows = [ln.split() for ln in open(path) if ln.strip() and not ln.startswith("#")]
+    n = int(rows[0][0])
+    numer = np.array([[int(v) for v in r] for r in rows[1:1 + n]], dtype=np.float64)
+    assert numer.shape == (n, n)
+    a = np.full((1, n, n), -1.0)
+    c = np.full((1, n, n), -1.0)
+    b = np.full((1, n, n), 2.0)
+    d = np.zeros((1, n, n))
+    for q in range(n):
+        d[0, q, q] = 1.0                    # column q of the identity as RHS of line q
+    x = oracle.solve_y(a, b, c, d)[0]       # x[:, q] = column q of the inverse
+    assert np.max(np.abs(x * (n + 1) - numer)) <= 1e-12
+
+
+# ----------------------------------------------------------------------------------------------
+# P7 degenerate / plumbing cases
+# ----------------------------------------------------------------------------------------------
+def test_p7_identity_and_diagonal():
+    rng = np.random.default_rng(9)
+    shape = (2, 10, 3)
+    d = rng.uniform(-1, 1, shape)
+    z = np.zeros(shape)
+    assert np.array_equal(oracle.solve_y(z, np.ones(shape), z, d), d)
+    b = rng.uniform(1, 2, shape)
+    assert np.array_equal(oracle.solve_y(z, b, z, d), d / b)
+
+
+def test_p7_ignored_corner_entries():
+    rng = np.random.default_rng(10)
+    a, b, c, d = random_lines(rng, 2, 12, 3)
+    x0 = oracle.solve_y(a, b, c, d)
+    a2, c2 = a.copy(), c.copy()
+    a2[:, 0, :] = np.nan
+    c2[:, -1, :] = np.inf
+    assert np.array_equal(oracle.solve_y(a2, b, c2, d), x0)
+    assert np.array_equal(oracle.solve_y(a2, b, c2, d, "ld"), oracle.solve_y(a, b, c, d, "ld"))
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 2, 1), (1, 7, 1), (5, 7, 1), (1, 7, 5)])
+def test_p7_small_shapes(shape):
+    rng = np.random.default_rng(21)
+    nz, ny, nx = shape
+    a, b, c, d = random_lines(rng, nz, ny, nx)
+    x = oracle.solve_y(a, b, c, d)
+    for k in range(nz):
+        for i in range(nx):
+            A = dense_from_line(a[k, :, i], b[k, :, i], c[k, :, i]).astype(np.float64)
+            assert np.allclose(A @ x[k, :, i], d[k, :, i], rtol=0, atol=1e-14)
+
+
+def test_layout_is_x_fastest_lines_along_y():
+    """A line-dependent matrix: the solution of line (i,k) must only see data of that line."""
+    rng = np.random.default_rng(33)
+    a, b, c, d = random_lines(rng, 3, 9, 4)
+    x = oracle.solve_y(a, b, c, d)
+    d2 = d.copy()
+    d2[1, :, 2] += 1.0                                  # perturb one line only
+    x2 = oracle.solve_y(a, b, c, d2)
+    changed = np.any(x2 != x, axis=1)
+    expect = np.zeros((3, 4), dtype=bool)
+    expect[1, 2] = True
+    assert np.array_equal(changed, expect)
+
+
+def test_thread_count_does_not_change_bits():
+    rng = np.random.default_rng(4)
+    a, b, c, d = random_lines(rng, 4, 33, 9)
+    nmax = oracle.max_threads()
+    oracle.set_threads(1)
+    x1 = oracle.solve_y(a, b, c, d)
+    oracle.set_threads(nmax)
+    xn = oracle.solve_y(a, b, c, d)
+    assert np.array_equal(x1, xn)
