@@ -1,0 +1,401 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json metric: fp64 TDMA grid cells/s (+ achieved HBM GB/s vs peak) on the
+1024^3 y-systems workload (cfg3_weak: 1024 x 1024 x 1024, P = 16), one B200 per rank.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfg3_weak] [--variant fused|pipelined] [--batch BZ] [--nstreams S]
+                    [--sweep]           # S7 batch / stream sweep, JSON lines to stdout
+
+A "step" is one pass of the whole hot path (partition reduce -> gather -> reduced solve ->
+back-substitution, all batches) over the slab, inputs resident in HBM.  Timing: CUDA events on the
+stream the solve is launched on, bracketed by barrier + synchronize, max over ranks.  The slab
+(5 x 8 GiB) is far larger than L2 (126 MB), so no explicit L2 flush is needed between steps.
+Multi-GPU: the path shards by lines with no exchange step, so every rank solves its own slab of the
+same shape (weak scaling, no data-path collective); torch.distributed (NCCL) is used only for the
+barrier and the max-over-ranks reduction.
+
+Rank 0 prints ONE JSON line.  Extra keys: "roofline" (dominant kernel against the measured HBM
+copy bandwidth in MEASURED_PEAKS.json), "cpu_baseline" (the oracle, as it stands, on the host
+cores for a bounded sample), "e2e" (same metric through tdma_solve_host with pinned HOST buffers,
+H2D/D2H inside the timed region), "clocks", "gpu_launches", "variants".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64_tdma_grid_cells_per_s"
+UNIT = "cells/s"
+ALG_BYTES_PER_CELL = 40.0        # read a, b, c, d (32 B) + write x (8 B): SURVEY.md 8(d)
+FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu_index = gpu_index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu_index), "--query-gpu=" + self.QUERY,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); smax.append(float(r[2]))
+            except Exception:
+                continue
+            for name, val in zip(names, r[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None,
+                "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_oracle_rate(w_host, min_seconds=10.0, max_repeats=64):
+    """The oracle as it stands (OpenMP over lines, all host cores) on the given host sample."""
+    import oracle
+    arrs = [t.numpy() for t in w_host]
+    cells = arrs[0].size
+    oracle.solve_y(*arrs)                                   # warm-up (page faults, thread pool)
+    t0 = time.perf_counter()
+    reps = 0
+    while True:
+        oracle.solve_y(*arrs)
+        reps += 1
+        el = time.perf_counter() - t0
+        if el >= min_seconds or reps >= max_repeats:
+            break
+    return cells * reps / el, reps, el, oracle.max_threads()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the box's host cores, same metric / config keys."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import torch
+    import tdma_inputs
+    spec = tdma_inputs.config_spec(args.workload)
+    nzs = min(spec["nz"], args.ref_slices)
+    w = tdma_inputs.make_workload(args.workload, device="cpu", nz=nzs)
+    host = (w.a, w.b, w.c, w.d)
+    import oracle
+    arrs = [t.numpy() for t in host]
+    for _ in range(max(1, args.warmup if args.warmup <= 2 else 2)):
+        oracle.solve_y(*arrs)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.solve_y(*arrs)
+    el = time.perf_counter() - t0
+    value = w.cells * args.steps / el
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": args.workload, "nx": w.nx, "ny": w.ny, "nz": spec["nz"], "P": w.P,
+                   "sample": "each step = oracle Thomas solve of %d of the %d z-slices" % (nzs, spec["nz"])},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+                         "sample": "%d z-slices (%d cells) per step" % (nzs, w.cells)},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def time_solve(torch, plan, w, x, steps, warmup, barrier):
+    """Returns seconds per step (device time, CUDA events on the launching stream)."""
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        plan.solve(w.a, w.b, w.c, w.d, x, stream)
+    torch.cuda.synchronize()
+    barrier()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        plan.solve(w.a, w.b, w.c, w.d, x, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1) * 1e-3 / steps
+
+
+def stage_times(torch, tdma, plan, w, x, reps=3):
+    """Stage-isolated mean time per batch, PIPELINED plans."""
+    nb = plan.get(tdma.TDMA_GET_NB)
+    stream = torch.cuda.current_stream()
+    out = {}
+    for name, st in (("A", tdma.TDMA_STAGE_A), ("B", tdma.TDMA_STAGE_B), ("C", tdma.TDMA_STAGE_C)):
+        nbt = min(nb, 64)
+        for n in range(min(nbt, 4)):
+            plan.stage(st, n, w.a, w.b, w.c, w.d, x, stream)
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            for n in range(nbt):
+                plan.stage(st, n, w.a, w.b, w.c, w.d, x, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        out[name] = e0.elapsed_time(e1) * 1e-3 / (reps * nbt)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3_weak")
+    ap.add_argument("--variant", default="auto", choices=["auto", "fused", "pipelined"])
+    ap.add_argument("--batch", type=int, default=-1, help="z-slices per batch (-1: workload default)")
+    ap.add_argument("--nstreams", type=int, default=0)
+    ap.add_argument("--nz", type=int, default=0, help="restrict the slab to the first NZ slices")
+    ap.add_argument("--ref-slices", type=int, default=16)
+    ap.add_argument("--e2e-slices", type=int, default=128)
+    ap.add_argument("--cpu-seconds", type=float, default=10.0)
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e / cpu_baseline / stage legs")
+    ap.add_argument("--sweep", action="store_true", help="S7 batch x stream sweep (JSON lines)")
+    args = ap.parse_args()
+
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import tdma_inputs
+    import paper_2509_03933_b200 as tdma
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    def max_over_ranks(v: float) -> float:
+        if dist is None:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    spec = tdma_inputs.config_spec(args.workload)
+    nz = args.nz if args.nz > 0 else spec["nz"]
+    w = tdma_inputs.make_workload(args.workload, device=dev, nz=nz)
+    x = torch.empty_like(w.d)
+    batch = spec["batch"] if args.batch < 0 else args.batch
+    cells = w.cells
+    peak, peak_src = measured_peak()
+    vmap = {"fused": tdma.TDMA_VARIANT_FUSED, "pipelined": tdma.TDMA_VARIANT_PIPELINED}
+
+    if args.sweep:
+        return sweep(torch, tdma, w, x, args, barrier, rank)
+
+    # ---- candidate variants: the headline is the faster one; both are reported ---------------
+    names = ["fused", "pipelined"] if args.variant == "auto" else [args.variant]
+    results = {}
+    for name in names:
+        opts = dict(variant=vmap[name])
+        bz = batch
+        if name == "fused":
+            bz = 0 if args.batch < 0 else args.batch      # one launch covers the slab by default
+        if args.nstreams:
+            opts["nstreams"] = args.nstreams
+        try:
+            plan = tdma.Plan(w.nx, w.ny, w.nz, w.P, bz, **opts)
+        except tdma.TdmaError as exc:
+            results[name] = {"error": str(exc)}
+            continue
+        quick = time_solve(torch, plan, w, x, max(2, args.steps // 4), max(3, args.warmup), barrier)
+        results[name] = {"plan": plan, "quick_s": quick, "batch": plan.get(tdma.TDMA_GET_BATCH),
+                         "launches": plan.get(tdma.TDMA_GET_LAUNCHES),
+                         "nstreams": plan.get(tdma.TDMA_GET_NSTREAMS)}
+    ok = {k: v for k, v in results.items() if "plan" in v}
+    if not ok:
+        raise SystemExit("no variant could be planned: %r" % results)
+    best = min(ok, key=lambda k: ok[k]["quick_s"])
+    plan = ok[best]["plan"]
+
+    # ---- timed region ------------------------------------------------------------------------
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    sec = time_solve(torch, plan, w, x, args.steps, max(3, args.warmup), barrier)
+    clocks = sampler.stop() if rank == 0 else None
+    sec = max_over_ranks(sec)
+    value = cells * world / sec
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(3, args.warmup), "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "nx": w.nx, "ny": w.ny, "nz": w.nz, "P": w.P,
+                   "variant": best, "batch": ok[best]["batch"], "nstreams": ok[best]["nstreams"],
+                   "cells_per_gpu": cells, "l2": "inputs (5 x %.1f GiB) far larger than L2" % (cells * 8 / 2 ** 30),
+                   "parallelism": "lines sharded, one slab per rank, no collective"},
+        "gpu_launches": ok[best]["launches"] * args.steps,
+        "hbm_gbs_40B": ALG_BYTES_PER_CELL * cells / sec / 1e9,
+        "hbm_frac_of_8TBs": ALG_BYTES_PER_CELL * cells / sec / 8e12,
+    }
+    if clocks is not None:
+        out["clocks"] = clocks
+    out["variants"] = {k: ({"ms_per_step": v["quick_s"] * 1e3, "batch": v["batch"], "launches": v["launches"]}
+                           if "plan" in v else v) for k, v in results.items()}
+
+    # ---- roofline of the dominant kernel -----------------------------------------------------
+    if best == "fused":
+        # one kernel per batch does the whole step; its launches fill the timed region back to back
+        launches = ok[best]["launches"]
+        alg_bytes = ALG_BYTES_PER_CELL * cells / launches
+        dur = sec / launches
+        achieved = alg_bytes / dur / 1e9
+        out["roofline"] = {"bound": "hbm", "kernel": "fused_kernel", "achieved": achieved, "peak": peak,
+                           "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                           "alg_bytes_per_launch": alg_bytes, "launch_ms": dur * 1e3, "peak_source": peak_src}
+    else:
+        st = stage_times(torch, tdma, plan, w, x) if not args.no_extras else None
+        if st:
+            bz = ok[best]["batch"]
+            bcells = w.nx * w.ny * bz
+            alg_bytes = (32.0 + 24.0) * bcells + 48.0 * w.P * w.nx * bz   # read a,b,c,d; write a',c',d' + reduced rows
+            achieved = alg_bytes / st["A"] / 1e9
+            out["roofline"] = {"bound": "hbm", "kernel": "stage_a_kernel", "achieved": achieved, "peak": peak,
+                               "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                               "alg_bytes_per_launch": alg_bytes, "launch_ms": st["A"] * 1e3,
+                               "peak_source": peak_src}
+            out["stage_ms_per_batch"] = {k: v * 1e3 for k, v in st.items()}
+            nb = plan.get(tdma.TDMA_GET_NB)
+            tot_b = st["B"] * nb
+            exposed = sec - (st["A"] + st["C"]) * nb
+            out["stage_b_hidden_frac"] = 1.0 - max(0.0, exposed) / tot_b if tot_b > 0 else None
+
+    # ---- extras on rank 0, N = 1 only --------------------------------------------------------
+    if rank == 0 and world == 1 and not args.no_extras:
+        for v in ok.values():
+            if v["plan"] is not plan:
+                v["plan"].close()
+        # e2e: C ABI with pinned HOST buffers, copies inside the timed region
+        nze = min(w.nz, args.e2e_slices)
+        try:
+            host = [t[:nze].cpu().pin_memory() for t in (w.a, w.b, w.c, w.d)]
+            xh = torch.empty_like(host[3]).pin_memory()
+            bze = min(ok[best]["batch"], nze) if ok[best]["batch"] < w.nz else 0
+            with tdma.Plan(w.nx, w.ny, nze, w.P, bze, variant=vmap[best]) as hplan:
+                for _ in range(2):
+                    hplan.solve_host(*host, xh)
+                t0 = time.perf_counter()
+                reps = 3
+                for _ in range(reps):
+                    hplan.solve_host(*host, xh)
+                el = (time.perf_counter() - t0) / reps
+            ecells = w.nx * w.ny * nze
+            out["e2e"] = {"value": ecells / el, "unit": UNIT, "h2d_bytes_per_step": 32 * ecells,
+                          "d2h_bytes_per_step": 8 * ecells, "ms_per_step": el * 1e3,
+                          "sample": "first %d of %d z-slices through tdma_solve_host (pinned host buffers)" % (nze, w.nz)}
+            # cpu baseline on the same host sample (bounded)
+            nzc = min(nze, 64)
+            rate, reps, el, cores = cpu_oracle_rate([t[:nzc] for t in host], args.cpu_seconds)
+            out["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                   "sample": "%d z-slices (%d cells) x %d repeats, %.1f s" % (nzc, w.nx * w.ny * nzc, reps, el)}
+        except Exception as exc:                      # report, never hide
+            out["e2e_error"] = repr(exc)
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def sweep(torch, tdma, w, x, args, barrier, rank):
+    """S7: batch x stream sweep; one JSON line per point."""
+    nz = w.nz
+    batches = [b for b in (1, 2, 4, 8, 16, 32, 64, 128) if b <= nz]
+    points = []
+    for variant, streams_list in (("pipelined", (1, 2, 3, 4)), ("fused", (1,))):
+        for ns in streams_list:
+            for bz in batches + ([0] if variant == "fused" else []):
+                opts = dict(variant={"fused": tdma.TDMA_VARIANT_FUSED, "pipelined": tdma.TDMA_VARIANT_PIPELINED}[variant])
+                if variant == "pipelined":
+                    opts["nstreams"] = ns
+                try:
+                    with tdma.Plan(w.nx, w.ny, nz, w.P, bz, **opts) as plan:
+                        sec = time_solve(torch, plan, w, x, args.steps, max(3, args.warmup), barrier)
+                        rec = {"sweep": True, "workload": args.workload, "variant": variant, "nstreams": ns,
+                               "batch": plan.get(tdma.TDMA_GET_BATCH), "nb": plan.get(tdma.TDMA_GET_NB),
+                               "ms": sec * 1e3, "cells_per_s": w.cells / sec,
+                               "gbs_40B": 40.0 * w.cells / sec / 1e9,
+                               "workspace_MiB": plan.workspace_bytes / 2 ** 20}
+                except tdma.TdmaError as exc:
+                    rec = {"sweep": True, "variant": variant, "nstreams": ns, "batch": bz, "error": str(exc)}
+                points.append(rec)
+                if rank == 0:
+                    print(json.dumps(rec), flush=True)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

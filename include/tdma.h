@@ -1,0 +1,155 @@
+/*
+ * tdma.h -- C ABI of the B200-native Pipelined-TDMA hot path (arxiv 2509.03933).
+ *
+ * One thing is solved: for every (i,k) line of an nx*ny*nz fp64 slab, the tridiagonal system
+ *
+ *        a_j x_{j-1} + b_j x_j + c_j x_{j+1} = d_j ,     j = 0 .. ny-1
+ *
+ * ("Problem: Ax = d (N times); Input a, b, c, d; Output x", PAPER.md:127-131 / Alg. 1 and
+ * PAPER.md:169-173 / Alg. 2; a, b, c = sub-, main, super-diagonal), with the
+ * systems aligned with y (Fig. 1c) and the y direction split into P partitions
+ * (the paper's processors p).
+ *
+ * LAYOUT.  Every array holds nx*ny*nz doubles, element (i,j,k) at  i + nx*(j + ny*k)  (x fastest,
+ * then y, then z).  a at j = 0 and c at j = ny-1 are IGNORED (treated as 0); they need not be
+ * valid numbers.  A batch is a contiguous range of z-slices.
+ *
+ * OWNERSHIP.  a, b, c, d, x are caller-owned.  For tdma_solve / tdma_stage they are DEVICE
+ * pointers, for tdma_solve_host they are HOST pointers (pinned memory recommended).  Inputs are
+ * never written.  x may alias d exactly (in place); any other overlap is undefined.  The plan
+ * owns its scratch ring, reduced-system buffers, streams, events and CUDA graphs.
+ *
+ * ASYNCHRONY.  tdma_solve only enqueues work: it forks the plan's internal streams from `stream`
+ * and joins them back, so work enqueued later on `stream` sees x.  No host synchronisation
+ * inside.  One solve in flight per plan; concurrent solves need separate plans.
+ *
+ * ERRORS.  tdma_plan_create* return NULL on failure; the int-returning calls return TDMA_OK (0)
+ * or a negative tdma_status; a message for the calling thread is in tdma_last_error().
+ * There is no CPU fallback: without a CUDA device every compute call fails with TDMA_ERR_CUDA.
+ */
+#ifndef TDMA_H_
+#define TDMA_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tdma_plan tdma_plan; /* opaque, library-owned */
+
+typedef enum tdma_dtype {
+    TDMA_F64 = 0 /* the only arithmetic type of the path (BASELINE.json: fp64) */
+} tdma_dtype;
+
+typedef enum tdma_status {
+    TDMA_OK = 0,
+    TDMA_ERR_INVALID_ARG = -1,
+    TDMA_ERR_UNSUPPORTED = -2,
+    TDMA_ERR_ALLOC = -3,
+    TDMA_ERR_CUDA = -4
+} tdma_status;
+
+/* How the three compute stages of the divide-and-conquer solve (Fig. 5) are
+ * mapped onto the GPU. */
+typedef enum tdma_variant {
+    TDMA_VARIANT_AUTO = 0,
+    /* Stage A (partition reduce, fused gather) / Stage B (reduced 2P-row solve) / Stage C
+     * (back-substitution) as separate kernels, z-batches pipelined over CUDA streams with events
+     * exactly as Alg. 2: A(n) || B(n-1) || C(n-2).  The partition results
+     * travel A -> C through a plan-owned scratch ring in HBM/L2. */
+    TDMA_VARIANT_PIPELINED = 1,
+    /* One persistent kernel: a thread-block cluster owns whole lines, the partitions of a line
+     * live in the shared memory of the cluster's CTAs (the paper's ranks), the reduced system is
+     * exchanged through distributed shared memory (the paper's MPI_Alltoall) and
+     * solved inside the cluster, so HBM sees a, b, c, d once and x once (40 B/cell). */
+    TDMA_VARIANT_FUSED = 2
+} tdma_variant;
+
+/* Optional tuning knobs for tdma_plan_create_ex.  Zero-initialise, set struct_size =
+ * sizeof(tdma_options); every field set to 0 means "library default". */
+typedef struct tdma_options {
+    int struct_size;
+    int variant;         /* tdma_variant */
+    int nstreams;        /* PIPELINED: 1 = sequential Alg. 1 order on one stream; 2 = {A+C, B}
+                            (paper); 3..8 = (nstreams-1) A+C lanes + 1 B stream.
+                            default 2 */
+    int use_graph;       /* 1 = capture the schedule once per pointer set into a CUDA graph
+                            (default), -1 = plain stream launches */
+    int separate_gather; /* 1 = stage A writes a send_A buffer and a separate gather kernel
+                            assembles the reduced system (the paper's A2B);
+                            default 0 = gather fused into stage A's epilogue */
+    int fused_lines;     /* FUSED: lines (x extent) per cluster tile, 0 = auto */
+    int fused_cluster;   /* FUSED: CTAs per cluster (1, 2, 4, 8), 0 = auto */
+    int reserved[8];
+} tdma_options;
+
+/* Plan for an nx*ny*nz slab with y split into P partitions of ny/P rows and `batch` z-slices per
+ * pipeline stage (batch_z of PAPER.md:236; 0 = all slices in one batch; a last smaller batch is
+ * created when nz % batch != 0).
+ * Invalid: any dimension < 1, P < 1, ny % P != 0, ny/P < 2 when P > 1, batch < 0 or > nz,
+ * dtype != TDMA_F64.  Returns NULL and sets tdma_last_error() on failure. */
+tdma_plan *tdma_plan_create(int nx, int ny, int nz, int P, int batch, int dtype);
+tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dtype,
+                               const tdma_options *options /* may be NULL */);
+
+/* Solve all nx*nz systems.  a, b, c, d, x: DEVICE pointers to nx*ny*nz doubles (layout above).
+ * stream: a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * Enqueue-only; returns TDMA_OK or a negative status. */
+int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,
+               void *x, void *stream);
+
+/* Same solve with HOST buffers: the slab is streamed through plan-owned device staging buffers
+ * in z-chunks (H2D copy of chunk n+1 and D2H copy of chunk n-1 overlap the solve of chunk n).
+ * Blocks until x is complete on the host.  Pinned host memory gives asynchronous copies;
+ * pageable memory works but serialises. */
+int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,
+                    void *x);
+
+/* Run ONE stage of ONE batch on `stream` (stage-isolated timing as in PAPER.md:415 "each stage
+ * was timed independently", and stage-level tests).  PIPELINED plans only.  Pointers are the
+ * slab base pointers as for tdma_solve; the batch's z-range is derived from batch_index.
+ * Ring slot used: batch_index % TDMA_GET_DEPTH. */
+typedef enum tdma_stage_id {
+    TDMA_STAGE_A = 0,      /* partition reduce (+ fused gather unless separate_gather) */
+    TDMA_STAGE_GATHER = 1, /* separate gather kernel (separate_gather plans only)      */
+    TDMA_STAGE_B = 2,      /* reduced 2P-row solve                                      */
+    TDMA_STAGE_C = 3       /* back-substitution                                         */
+} tdma_stage_id;
+int tdma_stage(tdma_plan *plan, int stage, int batch_index, const void *a, const void *b,
+               const void *c, const void *d, void *x, void *stream);
+
+/* Introspection. */
+typedef enum tdma_query {
+    TDMA_GET_NB = 0,       /* number of batches, ceil(nz / batch)                   */
+    TDMA_GET_M = 1,        /* rows per partition, ny / P                            */
+    TDMA_GET_BATCH = 2,    /* effective z-slices per batch                          */
+    TDMA_GET_NSTREAMS = 3, /* internal streams used                                 */
+    TDMA_GET_DEPTH = 4,    /* scratch ring depth (batches in flight)                */
+    TDMA_GET_VARIANT = 5,  /* resolved tdma_variant                                 */
+    TDMA_GET_LAUNCHES = 6, /* kernel launches one tdma_solve enqueues               */
+    TDMA_GET_FUSED_LINES = 7,
+    TDMA_GET_FUSED_CLUSTER = 8,
+    TDMA_GET_GRAPH_BUILDS = 9 /* CUDA graphs captured so far (cache misses)        */
+} tdma_query;
+int tdma_plan_get(const tdma_plan *plan, int what); /* < 0 on error */
+size_t tdma_plan_workspace_bytes(const tdma_plan *plan); /* device bytes the plan owns */
+
+/* Device pointer + size of a plan-owned buffer of ring slot `slot` (tests only; PIPELINED).
+ * Reduced-system buffers are [2P][Lb] doubles, line fastest (Lb = nx * batch lines), unit
+ * diagonal implicit; row 2p is partition p's first-row equation, row 2p+1 its last-row
+ * equation.  Scratch buffers have the slab layout restricted to the batch. */
+typedef enum tdma_buffer_id {
+    TDMA_BUF_RA = 0, TDMA_BUF_RC = 1, TDMA_BUF_RD = 2, TDMA_BUF_Y = 3,
+    TDMA_BUF_SA = 4, TDMA_BUF_SC = 5, TDMA_BUF_SD = 6
+} tdma_buffer_id;
+int tdma_plan_buffer(const tdma_plan *plan, int which, int slot, void **device_ptr, size_t *bytes);
+
+int tdma_plan_destroy(tdma_plan *plan);
+const char *tdma_last_error(void); /* thread-local, never NULL */
+int tdma_version(void);            /* 10000*major + 100*minor + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDMA_H_ */

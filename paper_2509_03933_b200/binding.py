@@ -1,0 +1,242 @@
+"""Thin Python binding of the C ABI in ``include/tdma.h`` (argument marshalling only).
+
+Same names as the C entry points: ``tdma_plan_create``, ``tdma_plan_create_ex``, ``tdma_solve``,
+``tdma_solve_host``, ``tdma_stage``, ``tdma_plan_get``, ``tdma_plan_workspace_bytes``,
+``tdma_plan_buffer``, ``tdma_plan_destroy``, ``tdma_last_error``, ``tdma_version`` -- plus a small
+``Plan`` convenience class.  Every step of the path runs inside ``libtdma.so``'s kernels; PyTorch
+is used by callers only for device memory and streams.  There is no CPU fallback: if the shared
+library is missing (and cannot be built) importing a compute entry point raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+from . import build as _build
+
+# enums of include/tdma.h
+TDMA_F64 = 0
+TDMA_OK, TDMA_ERR_INVALID_ARG, TDMA_ERR_UNSUPPORTED, TDMA_ERR_ALLOC, TDMA_ERR_CUDA = 0, -1, -2, -3, -4
+TDMA_VARIANT_AUTO, TDMA_VARIANT_PIPELINED, TDMA_VARIANT_FUSED = 0, 1, 2
+TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
+(TDMA_GET_NB, TDMA_GET_M, TDMA_GET_BATCH, TDMA_GET_NSTREAMS, TDMA_GET_DEPTH, TDMA_GET_VARIANT,
+ TDMA_GET_LAUNCHES, TDMA_GET_FUSED_LINES, TDMA_GET_FUSED_CLUSTER, TDMA_GET_GRAPH_BUILDS) = range(10)
+(TDMA_BUF_RA, TDMA_BUF_RC, TDMA_BUF_RD, TDMA_BUF_Y, TDMA_BUF_SA, TDMA_BUF_SC, TDMA_BUF_SD) = range(7)
+
+EXPORTED_SYMBOLS = (
+    "tdma_plan_create", "tdma_plan_create_ex", "tdma_solve", "tdma_solve_host", "tdma_stage",
+    "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
+    "tdma_last_error", "tdma_version",
+)
+
+
+class tdma_options(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_int), ("variant", ctypes.c_int), ("nstreams", ctypes.c_int),
+        ("use_graph", ctypes.c_int), ("separate_gather", ctypes.c_int),
+        ("fused_lines", ctypes.c_int), ("fused_cluster", ctypes.c_int),
+        ("reserved", ctypes.c_int * 8),
+    ]
+
+
+class TdmaError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__("tdma error %d: %s" % (status, message))
+        self.status = status
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def library_path() -> str:
+    return _build.LIB_PATH
+
+
+def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
+    """dlopen libtdma.so (building it with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB_PATH
+    if build_if_missing:
+        try:
+            path = _build.build()
+        except Exception as exc:            # stale-but-present library is still usable
+            if not os.path.exists(path):
+                raise RuntimeError("libtdma.so is missing and could not be built: %s" % exc)
+    if not os.path.exists(path):
+        raise RuntimeError("libtdma.so not found at %s (run __graft_entry__.build())" % path)
+    lib = ctypes.CDLL(path)
+    vp, ci, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+    lib.tdma_plan_create.argtypes = [ci] * 6
+    lib.tdma_plan_create.restype = vp
+    lib.tdma_plan_create_ex.argtypes = [ci] * 6 + [ctypes.POINTER(tdma_options)]
+    lib.tdma_plan_create_ex.restype = vp
+    lib.tdma_solve.argtypes = [vp] * 7
+    lib.tdma_solve.restype = ci
+    lib.tdma_solve_host.argtypes = [vp] * 6
+    lib.tdma_solve_host.restype = ci
+    lib.tdma_stage.argtypes = [vp, ci, ci] + [vp] * 6
+    lib.tdma_stage.restype = ci
+    lib.tdma_plan_get.argtypes = [vp, ci]
+    lib.tdma_plan_get.restype = ci
+    lib.tdma_plan_workspace_bytes.argtypes = [vp]
+    lib.tdma_plan_workspace_bytes.restype = sz
+    lib.tdma_plan_buffer.argtypes = [vp, ci, ci, ctypes.POINTER(vp), ctypes.POINTER(sz)]
+    lib.tdma_plan_buffer.restype = ci
+    lib.tdma_plan_destroy.argtypes = [vp]
+    lib.tdma_plan_destroy.restype = ci
+    lib.tdma_last_error.argtypes = []
+    lib.tdma_last_error.restype = ctypes.c_char_p
+    lib.tdma_version.argtypes = []
+    lib.tdma_version.restype = ci
+    _lib = lib
+    return lib
+
+
+def tdma_last_error() -> str:
+    return load_library().tdma_last_error().decode("utf-8", "replace")
+
+
+def tdma_version() -> int:
+    return int(load_library().tdma_version())
+
+
+def _check(status: int) -> int:
+    if status != TDMA_OK:
+        raise TdmaError(status, tdma_last_error())
+    return status
+
+
+def _ptr(t) -> int:
+    """Device (or host) address of a torch tensor / numpy array / int."""
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return int(t.data_ptr())
+    if hasattr(t, "ctypes"):
+        return int(t.ctypes.data)
+    raise TypeError("cannot take the address of %r" % type(t))
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)
+
+
+def tdma_plan_create(nx: int, ny: int, nz: int, P: int, batch: int, dtype: int = TDMA_F64) -> int:
+    h = load_library().tdma_plan_create(nx, ny, nz, P, batch, dtype)
+    if not h:
+        raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())
+    return int(h)
+
+
+def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: int = TDMA_F64, *,
+                        variant: int = 0, nstreams: int = 0, use_graph: int = 0,
+                        separate_gather: int = 0, fused_lines: int = 0, fused_cluster: int = 0) -> int:
+    opt = tdma_options()
+    opt.struct_size = ctypes.sizeof(tdma_options)
+    opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
+    opt.separate_gather, opt.fused_lines, opt.fused_cluster = separate_gather, fused_lines, fused_cluster
+    h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
+    if not h:
+        raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())
+    return int(h)
+
+
+def tdma_solve(plan: int, a, b, c, d, x, stream=None) -> None:
+    _check(load_library().tdma_solve(plan, _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(x),
+                                     _stream_handle(stream)))
+
+
+def tdma_solve_host(plan: int, a, b, c, d, x) -> None:
+    _check(load_library().tdma_solve_host(plan, _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(x)))
+
+
+def tdma_stage(plan: int, stage: int, batch_index: int, a, b, c, d, x, stream=None) -> None:
+    _check(load_library().tdma_stage(plan, stage, batch_index, _ptr(a), _ptr(b), _ptr(c), _ptr(d),
+                                     _ptr(x), _stream_handle(stream)))
+
+
+def tdma_plan_get(plan: int, what: int) -> int:
+    v = int(load_library().tdma_plan_get(plan, what))
+    if v < 0:
+        raise TdmaError(v, tdma_last_error())
+    return v
+
+
+def tdma_plan_workspace_bytes(plan: int) -> int:
+    return int(load_library().tdma_plan_workspace_bytes(plan))
+
+
+def tdma_plan_buffer(plan: int, which: int, slot: int = 0):
+    """(device address, bytes) of a plan-owned stage buffer."""
+    p, n = ctypes.c_void_p(), ctypes.c_size_t()
+    _check(load_library().tdma_plan_buffer(plan, which, slot, ctypes.byref(p), ctypes.byref(n)))
+    return int(p.value), int(n.value)
+
+
+def tdma_plan_destroy(plan: int) -> None:
+    _check(load_library().tdma_plan_destroy(plan))
+
+
+class Plan:
+    """RAII wrapper: ``Plan(nx, ny, nz, P, batch).solve(a, b, c, d, x)``."""
+
+    def __init__(self, nx: int, ny: int, nz: int, P: int, batch: int = 0, **options):
+        self.shape = (nz, ny, nx)
+        self.P = P
+        self.handle = (tdma_plan_create_ex(nx, ny, nz, P, batch, TDMA_F64, **options)
+                       if options else tdma_plan_create(nx, ny, nz, P, batch, TDMA_F64))
+
+    def _validate(self, tensors):
+        n = self.shape[0] * self.shape[1] * self.shape[2]
+        for t in tensors:
+            if hasattr(t, "numel"):
+                if t.numel() != n or not t.is_contiguous() or t.element_size() != 8:
+                    raise ValueError("arrays must be contiguous fp64 with nz*ny*nx elements")
+
+    def solve(self, a, b, c, d, x, stream=None):
+        self._validate((a, b, c, d, x))
+        tdma_solve(self.handle, a, b, c, d, x, stream)
+        return x
+
+    def solve_host(self, a, b, c, d, x):
+        self._validate((a, b, c, d, x))
+        tdma_solve_host(self.handle, a, b, c, d, x)
+        return x
+
+    def stage(self, stage: int, batch_index: int, a, b, c, d, x, stream=None):
+        tdma_stage(self.handle, stage, batch_index, a, b, c, d, x, stream)
+
+    def get(self, what: int) -> int:
+        return tdma_plan_get(self.handle, what)
+
+    @property
+    def workspace_bytes(self) -> int:
+        return tdma_plan_workspace_bytes(self.handle)
+
+    def buffer(self, which: int, slot: int = 0):
+        return tdma_plan_buffer(self.handle, which, slot)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            h, self.handle = self.handle, None
+            tdma_plan_destroy(h)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,552 @@
+// C-ABI implementation (include/tdma.h): plan management, the batch-pipeline scheduler
+// (Alg. 2, re-expressed with CUDA events instead of cudaStreamSynchronize),
+// CUDA-graph capture of the schedule, stage-isolated entry point, host-buffer solve.
+#include "../../include/tdma.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "tdma_stage_kernels.cuh"
+#include "tdma_fused.cuh"
+
+#define TDMA_VERSION_NUM 10100
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int set_err(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                       \
+    do {                                                                                     \
+        cudaError_t e_ = (expr);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return set_err(TDMA_ERR_CUDA, "%s failed: %s (%s:%d)", #expr,                    \
+                           cudaGetErrorString(e_), __FILE__, __LINE__);                      \
+    } while (0)
+
+constexpr int kMaxLanes = 7;
+constexpr int kMaxDepth = kMaxLanes + 2;
+constexpr int kPrefetchRows = 4;  // U of the stage kernels
+
+struct SlabPtrs {
+    const double *a, *b, *c, *d;
+    double *x;
+};
+
+struct GraphEntry {
+    SlabPtrs ptr;
+    int nz;
+    cudaGraphExec_t exec;
+    unsigned long long stamp;
+};
+
+}  // namespace
+
+struct tdma_plan {
+    int nx = 0, ny = 0, nz = 0, P = 0, m = 0, bz = 0, nb = 0;
+    int variant = TDMA_VARIANT_PIPELINED, nstreams = 2, nlanes = 1, depth = 3;
+    int use_graph = 1, separate_gather = 0;
+    int device = 0;
+    size_t slice = 0;   // nx * ny
+    size_t Lb_max = 0;  // nx * bz
+    size_t workspace = 0;
+    // PIPELINED buffers (ring of `depth` slots)
+    double *scratch = nullptr;  // depth x {SA, SC, SD} x [bz][ny][nx]
+    double *red = nullptr;      // depth x {RA, RC, RD, CP, Y} x [2P][Lb_max]
+    double *send = nullptr;     // depth x [P][6][Lb_max]            (separate_gather)
+    cudaStream_t sMain = nullptr, sB = nullptr, lane[kMaxLanes] = {};
+    cudaEvent_t evFork = nullptr, evBJoin = nullptr, evLaneJoin[kMaxLanes] = {};
+    cudaEvent_t evA[kMaxDepth] = {}, evB[kMaxDepth] = {}, evC[kMaxDepth] = {};
+    std::vector<GraphEntry> graphs;
+    unsigned long long stamp = 0;
+    int graph_builds = 0;
+    // FUSED
+    tdma::FusedConfig fused;
+    // host staging (tdma_solve_host), allocated on first use
+    int hz = 0;  // slices per host chunk
+    double *stage_dev[2][5] = {};
+    cudaStream_t sH2D = nullptr, sD2H = nullptr;
+    cudaEvent_t evH2D[2] = {}, evDone[2] = {}, evD2H[2] = {};
+};
+
+namespace {
+
+double *slot_scratch(const tdma_plan *pl, int slot, int which)
+{
+    const size_t per = (size_t)pl->bz * pl->slice;
+    return pl->scratch + ((size_t)slot * 3 + which) * per;
+}
+double *slot_red(const tdma_plan *pl, int slot, int which)
+{
+    const size_t per = (size_t)2 * pl->P * pl->Lb_max;
+    return pl->red + ((size_t)slot * 5 + which) * per;
+}
+
+tdma::StageParams batch_params(const tdma_plan *pl, const SlabPtrs &ptr, int nz_count, int n)
+{
+    const int k0 = n * pl->bz;
+    const int bzn = std::min(pl->bz, nz_count - k0);
+    const int slot = n % pl->depth;
+    const size_t off = (size_t)k0 * pl->slice;
+    tdma::StageParams prm;
+    prm.a = ptr.a + off; prm.b = ptr.b + off; prm.c = ptr.c + off; prm.d = ptr.d + off;
+    prm.x = ptr.x + off;
+    prm.sa = slot_scratch(pl, slot, 0); prm.sc = slot_scratch(pl, slot, 1);
+    prm.sd = slot_scratch(pl, slot, 2);
+    prm.ra = slot_red(pl, slot, 0); prm.rc = slot_red(pl, slot, 1); prm.rd = slot_red(pl, slot, 2);
+    prm.cp = slot_red(pl, slot, 3); prm.y = slot_red(pl, slot, 4);
+    prm.send = pl->send ? pl->send + (size_t)slot * 6 * pl->P * pl->Lb_max : nullptr;
+    prm.Lb = (long long)pl->nx * bzn;
+    prm.nx = pl->nx; prm.ny = pl->ny; prm.m = pl->m; prm.P = pl->P;
+    return prm;
+}
+
+int launch_stage(const tdma_plan *pl, int stage, const tdma::StageParams &prm, cudaStream_t st)
+{
+    const unsigned Lb = (unsigned)prm.Lb;
+    switch (stage) {
+    case TDMA_STAGE_A: {
+        dim3 grid((Lb + 127) / 128, pl->P);
+        if (pl->separate_gather)
+            tdma::stage_a_kernel<kPrefetchRows, true><<<grid, 128, 0, st>>>(prm);
+        else
+            tdma::stage_a_kernel<kPrefetchRows, false><<<grid, 128, 0, st>>>(prm);
+        break;
+    }
+    case TDMA_STAGE_GATHER: {
+        dim3 grid((Lb + 255) / 256, pl->P);
+        tdma::gather_kernel<<<grid, 256, 0, st>>>(prm);
+        break;
+    }
+    case TDMA_STAGE_B:
+        tdma::stage_b_kernel<kPrefetchRows><<<(Lb + 63) / 64, 64, 0, st>>>(prm);
+        break;
+    case TDMA_STAGE_C: {
+        dim3 grid((Lb + 127) / 128, pl->P);
+        tdma::stage_c_kernel<kPrefetchRows><<<grid, 128, 0, st>>>(prm);
+        break;
+    }
+    default:
+        return set_err(TDMA_ERR_INVALID_ARG, "unknown stage %d", stage);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return TDMA_OK;
+}
+
+// Alg. 2 with events.  Iteration n enqueues A(n) on an A+C lane, B(n-1) on the B stream and
+// C(n-2) on the lane that ran A(n-2); indices outside [0, nb) are skipped.
+// Ring slot of batch n is n % depth with depth = nlanes + 2 >= 3 ("three batched systems
+// concurrently"): A(n) may only overwrite a slot after C(n - depth) has read it.
+int enqueue_pipelined(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t origin)
+{
+    if (pl->ny == 1) {
+        const size_t n = (size_t)pl->nx * nz_count;
+        tdma::diagonal_kernel<<<(unsigned)((n + 255) / 256), 256, 0, origin>>>(ptr.b, ptr.d, ptr.x, n);
+        CUDA_TRY(cudaGetLastError());
+        return TDMA_OK;
+    }
+    const int nb = (nz_count + pl->bz - 1) / pl->bz;
+    int rc;
+    if (pl->nstreams == 1) {  // Alg. 1 order: A, [A2B], B, C per batch
+        for (int n = 0; n < nb; ++n) {
+            const tdma::StageParams prm = batch_params(pl, ptr, nz_count, n);
+            if ((rc = launch_stage(pl, TDMA_STAGE_A, prm, origin))) return rc;
+            if (pl->separate_gather && (rc = launch_stage(pl, TDMA_STAGE_GATHER, prm, origin))) return rc;
+            if ((rc = launch_stage(pl, TDMA_STAGE_B, prm, origin))) return rc;
+            if ((rc = launch_stage(pl, TDMA_STAGE_C, prm, origin))) return rc;
+        }
+        return TDMA_OK;
+    }
+    CUDA_TRY(cudaEventRecord(pl->evFork, origin));
+    for (int i = 0; i < pl->nlanes; ++i) CUDA_TRY(cudaStreamWaitEvent(pl->lane[i], pl->evFork, 0));
+    CUDA_TRY(cudaStreamWaitEvent(pl->sB, pl->evFork, 0));
+    for (int n = 0; n < nb + 2; ++n) {
+        if (n < nb) {  // Stage A (n)
+            const int slot = n % pl->depth;
+            cudaStream_t st = pl->lane[n % pl->nlanes];
+            if (n >= pl->depth) CUDA_TRY(cudaStreamWaitEvent(st, pl->evC[slot], 0));
+            const tdma::StageParams prm = batch_params(pl, ptr, nz_count, n);
+            if ((rc = launch_stage(pl, TDMA_STAGE_A, prm, st))) return rc;
+            CUDA_TRY(cudaEventRecord(pl->evA[slot], st));
+        }
+        if (n - 1 >= 0 && n - 1 < nb) {  // Stage A2B + B (n-1)
+            const int q = n - 1, slot = q % pl->depth;
+            const tdma::StageParams prm = batch_params(pl, ptr, nz_count, q);
+            CUDA_TRY(cudaStreamWaitEvent(pl->sB, pl->evA[slot], 0));
+            if (pl->separate_gather && (rc = launch_stage(pl, TDMA_STAGE_GATHER, prm, pl->sB))) return rc;
+            if ((rc = launch_stage(pl, TDMA_STAGE_B, prm, pl->sB))) return rc;
+            CUDA_TRY(cudaEventRecord(pl->evB[slot], pl->sB));
+        }
+        if (n - 2 >= 0 && n - 2 < nb) {  // Stage B2C + C (n-2): C reads Y in place, no scatter
+            const int q = n - 2, slot = q % pl->depth;
+            cudaStream_t st = pl->lane[q % pl->nlanes];
+            const tdma::StageParams prm = batch_params(pl, ptr, nz_count, q);
+            CUDA_TRY(cudaStreamWaitEvent(st, pl->evB[slot], 0));
+            if ((rc = launch_stage(pl, TDMA_STAGE_C, prm, st))) return rc;
+            CUDA_TRY(cudaEventRecord(pl->evC[slot], st));
+        }
+    }
+    for (int i = 0; i < pl->nlanes; ++i) {
+        CUDA_TRY(cudaEventRecord(pl->evLaneJoin[i], pl->lane[i]));
+        CUDA_TRY(cudaStreamWaitEvent(origin, pl->evLaneJoin[i], 0));
+    }
+    CUDA_TRY(cudaEventRecord(pl->evBJoin, pl->sB));
+    CUDA_TRY(cudaStreamWaitEvent(origin, pl->evBJoin, 0));
+    return TDMA_OK;
+}
+
+int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t origin)
+{
+    if (pl->ny == 1) return enqueue_pipelined(pl, ptr, nz_count, origin);
+    // batches are contiguous z ranges; consecutive launches on one stream overlap their tails
+    // only through the hardware's block scheduler, so by default one launch covers all slices
+    const int nb = (nz_count + pl->bz - 1) / pl->bz;
+    for (int n = 0; n < nb; ++n) {
+        const int k0 = n * pl->bz;
+        const int bzn = std::min(pl->bz, nz_count - k0);
+        const size_t off = (size_t)k0 * pl->slice;
+        cudaError_t e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
+                                           ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, pl->P,
+                                           origin);
+        if (e != cudaSuccess)
+            return set_err(TDMA_ERR_CUDA, "fused launch failed: %s", cudaGetErrorString(e));
+    }
+    return TDMA_OK;
+}
+
+int enqueue_schedule(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t origin)
+{
+    return pl->variant == TDMA_VARIANT_FUSED ? enqueue_fused(pl, ptr, nz_count, origin)
+                                             : enqueue_pipelined(pl, ptr, nz_count, origin);
+}
+
+int launches_per_solve(const tdma_plan *pl)
+{
+    if (pl->ny == 1) return 1;
+    if (pl->variant == TDMA_VARIANT_FUSED) return pl->nb;
+    return pl->nb * (3 + (pl->separate_gather ? 1 : 0));
+}
+
+// Look up / build the CUDA graph of the whole schedule for this pointer set.
+int graph_for(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaGraphExec_t *out)
+{
+    for (auto &g : pl->graphs)
+        if (g.nz == nz_count && g.ptr.a == ptr.a && g.ptr.b == ptr.b && g.ptr.c == ptr.c &&
+            g.ptr.d == ptr.d && g.ptr.x == ptr.x) {
+            g.stamp = ++pl->stamp;
+            *out = g.exec;
+            return TDMA_OK;
+        }
+    cudaGraph_t graph = nullptr;
+    CUDA_TRY(cudaStreamBeginCapture(pl->sMain, cudaStreamCaptureModeThreadLocal));
+    int rc = enqueue_schedule(pl, ptr, nz_count, pl->sMain);
+    cudaError_t e = cudaStreamEndCapture(pl->sMain, &graph);
+    if (rc != TDMA_OK) {
+        if (graph) cudaGraphDestroy(graph);
+        return rc;
+    }
+    if (e != cudaSuccess)
+        return set_err(TDMA_ERR_CUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess)
+        return set_err(TDMA_ERR_CUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e));
+    if (pl->graphs.size() >= 8) {  // evict least recently used
+        auto it = std::min_element(pl->graphs.begin(), pl->graphs.end(),
+                                   [](const GraphEntry &x, const GraphEntry &y) { return x.stamp < y.stamp; });
+        cudaGraphExecDestroy(it->exec);
+        pl->graphs.erase(it);
+    }
+    pl->graphs.push_back(GraphEntry{ptr, nz_count, exec, ++pl->stamp});
+    pl->graph_builds++;
+    *out = exec;
+    return TDMA_OK;
+}
+
+int run_solve(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t stream)
+{
+    if (pl->use_graph) {
+        cudaGraphExec_t exec = nullptr;
+        int rc = graph_for(pl, ptr, nz_count, &exec);
+        if (rc != TDMA_OK) return rc;
+        CUDA_TRY(cudaGraphLaunch(exec, stream));
+        return TDMA_OK;
+    }
+    return enqueue_schedule(pl, ptr, nz_count, stream);
+}
+
+void free_plan(tdma_plan *pl)
+{
+    if (!pl) return;
+    for (auto &g : pl->graphs) cudaGraphExecDestroy(g.exec);
+    cudaFree(pl->scratch); cudaFree(pl->red); cudaFree(pl->send);
+    for (int s = 0; s < 2; ++s)
+        for (int i = 0; i < 5; ++i) cudaFree(pl->stage_dev[s][i]);
+    auto ds = [](cudaStream_t s) { if (s) cudaStreamDestroy(s); };
+    auto de = [](cudaEvent_t e) { if (e) cudaEventDestroy(e); };
+    ds(pl->sMain); ds(pl->sB); ds(pl->sH2D); ds(pl->sD2H);
+    for (int i = 0; i < kMaxLanes; ++i) { ds(pl->lane[i]); de(pl->evLaneJoin[i]); }
+    for (int i = 0; i < kMaxDepth; ++i) { de(pl->evA[i]); de(pl->evB[i]); de(pl->evC[i]); }
+    for (int i = 0; i < 2; ++i) { de(pl->evH2D[i]); de(pl->evDone[i]); de(pl->evD2H[i]); }
+    de(pl->evFork); de(pl->evBJoin);
+    delete pl;
+}
+
+int init_plan(tdma_plan *pl, const tdma_options *opt)
+{
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1)
+        return set_err(TDMA_ERR_CUDA, "no CUDA device (%s); this library has no CPU fallback",
+                       e != cudaSuccess ? cudaGetErrorString(e) : "device count is 0");
+    CUDA_TRY(cudaGetDevice(&pl->device));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, pl->device));
+    if (prop.major < 10)
+        return set_err(TDMA_ERR_UNSUPPORTED, "device sm_%d%d: this build targets sm_100a only",
+                       prop.major, prop.minor);
+
+    int variant = opt ? opt->variant : 0;
+    if (variant == TDMA_VARIANT_AUTO) variant = TDMA_VARIANT_PIPELINED;
+    if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED)
+        return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
+    pl->variant = variant;
+    pl->use_graph = (opt && opt->use_graph < 0) ? 0 : 1;
+    pl->separate_gather = (opt && opt->separate_gather > 0) ? 1 : 0;
+    pl->nstreams = (opt && opt->nstreams > 0) ? opt->nstreams : 2;
+    if (pl->nstreams > kMaxLanes + 1)
+        return set_err(TDMA_ERR_INVALID_ARG, "nstreams %d > %d", pl->nstreams, kMaxLanes + 1);
+    pl->nlanes = std::max(1, pl->nstreams - 1);
+    pl->depth = pl->nstreams == 1 ? 1 : pl->nlanes + 2;
+
+    int lo = 0, hi = 0;  // stage B's stream gets the highest priority so its small kernels are
+    CUDA_TRY(cudaDeviceGetStreamPriorityRange(&lo, &hi));  // scheduled as soon as SM slots free up
+    CUDA_TRY(cudaStreamCreateWithPriority(&pl->sMain, cudaStreamNonBlocking, lo));
+    CUDA_TRY(cudaStreamCreateWithPriority(&pl->sB, cudaStreamNonBlocking, hi));
+    for (int i = 0; i < pl->nlanes; ++i)
+        CUDA_TRY(cudaStreamCreateWithPriority(&pl->lane[i], cudaStreamNonBlocking, lo));
+    auto mk = [](cudaEvent_t *ev) { return cudaEventCreateWithFlags(ev, cudaEventDisableTiming); };
+    CUDA_TRY(mk(&pl->evFork)); CUDA_TRY(mk(&pl->evBJoin));
+    for (int i = 0; i < pl->nlanes; ++i) CUDA_TRY(mk(&pl->evLaneJoin[i]));
+    for (int i = 0; i < pl->depth; ++i) { CUDA_TRY(mk(&pl->evA[i])); CUDA_TRY(mk(&pl->evB[i])); CUDA_TRY(mk(&pl->evC[i])); }
+
+    if (variant == TDMA_VARIANT_PIPELINED && pl->ny > 1) {
+        const size_t sbytes = (size_t)pl->depth * 3 * pl->bz * pl->slice * sizeof(double);
+        const size_t rbytes = (size_t)pl->depth * 5 * 2 * pl->P * pl->Lb_max * sizeof(double);
+        if (cudaMalloc(&pl->scratch, sbytes) != cudaSuccess || cudaMalloc(&pl->red, rbytes) != cudaSuccess) {
+            cudaGetLastError();
+            return set_err(TDMA_ERR_ALLOC, "cannot allocate %zu bytes of scratch ring", sbytes + rbytes);
+        }
+        pl->workspace = sbytes + rbytes;
+        if (pl->separate_gather) {
+            const size_t gbytes = (size_t)pl->depth * 6 * pl->P * pl->Lb_max * sizeof(double);
+            if (cudaMalloc(&pl->send, gbytes) != cudaSuccess) {
+                cudaGetLastError();
+                return set_err(TDMA_ERR_ALLOC, "cannot allocate %zu bytes of send_A buffer", gbytes);
+            }
+            pl->workspace += gbytes;
+        }
+    }
+    if (variant == TDMA_VARIANT_FUSED && pl->ny > 1) {
+        const char *why = nullptr;
+        if (!tdma::configure_fused(&pl->fused, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
+                                   opt ? opt->fused_cluster : 0, prop, &why))
+            return set_err(TDMA_ERR_UNSUPPORTED, "fused variant unavailable: %s", why ? why : "?");
+    }
+    return TDMA_OK;
+}
+
+int check_ptrs(const tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,
+               const void *x)
+{
+    if (!plan) return set_err(TDMA_ERR_INVALID_ARG, "plan is NULL");
+    if (!a || !b || !c || !d || !x) return set_err(TDMA_ERR_INVALID_ARG, "NULL array pointer");
+    return TDMA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dtype,
+                               const tdma_options *options)
+{
+    g_err[0] = 0;
+    if (nx < 1 || ny < 1 || nz < 1) { set_err(TDMA_ERR_INVALID_ARG, "dimensions must be >= 1 (got %d x %d x %d)", nx, ny, nz); return nullptr; }
+    if (P < 1) { set_err(TDMA_ERR_INVALID_ARG, "P must be >= 1 (got %d)", P); return nullptr; }
+    if (ny % P != 0) { set_err(TDMA_ERR_INVALID_ARG, "ny = %d is not divisible by P = %d", ny, P); return nullptr; }
+    if (P > 1 && ny / P < 2) { set_err(TDMA_ERR_INVALID_ARG, "partitions need >= 2 rows (ny/P = %d)", ny / P); return nullptr; }
+    if (batch < 0 || batch > nz) { set_err(TDMA_ERR_INVALID_ARG, "batch = %d outside [0, nz = %d]", batch, nz); return nullptr; }
+    if (dtype != TDMA_F64) { set_err(TDMA_ERR_UNSUPPORTED, "dtype %d: only TDMA_F64 is implemented", dtype); return nullptr; }
+    if (options && options->struct_size != (int)sizeof(tdma_options)) { set_err(TDMA_ERR_INVALID_ARG, "tdma_options.struct_size = %d, expected %zu", options->struct_size, sizeof(tdma_options)); return nullptr; }
+    if ((long long)nx * (batch ? batch : nz) > 0x7fffffffLL) { set_err(TDMA_ERR_UNSUPPORTED, "nx * batch exceeds 2^31-1 lines per batch"); return nullptr; }
+    tdma_plan *pl = new (std::nothrow) tdma_plan();
+    if (!pl) { set_err(TDMA_ERR_ALLOC, "out of host memory"); return nullptr; }
+    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->P = P; pl->m = ny / P;
+    pl->bz = batch == 0 ? nz : batch;
+    pl->nb = (nz + pl->bz - 1) / pl->bz;
+    pl->slice = (size_t)nx * ny;
+    pl->Lb_max = (size_t)nx * pl->bz;
+    if (init_plan(pl, options) != TDMA_OK) { free_plan(pl); return nullptr; }
+    return pl;
+}
+
+tdma_plan *tdma_plan_create(int nx, int ny, int nz, int P, int batch, int dtype)
+{
+    return tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, nullptr);
+}
+
+int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,
+               void *x, void *stream)
+{
+    int rc = check_ptrs(plan, a, b, c, d, x);
+    if (rc != TDMA_OK) return rc;
+    const SlabPtrs ptr{(const double *)a, (const double *)b, (const double *)c, (const double *)d, (double *)x};
+    return run_solve(plan, ptr, plan->nz, (cudaStream_t)stream);
+}
+
+int tdma_stage(tdma_plan *plan, int stage, int batch_index, const void *a, const void *b,
+               const void *c, const void *d, void *x, void *stream)
+{
+    int rc = check_ptrs(plan, a, b, c, d, x);
+    if (rc != TDMA_OK) return rc;
+    if (plan->variant != TDMA_VARIANT_PIPELINED || plan->ny == 1)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_stage needs a PIPELINED plan with ny > 1");
+    if (batch_index < 0 || batch_index >= plan->nb)
+        return set_err(TDMA_ERR_INVALID_ARG, "batch_index %d outside [0, %d)", batch_index, plan->nb);
+    if (stage == TDMA_STAGE_GATHER && !plan->separate_gather)
+        return set_err(TDMA_ERR_INVALID_ARG, "plan has no separate gather stage");
+    const SlabPtrs ptr{(const double *)a, (const double *)b, (const double *)c, (const double *)d, (double *)x};
+    const tdma::StageParams prm = batch_params(plan, ptr, plan->nz, batch_index);
+    return launch_stage(plan, stage, prm, (cudaStream_t)stream);
+}
+
+int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,
+                    void *x)
+{
+    int rc = check_ptrs(plan, a, b, c, d, x);
+    if (rc != TDMA_OK) return rc;
+    tdma_plan *pl = plan;
+    if (!pl->sH2D) {  // first use: staging buffers, copy streams
+        // chunk = whole batches, about 64 Mi cells (512 MiB per array) or the slab if smaller
+        const size_t target = (size_t)1 << 26;
+        long long hz = (long long)std::max<size_t>(1, target / pl->slice);
+        hz = std::max<long long>(pl->bz, hz / pl->bz * pl->bz);
+        pl->hz = (int)std::min<long long>(hz, pl->nz);
+        const size_t bytes = (size_t)pl->hz * pl->slice * sizeof(double);
+        for (int s = 0; s < 2; ++s)
+            for (int i = 0; i < 5; ++i)
+                if (cudaMalloc(&pl->stage_dev[s][i], bytes) != cudaSuccess) {
+                    cudaGetLastError();
+                    return set_err(TDMA_ERR_ALLOC, "cannot allocate %zu bytes of host staging", bytes);
+                }
+        pl->workspace += 10 * bytes;
+        CUDA_TRY(cudaStreamCreateWithFlags(&pl->sH2D, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&pl->sD2H, cudaStreamNonBlocking));
+        for (int s = 0; s < 2; ++s) {
+            CUDA_TRY(cudaEventCreateWithFlags(&pl->evH2D[s], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&pl->evDone[s], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&pl->evD2H[s], cudaEventDisableTiming));
+        }
+    }
+    const double *h[4] = {(const double *)a, (const double *)b, (const double *)c, (const double *)d};
+    double *hx = (double *)x;
+    const int nchunks = (pl->nz + pl->hz - 1) / pl->hz;
+    for (int q = 0; q < nchunks; ++q) {
+        const int s = q & 1;
+        const int k0 = q * pl->hz;
+        const int nzc = std::min(pl->hz, pl->nz - k0);
+        const size_t off = (size_t)k0 * pl->slice;
+        const size_t bytes = (size_t)nzc * pl->slice * sizeof(double);
+        if (q >= 2) {  // staging slot s is free once chunk q-2 is solved and copied out
+            CUDA_TRY(cudaStreamWaitEvent(pl->sH2D, pl->evDone[s], 0));
+            CUDA_TRY(cudaStreamWaitEvent(pl->sH2D, pl->evD2H[s], 0));
+        }
+        for (int i = 0; i < 4; ++i)
+            CUDA_TRY(cudaMemcpyAsync(pl->stage_dev[s][i], h[i] + off, bytes, cudaMemcpyHostToDevice, pl->sH2D));
+        CUDA_TRY(cudaEventRecord(pl->evH2D[s], pl->sH2D));
+        CUDA_TRY(cudaStreamWaitEvent(pl->sMain, pl->evH2D[s], 0));
+        const SlabPtrs ptr{pl->stage_dev[s][0], pl->stage_dev[s][1], pl->stage_dev[s][2],
+                           pl->stage_dev[s][3], pl->stage_dev[s][4]};
+        if ((rc = run_solve(pl, ptr, nzc, pl->sMain)) != TDMA_OK) return rc;
+        CUDA_TRY(cudaEventRecord(pl->evDone[s], pl->sMain));
+        CUDA_TRY(cudaStreamWaitEvent(pl->sD2H, pl->evDone[s], 0));
+        CUDA_TRY(cudaMemcpyAsync(hx + off, pl->stage_dev[s][4], bytes, cudaMemcpyDeviceToHost, pl->sD2H));
+        CUDA_TRY(cudaEventRecord(pl->evD2H[s], pl->sD2H));
+    }
+    CUDA_TRY(cudaStreamSynchronize(pl->sD2H));
+    CUDA_TRY(cudaStreamSynchronize(pl->sMain));
+    return TDMA_OK;
+}
+
+int tdma_plan_get(const tdma_plan *plan, int what)
+{
+    if (!plan) return set_err(TDMA_ERR_INVALID_ARG, "plan is NULL");
+    switch (what) {
+    case TDMA_GET_NB: return plan->nb;
+    case TDMA_GET_M: return plan->m;
+    case TDMA_GET_BATCH: return plan->bz;
+    case TDMA_GET_NSTREAMS: return plan->variant == TDMA_VARIANT_FUSED ? 1 : plan->nstreams;
+    case TDMA_GET_DEPTH: return plan->depth;
+    case TDMA_GET_VARIANT: return plan->variant;
+    case TDMA_GET_LAUNCHES: return launches_per_solve(plan);
+    case TDMA_GET_FUSED_LINES: return plan->fused.lines;
+    case TDMA_GET_FUSED_CLUSTER: return plan->fused.cluster;
+    case TDMA_GET_GRAPH_BUILDS: return plan->graph_builds;
+    default: return set_err(TDMA_ERR_INVALID_ARG, "unknown query %d", what);
+    }
+}
+
+size_t tdma_plan_workspace_bytes(const tdma_plan *plan) { return plan ? plan->workspace : 0; }
+
+int tdma_plan_buffer(const tdma_plan *plan, int which, int slot, void **device_ptr, size_t *bytes)
+{
+    if (!plan || !device_ptr || !bytes) return set_err(TDMA_ERR_INVALID_ARG, "NULL argument");
+    if (plan->variant != TDMA_VARIANT_PIPELINED || !plan->scratch)
+        return set_err(TDMA_ERR_UNSUPPORTED, "plan has no stage buffers");
+    if (slot < 0 || slot >= plan->depth) return set_err(TDMA_ERR_INVALID_ARG, "slot %d outside [0, %d)", slot, plan->depth);
+    switch (which) {
+    case TDMA_BUF_RA: case TDMA_BUF_RC: case TDMA_BUF_RD:
+        *device_ptr = slot_red(plan, slot, which - TDMA_BUF_RA);
+        *bytes = (size_t)2 * plan->P * plan->Lb_max * sizeof(double);
+        return TDMA_OK;
+    case TDMA_BUF_Y:
+        *device_ptr = slot_red(plan, slot, 4);
+        *bytes = (size_t)2 * plan->P * plan->Lb_max * sizeof(double);
+        return TDMA_OK;
+    case TDMA_BUF_SA: case TDMA_BUF_SC: case TDMA_BUF_SD:
+        *device_ptr = slot_scratch(plan, slot, which - TDMA_BUF_SA);
+        *bytes = (size_t)plan->bz * plan->slice * sizeof(double);
+        return TDMA_OK;
+    default: return set_err(TDMA_ERR_INVALID_ARG, "unknown buffer %d", which);
+    }
+}
+
+int tdma_plan_destroy(tdma_plan *plan)
+{
+    if (!plan) return set_err(TDMA_ERR_INVALID_ARG, "plan is NULL");
+    cudaError_t e = cudaDeviceSynchronize();
+    free_plan(plan);
+    if (e != cudaSuccess) return set_err(TDMA_ERR_CUDA, "cudaDeviceSynchronize: %s", cudaGetErrorString(e));
+    return TDMA_OK;
+}
+
+const char *tdma_last_error(void) { return g_err; }
+int tdma_version(void) { return TDMA_VERSION_NUM; }
+
+}  // extern "C"

@@ -1,0 +1,272 @@
+// Stage kernels of the PIPELINED variant (sm_100a): partition reduce (stage A, with the gather
+// fused as its epilogue or as a separate A2B kernel), reduced 2P-row solve (stage B) and
+// back-substitution (stage C).  PAPER.md:49-58 (five stages), Alg. 2 PAPER.md:166-214.
+//
+// Thread mapping (all three): one thread per (line, partition) -- or per line for stage B -- with
+// consecutive threads on consecutive x, so every row access of a warp is one 256 B segment.
+// The recurrences along y are serial per thread; bandwidth comes from U rows x 3-4 arrays of
+// independent loads kept in flight per thread (register double buffer).
+//
+// Arithmetic of one partition (local rows r = 0..m-1, x_{-1} = previous partition's last unknown,
+// x_m = next partition's first; global a_0 := 0, c_{ny-1} := 0):
+//   rows 0 and 1 are normalised by their b;
+//   r = 2..m-1 (forward elimination with x_0 kept as a parameter):
+//        inv = 1/(b_r - a_r c'_{r-1});  d'_r = (d_r - a_r d'_{r-1}) inv;  c'_r = c_r inv;
+//        a'_r = -a_r a'_{r-1} inv          =>  a'_r x_0 + x_r + c'_r x_{r+1} = d'_r   (r >= 1)
+//   while sweeping, row r-1 is folded into the FIRST-ROW equation
+//        fa x_{-1} + fb x_0 + fc x_{r-1} = fd   ->   fb -= fc a'_{r-1}; fd -= fc d'_{r-1};
+//        fc = -fc c'_{r-1}                      (now couples x_r)
+//   so that after the sweep it reads fa x_{-1} + fb x_0 + fc x_{m-1} = fd and is normalised by fb.
+//   Reduced rows (unit diagonal): 2p = (fa, fc | fd)/fb, 2p+1 = (a'_{m-1}, c'_{m-1} | d'_{m-1}).
+//   Stage C: x_0 = Y[2p], x_{m-1} = Y[2p+1], r = m-2..1: x_r = d'_r - a'_r x_0 - c'_r x_{r+1}.
+// One division per cell; nothing is re-read inside stage A.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tdma {
+
+// read-once inputs / write-once output: streaming (evict-first) so they do not displace the
+// scratch ring in L2; scratch and reduced buffers: L2-only (.cg), they are re-read by the next stage
+__device__ __forceinline__ double ld_stream(const double *p) { return __ldcs(p); }
+__device__ __forceinline__ void st_stream(double *p, double v) { __stcs(p, v); }
+__device__ __forceinline__ double ld_keep(const double *p) { return __ldcg(p); }
+__device__ __forceinline__ void st_keep(double *p, double v) { __stcg(p, v); }
+
+struct StageParams {
+    const double *a, *b, *c, *d;  // batch base (slice k0 of the slab)
+    double *x;                    // batch base of the output
+    double *sa, *sc, *sd;         // scratch slot, batch layout [bz][ny][nx]
+    double *ra, *rc, *rd, *cp, *y;  // reduced system [2P][Lb], line fastest
+    double *send;                 // separate gather: send_A buffer [P][6][Lb]
+    long long Lb;                 // lines in this batch = nx * slices
+    int nx, ny, m, P;
+};
+
+// ------------------------------------------------------------------------------------------
+// Stage A
+// ------------------------------------------------------------------------------------------
+template <int U, bool kSeparateGather>
+__global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
+{
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= prm.Lb) return;
+    const int p = blockIdx.y;
+    const int nx = prm.nx, m = prm.m;
+    const long long kk = l / nx;
+    const int i = (int)(l - kk * nx);
+    const size_t off0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
+    const double *__restrict__ a = prm.a + off0;
+    const double *__restrict__ b = prm.b + off0;
+    const double *__restrict__ c = prm.c + off0;
+    const double *__restrict__ d = prm.d + off0;
+    double *__restrict__ sa = prm.sa + off0;
+    double *__restrict__ sc = prm.sc + off0;
+    double *__restrict__ sd = prm.sd + off0;
+    const size_t s = (size_t)nx;
+    const bool first_part = (p == 0), last_part = (p == prm.P - 1);
+
+    // first-row equation  fa x_{-1} + fb x_0 + fc x_frontier = fd
+    double inv = 1.0 / ld_stream(b);
+    double fa = first_part ? 0.0 : ld_stream(a) * inv;
+    double fc = ld_stream(c) * inv;
+    double fd = ld_stream(d) * inv;
+    double fb = 1.0;
+    // row 1 in forward form  pa x_0 + x_1 + pc x_2 = pd
+    double pa, pc, pd;
+    {
+        const double a1 = ld_stream(a + s), b1 = ld_stream(b + s);
+        double c1 = ld_stream(c + s);
+        const double d1 = ld_stream(d + s);
+        if (last_part && m == 2) c1 = 0.0;
+        inv = 1.0 / b1;
+        pa = a1 * inv; pc = c1 * inv; pd = d1 * inv;
+    }
+
+    double na[U], nb[U], nc[U], nd[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const int r = 2 + u;
+        if (r < m) {
+            na[u] = ld_stream(a + r * s); nb[u] = ld_stream(b + r * s);
+            nc[u] = ld_stream(c + r * s); nd[u] = ld_stream(d + r * s);
+        }
+    }
+    for (int r0 = 2; r0 < m; r0 += U) {
+        double ca[U], cb[U], cc[U], cd[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { ca[u] = na[u]; cb[u] = nb[u]; cc[u] = nc[u]; cd[u] = nd[u]; }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {                    // next chunk's loads go out first
+            const int r = r0 + U + u;
+            if (r < m) {
+                na[u] = ld_stream(a + r * s); nb[u] = ld_stream(b + r * s);
+                nc[u] = ld_stream(c + r * s); nd[u] = ld_stream(d + r * s);
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int r = r0 + u;
+            if (r < m) {
+                // fold row r-1 into the first-row equation, then hand it to stage C
+                fb = fma(-fc, pa, fb);
+                fd = fma(-fc, pd, fd);
+                fc = -fc * pc;
+                st_keep(sa + (r - 1) * s, pa);
+                st_keep(sc + (r - 1) * s, pc);
+                st_keep(sd + (r - 1) * s, pd);
+                const double ar = ca[u];
+                const double cr = (last_part && r == m - 1) ? 0.0 : cc[u];
+                inv = 1.0 / fma(-ar, pc, cb[u]);
+                pd = fma(-ar, pd, cd[u]) * inv;
+                pc = cr * inv;
+                pa = -(ar * pa) * inv;
+            }
+        }
+    }
+    // m == 2: first-row equation is already (fa, 1, fc | fd) with frontier x_1 = x_{m-1}
+    inv = 1.0 / fb;
+    const size_t Lb = (size_t)prm.Lb;
+    if (kSeparateGather) {
+        double *__restrict__ sp = prm.send + (size_t)p * 6 * Lb + l;
+        st_keep(sp, fa * inv); st_keep(sp + Lb, fc * inv); st_keep(sp + 2 * Lb, fd * inv);
+        st_keep(sp + 3 * Lb, pa); st_keep(sp + 4 * Lb, pc); st_keep(sp + 5 * Lb, pd);
+    } else {
+        const size_t q0 = (size_t)(2 * p) * Lb + l, q1 = q0 + Lb;
+        st_keep(prm.ra + q0, fa * inv); st_keep(prm.rc + q0, fc * inv); st_keep(prm.rd + q0, fd * inv);
+        st_keep(prm.ra + q1, pa); st_keep(prm.rc + q1, pc); st_keep(prm.rd + q1, pd);
+    }
+}
+
+// Separate A2B gather ("Save data in send_A" / "Get data from recv_B"):
+// send[p][6][Lb] -> RA/RC/RD[2P][Lb].  One thread per (line, partition).
+__global__ void __launch_bounds__(256) gather_kernel(const StageParams prm)
+{
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= prm.Lb) return;
+    const int p = blockIdx.y;
+    const size_t Lb = (size_t)prm.Lb;
+    const double *__restrict__ sp = prm.send + (size_t)p * 6 * Lb + l;
+    const size_t q0 = (size_t)(2 * p) * Lb + l, q1 = q0 + Lb;
+    st_keep(prm.ra + q0, ld_keep(sp)); st_keep(prm.rc + q0, ld_keep(sp + Lb));
+    st_keep(prm.rd + q0, ld_keep(sp + 2 * Lb));
+    st_keep(prm.ra + q1, ld_keep(sp + 3 * Lb)); st_keep(prm.rc + q1, ld_keep(sp + 4 * Lb));
+    st_keep(prm.rd + q1, ld_keep(sp + 5 * Lb));
+}
+
+// ------------------------------------------------------------------------------------------
+// Stage B: Thomas on the 2P-row reduced system (unit diagonal), one thread per line.
+// Low occupancy by construction; runs on its own high-priority stream.
+// ------------------------------------------------------------------------------------------
+template <int U>
+__global__ void __launch_bounds__(64) stage_b_kernel(const StageParams prm)
+{
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= prm.Lb) return;
+    const size_t Lb = (size_t)prm.Lb;
+    const int Q = 2 * prm.P;
+    const double *__restrict__ ra = prm.ra + l;
+    const double *__restrict__ rc = prm.rc + l;
+    const double *__restrict__ rd = prm.rd + l;
+    double *__restrict__ cpb = prm.cp + l;
+    double *__restrict__ y = prm.y + l;
+
+    double cp = ld_keep(rc), dp = ld_keep(rd);          // row 0: sub-diagonal is 0
+    st_keep(cpb, cp); st_keep(y, dp);
+    double na[U], nc[U], nd[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const int q = 1 + u;
+        if (q < Q) { na[u] = ld_keep(ra + q * Lb); nc[u] = ld_keep(rc + q * Lb); nd[u] = ld_keep(rd + q * Lb); }
+    }
+    for (int q0 = 1; q0 < Q; q0 += U) {
+        double ca[U], cc[U], cd[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { ca[u] = na[u]; cc[u] = nc[u]; cd[u] = nd[u]; }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int q = q0 + U + u;
+            if (q < Q) { na[u] = ld_keep(ra + q * Lb); nc[u] = ld_keep(rc + q * Lb); nd[u] = ld_keep(rd + q * Lb); }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int q = q0 + u;
+            if (q < Q) {
+                const double inv = 1.0 / fma(-ca[u], cp, 1.0);
+                dp = fma(-ca[u], dp, cd[u]) * inv;
+                cp = cc[u] * inv;
+                st_keep(cpb + q * Lb, cp);
+                st_keep(y + q * Lb, dp);
+            }
+        }
+    }
+    // back substitution; the last row's cp is 0 by construction (c_{ny-1} := 0)
+    double xq = dp;
+    for (int q = Q - 2; q >= 0; --q) {
+        xq = fma(-ld_keep(cpb + q * Lb), xq, ld_keep(y + q * Lb));
+        st_keep(y + q * Lb, xq);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Stage C: back-substitution inside each partition, one thread per (line, partition).
+// ------------------------------------------------------------------------------------------
+template <int U>
+__global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
+{
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= prm.Lb) return;
+    const int p = blockIdx.y;
+    const int nx = prm.nx, m = prm.m;
+    const long long kk = l / nx;
+    const int i = (int)(l - kk * nx);
+    const size_t off0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
+    const double *__restrict__ sa = prm.sa + off0;
+    const double *__restrict__ sc = prm.sc + off0;
+    const double *__restrict__ sd = prm.sd + off0;
+    double *__restrict__ x = prm.x + off0;
+    const size_t s = (size_t)nx;
+    const size_t Lb = (size_t)prm.Lb;
+
+    const double xf = ld_keep(prm.y + (size_t)(2 * p) * Lb + l);
+    const double xl = ld_keep(prm.y + (size_t)(2 * p + 1) * Lb + l);
+    st_stream(x, xf);
+    st_stream(x + (size_t)(m - 1) * s, xl);
+    double xn = xl;
+
+    double na[U], nc[U], nd[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        const int r = m - 2 - u;
+        if (r >= 1) { na[u] = ld_keep(sa + r * s); nc[u] = ld_keep(sc + r * s); nd[u] = ld_keep(sd + r * s); }
+    }
+    for (int r0 = m - 2; r0 >= 1; r0 -= U) {
+        double ca[U], cc[U], cd[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { ca[u] = na[u]; cc[u] = nc[u]; cd[u] = nd[u]; }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int r = r0 - U - u;
+            if (r >= 1) { na[u] = ld_keep(sa + r * s); nc[u] = ld_keep(sc + r * s); nd[u] = ld_keep(sd + r * s); }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int r = r0 - u;
+            if (r >= 1) {
+                xn = fma(-cc[u], xn, fma(-ca[u], xf, cd[u]));
+                st_stream(x + r * s, xn);
+            }
+        }
+    }
+}
+
+// ny == 1 (only possible with P == 1): x = d / b.
+__global__ void __launch_bounds__(256) diagonal_kernel(const double *__restrict__ b,
+                                                       const double *__restrict__ d,
+                                                       double *__restrict__ x, size_t n)
+{
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n) x[t] = d[t] / b[t];
+}
+
+}  // namespace tdma

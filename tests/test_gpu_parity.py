@@ -1,0 +1,398 @@
+"""Parity tests proper: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances (BASELINE.json north_star):
+
+  * strictly dominant configs (1, 4-y, 5):  E = max_lines ||x - x_or||_inf / ||x_or||_inf <= 1e-11
+    and the literal residual  ||Ax - d||_inf <= 1e-12 ||d||_inf  per line;
+  * weakly dominant Poisson configs (2, 3): E <= 1e-11 against the LONG-DOUBLE oracle and the
+    normwise backward error ||Ax-d||_inf / (||A||_inf ||x||_inf + ||d||_inf) <= 1e-12; the literal
+    residual is reported next to the oracle's own (fp64 Thomas does not meet it either on the
+    lowest wavenumbers).
+Residuals are evaluated on the host in long double.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import tdma_inputs
+import paper_2509_03933_b200 as tdma
+
+from test_golden import load_cfg1_golden
+
+pytestmark = pytest.mark.gpu
+
+TOL_E = 1e-11
+TOL_RES = 1e-12
+VARIANTS = [tdma.TDMA_VARIANT_PIPELINED, tdma.TDMA_VARIANT_FUSED]
+
+
+def dev():
+    return torch.device("cuda:0")
+
+
+def gpu_solve(a, b, c, d, P, batch=0, out=None, **opts):
+    nz, ny, nx = a.shape
+    x = torch.full_like(d, float("nan")) if out is None else out
+    with tdma.Plan(nx, ny, nz, P, batch, **opts) as plan:
+        plan.solve(a, b, c, d, x)
+        torch.cuda.synchronize()
+    return x
+
+
+def to_np(*ts):
+    return [t.detach().cpu().numpy() for t in ts]
+
+
+def check_against_oracle(a, b, c, d, x, strictly_dominant, precision=None):
+    an, bn, cn, dn, xn = to_np(a, b, c, d, x)
+    assert np.isfinite(xn).all()
+    prec = precision or ("f64" if strictly_dominant else "ld")
+    ref = oracle.solve_y(an, bn, cn, dn, prec)
+    E = oracle.normwise_error(xn, ref)
+    res, dinf, xinf, ainf = oracle.residual_y(an, bn, cn, dn, xn)
+    assert E.max() <= TOL_E, "normwise error %.3e" % E.max()
+    bwd = res / (ainf * xinf + dinf + 1e-300)
+    assert bwd.max() <= TOL_RES
+    if strictly_dominant:
+        assert (res <= TOL_RES * dinf).all(), "literal residual %.3e" % (res / dinf).max()
+    return E.max()
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE configs
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("batch", [0, 1, 24])
+def test_cfg1_tiny_full(variant, batch):
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, variant=variant)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, True)
+    xn = x.cpu().numpy()
+    for i, k, ref in load_cfg1_golden():
+        assert np.max(np.abs(xn[k, :, i] - ref)) <= TOL_E * np.max(np.abs(ref))
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_cfg2_poisson_full(variant):
+    w = tdma_inputs.make_workload("cfg2_poisson", device=dev())
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, w.batch, variant=variant)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, False)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_cfg4_adi_y_slab(variant):
+    """512 x 512 x 48 slices of cfg 4 (full nx, ny, P; ragged last batch 48 = 32 + 16)."""
+    w = tdma_inputs.make_workload("cfg4_adi_y", device=dev(), nz=48)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 32, variant=variant)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, True)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_cfg5_stress_slab(variant):
+    """2048 x 512 x 20 slices of cfg 5 (m = 8, 128-row reduced system), batch 8 -> 8+8+4."""
+    w = tdma_inputs.make_workload("cfg5_stress", device=dev(), nz=20)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=variant, nstreams=3)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, True)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_cfg3_weak_slab(variant):
+    """1024 x 1024 x 12 slices of cfg 3 starting at k = 0 (holds the pinned (0,0) mode and the
+    lowest wavenumbers = the worst-conditioned lines), batch 8 -> 8 + 4."""
+    w = tdma_inputs.make_workload("cfg3_weak", device=dev(), nz=12)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=variant)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, False)
+
+
+# ---------------------------------------------------------------------------------------------
+# Full-size runs in the launch configuration bench.py times, sampled slices
+# ---------------------------------------------------------------------------------------------
+def _sampled_full(name, variant, batch, slices, strictly, **opts):
+    free, _ = torch.cuda.mem_get_info()
+    spec = tdma_inputs.config_spec(name)
+    need = spec["nx"] * spec["ny"] * spec["nz"] * 8 * 5 * 1.25
+    if free < need:
+        pytest.skip("needs %.0f GB of device memory" % (need / 1e9))
+    w = tdma_inputs.make_workload(name, device=dev())
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, variant=variant, **opts)
+    assert bool(torch.isfinite(x).all())
+    worst = 0.0
+    for k in slices:
+        sl = slice(k, k + 1)
+        worst = max(worst, check_against_oracle(w.a[sl], w.b[sl], w.c[sl], w.d[sl], x[sl], strictly))
+    # a property that holds at any size: for the Poisson lines away from the pinned mode the
+    # column sums of A vanish except for -k^2, so sum_j d_j = -(kx^2+kz^2) sum_j x_j  (Neumann)
+    del w, x
+    torch.cuda.empty_cache()
+    return worst
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_cfg3_full_size_sampled(variant):
+    _sampled_full("cfg3_weak", variant, 32, [0, 1, 513, 1023], False)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_cfg5_full_size_sampled(variant):
+    _sampled_full("cfg5_stress", variant, 16, [0, 777, 1023], True, nstreams=3)
+
+
+# ---------------------------------------------------------------------------------------------
+# Schedule invariance: per-line arithmetic does not depend on batching,
+# stream count, graph capture or gather placement -> bitwise identical x
+# ---------------------------------------------------------------------------------------------
+def test_schedule_invariance_pipelined():
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    base = gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_PIPELINED, nstreams=1)
+    for batch in (1, 2, 7, 16, 64):
+        for opts in (dict(nstreams=2), dict(nstreams=3), dict(nstreams=4, use_graph=-1),
+                     dict(nstreams=2, separate_gather=1), dict(nstreams=1, use_graph=-1)):
+            x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, variant=tdma.TDMA_VARIANT_PIPELINED, **opts)
+            assert torch.equal(x, base), (batch, opts)
+
+
+def test_schedule_invariance_fused_batches():
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    base = gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED)
+    for batch in (1, 5, 32):
+        x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, variant=tdma.TDMA_VARIANT_FUSED)
+        assert torch.equal(x, base)
+
+
+@pytest.mark.parametrize("cluster,lines", [(1, 32), (2, 32), (4, 16), (4, 32), (2, 8), (4, 64)])
+def test_fused_cluster_shapes(cluster, lines):
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED,
+                  fused_cluster=cluster, fused_lines=lines)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, True)
+
+
+def test_fused_cluster8():
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev(), P=8)
+    x = gpu_solve(w.a, w.b, w.c, w.d, 8, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_cluster=8,
+                  fused_lines=32)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, True)
+
+
+def _view(ptr, nbytes, shape):
+    """Wrap a plan-owned device buffer as a torch tensor without copying."""
+    n = int(np.prod(shape))
+    assert n * 8 <= nbytes
+
+    class _Holder:
+        pass
+    h = _Holder()
+    h.__cuda_array_interface__ = {"shape": tuple(shape), "typestr": "<f8", "data": (ptr, False),
+                                  "version": 3, "strides": None}
+    return torch.as_tensor(h, device=dev())
+
+
+def test_repeated_solves_with_poisoned_scratch_and_graph_cache():
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    x1 = torch.empty_like(w.d)
+    x2 = torch.empty_like(w.d)
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 8, variant=tdma.TDMA_VARIANT_PIPELINED, nstreams=3) as plan:
+        plan.solve(w.a, w.b, w.c, w.d, x1)
+        torch.cuda.synchronize()
+        for which in (tdma.TDMA_BUF_SA, tdma.TDMA_BUF_SC, tdma.TDMA_BUF_SD, tdma.TDMA_BUF_RA,
+                      tdma.TDMA_BUF_RC, tdma.TDMA_BUF_RD, tdma.TDMA_BUF_Y):
+            for slot in range(plan.get(tdma.TDMA_GET_DEPTH)):
+                ptr, nbytes = plan.buffer(which, slot)
+                _view(ptr, nbytes, (nbytes // 8,)).fill_(float("nan"))
+        torch.cuda.synchronize()
+        plan.solve(w.a, w.b, w.c, w.d, x2)          # same inputs, other x -> a second graph
+        x1.fill_(float("nan"))
+        plan.solve(w.a, w.b, w.c, w.d, x1)          # cached graph
+        torch.cuda.synchronize()
+        assert plan.get(tdma.TDMA_GET_GRAPH_BUILDS) == 2
+    assert torch.equal(x1, x2)
+    check_against_oracle(w.a, w.b, w.c, w.d, x1, True)
+
+
+# ---------------------------------------------------------------------------------------------
+# Degenerate and ragged cases
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("shape,P,batch", [
+    ((7, 64, 100), 4, 3),      # nx not a multiple of 32 (pipelined) / of 8 handled below
+    ((3, 32, 8), 16, 2),       # m = 2: partitions without interior rows
+    ((1, 48, 64), 1, 0),       # P = 1 degenerates to a plain solve
+    ((5, 6, 16), 3, 5),        # m = 2, tiny
+    ((2, 96, 40), 2, 1),       # m = 48
+    ((9, 30, 24), 5, 4),       # m = 6, nz % batch != 0
+    ((1, 2, 8), 1, 0),         # ny = 2
+])
+def test_shapes(variant, shape, P, batch):
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 11, dev())
+    try:
+        x = gpu_solve(a, b, c, d, P, batch, variant=variant)
+    except tdma.TdmaError as exc:
+        if variant == tdma.TDMA_VARIANT_FUSED and "fused variant unavailable" in str(exc):
+            pytest.skip(str(exc))
+        raise
+    check_against_oracle(a, b, c, d, x, True)
+
+
+@pytest.mark.parametrize("shape,P", [((4, 16, 1), 4), ((1, 16, 37), 2), ((3, 1, 5), 1), ((2, 10, 3), 1)])
+def test_odd_nx_pipelined(shape, P):
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 5, dev())
+    x = gpu_solve(a, b, c, d, P, 0, variant=tdma.TDMA_VARIANT_PIPELINED)
+    check_against_oracle(a, b, c, d, x, True)
+
+
+def test_fused_rejects_unsupported_nx():
+    with pytest.raises(tdma.TdmaError) as ei:
+        tdma.Plan(37, 16, 2, 2, 0, variant=tdma.TDMA_VARIANT_FUSED)
+    assert "fused variant unavailable" in str(ei.value)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_identity_and_diagonal(variant):
+    for diag in (False, True):
+        a, b, c, d = tdma_inputs.identity_system(32, 16, 3, 2, dev(), diagonal_only=diag)
+        x = gpu_solve(a, b, c, d, 4, 2, variant=variant)
+        assert torch.allclose(x, d / b, rtol=4e-16, atol=0)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_corner_entries_are_ignored(variant):
+    a, b, c, d = tdma_inputs.dominant_random(32, 24, 2, 3, dev())
+    x0 = gpu_solve(a, b, c, d, 4, 0, variant=variant)
+    a2, c2 = a.clone(), c.clone()
+    a2[:, 0, :] = float("nan")
+    c2[:, -1, :] = float("inf")
+    x1 = gpu_solve(a2, b, c2, d, 4, 0, variant=variant)
+    assert torch.equal(x0, x1)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_in_place_x_aliases_d(variant):
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    ref = gpu_solve(w.a, w.b, w.c, w.d, w.P, 16, variant=variant)
+    buf = w.d.clone()
+    gpu_solve(w.a, w.b, w.c, buf, w.P, 16, out=buf, variant=variant)
+    assert torch.equal(buf, ref)
+
+
+def test_inputs_are_not_written():
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    keep = [t.clone() for t in (w.a, w.b, w.c, w.d)]
+    for variant in VARIANTS:
+        gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=variant)
+    for t, k in zip((w.a, w.b, w.c, w.d), keep):
+        assert torch.equal(t, k)
+
+
+def test_manufactured_solution_on_gpu():
+    """P2 through the CUDA path: d = A x* (long double on the host), recover x*."""
+    rng = np.random.default_rng(0)
+    a, b, c, _ = tdma_inputs.dominant_random(64, 128, 3, 9, "cpu")
+    xstar = rng.uniform(-1, 1, (3, 128, 64))
+    d = oracle.apply_y(a.numpy(), b.numpy(), c.numpy(), xstar)
+    dd = torch.from_numpy(d).to(dev())
+    for variant in VARIANTS:
+        x = gpu_solve(a.to(dev()), b.to(dev()), c.to(dev()), dd, 8, 2, variant=variant)
+        assert oracle.normwise_error(x.cpu().numpy(), xstar).max() <= 1e-14
+
+
+def test_toeplitz_closed_form_on_gpu():
+    """P4 through the CUDA path: eigen-form of a=c=-alpha, b=1+2alpha."""
+    n, alpha, nx = 512, 3.7, 32
+    j = np.arange(1, n + 1)
+    a = torch.full((1, n, nx), -alpha, dtype=torch.float64, device=dev())
+    b = torch.full((1, n, nx), 1 + 2 * alpha, dtype=torch.float64, device=dev())
+    d = np.zeros((1, n, nx))
+    ref = np.zeros((1, n, nx))
+    for q in range(1, nx + 1):
+        mode = np.sin(np.pi * q * j / (n + 1))
+        lam = 1 + 2 * alpha - 2 * alpha * np.cos(np.pi * q / (n + 1))
+        d[0, :, q - 1] = mode
+        ref[0, :, q - 1] = mode / lam
+    dd = torch.from_numpy(d).to(dev())
+    for variant in VARIANTS:
+        x = gpu_solve(a, b, a, dd, 8, 0, variant=variant)
+        assert oracle.normwise_error(x.cpu().numpy(), ref).max() <= (1 + 4 * alpha) * 2e-14
+
+
+# ---------------------------------------------------------------------------------------------
+# Stage level
+# ---------------------------------------------------------------------------------------------
+def test_stage_level_reduced_system_and_forward_rows():
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    P, m, Lb = w.P, w.ny // w.P, w.nx * w.nz
+    an, bn, cn, dn = to_np(w.a, w.b, w.c, w.d)
+    ref = oracle.solve_y(an, bn, cn, dn)                          # (nz, ny, nx)
+    x = torch.empty_like(w.d)
+    with tdma.Plan(w.nx, w.ny, w.nz, P, 0, variant=tdma.TDMA_VARIANT_PIPELINED) as plan:
+        # stage-isolated entry point, in Alg. 1 order
+        for st in (tdma.TDMA_STAGE_A, tdma.TDMA_STAGE_B, tdma.TDMA_STAGE_C):
+            plan.stage(st, 0, w.a, w.b, w.c, w.d, x)
+        torch.cuda.synchronize()
+        bufs = {}
+        for name, which, shape in [("RA", tdma.TDMA_BUF_RA, (2 * P, Lb)), ("RC", tdma.TDMA_BUF_RC, (2 * P, Lb)),
+                                   ("RD", tdma.TDMA_BUF_RD, (2 * P, Lb)), ("Y", tdma.TDMA_BUF_Y, (2 * P, Lb)),
+                                   ("SA", tdma.TDMA_BUF_SA, (w.nz, w.ny, w.nx)),
+                                   ("SC", tdma.TDMA_BUF_SC, (w.nz, w.ny, w.nx)),
+                                   ("SD", tdma.TDMA_BUF_SD, (w.nz, w.ny, w.nx))]:
+            ptr, nbytes = plan.buffer(which, 0)
+            bufs[name] = _view(ptr, nbytes, shape).clone().cpu().numpy()
+        x_full = torch.empty_like(w.d)
+        plan.solve(w.a, w.b, w.c, w.d, x_full)
+        torch.cuda.synchronize()
+    assert torch.equal(x, x_full)                                  # stage API == whole solve
+    RA, RC, RD, Y = bufs["RA"], bufs["RC"], bufs["RD"], bufs["Y"]
+    # P6: diagonal dominance of the reduced system, zero corners, Y = oracle x at partition ends
+    assert (np.abs(RA) + np.abs(RC) < 1).all()
+    assert (RA[0] == 0).all() and (RC[2 * P - 1] == 0).all()
+    ref_lines = ref.transpose(1, 0, 2).reshape(w.ny, Lb)           # line index = i + nx*k
+    for p in range(P):
+        assert np.max(np.abs(Y[2 * p] - ref_lines[p * m])) <= 1e-14
+        assert np.max(np.abs(Y[2 * p + 1] - ref_lines[p * m + m - 1])) <= 1e-14
+        # reduced rows hold for the oracle solution
+        xf, xl = ref_lines[p * m], ref_lines[p * m + m - 1]
+        xprev = ref_lines[p * m - 1] if p > 0 else 0 * xf
+        xnext = ref_lines[p * m + m] if p < P - 1 else 0 * xf
+        assert np.max(np.abs(RA[2 * p] * xprev + xf + RC[2 * p] * xl - RD[2 * p])) <= 1e-14
+        assert np.max(np.abs(RA[2 * p + 1] * xf + xl + RC[2 * p + 1] * xnext - RD[2 * p + 1])) <= 1e-14
+    # P5 (forward-form rows): a'_r x_0 + x_r + c'_r x_{r+1} = d'_r for interior rows
+    SA, SC, SD = bufs["SA"], bufs["SC"], bufs["SD"]
+    for p in range(P):
+        x0 = ref[:, p * m, :]
+        for r in range(1, m - 1):
+            j = p * m + r
+            lhs = SA[:, j, :] * x0 + ref[:, j, :] + SC[:, j, :] * ref[:, j + 1, :]
+            assert np.max(np.abs(lhs - SD[:, j, :])) <= 1e-14
+
+
+# ---------------------------------------------------------------------------------------------
+# Host-buffer entry point
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_solve_host_matches_device_solve(variant):
+    w = tdma_inputs.make_workload("cfg2_poisson", device="cpu", nx=64, nz=40)
+    host = [t.pin_memory() for t in (w.a, w.b, w.c, w.d)]
+    xh = torch.empty_like(w.d).pin_memory()
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 4, variant=variant) as plan:
+        plan.solve_host(*host, xh)
+        xd = torch.empty_like(w.d, device=dev())
+        plan.solve(*[t.to(dev()) for t in host], xd)
+        torch.cuda.synchronize()
+    assert torch.equal(xh, xd.cpu())
+    check_against_oracle(w.a, w.b, w.c, w.d, xh, False)
+
+
+def test_solve_on_non_default_stream_orders_with_later_work():
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    ref = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=tdma.TDMA_VARIANT_PIPELINED)
+    s = torch.cuda.Stream()
+    x = torch.zeros_like(w.d)
+    y = torch.zeros_like(w.d)
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 8, variant=tdma.TDMA_VARIANT_PIPELINED, use_graph=-1) as plan:
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            plan.solve(w.a, w.b, w.c, w.d, x, stream=s)
+            y.copy_(x)                       # later work on the same stream must see x
+        s.synchronize()
+    assert torch.equal(y, ref)
