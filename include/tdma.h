@@ -79,9 +79,13 @@ typedef struct tdma_options {
     int separate_gather; /* 1 = stage A writes a send_A buffer and a separate gather kernel
                             assembles the reduced system (the paper's A2B);
                             default 0 = gather fused into stage A's epilogue */
-    int fused_lines;     /* FUSED: lines (x extent) per cluster tile, 0 = auto */
-    int fused_cluster;   /* FUSED: CTAs per cluster (1, 2, 4, 8), 0 = auto */
-    int reserved[8];
+    int fused_lines;     /* FUSED: lines (x extent) per cluster tile (8, 16, 32), 0 = auto */
+    int fused_cluster;   /* FUSED: CTAs per cluster (1, 2, 4, 8, 16), 0 = auto */
+    int fused_leaf_rows; /* FUSED: rows per thread-level leaf (a divisor of ny/P, >= 2), 0 = auto */
+    int fused_top;       /* FUSED: 1 = the cluster exchanges / solves the 2P-row reduced system as
+                            is; 2 = every CTA first reduces its 2P/cluster rows to two (same
+                            recursion), the cluster solves 2*cluster rows; 0 = auto */
+    int reserved[6];
 } tdma_options;
 
 /* Plan for an nx*ny*nz slab with y split into P partitions of ny/P rows and `batch` z-slices per
@@ -130,7 +134,12 @@ typedef enum tdma_query {
     TDMA_GET_LAUNCHES = 6, /* kernel launches one tdma_solve enqueues               */
     TDMA_GET_FUSED_LINES = 7,
     TDMA_GET_FUSED_CLUSTER = 8,
-    TDMA_GET_GRAPH_BUILDS = 9 /* CUDA graphs captured so far (cache misses)        */
+    TDMA_GET_GRAPH_BUILDS = 9, /* CUDA graphs captured so far (cache misses)       */
+    TDMA_GET_FUSED_LEAF_ROWS = 10, /* rows per thread-level leaf                    */
+    TDMA_GET_FUSED_TOP = 11,       /* resolved fused_top                            */
+    TDMA_GET_FUSED_THREADS = 12,   /* threads per CTA                               */
+    TDMA_GET_FUSED_SMEM = 13,      /* dynamic shared memory per CTA, bytes          */
+    TDMA_GET_FUSED_TOP_ROWS = 14   /* rows of the cluster-level system per line     */
 } tdma_query;
 int tdma_plan_get(const tdma_plan *plan, int what); /* < 0 on error */
 size_t tdma_plan_workspace_bytes(const tdma_plan *plan); /* device bytes the plan owns */

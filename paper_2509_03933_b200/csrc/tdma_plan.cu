@@ -220,8 +220,7 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
         const int bzn = std::min(pl->bz, nz_count - k0);
         const size_t off = (size_t)k0 * pl->slice;
         cudaError_t e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
-                                           ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, pl->P,
-                                           origin);
+                                           ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
         if (e != cudaSuccess)
             return set_err(TDMA_ERR_CUDA, "fused launch failed: %s", cudaGetErrorString(e));
     }
@@ -364,8 +363,11 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
     }
     if (variant == TDMA_VARIANT_FUSED && pl->ny > 1) {
         const char *why = nullptr;
+        if ((size_t)pl->nx * (size_t)pl->m >= ((size_t)1 << 32))
+            return set_err(TDMA_ERR_UNSUPPORTED, "fused variant: nx * ny/P exceeds 2^32 elements");
         if (!tdma::configure_fused(&pl->fused, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
-                                   opt ? opt->fused_cluster : 0, prop, &why))
+                                   opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
+                                   opt ? opt->fused_top : 0, prop, &why))
             return set_err(TDMA_ERR_UNSUPPORTED, "fused variant unavailable: %s", why ? why : "?");
     }
     return TDMA_OK;
@@ -508,6 +510,11 @@ int tdma_plan_get(const tdma_plan *plan, int what)
     case TDMA_GET_FUSED_LINES: return plan->fused.lines;
     case TDMA_GET_FUSED_CLUSTER: return plan->fused.cluster;
     case TDMA_GET_GRAPH_BUILDS: return plan->graph_builds;
+    case TDMA_GET_FUSED_LEAF_ROWS: return plan->fused.leaf_rows;
+    case TDMA_GET_FUSED_TOP: return plan->fused.top_mode;
+    case TDMA_GET_FUSED_THREADS: return plan->fused.threads;
+    case TDMA_GET_FUSED_SMEM: return (int)plan->fused.smem;
+    case TDMA_GET_FUSED_TOP_ROWS: return 2 * plan->fused.top_nodes * plan->fused.cluster;
     default: return set_err(TDMA_ERR_INVALID_ARG, "unknown query %d", what);
     }
 }

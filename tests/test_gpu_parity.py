@@ -159,19 +159,48 @@ def test_schedule_invariance_fused_batches():
         assert torch.equal(x, base)
 
 
-@pytest.mark.parametrize("cluster,lines", [(1, 32), (2, 32), (4, 16), (4, 32), (2, 8), (4, 64)])
-def test_fused_cluster_shapes(cluster, lines):
+@pytest.mark.parametrize("cluster,lines,leaf,top", [
+    (1, 32, 0, 0), (2, 32, 0, 0), (4, 16, 0, 0), (4, 32, 0, 0), (2, 8, 0, 0),
+    (1, 32, 16, 1), (1, 32, 16, 2),      # leaf = partition: no partition level
+    (1, 32, 4, 1), (1, 32, 4, 2),        # 4 leaves per partition, 2P-row / 2-row top system
+    (2, 32, 2, 1), (2, 32, 2, 2),        # two-row leaves (no interior)
+    (4, 32, 8, 1), (4, 32, 8, 2), (2, 16, 8, 2), (4, 8, 4, 1),
+])
+def test_fused_cluster_shapes(cluster, lines, leaf, top):
     w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED,
-                  fused_cluster=cluster, fused_lines=lines)
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_cluster=cluster,
+                   fused_lines=lines, fused_leaf_rows=leaf, fused_top=top) as plan:
+        assert plan.get(tdma.TDMA_GET_FUSED_CLUSTER) == cluster
+        assert plan.get(tdma.TDMA_GET_FUSED_LINES) == lines
+        if leaf:
+            assert plan.get(tdma.TDMA_GET_FUSED_LEAF_ROWS) == leaf
+        if top == 1:
+            assert plan.get(tdma.TDMA_GET_FUSED_TOP_ROWS) == 2 * w.P
+        if top == 2:
+            assert plan.get(tdma.TDMA_GET_FUSED_TOP_ROWS) == 2 * cluster
+        x = torch.full_like(w.d, float("nan"))
+        plan.solve(w.a, w.b, w.c, w.d, x)
+        torch.cuda.synchronize()
     check_against_oracle(w.a, w.b, w.c, w.d, x, True)
 
 
-def test_fused_cluster8():
-    w = tdma_inputs.make_workload("cfg1_tiny", device=dev(), P=8)
-    x = gpu_solve(w.a, w.b, w.c, w.d, 8, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_cluster=8,
-                  fused_lines=32)
+@pytest.mark.parametrize("cluster,top", [(8, 1), (8, 2), (16, 2)])
+def test_fused_cluster8_16(cluster, top):
+    P = 16 if cluster == 16 else 8
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev(), P=P)
+    x = gpu_solve(w.a, w.b, w.c, w.d, P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_cluster=cluster,
+                  fused_lines=32, fused_top=top)
     check_against_oracle(w.a, w.b, w.c, w.d, x, True)
+
+
+def test_fused_top_modes_agree_with_pipelined_to_rounding():
+    """The 2P-row reduced system is a Schur complement: however the recursion is cut, the result
+    is the same up to rounding (cfg 2 slab, weakly dominant lines included)."""
+    w = tdma_inputs.make_workload("cfg2_poisson", device=dev(), nz=6)
+    xs = [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_top=top,
+                    fused_leaf_rows=leaf) for top, leaf in ((1, 0), (2, 0), (1, 32), (2, 4))]
+    for x in xs:
+        check_against_oracle(w.a, w.b, w.c, w.d, x, False)
 
 
 def _view(ptr, nbytes, shape):
@@ -242,10 +271,24 @@ def test_odd_nx_pipelined(shape, P):
     check_against_oracle(a, b, c, d, x, True)
 
 
-def test_fused_rejects_unsupported_nx():
-    with pytest.raises(tdma.TdmaError) as ei:
-        tdma.Plan(37, 16, 2, 2, 0, variant=tdma.TDMA_VARIANT_FUSED)
+@pytest.mark.parametrize("shape,P", [((4, 16, 1), 4), ((1, 16, 37), 2), ((2, 10, 3), 1), ((3, 64, 45), 4)])
+def test_odd_nx_fused(shape, P):
+    """Ragged x tail: lanes past nx compute a copy of the last line and store nothing."""
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 5, dev())
+    guard = torch.full((nz * ny * nx + 64,), float("nan"), dtype=torch.float64, device=dev())
+    x = guard[:nz * ny * nx].view(nz, ny, nx)
+    gpu_solve(a, b, c, d, P, 0, variant=tdma.TDMA_VARIANT_FUSED, out=x)
+    assert torch.isnan(guard[nz * ny * nx:]).all()
+    check_against_oracle(a, b, c, d, x, True)
+
+
+def test_fused_rejects_what_it_cannot_tile():
+    with pytest.raises(tdma.TdmaError) as ei:     # P = 1 keeps the whole line in one CTA
+        tdma.Plan(64, 4096, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED)
     assert "fused variant unavailable" in str(ei.value)
+    with pytest.raises(tdma.TdmaError):
+        tdma.Plan(64, 64, 2, 4, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_lines=64)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
