@@ -85,7 +85,11 @@ typedef struct tdma_options {
     int fused_top;       /* FUSED: 1 = the cluster exchanges / solves the 2P-row reduced system as
                             is; 2 = every CTA first reduces its 2P/cluster rows to two (same
                             recursion), the cluster solves 2*cluster rows; 0 = auto */
-    int reserved[6];
+    int fused_impl;      /* FUSED: 1 = register-staged kernel with a general fan-in tree (any nx,
+                            any divisor leaf); 2 = TMA kernel (tile fetched by bulk tensor copies,
+                            reduced in place, pairwise tree; needs even nx and power-of-two
+                            leaf counts); 0 = auto (2 when eligible, else 1) */
+    int reserved[5];
 } tdma_options;
 
 /* Plan for an nx*ny*nz slab with y split into P partitions of ny/P rows and `batch` z-slices per
@@ -139,7 +143,8 @@ typedef enum tdma_query {
     TDMA_GET_FUSED_TOP = 11,       /* resolved fused_top                            */
     TDMA_GET_FUSED_THREADS = 12,   /* threads per CTA                               */
     TDMA_GET_FUSED_SMEM = 13,      /* dynamic shared memory per CTA, bytes          */
-    TDMA_GET_FUSED_TOP_ROWS = 14   /* rows of the cluster-level system per line     */
+    TDMA_GET_FUSED_TOP_ROWS = 14,  /* rows of the cluster-level system per line     */
+    TDMA_GET_FUSED_IMPL = 15       /* resolved fused_impl                           */
 } tdma_query;
 int tdma_plan_get(const tdma_plan *plan, int what); /* < 0 on error */
 size_t tdma_plan_workspace_bytes(const tdma_plan *plan); /* device bytes the plan owns */

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libtdma.so")
 SOURCES = ["tdma_plan.cu"]
-HEADERS = ["tdma_stage_kernels.cuh", "tdma_fused.cuh", os.path.join("..", "..", "include", "tdma.h")]
+HEADERS = ["tdma_stage_kernels.cuh", "tdma_fused.cuh", "tdma_fused_tma.cuh", os.path.join("..", "..", "include", "tdma.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -12,8 +12,14 @@
 #include <new>
 #include <vector>
 
+#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
+namespace tdma { long long *g_tdma_dbg = nullptr; }
+extern "C" void *tdma_dbg_buffer(void) { return tdma::g_tdma_dbg; }
+#endif
+
 #include "tdma_stage_kernels.cuh"
 #include "tdma_fused.cuh"
+#include "tdma_fused_tma.cuh"
 
 #define TDMA_VERSION_NUM 10100
 
@@ -76,6 +82,8 @@ struct tdma_plan {
     int graph_builds = 0;
     // FUSED
     tdma::FusedConfig fused;
+    int fused_impl = 0;  // 1 = register-staged general tree, 2 = TMA / pairwise tree
+    tdma::TmaFusedConfig tfused;
     // host staging (tdma_solve_host), allocated on first use
     int hz = 0;  // slices per host chunk
     double *stage_dev[2][5] = {};
@@ -219,8 +227,17 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
         const int k0 = n * pl->bz;
         const int bzn = std::min(pl->bz, nz_count - k0);
         const size_t off = (size_t)k0 * pl->slice;
-        cudaError_t e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
-                                           ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
+        cudaError_t e;
+        const bool aligned = ((((uintptr_t)ptr.a | (uintptr_t)ptr.b | (uintptr_t)ptr.c |
+                                (uintptr_t)ptr.d | (uintptr_t)ptr.x) & 15) == 0);
+        if (pl->fused_impl == 2 && aligned)
+            e = tdma::launch_tma_fused(pl->tfused, ptr.a + off, ptr.b + off, ptr.c + off, ptr.d + off,
+                                       ptr.x + off, pl->nx, pl->ny, bzn, origin);
+        else if (pl->fused.threads > 0)
+            e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
+                                   ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
+        else
+            return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel needs 16-byte aligned arrays");
         if (e != cudaSuccess)
             return set_err(TDMA_ERR_CUDA, "fused launch failed: %s", cudaGetErrorString(e));
     }
@@ -365,10 +382,31 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         const char *why = nullptr;
         if ((size_t)pl->nx * (size_t)pl->m >= ((size_t)1 << 32))
             return set_err(TDMA_ERR_UNSUPPORTED, "fused variant: nx * ny/P exceeds 2^32 elements");
-        if (!tdma::configure_fused(&pl->fused, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
-                                   opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
-                                   opt ? opt->fused_top : 0, prop, &why))
+        const int want_impl = opt ? opt->fused_impl : 0;
+        if (want_impl < 0 || want_impl > 2)
+            return set_err(TDMA_ERR_INVALID_ARG, "unknown fused_impl %d", want_impl);
+        bool have_tma = false;
+        if (want_impl != 1) {
+            have_tma = tdma::get_encode_tiled() != nullptr &&
+                       tdma::configure_tma_fused(&pl->tfused, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
+                                                 opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
+                                                 prop, &why);
+            if (!have_tma && want_impl == 2)
+                return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel unavailable: %s",
+                               why ? why : "cuTensorMapEncodeTiled not found");
+        }
+        // the register-staged kernel is the fallback for unaligned pointers (explicit options
+        // are only forwarded to it when it was asked for)
+        const bool fwd = want_impl == 1 || !have_tma;
+        const bool have_reg = tdma::configure_fused(&pl->fused, pl->nx, pl->ny, pl->P,
+                                                    fwd && opt ? opt->fused_lines : 0,
+                                                    fwd && opt ? opt->fused_cluster : 0,
+                                                    fwd && opt ? opt->fused_leaf_rows : 0,
+                                                    opt ? opt->fused_top : 0, prop, &why);
+        if (!have_reg) pl->fused = tdma::FusedConfig();
+        if (!have_tma && !have_reg)
             return set_err(TDMA_ERR_UNSUPPORTED, "fused variant unavailable: %s", why ? why : "?");
+        pl->fused_impl = have_tma ? 2 : 1;
     }
     return TDMA_OK;
 }
@@ -507,14 +545,16 @@ int tdma_plan_get(const tdma_plan *plan, int what)
     case TDMA_GET_DEPTH: return plan->depth;
     case TDMA_GET_VARIANT: return plan->variant;
     case TDMA_GET_LAUNCHES: return launches_per_solve(plan);
-    case TDMA_GET_FUSED_LINES: return plan->fused.lines;
-    case TDMA_GET_FUSED_CLUSTER: return plan->fused.cluster;
+    case TDMA_GET_FUSED_IMPL: return plan->fused_impl;
+    case TDMA_GET_FUSED_LINES: return plan->fused_impl == 2 ? plan->tfused.lines : plan->fused.lines;
+    case TDMA_GET_FUSED_CLUSTER: return plan->fused_impl == 2 ? plan->tfused.cluster : plan->fused.cluster;
     case TDMA_GET_GRAPH_BUILDS: return plan->graph_builds;
-    case TDMA_GET_FUSED_LEAF_ROWS: return plan->fused.leaf_rows;
-    case TDMA_GET_FUSED_TOP: return plan->fused.top_mode;
-    case TDMA_GET_FUSED_THREADS: return plan->fused.threads;
-    case TDMA_GET_FUSED_SMEM: return (int)plan->fused.smem;
-    case TDMA_GET_FUSED_TOP_ROWS: return 2 * plan->fused.top_nodes * plan->fused.cluster;
+    case TDMA_GET_FUSED_LEAF_ROWS: return plan->fused_impl == 2 ? plan->tfused.leaf_rows : plan->fused.leaf_rows;
+    case TDMA_GET_FUSED_TOP: return plan->fused_impl == 2 ? 2 : plan->fused.top_mode;
+    case TDMA_GET_FUSED_THREADS: return plan->fused_impl == 2 ? plan->tfused.threads : plan->fused.threads;
+    case TDMA_GET_FUSED_SMEM: return (int)(plan->fused_impl == 2 ? plan->tfused.smem : plan->fused.smem);
+    case TDMA_GET_FUSED_TOP_ROWS:
+        return plan->fused_impl == 2 ? 2 * plan->tfused.cluster : 2 * plan->fused.top_nodes * plan->fused.cluster;
     default: return set_err(TDMA_ERR_INVALID_ARG, "unknown query %d", what);
     }
 }

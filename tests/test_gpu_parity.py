@@ -23,7 +23,13 @@ pytestmark = pytest.mark.gpu
 
 TOL_E = 1e-11
 TOL_RES = 1e-12
-VARIANTS = [tdma.TDMA_VARIANT_PIPELINED, tdma.TDMA_VARIANT_FUSED]
+# the three code paths behind tdma_solve: stage kernels + stream pipeline, the register-staged
+# fused kernel, and FUSED with fused_impl = auto (the TMA kernel wherever it is eligible)
+VARIANT_OPTS = [dict(variant=tdma.TDMA_VARIANT_PIPELINED),
+                dict(variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1),
+                dict(variant=tdma.TDMA_VARIANT_FUSED)]
+VARIANTS = [pytest.param(o, id=i) for o, i in zip(VARIANT_OPTS, ("pipelined", "fused_reg", "fused_tma"))]
+TMA = dict(variant=tdma.TDMA_VARIANT_FUSED, fused_impl=2)
 
 
 def dev():
@@ -65,7 +71,7 @@ def check_against_oracle(a, b, c, d, x, strictly_dominant, precision=None):
 @pytest.mark.parametrize("batch", [0, 1, 24])
 def test_cfg1_tiny_full(variant, batch):
     w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, variant=variant)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, **variant)
     check_against_oracle(w.a, w.b, w.c, w.d, x, True)
     xn = x.cpu().numpy()
     for i, k, ref in load_cfg1_golden():
@@ -75,7 +81,7 @@ def test_cfg1_tiny_full(variant, batch):
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_cfg2_poisson_full(variant):
     w = tdma_inputs.make_workload("cfg2_poisson", device=dev())
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, w.batch, variant=variant)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, w.batch, **variant)
     check_against_oracle(w.a, w.b, w.c, w.d, x, False)
 
 
@@ -83,7 +89,7 @@ def test_cfg2_poisson_full(variant):
 def test_cfg4_adi_y_slab(variant):
     """512 x 512 x 48 slices of cfg 4 (full nx, ny, P; ragged last batch 48 = 32 + 16)."""
     w = tdma_inputs.make_workload("cfg4_adi_y", device=dev(), nz=48)
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 32, variant=variant)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 32, **variant)
     check_against_oracle(w.a, w.b, w.c, w.d, x, True)
 
 
@@ -91,7 +97,7 @@ def test_cfg4_adi_y_slab(variant):
 def test_cfg5_stress_slab(variant):
     """2048 x 512 x 20 slices of cfg 5 (m = 8, 128-row reduced system), batch 8 -> 8+8+4."""
     w = tdma_inputs.make_workload("cfg5_stress", device=dev(), nz=20)
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=variant, nstreams=3)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, **variant, nstreams=3)
     check_against_oracle(w.a, w.b, w.c, w.d, x, True)
 
 
@@ -100,7 +106,7 @@ def test_cfg3_weak_slab(variant):
     """1024 x 1024 x 12 slices of cfg 3 starting at k = 0 (holds the pinned (0,0) mode and the
     lowest wavenumbers = the worst-conditioned lines), batch 8 -> 8 + 4."""
     w = tdma_inputs.make_workload("cfg3_weak", device=dev(), nz=12)
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=variant)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, **variant)
     check_against_oracle(w.a, w.b, w.c, w.d, x, False)
 
 
@@ -114,7 +120,7 @@ def _sampled_full(name, variant, batch, slices, strictly, **opts):
     if free < need:
         pytest.skip("needs %.0f GB of device memory" % (need / 1e9))
     w = tdma_inputs.make_workload(name, device=dev())
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, variant=variant, **opts)
+    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, **variant, **opts)
     assert bool(torch.isfinite(x).all())
     worst = 0.0
     for k in slices:
@@ -168,8 +174,8 @@ def test_schedule_invariance_fused_batches():
 ])
 def test_fused_cluster_shapes(cluster, lines, leaf, top):
     w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
-    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_cluster=cluster,
-                   fused_lines=lines, fused_leaf_rows=leaf, fused_top=top) as plan:
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1,
+                   fused_cluster=cluster, fused_lines=lines, fused_leaf_rows=leaf, fused_top=top) as plan:
         assert plan.get(tdma.TDMA_GET_FUSED_CLUSTER) == cluster
         assert plan.get(tdma.TDMA_GET_FUSED_LINES) == lines
         if leaf:
@@ -188,8 +194,8 @@ def test_fused_cluster_shapes(cluster, lines, leaf, top):
 def test_fused_cluster8_16(cluster, top):
     P = 16 if cluster == 16 else 8
     w = tdma_inputs.make_workload("cfg1_tiny", device=dev(), P=P)
-    x = gpu_solve(w.a, w.b, w.c, w.d, P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_cluster=cluster,
-                  fused_lines=32, fused_top=top)
+    x = gpu_solve(w.a, w.b, w.c, w.d, P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1,
+                  fused_cluster=cluster, fused_lines=32, fused_top=top)
     check_against_oracle(w.a, w.b, w.c, w.d, x, True)
 
 
@@ -197,8 +203,10 @@ def test_fused_top_modes_agree_with_pipelined_to_rounding():
     """The 2P-row reduced system is a Schur complement: however the recursion is cut, the result
     is the same up to rounding (cfg 2 slab, weakly dominant lines included)."""
     w = tdma_inputs.make_workload("cfg2_poisson", device=dev(), nz=6)
-    xs = [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_top=top,
-                    fused_leaf_rows=leaf) for top, leaf in ((1, 0), (2, 0), (1, 32), (2, 4))]
+    xs = [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1,
+                    fused_top=top, fused_leaf_rows=leaf) for top, leaf in ((1, 0), (2, 0), (1, 32), (2, 4))]
+    xs += [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, fused_leaf_rows=leaf, fused_cluster=cl, **TMA)
+           for leaf, cl in ((0, 0), (2, 1), (32, 2), (4, 8))]
     for x in xs:
         check_against_oracle(w.a, w.b, w.c, w.d, x, False)
 
@@ -255,9 +263,9 @@ def test_shapes(variant, shape, P, batch):
     nz, ny, nx = shape
     a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 11, dev())
     try:
-        x = gpu_solve(a, b, c, d, P, batch, variant=variant)
+        x = gpu_solve(a, b, c, d, P, batch, **variant)
     except tdma.TdmaError as exc:
-        if variant == tdma.TDMA_VARIANT_FUSED and "fused variant unavailable" in str(exc):
+        if variant["variant"] == tdma.TDMA_VARIANT_FUSED and "fused variant unavailable" in str(exc):
             pytest.skip(str(exc))
         raise
     check_against_oracle(a, b, c, d, x, True)
@@ -285,45 +293,107 @@ def test_odd_nx_fused(shape, P):
 
 def test_fused_rejects_what_it_cannot_tile():
     with pytest.raises(tdma.TdmaError) as ei:     # P = 1 keeps the whole line in one CTA
-        tdma.Plan(64, 4096, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED)
+        tdma.Plan(64, 4096, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1)
     assert "fused variant unavailable" in str(ei.value)
     with pytest.raises(tdma.TdmaError):
         tdma.Plan(64, 64, 2, 4, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_lines=64)
+    with pytest.raises(tdma.TdmaError) as ei:     # TMA needs 16-byte global strides
+        tdma.Plan(45, 64, 2, 4, 0, **TMA)
+    assert "even nx" in str(ei.value)
+    with pytest.raises(tdma.TdmaError):           # 48 = 3 * 16: no power-of-two tree
+        tdma.Plan(64, 96, 2, 2, 0, fused_leaf_rows=16, **TMA)
+
+
+# ---------------------------------------------------------------------------------------------
+# TMA fused kernel: tilings (lines x cluster x leaf), ragged x tiles, alignment fallback
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cluster,lines,leaf", [
+    (1, 16, 0), (1, 32, 2), (1, 8, 16), (1, 16, 4), (2, 16, 8), (2, 32, 4), (4, 16, 2), (4, 8, 16),
+    (8, 16, 8), (8, 32, 4), (8, 8, 2), (16, 16, 4), (16, 32, 2),
+])
+def test_tma_fused_tilings(cluster, lines, leaf):
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, fused_cluster=cluster, fused_lines=lines,
+                   fused_leaf_rows=leaf, **TMA) as plan:
+        assert plan.get(tdma.TDMA_GET_FUSED_IMPL) == 2
+        assert plan.get(tdma.TDMA_GET_FUSED_CLUSTER) == cluster
+        assert plan.get(tdma.TDMA_GET_FUSED_LINES) == lines
+        if leaf:
+            assert plan.get(tdma.TDMA_GET_FUSED_LEAF_ROWS) == leaf
+        assert plan.get(tdma.TDMA_GET_FUSED_TOP_ROWS) == 2 * cluster
+        x = torch.full_like(w.d, float("nan"))
+        plan.solve(w.a, w.b, w.c, w.d, x)
+        torch.cuda.synchronize()
+    check_against_oracle(w.a, w.b, w.c, w.d, x, True)
+
+
+@pytest.mark.parametrize("shape,P,cluster,lines", [
+    ((3, 64, 46), 4, 2, 16),      # ragged last x tile (46 = 2*16 + 14): TMA zero-fills / clips
+    ((2, 1024, 20), 16, 8, 16),   # cfg-3 line length, tile wider than the ragged remainder
+    ((2, 2048, 8), 32, 8, 8),     # two TMA boxes per array (R = 256 rows, box 256) -> R > 256 with CL = 4
+    ((2, 2048, 8), 32, 4, 8),
+    ((1, 2, 8), 1, 1, 8),         # ny = 2
+    ((3, 32, 8), 16, 2, 8),       # m = 2: partitions without interior rows
+])
+def test_tma_fused_shapes(shape, P, cluster, lines):
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 13, dev())
+    guard = torch.full((nz * ny * nx + 64,), float("nan"), dtype=torch.float64, device=dev())
+    x = guard[:nz * ny * nx].view(nz, ny, nx)
+    gpu_solve(a, b, c, d, P, 0, out=x, fused_cluster=cluster, fused_lines=lines, **TMA)
+    assert torch.isnan(guard[nz * ny * nx:]).all()
+    check_against_oracle(a, b, c, d, x, True)
+
+
+def test_tma_fused_unaligned_pointers_fall_back():
+    """Arrays that are only 8-byte aligned cannot be described by a tensor map: the plan routes
+    the solve to the register-staged kernel instead of failing."""
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    n = w.d.numel()
+    bufs = [torch.empty(n + 1, dtype=torch.float64, device=dev()) for _ in range(5)]
+    views = [b[1:].view_as(w.d) for b in bufs]
+    for v, t in zip(views, (w.a, w.b, w.c, w.d)):
+        v.copy_(t)
+    assert views[0].data_ptr() % 16 == 8
+    x = gpu_solve(views[0], views[1], views[2], views[3], w.P, 0, out=views[4], variant=tdma.TDMA_VARIANT_FUSED)
+    check_against_oracle(w.a, w.b, w.c, w.d, x, True)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_identity_and_diagonal(variant):
     for diag in (False, True):
         a, b, c, d = tdma_inputs.identity_system(32, 16, 3, 2, dev(), diagonal_only=diag)
-        x = gpu_solve(a, b, c, d, 4, 2, variant=variant)
-        assert torch.allclose(x, d / b, rtol=4e-16, atol=0)
+        x = gpu_solve(a, b, c, d, 4, 2, **variant)
+        # the kernels multiply by reciprocals (and the TMA kernel carries rows un-normalised):
+        # a few ulp, not a correctly rounded quotient
+        assert torch.allclose(x, d / b, rtol=1e-15, atol=0)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_corner_entries_are_ignored(variant):
     a, b, c, d = tdma_inputs.dominant_random(32, 24, 2, 3, dev())
-    x0 = gpu_solve(a, b, c, d, 4, 0, variant=variant)
+    x0 = gpu_solve(a, b, c, d, 4, 0, **variant)
     a2, c2 = a.clone(), c.clone()
     a2[:, 0, :] = float("nan")
     c2[:, -1, :] = float("inf")
-    x1 = gpu_solve(a2, b, c2, d, 4, 0, variant=variant)
+    x1 = gpu_solve(a2, b, c2, d, 4, 0, **variant)
     assert torch.equal(x0, x1)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_in_place_x_aliases_d(variant):
     w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
-    ref = gpu_solve(w.a, w.b, w.c, w.d, w.P, 16, variant=variant)
+    ref = gpu_solve(w.a, w.b, w.c, w.d, w.P, 16, **variant)
     buf = w.d.clone()
-    gpu_solve(w.a, w.b, w.c, buf, w.P, 16, out=buf, variant=variant)
+    gpu_solve(w.a, w.b, w.c, buf, w.P, 16, out=buf, **variant)
     assert torch.equal(buf, ref)
 
 
 def test_inputs_are_not_written():
     w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
     keep = [t.clone() for t in (w.a, w.b, w.c, w.d)]
-    for variant in VARIANTS:
-        gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=variant)
+    for variant in VARIANT_OPTS:
+        gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, **variant)
     for t, k in zip((w.a, w.b, w.c, w.d), keep):
         assert torch.equal(t, k)
 
@@ -335,8 +405,8 @@ def test_manufactured_solution_on_gpu():
     xstar = rng.uniform(-1, 1, (3, 128, 64))
     d = oracle.apply_y(a.numpy(), b.numpy(), c.numpy(), xstar)
     dd = torch.from_numpy(d).to(dev())
-    for variant in VARIANTS:
-        x = gpu_solve(a.to(dev()), b.to(dev()), c.to(dev()), dd, 8, 2, variant=variant)
+    for variant in VARIANT_OPTS:
+        x = gpu_solve(a.to(dev()), b.to(dev()), c.to(dev()), dd, 8, 2, **variant)
         assert oracle.normwise_error(x.cpu().numpy(), xstar).max() <= 1e-14
 
 
@@ -354,8 +424,8 @@ def test_toeplitz_closed_form_on_gpu():
         d[0, :, q - 1] = mode
         ref[0, :, q - 1] = mode / lam
     dd = torch.from_numpy(d).to(dev())
-    for variant in VARIANTS:
-        x = gpu_solve(a, b, a, dd, 8, 0, variant=variant)
+    for variant in VARIANT_OPTS:
+        x = gpu_solve(a, b, a, dd, 8, 0, **variant)
         assert oracle.normwise_error(x.cpu().numpy(), ref).max() <= (1 + 4 * alpha) * 2e-14
 
 
@@ -417,7 +487,7 @@ def test_solve_host_matches_device_solve(variant):
     w = tdma_inputs.make_workload("cfg2_poisson", device="cpu", nx=64, nz=40)
     host = [t.pin_memory() for t in (w.a, w.b, w.c, w.d)]
     xh = torch.empty_like(w.d).pin_memory()
-    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 4, variant=variant) as plan:
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 4, **variant) as plan:
         plan.solve_host(*host, xh)
         xd = torch.empty_like(w.d, device=dev())
         plan.solve(*[t.to(dev()) for t in host], xd)
