@@ -1,37 +1,31 @@
-// FUSED variant, TMA / pairwise-tree implementation (sm_100a).
+// FUSED variant, persistent TMA / pairwise-tree implementation (sm_100a).
 //
 // Same mapping of the paper's objects as tdma_fused.cuh (rank -> CTA of a thread-block cluster,
 // MPI_Alltoall -> distributed shared memory), but built around what bounds the
-// path on B200: bytes in flight and the TIME a tile occupies shared memory (resident bytes /
-// tile lifetime = bandwidth).  Measured on B200 the lifetime is set by dependent-instruction
-// latency (an fp64 reciprocal is a ~150-cycle chain), so the arithmetic is arranged to keep
-// divisions OFF every serial chain.
+// path on B200: bandwidth = bytes in flight / latency, and the bytes in flight live in shared
+// memory.  So shared memory holds (almost) nothing but RAW tiles that are in flight or being
+// swept, everything that has to survive the reduced-system phase is parked elsewhere:
 //
-//   * The raw a, b, c, d tile of a CTA ([R rows][TX lines] per array) is fetched by TMA tensor
-//     copies (cp.async.bulk.tensor.3d) issued by one thread and completed on an mbarrier: the
-//     whole tile is in flight at once, no register staging.
-//   * The tile is reduced IN PLACE and the solution leaves through TMA tensor stores.
-//     HBM traffic = 40 B/cell exactly (read a, b, c, d once, write x once).
-//   * Leaf = M0 rows of one line, one thread.  Elimination is carried UN-NORMALISED: every row
-//     is kept as  alpha x_0 + beta x_r + gamma x_{r+1} = delta  (x_0 = leaf's first unknown),
-//         beta_r  = beta_{r-1} b_r - a_r gamma_{r-1},   gamma_r = beta_{r-1} c_r,
-//         alpha_r = -a_r alpha_{r-1},                   delta_r = beta_{r-1} d_r - a_r delta_{r-1},
-//     a chain of ONE fma per row (the textbook c'_r = c_r / (b_r - a_r c'_{r-1}) has a reciprocal
-//     per row on the chain).  The per-row reciprocals 1/beta_r that back-substitution needs are
-//     independent of each other and pipeline.  A second, independent sweep from the bottom
-//     (eliminating the super-diagonal) produces the leaf's first-row equation
-//         A x_prev + B x_0 + C x_last = D ;   the down sweep ends in  A x_0 + B x_last + C x_next = D.
-//     Rows are rescaled by exact powers of two (exponent arithmetic, no rounding) so that the
-//     products stay in range.  In exact arithmetic this is the modified Thomas reduction of
-//     tdma_stage_kernels.cuh; only the rounding order differs.
+//   * Persistent clusters.  A cluster of CL CTAs owns TX consecutive lines (CTA c the rows
+//     c*R .. c*R+R-1, R = ny/CL) and loops over tiles (tile = x-tile, z-slice) with a static
+//     stride.  The raw a, b, c, d tile of a CTA ([R][TX] per array) is fetched by TMA tensor copies
+//     (cp.async.bulk.tensor.3d) completed on an mbarrier.  As soon as the leaf sweep of tile i has
+//     consumed the raw buffer, the copies of tile i+1 are issued into it, so HBM latency runs
+//     behind the tree / cluster phases of tile i instead of in front of them.
+//   * Leaf = M0 rows of one line, one thread: modified Thomas reduction (tdma_stage_kernels.cuh)
+//     from shared memory.  The forward-eliminated interior rows (a', c', d') stay in the thread's
+//     REGISTERS until back-substitution; only the two boundary equations of the leaf go to a small
+//     node buffer in shared memory.  x is streamed to HBM straight from registers (128-byte
+//     segments per half warp).  HBM traffic = 40 B/cell exactly.
 //   * The leaf boundary equations of a line are merged PAIRWISE (binary tree, log2 W levels, one
-//     thread per pair and line).  With
+//     thread per pair and line), carried un-normalised (general diagonal B) so that no division
+//     sits on the way up.  With
 //         L.first: A1 x_p  + B1 x_fL + C1 x_lL = D1      R.first: A3 x_lL + B3 x_fR + C3 x_lR = D3
 //         L.last : A2 x_fL + B2 x_lL + C2 x_fR = D2      R.last : A4 x_fR + B4 x_lR + C4 x_n  = D4
 //     and det = B2 B3 - C2 A3, nL = B3 D2 - C2 D3, nR = B2 D3 - A3 D2, the merged node is (times det)
 //         first: (det A1, det B1 - C1 B3 A2, C1 C2 C3 | det D1 - C1 nL)
 //         last : (A4 A3 A2, det B4 - A4 B2 C3, det C4 | det D4 - A4 nR)
-//     -- no division on the way up; the eliminated unknowns are kept as
+//     rescaled by an exact power of two; the eliminated unknowns are kept as
 //         x_lL = (nL - B3 A2 x_fL + C2 C3 x_lR) / det ,   x_fR = (nR + A3 A2 x_fL - B2 C3 x_lR) / det
 //     whose 1/det is computed after the merged node has been handed to the next level.
 //     With m0 | m = ny/P and m/m0 a power of two, the nodes of level log2(m/m0) are exactly the
@@ -40,13 +34,14 @@
 //   * The node left per (CTA, line) is ALL-GATHERED over the cluster with asynchronous DSMEM stores
 //     that complete on the receiver's mbarrier (st.async ... mbarrier::complete_tx): no cluster
 //     barrier on the critical path.  Every CTA solves the 2*CL-row system with the same pairwise
-//     tree (a node = 2 rows) and keeps its own two boundary values; then the tree is walked
-//     top-down and the leaves back-substitute from shared memory.
+//     tree and keeps its own two boundary values; then the tree is walked top-down and the leaves
+//     back-substitute from registers.  Inbox and mbarrier are double-buffered by tile parity: a
+//     CTA that runs ahead can only be one tile ahead (it needs everybody's tile-i data to finish
+//     tile i), so its tile-(i+1) stores never land in a buffer that is still being read.
 //
-// In-place storage: a node spanning tile rows [s, e] keeps its first equation in the (A, B, C, D)
-// slots of row s and its last equation in those of row e; a merge overwrites the (A, C, D) slots of
-// the two eliminated unknowns with (a, c, d) of  x = d - a x_first - c x_last ; interior leaf
-// rows hold (a', c', d') of  x_r = d' - a' x_0 - c' x_{r+1} ; back-substitution overwrites D with x.
+// Node buffer: rows 2w / 2w+1 hold the first / last equation (A, B, C, D) of leaf w; a merge
+// overwrites the (A, C, D) slots of the two eliminated unknowns with (a, c, d) of
+// x = d - a x_first - c x_last ; back-substitution overwrites D with x.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda.h>
@@ -67,23 +62,26 @@ struct TmaFusedConfig {
     int nlev = 0;       // log2 W
     int threads = 0;    // W * TX
     int box_rows = 0;   // rows per TMA box (<= 256), divides R
+    int max_clusters = 0;  // co-resident clusters (persistent grid size), filled at first launch
     size_t smem = 0;
 };
 
 struct TmaFusedParams {
+    double *x;          // batch base of the output
     int nx, ny, nzs;
-    int CL, R, W, nlev;
-    int xtiles;
+    int CL, R, W;
+    int xtiles, ntiles;
     int box_rows, nbox;
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
     long long *dbg;                     // experiment: per-CTA phase time stamps [grid][16]
 #endif
 };
 
-__host__ __device__ inline size_t tma_fused_smem_bytes(int TX, int R, int CL)
+__host__ __device__ inline size_t tma_fused_smem_bytes(int TX, int R, int W, int CL)
 {
-    // tile: 4 arrays [R][TX]; cluster-level system 4 x [2 CL][TX]; two mbarriers (+ padding)
-    return (size_t)4 * R * TX * sizeof(double) + (size_t)4 * 2 * CL * TX * sizeof(double) + 128;
+    // raw tile: 4 arrays [R][TX]; node buffer 4 x [2 W][TX]; cluster-level system, two inboxes of
+    // 4 x [2 CL][TX]; three mbarriers (+ padding)
+    return ((size_t)4 * R * TX + (size_t)4 * 2 * W * TX + (size_t)2 * 4 * 2 * CL * TX) * sizeof(double) + 128;
 }
 
 namespace ptx {
@@ -280,64 +278,52 @@ __device__ __forceinline__ void solve_root(const double *__restrict__ sA, const 
     sD[oF] = fma(Bl, Df, -(Cf * Dl)) * inv;
 }
 
-// Leaf reduction of M0 rows starting at tile offset o0 (row stride TX), in place.
+// Leaf: modified Thomas reduction of M0 rows (tile offset o0, row stride TX) read from the raw
+// tile.  Interior rows r = 1 .. M0-2 are returned in registers as (ia, ic, id)[r-1] of
+// x_r = id - ia x_0 - ic x_{r+1}; the two boundary equations (unit diagonal) go to `f` and `l`:
+//   f: A x_prev + x_0 + C x_last = D        l: A x_0 + x_last + C x_next = D
 template <int TX, int M0>
-__device__ __forceinline__ void leaf_reduce(double *__restrict__ sA, double *__restrict__ sB,
-                                            double *__restrict__ sC, double *__restrict__ sD,
-                                            int o0, bool first_leaf, bool last_leaf)
+__device__ __forceinline__ void leaf_reduce(const double *__restrict__ sA, const double *__restrict__ sB,
+                                            const double *__restrict__ sC, const double *__restrict__ sD,
+                                            int o0, bool first_leaf, bool last_leaf, Eq &f, Eq &l,
+                                            double (&ia)[M0 > 2 ? M0 - 2 : 1], double (&ic)[M0 > 2 ? M0 - 2 : 1],
+                                            double (&id)[M0 > 2 ? M0 - 2 : 1])
 {
-    // ---- up sweep (rows M0-2 .. 0, eliminating the super-diagonal): first-row equation
-    Eq u;
+    double inv = 1.0 / sB[o0];
+    double fa = first_leaf ? 0.0 : sA[o0] * inv;      // global a_0 := 0
+    double fc = sC[o0] * inv;
+    double fd = sD[o0] * inv;
+    double fb = 1.0;
+    double pa, pc, pd;
     {
-        const int o = o0 + (M0 - 2) * TX;
-        u.a = sA[o]; u.b = sB[o]; u.c = sC[o]; u.d = sD[o];
-    }
-#pragma unroll
-    for (int r = M0 - 3; r >= 0; --r) {
-        const int o = o0 + r * TX;
-        const double a = sA[o], b = sB[o], c = sC[o], d = sD[o];
-        Eq n;
-        n.a = u.b * a;
-        n.b = fma(u.b, b, -(c * u.a));
-        n.c = -(c * u.c);
-        n.d = fma(-c, u.d, u.b * d);
-        u = n;
-        if (((M0 - 3 - r) & 3) == 3 && r > 0) eq_rescale(u);
-    }
-    if (first_leaf) u.a = 0.0;          // global a_0 := 0
-    eq_rescale(u);
-
-    // ---- down sweep (rows 1 .. M0-1, eliminating the sub-diagonal, x_0 kept as a parameter)
-    Eq p;
-    {
-        const int o = o0 + TX;
-        p.a = sA[o]; p.b = sB[o]; p.c = sC[o]; p.d = sD[o];
+        double c1 = sC[o0 + TX];
+        if (M0 == 2 && last_leaf) c1 = 0.0;            // global c_{ny-1} := 0
+        inv = 1.0 / sB[o0 + TX];
+        pa = sA[o0 + TX] * inv; pc = c1 * inv; pd = sD[o0 + TX] * inv;
     }
 #pragma unroll
     for (int r = 2; r < M0; ++r) {
         const int o = o0 + r * TX;
-        const double a = sA[o], b = sB[o], c = sC[o], d = sD[o];
-        {   // row r-1 is interior: x_{r-1} = d' - a' x_0 - c' x_r
-            const double inv = 1.0 / p.b;
-            sA[o - TX] = p.a * inv; sC[o - TX] = p.c * inv; sD[o - TX] = p.d * inv;
-        }
-        Eq n;
-        n.b = fma(p.b, b, -(a * p.c));
-        n.c = p.b * c;
-        n.a = -(a * p.a);
-        n.d = fma(-a, p.d, p.b * d);
-        p = n;
-        if ((r & 3) == 1 && r < M0 - 1) eq_rescale(p);
+        const double ar = sA[o], br = sB[o], dr = sD[o];
+        double cr = sC[o];
+        if (r == M0 - 1 && last_leaf) cr = 0.0;
+        // fold row r-1 into the first-row equation, park it for back-substitution
+        fb = fma(-fc, pa, fb);
+        fd = fma(-fc, pd, fd);
+        fc = -fc * pc;
+        ia[r - 2] = pa; ic[r - 2] = pc; id[r - 2] = pd;
+        inv = 1.0 / fma(-ar, pc, br);
+        pd = fma(-ar, pd, dr) * inv;
+        pc = cr * inv;
+        pa = -(ar * pa) * inv;
     }
-    if (last_leaf) p.c = 0.0;           // global c_{ny-1} := 0
-    eq_rescale(p);
-    sA[o0] = u.a; sB[o0] = u.b; sC[o0] = u.c; sD[o0] = u.d;
-    const int oe = o0 + (M0 - 1) * TX;
-    sA[oe] = p.a; sB[oe] = p.b; sC[oe] = p.c; sD[oe] = p.d;
+    inv = 1.0 / fb;                                    // M0 == 2: fb = 1, frontier is x_1
+    f.a = fa * inv; f.b = 1.0; f.c = fc * inv; f.d = fd * inv;
+    l.a = pa; l.b = 1.0; l.c = pc; l.d = pd;
 }
 
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-#define TDMA_STAMP(i) do { if (threadIdx.x == 0) prm.dbg[(size_t)blockIdx.x * 16 + (i)] = clock64(); } while (0)
+#define TDMA_STAMP(i) do { if (threadIdx.x == 0 && it == 1) prm.dbg[(size_t)blockIdx.x * 16 + (i)] = clock64(); } while (0)
 #else
 #define TDMA_STAMP(i) do { } while (0)
 #endif
@@ -346,39 +332,36 @@ template <int TX, int M0, bool kCluster, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
                  const __grid_constant__ CUtensorMap tm_c, const __grid_constant__ CUtensorMap tm_d,
-                 const __grid_constant__ CUtensorMap tm_x, const TmaFusedParams prm)
+                 const TmaFusedParams prm)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const int R = prm.R, CL = prm.CL, W = prm.W;
     const int arr = R * TX;
-    double *__restrict__ sA = reinterpret_cast<double *>(smem_raw);
+    double *__restrict__ sA = reinterpret_cast<double *>(smem_raw);   // raw tile
     double *__restrict__ sB = sA + arr;
     double *__restrict__ sC = sB + arr;
     double *__restrict__ sD = sC + arr;
+    const int narr = 2 * W * TX;
+    double *__restrict__ nA = sD + arr;                               // node buffer
+    double *__restrict__ nB = nA + narr;
+    double *__restrict__ nC = nB + narr;
+    double *__restrict__ nD = nC + narr;
     const int NTR = 2 * CL;                                    // rows of the cluster-level system
     const int tarr = NTR * TX;
-    double *__restrict__ tA = sD + arr;                        // [NTR][TX] x 4: every CTA holds a copy
-    double *__restrict__ tB = tA + tarr;
-    double *__restrict__ tC = tB + tarr;
-    double *__restrict__ tD = tC + tarr;
-    uint64_t *bar = reinterpret_cast<uint64_t *>(tD + tarr);   // [0]: TMA tile, [1]: all-gather
+    double *__restrict__ top = nD + narr;                      // 2 inboxes x 4 x [NTR][TX]
+    uint64_t *bar = reinterpret_cast<uint64_t *>(top + 8 * tarr);   // [0]: raw tile, [1], [2]: inboxes
 
     const int t = threadIdx.x;
     unsigned crank = 0;
     if (kCluster) crank = cg::this_cluster().block_rank();
-    const int tile = blockIdx.x / CL;
-    const int xt = tile % prm.xtiles;
-    const int k = tile / prm.xtiles;
+    const int g = blockIdx.x / CL, NC = gridDim.x / CL;        // cluster index / number of clusters
     const int lx = t % TX, leaf = t / TX;
-    const int x0 = xt * TX;
     const int y0 = (int)crank * R;
+    const int o0 = leaf * M0 * TX + lx;
+    const bool first_leaf = (y0 + leaf * M0 == 0), last_leaf = (y0 + leaf * M0 + M0 == prm.ny);
 
-    TDMA_STAMP(0);
-    // ---------------- TMA: the whole raw tile in flight at once ----------------
-    if (t == 0) {
-        ptx::mbar_init(&bar[0], 1);
-        if (kCluster) ptx::mbar_init(&bar[1], 1);
-        ptx::fence_mbar_init();
+    auto issue_tile = [&](int tile) {   // thread 0: the whole raw tile of `tile` in flight at once
+        const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
         ptx::mbar_expect_tx(&bar[0], (unsigned)(4 * arr * sizeof(double)));
         for (int q = 0; q < prm.nbox; ++q) {
             const int yy = y0 + q * prm.box_rows;
@@ -388,110 +371,120 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             ptx::tma_load_3d(sC + so, &tm_c, x0, yy, k, &bar[0]);
             ptx::tma_load_3d(sD + so, &tm_d, x0, yy, k, &bar[0]);
         }
-        // the all-gather below delivers 4 doubles per (node equation, line) from every CTA
-        if (kCluster) ptx::mbar_expect_tx(&bar[1], (unsigned)(4 * tarr * sizeof(double)));
+    };
+
+    if (t == 0) {
+        ptx::mbar_init(&bar[0], 1);
+        ptx::mbar_init(&bar[1], 1);
+        ptx::mbar_init(&bar[2], 1);
+        ptx::fence_mbar_init();
+        issue_tile(g);
     }
     __syncthreads();                    // mbarriers initialised before anyone waits on them
     // split-phase cluster barrier: "every CTA of the cluster has started and initialised its
-    // all-gather mbarrier" must hold before the first remote store; the matching wait sits right
-    // before the exchange, where it is satisfied long ago
+    // inbox mbarriers" must hold before the first remote store; the matching wait sits right
+    // before the first exchange, where it is satisfied long ago
     if (kCluster) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-    ptx::mbar_wait(&bar[0], 0);
-    TDMA_STAMP(1);
 
-    // ---------------- leaves ----------------
-    const int o0 = leaf * M0 * TX + lx;
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 1
-    if (prm.nx > 0) goto store_x;       // experiment: data movement only
-#endif
-    {
-        const int grow0 = y0 + leaf * M0;
-        leaf_reduce<TX, M0>(sA, sB, sC, sD, o0, grow0 == 0, grow0 + M0 == prm.ny);
-    }
-    TDMA_STAMP(2);
+    int it = 0;
+    for (int tile = g; tile < prm.ntiles; tile += NC, ++it) {
+        const int par = it & 1;
+        double *__restrict__ tA = top + par * 4 * tarr;
+        double *__restrict__ tB = tA + tarr;
+        double *__restrict__ tC = tB + tarr;
+        double *__restrict__ tD = tC + tarr;
+        // arm this tile's inbox: 4 doubles per (node equation, line) from every CTA
+        if (kCluster && t == 0) ptx::mbar_expect_tx(&bar[1 + par], (unsigned)(4 * tarr * sizeof(double)));
+        TDMA_STAMP(0);
+        ptx::mbar_wait(&bar[0], (unsigned)par);
+        TDMA_STAMP(1);
 
-    // ---------------- pairwise tree inside the CTA, bottom-up ----------------
-    tree_up<TX>(sA, sB, sC, sD, lx, leaf, W, W, M0);
-    TDMA_STAMP(4);
-
-    // ---------------- cluster level ----------------
-    // the CTA's node: first equation in row 0, last equation in row R-1
-    if (!kCluster) {
-        if (t < TX) solve_root(sA, sB, sC, sD, lx, (R - 1) * TX + lx);
-        __syncthreads();
-    } else {
-        // A2B as an all-gather (the paper's MPI_Alltoall, with every rank keeping a
-        // copy): asynchronous DSMEM stores that complete on the RECEIVER's mbarrier -- no cluster
-        // barrier on the critical path, a CTA waits only for its own inbox
-        asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-        const uint32_t tA_s = ptx::smem_u32(tA), bar_s = ptx::smem_u32(&bar[1]);
-        const uint32_t plane = (uint32_t)tarr * 8u;
-        for (int e = t; e < 2 * TX * CL; e += (int)blockDim.x) {
-            const int dest = e / (2 * TX), r = e - dest * 2 * TX;
-            const int j = r / TX, l = r - j * TX;          // j: 0 = first eq, 1 = last eq
-            const int o = (j ? (R - 1) * TX : 0) + l;
-            const uint32_t row = (uint32_t)(((int)crank * 2 + j) * TX + l) * 8u;
-            const uint32_t dst = ptx::mapa(tA_s + row, (unsigned)dest), dbar = ptx::mapa(bar_s, (unsigned)dest);
-            ptx::st_async_f64(dst, sA[o], dbar);
-            ptx::st_async_f64(dst + plane, sB[o], dbar);
-            ptx::st_async_f64(dst + 2 * plane, sC[o], dbar);
-            ptx::st_async_f64(dst + 3 * plane, sD[o], dbar);
+        // ---------------- leaves ----------------
+        double ia[M0 > 2 ? M0 - 2 : 1], ic[M0 > 2 ? M0 - 2 : 1], id[M0 > 2 ? M0 - 2 : 1];
+        {
+            Eq f, l;
+            leaf_reduce<TX, M0>(sA, sB, sC, sD, o0, first_leaf, last_leaf, f, l, ia, ic, id);
+            const int of = 2 * leaf * TX + lx, ol = of + TX;
+            nA[of] = f.a; nB[of] = f.b; nC[of] = f.c; nD[of] = f.d;
+            nA[ol] = l.a; nB[ol] = l.b; nC[ol] = l.c; nD[ol] = l.d;
         }
-        TDMA_STAMP(5);
-        ptx::mbar_wait(&bar[1], 0);
+        __syncthreads();                // raw tile consumed, node equations visible
+        TDMA_STAMP(2);
+        if (t == 0 && tile + NC < prm.ntiles) issue_tile(tile + NC);   // prefetch behind the tree
+
+        // ---------------- pairwise tree inside the CTA, bottom-up ----------------
+        tree_up<TX>(nA, nB, nC, nD, lx, leaf, W, W, 2);
+        TDMA_STAMP(3);
+
+        // ---------------- cluster level ----------------
+        // the CTA's node: first equation in node row 0, last equation in node row 2W-1
+        if (!kCluster) {
+            if (t < TX) solve_root(nA, nB, nC, nD, lx, (2 * W - 1) * TX + lx);
+            __syncthreads();
+        } else {
+            // A2B as an all-gather (the paper's MPI_Alltoall, with every rank
+            // keeping a copy): asynchronous DSMEM stores that complete on the RECEIVER's mbarrier
+            if (it == 0) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+            const uint32_t tA_s = ptx::smem_u32(tA), bar_s = ptx::smem_u32(&bar[1 + par]);
+            const uint32_t plane = (uint32_t)tarr * 8u;
+            for (int e = t; e < 2 * TX * CL; e += (int)blockDim.x) {
+                const int dest = e / (2 * TX), r = e - dest * 2 * TX;
+                const int j = r / TX, l = r - j * TX;      // j: 0 = first eq, 1 = last eq
+                const int o = (j ? (2 * W - 1) * TX : 0) + l;
+                const uint32_t row = (uint32_t)(((int)crank * 2 + j) * TX + l) * 8u;
+                const uint32_t dst = ptx::mapa(tA_s + row, (unsigned)dest), dbar = ptx::mapa(bar_s, (unsigned)dest);
+                ptx::st_async_f64(dst, nA[o], dbar);
+                ptx::st_async_f64(dst + plane, nB[o], dbar);
+                ptx::st_async_f64(dst + 2 * plane, nC[o], dbar);
+                ptx::st_async_f64(dst + 3 * plane, nD[o], dbar);
+            }
+            TDMA_STAMP(4);
+            ptx::mbar_wait(&bar[1 + par], (unsigned)((it >> 1) & 1));
+            TDMA_STAMP(5);
+            // Stage B: the 2*CL-row system, solved redundantly by every CTA with the same
+            // pairwise tree, so no second exchange is needed
+            tree_up<TX>(tA, tB, tC, tD, lx, leaf, W, CL, 2);
+            if (t < TX) solve_root(tA, tB, tC, tD, lx, (NTR - 1) * TX + lx);
+            __syncthreads();
+            tree_down<TX>(tA, tC, tD, lx, leaf, W, CL, 2);
+            // B2C: my node's boundary values
+            for (int e = t; e < 2 * TX; e += (int)blockDim.x) {
+                const int j = e / TX, l = e - j * TX;
+                nD[(j ? (2 * W - 1) * TX : 0) + l] = tD[((int)crank * 2 + j) * TX + l];
+            }
+            __syncthreads();
+        }
         TDMA_STAMP(6);
-        // Stage B: the 2*CL-row system, solved redundantly by every CTA with the same pairwise
-        // tree (a node = 2 rows), so no second exchange is needed
-        tree_up<TX>(tA, tB, tC, tD, lx, leaf, W, CL, 2);
-        if (t < TX) solve_root(tA, tB, tC, tD, lx, (NTR - 1) * TX + lx);
-        __syncthreads();
-        tree_down<TX>(tA, tC, tD, lx, leaf, W, CL, 2);
-        // B2C: my node's boundary values
-        for (int e = t; e < 2 * TX; e += (int)blockDim.x) {
-            const int j = e / TX, l = e - j * TX;
-            sD[(j ? (R - 1) * TX : 0) + l] = tD[((int)crank * 2 + j) * TX + l];
-        }
-        __syncthreads();
-    }
-    TDMA_STAMP(7);
 
-    // ---------------- pairwise tree inside the CTA, top-down ----------------
-    tree_down<TX>(sA, sC, sD, lx, leaf, W, W, M0);
-    TDMA_STAMP(8);
+        // ---------------- pairwise tree inside the CTA, top-down ----------------
+        tree_down<TX>(nA, nC, nD, lx, leaf, W, W, 2);
+        TDMA_STAMP(7);
 
-    // ---------------- leaves: back-substitution, x overwrites d' ----------------
-    {
-        const double xf = sD[o0];
-        double xn = sD[o0 + (M0 - 1) * TX];
+        // ---------------- leaves: back-substitution from registers, x streamed to HBM --------
+        {
+            const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
+            const double xf = nD[2 * leaf * TX + lx];
+            double xn = nD[(2 * leaf + 1) * TX + lx];
+            if (x0 + lx < prm.nx) {     // ragged last x tile: TMA zero-filled those lanes
+                const size_t nx = (size_t)prm.nx;
+                double *__restrict__ xp = prm.x + ((size_t)k * prm.ny + (size_t)(y0 + leaf * M0)) * nx + (size_t)(x0 + lx);
+                __stcs(xp, xf);
+                __stcs(xp + (size_t)(M0 - 1) * nx, xn);
 #pragma unroll
-        for (int r = M0 - 2; r >= 1; --r) {
-            const int o = o0 + r * TX;
-            xn = fma(-sC[o], xn, fma(-sA[o], xf, sD[o]));
-            sD[o] = xn;
+                for (int r = M0 - 2; r >= 1; --r) {
+                    xn = fma(-ic[r - 1], xn, fma(-ia[r - 1], xf, id[r - 1]));
+                    __stcs(xp + (size_t)r * nx, xn);
+                }
+            }
         }
-    }
-    TDMA_STAMP(9);
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 1
-store_x:
-    if (kCluster) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-#endif
-    ptx::fence_proxy_async_smem();      // generic-proxy writes of D visible to the TMA engine
-    __syncthreads();
-    TDMA_STAMP(10);
-    if (t == 0) {
-        for (int q = 0; q < prm.nbox; ++q)
-            ptx::tma_store_3d(&tm_x, x0, y0 + q * prm.box_rows, k, sD + q * prm.box_rows * TX);
-        ptx::tma_store_commit_and_wait_read();   // smem must stay valid until the engine has read it
-    }
-    TDMA_STAMP(11);
+        TDMA_STAMP(8);
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-    if (t == 0) {
-        unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        long long gt; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt));
-        prm.dbg[(size_t)blockIdx.x * 16 + 12] = smid;
-        prm.dbg[(size_t)blockIdx.x * 16 + 13] = gt;
-    }
+        if (t == 0 && it == 1) {
+            unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+            prm.dbg[(size_t)blockIdx.x * 16 + 12] = smid;
+        }
 #endif
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -536,16 +529,18 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
                 c.box_rows = R;
                 while (c.box_rows > 256) c.box_rows /= 2;
                 if (R % c.box_rows) continue;
-                c.smem = tma_fused_smem_bytes(TX, R, CL);
+                c.smem = tma_fused_smem_bytes(TX, R, c.leaves, CL);
                 if (c.smem > max_smem) continue;
                 long ctas = (long)(sm_smem / (c.smem + 1024));
                 const long by_thr = 2048 / c.threads;
                 if (by_thr < ctas) ctas = by_thr;
                 if (ctas < 1) continue;
-                // resident cells per SM first; then >= 3 CTAs per SM (overlap of tile phases),
-                // 8-row leaves, 128 B row segments, small clusters
-                const double cells = (double)ctas * R * TX;
-                double score = cells + (c.threads >= 32 ? 4000.0 : 0.0) + (ctas >= 3 ? 2000.0 : 0.0) + (m0 == 8 ? 1000.0 : (m0 == 16 ? 500.0 : 0.0)) +
+                // persistent CTAs prefetch their next tile behind the tree phases: two or three
+                // CTAs per SM keep the raw buffers (= the bytes in flight) busy; then 8-row
+                // leaves (interior rows parked in 36 registers), 128 B row segments, small clusters
+                const double cells = (double)(ctas > 3 ? 3 : ctas) * R * TX;
+                double score = cells + (c.threads >= 32 ? 4000.0 : 0.0) + (ctas >= 2 ? 2000.0 : 0.0) +
+                               (m0 == 8 ? 1000.0 : (m0 == 4 ? 500.0 : 0.0)) +
                                (TX == 16 ? 300.0 : (TX == 32 ? 200.0 : 0.0)) - 10.0 * CL;
                 if (score > best_score) { best_score = score; best = c; }
             }
@@ -596,7 +591,7 @@ inline bool make_slab_tensor_map(CUtensorMap *tm, const void *base, int nx, int 
 }
 
 template <int TX, int M0, bool kCluster, int MAXT, int MINB>
-inline cudaError_t launch_tma_inst(const TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
+inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                    cudaStream_t st)
 {
     auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, MINB>;
@@ -604,14 +599,7 @@ inline cudaError_t launch_tma_inst(const TmaFusedConfig &cfg, const CUtensorMap 
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
     if (const char *pad = getenv("TDMA_PAD")) smem_bytes += (size_t)atoi(pad);   // experiment: fewer CTAs per SM
 #endif
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
-    if (e != cudaSuccess) return e;
-    if (cfg.cluster > 8) {
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        if (e != cudaSuccess) return e;
-    }
     cudaLaunchConfig_t lc = {};
-    lc.gridDim = dim3((unsigned)((size_t)prm.xtiles * prm.nzs * cfg.cluster));
     lc.blockDim = dim3(cfg.threads);
     lc.dynamicSmemBytes = smem_bytes;
     lc.stream = st;
@@ -620,20 +608,46 @@ inline cudaError_t launch_tma_inst(const TmaFusedConfig &cfg, const CUtensorMap 
     attr[0].val.clusterDim.x = cfg.cluster; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     lc.attrs = attr;
     lc.numAttrs = kCluster ? 1 : 0;
-    return cudaLaunchKernelEx(&lc, kern, tm[0], tm[1], tm[2], tm[3], tm[4], prm);
+    if (cfg.max_clusters <= 0) {        // first launch of this plan: attributes + persistent grid size
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return e;
+        if (cfg.cluster > 8) {
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (e != cudaSuccess) return e;
+        }
+        int dev = 0, sms = 0, n = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (kCluster) {
+            lc.gridDim = dim3((unsigned)(cfg.cluster * sms));
+            e = cudaOccupancyMaxActiveClusters(&n, kern, &lc);
+            if (e != cudaSuccess) return e;
+        } else {
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, cfg.threads, smem_bytes);
+            if (e != cudaSuccess) return e;
+            n *= sms;
+        }
+        if (n < 1) return cudaErrorLaunchOutOfResources;
+        cfg.max_clusters = n;
+    }
+    const int nc = prm.ntiles < cfg.max_clusters ? prm.ntiles : cfg.max_clusters;
+    lc.gridDim = dim3((unsigned)(nc * cfg.cluster));
+    return cudaLaunchKernelEx(&lc, kern, tm[0], tm[1], tm[2], tm[3], prm);
 }
 
 template <int TX, int M0, bool kCluster>
-inline cudaError_t launch_tma_m0(const TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
+inline cudaError_t launch_tma_m0(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                  cudaStream_t st)
 {
-    // shared memory allows about three tiles per SM: 256-thread CTAs may use up to 85 registers
-    if (cfg.threads <= 256) return launch_tma_inst<TX, M0, kCluster, 256, 3>(cfg, tm, prm, st);
+    // registers: the parked interior rows take 6 (M0 - 2) of them
+    if (M0 >= 16 && cfg.threads <= 256) return launch_tma_inst<TX, M0, kCluster, 256, 1>(cfg, tm, prm, st);
+    if (cfg.threads <= 256) return launch_tma_inst<TX, M0, kCluster, 256, 2>(cfg, tm, prm, st);
+    if (cfg.threads <= 512) return launch_tma_inst<TX, M0, kCluster, 512, 1>(cfg, tm, prm, st);
     return launch_tma_inst<TX, M0, kCluster, 1024, 1>(cfg, tm, prm, st);
 }
 
 template <int TX, bool kCluster>
-inline cudaError_t launch_tma_tx(const TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
+inline cudaError_t launch_tma_tx(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                  cudaStream_t st)
 {
     switch (cfg.leaf_rows) {
@@ -645,20 +659,22 @@ inline cudaError_t launch_tma_tx(const TmaFusedConfig &cfg, const CUtensorMap *t
     }
 }
 
-// a, b, c, d, x: batch base pointers (slice 0 of the launch), 16-byte aligned.
-inline cudaError_t launch_tma_fused(const TmaFusedConfig &cfg, const double *a, const double *b,
+// a, b, c, d: batch base pointers (slice 0 of the launch), 16-byte aligned; x: 8-byte aligned.
+inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const double *b,
                                     const double *c, const double *d, double *x, int nx, int ny,
                                     int nzs, cudaStream_t st)
 {
-    CUtensorMap tm[5];
-    const void *ptr[5] = {a, b, c, d, x};
-    for (int i = 0; i < 5; ++i)
+    CUtensorMap tm[4];
+    const void *ptr[4] = {a, b, c, d};
+    for (int i = 0; i < 4; ++i)
         if (!make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, cfg.lines, cfg.box_rows))
             return cudaErrorInvalidValue;
     TmaFusedParams prm;
     prm.nx = nx; prm.ny = ny; prm.nzs = nzs;
-    prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves; prm.nlev = cfg.nlev;
+    prm.x = x;
+    prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves;
     prm.xtiles = (nx + cfg.lines - 1) / cfg.lines;
+    prm.ntiles = prm.xtiles * nzs;
     prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
     {

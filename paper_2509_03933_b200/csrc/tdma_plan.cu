@@ -229,7 +229,7 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
         const size_t off = (size_t)k0 * pl->slice;
         cudaError_t e;
         const bool aligned = ((((uintptr_t)ptr.a | (uintptr_t)ptr.b | (uintptr_t)ptr.c |
-                                (uintptr_t)ptr.d | (uintptr_t)ptr.x) & 15) == 0);
+                                (uintptr_t)ptr.d) & 15) == 0);   // tensor maps of the inputs
         if (pl->fused_impl == 2 && aligned)
             e = tdma::launch_tma_fused(pl->tfused, ptr.a + off, ptr.b + off, ptr.c + off, ptr.d + off,
                                        ptr.x + off, pl->nx, pl->ny, bzn, origin);
