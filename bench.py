@@ -48,6 +48,19 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(alg_bytes_per_launch):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed `ncu --set full` capture (profiles/traffic.json, written from the .ncu-rep by hand;
+    a profiler cannot run inside the timed region).  The capture is of a shorter slab; traffic is
+    proportional to cells, so it is rescaled to this launch's algorithmic bytes.  None if absent."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            t = json.load(f)
+        return (t["dram_bytes_read"] + t["dram_bytes_write"]) / t["alg_bytes"] * alg_bytes_per_launch
+    except Exception:
+        return None
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
     QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
@@ -313,8 +326,16 @@ def main():
         alg_bytes = ALG_BYTES_PER_CELL * cells / launches
         dur = sec / launches
         achieved = alg_bytes / dur / 1e9
-        out["roofline"] = {"bound": "hbm", "kernel": "fused_kernel", "achieved": achieved, "peak": peak,
-                           "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+        impl = plan.get(tdma.TDMA_GET_FUSED_IMPL)
+        out["config"]["fused"] = {"impl": "tma" if impl == 2 else "reg",
+                                  "lines": plan.get(tdma.TDMA_GET_FUSED_LINES),
+                                  "cluster": plan.get(tdma.TDMA_GET_FUSED_CLUSTER),
+                                  "leaf_rows": plan.get(tdma.TDMA_GET_FUSED_LEAF_ROWS),
+                                  "threads": plan.get(tdma.TDMA_GET_FUSED_THREADS),
+                                  "smem": plan.get(tdma.TDMA_GET_FUSED_SMEM)}
+        out["roofline"] = {"bound": "hbm", "kernel": "fused_tma_kernel" if impl == 2 else "fused_kernel",
+                           "achieved": achieved, "peak": peak,
+                           "unit": "GB/s", "frac": achieved / peak, "traffic": ncu_traffic(alg_bytes),
                            "alg_bytes_per_launch": alg_bytes, "launch_ms": dur * 1e3, "peak_source": peak_src}
     else:
         st = stage_times(torch, tdma, plan, w, x) if not args.no_extras else None

@@ -535,13 +535,21 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
                 const long by_thr = 2048 / c.threads;
                 if (by_thr < ctas) ctas = by_thr;
                 if (ctas < 1) continue;
-                // persistent CTAs prefetch their next tile behind the tree phases: two or three
-                // CTAs per SM keep the raw buffers (= the bytes in flight) busy; then 8-row
-                // leaves (interior rows parked in 36 registers), 128 B row segments, small clusters
-                const double cells = (double)(ctas > 3 ? 3 : ctas) * R * TX;
-                double score = cells + (c.threads >= 32 ? 4000.0 : 0.0) + (ctas >= 2 ? 2000.0 : 0.0) +
-                               (m0 == 8 ? 1000.0 : (m0 == 4 ? 500.0 : 0.0)) +
-                               (TX == 16 ? 300.0 : (TX == 32 ? 200.0 : 0.0)) - 10.0 * CL;
+                // Measured on B200 (cfg 3 shapes): the tile period is set by the serial phases, so
+                // long leaves (fewer tree levels) win first; then two CTAs per SM (one sweeps while
+                // the other walks its tree), resident cells, small clusters, 64-128 B row segments.
+                // registers per thread of the instantiation (see launch_tma_m0)
+                const long regs = c.threads > 512 ? 64 : (c.threads > 256 || m0 < 16 ? 128 : 256);
+                const long by_regs = 65536 / (regs * c.threads);
+                if (by_regs < ctas) ctas = by_regs;
+                if (ctas < 1) continue;
+                double cells = (double)ctas * R * TX;
+                if (cells > 8192.0) cells = 8192.0;
+                // 128 B row segments: with 64 B segments the persistent clusters drift apart in a
+                // long run and DRAM row-buffer locality between neighbouring x tiles is lost
+                // (measured: 4.4 -> 3.1 TB/s from 256 to 1024 slices at TX = 8, flat at TX = 16)
+                double score = 10000.0 * m0 + cells + (c.threads >= 32 ? 4000.0 : 0.0) + (ctas >= 2 ? 100.0 : 0.0) -
+                               50.0 * CL + (TX == 16 ? 3000.0 : (TX == 32 ? 1000.0 : 0.0));
                 if (score > best_score) { best_score = score; best = c; }
             }
         }

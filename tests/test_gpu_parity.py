@@ -206,7 +206,7 @@ def test_fused_top_modes_agree_with_pipelined_to_rounding():
     xs = [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1,
                     fused_top=top, fused_leaf_rows=leaf) for top, leaf in ((1, 0), (2, 0), (1, 32), (2, 4))]
     xs += [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, fused_leaf_rows=leaf, fused_cluster=cl, **TMA)
-           for leaf, cl in ((0, 0), (2, 1), (32, 2), (4, 8))]
+           for leaf, cl in ((0, 0), (2, 1), (16, 2), (4, 8))]
     for x in xs:
         check_against_oracle(w.a, w.b, w.c, w.d, x, False)
 
