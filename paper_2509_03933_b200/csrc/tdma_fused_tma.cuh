@@ -39,9 +39,10 @@
 //     CTA that runs ahead can only be one tile ahead (it needs everybody's tile-i data to finish
 //     tile i), so its tile-(i+1) stores never land in a buffer that is still being read.
 //
-// Node buffer: rows 2w / 2w+1 hold the first / last equation (A, B, C, D) of leaf w; a merge
-// overwrites the (A, C, D) slots of the two eliminated unknowns with (a, c, d) of
-// x = d - a x_first - c x_last ; back-substitution overwrites D with x.
+// Node buffer: rows 2w / 2w+1 hold the first / last equation of leaf w as 16-byte pairs (A, B) and
+// (C, D); after the climb, one pass over all merges (one per thread, behind the exchange) turns the
+// rows a merge eliminated into (a, c | d) of  x = d - a x_first - c x_last ; back-substitution
+// overwrites D with x.  All node-buffer traffic uses explicit shared-space addresses.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda.h>
@@ -147,7 +148,40 @@ __device__ __forceinline__ void st_async_f64(uint32_t dst_cluster, double v, uin
                  ::"r"(dst_cluster), "l"(__double_as_longlong(v)), "r"(bar_cluster) : "memory");
 }
 
+// the same for a 16-byte pair
+__device__ __forceinline__ void st_async_2f64(uint32_t dst_cluster, double v0, double v1, uint32_t bar_cluster)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1, %2}, [%3];"
+                 ::"r"(dst_cluster), "l"(__double_as_longlong(v0)), "l"(__double_as_longlong(v1)), "r"(bar_cluster)
+                 : "memory");
+}
+
 }  // namespace ptx
+
+// ------------------------------------------------------------------------------------------
+// Shared-memory access by explicit 32-bit shared-space addresses (no generic-pointer arithmetic
+// on the serial path), 16 bytes at a time.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double2 lds2(uint32_t a)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds1(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts2(uint32_t a, double x, double y)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void sts1(uint32_t a, double x)
+{
+    asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(x) : "memory");
+}
 
 // 2^-e for |v| in [2^e, 2^(e+1)): multiplying an equation by it is exact and brings v into [1, 2)
 __device__ __forceinline__ double pow2_unscale(double v)
@@ -158,124 +192,115 @@ __device__ __forceinline__ double pow2_unscale(double v)
 
 struct Eq { double a, b, c, d; };
 
-__device__ __forceinline__ void eq_rescale(Eq &q)
-{
-    const double s = pow2_unscale(q.b);
-    q.a *= s; q.b *= s; q.c *= s; q.d *= s;
-}
+// Node buffer: `rows` equations x TX lines, stored as two planes of 16-byte pairs,
+//   AB[row][line] = (A, B)   and   CD[row][line] = (C, D),   CD plane `plane` bytes after AB.
+// An eliminated row keeps (a, c) in its AB slot and d (later x) in the D half of its CD slot.
+struct NodeBuf { uint32_t ab, plane; };
 
-// What a merge leaves for after the barrier: 1/det and the six numerators of the eliminated rows.
-struct MergeTail { double det, p1, p2, p3, p4, nL, nR; };
-
-// First half of a pairwise merge (see the header): rows o1 < o2 < o3 < o4 hold L.first, L.last,
-// R.first, R.last; o1 / o4 receive the merged node's equations.  Division-free.
-__device__ __forceinline__ MergeTail merge_head(double *__restrict__ sA, double *__restrict__ sB,
-                                                double *__restrict__ sC, double *__restrict__ sD,
-                                                int o1, int o2, int o3, int o4)
-{
-    const double A2 = sA[o2], B2 = sB[o2], C2 = sC[o2], D2 = sD[o2];
-    const double A3 = sA[o3], B3 = sB[o3], C3 = sC[o3], D3 = sD[o3];
-    const double A1 = sA[o1], B1 = sB[o1], C1 = sC[o1], D1 = sD[o1];
-    const double A4 = sA[o4], B4 = sB[o4], C4 = sC[o4], D4 = sD[o4];
-    MergeTail m;
-    m.det = fma(B2, B3, -(C2 * A3));
-    m.nL = fma(B3, D2, -(C2 * D3));
-    m.nR = fma(B2, D3, -(A3 * D2));
-    m.p1 = B3 * A2; m.p2 = C2 * C3; m.p3 = A3 * A2; m.p4 = B2 * C3;
-    Eq f, l;
-    f.a = m.det * A1; f.b = fma(m.det, B1, -(C1 * m.p1)); f.c = C1 * m.p2; f.d = fma(m.det, D1, -(C1 * m.nL));
-    l.a = A4 * m.p3; l.b = fma(m.det, B4, -(A4 * m.p4)); l.c = m.det * C4; l.d = fma(m.det, D4, -(A4 * m.nR));
-    eq_rescale(f); eq_rescale(l);
-    sA[o1] = f.a; sB[o1] = f.b; sC[o1] = f.c; sD[o1] = f.d;
-    sA[o4] = l.a; sB[o4] = l.b; sC[o4] = l.c; sD[o4] = l.d;
-    return m;
-}
-
-// Second half: the eliminated unknowns as  x = d - a x_first - c x_last  in rows o2, o3.
-__device__ __forceinline__ void merge_tail(double *__restrict__ sA, double *__restrict__ sC,
-                                           double *__restrict__ sD, int o2, int o3, const MergeTail &m)
-{
-    const double inv = 1.0 / m.det;
-    sA[o2] = m.p1 * inv; sC[o2] = -(m.p2 * inv); sD[o2] = m.nL * inv;
-    sA[o3] = -(m.p3 * inv); sC[o3] = m.p4 * inv; sD[o3] = m.nR * inv;
-}
-
-__device__ __forceinline__ void unmerge_pair(const double *__restrict__ sA, const double *__restrict__ sC,
-                                             double *__restrict__ sD, int o1, int o2, int o3, int o4)
-{
-    const double xf = sD[o1], xl = sD[o4];
-    sD[o2] = fma(-sC[o2], xl, fma(-sA[o2], xf, sD[o2]));
-    sD[o3] = fma(-sC[o3], xl, fma(-sA[o3], xf, sD[o3]));
-}
-
-// Pairwise tree over `nodes` nodes (a power of two) of `span` rows each, one line per lx, thread
-// rows `slot` of `nslots`.  Bottom-up: on return the single remaining node has its first equation
-// in row 0 and its last equation in row nodes*span-1.  Ends with a __syncthreads().
 template <int TX>
-__device__ __forceinline__ void tree_up(double *__restrict__ sA, double *__restrict__ sB,
-                                        double *__restrict__ sC, double *__restrict__ sD,
-                                        int lx, int slot, int nslots, int nodes, int span)
+__device__ __forceinline__ uint32_t nb_ab(const NodeBuf &nb, int row, int lx) { return nb.ab + (uint32_t)(row * TX + lx) * 16u; }
+
+// Pairwise merge, first half (see the header): rows r1 < r2 < r3 < r4 hold L.first, L.last,
+// R.first, R.last; r1 / r4 receive the merged node's equations.  Division-free.
+template <int TX>
+__device__ __forceinline__ void merge_head(const NodeBuf &nb, int lx, int r1, int r2, int r3, int r4)
 {
-    if (nodes / 2 <= nslots) {
-        // one pair per thread and level: the reciprocal of a level runs behind the next barrier
-        MergeTail carry;
-        int c2 = 0, c3 = 0;
-        bool have = false;
-        for (int n = nodes, sp = span; n > 1; n >>= 1, sp <<= 1) {
-            __syncthreads();
-            const bool act = slot < (n >> 1);
-            MergeTail cur;
-            int o2 = 0;
-            if (act) {
-                const int rs = slot * 2 * sp;
-                o2 = (rs + sp - 1) * TX + lx;
-                cur = merge_head(sA, sB, sC, sD, rs * TX + lx, o2, o2 + TX, (rs + 2 * sp - 1) * TX + lx);
-            }
-            if (have) merge_tail(sA, sC, sD, c2, c3, carry);
-            have = act;
-            if (act) { carry = cur; c2 = o2; c3 = o2 + TX; }
-        }
-        if (have) merge_tail(sA, sC, sD, c2, c3, carry);
-    } else {
-        for (int n = nodes, sp = span; n > 1; n >>= 1, sp <<= 1) {
-            __syncthreads();
-            for (int q = slot; q < (n >> 1); q += nslots) {
-                const int rs = q * 2 * sp;
-                const int o2 = (rs + sp - 1) * TX + lx;
-                const MergeTail m = merge_head(sA, sB, sC, sD, rs * TX + lx, o2, o2 + TX, (rs + 2 * sp - 1) * TX + lx);
-                merge_tail(sA, sC, sD, o2, o2 + TX, m);
-            }
+    const uint32_t o1 = nb_ab<TX>(nb, r1, lx), o2 = nb_ab<TX>(nb, r2, lx), o3 = nb_ab<TX>(nb, r3, lx), o4 = nb_ab<TX>(nb, r4, lx);
+    const double2 ab2 = lds2(o2), cd2 = lds2(o2 + nb.plane), ab3 = lds2(o3), cd3 = lds2(o3 + nb.plane);
+    const double2 ab1 = lds2(o1), cd1 = lds2(o1 + nb.plane), ab4 = lds2(o4), cd4 = lds2(o4 + nb.plane);
+    const double A2 = ab2.x, B2 = ab2.y, C2 = cd2.x, D2 = cd2.y, A3 = ab3.x, B3 = ab3.y, C3 = cd3.x, D3 = cd3.y;
+    const double A1 = ab1.x, B1 = ab1.y, C1 = cd1.x, D1 = cd1.y, A4 = ab4.x, B4 = ab4.y, C4 = cd4.x, D4 = cd4.y;
+    const double det = fma(B2, B3, -(C2 * A3));
+    const double nL = fma(B3, D2, -(C2 * D3)), nR = fma(B2, D3, -(A3 * D2));
+    const double p1 = B3 * A2, p2 = C2 * C3, p3 = A3 * A2, p4 = B2 * C3;
+    double fb = fma(det, B1, -(C1 * p1)), lb = fma(det, B4, -(A4 * p4));
+    const double sf = pow2_unscale(fb), sl = pow2_unscale(lb);
+    sts2(o1, det * A1 * sf, fb * sf);
+    sts2(o1 + nb.plane, C1 * p2 * sf, fma(det, D1, -(C1 * nL)) * sf);
+    sts2(o4, A4 * p3 * sl, lb * sl);
+    sts2(o4 + nb.plane, det * C4 * sl, fma(det, D4, -(A4 * nR)) * sl);
+}
+
+// Second half, recomputed from the two rows the merge eliminated (they are untouched until now):
+// x_lL = d - a x_first - c x_last in row r2, x_fR likewise in row r3.
+template <int TX>
+__device__ __forceinline__ void merge_tail(const NodeBuf &nb, int lx, int r2, int r3)
+{
+    const uint32_t o2 = nb_ab<TX>(nb, r2, lx), o3 = nb_ab<TX>(nb, r3, lx);
+    const double2 ab2 = lds2(o2), cd2 = lds2(o2 + nb.plane), ab3 = lds2(o3), cd3 = lds2(o3 + nb.plane);
+    const double A2 = ab2.x, B2 = ab2.y, C2 = cd2.x, D2 = cd2.y, A3 = ab3.x, B3 = ab3.y, C3 = cd3.x, D3 = cd3.y;
+    const double inv = 1.0 / fma(B2, B3, -(C2 * A3));
+    const double nL = fma(B3, D2, -(C2 * D3)), nR = fma(B2, D3, -(A3 * D2));
+    sts2(o2, (B3 * A2) * inv, -((C2 * C3) * inv));
+    sts1(o2 + nb.plane + 8, nL * inv);
+    sts2(o3, -((A3 * A2) * inv), (B2 * C3) * inv);
+    sts1(o3 + nb.plane + 8, nR * inv);
+}
+
+template <int TX>
+__device__ __forceinline__ void unmerge_pair(const NodeBuf &nb, int lx, int r1, int r2, int r3, int r4)
+{
+    const uint32_t o2 = nb_ab<TX>(nb, r2, lx), o3 = nb_ab<TX>(nb, r3, lx);
+    const double xf = lds1(nb_ab<TX>(nb, r1, lx) + nb.plane + 8), xl = lds1(nb_ab<TX>(nb, r4, lx) + nb.plane + 8);
+    const double2 ac2 = lds2(o2), ac3 = lds2(o3);
+    const double d2 = lds1(o2 + nb.plane + 8), d3 = lds1(o3 + nb.plane + 8);
+    sts1(o2 + nb.plane + 8, fma(-ac2.y, xl, fma(-ac2.x, xf, d2)));
+    sts1(o3 + nb.plane + 8, fma(-ac3.y, xl, fma(-ac3.x, xf, d3)));
+}
+
+// Pairwise tree over `nodes` nodes (a power of two) of 2 rows each, one line per lx, thread rows
+// `slot` of `nslots`.  Bottom-up, heads only: on return (after its closing __syncthreads) the root
+// has its first equation in row 0 and its last equation in row 2*nodes-1.
+template <int TX>
+__device__ __forceinline__ void tree_up(const NodeBuf &nb, int lx, int slot, int nslots, int nodes)
+{
+    for (int n = nodes, sp = 2; n > 1; n >>= 1, sp <<= 1) {
+        __syncthreads();
+        for (int q = slot; q < (n >> 1); q += nslots) {
+            const int rs = q * 2 * sp;
+            merge_head<TX>(nb, lx, rs, rs + sp - 1, rs + sp, rs + 2 * sp - 1);
         }
     }
     __syncthreads();
 }
 
-// Top-down: needs x_first / x_last of the root in D of row 0 / row nodes*span-1 (visible to all
-// threads); ends with a __syncthreads().
+// The tails of ALL merges of tree_up, one per thread row: merge j of the flat list (level 1 pairs,
+// then level 2 pairs, ...) goes to slot j.  No barrier inside; needs one before tree_down.
 template <int TX>
-__device__ __forceinline__ void tree_down(const double *__restrict__ sA, const double *__restrict__ sC,
-                                          double *__restrict__ sD, int lx, int slot, int nslots,
-                                          int nodes, int span)
+__device__ __forceinline__ void tree_tails(const NodeBuf &nb, int lx, int slot, int nslots, int nodes)
 {
-    for (int n = 2, sp = span * (nodes >> 1); n <= nodes; n <<= 1, sp >>= 1) {
+    for (int j = slot; j < nodes - 1; j += nslots) {
+        int base = 0, n = nodes, sp = 2;
+        while (j - base >= (n >> 1)) { base += n >> 1; n >>= 1; sp <<= 1; }
+        const int rs = (j - base) * 2 * sp;
+        merge_tail<TX>(nb, lx, rs + sp - 1, rs + sp);
+    }
+}
+
+// Top-down: needs x_first / x_last of the root in D of row 0 / row 2*nodes-1 and all tails
+// (visible to all threads); ends with a __syncthreads().
+template <int TX>
+__device__ __forceinline__ void tree_down(const NodeBuf &nb, int lx, int slot, int nslots, int nodes)
+{
+    for (int n = 2, sp = nodes; n <= nodes; n <<= 1, sp >>= 1) {
         for (int q = slot; q < (n >> 1); q += nslots) {
             const int rs = q * 2 * sp;
-            const int o2 = (rs + sp - 1) * TX + lx;
-            unmerge_pair(sA, sC, sD, rs * TX + lx, o2, o2 + TX, (rs + 2 * sp - 1) * TX + lx);
+            unmerge_pair<TX>(nb, lx, rs, rs + sp - 1, rs + sp, rs + 2 * sp - 1);
         }
         __syncthreads();
     }
 }
 
-// Root of a tree: first equation  B x_f + C x_l = D  (row oF, A = 0), last equation
-// A x_f + B x_l = D  (row oL, C = 0)  ->  x_f, x_l into D.
-__device__ __forceinline__ void solve_root(const double *__restrict__ sA, const double *__restrict__ sB,
-                                           const double *__restrict__ sC, double *__restrict__ sD, int oF, int oL)
+// Root of a tree: first equation  B x_f + C x_l = D  (row 0, A = 0), last equation
+// A x_f + B x_l = D  (row rl, C = 0)  ->  x_f, x_l into D.
+template <int TX>
+__device__ __forceinline__ void solve_root(const NodeBuf &nb, int lx, int rl)
 {
-    const double Bf = sB[oF], Cf = sC[oF], Df = sD[oF], Al = sA[oL], Bl = sB[oL], Dl = sD[oL];
-    const double inv = 1.0 / fma(Bf, Bl, -(Cf * Al));
-    sD[oL] = fma(Bf, Dl, -(Al * Df)) * inv;
-    sD[oF] = fma(Bl, Df, -(Cf * Dl)) * inv;
+    const uint32_t oF = nb_ab<TX>(nb, 0, lx), oL = nb_ab<TX>(nb, rl, lx);
+    const double2 abf = lds2(oF), cdf = lds2(oF + nb.plane), abl = lds2(oL), cdl = lds2(oL + nb.plane);
+    const double inv = 1.0 / fma(abf.y, abl.y, -(cdf.x * abl.x));
+    sts1(oL + nb.plane + 8, fma(abf.y, cdl.y, -(abl.x * cdf.y)) * inv);
+    sts1(oF + nb.plane + 8, fma(abl.y, cdf.y, -(cdf.x * cdl.y)) * inv);
 }
 
 // Leaf: modified Thomas reduction of M0 rows (tile offset o0, row stride TX) read from the raw
@@ -342,14 +367,13 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     double *__restrict__ sC = sB + arr;
     double *__restrict__ sD = sC + arr;
     const int narr = 2 * W * TX;
-    double *__restrict__ nA = sD + arr;                               // node buffer
-    double *__restrict__ nB = nA + narr;
-    double *__restrict__ nC = nB + narr;
-    double *__restrict__ nD = nC + narr;
+    double *node = sD + arr;                                          // node buffer, 4 x [2W][TX]
     const int NTR = 2 * CL;                                    // rows of the cluster-level system
     const int tarr = NTR * TX;
-    double *__restrict__ top = nD + narr;                      // 2 inboxes x 4 x [NTR][TX]
+    double *top = node + 4 * narr;                             // 2 inboxes x 4 x [NTR][TX]
     uint64_t *bar = reinterpret_cast<uint64_t *>(top + 8 * tarr);   // [0]: raw tile, [1], [2]: inboxes
+    NodeBuf nb;
+    nb.ab = ptx::smem_u32(node); nb.plane = (uint32_t)narr * 16u;
 
     const int t = threadIdx.x;
     unsigned crank = 0;
@@ -389,10 +413,8 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     int it = 0;
     for (int tile = g; tile < prm.ntiles; tile += NC, ++it) {
         const int par = it & 1;
-        double *__restrict__ tA = top + par * 4 * tarr;
-        double *__restrict__ tB = tA + tarr;
-        double *__restrict__ tC = tB + tarr;
-        double *__restrict__ tD = tC + tarr;
+        NodeBuf tb;                                            // this tile's inbox
+        tb.ab = ptx::smem_u32(top + par * 4 * tarr); tb.plane = (uint32_t)tarr * 16u;
         // arm this tile's inbox: 4 doubles per (node equation, line) from every CTA
         if (kCluster && t == 0) ptx::mbar_expect_tx(&bar[1 + par], (unsigned)(4 * tarr * sizeof(double)));
         TDMA_STAMP(0);
@@ -404,67 +426,70 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         {
             Eq f, l;
             leaf_reduce<TX, M0>(sA, sB, sC, sD, o0, first_leaf, last_leaf, f, l, ia, ic, id);
-            const int of = 2 * leaf * TX + lx, ol = of + TX;
-            nA[of] = f.a; nB[of] = f.b; nC[of] = f.c; nD[of] = f.d;
-            nA[ol] = l.a; nB[ol] = l.b; nC[ol] = l.c; nD[ol] = l.d;
+            const uint32_t of = nb_ab<TX>(nb, 2 * leaf, lx), ol = of + TX * 16u;
+            sts2(of, f.a, f.b); sts2(of + nb.plane, f.c, f.d);
+            sts2(ol, l.a, l.b); sts2(ol + nb.plane, l.c, l.d);
         }
         __syncthreads();                // raw tile consumed, node equations visible
         TDMA_STAMP(2);
         if (t == 0 && tile + NC < prm.ntiles) issue_tile(tile + NC);   // prefetch behind the tree
 
         // ---------------- pairwise tree inside the CTA, bottom-up ----------------
-        tree_up<TX>(nA, nB, nC, nD, lx, leaf, W, W, 2);
+        tree_up<TX>(nb, lx, leaf, W, W);
         TDMA_STAMP(3);
 
         // ---------------- cluster level ----------------
         // the CTA's node: first equation in node row 0, last equation in node row 2W-1
         if (!kCluster) {
-            if (t < TX) solve_root(nA, nB, nC, nD, lx, (2 * W - 1) * TX + lx);
+            if (t < TX) solve_root<TX>(nb, lx, 2 * W - 1);
+            tree_tails<TX>(nb, lx, leaf, W, W);
             __syncthreads();
         } else {
             // A2B as an all-gather (the paper's MPI_Alltoall, with every rank
             // keeping a copy): asynchronous DSMEM stores that complete on the RECEIVER's mbarrier
             if (it == 0) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-            const uint32_t tA_s = ptx::smem_u32(tA), bar_s = ptx::smem_u32(&bar[1 + par]);
-            const uint32_t plane = (uint32_t)tarr * 8u;
+            const uint32_t bar_s = ptx::smem_u32(&bar[1 + par]);
             for (int e = t; e < 2 * TX * CL; e += (int)blockDim.x) {
                 const int dest = e / (2 * TX), r = e - dest * 2 * TX;
                 const int j = r / TX, l = r - j * TX;      // j: 0 = first eq, 1 = last eq
-                const int o = (j ? (2 * W - 1) * TX : 0) + l;
-                const uint32_t row = (uint32_t)(((int)crank * 2 + j) * TX + l) * 8u;
-                const uint32_t dst = ptx::mapa(tA_s + row, (unsigned)dest), dbar = ptx::mapa(bar_s, (unsigned)dest);
-                ptx::st_async_f64(dst, nA[o], dbar);
-                ptx::st_async_f64(dst + plane, nB[o], dbar);
-                ptx::st_async_f64(dst + 2 * plane, nC[o], dbar);
-                ptx::st_async_f64(dst + 3 * plane, nD[o], dbar);
+                const uint32_t src = nb_ab<TX>(nb, j ? 2 * W - 1 : 0, l);
+                const double2 ab = lds2(src), cd = lds2(src + nb.plane);
+                const uint32_t dst = ptx::mapa(nb_ab<TX>(tb, (int)crank * 2 + j, l), (unsigned)dest);
+                const uint32_t dbar = ptx::mapa(bar_s, (unsigned)dest);
+                ptx::st_async_2f64(dst, ab.x, ab.y, dbar);
+                ptx::st_async_2f64(dst + tb.plane, cd.x, cd.y, dbar);
             }
             TDMA_STAMP(4);
+            // the reciprocals of the tree just climbed run behind the exchange
+            tree_tails<TX>(nb, lx, leaf, W, W);
             ptx::mbar_wait(&bar[1 + par], (unsigned)((it >> 1) & 1));
             TDMA_STAMP(5);
             // Stage B: the 2*CL-row system, solved redundantly by every CTA with the same
             // pairwise tree, so no second exchange is needed
-            tree_up<TX>(tA, tB, tC, tD, lx, leaf, W, CL, 2);
-            if (t < TX) solve_root(tA, tB, tC, tD, lx, (NTR - 1) * TX + lx);
+            tree_up<TX>(tb, lx, leaf, W, CL);
+            if (t < TX) solve_root<TX>(tb, lx, NTR - 1);
+            tree_tails<TX>(tb, lx, leaf, W, CL);
             __syncthreads();
-            tree_down<TX>(tA, tC, tD, lx, leaf, W, CL, 2);
+            tree_down<TX>(tb, lx, leaf, W, CL);
             // B2C: my node's boundary values
             for (int e = t; e < 2 * TX; e += (int)blockDim.x) {
                 const int j = e / TX, l = e - j * TX;
-                nD[(j ? (2 * W - 1) * TX : 0) + l] = tD[((int)crank * 2 + j) * TX + l];
+                sts1(nb_ab<TX>(nb, j ? 2 * W - 1 : 0, l) + nb.plane + 8,
+                     lds1(nb_ab<TX>(tb, (int)crank * 2 + j, l) + tb.plane + 8));
             }
             __syncthreads();
         }
         TDMA_STAMP(6);
 
         // ---------------- pairwise tree inside the CTA, top-down ----------------
-        tree_down<TX>(nA, nC, nD, lx, leaf, W, W, 2);
+        tree_down<TX>(nb, lx, leaf, W, W);
         TDMA_STAMP(7);
 
         // ---------------- leaves: back-substitution from registers, x streamed to HBM --------
         {
             const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
-            const double xf = nD[2 * leaf * TX + lx];
-            double xn = nD[(2 * leaf + 1) * TX + lx];
+            const double xf = lds1(nb_ab<TX>(nb, 2 * leaf, lx) + nb.plane + 8);
+            double xn = lds1(nb_ab<TX>(nb, 2 * leaf + 1, lx) + nb.plane + 8);
             if (x0 + lx < prm.nx) {     // ragged last x tile: TMA zero-filled those lanes
                 const size_t nx = (size_t)prm.nx;
                 double *__restrict__ xp = prm.x + ((size_t)k * prm.ny + (size_t)(y0 + leaf * M0)) * nx + (size_t)(x0 + lx);
