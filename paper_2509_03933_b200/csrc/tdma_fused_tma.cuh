@@ -190,6 +190,19 @@ __device__ __forceinline__ double pow2_unscale(double v)
     return __hiloint2double((2046 - e) << 20, 0);
 }
 
+// Branch-free reciprocal: hardware seed (MUFU.RCP64H, ~2^-20) + two Newton steps, within about
+// one ulp.  Unlike 1.0 / x it has no slow-path branch, so independent recurrences interleave in
+// one basic block.  Valid for normal, non-huge |x| (2^-1021 < |x| < 2^1021); x = 0 gives inf.
+__device__ __forceinline__ double rcp_nr(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+
 struct Eq { double a, b, c, d; };
 
 // Node buffer: `rows` equations x TX lines, stored as two planes of 16-byte pairs,
@@ -229,7 +242,7 @@ __device__ __forceinline__ void merge_tail(const NodeBuf &nb, int lx, int r2, in
     const uint32_t o2 = nb_ab<TX>(nb, r2, lx), o3 = nb_ab<TX>(nb, r3, lx);
     const double2 ab2 = lds2(o2), cd2 = lds2(o2 + nb.plane), ab3 = lds2(o3), cd3 = lds2(o3 + nb.plane);
     const double A2 = ab2.x, B2 = ab2.y, C2 = cd2.x, D2 = cd2.y, A3 = ab3.x, B3 = ab3.y, C3 = cd3.x, D3 = cd3.y;
-    const double inv = 1.0 / fma(B2, B3, -(C2 * A3));
+    const double inv = rcp_nr(fma(B2, B3, -(C2 * A3)));
     const double nL = fma(B3, D2, -(C2 * D3)), nR = fma(B2, D3, -(A3 * D2));
     sts2(o2, (B3 * A2) * inv, -((C2 * C3) * inv));
     sts1(o2 + nb.plane + 8, nL * inv);
@@ -298,53 +311,122 @@ __device__ __forceinline__ void solve_root(const NodeBuf &nb, int lx, int rl)
 {
     const uint32_t oF = nb_ab<TX>(nb, 0, lx), oL = nb_ab<TX>(nb, rl, lx);
     const double2 abf = lds2(oF), cdf = lds2(oF + nb.plane), abl = lds2(oL), cdl = lds2(oL + nb.plane);
-    const double inv = 1.0 / fma(abf.y, abl.y, -(cdf.x * abl.x));
+    const double inv = rcp_nr(fma(abf.y, abl.y, -(cdf.x * abl.x)));
     sts1(oL + nb.plane + 8, fma(abf.y, cdl.y, -(abl.x * cdf.y)) * inv);
     sts1(oF + nb.plane + 8, fma(abl.y, cdf.y, -(cdf.x * cdl.y)) * inv);
 }
 
-// Leaf: modified Thomas reduction of M0 rows (tile offset o0, row stride TX) read from the raw
-// tile.  Interior rows r = 1 .. M0-2 are returned in registers as (ia, ic, id)[r-1] of
-// x_r = id - ia x_0 - ic x_{r+1}; the two boundary equations (unit diagonal) go to `f` and `l`:
-//   f: A x_prev + x_0 + C x_last = D        l: A x_0 + x_last + C x_next = D
+// Leaf state of one thread: M0 rows of one line, swept as K = M0/H independent sub-leaves of H rows
+// (two interleaved recurrences when M0 >= 8) that are merged in registers.  What stays in
+// registers until back-substitution: the interior rows of every sub-leaf, (ia, ic, id) of
+// x_r = id - ia x_first - ic x_{r+1}, and for K = 2 the two unknowns the in-register merge
+// eliminated, (ma, mc, md)[j] of x = md - ma x_0 - mc x_{M0-1}  (j = 0: row H-1, j = 1: row H).
+template <int M0>
+struct LeafRegs {
+    static constexpr int K = M0 >= 8 ? 2 : 1;
+    static constexpr int H = M0 / K;
+    static constexpr int HI = H > 2 ? H - 2 : 1;
+    double ia[K][HI], ic[K][HI], id[K][HI];
+    double ma[2], mc[2], md[2];
+};
+
+// Modified Thomas reduction (tdma_stage_kernels.cuh) of the sub-leaves, read from the raw tile at
+// offset o0 (row stride TX).  Returns the leaf's two boundary equations
+//   f: A x_prev + B x_0 + C x_last = D        l: A x_0 + B x_last + C x_next = D
 template <int TX, int M0>
 __device__ __forceinline__ void leaf_reduce(const double *__restrict__ sA, const double *__restrict__ sB,
                                             const double *__restrict__ sC, const double *__restrict__ sD,
                                             int o0, bool first_leaf, bool last_leaf, Eq &f, Eq &l,
-                                            double (&ia)[M0 > 2 ? M0 - 2 : 1], double (&ic)[M0 > 2 ? M0 - 2 : 1],
-                                            double (&id)[M0 > 2 ? M0 - 2 : 1])
+                                            LeafRegs<M0> &R)
 {
-    double inv = 1.0 / sB[o0];
-    double fa = first_leaf ? 0.0 : sA[o0] * inv;      // global a_0 := 0
-    double fc = sC[o0] * inv;
-    double fd = sD[o0] * inv;
-    double fb = 1.0;
-    double pa, pc, pd;
-    {
-        double c1 = sC[o0 + TX];
-        if (M0 == 2 && last_leaf) c1 = 0.0;            // global c_{ny-1} := 0
-        inv = 1.0 / sB[o0 + TX];
-        pa = sA[o0 + TX] * inv; pc = c1 * inv; pd = sD[o0 + TX] * inv;
+    constexpr int K = LeafRegs<M0>::K, H = LeafRegs<M0>::H;
+    double fa[K], fb[K], fc[K], fd[K], pa[K], pc[K], pd[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const int o = o0 + h * H * TX;
+        double inv = rcp_nr(sB[o]);
+        fa[h] = (h == 0 && first_leaf) ? 0.0 : sA[o] * inv;      // global a_0 := 0
+        fc[h] = sC[o] * inv;
+        fd[h] = sD[o] * inv;
+        fb[h] = 1.0;
+        double c1 = sC[o + TX];
+        if (H == 2 && h == K - 1 && last_leaf) c1 = 0.0;         // global c_{ny-1} := 0
+        inv = rcp_nr(sB[o + TX]);
+        pa[h] = sA[o + TX] * inv; pc[h] = c1 * inv; pd[h] = sD[o + TX] * inv;
     }
 #pragma unroll
-    for (int r = 2; r < M0; ++r) {
-        const int o = o0 + r * TX;
-        const double ar = sA[o], br = sB[o], dr = sD[o];
-        double cr = sC[o];
-        if (r == M0 - 1 && last_leaf) cr = 0.0;
-        // fold row r-1 into the first-row equation, park it for back-substitution
-        fb = fma(-fc, pa, fb);
-        fd = fma(-fc, pd, fd);
-        fc = -fc * pc;
-        ia[r - 2] = pa; ic[r - 2] = pc; id[r - 2] = pd;
-        inv = 1.0 / fma(-ar, pc, br);
-        pd = fma(-ar, pd, dr) * inv;
-        pc = cr * inv;
-        pa = -(ar * pa) * inv;
+    for (int r = 2; r < H; ++r) {
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            const int o = o0 + (h * H + r) * TX;
+            const double ar = sA[o], br = sB[o], dr = sD[o];
+            double cr = sC[o];
+            if (r == H - 1 && h == K - 1 && last_leaf) cr = 0.0;
+            // fold row r-1 into the first-row equation, park it for back-substitution
+            fb[h] = fma(-fc[h], pa[h], fb[h]);
+            fd[h] = fma(-fc[h], pd[h], fd[h]);
+            fc[h] = -fc[h] * pc[h];
+            R.ia[h][r - 2] = pa[h]; R.ic[h][r - 2] = pc[h]; R.id[h][r - 2] = pd[h];
+            const double inv = rcp_nr(fma(-ar, pc[h], br));
+            pd[h] = fma(-ar, pd[h], dr) * inv;
+            pc[h] = cr * inv;
+            pa[h] = -(ar * pa[h]) * inv;
+        }
     }
-    inv = 1.0 / fb;                                    // M0 == 2: fb = 1, frontier is x_1
-    f.a = fa * inv; f.b = 1.0; f.c = fc * inv; f.d = fd * inv;
-    l.a = pa; l.b = 1.0; l.c = pc; l.d = pd;
+#pragma unroll
+    for (int h = 0; h < K; ++h) {                                // H == 2: fb = 1, frontier is x_1
+        const double inv = rcp_nr(fb[h]);
+        fa[h] *= inv; fc[h] *= inv; fd[h] *= inv;
+    }
+    if (K == 1) {
+        f.a = fa[0]; f.b = 1.0; f.c = fc[0]; f.d = fd[0];
+        l.a = pa[0]; l.b = 1.0; l.c = pc[0]; l.d = pd[0];
+    } else {
+        // pairwise merge of the two sub-leaves in registers (unit diagonals):
+        // (A1, C1, D1) = first / (A2, C2, D2) = last eq of sub-leaf 0, (A3..), (A4..) of sub-leaf 1
+        const double A1 = fa[0], C1 = fc[0], D1 = fd[0], A2 = pa[0], C2 = pc[0], D2 = pd[0];
+        const double A3 = fa[K - 1], C3 = fc[K - 1], D3 = fd[K - 1], A4 = pa[K - 1], C4 = pc[K - 1], D4 = pd[K - 1];
+        const double det = fma(-C2, A3, 1.0);
+        const double nL = fma(-C2, D3, D2), nR = fma(-A3, D2, D3);
+        const double p2 = C2 * C3, p3 = A3 * A2;
+        f.b = fma(-C1, A2, det); l.b = fma(-A4, C3, det);
+        const double sf = pow2_unscale(f.b), sl = pow2_unscale(l.b);
+        f.a = det * A1 * sf; f.b *= sf; f.c = C1 * p2 * sf; f.d = fma(det, D1, -(C1 * nL)) * sf;
+        l.a = A4 * p3 * sl; l.b *= sl; l.c = det * C4 * sl; l.d = fma(det, D4, -(A4 * nR)) * sl;
+        const double inv = rcp_nr(det);
+        R.ma[0] = A2 * inv; R.mc[0] = -(p2 * inv); R.md[0] = nL * inv;
+        R.ma[1] = -(p3 * inv); R.mc[1] = C3 * inv; R.md[1] = nR * inv;
+    }
+}
+
+// Back-substitution of the leaf from registers given its first and last unknown; x streamed to
+// HBM (row stride nx elements).
+template <int M0>
+__device__ __forceinline__ void leaf_back(const LeafRegs<M0> &R, double xf, double xl, double *__restrict__ xp,
+                                          size_t nx)
+{
+    constexpr int K = LeafRegs<M0>::K, H = LeafRegs<M0>::H;
+    double first[K], last[K];
+    first[0] = xf; last[K - 1] = xl;
+    if (K == 2) {
+        last[0] = fma(-R.mc[0], xl, fma(-R.ma[0], xf, R.md[0]));
+        first[K - 1] = fma(-R.mc[1], xl, fma(-R.ma[1], xf, R.md[1]));
+    }
+    double xn[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        xn[h] = last[h];
+        __stcs(xp + (size_t)(h * H) * nx, first[h]);
+        __stcs(xp + (size_t)(h * H + H - 1) * nx, last[h]);
+    }
+#pragma unroll
+    for (int r = H - 2; r >= 1; --r) {
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            xn[h] = fma(-R.ic[h][r - 1], xn[h], fma(-R.ia[h][r - 1], first[h], R.id[h][r - 1]));
+            __stcs(xp + (size_t)(h * H + r) * nx, xn[h]);
+        }
+    }
 }
 
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
@@ -422,10 +504,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         TDMA_STAMP(1);
 
         // ---------------- leaves ----------------
-        double ia[M0 > 2 ? M0 - 2 : 1], ic[M0 > 2 ? M0 - 2 : 1], id[M0 > 2 ? M0 - 2 : 1];
+        LeafRegs<M0> regs;
         {
             Eq f, l;
-            leaf_reduce<TX, M0>(sA, sB, sC, sD, o0, first_leaf, last_leaf, f, l, ia, ic, id);
+            leaf_reduce<TX, M0>(sA, sB, sC, sD, o0, first_leaf, last_leaf, f, l, regs);
             const uint32_t of = nb_ab<TX>(nb, 2 * leaf, lx), ol = of + TX * 16u;
             sts2(of, f.a, f.b); sts2(of + nb.plane, f.c, f.d);
             sts2(ol, l.a, l.b); sts2(ol + nb.plane, l.c, l.d);
@@ -489,17 +571,11 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         {
             const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
             const double xf = lds1(nb_ab<TX>(nb, 2 * leaf, lx) + nb.plane + 8);
-            double xn = lds1(nb_ab<TX>(nb, 2 * leaf + 1, lx) + nb.plane + 8);
+            const double xl = lds1(nb_ab<TX>(nb, 2 * leaf + 1, lx) + nb.plane + 8);
             if (x0 + lx < prm.nx) {     // ragged last x tile: TMA zero-filled those lanes
                 const size_t nx = (size_t)prm.nx;
-                double *__restrict__ xp = prm.x + ((size_t)k * prm.ny + (size_t)(y0 + leaf * M0)) * nx + (size_t)(x0 + lx);
-                __stcs(xp, xf);
-                __stcs(xp + (size_t)(M0 - 1) * nx, xn);
-#pragma unroll
-                for (int r = M0 - 2; r >= 1; --r) {
-                    xn = fma(-ic[r - 1], xn, fma(-ia[r - 1], xf, id[r - 1]));
-                    __stcs(xp + (size_t)r * nx, xn);
-                }
+                leaf_back<M0>(regs, xf, xl,
+                              prm.x + ((size_t)k * prm.ny + (size_t)(y0 + leaf * M0)) * nx + (size_t)(x0 + lx), nx);
             }
         }
         TDMA_STAMP(8);
