@@ -321,11 +321,16 @@ def main():
 
     # ---- roofline of the dominant kernel -----------------------------------------------------
     if best == "fused":
-        # one kernel per batch does the whole step; its launches fill the timed region back to back
-        launches = ok[best]["launches"]
-        alg_bytes = ALG_BYTES_PER_CELL * cells / launches
-        dur = sec / launches
+        # One persistent launch does the whole step.  When clusters of >= 4 CTAs leave SMs empty, a
+        # concurrent fill launch (clusters of 2) solves the last `fill` z-slices on them; the
+        # dominant kernel is the main launch, which spans the whole step (CUDA events around the
+        # step on the launching stream) and processes nz - fill slices.
+        fill = plan.get(tdma.TDMA_GET_FUSED_FILL)
+        nb_f = max(1, plan.get(tdma.TDMA_GET_NB))
+        alg_bytes = ALG_BYTES_PER_CELL * w.nx * w.ny * (w.nz - fill) / nb_f
+        dur = sec / nb_f
         achieved = alg_bytes / dur / 1e9
+        out["config"]["fill_slices"] = fill
         impl = plan.get(tdma.TDMA_GET_FUSED_IMPL)
         out["config"]["fused"] = {"impl": "tma" if impl == 2 else "reg",
                                   "lines": plan.get(tdma.TDMA_GET_FUSED_LINES),

@@ -89,7 +89,11 @@ typedef struct tdma_options {
                             any divisor leaf); 2 = TMA kernel (tile fetched by bulk tensor copies,
                             reduced in place, pairwise tree; needs even nx and power-of-two
                             leaf counts); 0 = auto (2 when eligible, else 1) */
-    int reserved[5];
+    int fused_fill;      /* FUSED, TMA kernel: clusters of 4 or more CTAs cannot be placed on every
+                            SM (a GPC holds 16-20 SMs); 0 = auto: a second, concurrent launch with
+                            clusters of 2 solves the last z-slices on the SMs the main launch
+                            leaves empty; N > 0: give it N/1000 of the slices; -1 = off */
+    int reserved[4];
 } tdma_options;
 
 /* Plan for an nx*ny*nz slab with y split into P partitions of ny/P rows and `batch` z-slices per
@@ -144,7 +148,8 @@ typedef enum tdma_query {
     TDMA_GET_FUSED_THREADS = 12,   /* threads per CTA                               */
     TDMA_GET_FUSED_SMEM = 13,      /* dynamic shared memory per CTA, bytes          */
     TDMA_GET_FUSED_TOP_ROWS = 14,  /* rows of the cluster-level system per line     */
-    TDMA_GET_FUSED_IMPL = 15       /* resolved fused_impl                           */
+    TDMA_GET_FUSED_IMPL = 15,      /* resolved fused_impl                           */
+    TDMA_GET_FUSED_FILL = 16       /* z-slices of the last solve given to the fill launch */
 } tdma_query;
 int tdma_plan_get(const tdma_plan *plan, int what); /* < 0 on error */
 size_t tdma_plan_workspace_bytes(const tdma_plan *plan); /* device bytes the plan owns */

@@ -739,6 +739,7 @@ inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, c
         if (n < 1) return cudaErrorLaunchOutOfResources;
         cfg.max_clusters = n;
     }
+    if (prm.ntiles <= 0) return cudaSuccess;    // prepare only (attributes + persistent grid size)
     const int nc = prm.ntiles < cfg.max_clusters ? prm.ntiles : cfg.max_clusters;
     lc.gridDim = dim3((unsigned)(nc * cfg.cluster));
     return cudaLaunchKernelEx(&lc, kern, tm[0], tm[1], tm[2], tm[3], prm);
@@ -775,7 +776,7 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
 {
     CUtensorMap tm[4];
     const void *ptr[4] = {a, b, c, d};
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 4 && nzs > 0; ++i)
         if (!make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, cfg.lines, cfg.box_rows))
             return cudaErrorInvalidValue;
     TmaFusedParams prm;

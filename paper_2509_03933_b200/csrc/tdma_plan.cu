@@ -84,6 +84,10 @@ struct tdma_plan {
     tdma::FusedConfig fused;
     int fused_impl = 0;  // 1 = register-staged general tree, 2 = TMA / pairwise tree
     tdma::TmaFusedConfig tfused;
+    tdma::TmaFusedConfig tfill;   // clusters of <= 2 CTAs for the SMs the main launch cannot use
+    bool have_fill = false;
+    int fill_opt = 0, fill_last = 0, sm_count = 0;
+    size_t sm_smem = 0;
     // host staging (tdma_solve_host), allocated on first use
     int hz = 0;  // slices per host chunk
     double *stage_dev[2][5] = {};
@@ -230,10 +234,47 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
         cudaError_t e;
         const bool aligned = ((((uintptr_t)ptr.a | (uintptr_t)ptr.b | (uintptr_t)ptr.c |
                                 (uintptr_t)ptr.d) & 15) == 0);   // tensor maps of the inputs
-        if (pl->fused_impl == 2 && aligned)
+        if (pl->fused_impl == 2 && aligned) {
+            // Fill launch: a cluster of >= 4 CTAs cannot be placed on every SM.  With one main CTA
+            // per SM the SMs left over take a second persistent launch with clusters of 2 that
+            // solves the last nzf slices concurrently (forked from / joined to `origin`).
+            int nzf = 0;
+            if (pl->have_fill) {
+                e = tdma::launch_tma_fused(pl->tfused, ptr.a, ptr.b, ptr.c, ptr.d, ptr.x, pl->nx, pl->ny, 0, origin);
+                if (e == cudaSuccess)
+                    e = tdma::launch_tma_fused(pl->tfill, ptr.a, ptr.b, ptr.c, ptr.d, ptr.x, pl->nx, pl->ny, 0, origin);
+                if (e != cudaSuccess)
+                    return set_err(TDMA_ERR_CUDA, "fused launch preparation failed: %s", cudaGetErrorString(e));
+                const long per_sm = (long)(pl->sm_smem / (pl->tfused.smem + 1024));
+                const int main_ctas = pl->tfused.max_clusters * pl->tfused.cluster;
+                const int idle = per_sm == 1 ? pl->sm_count - main_ctas : 0;
+                int fc = idle / pl->tfill.cluster;
+                if (fc > pl->tfill.max_clusters) fc = pl->tfill.max_clusters;
+                if (fc > 0) {
+                    // measured on cfg 3: an SM of the fill launch (64 B row segments, clusters far
+                    // apart in x) sustains about 0.55 of a main SM
+                    const double w = 0.55 * fc * pl->tfill.cluster;
+                    double share = pl->fill_opt > 0 ? pl->fill_opt * 1e-3 : w / (w + main_ctas);
+                    nzf = (int)(bzn * share + 0.5);
+                    if (nzf >= bzn) nzf = bzn - 1;
+                    if (nzf > 0) pl->tfill.max_clusters = fc;     // never more than the idle SMs
+                }
+            }
+            pl->fill_last = nzf;
+            if (nzf > 0) {
+                CUDA_TRY(cudaEventRecord(pl->evFork, origin));
+                CUDA_TRY(cudaStreamWaitEvent(pl->sB, pl->evFork, 0));
+            }
             e = tdma::launch_tma_fused(pl->tfused, ptr.a + off, ptr.b + off, ptr.c + off, ptr.d + off,
-                                       ptr.x + off, pl->nx, pl->ny, bzn, origin);
-        else if (pl->fused.threads > 0)
+                                       ptr.x + off, pl->nx, pl->ny, bzn - nzf, origin);
+            if (e == cudaSuccess && nzf > 0) {
+                const size_t offf = off + (size_t)(bzn - nzf) * pl->slice;
+                e = tdma::launch_tma_fused(pl->tfill, ptr.a + offf, ptr.b + offf, ptr.c + offf, ptr.d + offf,
+                                           ptr.x + offf, pl->nx, pl->ny, nzf, pl->sB);
+                CUDA_TRY(cudaEventRecord(pl->evBJoin, pl->sB));
+                CUDA_TRY(cudaStreamWaitEvent(origin, pl->evBJoin, 0));
+            }
+        } else if (pl->fused.threads > 0)
             e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
                                    ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
         else
@@ -253,7 +294,7 @@ int enqueue_schedule(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStrea
 int launches_per_solve(const tdma_plan *pl)
 {
     if (pl->ny == 1) return 1;
-    if (pl->variant == TDMA_VARIANT_FUSED) return pl->nb;
+    if (pl->variant == TDMA_VARIANT_FUSED) return pl->nb * (pl->fill_last > 0 ? 2 : 1);   // after a solve: main + fill launch
     return pl->nb * (3 + (pl->separate_gather ? 1 : 0));
 }
 
@@ -407,6 +448,14 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         if (!have_tma && !have_reg)
             return set_err(TDMA_ERR_UNSUPPORTED, "fused variant unavailable: %s", why ? why : "?");
         pl->fused_impl = have_tma ? 2 : 1;
+        pl->sm_count = prop.multiProcessorCount;
+        pl->sm_smem = prop.sharedMemPerMultiprocessor;
+        pl->fill_opt = opt ? opt->fused_fill : 0;
+        if (have_tma && pl->tfused.cluster >= 4 && pl->fill_opt >= 0) {
+            const char *why2 = nullptr;
+            pl->have_fill = tdma::configure_tma_fused(&pl->tfill, pl->nx, pl->ny, pl->P, 0,
+                                                      pl->ny % 2 == 0 ? 2 : 1, 0, prop, &why2);
+        }
     }
     return TDMA_OK;
 }
@@ -546,6 +595,7 @@ int tdma_plan_get(const tdma_plan *plan, int what)
     case TDMA_GET_VARIANT: return plan->variant;
     case TDMA_GET_LAUNCHES: return launches_per_solve(plan);
     case TDMA_GET_FUSED_IMPL: return plan->fused_impl;
+    case TDMA_GET_FUSED_FILL: return plan->fill_last;
     case TDMA_GET_FUSED_LINES: return plan->fused_impl == 2 ? plan->tfused.lines : plan->fused.lines;
     case TDMA_GET_FUSED_CLUSTER: return plan->fused_impl == 2 ? plan->tfused.cluster : plan->fused.cluster;
     case TDMA_GET_GRAPH_BUILDS: return plan->graph_builds;
