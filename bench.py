@@ -61,6 +61,43 @@ def ncu_traffic(alg_bytes_per_launch):
         return None
 
 
+class RankGroup:
+    """One process per GPU.  The path shards by lines with no exchange step, so every rank solves
+    its own slab of the same shape (weak scaling); torch.distributed is used for the barrier and
+    the max-over-ranks of the device time only.  backend None = single process."""
+
+    def __init__(self, backend, device=None):
+        self.dist = None
+        self.device = device
+        self.world = int(os.environ.get("WORLD_SIZE", "1")) if backend else 1
+        self.rank = int(os.environ.get("RANK", "0")) if backend else 0
+        if backend:
+            import torch.distributed as dist_mod
+            self.dist = dist_mod
+            kw = {"device_id": device} if backend == "nccl" else {}
+            dist_mod.init_process_group(backend, **kw)
+
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+
+    def max(self, v: float) -> float:
+        if self.dist is None:
+            return v
+        import torch
+        t = torch.tensor([v], dtype=torch.float64, device=self.device if self.device is not None else "cpu")
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def aggregate(self, cells_per_rank: int, max_seconds: float) -> float:
+        """Whole-job throughput: the cells all ranks processed / the slowest rank's time."""
+        return cells_per_rank * self.world / max_seconds
+
+    def close(self):
+        if self.dist is not None:
+            self.dist.destroy_process_group()
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks / throttle reasons every 200 ms while the timed region runs."""
     QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
@@ -239,22 +276,8 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist_mod
-        dist = dist_mod
-        dist.init_process_group("nccl", device_id=dev)
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-
-    def max_over_ranks(v: float) -> float:
-        if dist is None:
-            return v
-        t = torch.tensor([v], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    group = RankGroup("nccl" if world > 1 else None, dev)
+    barrier, max_over_ranks = group.barrier, group.max
 
     spec = tdma_inputs.config_spec(args.workload)
     nz = args.nz if args.nz > 0 else spec["nz"]
@@ -300,7 +323,7 @@ def main():
     sec = time_solve(torch, plan, w, x, args.steps, max(3, args.warmup), barrier)
     clocks = sampler.stop() if rank == 0 else None
     sec = max_over_ranks(sec)
-    value = cells * world / sec
+    value = group.aggregate(cells, sec)
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -391,8 +414,7 @@ def main():
             out["e2e_error"] = repr(exc)
     if rank == 0:
         print(json.dumps(out))
-    if dist is not None:
-        dist.destroy_process_group()
+    group.close()
     return 0
 
 
