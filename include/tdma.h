@@ -164,6 +164,25 @@ typedef enum tdma_buffer_id {
 } tdma_buffer_id;
 int tdma_plan_buffer(const tdma_plan *plan, int which, int slot, void **device_ptr, size_t *bytes);
 
+/* Batch-size optimiser of the paper (sections 4.2-4.2.3), PIPELINED variant.
+ *
+ * tdma_pipeline_model: the "simplified pipelining structure" (Fig. 6b) as a pure host
+ * function: makespan of Alg. 2's schedule (A(n) and C(n-2) on the A+C lanes, B(n-1) on its own
+ * stream, event dependencies A(n) -> B(n) -> C(n), ring of nstreams+1 scratch slots) for nb batches
+ * whose stages take tA, tB, tC when run alone and overlap perfectly across streams; the last batch
+ * is scaled by last_frac in (0, 1] (remainder batch).  nstreams as in tdma_options
+ * (1 = sequential Alg. 1 order).  Returns the time in the unit of tA/tB/tC, < 0 on bad arguments.
+ *
+ * tdma_plan_autotune: for every candidate batch size, times the three stages separately on the
+ * first few batches of the caller's slab (mean per batch, "each stage timed independently",
+ * PAPER.md:415), evaluates the model for all nz slices and returns the argmin in *best_batch and
+ * the estimates (ms) in est_ms[0..ncand).  a, b, c, d, x: DEVICE pointers as for tdma_solve; x is
+ * used as scratch.  Synchronises the device; not for use inside a timed region. */
+double tdma_pipeline_model(int nb, double tA, double tB, double tC, int nstreams, double last_frac);
+int tdma_plan_autotune(int nx, int ny, int nz, int P, int dtype, int nstreams, const int *candidates,
+                       int ncand, const void *a, const void *b, const void *c, const void *d, void *x,
+                       int *best_batch, double *est_ms);
+
 int tdma_plan_destroy(tdma_plan *plan);
 const char *tdma_last_error(void); /* thread-local, never NULL */
 int tdma_version(void);            /* 10000*major + 100*minor + patch */

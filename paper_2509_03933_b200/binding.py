@@ -29,7 +29,7 @@ TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
 EXPORTED_SYMBOLS = (
     "tdma_plan_create", "tdma_plan_create_ex", "tdma_solve", "tdma_solve_host", "tdma_stage",
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
-    "tdma_last_error", "tdma_version",
+    "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune",
 )
 
 
@@ -94,6 +94,11 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_last_error.restype = ctypes.c_char_p
     lib.tdma_version.argtypes = []
     lib.tdma_version.restype = ci
+    lib.tdma_pipeline_model.argtypes = [ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, ctypes.c_double]
+    lib.tdma_pipeline_model.restype = ctypes.c_double
+    lib.tdma_plan_autotune.argtypes = [ci] * 6 + [ctypes.POINTER(ci), ci] + [vp] * 5 + [
+        ctypes.POINTER(ci), ctypes.POINTER(ctypes.c_double)]
+    lib.tdma_plan_autotune.restype = ci
     _lib = lib
     return lib
 
@@ -185,6 +190,23 @@ def tdma_plan_buffer(plan: int, which: int, slot: int = 0):
     p, n = ctypes.c_void_p(), ctypes.c_size_t()
     _check(load_library().tdma_plan_buffer(plan, which, slot, ctypes.byref(p), ctypes.byref(n)))
     return int(p.value), int(n.value)
+
+
+def tdma_pipeline_model(nb: int, tA: float, tB: float, tC: float, nstreams: int = 2,
+                        last_frac: float = 1.0) -> float:
+    return float(load_library().tdma_pipeline_model(nb, tA, tB, tC, nstreams, last_frac))
+
+
+def tdma_plan_autotune(nx: int, ny: int, nz: int, P: int, candidates, a, b, c, d, x, nstreams: int = 2,
+                       dtype: int = TDMA_F64):
+    """(best batch size, [estimated ms per candidate])."""
+    n = len(candidates)
+    cand = (ctypes.c_int * n)(*candidates)
+    est = (ctypes.c_double * n)()
+    best = ctypes.c_int(0)
+    _check(load_library().tdma_plan_autotune(nx, ny, nz, P, dtype, nstreams, cand, n, _ptr(a), _ptr(b),
+                                             _ptr(c), _ptr(d), _ptr(x), ctypes.byref(best), est))
+    return int(best.value), [float(v) for v in est]
 
 
 def tdma_plan_destroy(plan: int) -> None:

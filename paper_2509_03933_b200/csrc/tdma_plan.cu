@@ -583,6 +583,96 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
     return TDMA_OK;
 }
 
+double tdma_pipeline_model(int nb, double tA, double tB, double tC, int nstreams, double last_frac)
+{
+    if (nb < 1 || nstreams < 1 || nstreams > kMaxLanes + 1 || !(last_frac > 0.0) || last_frac > 1.0 ||
+        tA < 0 || tB < 0 || tC < 0)
+        return -1.0;
+    auto dur = [&](double t, int n) { return n == nb - 1 ? t * last_frac : t; };
+    if (nstreams == 1) {
+        double T = 0;
+        for (int n = 0; n < nb; ++n) T += dur(tA, n) + dur(tB, n) + dur(tC, n);
+        return T;
+    }
+    // the event graph of enqueue_pipelined, stream clocks instead of launches
+    const int nl = nstreams - 1, depth = nl + 2;
+    std::vector<double> lane(nl, 0.0), evA(depth, 0.0), evB(depth, 0.0), evC(depth, 0.0);
+    double sB = 0.0;
+    for (int n = 0; n < nb + 2; ++n) {
+        if (n < nb) {
+            double &st = lane[n % nl];
+            if (n >= depth) st = std::max(st, evC[n % depth]);
+            st += dur(tA, n);
+            evA[n % depth] = st;
+        }
+        if (n - 1 >= 0 && n - 1 < nb) {
+            const int q = n - 1;
+            sB = std::max(sB, evA[q % depth]) + dur(tB, q);
+            evB[q % depth] = sB;
+        }
+        if (n - 2 >= 0 && n - 2 < nb) {
+            const int q = n - 2;
+            double &st = lane[q % nl];
+            st = std::max(st, evB[q % depth]) + dur(tC, q);
+            evC[q % depth] = st;
+        }
+    }
+    double T = sB;
+    for (double v : lane) T = std::max(T, v);
+    return T;
+}
+
+int tdma_plan_autotune(int nx, int ny, int nz, int P, int dtype, int nstreams, const int *candidates,
+                       int ncand, const void *a, const void *b, const void *c, const void *d, void *x,
+                       int *best_batch, double *est_ms)
+{
+    if (!candidates || ncand < 1 || !best_batch || !a || !b || !c || !d || !x)
+        return set_err(TDMA_ERR_INVALID_ARG, "NULL argument or no candidates");
+    if (nstreams == 0) nstreams = 2;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    double best = -1.0;
+    int rc = TDMA_OK;
+    for (int i = 0; i < ncand && rc == TDMA_OK; ++i) {
+        const int bz = candidates[i];
+        if (est_ms) est_ms[i] = -1.0;
+        if (bz < 1 || bz > nz) continue;
+        const int nzs = (int)std::min<long long>(nz, 4LL * bz);          // a few batches are enough
+        tdma_options opt;
+        memset(&opt, 0, sizeof(opt));
+        opt.struct_size = (int)sizeof(opt); opt.variant = TDMA_VARIANT_PIPELINED; opt.nstreams = nstreams;
+        tdma_plan *pl = tdma_plan_create_ex(nx, ny, nzs, P, bz, dtype, &opt);
+        if (!pl) { rc = TDMA_ERR_INVALID_ARG; break; }
+        const int nbs = nzs / bz > 0 ? nzs / bz : 1;                     // full batches only
+        double t[3] = {0, 0, 0};
+        const int stages[3] = {TDMA_STAGE_A, TDMA_STAGE_B, TDMA_STAGE_C};
+        for (int s = 0; s < 3 && rc == TDMA_OK; ++s) {
+            for (int pass = 0; pass < 3 && rc == TDMA_OK; ++pass) {      // pass 0 warms up
+                if (pass == 1) cudaEventRecord(e0, nullptr);
+                for (int n = 0; n < nbs && rc == TDMA_OK; ++n)
+                    rc = tdma_stage(pl, stages[s], n, a, b, c, d, x, nullptr);
+            }
+            cudaEventRecord(e1, nullptr);
+            if (cudaEventSynchronize(e1) != cudaSuccess) rc = set_err(TDMA_ERR_CUDA, "autotune timing failed");
+            float ms = 0;
+            cudaEventElapsedTime(&ms, e0, e1);
+            t[s] = ms / (2.0 * nbs);
+        }
+        tdma_plan_destroy(pl);
+        if (rc != TDMA_OK) break;
+        const int nb = (nz + bz - 1) / bz;
+        const double last = (double)(nz - (nb - 1) * bz) / bz;
+        const double est = tdma_pipeline_model(nb, t[0], t[1], t[2], nstreams, last);
+        if (est_ms) est_ms[i] = est;
+        if (best < 0 || est < best) { best = est; *best_batch = bz; }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (rc == TDMA_OK && best < 0) return set_err(TDMA_ERR_INVALID_ARG, "no valid candidate batch size");
+    return rc;
+}
+
 int tdma_plan_get(const tdma_plan *plan, int what)
 {
     if (!plan) return set_err(TDMA_ERR_INVALID_ARG, "plan is NULL");
