@@ -93,8 +93,18 @@ typedef struct tdma_options {
                             SM (a GPC holds 16-20 SMs); 0 = auto: a second, concurrent launch with
                             clusters of 2 solves the last z-slices on the SMs the main launch
                             leaves empty; N > 0: give it N/1000 of the slices; -1 = off */
-    int reserved[4];
+    int axis;            /* direction of the systems (BASELINE cfg 4): TDMA_AXIS_Y = 0
+                            (default; lines along y, y split into P partitions, `batch` counts
+                            z-slices) or TDMA_AXIS_Z = 2 (lines along z, stride nx*ny, z split into
+                            P partitions, `batch` counts y-slices).  x sweeps are not implemented */
+    int periodic;        /* 1 = cyclic lines: row 0 couples to row n-1 through a_0 and row n-1 to
+                            row 0 through c_{n-1} (both entries are then USED).  The cyclic
+                            coupling is resolved at the root of the recursion, so only the FUSED
+                            TMA kernel supports it */
+    int reserved[2];
 } tdma_options;
+
+enum { TDMA_AXIS_Y = 0, TDMA_AXIS_Z = 2 };
 
 /* Plan for an nx*ny*nz slab with y split into P partitions of ny/P rows and `batch` z-slices per
  * pipeline stage (batch_z of PAPER.md:236; 0 = all slices in one batch; a last smaller batch is

@@ -144,3 +144,45 @@ def normwise_error(x: np.ndarray, x_ref: np.ndarray) -> np.ndarray:
     num = np.max(np.abs(x - x_ref), axis=1)
     den = np.max(np.abs(x_ref), axis=1)
     return np.where(den > 0, num / np.where(den > 0, den, 1.0), num)
+
+
+# ---------------------------------------------------------------------------------------------
+# sweeps along z and cyclic (periodic) lines (BASELINE cfg 4)
+# ---------------------------------------------------------------------------------------------
+def solve_cyclic_y(a, b, c, d, precision: str = "f64") -> np.ndarray:
+    """Cyclic tridiagonal lines along y: row 0 couples to row n-1 through a_0 and row n-1 to row 0
+    through c_{n-1}.  Sherman-Morrison on top of the Thomas oracle, exactly as written in
+    SURVEY.md 8(f) f1:  gamma = -b_0;  b'_0 = b_0 - gamma;  b'_{n-1} = b_{n-1} - c_{n-1} a_0/gamma;
+    A' y = d;  A' q = u,  u = (gamma, 0, ..., 0, c_{n-1})^T;
+    x = y - q (y_0 + a_0 y_{n-1}/gamma) / (1 + q_0 + a_0 q_{n-1}/gamma).
+    Pinned in tests/test_oracle_pins.py against dense LAPACK solves of the full cyclic matrix and
+    the circulant closed form x = IFFT(FFT(d)/lambda)."""
+    a, b, c, d = map(_as3, (a, b, c, d))
+    n = a.shape[1]
+    if n < 3:
+        raise ValueError("cyclic lines need n >= 3")
+    a0, cn = a[:, 0, :], c[:, n - 1, :]
+    gamma = -b[:, 0, :]
+    bp = b.copy()
+    bp[:, 0, :] = b[:, 0, :] - gamma
+    bp[:, n - 1, :] = b[:, n - 1, :] - cn * a0 / gamma
+    u = np.zeros_like(d)
+    u[:, 0, :] = gamma
+    u[:, n - 1, :] = cn
+    y = solve_y(a, bp, c, d, precision).astype(np.longdouble)
+    q = solve_y(a, bp, c, u, precision).astype(np.longdouble)
+    g = gamma.astype(np.longdouble)
+    fac = (y[:, 0, :] + a0 * y[:, n - 1, :] / g) / (1.0 + q[:, 0, :] + a0 * q[:, n - 1, :] / g)
+    return np.asarray(y - q * fac[:, None, :], dtype=np.float64)
+
+
+def solve_axis(a, b, c, d, axis: str = "y", periodic: bool = False, precision: str = "f64") -> np.ndarray:
+    """Lines along y or z of (nz, ny, nx) arrays; a z sweep is the y sweep of the arrays with
+    their first two axes exchanged."""
+    if axis not in ("y", "z"):
+        raise ValueError(axis)
+    arrs = [_as3(t) for t in (a, b, c, d)]
+    if axis == "z":
+        arrs = [np.ascontiguousarray(t.transpose(1, 0, 2)) for t in arrs]
+    x = (solve_cyclic_y if periodic else solve_y)(*arrs, precision)
+    return np.ascontiguousarray(x.transpose(1, 0, 2)) if axis == "z" else x

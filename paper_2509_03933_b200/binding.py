@@ -19,6 +19,7 @@ from . import build as _build
 TDMA_F64 = 0
 TDMA_OK, TDMA_ERR_INVALID_ARG, TDMA_ERR_UNSUPPORTED, TDMA_ERR_ALLOC, TDMA_ERR_CUDA = 0, -1, -2, -3, -4
 TDMA_VARIANT_AUTO, TDMA_VARIANT_PIPELINED, TDMA_VARIANT_FUSED = 0, 1, 2
+TDMA_AXIS_Y, TDMA_AXIS_Z = 0, 2
 TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
 (TDMA_GET_NB, TDMA_GET_M, TDMA_GET_BATCH, TDMA_GET_NSTREAMS, TDMA_GET_DEPTH, TDMA_GET_VARIANT,
  TDMA_GET_LAUNCHES, TDMA_GET_FUSED_LINES, TDMA_GET_FUSED_CLUSTER, TDMA_GET_GRAPH_BUILDS,
@@ -39,7 +40,8 @@ class tdma_options(ctypes.Structure):
         ("use_graph", ctypes.c_int), ("separate_gather", ctypes.c_int),
         ("fused_lines", ctypes.c_int), ("fused_cluster", ctypes.c_int),
         ("fused_leaf_rows", ctypes.c_int), ("fused_top", ctypes.c_int),
-        ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("reserved", ctypes.c_int * 4),
+        ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("axis", ctypes.c_int), ("periodic", ctypes.c_int),
+        ("reserved", ctypes.c_int * 2),
     ]
 
 
@@ -147,13 +149,14 @@ def tdma_plan_create(nx: int, ny: int, nz: int, P: int, batch: int, dtype: int =
 def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: int = TDMA_F64, *,
                         variant: int = 0, nstreams: int = 0, use_graph: int = 0,
                         separate_gather: int = 0, fused_lines: int = 0, fused_cluster: int = 0,
-                        fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0) -> int:
+                        fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0,
+                        axis: int = 0, periodic: int = 0) -> int:
     opt = tdma_options()
     opt.struct_size = ctypes.sizeof(tdma_options)
     opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
     opt.separate_gather, opt.fused_lines, opt.fused_cluster = separate_gather, fused_lines, fused_cluster
     opt.fused_leaf_rows, opt.fused_top, opt.fused_impl = fused_leaf_rows, fused_top, fused_impl
-    opt.fused_fill = fused_fill
+    opt.fused_fill, opt.axis, opt.periodic = fused_fill, axis, periodic
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
         raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())

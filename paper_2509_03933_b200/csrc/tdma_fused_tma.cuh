@@ -69,7 +69,11 @@ struct TmaFusedConfig {
 
 struct TmaFusedParams {
     double *x;          // batch base of the output
-    int nx, ny, nzs;
+    long long rs, os;   // element stride between rows of a line / between slices of the caller's
+                        // arrays (y sweep: nx, nx*ny; z sweep: nx*ny, nx)
+    int axis_z;         // 0: rows = tensor dim 1, slices = dim 2;  1: rows = dim 2, slices = dim 1
+    int periodic;       // cyclic lines: x_{-1} = x_{n-1}, x_n = x_0 (a_0, c_{n-1} are used)
+    int nx, ny, nzs;    // ny = rows per line, nzs = slices in this launch
     int CL, R, W;
     int xtiles, ntiles;
     int box_rows, nbox;
@@ -304,16 +308,20 @@ __device__ __forceinline__ void tree_down(const NodeBuf &nb, int lx, int slot, i
     }
 }
 
-// Root of a tree: first equation  B x_f + C x_l = D  (row 0, A = 0), last equation
-// A x_f + B x_l = D  (row rl, C = 0)  ->  x_f, x_l into D.
+// Root of a tree: first equation  A x_prev + B x_f + C x_l = D  (row 0), last equation
+// A x_f + B x_l + C x_next = D  (row rl)  ->  x_f, x_l into D.  Plain lines: the root's A_first and
+// C_last are 0.  Cyclic lines (wrap): x_prev = x_l and x_next = x_f, i.e. the periodic coupling is
+// resolved here, at the top of the recursion, as  B_f x_f + (A_f + C_f) x_l = D_f ,
+// (A_l + C_l) x_f + B_l x_l = D_l  -- no Sherman-Morrison correction is needed.
 template <int TX>
-__device__ __forceinline__ void solve_root(const NodeBuf &nb, int lx, int rl)
+__device__ __forceinline__ void solve_root(const NodeBuf &nb, int lx, int rl, bool wrap)
 {
     const uint32_t oF = nb_ab<TX>(nb, 0, lx), oL = nb_ab<TX>(nb, rl, lx);
     const double2 abf = lds2(oF), cdf = lds2(oF + nb.plane), abl = lds2(oL), cdl = lds2(oL + nb.plane);
-    const double inv = rcp_nr(fma(abf.y, abl.y, -(cdf.x * abl.x)));
-    sts1(oL + nb.plane + 8, fma(abf.y, cdl.y, -(abl.x * cdf.y)) * inv);
-    sts1(oF + nb.plane + 8, fma(abl.y, cdf.y, -(cdf.x * cdl.y)) * inv);
+    const double Cf = wrap ? cdf.x + abf.x : cdf.x, Al = wrap ? abl.x + cdl.x : abl.x;
+    const double inv = rcp_nr(fma(abf.y, abl.y, -(Cf * Al)));
+    sts1(oL + nb.plane + 8, fma(abf.y, cdl.y, -(Al * cdf.y)) * inv);
+    sts1(oF + nb.plane + 8, fma(abl.y, cdf.y, -(Cf * cdl.y)) * inv);
 }
 
 // Leaf state of one thread: M0 rows of one line, swept as K = M0/H independent sub-leaves of H rows
@@ -464,7 +472,8 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     const int lx = t % TX, leaf = t / TX;
     const int y0 = (int)crank * R;
     const int o0 = leaf * M0 * TX + lx;
-    const bool first_leaf = (y0 + leaf * M0 == 0), last_leaf = (y0 + leaf * M0 + M0 == prm.ny);
+    const bool first_leaf = !prm.periodic && (y0 + leaf * M0 == 0);
+    const bool last_leaf = !prm.periodic && (y0 + leaf * M0 + M0 == prm.ny);
 
     auto issue_tile = [&](int tile) {   // thread 0: the whole raw tile of `tile` in flight at once
         const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
@@ -472,10 +481,11 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         for (int q = 0; q < prm.nbox; ++q) {
             const int yy = y0 + q * prm.box_rows;
             const int so = q * prm.box_rows * TX;
-            ptx::tma_load_3d(sB + so, &tm_b, x0, yy, k, &bar[0]);
-            ptx::tma_load_3d(sA + so, &tm_a, x0, yy, k, &bar[0]);
-            ptx::tma_load_3d(sC + so, &tm_c, x0, yy, k, &bar[0]);
-            ptx::tma_load_3d(sD + so, &tm_d, x0, yy, k, &bar[0]);
+            const int c1 = prm.axis_z ? k : yy, c2 = prm.axis_z ? yy : k;
+            ptx::tma_load_3d(sB + so, &tm_b, x0, c1, c2, &bar[0]);
+            ptx::tma_load_3d(sA + so, &tm_a, x0, c1, c2, &bar[0]);
+            ptx::tma_load_3d(sC + so, &tm_c, x0, c1, c2, &bar[0]);
+            ptx::tma_load_3d(sD + so, &tm_d, x0, c1, c2, &bar[0]);
         }
     };
 
@@ -523,7 +533,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         // ---------------- cluster level ----------------
         // the CTA's node: first equation in node row 0, last equation in node row 2W-1
         if (!kCluster) {
-            if (t < TX) solve_root<TX>(nb, lx, 2 * W - 1);
+            if (t < TX) solve_root<TX>(nb, lx, 2 * W - 1, prm.periodic != 0);
             tree_tails<TX>(nb, lx, leaf, W, W);
             __syncthreads();
         } else {
@@ -549,7 +559,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             // Stage B: the 2*CL-row system, solved redundantly by every CTA with the same
             // pairwise tree, so no second exchange is needed
             tree_up<TX>(tb, lx, leaf, W, CL);
-            if (t < TX) solve_root<TX>(tb, lx, NTR - 1);
+            if (t < TX) solve_root<TX>(tb, lx, NTR - 1, prm.periodic != 0);
             tree_tails<TX>(tb, lx, leaf, W, CL);
             __syncthreads();
             tree_down<TX>(tb, lx, leaf, W, CL);
@@ -573,9 +583,9 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             const double xf = lds1(nb_ab<TX>(nb, 2 * leaf, lx) + nb.plane + 8);
             const double xl = lds1(nb_ab<TX>(nb, 2 * leaf + 1, lx) + nb.plane + 8);
             if (x0 + lx < prm.nx) {     // ragged last x tile: TMA zero-filled those lanes
-                const size_t nx = (size_t)prm.nx;
                 leaf_back<M0>(regs, xf, xl,
-                              prm.x + ((size_t)k * prm.ny + (size_t)(y0 + leaf * M0)) * nx + (size_t)(x0 + lx), nx);
+                              prm.x + (size_t)k * (size_t)prm.os + (size_t)(y0 + leaf * M0) * (size_t)prm.rs +
+                                  (size_t)(x0 + lx), (size_t)prm.rs);
             }
         }
         TDMA_STAMP(8);
@@ -681,14 +691,17 @@ inline tdma_encode_tiled_fn get_encode_tiled()
     return fn;
 }
 
-// fp64 [nzs][ny][nx] slab, box = [1][box_rows][TX]
-inline bool make_slab_tensor_map(CUtensorMap *tm, const void *base, int nx, int ny, int nzs, int TX, int box_rows)
+// fp64 slab with x fastest; rows of a line rs elements apart, slices os elements apart.
+// y sweep: tensor (nx, rows, slices), box (TX, box_rows, 1); z sweep: tensor (nx, slices, rows),
+// box (TX, 1, box_rows) -- either way the box lands in shared memory as [box_rows][TX].
+inline bool make_slab_tensor_map(CUtensorMap *tm, const void *base, int nx, int nrows, int nslices,
+                                 long long rs, long long os, bool axis_z, int TX, int box_rows)
 {
     tdma_encode_tiled_fn enc = get_encode_tiled();
     if (!enc) return false;
-    cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nzs};
-    cuuint64_t gstr[2] = {(cuuint64_t)nx * sizeof(double), (cuuint64_t)nx * ny * sizeof(double)};
-    cuuint32_t box[3] = {(cuuint32_t)TX, (cuuint32_t)box_rows, 1};
+    cuuint64_t gdim[3] = {(cuuint64_t)nx, (cuuint64_t)(axis_z ? nslices : nrows), (cuuint64_t)(axis_z ? nrows : nslices)};
+    cuuint64_t gstr[2] = {(cuuint64_t)(axis_z ? os : rs) * sizeof(double), (cuuint64_t)(axis_z ? rs : os) * sizeof(double)};
+    cuuint32_t box[3] = {(cuuint32_t)TX, (cuuint32_t)(axis_z ? 1 : box_rows), (cuuint32_t)(axis_z ? box_rows : 1)};
     cuuint32_t estr[3] = {1, 1, 1};
     const size_t inner = (size_t)TX * sizeof(double);   // one L2 request per row segment, no over-fetch
     const CUtensorMapL2promotion promo = inner >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
@@ -772,16 +785,18 @@ inline cudaError_t launch_tma_tx(TmaFusedConfig &cfg, const CUtensorMap *tm, con
 // a, b, c, d: batch base pointers (slice 0 of the launch), 16-byte aligned; x: 8-byte aligned.
 inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const double *b,
                                     const double *c, const double *d, double *x, int nx, int ny,
-                                    int nzs, cudaStream_t st)
+                                    int nzs, long long rs, long long os, bool axis_z, bool periodic,
+                                    cudaStream_t st)
 {
     CUtensorMap tm[4];
     const void *ptr[4] = {a, b, c, d};
     for (int i = 0; i < 4 && nzs > 0; ++i)
-        if (!make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, cfg.lines, cfg.box_rows))
+        if (!make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows))
             return cudaErrorInvalidValue;
     TmaFusedParams prm;
     prm.nx = nx; prm.ny = ny; prm.nzs = nzs;
     prm.x = x;
+    prm.rs = rs; prm.os = os; prm.axis_z = axis_z ? 1 : 0; prm.periodic = periodic ? 1 : 0;
     prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves;
     prm.xtiles = (nx + cfg.lines - 1) / cfg.lines;
     prm.ntiles = prm.xtiles * nzs;

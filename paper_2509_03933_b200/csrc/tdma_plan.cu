@@ -67,7 +67,11 @@ struct tdma_plan {
     int variant = TDMA_VARIANT_PIPELINED, nstreams = 2, nlanes = 1, depth = 3;
     int use_graph = 1, separate_gather = 0;
     int device = 0;
-    size_t slice = 0;   // nx * ny
+    // Inside the plan ny is the line length (rows along the solve axis) and nz the number of slices
+    // (the other axis); for a z sweep they are the caller's nz and ny.
+    int axis = TDMA_AXIS_Y, periodic = 0;
+    long long rs = 0, os = 0;  // caller arrays: element stride between rows / between slices
+    size_t slice = 0;   // nx * ny: one slice of the plan's scratch
     size_t Lb_max = 0;  // nx * bz
     size_t workspace = 0;
     // PIPELINED buffers (ring of `depth` slots)
@@ -113,7 +117,7 @@ tdma::StageParams batch_params(const tdma_plan *pl, const SlabPtrs &ptr, int nz_
     const int k0 = n * pl->bz;
     const int bzn = std::min(pl->bz, nz_count - k0);
     const int slot = n % pl->depth;
-    const size_t off = (size_t)k0 * pl->slice;
+    const size_t off = (size_t)k0 * (size_t)pl->os;
     tdma::StageParams prm;
     prm.a = ptr.a + off; prm.b = ptr.b + off; prm.c = ptr.c + off; prm.d = ptr.d + off;
     prm.x = ptr.x + off;
@@ -124,6 +128,7 @@ tdma::StageParams batch_params(const tdma_plan *pl, const SlabPtrs &ptr, int nz_
     prm.send = pl->send ? pl->send + (size_t)slot * 6 * pl->P * pl->Lb_max : nullptr;
     prm.Lb = (long long)pl->nx * bzn;
     prm.nx = pl->nx; prm.ny = pl->ny; prm.m = pl->m; prm.P = pl->P;
+    prm.rs = pl->rs; prm.os = pl->os;
     return prm;
 }
 
@@ -230,7 +235,8 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
     for (int n = 0; n < nb; ++n) {
         const int k0 = n * pl->bz;
         const int bzn = std::min(pl->bz, nz_count - k0);
-        const size_t off = (size_t)k0 * pl->slice;
+        const size_t off = (size_t)k0 * (size_t)pl->os;
+        const bool az = pl->axis == TDMA_AXIS_Z, per = pl->periodic != 0;
         cudaError_t e;
         const bool aligned = ((((uintptr_t)ptr.a | (uintptr_t)ptr.b | (uintptr_t)ptr.c |
                                 (uintptr_t)ptr.d) & 15) == 0);   // tensor maps of the inputs
@@ -240,9 +246,9 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
             // solves the last nzf slices concurrently (forked from / joined to `origin`).
             int nzf = 0;
             if (pl->have_fill) {
-                e = tdma::launch_tma_fused(pl->tfused, ptr.a, ptr.b, ptr.c, ptr.d, ptr.x, pl->nx, pl->ny, 0, origin);
+                e = tdma::launch_tma_fused(pl->tfused, ptr.a, ptr.b, ptr.c, ptr.d, ptr.x, pl->nx, pl->ny, 0, pl->rs, pl->os, az, per, origin);
                 if (e == cudaSuccess)
-                    e = tdma::launch_tma_fused(pl->tfill, ptr.a, ptr.b, ptr.c, ptr.d, ptr.x, pl->nx, pl->ny, 0, origin);
+                    e = tdma::launch_tma_fused(pl->tfill, ptr.a, ptr.b, ptr.c, ptr.d, ptr.x, pl->nx, pl->ny, 0, pl->rs, pl->os, az, per, origin);
                 if (e != cudaSuccess)
                     return set_err(TDMA_ERR_CUDA, "fused launch preparation failed: %s", cudaGetErrorString(e));
                 const long per_sm = (long)(pl->sm_smem / (pl->tfused.smem + 1024));
@@ -266,19 +272,20 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
                 CUDA_TRY(cudaStreamWaitEvent(pl->sB, pl->evFork, 0));
             }
             e = tdma::launch_tma_fused(pl->tfused, ptr.a + off, ptr.b + off, ptr.c + off, ptr.d + off,
-                                       ptr.x + off, pl->nx, pl->ny, bzn - nzf, origin);
+                                       ptr.x + off, pl->nx, pl->ny, bzn - nzf, pl->rs, pl->os, az, per, origin);
             if (e == cudaSuccess && nzf > 0) {
-                const size_t offf = off + (size_t)(bzn - nzf) * pl->slice;
+                const size_t offf = off + (size_t)(bzn - nzf) * (size_t)pl->os;
                 e = tdma::launch_tma_fused(pl->tfill, ptr.a + offf, ptr.b + offf, ptr.c + offf, ptr.d + offf,
-                                           ptr.x + offf, pl->nx, pl->ny, nzf, pl->sB);
+                                           ptr.x + offf, pl->nx, pl->ny, nzf, pl->rs, pl->os, az, per, pl->sB);
                 CUDA_TRY(cudaEventRecord(pl->evBJoin, pl->sB));
                 CUDA_TRY(cudaStreamWaitEvent(origin, pl->evBJoin, 0));
             }
-        } else if (pl->fused.threads > 0)
+        } else if (pl->fused.threads > 0 && !az && !per)
             e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
                                    ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
         else
-            return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel needs 16-byte aligned arrays");
+            return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel needs 16-byte aligned arrays%s",
+                           az || per ? " (z sweeps and cyclic lines have no other kernel)" : "");
         if (e != cudaSuccess)
             return set_err(TDMA_ERR_CUDA, "fused launch failed: %s", cudaGetErrorString(e));
     }
@@ -382,6 +389,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
     if (variant == TDMA_VARIANT_AUTO) variant = TDMA_VARIANT_PIPELINED;
     if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED)
         return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
+    if (pl->periodic && (variant != TDMA_VARIANT_FUSED || pl->ny < 2))
+        return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need the FUSED variant (TMA kernel) and >= 2 rows");
     pl->variant = variant;
     pl->use_graph = (opt && opt->use_graph < 0) ? 0 : 1;
     pl->separate_gather = (opt && opt->separate_gather > 0) ? 1 : 0;
@@ -423,9 +432,14 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         const char *why = nullptr;
         if ((size_t)pl->nx * (size_t)pl->m >= ((size_t)1 << 32))
             return set_err(TDMA_ERR_UNSUPPORTED, "fused variant: nx * ny/P exceeds 2^32 elements");
-        const int want_impl = opt ? opt->fused_impl : 0;
+        int want_impl = opt ? opt->fused_impl : 0;
         if (want_impl < 0 || want_impl > 2)
             return set_err(TDMA_ERR_INVALID_ARG, "unknown fused_impl %d", want_impl);
+        if (pl->axis == TDMA_AXIS_Z || pl->periodic) {
+            if (want_impl == 1)
+                return set_err(TDMA_ERR_UNSUPPORTED, "the register-staged fused kernel does y sweeps of plain lines only");
+            want_impl = 2;
+        }
         bool have_tma = false;
         if (want_impl != 1) {
             have_tma = tdma::get_encode_tiled() != nullptr &&
@@ -476,6 +490,9 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
                                const tdma_options *options)
 {
     g_err[0] = 0;
+    const int axis = options ? options->axis : TDMA_AXIS_Y, periodic = options && options->periodic ? 1 : 0;
+    if (axis != TDMA_AXIS_Y && axis != TDMA_AXIS_Z) { set_err(TDMA_ERR_UNSUPPORTED, "axis %d: only TDMA_AXIS_Y (0) and TDMA_AXIS_Z (2) are implemented", axis); return nullptr; }
+    if (axis == TDMA_AXIS_Z) std::swap(ny, nz);   // from here on: ny = line length, nz = slices
     if (nx < 1 || ny < 1 || nz < 1) { set_err(TDMA_ERR_INVALID_ARG, "dimensions must be >= 1 (got %d x %d x %d)", nx, ny, nz); return nullptr; }
     if (P < 1) { set_err(TDMA_ERR_INVALID_ARG, "P must be >= 1 (got %d)", P); return nullptr; }
     if (ny % P != 0) { set_err(TDMA_ERR_INVALID_ARG, "ny = %d is not divisible by P = %d", ny, P); return nullptr; }
@@ -486,7 +503,10 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     if ((long long)nx * (batch ? batch : nz) > 0x7fffffffLL) { set_err(TDMA_ERR_UNSUPPORTED, "nx * batch exceeds 2^31-1 lines per batch"); return nullptr; }
     tdma_plan *pl = new (std::nothrow) tdma_plan();
     if (!pl) { set_err(TDMA_ERR_ALLOC, "out of host memory"); return nullptr; }
-    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->P = P; pl->m = ny / P;
+    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->P = P; pl->m = ny / P;   // ny, nz already mapped
+    pl->axis = axis; pl->periodic = periodic;
+    pl->rs = axis == TDMA_AXIS_Z ? (long long)nx * nz : (long long)nx;   // z sweep: plan nz = caller ny
+    pl->os = axis == TDMA_AXIS_Z ? (long long)nx : (long long)nx * ny;
     pl->bz = batch == 0 ? nz : batch;
     pl->nb = (nz + pl->bz - 1) / pl->bz;
     pl->slice = (size_t)nx * ny;
@@ -531,6 +551,8 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
     int rc = check_ptrs(plan, a, b, c, d, x);
     if (rc != TDMA_OK) return rc;
     tdma_plan *pl = plan;
+    if (pl->axis != TDMA_AXIS_Y)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_host streams z-chunks: y sweeps only");
     if (!pl->sH2D) {  // first use: staging buffers, copy streams
         // chunk = whole batches, about 64 Mi cells (512 MiB per array) or the slab if smaller
         const size_t target = (size_t)1 << 26;

@@ -40,7 +40,10 @@ struct StageParams {
     double *ra, *rc, *rd, *cp, *y;  // reduced system [2P][Lb], line fastest
     double *send;                 // separate gather: send_A buffer [P][6][Lb]
     long long Lb;                 // lines in this batch = nx * slices
-    int nx, ny, m, P;
+    int nx, ny, m, P;             // ny = rows per line (the solve axis), slices = the other axis
+    long long rs, os;             // caller arrays: element stride between rows of a line / between
+                                  // slices (y sweep: nx, nx*ny; z sweep: nx*ny, nx); scratch is
+                                  // always [slice][row][x]
 };
 
 // ------------------------------------------------------------------------------------------
@@ -55,15 +58,16 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
     const int nx = prm.nx, m = prm.m;
     const long long kk = l / nx;
     const int i = (int)(l - kk * nx);
-    const size_t off0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
+    const size_t off0 = (size_t)kk * (size_t)prm.os + i + (size_t)p * m * (size_t)prm.rs;
+    const size_t soff0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
     const double *__restrict__ a = prm.a + off0;
     const double *__restrict__ b = prm.b + off0;
     const double *__restrict__ c = prm.c + off0;
     const double *__restrict__ d = prm.d + off0;
-    double *__restrict__ sa = prm.sa + off0;
-    double *__restrict__ sc = prm.sc + off0;
-    double *__restrict__ sd = prm.sd + off0;
-    const size_t s = (size_t)nx;
+    double *__restrict__ sa = prm.sa + soff0;
+    double *__restrict__ sc = prm.sc + soff0;
+    double *__restrict__ sd = prm.sd + soff0;
+    const size_t s = (size_t)prm.rs, ss = (size_t)nx;
     const bool first_part = (p == 0), last_part = (p == prm.P - 1);
 
     // first-row equation  fa x_{-1} + fb x_0 + fc x_frontier = fd
@@ -112,9 +116,9 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
                 fb = fma(-fc, pa, fb);
                 fd = fma(-fc, pd, fd);
                 fc = -fc * pc;
-                st_keep(sa + (r - 1) * s, pa);
-                st_keep(sc + (r - 1) * s, pc);
-                st_keep(sd + (r - 1) * s, pd);
+                st_keep(sa + (r - 1) * ss, pa);
+                st_keep(sc + (r - 1) * ss, pc);
+                st_keep(sd + (r - 1) * ss, pd);
                 const double ar = ca[u];
                 const double cr = (last_part && r == m - 1) ? 0.0 : cc[u];
                 inv = 1.0 / fma(-ar, pc, cb[u]);
@@ -220,12 +224,13 @@ __global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
     const int nx = prm.nx, m = prm.m;
     const long long kk = l / nx;
     const int i = (int)(l - kk * nx);
-    const size_t off0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
-    const double *__restrict__ sa = prm.sa + off0;
-    const double *__restrict__ sc = prm.sc + off0;
-    const double *__restrict__ sd = prm.sd + off0;
+    const size_t off0 = (size_t)kk * (size_t)prm.os + i + (size_t)p * m * (size_t)prm.rs;
+    const size_t soff0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
+    const double *__restrict__ sa = prm.sa + soff0;
+    const double *__restrict__ sc = prm.sc + soff0;
+    const double *__restrict__ sd = prm.sd + soff0;
     double *__restrict__ x = prm.x + off0;
-    const size_t s = (size_t)nx;
+    const size_t s = (size_t)prm.rs, ss = (size_t)nx;
     const size_t Lb = (size_t)prm.Lb;
 
     const double xf = ld_keep(prm.y + (size_t)(2 * p) * Lb + l);
@@ -238,7 +243,7 @@ __global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         const int r = m - 2 - u;
-        if (r >= 1) { na[u] = ld_keep(sa + r * s); nc[u] = ld_keep(sc + r * s); nd[u] = ld_keep(sd + r * s); }
+        if (r >= 1) { na[u] = ld_keep(sa + r * ss); nc[u] = ld_keep(sc + r * ss); nd[u] = ld_keep(sd + r * ss); }
     }
     for (int r0 = m - 2; r0 >= 1; r0 -= U) {
         double ca[U], cc[U], cd[U];
@@ -247,7 +252,7 @@ __global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
 #pragma unroll
         for (int u = 0; u < U; ++u) {
             const int r = r0 - U - u;
-            if (r >= 1) { na[u] = ld_keep(sa + r * s); nc[u] = ld_keep(sc + r * s); nd[u] = ld_keep(sd + r * s); }
+            if (r >= 1) { na[u] = ld_keep(sa + r * ss); nc[u] = ld_keep(sc + r * ss); nd[u] = ld_keep(sd + r * ss); }
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {

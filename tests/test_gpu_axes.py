@@ -1,0 +1,81 @@
+"""SURVEY 8(f) f1 (BASELINE cfg 4, ADI sweeps): z sweeps and cyclic lines through the C ABI against
+the oracle (oracle.solve_axis), element by element.  x sweeps are not implemented."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import tdma_inputs
+import paper_2509_03933_b200 as tdma
+
+pytestmark = pytest.mark.gpu
+TOL_E = 1e-11
+
+
+def dev():
+    return torch.device("cuda:0")
+
+
+def solve(a, b, c, d, P, batch, **opts):
+    nz, ny, nx = a.shape
+    x = torch.full_like(d, float("nan"))
+    with tdma.Plan(nx, ny, nz, P, batch, **opts) as plan:
+        plan.solve(a, b, c, d, x)
+        torch.cuda.synchronize()
+    return x
+
+
+def check(a, b, c, d, x, axis, periodic):
+    an, bn, cn, dn, xn = [t.cpu().numpy() for t in (a, b, c, d, x)]
+    assert np.isfinite(xn).all()
+    ref = oracle.solve_axis(an, bn, cn, dn, axis, periodic)
+    ax = 1 if axis == "y" else 0
+    err = np.max(np.abs(xn - ref), axis=ax) / np.max(np.abs(ref), axis=ax)
+    assert err.max() <= TOL_E, err.max()
+
+
+@pytest.mark.parametrize("opts", [dict(variant=tdma.TDMA_VARIANT_PIPELINED), dict(variant=tdma.TDMA_VARIANT_FUSED)],
+                         ids=["pipelined", "fused_tma"])
+@pytest.mark.parametrize("shape,P,batch", [((64, 48, 32), 4, 0), ((256, 20, 64), 8, 7), ((32, 3, 46), 16, 2),
+                                           ((512, 6, 128), 8, 4)])
+def test_z_sweep(opts, shape, P, batch):
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 21, dev())
+    x = solve(a, b, c, d, P, batch, axis=tdma.TDMA_AXIS_Z, **opts)
+    check(a, b, c, d, x, "z", False)
+
+
+@pytest.mark.parametrize("axis", ["y", "z"])
+@pytest.mark.parametrize("n,P,cluster", [(64, 4, 0), (64, 4, 1), (256, 8, 4), (512, 8, 0), (1024, 16, 0), (8, 2, 2)])
+def test_cyclic_lines(axis, n, P, cluster):
+    other, nx = 6, 64
+    shape = (other, n, nx) if axis == "y" else (n, other, nx)
+    a, b, c, d = tdma_inputs.dominant_random(shape[2], shape[1], shape[0], 31, dev())
+    x = solve(a, b, c, d, P, 0, variant=tdma.TDMA_VARIANT_FUSED, periodic=1, fused_cluster=cluster,
+              axis=tdma.TDMA_AXIS_Z if axis == "z" else tdma.TDMA_AXIS_Y)
+    check(a, b, c, d, x, axis, True)
+
+
+def test_cfg4_adi_y_then_z_periodic_circulant_closed_form():
+    """cfg 4 coefficients (a = c = -alpha, b = 1 + 2 alpha): Dirichlet y sweep followed by a
+    periodic z sweep, the second one checked against the circulant closed form as well."""
+    w = tdma_inputs.make_workload("cfg4_adi_y", device=dev(), nx=64, ny=128, nz=256, P=8)
+    alpha = w.meta["alpha"]
+    x1 = solve(w.a, w.b, w.c, w.d, w.P, 32, variant=tdma.TDMA_VARIANT_FUSED)
+    check(w.a, w.b, w.c, w.d, x1, "y", False)
+    x2 = solve(w.a, w.b, w.c, x1, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_Z, periodic=1)
+    check(w.a, w.b, w.c, x1, x2, "z", True)
+    lam = 1 + 2 * alpha - 2 * alpha * np.cos(2 * np.pi * np.arange(w.nz) / w.nz)
+    ref = np.fft.ifft(np.fft.fft(x1.cpu().numpy(), axis=0) / lam[:, None, None], axis=0).real
+    assert np.max(np.abs(x2.cpu().numpy() - ref)) <= (1 + 4 * alpha) * 1e-13 * np.max(np.abs(ref))
+
+
+def test_unsupported_combinations_fail_loudly():
+    with pytest.raises(tdma.TdmaError):
+        tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1)
+    with pytest.raises(tdma.TdmaError):
+        tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1, axis=tdma.TDMA_AXIS_Z)
+    with pytest.raises(tdma.TdmaError):
+        tdma.Plan(32, 32, 32, 4, 0, axis=1)
+    with pytest.raises(tdma.TdmaError):            # P must divide the line length (nz for a z sweep)
+        tdma.Plan(32, 64, 30, 4, 0, axis=tdma.TDMA_AXIS_Z)

@@ -321,3 +321,58 @@ def test_thread_count_does_not_change_bits():
     oracle.set_threads(nmax)
     xn = oracle.solve_y(a, b, c, d)
     assert np.array_equal(x1, xn)
+
+
+# ---------------------------------------------------------------------------------------------
+# f1: cyclic lines and z sweeps
+# ---------------------------------------------------------------------------------------------
+def _cyclic_dense(a, b, c):
+    n = len(b)
+    A = np.zeros((n, n))
+    for j in range(n):
+        A[j, j] = b[j]
+        A[j, (j - 1) % n] += a[j]
+        A[j, (j + 1) % n] += c[j]
+    return A
+
+
+@pytest.mark.parametrize("n", [3, 4, 5, 17, 32])
+def test_f1_cyclic_oracle_vs_dense_lapack(n):
+    rng = np.random.default_rng(100 + n)
+    nx, nz = 5, 2
+    a = rng.uniform(-1, 1, (nz, n, nx)); c = rng.uniform(-1, 1, (nz, n, nx))
+    b = 2 + np.abs(a) + np.abs(c) + rng.uniform(0, 1, (nz, n, nx))
+    d = rng.uniform(-1, 1, (nz, n, nx))
+    x = oracle.solve_cyclic_y(a, b, c, d)
+    for k in range(nz):
+        for i in range(nx):
+            ref = np.linalg.solve(_cyclic_dense(a[k, :, i], b[k, :, i], c[k, :, i]), d[k, :, i])
+            assert np.max(np.abs(x[k, :, i] - ref)) <= 1e-14 * np.max(np.abs(ref))
+
+
+@pytest.mark.parametrize("alpha,n", [(0.1, 16), (3.7, 64), (10.0, 512)])
+def test_f1_cyclic_oracle_circulant_closed_form(alpha, n):
+    """a = c = -alpha, b = 1 + 2 alpha, periodic: the matrix is circulant, its eigenvalues are
+    lambda_q = 1 + 2 alpha - 2 alpha cos(2 pi q / n), so x = IFFT(FFT(d) / lambda)."""
+    rng = np.random.default_rng(7)
+    d = rng.uniform(-1, 1, (1, n, 3))
+    a = np.full_like(d, -alpha); b = np.full_like(d, 1 + 2 * alpha)
+    lam = 1 + 2 * alpha - 2 * alpha * np.cos(2 * np.pi * np.arange(n) / n)
+    ref = np.fft.ifft(np.fft.fft(d, axis=1) / lam[None, :, None], axis=1).real
+    x = oracle.solve_cyclic_y(a, b, a, d)
+    assert np.max(np.abs(x - ref)) <= (1 + 4 * alpha) * 4e-15 * np.max(np.abs(ref))
+
+
+def test_f1_solve_axis_z_is_the_transposed_problem():
+    rng = np.random.default_rng(3)
+    shape = (12, 5, 4)                                      # (nz, ny, nx): lines of length 12 along z
+    a = rng.uniform(-1, 1, shape); c = rng.uniform(-1, 1, shape)
+    b = 2 + np.abs(a) + np.abs(c); d = rng.uniform(-1, 1, shape)
+    x = oracle.solve_axis(a, b, c, d, "z")
+    for j in range(shape[1]):
+        for i in range(shape[2]):
+            ref = oracle.thomas_line(a[:, j, i], b[:, j, i], c[:, j, i], d[:, j, i])
+            assert np.allclose(x[:, j, i], ref, rtol=0, atol=1e-15)
+    xp = oracle.solve_axis(a, b, c, d, "z", periodic=True)
+    ref = np.linalg.solve(_cyclic_dense(a[:, 2, 1], b[:, 2, 1], c[:, 2, 1]), d[:, 2, 1])
+    assert np.max(np.abs(xp[:, 2, 1] - ref)) <= 1e-14
