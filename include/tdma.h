@@ -96,7 +96,10 @@ typedef struct tdma_options {
     int axis;            /* direction of the systems (BASELINE cfg 4): TDMA_AXIS_Y = 0
                             (default; lines along y, y split into P partitions, `batch` counts
                             z-slices) or TDMA_AXIS_Z = 2 (lines along z, stride nx*ny, z split into
-                            P partitions, `batch` counts y-slices).  x sweeps are not implemented */
+                            P partitions, `batch` counts y-slices) or TDMA_AXIS_X = 1 (lines along
+                            x, the contiguous axis, x split into P partitions, `batch` counts
+                            z-slices; FUSED TMA kernel only, nx a multiple of 16, 16-byte aligned
+                            arrays including x) */
     int periodic;        /* 1 = cyclic lines: row 0 couples to row n-1 through a_0 and row n-1 to
                             row 0 through c_{n-1} (both entries are then USED).  The cyclic
                             coupling is resolved at the root of the recursion, so only the FUSED
@@ -104,7 +107,7 @@ typedef struct tdma_options {
     int reserved[2];
 } tdma_options;
 
-enum { TDMA_AXIS_Y = 0, TDMA_AXIS_Z = 2 };
+enum { TDMA_AXIS_Y = 0, TDMA_AXIS_X = 1, TDMA_AXIS_Z = 2 };
 
 /* Plan for an nx*ny*nz slab with y split into P partitions of ny/P rows and `batch` z-slices per
  * pipeline stage (batch_z of PAPER.md:236; 0 = all slices in one batch; a last smaller batch is

@@ -177,12 +177,11 @@ def solve_cyclic_y(a, b, c, d, precision: str = "f64") -> np.ndarray:
 
 
 def solve_axis(a, b, c, d, axis: str = "y", periodic: bool = False, precision: str = "f64") -> np.ndarray:
-    """Lines along y or z of (nz, ny, nx) arrays; a z sweep is the y sweep of the arrays with
-    their first two axes exchanged."""
-    if axis not in ("y", "z"):
-        raise ValueError(axis)
+    """Lines along x, y or z of (nz, ny, nx) arrays: an x / z sweep is the y sweep of the arrays
+    with the solve axis exchanged with y."""
+    perm = {"y": None, "z": (1, 0, 2), "x": (0, 2, 1)}[axis]     # brings the solve axis to position 1
     arrs = [_as3(t) for t in (a, b, c, d)]
-    if axis == "z":
-        arrs = [np.ascontiguousarray(t.transpose(1, 0, 2)) for t in arrs]
+    if perm:
+        arrs = [np.ascontiguousarray(t.transpose(perm)) for t in arrs]
     x = (solve_cyclic_y if periodic else solve_y)(*arrs, precision)
-    return np.ascontiguousarray(x.transpose(1, 0, 2)) if axis == "z" else x
+    return np.ascontiguousarray(x.transpose(perm)) if perm else x

@@ -19,7 +19,7 @@ from . import build as _build
 TDMA_F64 = 0
 TDMA_OK, TDMA_ERR_INVALID_ARG, TDMA_ERR_UNSUPPORTED, TDMA_ERR_ALLOC, TDMA_ERR_CUDA = 0, -1, -2, -3, -4
 TDMA_VARIANT_AUTO, TDMA_VARIANT_PIPELINED, TDMA_VARIANT_FUSED = 0, 1, 2
-TDMA_AXIS_Y, TDMA_AXIS_Z = 0, 2
+TDMA_AXIS_Y, TDMA_AXIS_X, TDMA_AXIS_Z = 0, 1, 2
 TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
 (TDMA_GET_NB, TDMA_GET_M, TDMA_GET_BATCH, TDMA_GET_NSTREAMS, TDMA_GET_DEPTH, TDMA_GET_VARIANT,
  TDMA_GET_LAUNCHES, TDMA_GET_FUSED_LINES, TDMA_GET_FUSED_CLUSTER, TDMA_GET_GRAPH_BUILDS,

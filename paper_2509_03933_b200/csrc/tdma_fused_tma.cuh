@@ -64,6 +64,7 @@ struct TmaFusedConfig {
     int threads = 0;    // W * TX
     int box_rows = 0;   // rows per TMA box (<= 256), divides R
     int max_clusters = 0;  // co-resident clusters (persistent grid size), filled at first launch
+    bool xaxis = false;    // x sweep: 16-row leaves, swizzled boxes, staging tile for x
     size_t smem = 0;
 };
 
@@ -82,8 +83,10 @@ struct TmaFusedParams {
 #endif
 };
 
-__host__ __device__ inline size_t tma_fused_smem_bytes(int TX, int R, int W, int CL)
+__host__ __device__ inline size_t tma_fused_smem_bytes(int TX, int R, int W, int CL, bool xaxis = false)
 {
+    if (xaxis)   // + staging tile [R][TX] for x
+        return ((size_t)5 * R * TX + (size_t)4 * 2 * W * TX + (size_t)2 * 4 * 2 * CL * TX) * sizeof(double) + 128;
     // raw tile: 4 arrays [R][TX]; node buffer 4 x [2 W][TX]; cluster-level system, two inboxes of
     // 4 x [2 CL][TX]; three mbarriers (+ padding)
     return ((size_t)4 * R * TX + (size_t)4 * 2 * W * TX + (size_t)2 * 4 * 2 * CL * TX) * sizeof(double) + 128;
@@ -338,6 +341,41 @@ struct LeafRegs {
     double ma[2], mc[2], md[2];
 };
 
+// Last step of a leaf sweep: normalise the first-row equations of the sub-leaves and, for two
+// sub-leaves, merge them pairwise in registers.
+template <int M0>
+__device__ __forceinline__ void leaf_finish(double (&fa)[LeafRegs<M0>::K], double (&fb)[LeafRegs<M0>::K],
+                                            double (&fc)[LeafRegs<M0>::K], double (&fd)[LeafRegs<M0>::K],
+                                            double (&pa)[LeafRegs<M0>::K], double (&pc)[LeafRegs<M0>::K],
+                                            double (&pd)[LeafRegs<M0>::K], Eq &f, Eq &l, LeafRegs<M0> &R)
+{
+    constexpr int K = LeafRegs<M0>::K;
+#pragma unroll
+    for (int h = 0; h < K; ++h) {                                // H == 2: fb = 1, frontier is x_1
+        const double inv = rcp_nr(fb[h]);
+        fa[h] *= inv; fc[h] *= inv; fd[h] *= inv;
+    }
+    if (K == 1) {
+        f.a = fa[0]; f.b = 1.0; f.c = fc[0]; f.d = fd[0];
+        l.a = pa[0]; l.b = 1.0; l.c = pc[0]; l.d = pd[0];
+    } else {
+        // pairwise merge of the two sub-leaves in registers (unit diagonals):
+        // (A1, C1, D1) = first / (A2, C2, D2) = last eq of sub-leaf 0, (A3..), (A4..) of sub-leaf 1
+        const double A1 = fa[0], C1 = fc[0], D1 = fd[0], A2 = pa[0], C2 = pc[0], D2 = pd[0];
+        const double A3 = fa[K - 1], C3 = fc[K - 1], D3 = fd[K - 1], A4 = pa[K - 1], C4 = pc[K - 1], D4 = pd[K - 1];
+        const double det = fma(-C2, A3, 1.0);
+        const double nL = fma(-C2, D3, D2), nR = fma(-A3, D2, D3);
+        const double p2 = C2 * C3, p3 = A3 * A2;
+        f.b = fma(-C1, A2, det); l.b = fma(-A4, C3, det);
+        const double sf = pow2_unscale(f.b), sl = pow2_unscale(l.b);
+        f.a = det * A1 * sf; f.b *= sf; f.c = C1 * p2 * sf; f.d = fma(det, D1, -(C1 * nL)) * sf;
+        l.a = A4 * p3 * sl; l.b *= sl; l.c = det * C4 * sl; l.d = fma(det, D4, -(A4 * nR)) * sl;
+        const double inv = rcp_nr(det);
+        R.ma[0] = A2 * inv; R.mc[0] = -(p2 * inv); R.md[0] = nL * inv;
+        R.ma[1] = -(p3 * inv); R.mc[1] = C3 * inv; R.md[1] = nR * inv;
+    }
+}
+
 // Modified Thomas reduction (tdma_stage_kernels.cuh) of the sub-leaves, read from the raw tile at
 // offset o0 (row stride TX).  Returns the leaf's two boundary equations
 //   f: A x_prev + B x_0 + C x_last = D        l: A x_0 + B x_last + C x_next = D
@@ -381,30 +419,7 @@ __device__ __forceinline__ void leaf_reduce(const double *__restrict__ sA, const
             pa[h] = -(ar * pa[h]) * inv;
         }
     }
-#pragma unroll
-    for (int h = 0; h < K; ++h) {                                // H == 2: fb = 1, frontier is x_1
-        const double inv = rcp_nr(fb[h]);
-        fa[h] *= inv; fc[h] *= inv; fd[h] *= inv;
-    }
-    if (K == 1) {
-        f.a = fa[0]; f.b = 1.0; f.c = fc[0]; f.d = fd[0];
-        l.a = pa[0]; l.b = 1.0; l.c = pc[0]; l.d = pd[0];
-    } else {
-        // pairwise merge of the two sub-leaves in registers (unit diagonals):
-        // (A1, C1, D1) = first / (A2, C2, D2) = last eq of sub-leaf 0, (A3..), (A4..) of sub-leaf 1
-        const double A1 = fa[0], C1 = fc[0], D1 = fd[0], A2 = pa[0], C2 = pc[0], D2 = pd[0];
-        const double A3 = fa[K - 1], C3 = fc[K - 1], D3 = fd[K - 1], A4 = pa[K - 1], C4 = pc[K - 1], D4 = pd[K - 1];
-        const double det = fma(-C2, A3, 1.0);
-        const double nL = fma(-C2, D3, D2), nR = fma(-A3, D2, D3);
-        const double p2 = C2 * C3, p3 = A3 * A2;
-        f.b = fma(-C1, A2, det); l.b = fma(-A4, C3, det);
-        const double sf = pow2_unscale(f.b), sl = pow2_unscale(l.b);
-        f.a = det * A1 * sf; f.b *= sf; f.c = C1 * p2 * sf; f.d = fma(det, D1, -(C1 * nL)) * sf;
-        l.a = A4 * p3 * sl; l.b *= sl; l.c = det * C4 * sl; l.d = fma(det, D4, -(A4 * nR)) * sl;
-        const double inv = rcp_nr(det);
-        R.ma[0] = A2 * inv; R.mc[0] = -(p2 * inv); R.md[0] = nL * inv;
-        R.ma[1] = -(p3 * inv); R.mc[1] = C3 * inv; R.md[1] = nR * inv;
-    }
+    leaf_finish<M0>(fa, fb, fc, fd, pa, pc, pd, f, l, R);
 }
 
 // Back-substitution of the leaf from registers given its first and last unknown; x streamed to
@@ -437,18 +452,102 @@ __device__ __forceinline__ void leaf_back(const LeafRegs<M0> &R, double xf, doub
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// x sweeps (lines along the fastest axis).  A leaf is 16 consecutive x of one line = one 128-byte
+// row; the raw tile arrives as one (16 x, TX lines) TMA box per leaf and array with the 128-byte
+// swizzle: the 16-byte chunk q of box row l sits at chunk q ^ (l & 7).  A thread reads its row
+// with 16-byte loads; the 8 lanes of a quarter warp (8 consecutive lines) then touch 8 different
+// chunks, i.e. all 32 banks once.  x goes back through a staging tile with the same layout and
+// one TMA store per leaf box.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t xs_addr(uint32_t box, int l, int pair)
+{
+    return box + (uint32_t)l * 128u + (uint32_t)((pair ^ (l & 7)) << 4);
+}
+
+// bA..bD: shared addresses of this leaf's boxes.  Same arithmetic as leaf_reduce<TX, 16>.
+__device__ __forceinline__ void leaf_reduce_x(uint32_t bA, uint32_t bB, uint32_t bC, uint32_t bD, int l,
+                                              bool first_leaf, bool last_leaf, Eq &f, Eq &le, LeafRegs<16> &R)
+{
+    constexpr int K = 2, H = 8;
+    double fa[K], fb[K], fc[K], fd[K], pa[K], pc[K], pd[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const double2 a2 = lds2(xs_addr(bA, l, 4 * h)), b2 = lds2(xs_addr(bB, l, 4 * h));
+        const double2 c2 = lds2(xs_addr(bC, l, 4 * h)), d2 = lds2(xs_addr(bD, l, 4 * h));
+        double inv = rcp_nr(b2.x);
+        fa[h] = (h == 0 && first_leaf) ? 0.0 : a2.x * inv;
+        fc[h] = c2.x * inv; fd[h] = d2.x * inv; fb[h] = 1.0;
+        inv = rcp_nr(b2.y);
+        pa[h] = a2.y * inv; pc[h] = c2.y * inv; pd[h] = d2.y * inv;
+    }
+#pragma unroll
+    for (int p = 1; p < H / 2; ++p) {
+        double2 a2[K], b2[K], c2[K], d2[K];
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            a2[h] = lds2(xs_addr(bA, l, 4 * h + p)); b2[h] = lds2(xs_addr(bB, l, 4 * h + p));
+            c2[h] = lds2(xs_addr(bC, l, 4 * h + p)); d2[h] = lds2(xs_addr(bD, l, 4 * h + p));
+        }
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int r = 2 * p + e;
+#pragma unroll
+            for (int h = 0; h < K; ++h) {
+                const double ar = e ? a2[h].y : a2[h].x, br = e ? b2[h].y : b2[h].x, dr = e ? d2[h].y : d2[h].x;
+                double cr = e ? c2[h].y : c2[h].x;
+                if (r == H - 1 && h == K - 1 && last_leaf) cr = 0.0;
+                fb[h] = fma(-fc[h], pa[h], fb[h]);
+                fd[h] = fma(-fc[h], pd[h], fd[h]);
+                fc[h] = -fc[h] * pc[h];
+                R.ia[h][r - 2] = pa[h]; R.ic[h][r - 2] = pc[h]; R.id[h][r - 2] = pd[h];
+                const double inv = rcp_nr(fma(-ar, pc[h], br));
+                pd[h] = fma(-ar, pd[h], dr) * inv;
+                pc[h] = cr * inv;
+                pa[h] = -(ar * pa[h]) * inv;
+            }
+        }
+    }
+    leaf_finish<16>(fa, fb, fc, fd, pa, pc, pd, f, le, R);
+}
+
+// Back-substitution of a 16-row leaf into the staging box bX (row l).
+__device__ __forceinline__ void leaf_back_x(const LeafRegs<16> &R, double xf, double xl, uint32_t bX, int l)
+{
+    constexpr int K = 2, H = 8;
+    double xs[16];
+    double first[K], last[K];
+    first[0] = xf; last[1] = xl;
+    last[0] = fma(-R.mc[0], xl, fma(-R.ma[0], xf, R.md[0]));
+    first[1] = fma(-R.mc[1], xl, fma(-R.ma[1], xf, R.md[1]));
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        xs[h * H] = first[h]; xs[h * H + H - 1] = last[h];
+        double xn = last[h];
+#pragma unroll
+        for (int r = H - 2; r >= 1; --r) {
+            xn = fma(-R.ic[h][r - 1], xn, fma(-R.ia[h][r - 1], first[h], R.id[h][r - 1]));
+            xs[h * H + r] = xn;
+        }
+    }
+#pragma unroll
+    for (int p = 0; p < 8; ++p) sts2(xs_addr(bX, l, p), xs[2 * p], xs[2 * p + 1]);
+}
+
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
 #define TDMA_STAMP(i) do { if (threadIdx.x == 0 && it == 1) prm.dbg[(size_t)blockIdx.x * 16 + (i)] = clock64(); } while (0)
 #else
 #define TDMA_STAMP(i) do { } while (0)
 #endif
 
-template <int TX, int M0, bool kCluster, int MAXT, int MINB>
+// kX: x sweep (lanes = TX lines along y, rows = x; M0 = 16 only); tm_x is used by x sweeps only.
+template <int TX, int M0, bool kCluster, int MAXT, int MINB, bool kX>
 __global__ void __launch_bounds__(MAXT, MINB)
 fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
                  const __grid_constant__ CUtensorMap tm_c, const __grid_constant__ CUtensorMap tm_d,
-                 const TmaFusedParams prm)
+                 const __grid_constant__ CUtensorMap tm_x, const TmaFusedParams prm)
 {
+    static_assert(!kX || M0 == 16, "x sweeps use 16-row (128-byte) leaves");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const int R = prm.R, CL = prm.CL, W = prm.W;
     const int arr = R * TX;
@@ -457,7 +556,8 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     double *__restrict__ sC = sB + arr;
     double *__restrict__ sD = sC + arr;
     const int narr = 2 * W * TX;
-    double *node = sD + arr;                                          // node buffer, 4 x [2W][TX]
+    double *sX = sD + arr;                                            // x staging tile (x sweeps)
+    double *node = sX + (kX ? arr : 0);                               // node buffer, 4 x [2W][TX]
     const int NTR = 2 * CL;                                    // rows of the cluster-level system
     const int tarr = NTR * TX;
     double *top = node + 4 * narr;                             // 2 inboxes x 4 x [NTR][TX]
@@ -478,7 +578,15 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     auto issue_tile = [&](int tile) {   // thread 0: the whole raw tile of `tile` in flight at once
         const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
         ptx::mbar_expect_tx(&bar[0], (unsigned)(4 * arr * sizeof(double)));
-        for (int q = 0; q < prm.nbox; ++q) {
+        if (kX) {                       // one (16 x, TX lines) box per leaf; x0 = first line (y)
+            for (int w = 0; w < W; ++w) {
+                const int so = w * 16 * TX;
+                ptx::tma_load_3d(sB + so, &tm_b, y0 + 16 * w, x0, k, &bar[0]);
+                ptx::tma_load_3d(sA + so, &tm_a, y0 + 16 * w, x0, k, &bar[0]);
+                ptx::tma_load_3d(sC + so, &tm_c, y0 + 16 * w, x0, k, &bar[0]);
+                ptx::tma_load_3d(sD + so, &tm_d, y0 + 16 * w, x0, k, &bar[0]);
+            }
+        } else for (int q = 0; q < prm.nbox; ++q) {
             const int yy = y0 + q * prm.box_rows;
             const int so = q * prm.box_rows * TX;
             const int c1 = prm.axis_z ? k : yy, c2 = prm.axis_z ? yy : k;
@@ -509,6 +617,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         tb.ab = ptx::smem_u32(top + par * 4 * tarr); tb.plane = (uint32_t)tarr * 16u;
         // arm this tile's inbox: 4 doubles per (node equation, line) from every CTA
         if (kCluster && t == 0) ptx::mbar_expect_tx(&bar[1 + par], (unsigned)(4 * tarr * sizeof(double)));
+        if (kX && t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         TDMA_STAMP(0);
         ptx::mbar_wait(&bar[0], (unsigned)par);
         TDMA_STAMP(1);
@@ -517,7 +626,13 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         LeafRegs<M0> regs;
         {
             Eq f, l;
-            leaf_reduce<TX, M0>(sA, sB, sC, sD, o0, first_leaf, last_leaf, f, l, regs);
+            if constexpr (kX) {
+                const uint32_t bo = (uint32_t)(leaf * 16 * TX) * 8u;
+                leaf_reduce_x(ptx::smem_u32(sA) + bo, ptx::smem_u32(sB) + bo, ptx::smem_u32(sC) + bo,
+                              ptx::smem_u32(sD) + bo, lx, first_leaf, last_leaf, f, l, regs);
+            } else {
+                leaf_reduce<TX, M0>(sA, sB, sC, sD, o0, first_leaf, last_leaf, f, l, regs);
+            }
             const uint32_t of = nb_ab<TX>(nb, 2 * leaf, lx), ol = of + TX * 16u;
             sts2(of, f.a, f.b); sts2(of + nb.plane, f.c, f.d);
             sts2(ol, l.a, l.b); sts2(ol + nb.plane, l.c, l.d);
@@ -582,7 +697,18 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
             const double xf = lds1(nb_ab<TX>(nb, 2 * leaf, lx) + nb.plane + 8);
             const double xl = lds1(nb_ab<TX>(nb, 2 * leaf + 1, lx) + nb.plane + 8);
-            if (x0 + lx < prm.nx) {     // ragged last x tile: TMA zero-filled those lanes
+            if constexpr (kX) {
+                // the staging tile of the previous iteration has been read by the TMA engine
+                // (thread 0 waited at the top of this iteration, barriers in between)
+                leaf_back_x(regs, xf, xl, ptx::smem_u32(sX) + (uint32_t)(leaf * 16 * TX) * 8u, lx);
+                ptx::fence_proxy_async_smem();
+                __syncthreads();
+                if (t == 0) {
+                    for (int w = 0; w < W; ++w)
+                        ptx::tma_store_3d(&tm_x, y0 + 16 * w, x0, k, sX + w * 16 * TX);
+                    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                }
+            } else if (x0 + lx < prm.nx) {     // ragged last x tile: TMA zero-filled those lanes
                 leaf_back<M0>(regs, xf, xl,
                               prm.x + (size_t)k * (size_t)prm.os + (size_t)(y0 + leaf * M0) * (size_t)prm.rs +
                                   (size_t)(x0 + lx), (size_t)prm.rs);
@@ -596,6 +722,8 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         }
 #endif
     }
+    // the staging tile must outlive the last TMA store
+    if (kX && t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // ------------------------------------------------------------------------------------------
@@ -608,9 +736,16 @@ inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 // level is the paper's partition level), the tile fits shared memory.
 inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int want_lines,
                                 int want_cluster, int want_leaf, const cudaDeviceProp &prop,
-                                const char **why)
+                                const char **why, bool xaxis = false)
 {
-    if (nx % 2) { *why = "TMA path needs even nx (16-byte global strides)"; return false; }
+    // x sweep: nx = number of lanes (caller's ny), ny = line length (caller's nx)
+    if (xaxis) {
+        if (ny % 2) { *why = "TMA path needs even nx (16-byte global strides)"; return false; }
+        if ((want_lines && want_lines != 16) || (want_leaf && want_leaf != 16)) {
+            *why = "x sweeps use 16 lines per tile and 16-row leaves"; return false;
+        }
+        want_lines = 16; want_leaf = 16;
+    } else if (nx % 2) { *why = "TMA path needs even nx (16-byte global strides)"; return false; }
     const int m = ny / P;
     const size_t max_smem = prop.sharedMemPerBlockOptin;
     const size_t sm_smem = prop.sharedMemPerMultiprocessor;
@@ -634,13 +769,14 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
                 TmaFusedConfig c;
                 c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
                 c.threads = c.leaves * TX;
-                if (c.threads > 1024) continue;
+                if (c.threads > 1024 || (xaxis && c.threads > 256)) continue;
                 c.nlev = 0;
                 while ((1 << c.nlev) < c.leaves) ++c.nlev;
                 c.box_rows = R;
                 while (c.box_rows > 256) c.box_rows /= 2;
                 if (R % c.box_rows) continue;
-                c.smem = tma_fused_smem_bytes(TX, R, c.leaves, CL);
+                c.xaxis = xaxis;
+                c.smem = tma_fused_smem_bytes(TX, R, c.leaves, CL, xaxis);
                 if (c.smem > max_smem) continue;
                 long ctas = (long)(sm_smem / (c.smem + 1024));
                 const long by_thr = 2048 / c.threads;
@@ -712,11 +848,26 @@ inline bool make_slab_tensor_map(CUtensorMap *tm, const void *base, int nx, int 
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int TX, int M0, bool kCluster, int MAXT, int MINB>
+// x sweep: contiguous fp64 slab (rows = x fastest, lanes = y, slices); box (16 x, TX lanes, 1)
+// with the 128-byte swizzle.
+inline bool make_xsweep_tensor_map(CUtensorMap *tm, const void *base, int nrows, int nlanes, int nslices, int TX)
+{
+    tdma_encode_tiled_fn enc = get_encode_tiled();
+    if (!enc) return false;
+    cuuint64_t gdim[3] = {(cuuint64_t)nrows, (cuuint64_t)nlanes, (cuuint64_t)nslices};
+    cuuint64_t gstr[2] = {(cuuint64_t)nrows * sizeof(double), (cuuint64_t)nrows * nlanes * sizeof(double)};
+    cuuint32_t box[3] = {16, (cuuint32_t)TX, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), gdim, gstr, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int TX, int M0, bool kCluster, int MAXT, int MINB, bool kX = false>
 inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                    cudaStream_t st)
 {
-    auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, MINB>;
+    auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, MINB, kX>;
     size_t smem_bytes = cfg.smem;
 #if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
     if (const char *pad = getenv("TDMA_PAD")) smem_bytes += (size_t)atoi(pad);   // experiment: fewer CTAs per SM
@@ -755,7 +906,7 @@ inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, c
     if (prm.ntiles <= 0) return cudaSuccess;    // prepare only (attributes + persistent grid size)
     const int nc = prm.ntiles < cfg.max_clusters ? prm.ntiles : cfg.max_clusters;
     lc.gridDim = dim3((unsigned)(nc * cfg.cluster));
-    return cudaLaunchKernelEx(&lc, kern, tm[0], tm[1], tm[2], tm[3], prm);
+    return cudaLaunchKernelEx(&lc, kern, tm[0], tm[1], tm[2], tm[3], tm[4], prm);
 }
 
 template <int TX, int M0, bool kCluster>
@@ -788,11 +939,14 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
                                     int nzs, long long rs, long long os, bool axis_z, bool periodic,
                                     cudaStream_t st)
 {
-    CUtensorMap tm[4];
-    const void *ptr[4] = {a, b, c, d};
-    for (int i = 0; i < 4 && nzs > 0; ++i)
-        if (!make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows))
+    CUtensorMap tm[5];
+    const void *ptr[5] = {a, b, c, d, x};
+    for (int i = 0; i < 5 && nzs > 0; ++i) {
+        if (i == 4 && !cfg.xaxis) { tm[4] = tm[3]; break; }      // x is stored from registers
+        if (cfg.xaxis ? !make_xsweep_tensor_map(&tm[i], ptr[i], ny, nx, nzs, cfg.lines)
+                      : !make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows))
             return cudaErrorInvalidValue;
+    }
     TmaFusedParams prm;
     prm.nx = nx; prm.ny = ny; prm.nzs = nzs;
     prm.x = x;
@@ -809,6 +963,9 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
     }
 #endif
     const bool cl = cfg.cluster > 1;
+    if (cfg.xaxis)
+        return cl ? launch_tma_inst<16, 16, true, 256, 1, true>(cfg, tm, prm, st)
+                  : launch_tma_inst<16, 16, false, 256, 1, true>(cfg, tm, prm, st);
     switch (cfg.lines) {
     case 32: return cl ? launch_tma_tx<32, true>(cfg, tm, prm, st) : launch_tma_tx<32, false>(cfg, tm, prm, st);
     case 16: return cl ? launch_tma_tx<16, true>(cfg, tm, prm, st) : launch_tma_tx<16, false>(cfg, tm, prm, st);

@@ -237,9 +237,10 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
         const int bzn = std::min(pl->bz, nz_count - k0);
         const size_t off = (size_t)k0 * (size_t)pl->os;
         const bool az = pl->axis == TDMA_AXIS_Z, per = pl->periodic != 0;
+        const bool plain_y = pl->axis == TDMA_AXIS_Y && !per;
         cudaError_t e;
-        const bool aligned = ((((uintptr_t)ptr.a | (uintptr_t)ptr.b | (uintptr_t)ptr.c |
-                                (uintptr_t)ptr.d) & 15) == 0);   // tensor maps of the inputs
+        const bool aligned = ((((uintptr_t)ptr.a | (uintptr_t)ptr.b | (uintptr_t)ptr.c | (uintptr_t)ptr.d |
+                                (pl->axis == TDMA_AXIS_X ? (uintptr_t)ptr.x : 0)) & 15) == 0);   // tensor maps
         if (pl->fused_impl == 2 && aligned) {
             // Fill launch: a cluster of >= 4 CTAs cannot be placed on every SM.  With one main CTA
             // per SM the SMs left over take a second persistent launch with clusters of 2 that
@@ -280,12 +281,12 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
                 CUDA_TRY(cudaEventRecord(pl->evBJoin, pl->sB));
                 CUDA_TRY(cudaStreamWaitEvent(origin, pl->evBJoin, 0));
             }
-        } else if (pl->fused.threads > 0 && !az && !per)
+        } else if (pl->fused.threads > 0 && plain_y)
             e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
                                    ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
         else
             return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel needs 16-byte aligned arrays%s",
-                           az || per ? " (z sweeps and cyclic lines have no other kernel)" : "");
+                           plain_y ? "" : " (x / z sweeps and cyclic lines have no other kernel)");
         if (e != cudaSuccess)
             return set_err(TDMA_ERR_CUDA, "fused launch failed: %s", cudaGetErrorString(e));
     }
@@ -389,6 +390,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
     if (variant == TDMA_VARIANT_AUTO) variant = TDMA_VARIANT_PIPELINED;
     if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED)
         return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
+    if (pl->axis == TDMA_AXIS_X && variant != TDMA_VARIANT_FUSED)
+        return set_err(TDMA_ERR_UNSUPPORTED, "x sweeps need the FUSED variant (TMA kernel)");
     if (pl->periodic && (variant != TDMA_VARIANT_FUSED || pl->ny < 2))
         return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need the FUSED variant (TMA kernel) and >= 2 rows");
     pl->variant = variant;
@@ -435,7 +438,7 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         int want_impl = opt ? opt->fused_impl : 0;
         if (want_impl < 0 || want_impl > 2)
             return set_err(TDMA_ERR_INVALID_ARG, "unknown fused_impl %d", want_impl);
-        if (pl->axis == TDMA_AXIS_Z || pl->periodic) {
+        if (pl->axis != TDMA_AXIS_Y || pl->periodic) {
             if (want_impl == 1)
                 return set_err(TDMA_ERR_UNSUPPORTED, "the register-staged fused kernel does y sweeps of plain lines only");
             want_impl = 2;
@@ -445,7 +448,7 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
             have_tma = tdma::get_encode_tiled() != nullptr &&
                        tdma::configure_tma_fused(&pl->tfused, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
                                                  opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
-                                                 prop, &why);
+                                                 prop, &why, pl->axis == TDMA_AXIS_X);
             if (!have_tma && want_impl == 2)
                 return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel unavailable: %s",
                                why ? why : "cuTensorMapEncodeTiled not found");
@@ -453,7 +456,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         // the register-staged kernel is the fallback for unaligned pointers (explicit options
         // are only forwarded to it when it was asked for)
         const bool fwd = want_impl == 1 || !have_tma;
-        const bool have_reg = tdma::configure_fused(&pl->fused, pl->nx, pl->ny, pl->P,
+        const bool have_reg = pl->axis == TDMA_AXIS_Y && !pl->periodic &&
+                              tdma::configure_fused(&pl->fused, pl->nx, pl->ny, pl->P,
                                                     fwd && opt ? opt->fused_lines : 0,
                                                     fwd && opt ? opt->fused_cluster : 0,
                                                     fwd && opt ? opt->fused_leaf_rows : 0,
@@ -468,7 +472,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         if (have_tma && pl->tfused.cluster >= 4 && pl->fill_opt >= 0) {
             const char *why2 = nullptr;
             pl->have_fill = tdma::configure_tma_fused(&pl->tfill, pl->nx, pl->ny, pl->P, 0,
-                                                      pl->ny % 2 == 0 ? 2 : 1, 0, prop, &why2);
+                                                      pl->ny % 2 == 0 ? 2 : 1, 0, prop, &why2,
+                                                      pl->axis == TDMA_AXIS_X);
         }
     }
     return TDMA_OK;
@@ -491,8 +496,9 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
 {
     g_err[0] = 0;
     const int axis = options ? options->axis : TDMA_AXIS_Y, periodic = options && options->periodic ? 1 : 0;
-    if (axis != TDMA_AXIS_Y && axis != TDMA_AXIS_Z) { set_err(TDMA_ERR_UNSUPPORTED, "axis %d: only TDMA_AXIS_Y (0) and TDMA_AXIS_Z (2) are implemented", axis); return nullptr; }
-    if (axis == TDMA_AXIS_Z) std::swap(ny, nz);   // from here on: ny = line length, nz = slices
+    if (axis != TDMA_AXIS_Y && axis != TDMA_AXIS_Z && axis != TDMA_AXIS_X) { set_err(TDMA_ERR_INVALID_ARG, "unknown axis %d", axis); return nullptr; }
+    if (axis == TDMA_AXIS_Z) std::swap(ny, nz);   // from here on: ny = line length, nz = slices,
+    if (axis == TDMA_AXIS_X) std::swap(nx, ny);   // nx = lanes (lines side by side in a tile)
     if (nx < 1 || ny < 1 || nz < 1) { set_err(TDMA_ERR_INVALID_ARG, "dimensions must be >= 1 (got %d x %d x %d)", nx, ny, nz); return nullptr; }
     if (P < 1) { set_err(TDMA_ERR_INVALID_ARG, "P must be >= 1 (got %d)", P); return nullptr; }
     if (ny % P != 0) { set_err(TDMA_ERR_INVALID_ARG, "ny = %d is not divisible by P = %d", ny, P); return nullptr; }
@@ -506,7 +512,7 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->P = P; pl->m = ny / P;   // ny, nz already mapped
     pl->axis = axis; pl->periodic = periodic;
     pl->rs = axis == TDMA_AXIS_Z ? (long long)nx * nz : (long long)nx;   // z sweep: plan nz = caller ny
-    pl->os = axis == TDMA_AXIS_Z ? (long long)nx : (long long)nx * ny;
+    pl->os = axis == TDMA_AXIS_Z ? (long long)nx : (long long)nx * ny;   // x sweep: slices are z-slices
     pl->bz = batch == 0 ? nz : batch;
     pl->nb = (nz + pl->bz - 1) / pl->bz;
     pl->slice = (size_t)nx * ny;
@@ -551,8 +557,8 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
     int rc = check_ptrs(plan, a, b, c, d, x);
     if (rc != TDMA_OK) return rc;
     tdma_plan *pl = plan;
-    if (pl->axis != TDMA_AXIS_Y)
-        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_host streams z-chunks: y sweeps only");
+    if (pl->axis == TDMA_AXIS_Z)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_host streams z-chunks: x and y sweeps only");
     if (!pl->sH2D) {  // first use: staging buffers, copy streams
         // chunk = whole batches, about 64 Mi cells (512 MiB per array) or the slab if smaller
         const size_t target = (size_t)1 << 26;

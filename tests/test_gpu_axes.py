@@ -1,5 +1,5 @@
 """SURVEY 8(f) f1 (BASELINE cfg 4, ADI sweeps): z sweeps and cyclic lines through the C ABI against
-the oracle (oracle.solve_axis), element by element.  x sweeps are not implemented."""
+the oracle (oracle.solve_axis), element by element: x, y and z sweeps, plain and cyclic lines."""
 import numpy as np
 import pytest
 import torch
@@ -29,7 +29,7 @@ def check(a, b, c, d, x, axis, periodic):
     an, bn, cn, dn, xn = [t.cpu().numpy() for t in (a, b, c, d, x)]
     assert np.isfinite(xn).all()
     ref = oracle.solve_axis(an, bn, cn, dn, axis, periodic)
-    ax = 1 if axis == "y" else 0
+    ax = {"y": 1, "z": 0, "x": 2}[axis]
     err = np.max(np.abs(xn - ref), axis=ax) / np.max(np.abs(ref), axis=ax)
     assert err.max() <= TOL_E, err.max()
 
@@ -70,12 +70,47 @@ def test_cfg4_adi_y_then_z_periodic_circulant_closed_form():
     assert np.max(np.abs(x2.cpu().numpy() - ref)) <= (1 + 4 * alpha) * 1e-13 * np.max(np.abs(ref))
 
 
+@pytest.mark.parametrize("periodic", [0, 1])
+@pytest.mark.parametrize("shape,P,cluster", [((3, 40, 64), 4, 0), ((2, 16, 256), 8, 1), ((4, 37, 512), 8, 2),
+                                             ((2, 50, 1024), 16, 4), ((1, 20, 2048), 16, 8), ((5, 7, 16), 1, 1)])
+def test_x_sweep(periodic, shape, P, cluster):
+    """Lines along the contiguous axis: swizzled TMA boxes in, staging tile + TMA store out;
+    ny not a multiple of the 16-line tile exercises the zero-fill / clipping."""
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 41, dev())
+    guard = torch.full((nz * ny * nx + 64,), float("nan"), dtype=torch.float64, device=dev())
+    x = guard[:nz * ny * nx].view(nz, ny, nx)
+    with tdma.Plan(nx, ny, nz, P, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X, periodic=periodic,
+                   fused_cluster=cluster) as plan:
+        plan.solve(a, b, c, d, x)
+        torch.cuda.synchronize()
+    assert torch.isnan(guard[nz * ny * nx:]).all()
+    check(a, b, c, d, x, "x", bool(periodic))
+
+
+def test_cfg4_adi_three_sweeps():
+    """BASELINE cfg 4 at reduced size: successive solves along x (periodic), y (Dirichlet) and z
+    (periodic) with a = c = -alpha, b = 1 + 2 alpha; each against the oracle."""
+    w = tdma_inputs.make_workload("cfg4_adi_y", device=dev(), nx=256, ny=128, nz=64, P=8)
+    F = tdma.TDMA_VARIANT_FUSED
+    x1 = solve(w.a, w.b, w.c, w.d, w.P, 0, variant=F, axis=tdma.TDMA_AXIS_X, periodic=1)
+    check(w.a, w.b, w.c, w.d, x1, "x", True)
+    x2 = solve(w.a, w.b, w.c, x1, w.P, 0, variant=F)
+    check(w.a, w.b, w.c, x1, x2, "y", False)
+    x3 = solve(w.a, w.b, w.c, x2, w.P, 0, variant=F, axis=tdma.TDMA_AXIS_Z, periodic=1)
+    check(w.a, w.b, w.c, x2, x3, "z", True)
+
+
 def test_unsupported_combinations_fail_loudly():
     with pytest.raises(tdma.TdmaError):
         tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1)
     with pytest.raises(tdma.TdmaError):
         tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1, axis=tdma.TDMA_AXIS_Z)
+    with pytest.raises(tdma.TdmaError):            # x sweeps: FUSED only
+        tdma.Plan(32, 32, 32, 2, 0, variant=tdma.TDMA_VARIANT_PIPELINED, axis=tdma.TDMA_AXIS_X)
+    with pytest.raises(tdma.TdmaError):            # x sweeps: 16-row leaves must tile the partitions
+        tdma.Plan(24, 32, 32, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X)
     with pytest.raises(tdma.TdmaError):
-        tdma.Plan(32, 32, 32, 4, 0, axis=1)
+        tdma.Plan(32, 32, 32, 4, 0, axis=3)
     with pytest.raises(tdma.TdmaError):            # P must divide the line length (nz for a z sweep)
         tdma.Plan(32, 64, 30, 4, 0, axis=tdma.TDMA_AXIS_Z)

@@ -376,3 +376,17 @@ def test_f1_solve_axis_z_is_the_transposed_problem():
     xp = oracle.solve_axis(a, b, c, d, "z", periodic=True)
     ref = np.linalg.solve(_cyclic_dense(a[:, 2, 1], b[:, 2, 1], c[:, 2, 1]), d[:, 2, 1])
     assert np.max(np.abs(xp[:, 2, 1] - ref)) <= 1e-14
+
+
+def test_f1_solve_axis_x_is_the_transposed_problem():
+    rng = np.random.default_rng(4)
+    shape = (3, 4, 16)                                      # lines of length 16 along x
+    a = rng.uniform(-1, 1, shape); c = rng.uniform(-1, 1, shape)
+    b = 2 + np.abs(a) + np.abs(c); d = rng.uniform(-1, 1, shape)
+    x = oracle.solve_axis(a, b, c, d, "x")
+    for k in range(shape[0]):
+        for j in range(shape[1]):
+            assert np.allclose(x[k, j], oracle.thomas_line(a[k, j], b[k, j], c[k, j], d[k, j]), rtol=0, atol=1e-15)
+    xp = oracle.solve_axis(a, b, c, d, "x", periodic=True)
+    ref = np.linalg.solve(_cyclic_dense(a[1, 2], b[1, 2], c[1, 2]), d[1, 2])
+    assert np.max(np.abs(xp[1, 2] - ref)) <= 1e-14
