@@ -260,6 +260,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e / cpu_baseline / stage legs")
     ap.add_argument("--sweep", action="store_true", help="S7 batch x stream sweep (JSON lines)")
+    ap.add_argument("--adi", action="store_true",
+                    help="NEXT row f1 / BASELINE cfg 4: three successive FUSED solves along x (periodic), "
+                         "y (Dirichlet) and z (periodic); use with --workload cfg4_adi_y")
     args = ap.parse_args()
 
     if args.impl == "reference":
@@ -290,6 +293,8 @@ def main():
 
     if args.sweep:
         return sweep(torch, tdma, w, x, args, barrier, rank)
+    if args.adi:
+        return adi(torch, tdma, w, x, args, barrier, rank, peak)
 
     # ---- candidate variants: the headline is the faster one; both are reported ---------------
     names = ["fused", "pipelined"] if args.variant == "auto" else [args.variant]
@@ -415,6 +420,47 @@ def main():
     if rank == 0:
         print(json.dumps(out))
     group.close()
+    return 0
+
+
+def adi(torch, tdma, w, x, args, barrier, rank, peak):
+    """BASELINE cfg 4: ADI implicit viscous sweeps, three batched solves per step (x and z periodic,
+    y Dirichlet with P partitions), each a FUSED plan of its own; x1 -> x2 -> x3 chained as in an
+    ADI step.  One JSON line: time per sweep and for the whole step."""
+    F = tdma.TDMA_VARIANT_FUSED
+    plans = [("x", tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=F, axis=tdma.TDMA_AXIS_X, periodic=1)),
+             ("y", tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=F)),
+             ("z", tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=F, axis=tdma.TDMA_AXIS_Z, periodic=1))]
+    y = torch.empty_like(x)
+    stream = torch.cuda.current_stream()
+    bufs = [(w.d, x), (x, y), (y, x)]
+    def step():
+        for (name, plan), (src, dst) in zip(plans, bufs):
+            plan.solve(w.a, w.b, w.c, src, dst, stream)
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    tot = [0.0, 0.0, 0.0]
+    for _ in range(args.steps):
+        ev[0].record(stream)
+        for i, ((name, plan), (src, dst)) in enumerate(zip(plans, bufs)):
+            plan.solve(w.a, w.b, w.c, src, dst, stream)
+            ev[i + 1].record(stream)
+        torch.cuda.synchronize()
+        for i in range(3):
+            tot[i] += ev[i].elapsed_time(ev[i + 1])
+    ms = [t / args.steps for t in tot]
+    rec = {"adi": True, "workload": args.workload, "nx": w.nx, "ny": w.ny, "nz": w.nz, "P": w.P,
+           "ms_x_periodic": ms[0], "ms_y": ms[1], "ms_z_periodic": ms[2], "ms_step": sum(ms),
+           "cells_per_s_step": 3 * w.cells / (sum(ms) * 1e-3),
+           "gbs_40B": {n: 40.0 * w.cells / (m * 1e-3) / 1e9 for n, m in zip("xyz", ms)},
+           "frac_of_measured_peak": {n: 40.0 * w.cells / (m * 1e-3) / 1e9 / peak for n, m in zip("xyz", ms)}}
+    if rank == 0:
+        print(json.dumps(rec))
+    for _, plan in plans:
+        plan.close()
     return 0
 
 
