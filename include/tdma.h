@@ -53,6 +53,8 @@ typedef enum tdma_status {
 /* How the three compute stages of the divide-and-conquer solve (Fig. 5) are
  * mapped onto the GPU. */
 typedef enum tdma_variant {
+    /* The fastest variant that can run the plan: FUSED (TMA kernel, one persistent launch, `batch`
+     * ignored) when the shape tiles, else PIPELINED.  This is what tdma_plan_create uses. */
     TDMA_VARIANT_AUTO = 0,
     /* Stage A (partition reduce, fused gather) / Stage B (reduced 2P-row solve) / Stage C
      * (back-substitution) as separate kernels, z-batches pipelined over CUDA streams with events

@@ -387,7 +387,20 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
                        prop.major, prop.minor);
 
     int variant = opt ? opt->variant : 0;
-    if (variant == TDMA_VARIANT_AUTO) variant = TDMA_VARIANT_PIPELINED;
+    if (variant == TDMA_VARIANT_AUTO) {
+        // the fastest path that can run this plan: the fused TMA kernel in ONE persistent launch
+        // (batch is then only a hint for the pipelined variant), else the stage pipeline
+        tdma::TmaFusedConfig probe;
+        const char *why = nullptr;
+        const bool tma_ok = pl->ny > 1 && tdma::get_encode_tiled() != nullptr &&
+                            tdma::configure_tma_fused(&probe, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
+                                                      opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
+                                                      prop, &why, pl->axis == TDMA_AXIS_X);
+        variant = (tma_ok || pl->axis == TDMA_AXIS_X || pl->periodic) ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
+        if (variant == TDMA_VARIANT_FUSED) {
+            pl->bz = pl->nz; pl->nb = 1; pl->Lb_max = (size_t)pl->nx * pl->bz;
+        }
+    }
     if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED)
         return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
     if (pl->axis == TDMA_AXIS_X && variant != TDMA_VARIANT_FUSED)
