@@ -272,10 +272,11 @@ __device__ __forceinline__ void unmerge_pair(const NodeBuf &nb, int lx, int r1, 
 // `slot` of `nslots`.  Bottom-up, heads only: on return (after its closing __syncthreads) the root
 // has its first equation in row 0 and its last equation in row 2*nodes-1.
 template <int TX>
-__device__ __forceinline__ void tree_up(const NodeBuf &nb, int lx, int slot, int nslots, int nodes)
+__device__ __forceinline__ void tree_up(const NodeBuf &nb, int lx, int slot, int nslots, int nodes,
+                                        bool synced = false)
 {
     for (int n = nodes, sp = 2; n > 1; n >>= 1, sp <<= 1) {
-        __syncthreads();
+        if (!(synced && n == nodes)) __syncthreads();   // synced: the caller has just done the first one
         for (int q = slot; q < (n >> 1); q += nslots) {
             const int rs = q * 2 * sp;
             merge_head<TX>(nb, lx, rs, rs + sp - 1, rs + sp, rs + 2 * sp - 1);
@@ -575,34 +576,38 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     const bool first_leaf = !prm.periodic && (y0 + leaf * M0 == 0);
     const bool last_leaf = !prm.periodic && (y0 + leaf * M0 + M0 == prm.ny);
 
-    auto issue_tile = [&](int tile) {   // thread 0: the whole raw tile of `tile` in flight at once
+    // The whole raw tile of `tile` in flight at once.  One copy costs its issuing thread 150-200
+    // cycles (measured), so inside the loop the four arrays are issued by lane 0 of four DIFFERENT
+    // warps -- the last four, which have no merge to do at the first tree level -- and the climb
+    // does not wait for them.  sel < 0: all arrays (prologue); sel = 0..3: array sel only.
+    auto issue_tile = [&](int tile, int sel) {
         const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
-        ptx::mbar_expect_tx(&bar[0], (unsigned)(4 * arr * sizeof(double)));
-        if (kX) {                       // one (16 x, TX lines) box per leaf; x0 = first line (y)
-            for (int w = 0; w < W; ++w) {
-                const int so = w * 16 * TX;
-                ptx::tma_load_3d(sB + so, &tm_b, y0 + 16 * w, x0, k, &bar[0]);
-                ptx::tma_load_3d(sA + so, &tm_a, y0 + 16 * w, x0, k, &bar[0]);
-                ptx::tma_load_3d(sC + so, &tm_c, y0 + 16 * w, x0, k, &bar[0]);
-                ptx::tma_load_3d(sD + so, &tm_d, y0 + 16 * w, x0, k, &bar[0]);
+        if (sel <= 0) ptx::mbar_expect_tx(&bar[0], (unsigned)(4 * arr * sizeof(double)));
+        double *const dst[4] = {sB, sA, sC, sD};
+        const CUtensorMap *const tm[4] = {&tm_b, &tm_a, &tm_c, &tm_d};
+        for (int a = 0; a < 4; ++a) {
+            if (sel >= 0 && sel != a) continue;
+            if (kX) {                   // one (16 x, TX lines) box per leaf; x0 = first line (y)
+                for (int w = 0; w < W; ++w)
+                    ptx::tma_load_3d(dst[a] + w * 16 * TX, tm[a], y0 + 16 * w, x0, k, &bar[0]);
+            } else for (int q = 0; q < prm.nbox; ++q) {
+                const int yy = y0 + q * prm.box_rows;
+                const int c1 = prm.axis_z ? k : yy, c2 = prm.axis_z ? yy : k;
+                ptx::tma_load_3d(dst[a] + q * prm.box_rows * TX, tm[a], x0, c1, c2, &bar[0]);
             }
-        } else for (int q = 0; q < prm.nbox; ++q) {
-            const int yy = y0 + q * prm.box_rows;
-            const int so = q * prm.box_rows * TX;
-            const int c1 = prm.axis_z ? k : yy, c2 = prm.axis_z ? yy : k;
-            ptx::tma_load_3d(sB + so, &tm_b, x0, c1, c2, &bar[0]);
-            ptx::tma_load_3d(sA + so, &tm_a, x0, c1, c2, &bar[0]);
-            ptx::tma_load_3d(sC + so, &tm_c, x0, c1, c2, &bar[0]);
-            ptx::tma_load_3d(sD + so, &tm_d, x0, c1, c2, &bar[0]);
         }
     };
+    const int nwarps = ((int)blockDim.x + 31) / 32;
+    // my role in the in-loop issue: -1 none, -2 everything (CTAs with fewer than 8 warps), 0..3 array
+    const int issue_sel = nwarps >= 8 ? (((t & 31) == 0 && t / 32 >= nwarps - 4) ? t / 32 - (nwarps - 4) : -1)
+                                      : (t == 0 ? -2 : -1);
 
     if (t == 0) {
         ptx::mbar_init(&bar[0], 1);
         ptx::mbar_init(&bar[1], 1);
         ptx::mbar_init(&bar[2], 1);
         ptx::fence_mbar_init();
-        issue_tile(g);
+        issue_tile(g, -1);
     }
     __syncthreads();                    // mbarriers initialised before anyone waits on them
     // split-phase cluster barrier: "every CTA of the cluster has started and initialised its
@@ -639,10 +644,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         }
         __syncthreads();                // raw tile consumed, node equations visible
         TDMA_STAMP(2);
-        if (t == 0 && tile + NC < prm.ntiles) issue_tile(tile + NC);   // prefetch behind the tree
+        if (issue_sel != -1 && tile + NC < prm.ntiles) issue_tile(tile + NC, issue_sel == -2 ? -1 : issue_sel);   // prefetch behind the tree
 
         // ---------------- pairwise tree inside the CTA, bottom-up ----------------
-        tree_up<TX>(nb, lx, leaf, W, W);
+        tree_up<TX>(nb, lx, leaf, W, W, true);
         TDMA_STAMP(3);
 
         // ---------------- cluster level ----------------
