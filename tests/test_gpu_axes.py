@@ -114,3 +114,29 @@ def test_unsupported_combinations_fail_loudly():
         tdma.Plan(32, 32, 32, 4, 0, axis=3)
     with pytest.raises(tdma.TdmaError):            # P must divide the line length (nz for a z sweep)
         tdma.Plan(32, 64, 30, 4, 0, axis=tdma.TDMA_AXIS_Z)
+
+
+@pytest.mark.parametrize("shape,opts", [
+    ((24, 1024, 1024), dict()), ((24, 1024, 1024), dict(fused_cluster=8)),
+    ((24, 1024, 1024), dict(fused_cluster=2, fused_lines=8)),
+    ((1024, 24, 1024), dict(axis=tdma.TDMA_AXIS_Z, periodic=1)), ((24, 512, 1024), dict(axis=tdma.TDMA_AXIS_X))],
+    ids=["y_cl4_fill", "y_cl8", "y_cl2_tx8", "z_periodic", "x"])
+def test_fused_tma_is_bitwise_reproducible(shape, opts):
+    """The persistent kernel hands data between threads, CTAs (DSMEM inboxes double-buffered by
+    tile parity) and launches (fill launch) with very few barriers; compute-sanitizer is closed on
+    this pool, so races are hunted the blunt way: many tiles per cluster, repeated solves, every
+    repeat must give the same bits (and a slab of the first one is checked against the oracle)."""
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 51, dev())
+    xs = []
+    with tdma.Plan(nx, ny, nz, 16, 0, variant=tdma.TDMA_VARIANT_FUSED, **opts) as plan:
+        for rep in range(8):
+            x = torch.full_like(d, float("nan"))
+            plan.solve(a, b, c, d, x)
+            xs.append(x)
+        torch.cuda.synchronize()
+    for x in xs[1:]:
+        assert torch.equal(x, xs[0])
+    axis = {0: "y", 1: "x", 2: "z"}[opts.get("axis", 0)]
+    sl = (slice(0, 2),) if axis != "z" else (slice(None), slice(0, 2))
+    check(a[sl], b[sl], c[sl], d[sl], xs[0][sl], axis, bool(opts.get("periodic", 0)))
