@@ -260,6 +260,9 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e / cpu_baseline / stage legs")
     ap.add_argument("--sweep", action="store_true", help="S7 batch x stream sweep (JSON lines)")
+    ap.add_argument("--timeline", action="store_true",
+                    help="S6 evidence without nsys: per-launch start/end of the PIPELINED stages of one solve "
+                         "(CUDA events on the plan's streams), overlap statistics as one JSON line")
     ap.add_argument("--adi", action="store_true",
                     help="NEXT row f1 / BASELINE cfg 4: three successive FUSED solves along x (periodic), "
                          "y (Dirichlet) and z (periodic); use with --workload cfg4_adi_y")
@@ -295,6 +298,8 @@ def main():
         return sweep(torch, tdma, w, x, args, barrier, rank)
     if args.adi:
         return adi(torch, tdma, w, x, args, barrier, rank, peak)
+    if args.timeline:
+        return timeline(torch, tdma, w, x, args, batch, rank)
 
     # ---- candidate variants: the headline is the faster one; both are reported ---------------
     names = ["fused", "pipelined"] if args.variant == "auto" else [args.variant]
@@ -420,6 +425,50 @@ def main():
     if rank == 0:
         print(json.dumps(out))
     group.close()
+    return 0
+
+
+def timeline(torch, tdma, w, x, args, batch, rank):
+    """Stream-overlap timeline of the PIPELINED variant (Alg. 2): how much of stage B's time runs
+    while a stage A or C kernel of another batch is running.  Plain stream launches (no graph)."""
+    ns = args.nstreams or 2
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, batch, variant=tdma.TDMA_VARIANT_PIPELINED, nstreams=ns, timeline=1) as plan:
+        for _ in range(max(3, args.warmup)):
+            plan.solve(w.a, w.b, w.c, w.d, x)
+        torch.cuda.synchronize()
+        plan.solve(w.a, w.b, w.c, w.d, x)
+        recs = plan.timeline()
+    names = {0: "A", 1: "G", 2: "B", 3: "C"}
+    t0 = min(r[2] for r in recs)
+    recs = sorted(((names[r[0]], r[1], r[2] - t0, r[3] - t0) for r in recs), key=lambda r: r[2])
+    ac = [(r[2], r[3]) for r in recs if r[0] in "AC"]
+    def covered(lo, hi):                       # length of [lo, hi] covered by the union of A/C intervals
+        tot, cur = 0.0, lo
+        for s0, s1 in sorted(ac):
+            s0, s1 = max(s0, cur), min(s1, hi)
+            if s1 > s0:
+                tot += s1 - s0
+                cur = s1
+        return tot
+    tb = sum(r[3] - r[2] for r in recs if r[0] == "B")
+    tb_hidden = sum(covered(r[2], r[3]) for r in recs if r[0] == "B")
+    span = max(r[3] for r in recs)
+    rec = {"timeline": True, "workload": args.workload, "batch": batch, "nstreams": ns, "launches": len(recs),
+           "span_ms": span, "sum_ms": {k: sum(r[3] - r[2] for r in recs if r[0] == k) for k in "ABC"},
+           "stage_b_overlapped_frac": tb_hidden / tb if tb > 0 else None,
+           "note": "events bracket each launch on its stream: an interval includes the time the kernel "
+                   "waits for SM slots, so overlapped_frac is an upper bound of true co-execution"}
+    if rank == 0:
+        print(json.dumps(rec))
+        path = os.path.join(ROOT, "gpurun_out", "timeline.txt")
+        try:
+            os.makedirs(os.path.dirname(path), exist_ok=True)
+            with open(path, "w") as f:
+                f.write("# stage batch start_ms end_ms   (first 60 launches by start time)\n")
+                for r in recs[:60]:
+                    f.write("%s %4d %9.4f %9.4f\n" % r)
+        except OSError:
+            pass
     return 0
 
 

@@ -106,7 +106,9 @@ typedef struct tdma_options {
                             row 0 through c_{n-1} (both entries are then USED).  The cyclic
                             coupling is resolved at the root of the recursion, so only the FUSED
                             TMA kernel supports it */
-    int reserved[2];
+    int timeline;        /* PIPELINED, 1 = record a timing event before and after every stage launch
+                            (forces plain stream launches); read back with tdma_plan_timeline */
+    int reserved[1];
 } tdma_options;
 
 enum { TDMA_AXIS_Y = 0, TDMA_AXIS_X = 1, TDMA_AXIS_Z = 2 };
@@ -193,6 +195,13 @@ int tdma_plan_buffer(const tdma_plan *plan, int which, int slot, void **device_p
  * PAPER.md:415), evaluates the model for all nz slices and returns the argmin in *best_batch and
  * the estimates (ms) in est_ms[0..ncand).  a, b, c, d, x: DEVICE pointers as for tdma_solve; x is
  * used as scratch.  Synchronises the device; not for use inside a timed region. */
+/* Stream-overlap timeline of the LAST tdma_solve of a plan created with options.timeline = 1
+ * (S6 evidence where nsys is not available): for launch i, rec[4i..4i+3] = stage (tdma_stage_id),
+ * batch index, start and end in ms relative to the first launch of the solve, measured with CUDA
+ * events on the stream the stage ran on.  Synchronises.  Returns the number of launches written
+ * (<= max_launches) or a negative status. */
+int tdma_plan_timeline(tdma_plan *plan, double *rec, int max_launches);
+
 double tdma_pipeline_model(int nb, double tA, double tB, double tC, int nstreams, double last_frac);
 int tdma_plan_autotune(int nx, int ny, int nz, int P, int dtype, int nstreams, const int *candidates,
                        int ncand, const void *a, const void *b, const void *c, const void *d, void *x,

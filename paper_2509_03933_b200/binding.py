@@ -30,7 +30,7 @@ TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
 EXPORTED_SYMBOLS = (
     "tdma_plan_create", "tdma_plan_create_ex", "tdma_solve", "tdma_solve_host", "tdma_stage",
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
-    "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune",
+    "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
 )
 
 
@@ -41,7 +41,7 @@ class tdma_options(ctypes.Structure):
         ("fused_lines", ctypes.c_int), ("fused_cluster", ctypes.c_int),
         ("fused_leaf_rows", ctypes.c_int), ("fused_top", ctypes.c_int),
         ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("axis", ctypes.c_int), ("periodic", ctypes.c_int),
-        ("reserved", ctypes.c_int * 2),
+        ("timeline", ctypes.c_int), ("reserved", ctypes.c_int * 1),
     ]
 
 
@@ -96,6 +96,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_last_error.restype = ctypes.c_char_p
     lib.tdma_version.argtypes = []
     lib.tdma_version.restype = ci
+    lib.tdma_plan_timeline.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ci]
+    lib.tdma_plan_timeline.restype = ci
     lib.tdma_pipeline_model.argtypes = [ci, ctypes.c_double, ctypes.c_double, ctypes.c_double, ci, ctypes.c_double]
     lib.tdma_pipeline_model.restype = ctypes.c_double
     lib.tdma_plan_autotune.argtypes = [ci] * 6 + [ctypes.POINTER(ci), ci] + [vp] * 5 + [
@@ -150,13 +152,13 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
                         variant: int = 0, nstreams: int = 0, use_graph: int = 0,
                         separate_gather: int = 0, fused_lines: int = 0, fused_cluster: int = 0,
                         fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0,
-                        axis: int = 0, periodic: int = 0) -> int:
+                        axis: int = 0, periodic: int = 0, timeline: int = 0) -> int:
     opt = tdma_options()
     opt.struct_size = ctypes.sizeof(tdma_options)
     opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
     opt.separate_gather, opt.fused_lines, opt.fused_cluster = separate_gather, fused_lines, fused_cluster
     opt.fused_leaf_rows, opt.fused_top, opt.fused_impl = fused_leaf_rows, fused_top, fused_impl
-    opt.fused_fill, opt.axis, opt.periodic = fused_fill, axis, periodic
+    opt.fused_fill, opt.axis, opt.periodic, opt.timeline = fused_fill, axis, periodic, timeline
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
         raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())
@@ -193,6 +195,15 @@ def tdma_plan_buffer(plan: int, which: int, slot: int = 0):
     p, n = ctypes.c_void_p(), ctypes.c_size_t()
     _check(load_library().tdma_plan_buffer(plan, which, slot, ctypes.byref(p), ctypes.byref(n)))
     return int(p.value), int(n.value)
+
+
+def tdma_plan_timeline(plan: int, max_launches: int = 1 << 16):
+    """[(stage, batch, start_ms, end_ms)] of the last solve of a plan created with timeline=1."""
+    buf = (ctypes.c_double * (4 * max_launches))()
+    n = int(load_library().tdma_plan_timeline(plan, buf, max_launches))
+    if n < 0:
+        raise TdmaError(n, tdma_last_error())
+    return [(int(buf[4 * i]), int(buf[4 * i + 1]), float(buf[4 * i + 2]), float(buf[4 * i + 3])) for i in range(n)]
 
 
 def tdma_pipeline_model(nb: int, tA: float, tB: float, tC: float, nstreams: int = 2,
@@ -244,6 +255,9 @@ class Plan:
 
     def stage(self, stage: int, batch_index: int, a, b, c, d, x, stream=None):
         tdma_stage(self.handle, stage, batch_index, a, b, c, d, x, stream)
+
+    def timeline(self):
+        return tdma_plan_timeline(self.handle)
 
     def get(self, what: int) -> int:
         return tdma_plan_get(self.handle, what)

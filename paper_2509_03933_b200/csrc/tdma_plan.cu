@@ -66,6 +66,9 @@ struct tdma_plan {
     int nx = 0, ny = 0, nz = 0, P = 0, m = 0, bz = 0, nb = 0;
     int variant = TDMA_VARIANT_PIPELINED, nstreams = 2, nlanes = 1, depth = 3;
     int use_graph = 1, separate_gather = 0;
+    int timeline = 0;                      // timing events around every stage launch
+    std::vector<cudaEvent_t> tl_ev;        // 2 per launch, reused across solves
+    std::vector<int> tl_tag;               // stage * 2^20 + batch, per launch of the last solve
     int device = 0;
     // Inside the plan ny is the line length (rows along the solve axis) and nz the number of slices
     // (the other axis); for a z sweep they are the caller's nz and ny.
@@ -178,13 +181,29 @@ int enqueue_pipelined(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStre
     }
     const int nb = (nz_count + pl->bz - 1) / pl->bz;
     int rc;
+    if (pl->timeline) pl->tl_tag.clear();
+    // stage launch, bracketed by timing events when the plan records a timeline
+    auto run_stage = [&](int stage, const tdma::StageParams &prm, cudaStream_t st, int batch) -> int {
+        if (!pl->timeline) return launch_stage(pl, stage, prm, st);
+        const size_t i = pl->tl_tag.size();
+        while (pl->tl_ev.size() < 2 * (i + 1)) {
+            cudaEvent_t ev = nullptr;
+            if (cudaEventCreate(&ev) != cudaSuccess) return set_err(TDMA_ERR_CUDA, "cudaEventCreate failed");
+            pl->tl_ev.push_back(ev);
+        }
+        cudaEventRecord(pl->tl_ev[2 * i], st);
+        const int r = launch_stage(pl, stage, prm, st);
+        cudaEventRecord(pl->tl_ev[2 * i + 1], st);
+        pl->tl_tag.push_back(stage * (1 << 20) + batch);
+        return r;
+    };
     if (pl->nstreams == 1) {  // Alg. 1 order: A, [A2B], B, C per batch
         for (int n = 0; n < nb; ++n) {
             const tdma::StageParams prm = batch_params(pl, ptr, nz_count, n);
-            if ((rc = launch_stage(pl, TDMA_STAGE_A, prm, origin))) return rc;
-            if (pl->separate_gather && (rc = launch_stage(pl, TDMA_STAGE_GATHER, prm, origin))) return rc;
-            if ((rc = launch_stage(pl, TDMA_STAGE_B, prm, origin))) return rc;
-            if ((rc = launch_stage(pl, TDMA_STAGE_C, prm, origin))) return rc;
+            if ((rc = run_stage(TDMA_STAGE_A, prm, origin, n))) return rc;
+            if (pl->separate_gather && (rc = run_stage(TDMA_STAGE_GATHER, prm, origin, n))) return rc;
+            if ((rc = run_stage(TDMA_STAGE_B, prm, origin, n))) return rc;
+            if ((rc = run_stage(TDMA_STAGE_C, prm, origin, n))) return rc;
         }
         return TDMA_OK;
     }
@@ -197,15 +216,15 @@ int enqueue_pipelined(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStre
             cudaStream_t st = pl->lane[n % pl->nlanes];
             if (n >= pl->depth) CUDA_TRY(cudaStreamWaitEvent(st, pl->evC[slot], 0));
             const tdma::StageParams prm = batch_params(pl, ptr, nz_count, n);
-            if ((rc = launch_stage(pl, TDMA_STAGE_A, prm, st))) return rc;
+            if ((rc = run_stage(TDMA_STAGE_A, prm, st, n))) return rc;
             CUDA_TRY(cudaEventRecord(pl->evA[slot], st));
         }
         if (n - 1 >= 0 && n - 1 < nb) {  // Stage A2B + B (n-1)
             const int q = n - 1, slot = q % pl->depth;
             const tdma::StageParams prm = batch_params(pl, ptr, nz_count, q);
             CUDA_TRY(cudaStreamWaitEvent(pl->sB, pl->evA[slot], 0));
-            if (pl->separate_gather && (rc = launch_stage(pl, TDMA_STAGE_GATHER, prm, pl->sB))) return rc;
-            if ((rc = launch_stage(pl, TDMA_STAGE_B, prm, pl->sB))) return rc;
+            if (pl->separate_gather && (rc = run_stage(TDMA_STAGE_GATHER, prm, pl->sB, q))) return rc;
+            if ((rc = run_stage(TDMA_STAGE_B, prm, pl->sB, q))) return rc;
             CUDA_TRY(cudaEventRecord(pl->evB[slot], pl->sB));
         }
         if (n - 2 >= 0 && n - 2 < nb) {  // Stage B2C + C (n-2): C reads Y in place, no scatter
@@ -213,7 +232,7 @@ int enqueue_pipelined(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStre
             cudaStream_t st = pl->lane[q % pl->nlanes];
             const tdma::StageParams prm = batch_params(pl, ptr, nz_count, q);
             CUDA_TRY(cudaStreamWaitEvent(st, pl->evB[slot], 0));
-            if ((rc = launch_stage(pl, TDMA_STAGE_C, prm, st))) return rc;
+            if ((rc = run_stage(TDMA_STAGE_C, prm, st, q))) return rc;
             CUDA_TRY(cudaEventRecord(pl->evC[slot], st));
         }
     }
@@ -359,6 +378,7 @@ void free_plan(tdma_plan *pl)
 {
     if (!pl) return;
     for (auto &g : pl->graphs) cudaGraphExecDestroy(g.exec);
+    for (auto ev : pl->tl_ev) cudaEventDestroy(ev);
     cudaFree(pl->scratch); cudaFree(pl->red); cudaFree(pl->send);
     for (int s = 0; s < 2; ++s)
         for (int i = 0; i < 5; ++i) cudaFree(pl->stage_dev[s][i]);
@@ -409,6 +429,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need the FUSED variant (TMA kernel) and >= 2 rows");
     pl->variant = variant;
     pl->use_graph = (opt && opt->use_graph < 0) ? 0 : 1;
+    pl->timeline = (opt && opt->timeline > 0) ? 1 : 0;
+    if (pl->timeline) pl->use_graph = 0;
     pl->separate_gather = (opt && opt->separate_gather > 0) ? 1 : 0;
     pl->nstreams = (opt && opt->nstreams > 0) ? opt->nstreams : 2;
     if (pl->nstreams > kMaxLanes + 1)
@@ -622,6 +644,23 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
     CUDA_TRY(cudaStreamSynchronize(pl->sD2H));
     CUDA_TRY(cudaStreamSynchronize(pl->sMain));
     return TDMA_OK;
+}
+
+int tdma_plan_timeline(tdma_plan *plan, double *rec, int max_launches)
+{
+    if (!plan || !rec || max_launches < 0) return set_err(TDMA_ERR_INVALID_ARG, "NULL argument");
+    if (!plan->timeline) return set_err(TDMA_ERR_UNSUPPORTED, "plan was not created with options.timeline = 1");
+    CUDA_TRY(cudaDeviceSynchronize());
+    const int n = std::min<int>((int)plan->tl_tag.size(), max_launches);
+    // origin = the earliest start (launch order is not time order across streams)
+    for (int i = 0; i < n; ++i) {
+        float t0 = 0, t1 = 0;
+        CUDA_TRY(cudaEventElapsedTime(&t0, plan->tl_ev[0], plan->tl_ev[2 * i]));
+        CUDA_TRY(cudaEventElapsedTime(&t1, plan->tl_ev[0], plan->tl_ev[2 * i + 1]));
+        rec[4 * i] = plan->tl_tag[i] >> 20; rec[4 * i + 1] = plan->tl_tag[i] & ((1 << 20) - 1);
+        rec[4 * i + 2] = t0; rec[4 * i + 3] = t1;
+    }
+    return n;
 }
 
 double tdma_pipeline_model(int nb, double tA, double tB, double tC, int nstreams, double last_frac)

@@ -509,3 +509,22 @@ def test_solve_on_non_default_stream_orders_with_later_work():
             y.copy_(x)                       # later work on the same stream must see x
         s.synchronize()
     assert torch.equal(y, ref)
+
+
+def test_pipeline_timeline_records_alg2_order():
+    """options.timeline: every stage launch of the last solve with start <= end, per batch
+    A before B before C (the event dependencies of Alg. 2), results unchanged."""
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    ref = gpu_solve(w.a, w.b, w.c, w.d, w.P, 8, variant=tdma.TDMA_VARIANT_PIPELINED)
+    x = torch.empty_like(w.d)
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 8, variant=tdma.TDMA_VARIANT_PIPELINED, nstreams=3, timeline=1) as plan:
+        plan.solve(w.a, w.b, w.c, w.d, x)
+        recs = plan.timeline()
+    assert torch.equal(x, ref)
+    nb = w.nz // 8
+    assert len(recs) == 3 * nb
+    by = {(s, b): (t0, t1) for s, b, t0, t1 in recs}
+    for b in range(nb):
+        A, B, C = by[(tdma.TDMA_STAGE_A, b)], by[(tdma.TDMA_STAGE_B, b)], by[(tdma.TDMA_STAGE_C, b)]
+        assert A[0] <= A[1] and B[0] <= B[1] and C[0] <= C[1]
+        assert A[1] <= B[1] + 1e-3 and B[1] <= C[1] + 1e-3
