@@ -140,3 +140,23 @@ def test_fused_tma_is_bitwise_reproducible(shape, opts):
     axis = {0: "y", 1: "x", 2: "z"}[opts.get("axis", 0)]
     sl = (slice(0, 2),) if axis != "z" else (slice(None), slice(0, 2))
     check(a[sl], b[sl], c[sl], d[sl], xs[0][sl], axis, bool(opts.get("periodic", 0)))
+
+
+def test_auto_variant_and_host_buffers_on_x_sweep():
+    """tdma_plan_create (variant AUTO) resolves to FUSED when the shape tiles and to PIPELINED when
+    it does not; tdma_solve_host works for x sweeps (z-chunks are contiguous) and refuses z sweeps."""
+    with tdma.Plan(64, 64, 8, 4, 2) as plan:
+        assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_FUSED
+        assert plan.get(tdma.TDMA_GET_NB) == 1          # batch is a hint for the pipelined variant only
+    with tdma.Plan(45, 30, 8, 5, 2) as plan:            # odd nx, m = 6: no power-of-two tree
+        assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_PIPELINED
+        assert plan.get(tdma.TDMA_GET_NB) == 4
+    a, b, c, d = tdma_inputs.dominant_random(128, 24, 6, 61, "cpu")
+    host = [t.pin_memory() for t in (a, b, c, d)]
+    xh = torch.empty_like(d).pin_memory()
+    with tdma.Plan(128, 24, 6, 2, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X, periodic=1) as plan:
+        plan.solve_host(*host, xh)
+    check(a, b, c, d, xh, "x", True)
+    with tdma.Plan(32, 24, 16, 2, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_Z) as plan:
+        with pytest.raises(tdma.TdmaError):
+            plan.solve_host(*[torch.zeros(16, 24, 32, dtype=torch.float64) for _ in range(5)])
