@@ -595,8 +595,8 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
     if (pl->axis == TDMA_AXIS_Z)
         return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_host streams z-chunks: x and y sweeps only");
     if (!pl->sH2D) {  // first use: staging buffers, copy streams
-        // chunk = whole batches, about 64 Mi cells (512 MiB per array) or the slab if smaller
-        const size_t target = (size_t)1 << 26;
+        // chunk = whole batches, about 16 Mi cells (128 MiB per array) or the slab if smaller
+        const size_t target = (size_t)1 << 24;
         long long hz = (long long)std::max<size_t>(1, target / pl->slice);
         hz = std::max<long long>(pl->bz, hz / pl->bz * pl->bz);
         pl->hz = (int)std::min<long long>(hz, pl->nz);
