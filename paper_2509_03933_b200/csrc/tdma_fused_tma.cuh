@@ -741,7 +741,7 @@ inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 // level is the paper's partition level), the tile fits shared memory.
 inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int want_lines,
                                 int want_cluster, int want_leaf, const cudaDeviceProp &prop,
-                                const char **why, bool xaxis = false)
+                                const char **why, bool xaxis = false, bool zaxis = false)
 {
     // x sweep: nx = number of lanes (caller's ny), ny = line length (caller's nx)
     if (xaxis) {
@@ -801,7 +801,11 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
                 // long run and DRAM row-buffer locality between neighbouring x tiles is lost
                 // (measured: 4.4 -> 3.1 TB/s from 256 to 1024 slices at TX = 8, flat at TX = 16)
                 double score = 10000.0 * m0 + cells + (c.threads >= 32 ? 4000.0 : 0.0) + (ctas >= 2 ? 100.0 : 0.0) -
-                               50.0 * CL + (TX == 16 ? 3000.0 : (TX == 32 ? 1000.0 : 0.0));
+                               50.0 * CL +
+                               // z sweeps: rows of a line are whole slices apart (a DRAM page and a
+                               // TLB entry per row), 256 B segments pay (0.99 -> 0.91 ms on cfg 4)
+                               (zaxis ? (TX == 32 ? 3000.0 : (TX == 16 ? 1000.0 : 0.0))
+                                      : (TX == 16 ? 3000.0 : (TX == 32 ? 1000.0 : 0.0)));
                 if (score > best_score) { best_score = score; best = c; }
             }
         }

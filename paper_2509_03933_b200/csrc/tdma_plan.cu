@@ -415,7 +415,7 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         const bool tma_ok = pl->ny > 1 && tdma::get_encode_tiled() != nullptr &&
                             tdma::configure_tma_fused(&probe, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
                                                       opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
-                                                      prop, &why, pl->axis == TDMA_AXIS_X);
+                                                      prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z);
         variant = (tma_ok || pl->axis == TDMA_AXIS_X || pl->periodic) ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
         if (variant == TDMA_VARIANT_FUSED) {
             pl->bz = pl->nz; pl->nb = 1; pl->Lb_max = (size_t)pl->nx * pl->bz;
@@ -483,7 +483,7 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
             have_tma = tdma::get_encode_tiled() != nullptr &&
                        tdma::configure_tma_fused(&pl->tfused, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
                                                  opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
-                                                 prop, &why, pl->axis == TDMA_AXIS_X);
+                                                 prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z);
             if (!have_tma && want_impl == 2)
                 return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel unavailable: %s",
                                why ? why : "cuTensorMapEncodeTiled not found");
@@ -508,7 +508,7 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
             const char *why2 = nullptr;
             pl->have_fill = tdma::configure_tma_fused(&pl->tfill, pl->nx, pl->ny, pl->P, 0,
                                                       pl->ny % 2 == 0 ? 2 : 1, 0, prop, &why2,
-                                                      pl->axis == TDMA_AXIS_X);
+                                                      pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z);
         }
     }
     return TDMA_OK;
