@@ -108,7 +108,8 @@ typedef struct tdma_options {
                             TMA kernel supports it */
     int timeline;        /* PIPELINED, 1 = record a timing event before and after every stage launch
                             (forces plain stream launches); read back with tdma_plan_timeline */
-    int reserved[1];
+    int host_chunk;      /* tdma_solve_host: z-slices per host chunk (0 = auto, about 16 Mi cells;
+                            PIPELINED plans round it to whole batches) */
 } tdma_options;
 
 enum { TDMA_AXIS_Y = 0, TDMA_AXIS_X = 1, TDMA_AXIS_Z = 2 };

@@ -11,6 +11,7 @@ from __future__ import annotations
 
 import ctypes
 import os
+import sys
 from typing import Optional
 
 from . import build as _build
@@ -41,7 +42,7 @@ class tdma_options(ctypes.Structure):
         ("fused_lines", ctypes.c_int), ("fused_cluster", ctypes.c_int),
         ("fused_leaf_rows", ctypes.c_int), ("fused_top", ctypes.c_int),
         ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("axis", ctypes.c_int), ("periodic", ctypes.c_int),
-        ("timeline", ctypes.c_int), ("reserved", ctypes.c_int * 1),
+        ("timeline", ctypes.c_int), ("host_chunk", ctypes.c_int),
     ]
 
 
@@ -67,9 +68,12 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     if build_if_missing:
         try:
             path = _build.build()
-        except Exception as exc:            # stale-but-present library is still usable
+        except Exception as exc:
             if not os.path.exists(path):
                 raise RuntimeError("libtdma.so is missing and could not be built: %s" % exc)
+            # never silent: the library on disk is older than the sources
+            sys.stderr.write("paper_2509_03933_b200: WARNING: rebuilding libtdma.so failed (%s); "
+                             "loading the STALE library at %s\n" % (str(exc).splitlines()[0], path))
     if not os.path.exists(path):
         raise RuntimeError("libtdma.so not found at %s (run __graft_entry__.build())" % path)
     lib = ctypes.CDLL(path)
@@ -152,13 +156,14 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
                         variant: int = 0, nstreams: int = 0, use_graph: int = 0,
                         separate_gather: int = 0, fused_lines: int = 0, fused_cluster: int = 0,
                         fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0,
-                        axis: int = 0, periodic: int = 0, timeline: int = 0) -> int:
+                        axis: int = 0, periodic: int = 0, timeline: int = 0, host_chunk: int = 0) -> int:
     opt = tdma_options()
     opt.struct_size = ctypes.sizeof(tdma_options)
     opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
     opt.separate_gather, opt.fused_lines, opt.fused_cluster = separate_gather, fused_lines, fused_cluster
     opt.fused_leaf_rows, opt.fused_top, opt.fused_impl = fused_leaf_rows, fused_top, fused_impl
     opt.fused_fill, opt.axis, opt.periodic, opt.timeline = fused_fill, axis, periodic, timeline
+    opt.host_chunk = host_chunk
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
         raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())

@@ -119,6 +119,9 @@ __global__ void __launch_bounds__(MAXT, MINB) fused_kernel(const FusedParams prm
     const int grow0 = (int)crank * R + r0;                  // ... and global row
     const size_t off0 = ((size_t)k * prm.ny + grow0) * (size_t)nx + gx;
     const unsigned s = (unsigned)nx;
+    // split-phase cluster barrier: every CTA of the cluster must have started before the first
+    // distributed-shared-memory store; the matching wait sits right before the A2B loop
+    if (kCluster) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
 
     // ---------------- leaves: modified Thomas reduction straight from HBM ----------------
     {
@@ -225,6 +228,7 @@ __global__ void __launch_bounds__(MAXT, MINB) fused_kernel(const FusedParams prm
 
     // ---------------- A2B: top-level equations -> smem of the CTA that solves the line ------
     __syncthreads();
+    if (kCluster) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
     {
         const size_t plane = (size_t)NTR * TXS;
         for (int e = t; e < ntr_cta * TX; e += blockDim.x) {

@@ -78,9 +78,6 @@ struct TmaFusedParams {
     int CL, R, W;
     int xtiles, ntiles;
     int box_rows, nbox;
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-    long long *dbg;                     // experiment: per-CTA phase time stamps [grid][16]
-#endif
 };
 
 __host__ __device__ inline size_t tma_fused_smem_bytes(int TX, int R, int W, int CL, bool xaxis = false)
@@ -535,12 +532,6 @@ __device__ __forceinline__ void leaf_back_x(const LeafRegs<16> &R, double xf, do
     for (int p = 0; p < 8; ++p) sts2(xs_addr(bX, l, p), xs[2 * p], xs[2 * p + 1]);
 }
 
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-#define TDMA_STAMP(i) do { if (threadIdx.x == 0 && it == 1) prm.dbg[(size_t)blockIdx.x * 16 + (i)] = clock64(); } while (0)
-#else
-#define TDMA_STAMP(i) do { } while (0)
-#endif
-
 // kX: x sweep (lanes = TX lines along y, rows = x; M0 = 16 only); tm_x is used by x sweeps only.
 template <int TX, int M0, bool kCluster, int MAXT, int MINB, bool kX>
 __global__ void __launch_bounds__(MAXT, MINB)
@@ -623,9 +614,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         // arm this tile's inbox: 4 doubles per (node equation, line) from every CTA
         if (kCluster && t == 0) ptx::mbar_expect_tx(&bar[1 + par], (unsigned)(4 * tarr * sizeof(double)));
         if (kX && t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-        TDMA_STAMP(0);
         ptx::mbar_wait(&bar[0], (unsigned)par);
-        TDMA_STAMP(1);
 
         // ---------------- leaves ----------------
         LeafRegs<M0> regs;
@@ -643,12 +632,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             sts2(ol, l.a, l.b); sts2(ol + nb.plane, l.c, l.d);
         }
         __syncthreads();                // raw tile consumed, node equations visible
-        TDMA_STAMP(2);
         if (issue_sel != -1 && tile + NC < prm.ntiles) issue_tile(tile + NC, issue_sel == -2 ? -1 : issue_sel);   // prefetch behind the tree
 
         // ---------------- pairwise tree inside the CTA, bottom-up ----------------
         tree_up<TX>(nb, lx, leaf, W, W, true);
-        TDMA_STAMP(3);
 
         // ---------------- cluster level ----------------
         // the CTA's node: first equation in node row 0, last equation in node row 2W-1
@@ -671,11 +658,9 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                 ptx::st_async_2f64(dst, ab.x, ab.y, dbar);
                 ptx::st_async_2f64(dst + tb.plane, cd.x, cd.y, dbar);
             }
-            TDMA_STAMP(4);
             // the reciprocals of the tree just climbed run behind the exchange
             tree_tails<TX>(nb, lx, leaf, W, W);
             ptx::mbar_wait(&bar[1 + par], (unsigned)((it >> 1) & 1));
-            TDMA_STAMP(5);
             // Stage B: the 2*CL-row system, solved redundantly by every CTA with the same
             // pairwise tree, so no second exchange is needed
             tree_up<TX>(tb, lx, leaf, W, CL);
@@ -691,11 +676,9 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             }
             __syncthreads();
         }
-        TDMA_STAMP(6);
 
         // ---------------- pairwise tree inside the CTA, top-down ----------------
         tree_down<TX>(nb, lx, leaf, W, W);
-        TDMA_STAMP(7);
 
         // ---------------- leaves: back-substitution from registers, x streamed to HBM --------
         {
@@ -719,13 +702,6 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                                   (size_t)(x0 + lx), (size_t)prm.rs);
             }
         }
-        TDMA_STAMP(8);
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-        if (t == 0 && it == 1) {
-            unsigned smid; asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-            prm.dbg[(size_t)blockIdx.x * 16 + 12] = smid;
-        }
-#endif
     }
     // the staging tile must outlive the last TMA store
     if (kX && t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
@@ -878,9 +854,6 @@ inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, c
 {
     auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, MINB, kX>;
     size_t smem_bytes = cfg.smem;
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-    if (const char *pad = getenv("TDMA_PAD")) smem_bytes += (size_t)atoi(pad);   // experiment: fewer CTAs per SM
-#endif
     cudaLaunchConfig_t lc = {};
     lc.blockDim = dim3(cfg.threads);
     lc.dynamicSmemBytes = smem_bytes;
@@ -964,13 +937,6 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
     prm.xtiles = (nx + cfg.lines - 1) / cfg.lines;
     prm.ntiles = prm.xtiles * nzs;
     prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-    {
-        extern long long *g_tdma_dbg;
-        if (!g_tdma_dbg) cudaMalloc(&g_tdma_dbg, (size_t)1 << 28);
-        prm.dbg = g_tdma_dbg;
-    }
-#endif
     const bool cl = cfg.cluster > 1;
     if (cfg.xaxis)
         return cl ? launch_tma_inst<16, 16, true, 256, 1, true>(cfg, tm, prm, st)

@@ -12,11 +12,6 @@
 #include <new>
 #include <vector>
 
-#if defined(TDMA_DBG_MODE) && TDMA_DBG_MODE == 2
-namespace tdma { long long *g_tdma_dbg = nullptr; }
-extern "C" void *tdma_dbg_buffer(void) { return tdma::g_tdma_dbg; }
-#endif
-
 #include "tdma_stage_kernels.cuh"
 #include "tdma_fused.cuh"
 #include "tdma_fused_tma.cuh"
@@ -97,6 +92,7 @@ struct tdma_plan {
     size_t sm_smem = 0;
     // host staging (tdma_solve_host), allocated on first use
     int hz = 0;  // slices per host chunk
+    int host_chunk = 0;  // options.host_chunk (0 = auto)
     double *stage_dev[2][5] = {};
     cudaStream_t sH2D = nullptr, sD2H = nullptr;
     cudaEvent_t evH2D[2] = {}, evDone[2] = {}, evD2H[2] = {};
@@ -297,8 +293,10 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
                 const size_t offf = off + (size_t)(bzn - nzf) * (size_t)pl->os;
                 e = tdma::launch_tma_fused(pl->tfill, ptr.a + offf, ptr.b + offf, ptr.c + offf, ptr.d + offf,
                                            ptr.x + offf, pl->nx, pl->ny, nzf, pl->rs, pl->os, az, per, pl->sB);
-                CUDA_TRY(cudaEventRecord(pl->evBJoin, pl->sB));
-                CUDA_TRY(cudaStreamWaitEvent(origin, pl->evBJoin, 0));
+                // join even when the fill launch failed: `origin` must not be left forked
+                cudaError_t ej = cudaEventRecord(pl->evBJoin, pl->sB);
+                if (ej == cudaSuccess) ej = cudaStreamWaitEvent(origin, pl->evBJoin, 0);
+                if (e == cudaSuccess) e = ej;
             }
         } else if (pl->fused.threads > 0 && plain_y)
             e = tdma::launch_fused(pl->fused, ptr.a + off, ptr.b + off, ptr.c + off,
@@ -519,6 +517,11 @@ int check_ptrs(const tdma_plan *plan, const void *a, const void *b, const void *
 {
     if (!plan) return set_err(TDMA_ERR_INVALID_ARG, "plan is NULL");
     if (!a || !b || !c || !d || !x) return set_err(TDMA_ERR_INVALID_ARG, "NULL array pointer");
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != plan->device)
+        return set_err(TDMA_ERR_INVALID_ARG, "plan was created on device %d, the current device is %d",
+                       plan->device, dev);
     return TDMA_OK;
 }
 
@@ -530,6 +533,7 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
                                const tdma_options *options)
 {
     g_err[0] = 0;
+    if (options && options->struct_size != (int)sizeof(tdma_options)) { set_err(TDMA_ERR_INVALID_ARG, "tdma_options.struct_size = %d, expected %zu", options->struct_size, sizeof(tdma_options)); return nullptr; }
     const int axis = options ? options->axis : TDMA_AXIS_Y, periodic = options && options->periodic ? 1 : 0;
     if (axis != TDMA_AXIS_Y && axis != TDMA_AXIS_Z && axis != TDMA_AXIS_X) { set_err(TDMA_ERR_INVALID_ARG, "unknown axis %d", axis); return nullptr; }
     if (axis == TDMA_AXIS_Z) std::swap(ny, nz);   // from here on: ny = line length, nz = slices,
@@ -540,12 +544,13 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     if (P > 1 && ny / P < 2) { set_err(TDMA_ERR_INVALID_ARG, "partitions need >= 2 rows (ny/P = %d)", ny / P); return nullptr; }
     if (batch < 0 || batch > nz) { set_err(TDMA_ERR_INVALID_ARG, "batch = %d outside [0, nz = %d]", batch, nz); return nullptr; }
     if (dtype != TDMA_F64) { set_err(TDMA_ERR_UNSUPPORTED, "dtype %d: only TDMA_F64 is implemented", dtype); return nullptr; }
-    if (options && options->struct_size != (int)sizeof(tdma_options)) { set_err(TDMA_ERR_INVALID_ARG, "tdma_options.struct_size = %d, expected %zu", options->struct_size, sizeof(tdma_options)); return nullptr; }
+    if (options && options->host_chunk < 0) { set_err(TDMA_ERR_INVALID_ARG, "host_chunk = %d must be >= 0", options->host_chunk); return nullptr; }
     if ((long long)nx * (batch ? batch : nz) > 0x7fffffffLL) { set_err(TDMA_ERR_UNSUPPORTED, "nx * batch exceeds 2^31-1 lines per batch"); return nullptr; }
     tdma_plan *pl = new (std::nothrow) tdma_plan();
     if (!pl) { set_err(TDMA_ERR_ALLOC, "out of host memory"); return nullptr; }
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->P = P; pl->m = ny / P;   // ny, nz already mapped
     pl->axis = axis; pl->periodic = periodic;
+    pl->host_chunk = options ? options->host_chunk : 0;
     pl->rs = axis == TDMA_AXIS_Z ? (long long)nx * nz : (long long)nx;   // z sweep: plan nz = caller ny
     pl->os = axis == TDMA_AXIS_Z ? (long long)nx : (long long)nx * ny;   // x sweep: slices are z-slices
     pl->bz = batch == 0 ? nz : batch;
@@ -595,10 +600,12 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
     if (pl->axis == TDMA_AXIS_Z)
         return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_host streams z-chunks: x and y sweeps only");
     if (!pl->sH2D) {  // first use: staging buffers, copy streams
-        // chunk = whole batches, about 16 Mi cells (128 MiB per array) or the slab if smaller
+        // chunk = about 16 Mi cells (128 MiB per array), or options.host_chunk slices.  PIPELINED:
+        // rounded to whole batches so that the batch boundaries (and with them the bits of x) are
+        // those of tdma_solve; FUSED: `batch` only chunks launches, so the target alone decides.
         const size_t target = (size_t)1 << 24;
-        long long hz = (long long)std::max<size_t>(1, target / pl->slice);
-        hz = std::max<long long>(pl->bz, hz / pl->bz * pl->bz);
+        long long hz = pl->host_chunk > 0 ? pl->host_chunk : (long long)std::max<size_t>(1, target / pl->slice);
+        if (pl->variant == TDMA_VARIANT_PIPELINED) hz = std::max<long long>(pl->bz, hz / pl->bz * pl->bz);
         pl->hz = (int)std::min<long long>(hz, pl->nz);
         const size_t bytes = (size_t)pl->hz * pl->slice * sizeof(double);
         for (int s = 0; s < 2; ++s)

@@ -101,6 +101,31 @@ def test_cfg4_adi_three_sweeps():
     check(w.a, w.b, w.c, x2, x3, "z", True)
 
 
+def test_cfg4_adi_full_size_three_sweeps_sampled():
+    """BASELINE cfg 4 at FULL size (512^3, P = 8) in the plans `bench.py --adi` times (FUSED, auto
+    tiling, batch = 0): x periodic -> y Dirichlet -> z periodic, every
+    sweep against oracle.solve_axis on sampled z-slices (x, y sweeps) / y-planes (z sweep),
+    including the slices a fill launch wrote."""
+    w = tdma_inputs.make_workload("cfg4_adi_y", device=dev())
+    F = tdma.TDMA_VARIANT_FUSED
+    src = w.d
+    for axis, name, periodic in ((tdma.TDMA_AXIS_X, "x", 1), (tdma.TDMA_AXIS_Y, "y", 0), (tdma.TDMA_AXIS_Z, "z", 1)):
+        dst = torch.full_like(w.d, float("nan"))
+        with tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=F, axis=axis, periodic=periodic) as plan:
+            plan.solve(w.a, w.b, w.c, src, dst)
+            torch.cuda.synchronize()
+            fill = plan.get(tdma.TDMA_GET_FUSED_FILL)
+        assert bool(torch.isfinite(dst).all())
+        nsl = w.ny if name == "z" else w.nz
+        picks = {0, 1, nsl // 2 + 1, nsl - 1}
+        if fill > 0:
+            picks |= {nsl - fill, nsl - fill - 1}
+        for q in sorted(picks):
+            sl = (slice(None), slice(q, q + 1)) if name == "z" else (slice(q, q + 1),)
+            check(w.a[sl], w.b[sl], w.c[sl], src[sl], dst[sl], name, bool(periodic))
+        src = dst
+
+
 def test_unsupported_combinations_fail_loudly():
     with pytest.raises(tdma.TdmaError):
         tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1)
@@ -135,11 +160,15 @@ def test_fused_tma_is_bitwise_reproducible(shape, opts):
             plan.solve(a, b, c, d, x)
             xs.append(x)
         torch.cuda.synchronize()
+        fill = plan.get(tdma.TDMA_GET_FUSED_FILL)
     for x in xs[1:]:
         assert torch.equal(x, xs[0])
     axis = {0: "y", 1: "x", 2: "z"}[opts.get("axis", 0)]
-    sl = (slice(0, 2),) if axis != "z" else (slice(None), slice(0, 2))
-    check(a[sl], b[sl], c[sl], d[sl], xs[0][sl], axis, bool(opts.get("periodic", 0)))
+    nsl = nz if axis != "z" else ny                  # slices of the plan (z for x / y sweeps, y for z sweeps)
+    ranges = [(0, 2)] + ([(nsl - fill, nsl)] if fill > 0 else [(nsl - 2, nsl)])   # + what the fill launch wrote
+    for lo, hi in ranges:
+        sl = (slice(lo, hi),) if axis != "z" else (slice(None), slice(lo, hi))
+        check(a[sl], b[sl], c[sl], d[sl], xs[0][sl], axis, bool(opts.get("periodic", 0)))
 
 
 def test_auto_variant_and_host_buffers_on_x_sweep():

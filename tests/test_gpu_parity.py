@@ -114,23 +114,33 @@ def test_cfg3_weak_slab(variant):
 # Full-size runs in the launch configuration bench.py times, sampled slices
 # ---------------------------------------------------------------------------------------------
 def _sampled_full(name, variant, batch, slices, strictly, **opts):
+    """Full-size slab through one plan; `slices` are checked against the oracle one by one.  For
+    FUSED plans that use a fill launch (clusters of 2 on the SMs the main launch leaves empty) the
+    first, middle and last slice of the fill range are added, so both tilings are covered."""
     free, _ = torch.cuda.mem_get_info()
     spec = tdma_inputs.config_spec(name)
     need = spec["nx"] * spec["ny"] * spec["nz"] * 8 * 5 * 1.25
     if free < need:
         pytest.skip("needs %.0f GB of device memory" % (need / 1e9))
     w = tdma_inputs.make_workload(name, device=dev())
-    x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, **variant, **opts)
+    x = torch.full_like(w.d, float("nan"))
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, batch, **variant, **opts) as plan:
+        plan.solve(w.a, w.b, w.c, w.d, x)
+        torch.cuda.synchronize()
+        fill = plan.get(tdma.TDMA_GET_FUSED_FILL) if variant["variant"] == tdma.TDMA_VARIANT_FUSED else 0
+        launches = plan.get(tdma.TDMA_GET_LAUNCHES)
     assert bool(torch.isfinite(x).all())
+    slices = list(slices)
+    if fill > 0:
+        slices += [w.nz - fill, w.nz - fill // 2 - 1, w.nz - 1]
+        slices += [w.nz - fill - 1]                       # last slice of the main launch
     worst = 0.0
-    for k in slices:
+    for k in sorted(set(slices)):
         sl = slice(k, k + 1)
         worst = max(worst, check_against_oracle(w.a[sl], w.b[sl], w.c[sl], w.d[sl], x[sl], strictly))
-    # a property that holds at any size: for the Poisson lines away from the pinned mode the
-    # column sums of A vanish except for -k^2, so sum_j d_j = -(kx^2+kz^2) sum_j x_j  (Neumann)
     del w, x
     torch.cuda.empty_cache()
-    return worst
+    return worst, fill, launches
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -141,6 +151,16 @@ def test_cfg3_full_size_sampled(variant):
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_cfg5_full_size_sampled(variant):
     _sampled_full("cfg5_stress", variant, 16, [0, 777, 1023], True, nstreams=3)
+
+
+@pytest.mark.parametrize("name,slices,strictly", [("cfg3_weak", [0, 1, 2, 257, 513, 900], False),
+                                                  ("cfg5_stress", [0, 1, 300, 777], True)])
+def test_full_size_in_the_bench_launch_configuration(name, slices, strictly):
+    """Exactly what bench.py times: FUSED, batch = 0, i.e. ONE persistent launch over the slab
+    (~1900 tiles per cluster on cfg 3) plus, where clusters of 4 leave SMs empty, the concurrent
+    fill launch; slices of both ranges against the oracle."""
+    worst, fill, launches = _sampled_full(name, dict(variant=tdma.TDMA_VARIANT_FUSED), 0, slices, strictly)
+    assert launches == (2 if fill > 0 else 1)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -528,3 +548,46 @@ def test_pipeline_timeline_records_alg2_order():
         A, B, C = by[(tdma.TDMA_STAGE_A, b)], by[(tdma.TDMA_STAGE_B, b)], by[(tdma.TDMA_STAGE_C, b)]
         assert A[0] <= A[1] and B[0] <= B[1] and C[0] <= C[1]
         assert A[1] <= B[1] + 1e-3 and B[1] <= C[1] + 1e-3
+
+
+def test_fill_launch_changes_x_only_within_rounding():
+    """G13 scoped: the fill launch solves its slices with another tiling (clusters of 2,
+    8 lines), so the BITS of x in the fill range depend on where that range starts; the values
+    agree with the no-fill solve and with the oracle to the tolerance."""
+    w = tdma_inputs.make_workload("cfg3_weak", device=dev(), nz=48)
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED) as plan:
+        x_auto = torch.full_like(w.d, float("nan"))
+        plan.solve(w.a, w.b, w.c, w.d, x_auto)
+        torch.cuda.synchronize()
+        fill = plan.get(tdma.TDMA_GET_FUSED_FILL)
+    x_off = gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_fill=-1)
+    x_big = gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_fill=500)
+    if fill > 0:
+        assert torch.equal(x_auto[:w.nz - fill], x_off[:w.nz - fill])      # main range: same tiling, same bits
+    for x in (x_auto, x_off, x_big):
+        check_against_oracle(w.a, w.b, w.c, w.d, x, False)
+    E = oracle.normwise_error(x_auto.cpu().numpy(), x_off.cpu().numpy())
+    assert E.max() <= TOL_E
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("chunk", [3, 16])
+def test_solve_host_streams_several_chunks(variant, chunk):
+    """tdma_solve_host with >= 3 chunks and a ragged last one (40 = 3*13 + 1 / 16+16+8): the
+    double-buffered staging ring (slot reuse waits on solve + D2H of chunk q-2) and the second
+    graph of the ragged chunk are exercised; PIPELINED rounds the chunk to whole batches, so its
+    bits equal tdma_solve's."""
+    w = tdma_inputs.make_workload("cfg2_poisson", device="cpu", nx=64, nz=40)
+    host = [t.pin_memory() for t in (w.a, w.b, w.c, w.d)]
+    xh = torch.full_like(w.d, float("nan")).pin_memory()
+    batch = 4
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, batch, host_chunk=chunk, **variant) as plan:
+        plan.solve_host(*host, xh)
+        xh2 = torch.full_like(w.d, float("nan")).pin_memory()
+        plan.solve_host(*host, xh2)                  # staging buffers and graphs reused
+        xd = torch.empty_like(w.d, device=dev())
+        plan.solve(*[t.to(dev()) for t in host], xd)
+        torch.cuda.synchronize()
+    assert torch.equal(xh, xh2)
+    assert torch.equal(xh, xd.cpu())                 # no fill launch at this size: same tiling per slice
+    check_against_oracle(w.a, w.b, w.c, w.d, xh, False)
