@@ -108,6 +108,10 @@ typedef struct tdma_options {
                             TMA kernel supports it */
     int timeline;        /* PIPELINED, 1 = record a timing event before and after every stage launch
                             (forces plain stream launches); read back with tdma_plan_timeline */
+    int fused_slots;     /* FUSED, TMA kernel: ring slots of one raw array tile each: 4 = the next tile is
+                            fetched after the sweep of this one, 5 .. 8 = that many minus 4 arrays of the
+                            next tile stay in flight during the sweep; 0 = auto (as many as shared
+                            memory holds, at most 8) */
     int host_chunk;      /* tdma_solve_host: z-slices per host chunk (0 = auto, about 16 Mi cells;
                             PIPELINED plans round it to whole batches) */
 } tdma_options;

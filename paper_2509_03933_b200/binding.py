@@ -42,7 +42,7 @@ class tdma_options(ctypes.Structure):
         ("fused_lines", ctypes.c_int), ("fused_cluster", ctypes.c_int),
         ("fused_leaf_rows", ctypes.c_int), ("fused_top", ctypes.c_int),
         ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("axis", ctypes.c_int), ("periodic", ctypes.c_int),
-        ("timeline", ctypes.c_int), ("host_chunk", ctypes.c_int),
+        ("timeline", ctypes.c_int), ("fused_slots", ctypes.c_int), ("host_chunk", ctypes.c_int),
     ]
 
 
@@ -156,14 +156,14 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
                         variant: int = 0, nstreams: int = 0, use_graph: int = 0,
                         separate_gather: int = 0, fused_lines: int = 0, fused_cluster: int = 0,
                         fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0,
-                        axis: int = 0, periodic: int = 0, timeline: int = 0, host_chunk: int = 0) -> int:
+                        axis: int = 0, periodic: int = 0, timeline: int = 0, fused_slots: int = 0, host_chunk: int = 0) -> int:
     opt = tdma_options()
     opt.struct_size = ctypes.sizeof(tdma_options)
     opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
     opt.separate_gather, opt.fused_lines, opt.fused_cluster = separate_gather, fused_lines, fused_cluster
     opt.fused_leaf_rows, opt.fused_top, opt.fused_impl = fused_leaf_rows, fused_top, fused_impl
     opt.fused_fill, opt.axis, opt.periodic, opt.timeline = fused_fill, axis, periodic, timeline
-    opt.host_chunk = host_chunk
+    opt.host_chunk, opt.fused_slots = host_chunk, fused_slots
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
         raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())

@@ -61,8 +61,9 @@ struct TmaFusedConfig {
     int leaf_rows = 0;  // m0 (2, 4, 8 or 16)
     int leaves = 0;     // W = R / m0 (power of two)
     int nlev = 0;       // log2 W
-    int threads = 0;    // W * TX
+    int threads = 0;    // W * TX (the launch adds idle lanes up to a whole warp)
     int box_rows = 0;   // rows per TMA box (<= 256), divides R
+    int slots = 0;      // NA: ring slots of one raw array each (4 = single-buffered tile ... 8 = two tiles)
     int max_clusters = 0;  // co-resident clusters (persistent grid size), filled at first launch
     bool xaxis = false;    // x sweep: 16-row leaves, swizzled boxes, staging tile for x
     size_t smem = 0;
@@ -75,18 +76,21 @@ struct TmaFusedParams {
     int axis_z;         // 0: rows = tensor dim 1, slices = dim 2;  1: rows = dim 2, slices = dim 1
     int periodic;       // cyclic lines: x_{-1} = x_{n-1}, x_n = x_0 (a_0, c_{n-1} are used)
     int nx, ny, nzs;    // ny = rows per line, nzs = slices in this launch
-    int CL, R, W;
+    int CL, R, W, NS;
     int xtiles, ntiles;
     int box_rows, nbox;
 };
 
-__host__ __device__ inline size_t tma_fused_smem_bytes(int TX, int R, int W, int CL, bool xaxis = false)
+// Dynamic shared memory of one CTA: NA ring slots of one raw array [R][TX] each, the x staging
+// tile [R][TX], node buffer (2 planes of [2W][TX] 16-byte pairs), two inboxes of the
+// cluster-level system (2 planes of [2 CL][TX] pairs each), NA + 2 mbarriers.
+__host__ __device__ inline size_t tma_fused_smem_bytes(int TX, int R, int W, int CL, int NA, bool xaxis = false)
 {
-    if (xaxis)   // + staging tile [R][TX] for x
-        return ((size_t)5 * R * TX + (size_t)4 * 2 * W * TX + (size_t)2 * 4 * 2 * CL * TX) * sizeof(double) + 128;
-    // raw tile: 4 arrays [R][TX]; node buffer 4 x [2 W][TX]; cluster-level system, two inboxes of
-    // 4 x [2 CL][TX]; three mbarriers (+ padding)
-    return ((size_t)4 * R * TX + (size_t)4 * 2 * W * TX + (size_t)2 * 4 * 2 * CL * TX) * sizeof(double) + 128;
+    (void)xaxis;
+    const size_t raw = ((size_t)NA + 1) * R * TX * sizeof(double);
+    const size_t node = (size_t)2 * 2 * W * TX * 16;
+    const size_t inbox = CL > 1 ? (size_t)2 * 2 * 2 * CL * TX * 16 : 0;
+    return raw + node + inbox + 128;
 }
 
 namespace ptx {
@@ -211,102 +215,211 @@ struct Eq { double a, b, c, d; };
 
 // Node buffer: `rows` equations x TX lines, stored as two planes of 16-byte pairs,
 //   AB[row][line] = (A, B)   and   CD[row][line] = (C, D),   CD plane `plane` bytes after AB.
-// An eliminated row keeps (a, c) in its AB slot and d (later x) in the D half of its CD slot.
+// The lanes of a warp work on consecutive lines of the same row: conflict-free.  A row the tree
+// eliminated keeps (a, c) in its AB slot and d (later x) in the D half of its CD slot.
 struct NodeBuf { uint32_t ab, plane; };
 
 template <int TX>
 __device__ __forceinline__ uint32_t nb_ab(const NodeBuf &nb, int row, int lx) { return nb.ab + (uint32_t)(row * TX + lx) * 16u; }
 
-// Pairwise merge, first half (see the header): rows r1 < r2 < r3 < r4 hold L.first, L.last,
-// R.first, R.last; r1 / r4 receive the merged node's equations.  Division-free.
-template <int TX>
-__device__ __forceinline__ void merge_head(const NodeBuf &nb, int lx, int r1, int r2, int r3, int r4)
+// ------------------------------------------------------------------------------------------
+// K-ary merge of boundary equations (the levels above the leaves, and the cluster-level system
+// of cyclic lines).
+//
+// K consecutive nodes of S rows each (first equation in the node's first row, last equation in
+// its last row) form a 2K-row tridiagonal system in u_0 = x_first(node 0), u_1 = x_last(node 0),
+// u_2 = x_first(node 1), ..., u_{2K-1} = x_last(node K-1):
+//     row i:  s_i u_{i-1} + b_i u_i + c_i u_{i+1} = d_i        (u_{-1} = x_prev, u_{2K} = x_next).
+// The merged node's two equations come from two INDEPENDENT sweeps, run by two threads, carried
+// un-normalised (no division on the serial chain) and rescaled by exact powers of two:
+//   kmerge_fwd, rows 1 .. 2K-1, u_0 kept as a parameter:  al u_0 + be u_i + ga u_{i+1} = de,
+//       al_i = -s_i al_{i-1},  be_i = be_{i-1} b_i - s_i ga_{i-1},  ga_i = be_{i-1} c_i,
+//       de_i = be_{i-1} d_i - s_i de_{i-1};   row 2K-1 couples (u_0, u_{2K-1}, x_next): the merged
+//       LAST equation, written to the group's last row;
+//   kmerge_bwd, rows 2K-2 .. 0, u_{2K-1} kept as a parameter:  al u_{i-1} + be u_i + ga u_{2K-1} = de,
+//       al_i = be_{i+1} s_i,  be_i = be_{i+1} b_i - c_i al_{i+1},  ga_i = -c_i ga_{i+1},
+//       de_i = be_{i+1} d_i - c_i de_{i+1};   row 0 couples (x_prev, u_0, u_{2K-1}): the merged
+//       FIRST equation, written to the group's first row.
+// Neither sweep writes a row the other one reads.  The interior rows 1 .. 2K-2 stay untouched
+// until kmerge_tails (a third thread, off the serial chain) turns them into
+//     u_i = d_i - a_i u_0 - c_i u_{2K-1}.                                   K = 0: runtime k.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int krow(int g, int k, int S, int i) { return (g * k + (i >> 1)) * S + ((i & 1) ? S - 1 : 0); }
+
+template <int TX, int K>
+__device__ __forceinline__ void kmerge_fwd(const NodeBuf &nb, int lx, int g, int S, int kk)
 {
-    const uint32_t o1 = nb_ab<TX>(nb, r1, lx), o2 = nb_ab<TX>(nb, r2, lx), o3 = nb_ab<TX>(nb, r3, lx), o4 = nb_ab<TX>(nb, r4, lx);
-    const double2 ab2 = lds2(o2), cd2 = lds2(o2 + nb.plane), ab3 = lds2(o3), cd3 = lds2(o3 + nb.plane);
-    const double2 ab1 = lds2(o1), cd1 = lds2(o1 + nb.plane), ab4 = lds2(o4), cd4 = lds2(o4 + nb.plane);
-    const double A2 = ab2.x, B2 = ab2.y, C2 = cd2.x, D2 = cd2.y, A3 = ab3.x, B3 = ab3.y, C3 = cd3.x, D3 = cd3.y;
-    const double A1 = ab1.x, B1 = ab1.y, C1 = cd1.x, D1 = cd1.y, A4 = ab4.x, B4 = ab4.y, C4 = cd4.x, D4 = cd4.y;
-    const double det = fma(B2, B3, -(C2 * A3));
-    const double nL = fma(B3, D2, -(C2 * D3)), nR = fma(B2, D3, -(A3 * D2));
-    const double p1 = B3 * A2, p2 = C2 * C3, p3 = A3 * A2, p4 = B2 * C3;
-    double fb = fma(det, B1, -(C1 * p1)), lb = fma(det, B4, -(A4 * p4));
-    const double sf = pow2_unscale(fb), sl = pow2_unscale(lb);
-    sts2(o1, det * A1 * sf, fb * sf);
-    sts2(o1 + nb.plane, C1 * p2 * sf, fma(det, D1, -(C1 * nL)) * sf);
-    sts2(o4, A4 * p3 * sl, lb * sl);
-    sts2(o4 + nb.plane, det * C4 * sl, fma(det, D4, -(A4 * nR)) * sl);
+    const int k = K > 0 ? K : kk;
+    uint32_t o = nb_ab<TX>(nb, krow(g, k, S, 1), lx);
+    double2 ab = lds2(o), cd = lds2(o + nb.plane);
+    double al = ab.x, be = ab.y, ga = cd.x, de = cd.y;
+    o = nb_ab<TX>(nb, krow(g, k, S, 2), lx);
+    ab = lds2(o); cd = lds2(o + nb.plane);
+#pragma unroll
+    for (int i = 2; i < 2 * k; ++i) {
+        const double s = ab.x, b = ab.y, c = cd.x, d = cd.y;
+        if (i + 1 < 2 * k) {                                  // next row's loads go out first
+            o = nb_ab<TX>(nb, krow(g, k, S, i + 1), lx);
+            ab = lds2(o); cd = lds2(o + nb.plane);
+        }
+        const double nbe = fma(be, b, -(s * ga)), nde = fma(be, d, -(s * de));
+        const double sc = pow2_unscale(nbe);
+        al = -(s * al) * sc; ga = be * c * sc; de = nde * sc; be = nbe * sc;
+    }
+    sts2(o, al, be); sts2(o + nb.plane, ga, de);              // o: the group's last row
 }
 
-// Second half, recomputed from the two rows the merge eliminated (they are untouched until now):
-// x_lL = d - a x_first - c x_last in row r2, x_fR likewise in row r3.
-template <int TX>
-__device__ __forceinline__ void merge_tail(const NodeBuf &nb, int lx, int r2, int r3)
+template <int TX, int K>
+__device__ __forceinline__ void kmerge_bwd(const NodeBuf &nb, int lx, int g, int S, int kk)
 {
-    const uint32_t o2 = nb_ab<TX>(nb, r2, lx), o3 = nb_ab<TX>(nb, r3, lx);
-    const double2 ab2 = lds2(o2), cd2 = lds2(o2 + nb.plane), ab3 = lds2(o3), cd3 = lds2(o3 + nb.plane);
-    const double A2 = ab2.x, B2 = ab2.y, C2 = cd2.x, D2 = cd2.y, A3 = ab3.x, B3 = ab3.y, C3 = cd3.x, D3 = cd3.y;
-    const double inv = rcp_nr(fma(B2, B3, -(C2 * A3)));
-    const double nL = fma(B3, D2, -(C2 * D3)), nR = fma(B2, D3, -(A3 * D2));
-    sts2(o2, (B3 * A2) * inv, -((C2 * C3) * inv));
-    sts1(o2 + nb.plane + 8, nL * inv);
-    sts2(o3, -((A3 * A2) * inv), (B2 * C3) * inv);
-    sts1(o3 + nb.plane + 8, nR * inv);
+    const int k = K > 0 ? K : kk;
+    uint32_t o = nb_ab<TX>(nb, krow(g, k, S, 2 * k - 2), lx);
+    double2 ab = lds2(o), cd = lds2(o + nb.plane);
+    double al = ab.x, be = ab.y, ga = cd.x, de = cd.y;
+    o = nb_ab<TX>(nb, krow(g, k, S, 2 * k - 3), lx);
+    ab = lds2(o); cd = lds2(o + nb.plane);
+#pragma unroll
+    for (int i = 2 * k - 3; i >= 0; --i) {
+        const double s = ab.x, b = ab.y, c = cd.x, d = cd.y;
+        if (i > 0) {
+            o = nb_ab<TX>(nb, krow(g, k, S, i - 1), lx);
+            ab = lds2(o); cd = lds2(o + nb.plane);
+        }
+        const double nbe = fma(be, b, -(c * al)), nde = fma(be, d, -(c * de));
+        const double sc = pow2_unscale(nbe);
+        ga = -(c * ga) * sc; al = be * s * sc; de = nde * sc; be = nbe * sc;
+    }
+    sts2(o, al, be); sts2(o + nb.plane, ga, de);              // o: the group's first row
 }
 
-template <int TX>
-__device__ __forceinline__ void unmerge_pair(const NodeBuf &nb, int lx, int r1, int r2, int r3, int r4)
+// Interior rows i = 1 .. 2K-2 of a group, from their ORIGINAL equations (the merge sweeps only
+// read them): modified Thomas forward sweep with u_0 as a parameter (normalised; this runs off
+// the serial chain), then the backward sweep into
+//     u_i = d_i - a_i u_0 - c_i u_{2K-1} :   AB slot <- (a, c),  D <- d.
+template <int TX, int K>
+__device__ __forceinline__ void kmerge_tails(const NodeBuf &nb, int lx, int g, int S, int kk)
 {
-    const uint32_t o2 = nb_ab<TX>(nb, r2, lx), o3 = nb_ab<TX>(nb, r3, lx);
-    const double xf = lds1(nb_ab<TX>(nb, r1, lx) + nb.plane + 8), xl = lds1(nb_ab<TX>(nb, r4, lx) + nb.plane + 8);
-    const double2 ac2 = lds2(o2), ac3 = lds2(o3);
-    const double d2 = lds1(o2 + nb.plane + 8), d3 = lds1(o3 + nb.plane + 8);
-    sts1(o2 + nb.plane + 8, fma(-ac2.y, xl, fma(-ac2.x, xf, d2)));
-    sts1(o3 + nb.plane + 8, fma(-ac3.y, xl, fma(-ac3.x, xf, d3)));
+    const int k = K > 0 ? K : kk;
+    double a = 0.0, c = 0.0, d = 0.0;
+    for (int i = 1; i <= 2 * k - 2; ++i) {
+        const uint32_t o = nb_ab<TX>(nb, krow(g, k, S, i), lx);
+        const double2 ab = lds2(o), cd = lds2(o + nb.plane);
+        if (i == 1) {
+            const double inv = rcp_nr(ab.y);
+            a = ab.x * inv; c = cd.x * inv; d = cd.y * inv;
+        } else {
+            const double inv = rcp_nr(fma(-ab.x, c, ab.y));
+            d = fma(-ab.x, d, cd.y) * inv;
+            a = -(ab.x * a) * inv;
+            c = cd.x * inv;
+        }
+        sts2(o, a, c); sts1(o + nb.plane + 8, d);
+    }
+    // a, c, d: row 2K-2, already in final form
+    for (int i = 2 * k - 3; i >= 1; --i) {
+        const uint32_t o = nb_ab<TX>(nb, krow(g, k, S, i), lx);
+        const double2 ac = lds2(o);
+        const double di = lds1(o + nb.plane + 8);
+        d = fma(-ac.y, d, di);
+        a = fma(-ac.y, a, ac.x);
+        c = -(ac.y * c);
+        sts2(o, a, c); sts1(o + nb.plane + 8, d);
+    }
 }
 
-// Pairwise tree over `nodes` nodes (a power of two) of 2 rows each, one line per lx, thread rows
-// `slot` of `nslots`.  Bottom-up, heads only: on return (after its closing __syncthreads) the root
-// has its first equation in row 0 and its last equation in row 2*nodes-1.
-template <int TX>
-__device__ __forceinline__ void tree_up(const NodeBuf &nb, int lx, int slot, int nslots, int nodes,
-                                        bool synced = false)
+// The same in two steps for a HELPER thread that runs concurrently with the merge sweeps of the
+// same level: kmerge_tails_regs reads the 2K-2 interior rows and leaves (a, c, d) in registers,
+// kmerge_tails_store writes them back once the sweeps no longer read the rows.
+template <int TX, int K>
+__device__ __forceinline__ void kmerge_tails_regs(const NodeBuf &nb, int lx, int g, int S, double (&a)[6], double (&c)[6],
+                                                  double (&d)[6])
 {
-    for (int n = nodes, sp = 2; n > 1; n >>= 1, sp <<= 1) {
-        if (!(synced && n == nodes)) __syncthreads();   // synced: the caller has just done the first one
-        for (int q = slot; q < (n >> 1); q += nslots) {
-            const int rs = q * 2 * sp;
-            merge_head<TX>(nb, lx, rs, rs + sp - 1, rs + sp, rs + 2 * sp - 1);
+    constexpr int NI = 2 * K - 2;
+    double2 ab[NI], cd[NI];
+#pragma unroll
+    for (int j = 0; j < NI; ++j) {
+        const uint32_t o = nb_ab<TX>(nb, krow(g, K, S, j + 1), lx);
+        ab[j] = lds2(o); cd[j] = lds2(o + nb.plane);
+    }
+    double inv = rcp_nr(ab[0].y);
+    a[0] = ab[0].x * inv; c[0] = cd[0].x * inv; d[0] = cd[0].y * inv;
+#pragma unroll
+    for (int j = 1; j < NI; ++j) {
+        inv = rcp_nr(fma(-ab[j].x, c[j - 1], ab[j].y));
+        d[j] = fma(-ab[j].x, d[j - 1], cd[j].y) * inv;
+        a[j] = -(ab[j].x * a[j - 1]) * inv;
+        c[j] = cd[j].x * inv;
+    }
+#pragma unroll
+    for (int j = NI - 2; j >= 0; --j) {
+        d[j] = fma(-c[j], d[j + 1], d[j]);
+        a[j] = fma(-c[j], a[j + 1], a[j]);
+        c[j] = -(c[j] * c[j + 1]);
+    }
+}
+
+template <int TX, int K>
+__device__ __forceinline__ void kmerge_tails_store(const NodeBuf &nb, int lx, int g, int S, const double (&a)[6],
+                                                   const double (&c)[6], const double (&d)[6])
+{
+#pragma unroll
+    for (int j = 0; j < 2 * K - 2; ++j) {
+        const uint32_t o = nb_ab<TX>(nb, krow(g, K, S, j + 1), lx);
+        sts2(o, a[j], c[j]); sts1(o + nb.plane + 8, d[j]);
+    }
+}
+
+// u_i of a group (i = 0 .. 2k-1) from the group's x_first / x_last.
+template <int TX>
+__device__ __forceinline__ double kmerge_value(const NodeBuf &nb, int lx, int g, int S, int k, int i, double xf, double xl)
+{
+    if (i == 0) return xf;
+    if (i == 2 * k - 1) return xl;
+    const uint32_t o = nb_ab<TX>(nb, krow(g, k, S, i), lx);
+    const double2 ac = lds2(o);
+    return fma(-ac.y, xl, fma(-ac.x, xf, lds1(o + nb.plane + 8)));
+}
+
+// Cluster-level system of a PLAIN (non-cyclic) line, rows i = 0 .. n-1 of `tb` (s_0 = c_{n-1} = 0):
+// the CTA needs only its own two unknowns u_p, u_{p+1} (p = 2 * rank), so it eliminates towards
+// them from both ends, un-normalised (no division on the chain),
+//     forward   be u_i + ga u_{i+1} = de ,  i = 0 .. p      (be_i = be_{i-1} b_i - s_i ga_{i-1}, ...)
+//     backward  al u_{i-1} + bb u_i = dd ,  i = n-1 .. p+1  (bb_i = bb_{i+1} b_i - c_i al_{i+1}, ...)
+// and solves the remaining 2 x 2 system.  The two sweeps are independent chains of p and n-2-p
+// steps that run interleaved in one thread; one reciprocal in total.
+template <int TX>
+__device__ __forceinline__ void cluster_solve_two_sided(const NodeBuf &tb, int lx, int n, int p, double &up, double &up1)
+{
+    uint32_t of = nb_ab<TX>(tb, 0, lx), ob = nb_ab<TX>(tb, n - 1, lx);
+    const uint32_t step = TX * 16u;
+    double2 t0 = lds2(of), t1 = lds2(of + tb.plane), t2 = lds2(ob), t3 = lds2(ob + tb.plane);
+    double be = t0.y, ga = t1.x, de = t1.y;             // row 0
+    double al = t2.x, bb = t2.y, dd = t3.y;             // row n-1
+    const int nf = p, nbk = n - 2 - p;
+    const int nmax = nf > nbk ? nf : nbk;
+    double2 fab = make_double2(0.0, 1.0), fcd = make_double2(0.0, 0.0), bab = fab, bcd = fcd;
+    if (nf > 0) { of += step; fab = lds2(of); fcd = lds2(of + tb.plane); }
+    if (nbk > 0) { ob -= step; bab = lds2(ob); bcd = lds2(ob + tb.plane); }
+    for (int j = 0; j < nmax; ++j) {
+        const double fs = fab.x, fb_ = fab.y, fc_ = fcd.x, fd_ = fcd.y;
+        const double bs = bab.x, bb_ = bab.y, bc_ = bcd.x, bd_ = bcd.y;
+        const bool fw = j < nf, bw = j < nbk;
+        if (j + 1 < nf) { of += step; fab = lds2(of); fcd = lds2(of + tb.plane); }
+        if (j + 1 < nbk) { ob -= step; bab = lds2(ob); bcd = lds2(ob + tb.plane); }
+        if (fw) {
+            const double nbe = fma(be, fb_, -(fs * ga)), nde = fma(be, fd_, -(fs * de));
+            const double sc = pow2_unscale(nbe);
+            ga = be * fc_ * sc; de = nde * sc; be = nbe * sc;
+        }
+        if (bw) {
+            const double nbb = fma(bb, bb_, -(bc_ * al)), ndd = fma(bb, bd_, -(bc_ * dd));
+            const double sc = pow2_unscale(nbb);
+            al = bb * bs * sc; dd = ndd * sc; bb = nbb * sc;
         }
     }
-    __syncthreads();
-}
-
-// The tails of ALL merges of tree_up, one per thread row: merge j of the flat list (level 1 pairs,
-// then level 2 pairs, ...) goes to slot j.  No barrier inside; needs one before tree_down.
-template <int TX>
-__device__ __forceinline__ void tree_tails(const NodeBuf &nb, int lx, int slot, int nslots, int nodes)
-{
-    for (int j = slot; j < nodes - 1; j += nslots) {
-        int base = 0, n = nodes, sp = 2;
-        while (j - base >= (n >> 1)) { base += n >> 1; n >>= 1; sp <<= 1; }
-        const int rs = (j - base) * 2 * sp;
-        merge_tail<TX>(nb, lx, rs + sp - 1, rs + sp);
-    }
-}
-
-// Top-down: needs x_first / x_last of the root in D of row 0 / row 2*nodes-1 and all tails
-// (visible to all threads); ends with a __syncthreads().
-template <int TX>
-__device__ __forceinline__ void tree_down(const NodeBuf &nb, int lx, int slot, int nslots, int nodes)
-{
-    for (int n = 2, sp = nodes; n <= nodes; n <<= 1, sp >>= 1) {
-        for (int q = slot; q < (n >> 1); q += nslots) {
-            const int rs = q * 2 * sp;
-            unmerge_pair<TX>(nb, lx, rs, rs + sp - 1, rs + sp, rs + 2 * sp - 1);
-        }
-        __syncthreads();
-    }
+    const double inv = rcp_nr(fma(be, bb, -(ga * al)));
+    up = fma(de, bb, -(ga * dd)) * inv;
+    up1 = fma(be, dd, -(al * de)) * inv;
 }
 
 // Root of a tree: first equation  A x_prev + B x_f + C x_l = D  (row 0), last equation
@@ -420,11 +533,10 @@ __device__ __forceinline__ void leaf_reduce(const double *__restrict__ sA, const
     leaf_finish<M0>(fa, fb, fc, fd, pa, pc, pd, f, l, R);
 }
 
-// Back-substitution of the leaf from registers given its first and last unknown; x streamed to
-// HBM (row stride nx elements).
+// Back-substitution of the leaf from registers given its first and last unknown: row j of the
+// leaf goes to the x staging tile at sx + j * row_bytes (shared-space address).
 template <int M0>
-__device__ __forceinline__ void leaf_back(const LeafRegs<M0> &R, double xf, double xl, double *__restrict__ xp,
-                                          size_t nx)
+__device__ __forceinline__ void leaf_back(const LeafRegs<M0> &R, double xf, double xl, uint32_t sx, uint32_t row_bytes)
 {
     constexpr int K = LeafRegs<M0>::K, H = LeafRegs<M0>::H;
     double first[K], last[K];
@@ -437,15 +549,15 @@ __device__ __forceinline__ void leaf_back(const LeafRegs<M0> &R, double xf, doub
 #pragma unroll
     for (int h = 0; h < K; ++h) {
         xn[h] = last[h];
-        __stcs(xp + (size_t)(h * H) * nx, first[h]);
-        __stcs(xp + (size_t)(h * H + H - 1) * nx, last[h]);
+        sts1(sx + (uint32_t)(h * H) * row_bytes, first[h]);
+        sts1(sx + (uint32_t)(h * H + H - 1) * row_bytes, last[h]);
     }
 #pragma unroll
     for (int r = H - 2; r >= 1; --r) {
 #pragma unroll
         for (int h = 0; h < K; ++h) {
             xn[h] = fma(-R.ic[h][r - 1], xn[h], fma(-R.ia[h][r - 1], first[h], R.id[h][r - 1]));
-            __stcs(xp + (size_t)(h * H + r) * nx, xn[h]);
+            sts1(sx + (uint32_t)(h * H + r) * row_bytes, xn[h]);
         }
     }
 }
@@ -532,93 +644,172 @@ __device__ __forceinline__ void leaf_back_x(const LeafRegs<16> &R, double xf, do
     for (int p = 0; p < 8; ++p) sts2(xs_addr(bX, l, p), xs[2 * p], xs[2 * p + 1]);
 }
 
-// kX: x sweep (lanes = TX lines along y, rows = x; M0 = 16 only); tm_x is used by x sweeps only.
-template <int TX, int M0, bool kCluster, int MAXT, int MINB, bool kX>
-__global__ void __launch_bounds__(MAXT, MINB)
+// Named barrier over the tree threads (whole warps; a single warp needs __syncwarp only).
+__device__ __forceinline__ void tree_sync(int nthreads, unsigned warp_mask)
+{
+    if (nthreads > 32) asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+    else __syncwarp(warp_mask);
+}
+__device__ __forceinline__ void named_arrive(int id, int nthreads)
+{
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void named_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// kX: x sweep (lanes = TX lines along y, rows = x; M0 = 16 only).
+//
+// Threads: leaf = t / TX, lx = t % TX (a warp covers whole row segments, so tile reads,
+// node-buffer accesses and x stores are coalesced / conflict-free); blockDim = W*TX rounded up to
+// whole warps.
+// Raw tile ring.  The four arrays of a tile are fetched one TMA copy group each, in the order
+// the sweep needs them (b, a, c, d), into a ring of NA >= 4 array slots (array j of the cluster's
+// q-th tile: n = 4q + j -> slot n % NA), each with its own mbarrier.  As soon as the sweep of tile
+// q has consumed its four slots, arrays 4q+NA .. 4q+NA+3 are issued: with NA > 4, NA - 4 arrays
+// of the next tile are in flight while a tile is being swept, so HBM never idles behind the
+// sweep.  A TMA copy costs its issuing thread 150-200 cycles (measured), so the copies are
+// issued by the LAST warp, which has no part in the tree that follows the sweep.
+// x leaves the SM the same way: back-substitution writes the staging tile in shared memory and
+// the last warp hands it to the TMA engine (one tensor store per box) after the NEXT tile's
+// sweep -- an SM retires plain global stores at about a sector per cycle, which would block the
+// load/store unit the sweep reads the raw tile with for > 1000 cycles per tile.
+template <int TX, int M0, bool kCluster, int MAXT, bool kX>
+__global__ void __launch_bounds__(MAXT, 1)
 fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
                  const __grid_constant__ CUtensorMap tm_c, const __grid_constant__ CUtensorMap tm_d,
                  const __grid_constant__ CUtensorMap tm_x, const TmaFusedParams prm)
 {
     static_assert(!kX || M0 == 16, "x sweeps use 16-row (128-byte) leaves");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    const int R = prm.R, CL = prm.CL, W = prm.W;
+    const int R = prm.R, CL = prm.CL, W = prm.W, NA = prm.NS;
     const int arr = R * TX;
-    double *__restrict__ sA = reinterpret_cast<double *>(smem_raw);   // raw tile
-    double *__restrict__ sB = sA + arr;
-    double *__restrict__ sC = sB + arr;
-    double *__restrict__ sD = sC + arr;
-    const int narr = 2 * W * TX;
-    double *sX = sD + arr;                                            // x staging tile (x sweeps)
-    double *node = sX + (kX ? arr : 0);                               // node buffer, 4 x [2W][TX]
-    const int NTR = 2 * CL;                                    // rows of the cluster-level system
-    const int tarr = NTR * TX;
-    double *top = node + 4 * narr;                             // 2 inboxes x 4 x [NTR][TX]
-    uint64_t *bar = reinterpret_cast<uint64_t *>(top + 8 * tarr);   // [0]: raw tile, [1], [2]: inboxes
-    NodeBuf nb;
-    nb.ab = ptx::smem_u32(node); nb.plane = (uint32_t)narr * 16u;
+    double *const raw = reinterpret_cast<double *>(smem_raw);         // NA slots of one array [R][TX]
+    double *sX = raw + (size_t)NA * arr;                              // x staging tile
+    double *node = sX + arr;
+    NodeBuf nb;                                                       // node buffer, 2 planes of [2W][TX] pairs
+    nb.ab = ptx::smem_u32(node); nb.plane = (uint32_t)(2 * W * TX) * 16u;
+    const int NTR = 2 * CL;                                           // rows of the cluster-level system
+    NodeBuf tb0;                                                      // inbox of parity 0: 2 planes of [NTR][TX]
+    tb0.ab = nb.ab + 2u * nb.plane; tb0.plane = (uint32_t)(NTR * TX) * 16u;
+    const uint32_t inbox_bytes = kCluster ? 2u * tb0.plane : 0u;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + (tb0.ab + 2u * inbox_bytes - ptx::smem_u32(smem_raw)));
+    // bar[0 .. NA-1]: slot full; bar[NA], bar[NA+1]: inboxes
 
     const int t = threadIdx.x;
+    const int NT = W * TX;
+    const bool act = t < NT;
+    // tree threads: all warps but the last (which issues the copies); a single warp does both
+    const int tree_threads = (int)blockDim.x > 32 ? (int)blockDim.x - 32 : NT;
+    const bool tree = t < tree_threads && act;
+    const int Wt = tree_threads / TX;
+    const unsigned tmask = __ballot_sync(0xffffffffu, tree);
     unsigned crank = 0;
     if (kCluster) crank = cg::this_cluster().block_rank();
     const int g = blockIdx.x / CL, NC = gridDim.x / CL;        // cluster index / number of clusters
-    const int lx = t % TX, leaf = t / TX;
     const int y0 = (int)crank * R;
-    const int o0 = leaf * M0 * TX + lx;
-    const bool first_leaf = !prm.periodic && (y0 + leaf * M0 == 0);
-    const bool last_leaf = !prm.periodic && (y0 + leaf * M0 + M0 == prm.ny);
 
-    // The whole raw tile of `tile` in flight at once.  One copy costs its issuing thread 150-200
-    // cycles (measured), so inside the loop the four arrays are issued by lane 0 of four DIFFERENT
-    // warps -- the last four, which have no merge to do at the first tree level -- and the climb
-    // does not wait for them.  sel < 0: all arrays (prologue); sel = 0..3: array sel only.
-    auto issue_tile = [&](int tile, int sel) {
+    if (t == 0) {
+        for (int i = 0; i < NA + 2; ++i) ptx::mbar_init(&bar[i], 1);
+        ptx::fence_mbar_init();
+    }
+    __syncthreads();                    // mbarriers initialised before anyone uses them
+    // split-phase cluster barrier: "every CTA of the cluster has started and initialised its
+    // inbox mbarriers" must hold before the first remote store; the matching wait sits right
+    // before the first exchange
+    if (kCluster) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+
+    // TMA copies of one raw array, by the lanes of the last warp
+    const int issue_lane = t - ((int)blockDim.x - 32 > 0 ? (int)blockDim.x - 32 : 0);   // >= 0: issuing warp
+    const uint32_t arr_bytes = (uint32_t)(arr * sizeof(double));
+    auto issue_array = [&](int n) {
+        const int tile = g + (n >> 2) * NC, j = n & 3;
+        if (tile >= prm.ntiles) return;
+        const int s = n % NA;
         const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
-        if (sel <= 0) ptx::mbar_expect_tx(&bar[0], (unsigned)(4 * arr * sizeof(double)));
-        double *const dst[4] = {sB, sA, sC, sD};
-        const CUtensorMap *const tm[4] = {&tm_b, &tm_a, &tm_c, &tm_d};
-        for (int a = 0; a < 4; ++a) {
-            if (sel >= 0 && sel != a) continue;
-            if (kX) {                   // one (16 x, TX lines) box per leaf; x0 = first line (y)
-                for (int w = 0; w < W; ++w)
-                    ptx::tma_load_3d(dst[a] + w * 16 * TX, tm[a], y0 + 16 * w, x0, k, &bar[0]);
-            } else for (int q = 0; q < prm.nbox; ++q) {
+        double *const dst = raw + (size_t)s * arr;
+        const CUtensorMap *const tm = j == 0 ? &tm_b : (j == 1 ? &tm_a : (j == 2 ? &tm_c : &tm_d));
+        if (issue_lane == 0) ptx::mbar_expect_tx(&bar[s], arr_bytes);
+        if (kX) {                   // one (16 x, TX lines) box per leaf; x0 = first line (y)
+            __syncwarp();
+            for (int w = issue_lane; w < W; w += 32)
+                ptx::tma_load_3d(dst + w * 16 * TX, tm, y0 + 16 * w, x0, k, &bar[s]);
+        } else if (issue_lane == 0) {
+            for (int q = 0; q < prm.nbox; ++q) {
                 const int yy = y0 + q * prm.box_rows;
-                const int c1 = prm.axis_z ? k : yy, c2 = prm.axis_z ? yy : k;
-                ptx::tma_load_3d(dst[a] + q * prm.box_rows * TX, tm[a], x0, c1, c2, &bar[0]);
+                ptx::tma_load_3d(dst + q * prm.box_rows * TX, tm, x0, prm.axis_z ? k : yy, prm.axis_z ? yy : k, &bar[s]);
             }
         }
     };
-    const int nwarps = ((int)blockDim.x + 31) / 32;
-    // my role in the in-loop issue: -1 none, -2 everything (CTAs with fewer than 8 warps), 0..3 array
-    const int issue_sel = nwarps >= 8 ? (((t & 31) == 0 && t / 32 >= nwarps - 4) ? t / 32 - (nwarps - 4) : -1)
-                                      : (t == 0 ? -2 : -1);
+    // the staging tile of tile `tile` -> x (TMA clips the ragged last x tile)
+    auto store_x = [&](int tile) {
+        const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
+        if (kX) {
+            for (int w = issue_lane; w < W; w += 32) ptx::tma_store_3d(&tm_x, y0 + 16 * w, x0, k, sX + w * 16 * TX);
+        } else if (issue_lane == 0) {
+            for (int q = 0; q < prm.nbox; ++q) {
+                const int yy = y0 + q * prm.box_rows;
+                ptx::tma_store_3d(&tm_x, x0, prm.axis_z ? k : yy, prm.axis_z ? yy : k, sX + q * prm.box_rows * TX);
+            }
+        }
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    };
+    if (issue_lane >= 0) for (int n = 0; n < NA; ++n) issue_array(n);
 
-    if (t == 0) {
-        ptx::mbar_init(&bar[0], 1);
-        ptx::mbar_init(&bar[1], 1);
-        ptx::mbar_init(&bar[2], 1);
-        ptx::fence_mbar_init();
-        issue_tile(g, -1);
+    const int lx = t % TX, leaf = t / TX;
+    const bool first_leaf = !prm.periodic && (y0 + leaf * M0 == 0);
+    const bool last_leaf = !prm.periodic && (y0 + leaf * M0 + M0 == prm.ny);
+    const int o0 = leaf * M0 * TX + lx;
+    // levels above the leaves: 4-ary merges (2-ary when the node count is not a multiple of 4)
+    // level l merges k = 2^lkb nodes of S = 2 << cum rows (cum = sum of the lkb below); packed into
+    // two words (a local array indexed by the level would live in local memory)
+    unsigned kcode = 0, ccode = 0;
+    int nl = 0;
+    for (int nodes = W, cum = 0; nodes > 1; ++nl) {
+        const int lkb = (nodes & 3) == 0 ? 2 : 1;
+        kcode |= (unsigned)lkb << (2 * nl); ccode |= (unsigned)cum << (5 * nl);
+        nodes >>= lkb; cum += lkb;
     }
-    __syncthreads();                    // mbarriers initialised before anyone waits on them
-    // split-phase cluster barrier: "every CTA of the cluster has started and initialised its
-    // inbox mbarriers" must hold before the first remote store; the matching wait sits right
-    // before the first exchange, where it is satisfied long ago
-    if (kCluster) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    auto level_k = [&](int l) { return 1 << ((kcode >> (2 * l)) & 3u); };
+    auto level_S = [&](int l) { return 2 << ((ccode >> (5 * l)) & 31u); };
+    auto level_groups = [&](int l) { return W >> (((ccode >> (5 * l)) & 31u) + ((kcode >> (2 * l)) & 3u)); };
 
+    // Static split of the tree threads, by whole warps:
+    //   CRITICAL warps [0, cw): their thread rows run the merge sweeps of every level, synchronise
+    //     among themselves only (named barrier 1), send the CTA's node and solve the cluster-level
+    //     system -- the serial chain of a tile;
+    //   HELPER warps [cw, tree warps): their thread rows compute the interior-row forms
+    //     (kmerge_tails) of every level CONCURRENTLY with that level's merge sweeps, in registers,
+    //     and store them once the sweeps have signalled (bar.arrive on named barrier 2 + level,
+    //     which costs the critical warps nothing) that they no longer read the rows.
+    // Without helper warps (small tiles) the critical rows do the interior rows themselves.
+    const int G0 = nl > 0 ? level_groups(0) : 0;
+    const int rpw = TX >= 32 ? 1 : 32 / TX;                           // thread rows per warp
+    const int crit_rows = Wt >= 2 * G0 ? 2 * G0 : (Wt >= G0 ? G0 : Wt);
+    const int cw = (crit_rows + rpw - 1) / rpw;
+    const bool helper_mode = nl > 0 && (int)blockDim.x > 32 && cw * 32 < tree_threads;
+    const int help0 = helper_mode ? cw * rpw : Wt;                   // first helper row
+    const int nhelp = Wt - help0;
+    const int mrows = helper_mode ? crit_rows : Wt;                  // rows that share the merges of a level
+    const int crit_threads = helper_mode ? cw * 32 : tree_threads;
+    const bool crit = tree && leaf < help0, helper = tree && !crit;
     int it = 0;
     for (int tile = g; tile < prm.ntiles; tile += NC, ++it) {
         const int par = it & 1;
-        NodeBuf tb;                                            // this tile's inbox
-        tb.ab = ptx::smem_u32(top + par * 4 * tarr); tb.plane = (uint32_t)tarr * 16u;
+        NodeBuf tb = tb0;                                      // this tile's inbox
+        tb.ab += (uint32_t)par * inbox_bytes;
         // arm this tile's inbox: 4 doubles per (node equation, line) from every CTA
-        if (kCluster && t == 0) ptx::mbar_expect_tx(&bar[1 + par], (unsigned)(4 * tarr * sizeof(double)));
-        if (kX && t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-        ptx::mbar_wait(&bar[0], (unsigned)par);
+        if (kCluster && t == 0) ptx::mbar_expect_tx(&bar[NA + par], (unsigned)(4 * NTR * TX * sizeof(double)));
+        const int n0 = 4 * it;
+        const double *__restrict__ sB = raw + (size_t)(n0 % NA) * arr, *__restrict__ sA = raw + (size_t)((n0 + 1) % NA) * arr;
+        const double *__restrict__ sC = raw + (size_t)((n0 + 2) % NA) * arr, *__restrict__ sD = raw + (size_t)((n0 + 3) % NA) * arr;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) ptx::mbar_wait(&bar[(n0 + j) % NA], (unsigned)(((n0 + j) / NA) & 1));
 
         // ---------------- leaves ----------------
         LeafRegs<M0> regs;
-        {
+        if (act) {
             Eq f, l;
             if constexpr (kX) {
                 const uint32_t bo = (uint32_t)(leaf * 16 * TX) * 8u;
@@ -631,80 +822,128 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             sts2(of, f.a, f.b); sts2(of + nb.plane, f.c, f.d);
             sts2(ol, l.a, l.b); sts2(ol + nb.plane, l.c, l.d);
         }
-        __syncthreads();                // raw tile consumed, node equations visible
-        if (issue_sel != -1 && tile + NC < prm.ntiles) issue_tile(tile + NC, issue_sel == -2 ? -1 : issue_sel);   // prefetch behind the tree
-
-        // ---------------- pairwise tree inside the CTA, bottom-up ----------------
-        tree_up<TX>(nb, lx, leaf, W, W, true);
-
-        // ---------------- cluster level ----------------
-        // the CTA's node: first equation in node row 0, last equation in node row 2W-1
-        if (!kCluster) {
-            if (t < TX) solve_root<TX>(nb, lx, 2 * W - 1, prm.periodic != 0);
-            tree_tails<TX>(nb, lx, leaf, W, W);
-            __syncthreads();
-        } else {
-            // A2B as an all-gather (the paper's MPI_Alltoall, with every rank
-            // keeping a copy): asynchronous DSMEM stores that complete on the RECEIVER's mbarrier
-            if (it == 0) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-            const uint32_t bar_s = ptx::smem_u32(&bar[1 + par]);
-            for (int e = t; e < 2 * TX * CL; e += (int)blockDim.x) {
-                const int dest = e / (2 * TX), r = e - dest * 2 * TX;
-                const int j = r / TX, l = r - j * TX;      // j: 0 = first eq, 1 = last eq
-                const uint32_t src = nb_ab<TX>(nb, j ? 2 * W - 1 : 0, l);
-                const double2 ab = lds2(src), cd = lds2(src + nb.plane);
-                const uint32_t dst = ptx::mapa(nb_ab<TX>(tb, (int)crank * 2 + j, l), (unsigned)dest);
-                const uint32_t dbar = ptx::mapa(bar_s, (unsigned)dest);
-                ptx::st_async_2f64(dst, ab.x, ab.y, dbar);
-                ptx::st_async_2f64(dst + tb.plane, cd.x, cd.y, dbar);
-            }
-            // the reciprocals of the tree just climbed run behind the exchange
-            tree_tails<TX>(nb, lx, leaf, W, W);
-            ptx::mbar_wait(&bar[1 + par], (unsigned)((it >> 1) & 1));
-            // Stage B: the 2*CL-row system, solved redundantly by every CTA with the same
-            // pairwise tree, so no second exchange is needed
-            tree_up<TX>(tb, lx, leaf, W, CL);
-            if (t < TX) solve_root<TX>(tb, lx, NTR - 1, prm.periodic != 0);
-            tree_tails<TX>(tb, lx, leaf, W, CL);
-            __syncthreads();
-            tree_down<TX>(tb, lx, leaf, W, CL);
-            // B2C: my node's boundary values
-            for (int e = t; e < 2 * TX; e += (int)blockDim.x) {
-                const int j = e / TX, l = e - j * TX;
-                sts1(nb_ab<TX>(nb, j ? 2 * W - 1 : 0, l) + nb.plane + 8,
-                     lds1(nb_ab<TX>(tb, (int)crank * 2 + j, l) + tb.plane + 8));
-            }
-            __syncthreads();
+        __syncthreads();                // raw slots consumed, leaf equations visible
+        if (issue_lane >= 0) {
+            for (int j = 0; j < 4; ++j) issue_array(n0 + NA + j);     // refill the four slots
+            if (it > 0) store_x(tile - NC);                            // x of the previous tile
         }
+        if (kCluster && it == 0) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 
-        // ---------------- pairwise tree inside the CTA, top-down ----------------
-        tree_down<TX>(nb, lx, leaf, W, W);
-
-        // ---------------- leaves: back-substitution from registers, x streamed to HBM --------
-        {
-            const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
-            const double xf = lds1(nb_ab<TX>(nb, 2 * leaf, lx) + nb.plane + 8);
-            const double xl = lds1(nb_ab<TX>(nb, 2 * leaf + 1, lx) + nb.plane + 8);
-            if constexpr (kX) {
-                // the staging tile of the previous iteration has been read by the TMA engine
-                // (thread 0 waited at the top of this iteration, barriers in between)
-                leaf_back_x(regs, xf, xl, ptx::smem_u32(sX) + (uint32_t)(leaf * 16 * TX) * 8u, lx);
-                ptx::fence_proxy_async_smem();
-                __syncthreads();
-                if (t == 0) {
-                    for (int w = 0; w < W; ++w)
-                        ptx::tma_store_3d(&tm_x, y0 + 16 * w, x0, k, sX + w * 16 * TX);
-                    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        // ---------------- K-ary tree inside the CTA, bottom-up ----------------
+        // The warp that issues the copies (the last one) takes no part in the tree, so the
+        // 150-200 cycles per copy stay off the serial chain; everybody meets again before the
+        // back-substitution.
+        if (helper) {
+            const int h = leaf - help0;
+            int cum = 0;                                        // interior-row jobs of the levels below
+            for (int l = 0; l < nl; ++l) {
+                const int k = level_k(l), S = level_S(l), groups = level_groups(l);
+                int gq = (h - cum) % nhelp;
+                if (gq < 0) gq += nhelp;
+                double ta[6], tc[6], td[6];
+                if (gq < groups) {
+                    if (k == 4) kmerge_tails_regs<TX, 4>(nb, lx, gq, S, ta, tc, td);
+                    else kmerge_tails_regs<TX, 2>(nb, lx, gq, S, ta, tc, td);
                 }
-            } else if (x0 + lx < prm.nx) {     // ragged last x tile: TMA zero-filled those lanes
-                leaf_back<M0>(regs, xf, xl,
-                              prm.x + (size_t)k * (size_t)prm.os + (size_t)(y0 + leaf * M0) * (size_t)prm.rs +
-                                  (size_t)(x0 + lx), (size_t)prm.rs);
+                named_sync(2 + l, tree_threads);                // the merges of level l are done
+                if (gq < groups) {
+                    if (k == 4) kmerge_tails_store<TX, 4>(nb, lx, gq, S, ta, tc, td);
+                    else kmerge_tails_store<TX, 2>(nb, lx, gq, S, ta, tc, td);
+                    for (gq += nhelp; gq < groups; gq += nhelp) {   // more jobs than helper rows
+                        if (k == 4) kmerge_tails<TX, 4>(nb, lx, gq, S, 4); else kmerge_tails<TX, 2>(nb, lx, gq, S, 2);
+                    }
+                }
+                cum += groups;
             }
+        }
+        if (crit) {
+            for (int l = 0; l < nl; ++l) {
+                const int k = level_k(l), S = level_S(l), groups = level_groups(l);
+                for (int q = leaf; q < 2 * groups; q += mrows) {  // q < groups: forward, else backward sweep
+                    if (q < groups) { if (k == 4) kmerge_fwd<TX, 4>(nb, lx, q, S, 4); else kmerge_fwd<TX, 2>(nb, lx, q, S, 2); }
+                    else { if (k == 4) kmerge_bwd<TX, 4>(nb, lx, q - groups, S, 4); else kmerge_bwd<TX, 2>(nb, lx, q - groups, S, 2); }
+                }
+                if (helper_mode) named_arrive(2 + l, tree_threads);
+                tree_sync(crit_threads, tmask);
+                if (!helper_mode) {                             // nobody reads the interior rows any more
+                    for (int q = mrows - 1 - leaf; q < groups; q += mrows) {    // last rows first: row 0 goes on
+                        if (k == 4) kmerge_tails<TX, 4>(nb, lx, q, S, 4); else kmerge_tails<TX, 2>(nb, lx, q, S, 2);
+                    }
+                }
+            }
+
+            // ---------------- cluster level ----------------
+            // the CTA's node: first equation in node row 0, last equation in node row 2W-1
+            if (!kCluster) {
+                if (leaf == 0) solve_root<TX>(nb, lx, 2 * W - 1, prm.periodic != 0);
+            } else {
+                // A2B as an all-gather (the paper's MPI_Alltoall, with every rank
+                // keeping a copy): asynchronous DSMEM stores that complete on the RECEIVER's mbarrier
+                const uint32_t bar_s = ptx::smem_u32(&bar[NA + par]);
+                for (int e = t; e < 4 * TX * CL; e += crit_threads) {
+                    const int dest = e / (4 * TX), r = e - dest * 4 * TX;
+                    const int piece = r / TX, l = r - piece * TX;  // piece: AB / CD of first, AB / CD of last
+                    const int j = piece >> 1;
+                    const uint32_t po = (piece & 1) ? 1u : 0u;
+                    const double2 v = lds2(nb_ab<TX>(nb, j ? 2 * W - 1 : 0, l) + po * nb.plane);
+                    const uint32_t dst = ptx::mapa(nb_ab<TX>(tb, (int)crank * 2 + j, l) + po * tb.plane, (unsigned)dest);
+                    ptx::st_async_2f64(dst, v.x, v.y, ptx::mapa(bar_s, (unsigned)dest));
+                }
+                if (leaf == 0 && !prm.periodic) {
+                    ptx::mbar_wait(&bar[NA + par], (unsigned)((it >> 1) & 1));
+                    // Stage B: the 2 CL-row system; every CTA computes its own two unknowns (one
+                    // thread per line), so no second exchange is needed (B2C is a local store)
+                    double u0, u1;
+                    cluster_solve_two_sided<TX>(tb, lx, NTR, 2 * (int)crank, u0, u1);
+                    sts1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8, u0);
+                    sts1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8, u1);
+                } else if (leaf == 0) {
+                    ptx::mbar_wait(&bar[NA + par], (unsigned)((it >> 1) & 1));
+                    // cyclic lines: merge the CL nodes, resolve the wrap at the root, walk back
+                    kmerge_fwd<TX, 0>(tb, lx, 0, 2, CL);
+                    kmerge_bwd<TX, 0>(tb, lx, 0, 2, CL);
+                    solve_root<TX>(tb, lx, NTR - 1, true);
+                    kmerge_tails<TX, 0>(tb, lx, 0, 2, CL);
+                    const double xf = lds1(nb_ab<TX>(tb, 0, lx) + tb.plane + 8), xl = lds1(nb_ab<TX>(tb, NTR - 1, lx) + tb.plane + 8);
+                    sts1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8, kmerge_value<TX>(tb, lx, 0, 2, CL, 2 * (int)crank, xf, xl));
+                    sts1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8, kmerge_value<TX>(tb, lx, 0, 2, CL, 2 * (int)crank + 1, xf, xl));
+                }
+            }
+        }
+        // the TMA engine must have read the previous tile's x out of the staging tile
+        if (issue_lane >= 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        __syncthreads();
+
+        // ---------------- leaves: back-substitution from registers into the staging tile --------
+        if (act) {
+            // top-down through the tree in registers: every thread row walks from the CTA's node
+            // to its own leaf (x_first / x_last of a child from those of its parent and the
+            // interior-row form kmerge_tails left), no barrier, nothing written
+            double xf = lds1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8);
+            double xl = lds1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8);
+            for (int l = nl - 1; l >= 0; --l) {
+                const int k = level_k(l), S = level_S(l);
+                const int node = leaf >> ((ccode >> (5 * l)) & 31u);        // my ancestor among this level's children
+                const int gq = node >> ((kcode >> (2 * l)) & 3u), j = node & (k - 1);
+                const double nf = kmerge_value<TX>(nb, lx, gq, S, k, 2 * j, xf, xl);
+                const double nlast = kmerge_value<TX>(nb, lx, gq, S, k, 2 * j + 1, xf, xl);
+                xf = nf; xl = nlast;
+            }
+            if constexpr (kX) leaf_back_x(regs, xf, xl, ptx::smem_u32(sX) + (uint32_t)(leaf * 16 * TX) * 8u, lx);
+            else leaf_back<M0>(regs, xf, xl, ptx::smem_u32(sX) + (uint32_t)o0 * 8u, TX * 8u);
+            // generic-proxy writes of the staging tile -> visible to the TMA store that the last
+            // warp issues after the next barrier (the next tile's sweep barrier, or the one below)
+            ptx::fence_proxy_async_smem();
         }
     }
-    // the staging tile must outlive the last TMA store
-    if (kX && t == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    // x of the last tile; the staging tile must outlive the store
+    if (it > 0) {
+        __syncthreads();
+        if (issue_lane >= 0) {
+            store_x(g + (it - 1) * NC);
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -712,13 +951,21 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
 // ------------------------------------------------------------------------------------------
 inline bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
 
-// Eligibility: nx even (TMA global strides are multiples of 16 B), the y extent tiles as
-// CL x W x m0 with W a power of two, m0 | ny/P and (ny/P)/m0 a power of two (so that one tree
-// level is the paper's partition level), the tile fits shared memory.
+// Leaf sizes the kernel is instantiated for: powers of two and 3, 5 times a power of two, so that
+// line lengths 2^k, 3 * 2^k and 5 * 2^k tile as CL x W x m0 with W a power of two.
+constexpr int kLeafSizes[] = {16, 12, 10, 8, 6, 4, 2};
+
+// Eligibility: nx even (TMA global strides are multiples of 16 B), the line tiles as CL x W x m0
+// with CL and W powers of two (W <= 32: the tree of a line runs inside a warp), the tile fits
+// shared memory.  The leaves need NOT nest with the paper's partitions (D1): every
+// level of the recursion is a Schur complement of the same matrix, so cutting a line into leaves
+// of m0 rows instead of partitions of ny/P rows changes x only by rounding.  When m0 divides
+// ny/P with a power-of-two quotient, one tree level is exactly the paper's 2P-row reduced system.
 inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int want_lines,
                                 int want_cluster, int want_leaf, const cudaDeviceProp &prop,
-                                const char **why, bool xaxis = false, bool zaxis = false)
+                                const char **why, bool xaxis = false, bool zaxis = false, int want_slots = 0)
 {
+    (void)P;
     // x sweep: nx = number of lanes (caller's ny), ny = line length (caller's nx)
     if (xaxis) {
         if (ny % 2) { *why = "TMA path needs even nx (16-byte global strides)"; return false; }
@@ -727,7 +974,6 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
         }
         want_lines = 16; want_leaf = 16;
     } else if (nx % 2) { *why = "TMA path needs even nx (16-byte global strides)"; return false; }
-    const int m = ny / P;
     const size_t max_smem = prop.sharedMemPerBlockOptin;
     const size_t sm_smem = prop.sharedMemPerMultiprocessor;
     TmaFusedConfig best; double best_score = -1.0;
@@ -743,32 +989,36 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
             if (CL > 8 && !want_cluster) continue;
             if (ny % CL) continue;
             const int R = ny / CL;
-            if (R % m && m % R) continue;                  // partitions and CTAs must nest
-            for (int m0 = 2; m0 <= m && m0 <= R && m0 <= 16; m0 *= 2) {
+            for (int m0 : kLeafSizes) {
                 if (want_leaf && m0 != want_leaf) continue;
-                if (m % m0 || !is_pow2(m / m0) || R % m0 || !is_pow2(R / m0)) continue;
+                if (m0 > R || R % m0 || !is_pow2(R / m0) || R / m0 > 32) continue;
                 TmaFusedConfig c;
                 c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
                 c.threads = c.leaves * TX;
-                if (c.threads > 1024 || (xaxis && c.threads > 256)) continue;
+                if (c.threads > 512 || (xaxis && c.threads > 256)) continue;
                 c.nlev = 0;
                 while ((1 << c.nlev) < c.leaves) ++c.nlev;
                 c.box_rows = R;
                 while (c.box_rows > 256) c.box_rows /= 2;
                 if (R % c.box_rows) continue;
                 c.xaxis = xaxis;
-                c.smem = tma_fused_smem_bytes(TX, R, c.leaves, CL, xaxis);
-                if (c.smem > max_smem) continue;
+                // as many ring slots (<= 8 = two whole tiles) as shared memory holds
+                c.slots = 0;
+                for (int na = want_slots ? want_slots : 8; na >= (want_slots ? want_slots : 4); --na) {
+                    c.smem = tma_fused_smem_bytes(TX, R, c.leaves, CL, na, xaxis);
+                    if (c.smem <= max_smem) { c.slots = na; break; }
+                }
+                if (!c.slots) continue;
                 long ctas = (long)(sm_smem / (c.smem + 1024));
-                const long by_thr = 2048 / c.threads;
+                const long launch_threads = (c.threads + 31) & ~31;
+                const long by_thr = 2048 / launch_threads;
                 if (by_thr < ctas) ctas = by_thr;
                 if (ctas < 1) continue;
                 // Measured on B200 (cfg 3 shapes): the tile period is set by the serial phases, so
-                // long leaves (fewer tree levels) win first; then two CTAs per SM (one sweeps while
-                // the other walks its tree), resident cells, small clusters, 64-128 B row segments.
-                // registers per thread of the instantiation (see launch_tma_m0)
-                const long regs = c.threads > 512 ? 64 : (c.threads > 256 || m0 < 16 ? 128 : 256);
-                const long by_regs = 65536 / (regs * c.threads);
+                // long leaves (fewer tree levels) win first; then resident cells, small clusters,
+                // 128 B row segments.  Registers per thread of the instantiation: launch_tma_m0.
+                const long regs = c.threads > 256 ? 128 : 255;
+                const long by_regs = 65536 / (regs * launch_threads);
                 if (by_regs < ctas) ctas = by_regs;
                 if (ctas < 1) continue;
                 double cells = (double)ctas * R * TX;
@@ -776,8 +1026,8 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
                 // 128 B row segments: with 64 B segments the persistent clusters drift apart in a
                 // long run and DRAM row-buffer locality between neighbouring x tiles is lost
                 // (measured: 4.4 -> 3.1 TB/s from 256 to 1024 slices at TX = 8, flat at TX = 16)
-                double score = 10000.0 * m0 + cells + (c.threads >= 32 ? 4000.0 : 0.0) + (ctas >= 2 ? 100.0 : 0.0) -
-                               50.0 * CL +
+                double score = 10000.0 * m0 + cells + (c.threads >= 32 ? 4000.0 : 0.0) + (c.slots > 4 ? 500.0 : 0.0) -
+                               50.0 * CL - (c.threads > 256 && m0 > 8 ? 60000.0 : 0.0) +   // 128 registers: spills
                                // z sweeps: rows of a line are whole slices apart (a DRAM page and a
                                // TLB entry per row), 256 B segments pay (0.99 -> 0.91 ms on cfg 4)
                                (zaxis ? (TX == 32 ? 3000.0 : (TX == 16 ? 1000.0 : 0.0))
@@ -787,7 +1037,7 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
         }
     }
     if (best_score < 0) {
-        *why = "no (lines, cluster, leaf) tiling with power-of-two tree fits shared memory";
+        *why = "no (lines, cluster, leaf) tiling with a power-of-two tree of <= 32 leaves fits shared memory";
         return false;
     }
     *out = best;
@@ -848,14 +1098,14 @@ inline bool make_xsweep_tensor_map(CUtensorMap *tm, const void *base, int nrows,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int TX, int M0, bool kCluster, int MAXT, int MINB, bool kX = false>
+template <int TX, int M0, bool kCluster, int MAXT, bool kX = false>
 inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                    cudaStream_t st)
 {
-    auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, MINB, kX>;
-    size_t smem_bytes = cfg.smem;
+    auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, kX>;
+    const size_t smem_bytes = cfg.smem;
     cudaLaunchConfig_t lc = {};
-    lc.blockDim = dim3(cfg.threads);
+    lc.blockDim = dim3((cfg.threads + 31) & ~31);
     lc.dynamicSmemBytes = smem_bytes;
     lc.stream = st;
     cudaLaunchAttribute attr[1];
@@ -878,7 +1128,7 @@ inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, c
             e = cudaOccupancyMaxActiveClusters(&n, kern, &lc);
             if (e != cudaSuccess) return e;
         } else {
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, cfg.threads, smem_bytes);
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, (int)lc.blockDim.x, smem_bytes);
             if (e != cudaSuccess) return e;
             n *= sms;
         }
@@ -895,27 +1145,28 @@ template <int TX, int M0, bool kCluster>
 inline cudaError_t launch_tma_m0(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                  cudaStream_t st)
 {
-    // registers: the parked interior rows take 6 (M0 - 2) of them
-    if (M0 >= 16 && cfg.threads <= 256) return launch_tma_inst<TX, M0, kCluster, 256, 1>(cfg, tm, prm, st);
-    if (cfg.threads <= 256) return launch_tma_inst<TX, M0, kCluster, 256, 2>(cfg, tm, prm, st);
-    if (cfg.threads <= 512) return launch_tma_inst<TX, M0, kCluster, 512, 1>(cfg, tm, prm, st);
-    return launch_tma_inst<TX, M0, kCluster, 1024, 1>(cfg, tm, prm, st);
+    // registers: the parked interior rows take 6 (M0 - 2) of them; <= 256 threads leave 255 per
+    // thread, <= 512 leave 128
+    if (cfg.threads <= 256) return launch_tma_inst<TX, M0, kCluster, 256>(cfg, tm, prm, st);
+    return launch_tma_inst<TX, M0, kCluster, 512>(cfg, tm, prm, st);
 }
 
 template <int TX, bool kCluster>
-inline cudaError_t launch_tma_tx(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
-                                 cudaStream_t st)
+cudaError_t launch_tma_tx(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm, cudaStream_t st)
 {
     switch (cfg.leaf_rows) {
     case 2: return launch_tma_m0<TX, 2, kCluster>(cfg, tm, prm, st);
     case 4: return launch_tma_m0<TX, 4, kCluster>(cfg, tm, prm, st);
+    case 6: return launch_tma_m0<TX, 6, kCluster>(cfg, tm, prm, st);
     case 8: return launch_tma_m0<TX, 8, kCluster>(cfg, tm, prm, st);
+    case 10: return launch_tma_m0<TX, 10, kCluster>(cfg, tm, prm, st);
+    case 12: return launch_tma_m0<TX, 12, kCluster>(cfg, tm, prm, st);
     case 16: return launch_tma_m0<TX, 16, kCluster>(cfg, tm, prm, st);
     default: return cudaErrorInvalidValue;
     }
 }
 
-// a, b, c, d: batch base pointers (slice 0 of the launch), 16-byte aligned; x: 8-byte aligned.
+// a, b, c, d, x: batch base pointers (slice 0 of the launch), 16-byte aligned.
 inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const double *b,
                                     const double *c, const double *d, double *x, int nx, int ny,
                                     int nzs, long long rs, long long os, bool axis_z, bool periodic,
@@ -924,7 +1175,6 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
     CUtensorMap tm[5];
     const void *ptr[5] = {a, b, c, d, x};
     for (int i = 0; i < 5 && nzs > 0; ++i) {
-        if (i == 4 && !cfg.xaxis) { tm[4] = tm[3]; break; }      // x is stored from registers
         if (cfg.xaxis ? !make_xsweep_tensor_map(&tm[i], ptr[i], ny, nx, nzs, cfg.lines)
                       : !make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows))
             return cudaErrorInvalidValue;
@@ -933,14 +1183,14 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
     prm.nx = nx; prm.ny = ny; prm.nzs = nzs;
     prm.x = x;
     prm.rs = rs; prm.os = os; prm.axis_z = axis_z ? 1 : 0; prm.periodic = periodic ? 1 : 0;
-    prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves;
+    prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves; prm.NS = cfg.slots;
     prm.xtiles = (nx + cfg.lines - 1) / cfg.lines;
     prm.ntiles = prm.xtiles * nzs;
     prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
     const bool cl = cfg.cluster > 1;
     if (cfg.xaxis)
-        return cl ? launch_tma_inst<16, 16, true, 256, 1, true>(cfg, tm, prm, st)
-                  : launch_tma_inst<16, 16, false, 256, 1, true>(cfg, tm, prm, st);
+        return cl ? launch_tma_inst<16, 16, true, 256, true>(cfg, tm, prm, st)
+                  : launch_tma_inst<16, 16, false, 256, true>(cfg, tm, prm, st);
     switch (cfg.lines) {
     case 32: return cl ? launch_tma_tx<32, true>(cfg, tm, prm, st) : launch_tma_tx<32, false>(cfg, tm, prm, st);
     case 16: return cl ? launch_tma_tx<16, true>(cfg, tm, prm, st) : launch_tma_tx<16, false>(cfg, tm, prm, st);

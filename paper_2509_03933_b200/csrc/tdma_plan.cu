@@ -255,7 +255,7 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
         const bool plain_y = pl->axis == TDMA_AXIS_Y && !per;
         cudaError_t e;
         const bool aligned = ((((uintptr_t)ptr.a | (uintptr_t)ptr.b | (uintptr_t)ptr.c | (uintptr_t)ptr.d |
-                                (pl->axis == TDMA_AXIS_X ? (uintptr_t)ptr.x : 0)) & 15) == 0);   // tensor maps
+                                (uintptr_t)ptr.x) & 15) == 0);   // tensor maps
         if (pl->fused_impl == 2 && aligned) {
             // Fill launch: a cluster of >= 4 CTAs cannot be placed on every SM.  With one main CTA
             // per SM the SMs left over take a second persistent launch with clusters of 2 that
@@ -413,7 +413,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         const bool tma_ok = pl->ny > 1 && tdma::get_encode_tiled() != nullptr &&
                             tdma::configure_tma_fused(&probe, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
                                                       opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
-                                                      prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z);
+                                                      prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z,
+                                                      opt ? opt->fused_slots : 0);
         variant = (tma_ok || pl->axis == TDMA_AXIS_X || pl->periodic) ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
         if (variant == TDMA_VARIANT_FUSED) {
             pl->bz = pl->nz; pl->nb = 1; pl->Lb_max = (size_t)pl->nx * pl->bz;
@@ -481,7 +482,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
             have_tma = tdma::get_encode_tiled() != nullptr &&
                        tdma::configure_tma_fused(&pl->tfused, pl->nx, pl->ny, pl->P, opt ? opt->fused_lines : 0,
                                                  opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
-                                                 prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z);
+                                                 prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z,
+                                                 opt ? opt->fused_slots : 0);
             if (!have_tma && want_impl == 2)
                 return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel unavailable: %s",
                                why ? why : "cuTensorMapEncodeTiled not found");
@@ -544,6 +546,7 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     if (P > 1 && ny / P < 2) { set_err(TDMA_ERR_INVALID_ARG, "partitions need >= 2 rows (ny/P = %d)", ny / P); return nullptr; }
     if (batch < 0 || batch > nz) { set_err(TDMA_ERR_INVALID_ARG, "batch = %d outside [0, nz = %d]", batch, nz); return nullptr; }
     if (dtype != TDMA_F64) { set_err(TDMA_ERR_UNSUPPORTED, "dtype %d: only TDMA_F64 is implemented", dtype); return nullptr; }
+    if (options && options->fused_slots != 0 && (options->fused_slots < 4 || options->fused_slots > 8)) { set_err(TDMA_ERR_INVALID_ARG, "fused_slots = %d must be 0 or 4 .. 8", options->fused_slots); return nullptr; }
     if (options && options->host_chunk < 0) { set_err(TDMA_ERR_INVALID_ARG, "host_chunk = %d must be >= 0", options->host_chunk); return nullptr; }
     if ((long long)nx * (batch ? batch : nz) > 0x7fffffffLL) { set_err(TDMA_ERR_UNSUPPORTED, "nx * batch exceeds 2^31-1 lines per batch"); return nullptr; }
     tdma_plan *pl = new (std::nothrow) tdma_plan();

@@ -226,7 +226,7 @@ def test_fused_top_modes_agree_with_pipelined_to_rounding():
     xs = [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1,
                     fused_top=top, fused_leaf_rows=leaf) for top, leaf in ((1, 0), (2, 0), (1, 32), (2, 4))]
     xs += [gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, fused_leaf_rows=leaf, fused_cluster=cl, **TMA)
-           for leaf, cl in ((0, 0), (2, 1), (16, 2), (4, 8))]
+           for leaf, cl in ((0, 0), (2, 8), (16, 2), (4, 8))]
     for x in xs:
         check_against_oracle(w.a, w.b, w.c, w.d, x, False)
 
@@ -328,7 +328,7 @@ def test_fused_rejects_what_it_cannot_tile():
 # TMA fused kernel: tilings (lines x cluster x leaf), ragged x tiles, alignment fallback
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("cluster,lines,leaf", [
-    (1, 16, 0), (1, 32, 2), (1, 8, 16), (1, 16, 4), (2, 16, 8), (2, 32, 4), (4, 16, 2), (4, 8, 16),
+    (1, 16, 0), (1, 16, 2), (1, 8, 16), (1, 16, 4), (2, 16, 8), (2, 32, 4), (4, 16, 2), (4, 8, 16),
     (8, 16, 8), (8, 32, 4), (8, 8, 2), (16, 16, 4), (16, 32, 2),
 ])
 def test_tma_fused_tilings(cluster, lines, leaf):
