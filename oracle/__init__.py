@@ -7,6 +7,8 @@ Plain CPU definition of the batched y-direction tridiagonal solve, used by ``tes
     (problem statement PAPER.md:127-131, 210), implemented in
     ``thomas_oracle.c`` (gcc, fp-contraction off so no FMA sneaks in).
   * ``residual_y`` / ``apply_y``                   -- long-double residual and d = A x.
+  * ``solve_y_shared``                             -- SURVEY 8(f) f3: 1-D coefficients shared by all
+    lines, diagonal shifted per line, real or complex right-hand sides.
   * ``thomas_line``                                -- the same recurrence as a pure-Python loop
     for one small line (brute-force cross-checks).
 
@@ -56,6 +58,8 @@ def _load():
         lib.oracle_residual_y.restype = ctypes.c_int
         lib.oracle_apply_y.argtypes = [ctypes.c_int] * 3 + [dp] * 5
         lib.oracle_apply_y.restype = ctypes.c_int
+        lib.oracle_solve_y_shared.argtypes = [ctypes.c_int] * 4 + [dp] * 5 + [ctypes.c_int] + [dp] * 2 + [ctypes.c_int]
+        lib.oracle_solve_y_shared.restype = ctypes.c_int
         lib.oracle_max_threads.restype = ctypes.c_int
         lib.oracle_set_threads.argtypes = [ctypes.c_int]
         _lib = lib
@@ -185,3 +189,34 @@ def solve_axis(a, b, c, d, axis: str = "y", periodic: bool = False, precision: s
         arrs = [np.ascontiguousarray(t.transpose(perm)) for t in arrs]
     x = (solve_cyclic_y if periodic else solve_y)(*arrs, precision)
     return np.ascontiguousarray(x.transpose(perm)) if perm else x
+
+
+# ---------------------------------------------------------------------------------------------
+# shared coefficients, complex right-hand sides
+# ---------------------------------------------------------------------------------------------
+def solve_y_shared(a_y, b0_y, c_y, sx, sz, d, pin00: bool = False, precision: str = "f64") -> np.ndarray:
+    """Lines along y whose matrix is given by 1-D arrays: a_j = a_y[j], c_j = c_y[j],
+    b_j = b0_y[j] - (sx[i] + sz[k]) for line (i, k) (PAPER.md:286: (d2/dy2 - k_l - k_m) Phi = Q;
+    PAPER.md:318: the matrix depends solely on grid spacing).  ``d`` has shape (nz, ny, nx), real
+    or complex (complex-valued data, real coefficients: each of re / im is a
+    right-hand side of the same matrix).  pin00: row 0 of line (0, 0) is b = 1, c = 0.
+    Plain Thomas per line and component (thomas_oracle.c: oracle_solve_y_shared).
+    Pinned in tests/test_oracle_pins.py: bit-equal to ``solve_y`` on the materialised arrays,
+    dense LAPACK solve of the complex system for n <= 32, Toeplitz eigen-form with a shift."""
+    a_y, b0_y, c_y, sx, sz = [np.ascontiguousarray(np.asarray(t, dtype=np.float64)) for t in (a_y, b0_y, c_y, sx, sz)]
+    d = np.asarray(d)
+    cplx = np.iscomplexobj(d)
+    d = np.ascontiguousarray(d, dtype=np.complex128 if cplx else np.float64)
+    if d.ndim != 3:
+        raise ValueError("expected d of shape (nz, ny, nx)")
+    nz, ny, nx = d.shape
+    if a_y.shape != (ny,) or b0_y.shape != (ny,) or c_y.shape != (ny,) or sx.shape != (nx,) or sz.shape != (nz,):
+        raise ValueError("coefficient arrays must have lengths ny, ny, ny, nx, nz")
+    x = np.empty_like(d)
+    dv, xv = d.view(np.float64), x.view(np.float64)
+    rc = _load().oracle_solve_y_shared(nx, ny, nz, 2 if cplx else 1, _ptr(a_y), _ptr(b0_y), _ptr(c_y), _ptr(sx),
+                                       _ptr(sz), 1 if pin00 else 0, _ptr(dv), _ptr(xv),
+                                       {"f64": 0, "ld": 1}[precision])
+    if rc != 0:
+        raise RuntimeError("oracle_solve_y_shared failed (%d)" % rc)
+    return x

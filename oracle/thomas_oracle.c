@@ -186,3 +186,58 @@ int oracle_apply_y(int nx, int ny, int nz, const double *a, const double *b, con
     }
     return 0;
 }
+
+/* Shared-coefficient lines.  The paper's own workload: the coefficient
+ * matrix "depends solely on grid spacing", the FFT-reduced Poisson operator is
+ * (d^2/dy^2 - k_l - k_m) and the fields are complex with real coefficients
+ * (PAPER.md:377, 383).  So a, c and the y-part of the diagonal are 1-D arrays of length ny and
+ * line (i,k) has
+ *        a_j = a_y[j],   c_j = c_y[j],   b_j = b0_y[j] - (sx[i] + sz[k]),
+ * the shift s = sx[i] + sz[k] being formed once per line, in fp64, before it is subtracted.
+ * d and x hold ncomp (1 = real, 2 = complex, interleaved re/im) values per cell, element
+ * (i,j,k,q) at q + ncomp*(i + nx*(j + ny*k)); every component is a separate right-hand side of
+ * the same real matrix.  pin00 != 0: row 0 of line (0,0) is replaced by b = 1, c = 0 (the
+ * singular mean mode pinned by x_0 = d_0, BASELINE cfg 2/3).  Still the plain Thomas algorithm
+ * per line and component: nothing is shared between lines, nothing is precomputed. */
+int oracle_solve_y_shared(int nx, int ny, int nz, int ncomp, const double *a_y, const double *b0_y,
+                          const double *c_y, const double *sx, const double *sz, int pin00,
+                          const double *d, double *x, int use_ld)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || ncomp < 1 || ncomp > 2 || !a_y || !b0_y || !c_y || !sx || !sz || !d || !x)
+        return -1;
+    int fail = 0;
+    const long nlines = (long)nx * nz;
+#pragma omp parallel
+    {
+        double *buf = (double *)malloc(sizeof(double) * 5 * (size_t)ny);
+        void *work = malloc((use_ld ? sizeof(long double) : sizeof(double)) * 2 * (size_t)ny);
+        if (!buf || !work) {
+#pragma omp atomic write
+            fail = 1;
+        }
+        double *la = buf, *lb = buf + ny, *lc = buf + 2 * ny, *ld = buf + 3 * ny, *lx = buf + 4 * ny;
+#pragma omp for schedule(static)
+        for (long line = 0; line < nlines; ++line) {
+            if (!buf || !work) continue;
+            const long i = line % nx, k = line / nx;
+            const double s = sx[i] + sz[k];
+            for (int j = 0; j < ny; ++j) { la[j] = a_y[j]; lb[j] = b0_y[j] - s; lc[j] = c_y[j]; }
+            la[0] = 0.0;
+            lc[ny - 1] = 0.0;
+            if (pin00 && i == 0 && k == 0) { lb[0] = 1.0; lc[0] = 0.0; }
+            for (int q = 0; q < ncomp; ++q) {
+                const size_t base = (size_t)q + (size_t)ncomp * ((size_t)i + (size_t)nx * (size_t)ny * (size_t)k);
+                const size_t step = (size_t)ncomp * (size_t)nx;
+                for (int j = 0; j < ny; ++j) ld[j] = d[base + step * (size_t)j];
+                if (use_ld)
+                    thomas_line_ld(ny, la, lb, lc, ld, lx, (long double *)work, (long double *)work + ny);
+                else
+                    thomas_line_f64(ny, la, lb, lc, ld, lx, (double *)work, (double *)work + ny);
+                for (int j = 0; j < ny; ++j) x[base + step * (size_t)j] = lx[j];
+            }
+        }
+        free(buf);
+        free(work);
+    }
+    return fail ? -1 : 0;
+}

@@ -390,3 +390,87 @@ def test_f1_solve_axis_x_is_the_transposed_problem():
     xp = oracle.solve_axis(a, b, c, d, "x", periodic=True)
     ref = np.linalg.solve(_cyclic_dense(a[1, 2], b[1, 2], c[1, 2]), d[1, 2])
     assert np.max(np.abs(xp[1, 2] - ref)) <= 1e-14
+
+
+# ----------------------------------------------------------------------------------------------
+# shared coefficients, complex right-hand sides
+# ----------------------------------------------------------------------------------------------
+def _shared_case(rng, nz, ny, nx, cplx):
+    a_y, c_y = rng.uniform(-1, 1, ny), rng.uniform(-1, 1, ny)
+    b0_y = 2.5 + rng.uniform(0, 1, ny)
+    sx, sz = -rng.uniform(0, 2, nx), -rng.uniform(0, 2, nz)         # b = b0 - (sx + sz) >= 2.5
+    d = rng.normal(size=(nz, ny, nx))
+    if cplx:
+        d = d + 1j * rng.normal(size=(nz, ny, nx))
+    return a_y, b0_y, c_y, sx, sz, d
+
+
+def _materialise(a_y, b0_y, c_y, sx, sz, nz, ny, nx, pin00=False):
+    a = np.ascontiguousarray(np.broadcast_to(a_y[None, :, None], (nz, ny, nx)))
+    c = np.ascontiguousarray(np.broadcast_to(c_y[None, :, None], (nz, ny, nx)))
+    b = b0_y[None, :, None] - (sx[None, None, :] + sz[:, None, None])
+    if pin00:
+        b[0, 0, 0] = 1.0
+        c[0, 0, 0] = 0.0
+    return a, b, c
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("precision", ["f64", "ld"])
+@pytest.mark.parametrize("pin00", [False, True])
+def test_f3_shared_equals_materialised_bit_for_bit(cplx, precision, pin00):
+    rng = np.random.default_rng(31)
+    nz, ny, nx = 3, 24, 5
+    a_y, b0_y, c_y, sx, sz, d = _shared_case(rng, nz, ny, nx, cplx)
+    x = oracle.solve_y_shared(a_y, b0_y, c_y, sx, sz, d, pin00=pin00, precision=precision)
+    a, b, c = _materialise(a_y, b0_y, c_y, sx, sz, nz, ny, nx, pin00)
+    assert x.dtype == d.dtype and x.shape == d.shape
+    if cplx:
+        assert np.array_equal(x.real, oracle.solve_y(a, b, c, d.real, precision))
+        assert np.array_equal(x.imag, oracle.solve_y(a, b, c, d.imag, precision))
+    else:
+        assert np.array_equal(x, oracle.solve_y(a, b, c, d, precision))
+    if pin00:
+        assert x[0, 0, 0] == d[0, 0, 0]
+
+
+@pytest.mark.parametrize("n", [2, 3, 7, 16, 32])
+def test_f3_shared_complex_vs_dense_lapack(n):
+    """Every line as a dense complex system (np.linalg.solve = LAPACK zgesv): a wrong shift
+    index (sx/sz swapped), a shift with the wrong sign or re/im mixed up all fail here."""
+    rng = np.random.default_rng(100 + n)
+    nz, nx = 3, 4
+    a_y, b0_y, c_y, sx, sz, d = _shared_case(rng, nz, n, nx, True)
+    x = oracle.solve_y_shared(a_y, b0_y, c_y, sx, sz, d)
+    for k in range(nz):
+        for i in range(nx):
+            A = np.zeros((n, n))
+            for j in range(n):
+                A[j, j] = b0_y[j] - sx[i] - sz[k]
+                if j > 0:
+                    A[j, j - 1] = a_y[j]
+                if j < n - 1:
+                    A[j, j + 1] = c_y[j]
+            ref = np.linalg.solve(A.astype(np.complex128), d[k, :, i])
+            assert np.max(np.abs(x[k, :, i] - ref)) <= 1e-13 * np.max(np.abs(ref))
+
+
+@pytest.mark.parametrize("alpha,n", [(0.3, 17), (4.0, 64)])
+def test_f3_shared_toeplitz_eigenform_with_shift(alpha, n):
+    """a = c = -alpha, b0 = 1 + 2 alpha, shift s = sx + sz: d = z sin(pi q j/(n+1)) with a complex
+    amplitude z is an eigenvector, x = d / (lambda_q - s)."""
+    nz, nx = 2, 3
+    sx, sz = -np.array([0.0, 0.5, 2.0]), -np.array([0.0, 1.25])
+    j = np.arange(1, n + 1)
+    d = np.empty((nz, n, nx), dtype=np.complex128)
+    ref = np.empty_like(d)
+    for k in range(nz):
+        for i in range(nx):
+            q = 1 + (3 * k + i) % n
+            mode = np.sin(np.pi * q * j / (n + 1))
+            lam = 1 + 2 * alpha - 2 * alpha * np.cos(np.pi * q / (n + 1))
+            z = complex(1.0 + i, -2.0 + k)
+            d[k, :, i] = z * mode
+            ref[k, :, i] = z * mode / (lam - (sx[i] + sz[k]))
+    x = oracle.solve_y_shared(np.full(n, -alpha), np.full(n, 1 + 2 * alpha), np.full(n, -alpha), sx, sz, d)
+    assert np.max(np.abs(x - ref)) <= (1 + 4 * alpha) * 4e-15 * np.max(np.abs(ref))
