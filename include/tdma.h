@@ -114,6 +114,11 @@ typedef struct tdma_options {
                             memory holds, at most 8) */
     int host_chunk;      /* tdma_solve_host: z-slices per host chunk (0 = auto, about 16 Mi cells;
                             PIPELINED plans round it to whole batches) */
+    int shared_lines;    /* tdma_solve_shared: cells along x per tile (real: 16 or 32, complex: 8 or 16),
+                            0 = auto (128-byte row segments) */
+    int shared_cluster;  /* tdma_solve_shared: CTAs per cluster (1, 2, 4, 8), 0 = auto */
+    int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16), 0 = auto */
+    int shared_slots;    /* tdma_solve_shared: tiles in the shared-memory ring (2 .. 4), 0 = auto */
 } tdma_options;
 
 enum { TDMA_AXIS_Y = 0, TDMA_AXIS_X = 1, TDMA_AXIS_Z = 2 };
@@ -132,6 +137,30 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
  * Enqueue-only; returns TDMA_OK or a negative status. */
 int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,
                void *x, void *stream);
+
+/* Shared-coefficient / complex right-hand-side solve -- the paper's own
+ * benchmark configuration: "3D complex-valued data", a coefficient matrix
+ * that "depends solely on grid spacing", shared by all systems, with the
+ * FFT-reduced Poisson operator (d2/dy2 - k_l - k_m) Phi = Q.  Line (i,k) solves
+ *
+ *     a_y[j] x_{j-1} + (b0_y[j] - (sx[i] + sz[k])) x_j + c_y[j] x_{j+1} = d_j ,   j = 0 .. ny-1,
+ *
+ * the shift s = sx[i] + sz[k] being formed in fp64 before it is subtracted from b0_y[j].
+ * a_y, b0_y, c_y: DEVICE pointers to ny doubles (a_y[0], c_y[ny-1] ignored); sx: nx doubles; sz: nz
+ * doubles.  ncomp = 1: d, x hold nx*ny*nz doubles (layout above); ncomp = 2: complex cells,
+ * interleaved (re, im), component q of cell (i,j,k) at q + 2*(i + nx*(j + ny*k)); the matrix is
+ * real, so re and im are two right-hand sides of the same system.  pin00 != 0: row 0 of line
+ * (0,0) is replaced by b = 1, c = 0 (the singular mean mode of the Poisson problem pinned to
+ * x_0 = d_0, BASELINE cfg 2/3).  d, x: DEVICE pointers, 16-byte aligned; x may alias d exactly.
+ * HBM traffic: d read once, x written once (16 B per real cell, 32 B per complex cell); the
+ * matrix is rebuilt on chip.  Any plan with lines along y and no cyclic coupling can be used
+ * (nx, ny, nz are the plan's; P and batch are not used: the line is cut into the kernel's own
+ * leaves, D1); one persistent launch (plus the fill launch, see fused_fill) per call.
+ * TDMA_ERR_UNSUPPORTED when ny does not tile (ny = CL * W * M0, CL in 1,2,4,8, W a power of two
+ * <= 32, M0 in 4,8,16) or nx*ncomp is odd.  Enqueue-only. */
+int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const void *c_y,
+                      const void *sx, const void *sz, int ncomp, int pin00, const void *d, void *x,
+                      void *stream);
 
 /* Same solve with HOST buffers: the slab is streamed through plan-owned device staging buffers
  * in z-chunks (H2D copy of chunk n+1 and D2H copy of chunk n-1 overlap the solve of chunk n).
@@ -171,7 +200,11 @@ typedef enum tdma_query {
     TDMA_GET_FUSED_SMEM = 13,      /* dynamic shared memory per CTA, bytes          */
     TDMA_GET_FUSED_TOP_ROWS = 14,  /* rows of the cluster-level system per line     */
     TDMA_GET_FUSED_IMPL = 15,      /* resolved fused_impl                           */
-    TDMA_GET_FUSED_FILL = 16       /* z-slices of the last solve given to the fill launch */
+    TDMA_GET_FUSED_FILL = 16,      /* z-slices of the last solve given to the fill launch */
+    /* tiling of the last tdma_solve_shared (0 before the first one) */
+    TDMA_GET_SHARED_LINES = 17, TDMA_GET_SHARED_CLUSTER = 18, TDMA_GET_SHARED_LEAF_ROWS = 19,
+    TDMA_GET_SHARED_THREADS = 20, TDMA_GET_SHARED_SMEM = 21, TDMA_GET_SHARED_SLOTS = 22,
+    TDMA_GET_SHARED_FILL = 23      /* z-slices its fill launch took */
 } tdma_query;
 int tdma_plan_get(const tdma_plan *plan, int what); /* < 0 on error */
 size_t tdma_plan_workspace_bytes(const tdma_plan *plan); /* device bytes the plan owns */

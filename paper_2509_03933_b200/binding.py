@@ -25,13 +25,16 @@ TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
 (TDMA_GET_NB, TDMA_GET_M, TDMA_GET_BATCH, TDMA_GET_NSTREAMS, TDMA_GET_DEPTH, TDMA_GET_VARIANT,
  TDMA_GET_LAUNCHES, TDMA_GET_FUSED_LINES, TDMA_GET_FUSED_CLUSTER, TDMA_GET_GRAPH_BUILDS,
  TDMA_GET_FUSED_LEAF_ROWS, TDMA_GET_FUSED_TOP, TDMA_GET_FUSED_THREADS, TDMA_GET_FUSED_SMEM,
- TDMA_GET_FUSED_TOP_ROWS, TDMA_GET_FUSED_IMPL, TDMA_GET_FUSED_FILL) = range(17)
+ TDMA_GET_FUSED_TOP_ROWS, TDMA_GET_FUSED_IMPL, TDMA_GET_FUSED_FILL, TDMA_GET_SHARED_LINES,
+ TDMA_GET_SHARED_CLUSTER, TDMA_GET_SHARED_LEAF_ROWS, TDMA_GET_SHARED_THREADS, TDMA_GET_SHARED_SMEM,
+ TDMA_GET_SHARED_SLOTS, TDMA_GET_SHARED_FILL) = range(24)
 (TDMA_BUF_RA, TDMA_BUF_RC, TDMA_BUF_RD, TDMA_BUF_Y, TDMA_BUF_SA, TDMA_BUF_SC, TDMA_BUF_SD) = range(7)
 
 EXPORTED_SYMBOLS = (
     "tdma_plan_create", "tdma_plan_create_ex", "tdma_solve", "tdma_solve_host", "tdma_stage",
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
     "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
+    "tdma_solve_shared",
 )
 
 
@@ -43,6 +46,8 @@ class tdma_options(ctypes.Structure):
         ("fused_leaf_rows", ctypes.c_int), ("fused_top", ctypes.c_int),
         ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("axis", ctypes.c_int), ("periodic", ctypes.c_int),
         ("timeline", ctypes.c_int), ("fused_slots", ctypes.c_int), ("host_chunk", ctypes.c_int),
+        ("shared_lines", ctypes.c_int), ("shared_cluster", ctypes.c_int), ("shared_leaf_rows", ctypes.c_int),
+        ("shared_slots", ctypes.c_int),
     ]
 
 
@@ -84,6 +89,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_plan_create_ex.restype = vp
     lib.tdma_solve.argtypes = [vp] * 7
     lib.tdma_solve.restype = ci
+    lib.tdma_solve_shared.argtypes = [vp] * 6 + [ci, ci] + [vp] * 3
+    lib.tdma_solve_shared.restype = ci
     lib.tdma_solve_host.argtypes = [vp] * 6
     lib.tdma_solve_host.restype = ci
     lib.tdma_stage.argtypes = [vp, ci, ci] + [vp] * 6
@@ -156,7 +163,9 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
                         variant: int = 0, nstreams: int = 0, use_graph: int = 0,
                         separate_gather: int = 0, fused_lines: int = 0, fused_cluster: int = 0,
                         fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0,
-                        axis: int = 0, periodic: int = 0, timeline: int = 0, fused_slots: int = 0, host_chunk: int = 0) -> int:
+                        axis: int = 0, periodic: int = 0, timeline: int = 0, fused_slots: int = 0, host_chunk: int = 0,
+                        shared_lines: int = 0, shared_cluster: int = 0, shared_leaf_rows: int = 0,
+                        shared_slots: int = 0) -> int:
     opt = tdma_options()
     opt.struct_size = ctypes.sizeof(tdma_options)
     opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
@@ -164,6 +173,7 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
     opt.fused_leaf_rows, opt.fused_top, opt.fused_impl = fused_leaf_rows, fused_top, fused_impl
     opt.fused_fill, opt.axis, opt.periodic, opt.timeline = fused_fill, axis, periodic, timeline
     opt.host_chunk, opt.fused_slots = host_chunk, fused_slots
+    opt.shared_lines, opt.shared_cluster, opt.shared_leaf_rows, opt.shared_slots = shared_lines, shared_cluster, shared_leaf_rows, shared_slots
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
         raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())
@@ -173,6 +183,11 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
 def tdma_solve(plan: int, a, b, c, d, x, stream=None) -> None:
     _check(load_library().tdma_solve(plan, _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(x),
                                      _stream_handle(stream)))
+
+
+def tdma_solve_shared(plan: int, a_y, b0_y, c_y, sx, sz, ncomp: int, pin00: int, d, x, stream=None) -> None:
+    _check(load_library().tdma_solve_shared(plan, _ptr(a_y), _ptr(b0_y), _ptr(c_y), _ptr(sx), _ptr(sz),
+                                            int(ncomp), int(pin00), _ptr(d), _ptr(x), _stream_handle(stream)))
 
 
 def tdma_solve_host(plan: int, a, b, c, d, x) -> None:
@@ -251,6 +266,19 @@ class Plan:
     def solve(self, a, b, c, d, x, stream=None):
         self._validate((a, b, c, d, x))
         tdma_solve(self.handle, a, b, c, d, x, stream)
+        return x
+
+    def solve_shared(self, a_y, b0_y, c_y, sx, sz, d, x, pin00: bool = False, stream=None):
+        """Shared-coefficient solve; d, x real (nz, ny, nx) fp64 or complex128 tensors."""
+        nz, ny, nx = self.shape
+        ncomp = 2 if (hasattr(d, "is_complex") and d.is_complex()) else 1
+        for t, n in ((a_y, ny), (b0_y, ny), (c_y, ny), (sx, nx), (sz, nz)):
+            if t.numel() != n or not t.is_contiguous() or t.element_size() != 8:
+                raise ValueError("coefficient arrays must be contiguous fp64 of lengths ny, ny, ny, nx, nz")
+        for t in (d, x):
+            if t.numel() != nz * ny * nx or not t.is_contiguous() or t.element_size() != 8 * ncomp:
+                raise ValueError("d, x must be contiguous with nz*ny*nx cells of %d bytes" % (8 * ncomp))
+        tdma_solve_shared(self.handle, a_y, b0_y, c_y, sx, sz, ncomp, 1 if pin00 else 0, d, x, stream)
         return x
 
     def solve_host(self, a, b, c, d, x):

@@ -217,10 +217,35 @@ struct Eq { double a, b, c, d; };
 //   AB[row][line] = (A, B)   and   CD[row][line] = (C, D),   CD plane `plane` bytes after AB.
 // The lanes of a warp work on consecutive lines of the same row: conflict-free.  A row the tree
 // eliminated keeps (a, c) in its AB slot and d (later x) in the D half of its CD slot.
-struct NodeBuf { uint32_t ab, plane; };
+// NC = 2 (two right-hand sides of the same matrix: the re / im parts of a complex field,
+// tdma_shared_tma.cuh) adds a third plane of 8-byte entries, D1[row][line] at `d1`.
+struct NodeBuf { uint32_t ab, plane, d1; };
 
 template <int TX>
 __device__ __forceinline__ uint32_t nb_ab(const NodeBuf &nb, int row, int lx) { return nb.ab + (uint32_t)(row * TX + lx) * 16u; }
+
+// address of the D1 entry that belongs to the AB slot at address o
+__device__ __forceinline__ uint32_t nb_d1(const NodeBuf &nb, uint32_t o) { return nb.d1 + ((o - nb.ab) >> 1); }
+
+// the right-hand side(s) of the row whose AB slot is at o: cd = its CD pair, already loaded
+template <int NC>
+__device__ __forceinline__ void nb_load_d(const NodeBuf &nb, uint32_t o, const double2 &cd, double (&d)[NC])
+{
+    d[0] = cd.y;
+    if (NC == 2) d[NC - 1] = lds1(nb_d1(nb, o));
+}
+template <int NC>
+__device__ __forceinline__ void nb_store_d(const NodeBuf &nb, uint32_t o, const double (&d)[NC])
+{
+    sts1(o + nb.plane + 8, d[0]);
+    if (NC == 2) sts1(nb_d1(nb, o), d[NC - 1]);
+}
+template <int NC>
+__device__ __forceinline__ void nb_load_donly(const NodeBuf &nb, uint32_t o, double (&d)[NC])
+{
+    d[0] = lds1(o + nb.plane + 8);
+    if (NC == 2) d[NC - 1] = lds1(nb_d1(nb, o));
+}
 
 // ------------------------------------------------------------------------------------------
 // K-ary merge of boundary equations (the levels above the leaves, and the cluster-level system
@@ -246,93 +271,116 @@ __device__ __forceinline__ uint32_t nb_ab(const NodeBuf &nb, int row, int lx) { 
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ int krow(int g, int k, int S, int i) { return (g * k + (i >> 1)) * S + ((i & 1) ? S - 1 : 0); }
 
-template <int TX, int K>
+template <int TX, int K, int NC = 1>
 __device__ __forceinline__ void kmerge_fwd(const NodeBuf &nb, int lx, int g, int S, int kk)
 {
     const int k = K > 0 ? K : kk;
     uint32_t o = nb_ab<TX>(nb, krow(g, k, S, 1), lx);
     double2 ab = lds2(o), cd = lds2(o + nb.plane);
-    double al = ab.x, be = ab.y, ga = cd.x, de = cd.y;
+    double al = ab.x, be = ab.y, ga = cd.x, de[NC], dn[NC];
+    nb_load_d<NC>(nb, o, cd, de);
     o = nb_ab<TX>(nb, krow(g, k, S, 2), lx);
-    ab = lds2(o); cd = lds2(o + nb.plane);
+    ab = lds2(o); cd = lds2(o + nb.plane); nb_load_d<NC>(nb, o, cd, dn);
 #pragma unroll
     for (int i = 2; i < 2 * k; ++i) {
-        const double s = ab.x, b = ab.y, c = cd.x, d = cd.y;
+        const double s = ab.x, b = ab.y, c = cd.x;
+        double d[NC];
+#pragma unroll
+        for (int q = 0; q < NC; ++q) d[q] = dn[q];
         if (i + 1 < 2 * k) {                                  // next row's loads go out first
             o = nb_ab<TX>(nb, krow(g, k, S, i + 1), lx);
-            ab = lds2(o); cd = lds2(o + nb.plane);
+            ab = lds2(o); cd = lds2(o + nb.plane); nb_load_d<NC>(nb, o, cd, dn);
         }
-        const double nbe = fma(be, b, -(s * ga)), nde = fma(be, d, -(s * de));
+        const double nbe = fma(be, b, -(s * ga));
         const double sc = pow2_unscale(nbe);
-        al = -(s * al) * sc; ga = be * c * sc; de = nde * sc; be = nbe * sc;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) de[q] = fma(be, d[q], -(s * de[q])) * sc;
+        al = -(s * al) * sc; ga = be * c * sc; be = nbe * sc;
     }
-    sts2(o, al, be); sts2(o + nb.plane, ga, de);              // o: the group's last row
+    sts2(o, al, be); sts2(o + nb.plane, ga, de[0]);           // o: the group's last row
+    if (NC == 2) sts1(nb_d1(nb, o), de[NC - 1]);
 }
 
-template <int TX, int K>
+template <int TX, int K, int NC = 1>
 __device__ __forceinline__ void kmerge_bwd(const NodeBuf &nb, int lx, int g, int S, int kk)
 {
     const int k = K > 0 ? K : kk;
     uint32_t o = nb_ab<TX>(nb, krow(g, k, S, 2 * k - 2), lx);
     double2 ab = lds2(o), cd = lds2(o + nb.plane);
-    double al = ab.x, be = ab.y, ga = cd.x, de = cd.y;
+    double al = ab.x, be = ab.y, ga = cd.x, de[NC], dn[NC];
+    nb_load_d<NC>(nb, o, cd, de);
     o = nb_ab<TX>(nb, krow(g, k, S, 2 * k - 3), lx);
-    ab = lds2(o); cd = lds2(o + nb.plane);
+    ab = lds2(o); cd = lds2(o + nb.plane); nb_load_d<NC>(nb, o, cd, dn);
 #pragma unroll
     for (int i = 2 * k - 3; i >= 0; --i) {
-        const double s = ab.x, b = ab.y, c = cd.x, d = cd.y;
+        const double s = ab.x, b = ab.y, c = cd.x;
+        double d[NC];
+#pragma unroll
+        for (int q = 0; q < NC; ++q) d[q] = dn[q];
         if (i > 0) {
             o = nb_ab<TX>(nb, krow(g, k, S, i - 1), lx);
-            ab = lds2(o); cd = lds2(o + nb.plane);
+            ab = lds2(o); cd = lds2(o + nb.plane); nb_load_d<NC>(nb, o, cd, dn);
         }
-        const double nbe = fma(be, b, -(c * al)), nde = fma(be, d, -(c * de));
+        const double nbe = fma(be, b, -(c * al));
         const double sc = pow2_unscale(nbe);
-        ga = -(c * ga) * sc; al = be * s * sc; de = nde * sc; be = nbe * sc;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) de[q] = fma(be, d[q], -(c * de[q])) * sc;
+        ga = -(c * ga) * sc; al = be * s * sc; be = nbe * sc;
     }
-    sts2(o, al, be); sts2(o + nb.plane, ga, de);              // o: the group's first row
+    sts2(o, al, be); sts2(o + nb.plane, ga, de[0]);           // o: the group's first row
+    if (NC == 2) sts1(nb_d1(nb, o), de[NC - 1]);
 }
 
 // Interior rows i = 1 .. 2K-2 of a group, from their ORIGINAL equations (the merge sweeps only
 // read them): modified Thomas forward sweep with u_0 as a parameter (normalised; this runs off
 // the serial chain), then the backward sweep into
 //     u_i = d_i - a_i u_0 - c_i u_{2K-1} :   AB slot <- (a, c),  D <- d.
-template <int TX, int K>
+template <int TX, int K, int NC = 1>
 __device__ __forceinline__ void kmerge_tails(const NodeBuf &nb, int lx, int g, int S, int kk)
 {
     const int k = K > 0 ? K : kk;
-    double a = 0.0, c = 0.0, d = 0.0;
+    double a = 0.0, c = 0.0, d[NC];
+#pragma unroll
+    for (int q = 0; q < NC; ++q) d[q] = 0.0;
     for (int i = 1; i <= 2 * k - 2; ++i) {
         const uint32_t o = nb_ab<TX>(nb, krow(g, k, S, i), lx);
         const double2 ab = lds2(o), cd = lds2(o + nb.plane);
+        double di[NC];
+        nb_load_d<NC>(nb, o, cd, di);
         if (i == 1) {
             const double inv = rcp_nr(ab.y);
-            a = ab.x * inv; c = cd.x * inv; d = cd.y * inv;
+            a = ab.x * inv; c = cd.x * inv;
+#pragma unroll
+            for (int q = 0; q < NC; ++q) d[q] = di[q] * inv;
         } else {
             const double inv = rcp_nr(fma(-ab.x, c, ab.y));
-            d = fma(-ab.x, d, cd.y) * inv;
+#pragma unroll
+            for (int q = 0; q < NC; ++q) d[q] = fma(-ab.x, d[q], di[q]) * inv;
             a = -(ab.x * a) * inv;
             c = cd.x * inv;
         }
-        sts2(o, a, c); sts1(o + nb.plane + 8, d);
+        sts2(o, a, c); nb_store_d<NC>(nb, o, d);
     }
     // a, c, d: row 2K-2, already in final form
     for (int i = 2 * k - 3; i >= 1; --i) {
         const uint32_t o = nb_ab<TX>(nb, krow(g, k, S, i), lx);
         const double2 ac = lds2(o);
-        const double di = lds1(o + nb.plane + 8);
-        d = fma(-ac.y, d, di);
+        double di[NC];
+        nb_load_donly<NC>(nb, o, di);
+#pragma unroll
+        for (int q = 0; q < NC; ++q) d[q] = fma(-ac.y, d[q], di[q]);
         a = fma(-ac.y, a, ac.x);
         c = -(ac.y * c);
-        sts2(o, a, c); sts1(o + nb.plane + 8, d);
+        sts2(o, a, c); nb_store_d<NC>(nb, o, d);
     }
 }
 
 // The same in two steps for a HELPER thread that runs concurrently with the merge sweeps of the
 // same level: kmerge_tails_regs reads the 2K-2 interior rows and leaves (a, c, d) in registers,
 // kmerge_tails_store writes them back once the sweeps no longer read the rows.
-template <int TX, int K>
+template <int TX, int K, int NC = 1>
 __device__ __forceinline__ void kmerge_tails_regs(const NodeBuf &nb, int lx, int g, int S, double (&a)[6], double (&c)[6],
-                                                  double (&d)[6])
+                                                  double (&d)[6][NC])
 {
     constexpr int NI = 2 * K - 2;
     double2 ab[NI], cd[NI];
@@ -340,36 +388,55 @@ __device__ __forceinline__ void kmerge_tails_regs(const NodeBuf &nb, int lx, int
     for (int j = 0; j < NI; ++j) {
         const uint32_t o = nb_ab<TX>(nb, krow(g, K, S, j + 1), lx);
         ab[j] = lds2(o); cd[j] = lds2(o + nb.plane);
+        nb_load_d<NC>(nb, o, cd[j], d[j]);
     }
     double inv = rcp_nr(ab[0].y);
-    a[0] = ab[0].x * inv; c[0] = cd[0].x * inv; d[0] = cd[0].y * inv;
+    a[0] = ab[0].x * inv; c[0] = cd[0].x * inv;
+#pragma unroll
+    for (int q = 0; q < NC; ++q) d[0][q] *= inv;
 #pragma unroll
     for (int j = 1; j < NI; ++j) {
         inv = rcp_nr(fma(-ab[j].x, c[j - 1], ab[j].y));
-        d[j] = fma(-ab[j].x, d[j - 1], cd[j].y) * inv;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) d[j][q] = fma(-ab[j].x, d[j - 1][q], d[j][q]) * inv;
         a[j] = -(ab[j].x * a[j - 1]) * inv;
         c[j] = cd[j].x * inv;
     }
 #pragma unroll
     for (int j = NI - 2; j >= 0; --j) {
-        d[j] = fma(-c[j], d[j + 1], d[j]);
+#pragma unroll
+        for (int q = 0; q < NC; ++q) d[j][q] = fma(-c[j], d[j + 1][q], d[j][q]);
         a[j] = fma(-c[j], a[j + 1], a[j]);
         c[j] = -(c[j] * c[j + 1]);
     }
 }
 
-template <int TX, int K>
+template <int TX, int K, int NC = 1>
 __device__ __forceinline__ void kmerge_tails_store(const NodeBuf &nb, int lx, int g, int S, const double (&a)[6],
-                                                   const double (&c)[6], const double (&d)[6])
+                                                   const double (&c)[6], const double (&d)[6][NC])
 {
 #pragma unroll
     for (int j = 0; j < 2 * K - 2; ++j) {
         const uint32_t o = nb_ab<TX>(nb, krow(g, K, S, j + 1), lx);
-        sts2(o, a[j], c[j]); sts1(o + nb.plane + 8, d[j]);
+        sts2(o, a[j], c[j]); nb_store_d<NC>(nb, o, d[j]);
     }
 }
 
 // u_i of a group (i = 0 .. 2k-1) from the group's x_first / x_last.
+template <int TX, int NC = 1>
+__device__ __forceinline__ void kmerge_value_n(const NodeBuf &nb, int lx, int g, int S, int k, int i,
+                                               const double (&xf)[NC], const double (&xl)[NC], double (&out)[NC])
+{
+#pragma unroll
+    for (int q = 0; q < NC; ++q) out[q] = i == 0 ? xf[q] : xl[q];
+    if (i == 0 || i == 2 * k - 1) return;
+    const uint32_t o = nb_ab<TX>(nb, krow(g, k, S, i), lx);
+    const double2 ac = lds2(o);
+    double di[NC];
+    nb_load_donly<NC>(nb, o, di);
+#pragma unroll
+    for (int q = 0; q < NC; ++q) out[q] = fma(-ac.y, xl[q], fma(-ac.x, xf[q], di[q]));
+}
 template <int TX>
 __device__ __forceinline__ double kmerge_value(const NodeBuf &nb, int lx, int g, int S, int k, int i, double xf, double xl)
 {
@@ -387,39 +454,54 @@ __device__ __forceinline__ double kmerge_value(const NodeBuf &nb, int lx, int g,
 //     backward  al u_{i-1} + bb u_i = dd ,  i = n-1 .. p+1  (bb_i = bb_{i+1} b_i - c_i al_{i+1}, ...)
 // and solves the remaining 2 x 2 system.  The two sweeps are independent chains of p and n-2-p
 // steps that run interleaved in one thread; one reciprocal in total.
-template <int TX>
-__device__ __forceinline__ void cluster_solve_two_sided(const NodeBuf &tb, int lx, int n, int p, double &up, double &up1)
+template <int TX, int NC = 1>
+__device__ __forceinline__ void cluster_solve_two_sided(const NodeBuf &tb, int lx, int n, int p, double (&up)[NC], double (&up1)[NC])
 {
     uint32_t of = nb_ab<TX>(tb, 0, lx), ob = nb_ab<TX>(tb, n - 1, lx);
     const uint32_t step = TX * 16u;
     double2 t0 = lds2(of), t1 = lds2(of + tb.plane), t2 = lds2(ob), t3 = lds2(ob + tb.plane);
-    double be = t0.y, ga = t1.x, de = t1.y;             // row 0
-    double al = t2.x, bb = t2.y, dd = t3.y;             // row n-1
+    double be = t0.y, ga = t1.x, de[NC];                // row 0
+    double al = t2.x, bb = t2.y, dd[NC];                // row n-1
+    nb_load_d<NC>(tb, of, t1, de);
+    nb_load_d<NC>(tb, ob, t3, dd);
     const int nf = p, nbk = n - 2 - p;
     const int nmax = nf > nbk ? nf : nbk;
     double2 fab = make_double2(0.0, 1.0), fcd = make_double2(0.0, 0.0), bab = fab, bcd = fcd;
-    if (nf > 0) { of += step; fab = lds2(of); fcd = lds2(of + tb.plane); }
-    if (nbk > 0) { ob -= step; bab = lds2(ob); bcd = lds2(ob + tb.plane); }
+    double fdn[NC], bdn[NC];
+#pragma unroll
+    for (int q = 0; q < NC; ++q) fdn[q] = bdn[q] = 0.0;
+    if (nf > 0) { of += step; fab = lds2(of); fcd = lds2(of + tb.plane); nb_load_d<NC>(tb, of, fcd, fdn); }
+    if (nbk > 0) { ob -= step; bab = lds2(ob); bcd = lds2(ob + tb.plane); nb_load_d<NC>(tb, ob, bcd, bdn); }
     for (int j = 0; j < nmax; ++j) {
-        const double fs = fab.x, fb_ = fab.y, fc_ = fcd.x, fd_ = fcd.y;
-        const double bs = bab.x, bb_ = bab.y, bc_ = bcd.x, bd_ = bcd.y;
+        const double fs = fab.x, fb_ = fab.y, fc_ = fcd.x;
+        const double bs = bab.x, bb_ = bab.y, bc_ = bcd.x;
+        double fd_[NC], bd_[NC];
+#pragma unroll
+        for (int q = 0; q < NC; ++q) { fd_[q] = fdn[q]; bd_[q] = bdn[q]; }
         const bool fw = j < nf, bw = j < nbk;
-        if (j + 1 < nf) { of += step; fab = lds2(of); fcd = lds2(of + tb.plane); }
-        if (j + 1 < nbk) { ob -= step; bab = lds2(ob); bcd = lds2(ob + tb.plane); }
+        if (j + 1 < nf) { of += step; fab = lds2(of); fcd = lds2(of + tb.plane); nb_load_d<NC>(tb, of, fcd, fdn); }
+        if (j + 1 < nbk) { ob -= step; bab = lds2(ob); bcd = lds2(ob + tb.plane); nb_load_d<NC>(tb, ob, bcd, bdn); }
         if (fw) {
-            const double nbe = fma(be, fb_, -(fs * ga)), nde = fma(be, fd_, -(fs * de));
+            const double nbe = fma(be, fb_, -(fs * ga));
             const double sc = pow2_unscale(nbe);
-            ga = be * fc_ * sc; de = nde * sc; be = nbe * sc;
+#pragma unroll
+            for (int q = 0; q < NC; ++q) de[q] = fma(be, fd_[q], -(fs * de[q])) * sc;
+            ga = be * fc_ * sc; be = nbe * sc;
         }
         if (bw) {
-            const double nbb = fma(bb, bb_, -(bc_ * al)), ndd = fma(bb, bd_, -(bc_ * dd));
+            const double nbb = fma(bb, bb_, -(bc_ * al));
             const double sc = pow2_unscale(nbb);
-            al = bb * bs * sc; dd = ndd * sc; bb = nbb * sc;
+#pragma unroll
+            for (int q = 0; q < NC; ++q) dd[q] = fma(bb, bd_[q], -(bc_ * dd[q])) * sc;
+            al = bb * bs * sc; bb = nbb * sc;
         }
     }
     const double inv = rcp_nr(fma(be, bb, -(ga * al)));
-    up = fma(de, bb, -(ga * dd)) * inv;
-    up1 = fma(be, dd, -(al * de)) * inv;
+#pragma unroll
+    for (int q = 0; q < NC; ++q) {
+        up[q] = fma(de[q], bb, -(ga * dd[q])) * inv;
+        up1[q] = fma(be, dd[q], -(al * de[q])) * inv;
+    }
 }
 
 // Root of a tree: first equation  A x_prev + B x_f + C x_l = D  (row 0), last equation
@@ -427,15 +509,23 @@ __device__ __forceinline__ void cluster_solve_two_sided(const NodeBuf &tb, int l
 // C_last are 0.  Cyclic lines (wrap): x_prev = x_l and x_next = x_f, i.e. the periodic coupling is
 // resolved here, at the top of the recursion, as  B_f x_f + (A_f + C_f) x_l = D_f ,
 // (A_l + C_l) x_f + B_l x_l = D_l  -- no Sherman-Morrison correction is needed.
-template <int TX>
+template <int TX, int NC = 1>
 __device__ __forceinline__ void solve_root(const NodeBuf &nb, int lx, int rl, bool wrap)
 {
     const uint32_t oF = nb_ab<TX>(nb, 0, lx), oL = nb_ab<TX>(nb, rl, lx);
     const double2 abf = lds2(oF), cdf = lds2(oF + nb.plane), abl = lds2(oL), cdl = lds2(oL + nb.plane);
+    double df[NC], dl[NC], xf[NC], xl[NC];
+    nb_load_d<NC>(nb, oF, cdf, df);
+    nb_load_d<NC>(nb, oL, cdl, dl);
     const double Cf = wrap ? cdf.x + abf.x : cdf.x, Al = wrap ? abl.x + cdl.x : abl.x;
     const double inv = rcp_nr(fma(abf.y, abl.y, -(Cf * Al)));
-    sts1(oL + nb.plane + 8, fma(abf.y, cdl.y, -(Al * cdf.y)) * inv);
-    sts1(oF + nb.plane + 8, fma(abl.y, cdf.y, -(Cf * cdl.y)) * inv);
+#pragma unroll
+    for (int q = 0; q < NC; ++q) {
+        xl[q] = fma(abf.y, dl[q], -(Al * df[q])) * inv;
+        xf[q] = fma(abl.y, df[q], -(Cf * dl[q])) * inv;
+    }
+    nb_store_d<NC>(nb, oL, xl);
+    nb_store_d<NC>(nb, oF, xf);
 }
 
 // Leaf state of one thread: M0 rows of one line, swept as K = M0/H independent sub-leaves of H rows
@@ -689,10 +779,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     double *sX = raw + (size_t)NA * arr;                              // x staging tile
     double *node = sX + arr;
     NodeBuf nb;                                                       // node buffer, 2 planes of [2W][TX] pairs
-    nb.ab = ptx::smem_u32(node); nb.plane = (uint32_t)(2 * W * TX) * 16u;
+    nb.ab = ptx::smem_u32(node); nb.plane = (uint32_t)(2 * W * TX) * 16u; nb.d1 = 0;
     const int NTR = 2 * CL;                                           // rows of the cluster-level system
     NodeBuf tb0;                                                      // inbox of parity 0: 2 planes of [NTR][TX]
-    tb0.ab = nb.ab + 2u * nb.plane; tb0.plane = (uint32_t)(NTR * TX) * 16u;
+    tb0.ab = nb.ab + 2u * nb.plane; tb0.plane = (uint32_t)(NTR * TX) * 16u; tb0.d1 = 0;
     const uint32_t inbox_bytes = kCluster ? 2u * tb0.plane : 0u;
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + (tb0.ab + 2u * inbox_bytes - ptx::smem_u32(smem_raw)));
     // bar[0 .. NA-1]: slot full; bar[NA], bar[NA+1]: inboxes
@@ -840,7 +930,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                 const int k = level_k(l), S = level_S(l), groups = level_groups(l);
                 int gq = (h - cum) % nhelp;
                 if (gq < 0) gq += nhelp;
-                double ta[6], tc[6], td[6];
+                double ta[6], tc[6], td[6][1];
                 if (gq < groups) {
                     if (k == 4) kmerge_tails_regs<TX, 4>(nb, lx, gq, S, ta, tc, td);
                     else kmerge_tails_regs<TX, 2>(nb, lx, gq, S, ta, tc, td);
@@ -893,10 +983,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                     ptx::mbar_wait(&bar[NA + par], (unsigned)((it >> 1) & 1));
                     // Stage B: the 2 CL-row system; every CTA computes its own two unknowns (one
                     // thread per line), so no second exchange is needed (B2C is a local store)
-                    double u0, u1;
+                    double u0[1], u1[1];
                     cluster_solve_two_sided<TX>(tb, lx, NTR, 2 * (int)crank, u0, u1);
-                    sts1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8, u0);
-                    sts1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8, u1);
+                    sts1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8, u0[0]);
+                    sts1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8, u1[0]);
                 } else if (leaf == 0) {
                     ptx::mbar_wait(&bar[NA + par], (unsigned)((it >> 1) & 1));
                     // cyclic lines: merge the CL nodes, resolve the wrap at the root, walk back

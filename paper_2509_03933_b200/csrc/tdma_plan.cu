@@ -15,8 +15,9 @@
 #include "tdma_stage_kernels.cuh"
 #include "tdma_fused.cuh"
 #include "tdma_fused_tma.cuh"
+#include "tdma_shared.h"
 
-#define TDMA_VERSION_NUM 10100
+#define TDMA_VERSION_NUM 10200
 
 namespace {
 
@@ -90,6 +91,12 @@ struct tdma_plan {
     bool have_fill = false;
     int fill_opt = 0, fill_last = 0, sm_count = 0;
     size_t sm_smem = 0;
+    // shared-coefficient mode (tdma_solve_shared), configured at the first call per ncomp
+    tdma::SharedConfig sh[2], sh_fill[2];
+    int sh_state[2] = {0, 0};     // 0 = not configured, 1 = ready, -1 = does not tile
+    bool sh_have_fill[2] = {false, false};
+    int sh_opt[4] = {0, 0, 0, 0}; // options.shared_lines / _cluster / _leaf_rows / _slots
+    int sh_last = -1, sh_fill_last = 0;
     // host staging (tdma_solve_host), allocated on first use
     int hz = 0;  // slices per host chunk
     int host_chunk = 0;  // options.host_chunk (0 = auto)
@@ -554,6 +561,8 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->P = P; pl->m = ny / P;   // ny, nz already mapped
     pl->axis = axis; pl->periodic = periodic;
     pl->host_chunk = options ? options->host_chunk : 0;
+    pl->fill_opt = options ? options->fused_fill : 0;
+    if (options) { pl->sh_opt[0] = options->shared_lines; pl->sh_opt[1] = options->shared_cluster; pl->sh_opt[2] = options->shared_leaf_rows; pl->sh_opt[3] = options->shared_slots; }
     pl->rs = axis == TDMA_AXIS_Z ? (long long)nx * nz : (long long)nx;   // z sweep: plan nz = caller ny
     pl->os = axis == TDMA_AXIS_Z ? (long long)nx : (long long)nx * ny;   // x sweep: slices are z-slices
     pl->bz = batch == 0 ? nz : batch;
@@ -592,6 +601,92 @@ int tdma_stage(tdma_plan *plan, int stage, int batch_index, const void *a, const
     const SlabPtrs ptr{(const double *)a, (const double *)b, (const double *)c, (const double *)d, (double *)x};
     const tdma::StageParams prm = batch_params(plan, ptr, plan->nz, batch_index);
     return launch_stage(plan, stage, prm, (cudaStream_t)stream);
+}
+
+int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const void *c_y,
+                      const void *sx, const void *sz, int ncomp, int pin00, const void *d, void *x,
+                      void *stream)
+{
+    int rc = check_ptrs(plan, a_y, b0_y, c_y, d, x);
+    if (rc != TDMA_OK) return rc;
+    if (!sx || !sz) return set_err(TDMA_ERR_INVALID_ARG, "NULL shift array");
+    if (ncomp != 1 && ncomp != 2) return set_err(TDMA_ERR_INVALID_ARG, "ncomp = %d must be 1 (real) or 2 (complex)", ncomp);
+    tdma_plan *pl = plan;
+    if (pl->axis != TDMA_AXIS_Y || pl->periodic)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: lines along y without cyclic coupling only");
+    if ((((uintptr_t)d | (uintptr_t)x) & 15) != 0)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared needs 16-byte aligned d and x (tensor maps)");
+    const int q = ncomp - 1;
+    cudaStream_t origin = (cudaStream_t)stream;
+    if (pl->ny == 1) return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared needs ny >= 4");
+    if (pl->sh_state[q] == 0) {
+        cudaDeviceProp prop;
+        CUDA_TRY(cudaGetDeviceProperties(&prop, pl->device));
+        const char *why = nullptr;
+        if (!tdma::configure_shared(&pl->sh[q], pl->nx, pl->ny, ncomp, pl->sh_opt[0], pl->sh_opt[1], pl->sh_opt[2],
+                                    pl->sh_opt[3], prop, &why)) {
+            pl->sh_state[q] = -1;
+            return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared unavailable for this shape: %s", why ? why : "?");
+        }
+        pl->sm_count = prop.multiProcessorCount;
+        pl->sm_smem = prop.sharedMemPerMultiprocessor;
+        if (pl->sh[q].cluster >= 4 && pl->fill_opt >= 0) {
+            const char *why2 = nullptr;
+            pl->sh_have_fill[q] = tdma::configure_shared(&pl->sh_fill[q], pl->nx, pl->ny, ncomp, 0,
+                                                         pl->ny % 2 == 0 ? 2 : 1, 0, 0, prop, &why2);
+        }
+        pl->sh_state[q] = 1;
+    }
+    if (pl->sh_state[q] < 0)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared unavailable for this shape (see the first call)");
+    tdma::SharedArgs args;
+    args.a_y = (const double *)a_y; args.b0_y = (const double *)b0_y; args.c_y = (const double *)c_y;
+    args.sx = (const double *)sx; args.sz = (const double *)sz;
+    args.d = (const double *)d; args.x = (double *)x;
+    args.pin00 = pin00 ? 1 : 0;
+    args.nx = pl->nx; args.ny = pl->ny; args.nzs = 0;
+    cudaError_t e = tdma::launch_shared(pl->sh[q], args, origin);          // prepare: attributes, grid size
+    int nzf = 0;
+    if (e == cudaSuccess && pl->sh_have_fill[q]) {
+        e = tdma::launch_shared(pl->sh_fill[q], args, origin);
+        if (e == cudaSuccess) {
+            // the fill launch, as for the general kernel (enqueue_fused): clusters of 2 on the SMs
+            // the main launch's clusters cannot be placed on, solving the last nzf slices
+            const long per_sm = (long)(pl->sm_smem / (pl->sh[q].smem + 1024));
+            const int main_ctas = pl->sh[q].max_clusters * pl->sh[q].cluster;
+            const int idle = per_sm == 1 ? pl->sm_count - main_ctas : 0;
+            int fc = idle / pl->sh_fill[q].cluster;
+            if (fc > pl->sh_fill[q].max_clusters) fc = pl->sh_fill[q].max_clusters;
+            if (fc > 0) {
+                const double w = 0.8 * fc * pl->sh_fill[q].cluster;
+                const double share = pl->fill_opt > 0 ? pl->fill_opt * 1e-3 : w / (w + main_ctas);
+                nzf = (int)(pl->nz * share + 0.5);
+                if (nzf >= pl->nz) nzf = pl->nz - 1;
+                if (nzf > 0) pl->sh_fill[q].max_clusters = fc;
+            }
+        }
+    }
+    if (e != cudaSuccess) return set_err(TDMA_ERR_CUDA, "shared launch preparation failed: %s", cudaGetErrorString(e));
+    pl->sh_last = q; pl->sh_fill_last = nzf;
+    if (nzf > 0) {
+        CUDA_TRY(cudaEventRecord(pl->evFork, origin));
+        CUDA_TRY(cudaStreamWaitEvent(pl->sB, pl->evFork, 0));
+    }
+    args.nzs = pl->nz - nzf;
+    e = tdma::launch_shared(pl->sh[q], args, origin);
+    if (e == cudaSuccess && nzf > 0) {
+        tdma::SharedArgs fa = args;
+        const size_t off = (size_t)(pl->nz - nzf) * pl->slice * (size_t)ncomp;
+        fa.d = args.d + off; fa.x = args.x + off; fa.sz = args.sz + (pl->nz - nzf);
+        fa.pin00 = 0;                    // line (0,0) lies in slice 0, which the main launch owns
+        fa.nzs = nzf;
+        e = tdma::launch_shared(pl->sh_fill[q], fa, pl->sB);
+        cudaError_t ej = cudaEventRecord(pl->evBJoin, pl->sB);
+        if (ej == cudaSuccess) ej = cudaStreamWaitEvent(origin, pl->evBJoin, 0);
+        if (e == cudaSuccess) e = ej;
+    }
+    if (e != cudaSuccess) return set_err(TDMA_ERR_CUDA, "shared launch failed: %s", cudaGetErrorString(e));
+    return TDMA_OK;
 }
 
 int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,
@@ -785,6 +880,13 @@ int tdma_plan_get(const tdma_plan *plan, int what)
     case TDMA_GET_FUSED_SMEM: return (int)(plan->fused_impl == 2 ? plan->tfused.smem : plan->fused.smem);
     case TDMA_GET_FUSED_TOP_ROWS:
         return plan->fused_impl == 2 ? 2 * plan->tfused.cluster : 2 * plan->fused.top_nodes * plan->fused.cluster;
+    case TDMA_GET_SHARED_LINES: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].lines;
+    case TDMA_GET_SHARED_CLUSTER: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].cluster;
+    case TDMA_GET_SHARED_LEAF_ROWS: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].leaf_rows;
+    case TDMA_GET_SHARED_THREADS: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].threads;
+    case TDMA_GET_SHARED_SMEM: return plan->sh_last < 0 ? 0 : (int)plan->sh[plan->sh_last].smem;
+    case TDMA_GET_SHARED_SLOTS: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].slots;
+    case TDMA_GET_SHARED_FILL: return plan->sh_last < 0 ? 0 : plan->sh_fill_last;
     default: return set_err(TDMA_ERR_INVALID_ARG, "unknown query %d", what);
     }
 }

@@ -1,0 +1,45 @@
+// Shared-coefficient / complex-RHS mode: host-side interface between the plan
+// (tdma_plan.cu) and the kernel's translation unit (tdma_shared.cu).  Plain C++, no kernels here.
+//
+// The paper's own workload: complex-valued fields, a coefficient matrix that
+// "depends solely on grid spacing" and the FFT-reduced Poisson operator
+// (d2/dy2 - k_l - k_m): line (i,k) has a_j = a_y[j], c_j = c_y[j],
+// b_j = b0_y[j] - (sx[i] + sz[k]); d and x carry ncomp = 1 (real) or 2 (complex, interleaved
+// re/im) right-hand sides per cell.  HBM traffic: 8 ncomp bytes read + 8 ncomp written per cell.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+namespace tdma {
+
+struct SharedConfig {
+    int ncomp = 0;      // NC: right-hand sides per cell
+    int lines = 0;      // TX: lines (cells along x) per tile
+    int cluster = 0;    // CL
+    int rows = 0;       // R = ny / CL
+    int leaf_rows = 0;  // M0
+    int leaves = 0;     // W = R / M0 (power of two, <= 32)
+    int threads = 0;    // W * TX
+    int box_rows = 0;   // rows per TMA box (<= 256), divides R
+    int slots = 0;      // NA: ring slots of one d / x tile each (>= 2)
+    int max_clusters = 0;  // co-resident clusters (persistent grid), filled at first launch
+    size_t smem = 0;
+};
+
+struct SharedArgs {
+    const double *a_y, *b0_y, *c_y;   // [ny]   device
+    const double *sx, *sz;            // [nx], [nz] device; sz already offset to slice 0 of the launch
+    const double *d;                  // slice 0 of the launch
+    double *x;
+    int pin00;                        // row 0 of line (0, 0) of THIS launch's slice 0 is b = 1, c = 0
+    int nx, ny, nzs;
+};
+
+// Tiling for ny-row lines: CL x W x M0 with W a power of two.  want_* = 0: auto.
+bool configure_shared(SharedConfig *out, int nx, int ny, int ncomp, int want_lines, int want_cluster,
+                      int want_leaf, int want_slots, const cudaDeviceProp &prop, const char **why);
+
+// nzs = 0: prepare only (function attributes, persistent grid size).
+cudaError_t launch_shared(SharedConfig &cfg, const SharedArgs &args, cudaStream_t st);
+
+}  // namespace tdma

@@ -1,0 +1,583 @@
+// Shared-coefficient / complex-RHS lines, sm_100a.
+//
+// Same recursion, same cluster mapping and same tree code as tdma_fused_tma.cuh (leaf sweep ->
+// K-ary merges -> DSMEM all-gather -> cluster-level system -> top-down walk -> leaf
+// back-substitution), but the matrix of a line is not read from HBM: a_j, c_j and b0_j come from
+// three 1-D arrays that a CTA copies into shared memory once (its R rows), and the diagonal is
+// b_j = b0_j - s with the line's shift s = sx[i] + sz[k] (formed once per line in fp64, exactly
+// as include/tdma.h states it).  HBM sees d once and x once: 16 B/cell real, 32 B/cell complex.
+//
+// What that changes on chip:
+//   * only ONE array per tile travels (d), so a ring slot holds a whole tile and the ring is
+//     NA >= 2 tiles deep; the sweep writes the forward-eliminated right-hand side d' back into
+//     the slot IN PLACE, back-substitution overwrites it with x, and the TMA store reads x from
+//     the same slot: no staging tile, and only the matrix part (a', c') of the interior rows is
+//     parked in registers (4 (M0-2) instead of 6 (M0-2) registers);
+//   * NC = 2: one thread owns BOTH components of a line (a 16-byte cell), so the elimination of
+//     the matrix -- every reciprocal of the path -- is done once per complex line and each
+//     component only adds its 3 + 2 multiply-adds per row; the tree carries two right-hand sides
+//     per equation (third node-buffer plane, NodeBuf::d1).
+#pragma once
+#include "tdma_fused_tma.cuh"
+#include "tdma_shared.h"
+
+namespace tdma {
+
+struct SharedParams {
+    const double *a_y, *b0_y, *c_y, *sx, *sz;
+    int pin00;
+    int nx, ny, nzs;
+    int CL, R, W, NS;
+    int xtiles, ntiles;
+    int box_rows, nbox;
+};
+
+template <int NC>
+struct EqN { double a, b, c, d[NC]; };
+
+// the NC right-hand-side values of one cell at shared address a
+template <int NC>
+__device__ __forceinline__ void ld_rhs(uint32_t a, double (&v)[NC])
+{
+    if (NC == 2) { const double2 t = lds2(a); v[0] = t.x; v[NC - 1] = t.y; }
+    else v[0] = lds1(a);
+}
+template <int NC>
+__device__ __forceinline__ void st_rhs(uint32_t a, const double (&v)[NC])
+{
+    if (NC == 2) sts2(a, v[0], v[NC - 1]);
+    else sts1(a, v[0]);
+}
+
+// What a leaf keeps in registers between its sweep and its back-substitution: the matrix part of
+// the interior rows, x_r = d'_r - ia x_first - ic x_{r+1} (d'_r lives in the tile slot), and for two
+// sub-leaves the rows the in-register merge eliminated, x = md - ma x_0 - mc x_{M0-1}.
+template <int M0, int NC>
+struct ShLeafRegs {
+    static constexpr int K = M0 >= 8 ? 2 : 1;
+    static constexpr int H = M0 / K;
+    static constexpr int HI = H - 2;
+    double ia[K][HI], ic[K][HI];
+    double ma[2], mc[2], md[2][NC];
+};
+
+// Modified Thomas reduction of the leaf's K sub-leaves (same arithmetic as leaf_reduce in
+// tdma_fused_tma.cuh).  cA, cB, cC: the leaf's rows of a_y, b0_y, c_y in shared memory; s: the
+// line's shift; dbase: shared address of the leaf's first cell, rows row_bytes apart.
+template <int M0, int NC>
+__device__ __forceinline__ void leaf_reduce_sh(const double *__restrict__ cA, const double *__restrict__ cB,
+                                               const double *__restrict__ cC, double s, uint32_t dbase,
+                                               uint32_t row_bytes, bool first_leaf, bool last_leaf, bool pin,
+                                               EqN<NC> &f, EqN<NC> &l, ShLeafRegs<M0, NC> &R)
+{
+    constexpr int K = ShLeafRegs<M0, NC>::K, H = ShLeafRegs<M0, NC>::H;
+    static_assert(H >= 4, "leaves of 4, 8 or 16 rows");
+    double fa[K], fb[K], fc[K], fd[K][NC], pa[K], pc[K], pd[K][NC];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const int o = h * H;
+        double b0 = cB[o] - s, c0 = cC[o];
+        if (h == 0 && pin) { b0 = 1.0; c0 = 0.0; }             // pinned mean mode: x_0 = d_0
+        double inv = rcp_nr(b0);
+        double dv[NC];
+        ld_rhs<NC>(dbase + (uint32_t)o * row_bytes, dv);
+        fa[h] = (h == 0 && first_leaf) ? 0.0 : cA[o] * inv;    // global a_0 := 0
+        fc[h] = c0 * inv; fb[h] = 1.0;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) fd[h][q] = dv[q] * inv;
+        inv = rcp_nr(cB[o + 1] - s);
+        ld_rhs<NC>(dbase + (uint32_t)(o + 1) * row_bytes, dv);
+        pa[h] = cA[o + 1] * inv; pc[h] = cC[o + 1] * inv;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) pd[h][q] = dv[q] * inv;
+    }
+#pragma unroll
+    for (int r = 2; r < H; ++r) {
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            const int o = h * H + r;
+            const double ar = cA[o], br = cB[o] - s;
+            double cr = cC[o];
+            if (r == H - 1 && h == K - 1 && last_leaf) cr = 0.0;   // global c_{ny-1} := 0
+            double dr[NC];
+            ld_rhs<NC>(dbase + (uint32_t)o * row_bytes, dr);
+            // fold row r-1 into the first-row equation, park it for back-substitution
+            fb[h] = fma(-fc[h], pa[h], fb[h]);
+#pragma unroll
+            for (int q = 0; q < NC; ++q) fd[h][q] = fma(-fc[h], pd[h][q], fd[h][q]);
+            fc[h] = -fc[h] * pc[h];
+            R.ia[h][r - 2] = pa[h]; R.ic[h][r - 2] = pc[h];
+            st_rhs<NC>(dbase + (uint32_t)(o - 1) * row_bytes, pd[h]);   // d' of row r-1, in place
+            const double inv = rcp_nr(fma(-ar, pc[h], br));
+#pragma unroll
+            for (int q = 0; q < NC; ++q) pd[h][q] = fma(-ar, pd[h][q], dr[q]) * inv;
+            pc[h] = cr * inv;
+            pa[h] = -(ar * pa[h]) * inv;
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const double inv = rcp_nr(fb[h]);
+        fa[h] *= inv; fc[h] *= inv;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) fd[h][q] *= inv;
+    }
+    if (K == 1) {
+        f.a = fa[0]; f.b = 1.0; f.c = fc[0];
+        l.a = pa[0]; l.b = 1.0; l.c = pc[0];
+#pragma unroll
+        for (int q = 0; q < NC; ++q) { f.d[q] = fd[0][q]; l.d[q] = pd[0][q]; }
+    } else {
+        // pairwise merge of the two sub-leaves in registers (unit diagonals), as leaf_finish
+        const double A1 = fa[0], C1 = fc[0], A2 = pa[0], C2 = pc[0];
+        const double A3 = fa[K - 1], C3 = fc[K - 1], A4 = pa[K - 1], C4 = pc[K - 1];
+        const double det = fma(-C2, A3, 1.0);
+        const double p2 = C2 * C3, p3 = A3 * A2;
+        f.b = fma(-C1, A2, det); l.b = fma(-A4, C3, det);
+        const double sf = pow2_unscale(f.b), sl = pow2_unscale(l.b);
+        f.a = det * A1 * sf; f.b *= sf; f.c = C1 * p2 * sf;
+        l.a = A4 * p3 * sl; l.b *= sl; l.c = det * C4 * sl;
+        const double inv = rcp_nr(det);
+        R.ma[0] = A2 * inv; R.mc[0] = -(p2 * inv);
+        R.ma[1] = -(p3 * inv); R.mc[1] = C3 * inv;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) {
+            const double D1 = fd[0][q], D2 = pd[0][q], D3 = fd[K - 1][q], D4 = pd[K - 1][q];
+            const double nL = fma(-C2, D3, D2), nR = fma(-A3, D2, D3);
+            f.d[q] = fma(det, D1, -(C1 * nL)) * sf;
+            l.d[q] = fma(det, D4, -(A4 * nR)) * sl;
+            R.md[0][q] = nL * inv; R.md[1][q] = nR * inv;
+        }
+    }
+}
+
+// Back-substitution of the leaf given its first and last unknown: d' in the slot becomes x.
+template <int M0, int NC>
+__device__ __forceinline__ void leaf_back_sh(const ShLeafRegs<M0, NC> &R, const double (&xf)[NC], const double (&xl)[NC],
+                                             uint32_t dbase, uint32_t row_bytes)
+{
+    constexpr int K = ShLeafRegs<M0, NC>::K, H = ShLeafRegs<M0, NC>::H;
+    double first[K][NC], xn[K][NC];
+#pragma unroll
+    for (int q = 0; q < NC; ++q) {
+        first[0][q] = xf[q]; xn[K - 1][q] = xl[q];
+        if (K == 2) {
+            xn[0][q] = fma(-R.mc[0], xl[q], fma(-R.ma[0], xf[q], R.md[0][q]));
+            first[K - 1][q] = fma(-R.mc[1], xl[q], fma(-R.ma[1], xf[q], R.md[1][q]));
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        st_rhs<NC>(dbase + (uint32_t)(h * H) * row_bytes, first[h]);
+        st_rhs<NC>(dbase + (uint32_t)(h * H + H - 1) * row_bytes, xn[h]);
+    }
+#pragma unroll
+    for (int r = H - 2; r >= 1; --r) {
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            const uint32_t o = dbase + (uint32_t)(h * H + r) * row_bytes;
+            double dp[NC];
+            ld_rhs<NC>(o, dp);
+#pragma unroll
+            for (int q = 0; q < NC; ++q)
+                xn[h][q] = fma(-R.ic[h][r - 1], xn[h][q], fma(-R.ia[h][r - 1], first[h][q], dp[q]));
+            st_rhs<NC>(o, xn[h]);
+        }
+    }
+}
+
+// Threads: leaf = t / TX, lx = t % TX; the last warp issues the TMA copies and takes no part in
+// the tree (as in fused_tma_kernel).  Ring: tile q of the cluster lives in slot q % NA from its
+// load until the TMA store of its x has read the slot; then tile q + NA is loaded into it.
+template <int TX, int M0, bool kCluster, int MAXT, int NC>
+__global__ void __launch_bounds__(MAXT, 1)
+shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_x,
+                  const SharedParams prm)
+{
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    constexpr int TXD = TX * NC;                                      // doubles per tile row
+    const int R = prm.R, CL = prm.CL, W = prm.W, NA = prm.NS;
+    const int arr = R * TXD;
+    double *const raw = reinterpret_cast<double *>(smem_raw);         // NA slots of [R][TX][NC]
+    double *const cA = raw + (size_t)NA * arr, *const cB = cA + R, *const cC = cB + R;
+    NodeBuf nb;                                                       // node buffer: [2W][TX] per plane
+    nb.ab = ptx::smem_u32(cC + R); nb.plane = (uint32_t)(2 * W * TX) * 16u; nb.d1 = nb.ab + 2u * nb.plane;
+    const uint32_t nb_bytes = 2u * nb.plane + (NC == 2 ? (uint32_t)(2 * W * TX) * 8u : 0u);
+    const int NTR = 2 * CL;                                           // rows of the cluster-level system
+    NodeBuf tb0;                                                      // inbox of parity 0: [NTR][TX] per plane
+    tb0.ab = nb.ab + nb_bytes; tb0.plane = (uint32_t)(NTR * TX) * 16u; tb0.d1 = tb0.ab + 2u * tb0.plane;
+    const uint32_t inbox_bytes = kCluster ? 2u * tb0.plane + (NC == 2 ? (uint32_t)(NTR * TX) * 8u : 0u) : 0u;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw + (tb0.ab + 2u * inbox_bytes - ptx::smem_u32(smem_raw)));
+    // bar[0 .. NA-1]: slot full; bar[NA], bar[NA+1]: inboxes
+
+    const int t = threadIdx.x;
+    const int NT = W * TX;
+    const bool act = t < NT;
+    const int tree_threads = (int)blockDim.x > 32 ? (int)blockDim.x - 32 : NT;
+    const bool tree = t < tree_threads && act;
+    const int Wt = tree_threads / TX;
+    const unsigned tmask = __ballot_sync(0xffffffffu, tree);
+    unsigned crank = 0;
+    if (kCluster) crank = cg::this_cluster().block_rank();
+    const int g = blockIdx.x / CL, NC_ = gridDim.x / CL;       // cluster index / number of clusters
+    const int y0 = (int)crank * R;
+
+    if (t == 0) {
+        for (int i = 0; i < NA + 2; ++i) ptx::mbar_init(&bar[i], 1);
+        ptx::fence_mbar_init();
+    }
+    for (int r = t; r < R; r += (int)blockDim.x) {             // this CTA's rows of the 1-D coefficients
+        cA[r] = prm.a_y[y0 + r]; cB[r] = prm.b0_y[y0 + r]; cC[r] = prm.c_y[y0 + r];
+    }
+    __syncthreads();
+    if (kCluster) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+
+    const int issue_lane = t - ((int)blockDim.x - 32 > 0 ? (int)blockDim.x - 32 : 0);   // >= 0: issuing warp
+    const uint32_t arr_bytes = (uint32_t)(arr * sizeof(double));
+    auto issue_tile = [&](int q) {                             // load of the cluster's q-th tile
+        const int tile = g + q * NC_;
+        if (tile >= prm.ntiles || issue_lane != 0) return;
+        const int s = q % NA;
+        const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
+        double *const dst = raw + (size_t)s * arr;
+        ptx::mbar_expect_tx(&bar[s], arr_bytes);
+        for (int b = 0; b < prm.nbox; ++b)
+            ptx::tma_load_3d(dst + b * prm.box_rows * TXD, &tm_d, x0 * NC, y0 + b * prm.box_rows, k, &bar[s]);
+    };
+    auto store_tile = [&](int q) {                             // x of the q-th tile (TMA clips a ragged x tile)
+        const int tile = g + q * NC_;
+        if (issue_lane == 0) {
+            const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
+            const double *const src = raw + (size_t)(q % NA) * arr;
+            for (int b = 0; b < prm.nbox; ++b)
+                ptx::tma_store_3d(&tm_x, x0 * NC, y0 + b * prm.box_rows, k, src + b * prm.box_rows * TXD);
+        }
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    };
+    if (issue_lane >= 0) for (int q = 0; q < NA; ++q) issue_tile(q);
+
+    const int lx = t % TX, leaf = t / TX;
+    const bool first_leaf = y0 + leaf * M0 == 0;
+    const bool last_leaf = y0 + leaf * M0 + M0 == prm.ny;
+    const uint32_t row_bytes = TXD * 8u;
+    const uint32_t leaf_off = (uint32_t)(leaf * M0 * TXD + lx * NC) * 8u;
+    // K-ary tree levels, packed as in fused_tma_kernel
+    unsigned kcode = 0, ccode = 0;
+    int nl = 0;
+    for (int nodes = W, cum = 0; nodes > 1; ++nl) {
+        const int lkb = (nodes & 3) == 0 ? 2 : 1;
+        kcode |= (unsigned)lkb << (2 * nl); ccode |= (unsigned)cum << (5 * nl);
+        nodes >>= lkb; cum += lkb;
+    }
+    auto level_k = [&](int l) { return 1 << ((kcode >> (2 * l)) & 3u); };
+    auto level_S = [&](int l) { return 2 << ((ccode >> (5 * l)) & 31u); };
+    auto level_groups = [&](int l) { return W >> (((ccode >> (5 * l)) & 31u) + ((kcode >> (2 * l)) & 3u)); };
+    // critical / helper warps of the tree, as in fused_tma_kernel
+    const int G0 = nl > 0 ? level_groups(0) : 0;
+    const int rpw = TX >= 32 ? 1 : 32 / TX;
+    const int crit_rows = Wt >= 2 * G0 ? 2 * G0 : (Wt >= G0 ? G0 : Wt);
+    const int cw = (crit_rows + rpw - 1) / rpw;
+    const bool helper_mode = nl > 0 && (int)blockDim.x > 32 && cw * 32 < tree_threads;
+    const int help0 = helper_mode ? cw * rpw : Wt;
+    const int nhelp = Wt - help0;
+    const int mrows = helper_mode ? crit_rows : Wt;
+    const int crit_threads = helper_mode ? cw * 32 : tree_threads;
+    const bool crit = tree && leaf < help0, helper = tree && !crit;
+
+    int it = 0;
+    for (int tile = g; tile < prm.ntiles; tile += NC_, ++it) {
+        const int par = it & 1;
+        NodeBuf tb = tb0;
+        tb.ab += (uint32_t)par * inbox_bytes; tb.d1 += (uint32_t)par * inbox_bytes;
+        if (kCluster && t == 0)
+            ptx::mbar_expect_tx(&bar[NA + par], (unsigned)(NTR * TX * (32 + 8 * (NC - 1))));
+        const int slot = it % NA;
+        const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
+        const int gi = x0 + lx < prm.nx ? x0 + lx : prm.nx - 1;    // ragged x tile: lanes past nx solve a copy
+        const double s = prm.sx[gi] + prm.sz[k];                   // the line's shift
+        const bool pin = prm.pin00 != 0 && first_leaf && gi == 0 && k == 0;
+        const uint32_t dbase = ptx::smem_u32(raw + (size_t)slot * arr) + leaf_off;
+        ptx::mbar_wait(&bar[slot], (unsigned)((it / NA) & 1));
+
+        // ---------------- leaves ----------------
+        ShLeafRegs<M0, NC> regs;
+        if (act) {
+            EqN<NC> f, l;
+            leaf_reduce_sh<M0, NC>(cA + leaf * M0, cB + leaf * M0, cC + leaf * M0, s, dbase, row_bytes,
+                                   first_leaf, last_leaf, pin, f, l, regs);
+            const uint32_t of = nb_ab<TX>(nb, 2 * leaf, lx), ol = of + TX * 16u;
+            sts2(of, f.a, f.b); sts2(of + nb.plane, f.c, f.d[0]);
+            sts2(ol, l.a, l.b); sts2(ol + nb.plane, l.c, l.d[0]);
+            if (NC == 2) { sts1(nb_d1(nb, of), f.d[NC - 1]); sts1(nb_d1(nb, ol), l.d[NC - 1]); }
+        }
+        __syncthreads();                // leaf equations visible; previous tile's x complete in its slot
+        if (issue_lane >= 0 && it > 0) {
+            store_tile(it - 1);
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+            issue_tile(it - 1 + NA);    // the slot the store has just read out
+        }
+        if (kCluster && it == 0) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+
+        // ---------------- K-ary tree inside the CTA, bottom-up ----------------
+        if (helper) {
+            const int h = leaf - help0;
+            int cum = 0;
+            for (int l = 0; l < nl; ++l) {
+                const int kk = level_k(l), S = level_S(l), groups = level_groups(l);
+                int gq = (h - cum) % nhelp;
+                if (gq < 0) gq += nhelp;
+                double ta[6], tc[6], td[6][NC];
+                if (gq < groups) {
+                    if (kk == 4) kmerge_tails_regs<TX, 4, NC>(nb, lx, gq, S, ta, tc, td);
+                    else kmerge_tails_regs<TX, 2, NC>(nb, lx, gq, S, ta, tc, td);
+                }
+                named_sync(2 + l, tree_threads);
+                if (gq < groups) {
+                    if (kk == 4) kmerge_tails_store<TX, 4, NC>(nb, lx, gq, S, ta, tc, td);
+                    else kmerge_tails_store<TX, 2, NC>(nb, lx, gq, S, ta, tc, td);
+                    for (gq += nhelp; gq < groups; gq += nhelp) {
+                        if (kk == 4) kmerge_tails<TX, 4, NC>(nb, lx, gq, S, 4); else kmerge_tails<TX, 2, NC>(nb, lx, gq, S, 2);
+                    }
+                }
+                cum += groups;
+            }
+        }
+        if (crit) {
+            for (int l = 0; l < nl; ++l) {
+                const int kk = level_k(l), S = level_S(l), groups = level_groups(l);
+                for (int q = leaf; q < 2 * groups; q += mrows) {
+                    if (q < groups) { if (kk == 4) kmerge_fwd<TX, 4, NC>(nb, lx, q, S, 4); else kmerge_fwd<TX, 2, NC>(nb, lx, q, S, 2); }
+                    else { if (kk == 4) kmerge_bwd<TX, 4, NC>(nb, lx, q - groups, S, 4); else kmerge_bwd<TX, 2, NC>(nb, lx, q - groups, S, 2); }
+                }
+                if (helper_mode) named_arrive(2 + l, tree_threads);
+                tree_sync(crit_threads, tmask);
+                if (!helper_mode) {
+                    for (int q = mrows - 1 - leaf; q < groups; q += mrows) {
+                        if (kk == 4) kmerge_tails<TX, 4, NC>(nb, lx, q, S, 4); else kmerge_tails<TX, 2, NC>(nb, lx, q, S, 2);
+                    }
+                }
+            }
+            // ---------------- cluster level ----------------
+            if (!kCluster) {
+                if (leaf == 0) solve_root<TX, NC>(nb, lx, 2 * W - 1, false);
+            } else {
+                // all-gather of the CTA's node (the paper's MPI_Alltoall)
+                const uint32_t bar_s = ptx::smem_u32(&bar[NA + par]);
+                for (int e = t; e < 4 * TX * CL; e += crit_threads) {
+                    const int dest = e / (4 * TX), r = e - dest * 4 * TX;
+                    const int piece = r / TX, li = r - piece * TX;  // piece: AB / CD of first, AB / CD of last
+                    const int j = piece >> 1;
+                    const uint32_t po = (piece & 1) ? 1u : 0u;
+                    const double2 v = lds2(nb_ab<TX>(nb, j ? 2 * W - 1 : 0, li) + po * nb.plane);
+                    const uint32_t dst = ptx::mapa(nb_ab<TX>(tb, (int)crank * 2 + j, li) + po * tb.plane, (unsigned)dest);
+                    ptx::st_async_2f64(dst, v.x, v.y, ptx::mapa(bar_s, (unsigned)dest));
+                }
+                if (NC == 2) {
+                    for (int e = t; e < 2 * TX * CL; e += crit_threads) {
+                        const int dest = e / (2 * TX), r = e - dest * 2 * TX;
+                        const int j = r / TX, li = r - j * TX;
+                        const double v = lds1(nb_d1(nb, nb_ab<TX>(nb, j ? 2 * W - 1 : 0, li)));
+                        const uint32_t dst = ptx::mapa(nb_d1(tb, nb_ab<TX>(tb, (int)crank * 2 + j, li)), (unsigned)dest);
+                        ptx::st_async_f64(dst, v, ptx::mapa(bar_s, (unsigned)dest));
+                    }
+                }
+                if (leaf == 0) {
+                    ptx::mbar_wait(&bar[NA + par], (unsigned)((it >> 1) & 1));
+                    // Stage B: every CTA computes its own two unknowns of the 2 CL-row system
+                    double u0[NC], u1[NC];
+                    cluster_solve_two_sided<TX, NC>(tb, lx, NTR, 2 * (int)crank, u0, u1);
+                    nb_store_d<NC>(nb, nb_ab<TX>(nb, 0, lx), u0);
+                    nb_store_d<NC>(nb, nb_ab<TX>(nb, 2 * W - 1, lx), u1);
+                }
+            }
+        }
+        __syncthreads();
+
+        // ---------------- top-down walk + leaf back-substitution, x written in place ----------
+        if (act) {
+            double xf[NC], xl[NC];
+            nb_load_donly<NC>(nb, nb_ab<TX>(nb, 0, lx), xf);
+            nb_load_donly<NC>(nb, nb_ab<TX>(nb, 2 * W - 1, lx), xl);
+            for (int l = nl - 1; l >= 0; --l) {
+                const int kk = level_k(l), S = level_S(l);
+                const int node = leaf >> ((ccode >> (5 * l)) & 31u);
+                const int gq = node >> ((kcode >> (2 * l)) & 3u), j = node & (kk - 1);
+                double nf[NC], nla[NC];
+                kmerge_value_n<TX, NC>(nb, lx, gq, S, kk, 2 * j, xf, xl, nf);
+                kmerge_value_n<TX, NC>(nb, lx, gq, S, kk, 2 * j + 1, xf, xl, nla);
+#pragma unroll
+                for (int q = 0; q < NC; ++q) { xf[q] = nf[q]; xl[q] = nla[q]; }
+            }
+            leaf_back_sh<M0, NC>(regs, xf, xl, dbase, row_bytes);
+            ptx::fence_proxy_async_smem();      // x in the slot -> visible to the TMA store
+        }
+    }
+    if (it > 0) {
+        __syncthreads();
+        if (issue_lane >= 0) {
+            store_tile(it - 1);
+            asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Host side
+// ------------------------------------------------------------------------------------------
+inline size_t shared_smem_bytes(int TX, int R, int W, int CL, int NA, int NC)
+{
+    const size_t slots = (size_t)NA * R * TX * NC * sizeof(double);
+    const size_t coef = (size_t)3 * R * sizeof(double);
+    const size_t node = (size_t)2 * W * TX * (32 + 8 * (NC - 1));
+    const size_t inbox = CL > 1 ? (size_t)2 * 2 * CL * TX * (32 + 8 * (NC - 1)) : 0;
+    return slots + coef + node + inbox + 128;
+}
+
+// Leaf sizes the kernel is instantiated for.
+constexpr int kSharedLeafSizes[] = {16, 8, 4};
+
+inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int want_lines, int want_cluster,
+                                  int want_leaf, int want_slots, const cudaDeviceProp &prop, const char **why)
+{
+    if (NC != 1 && NC != 2) { *why = "ncomp must be 1 (real) or 2 (complex)"; return false; }
+    if ((nx * NC) % 2) { *why = "TMA path needs an even number of doubles per row (16-byte global strides)"; return false; }
+    const size_t max_smem = prop.sharedMemPerBlockOptin;
+    SharedConfig best; double best_score = -1.0;
+    // lines per tile: 128-byte row segments first (16 real / 8 complex cells), then 256-byte ones
+    const int tx_opts[2] = {NC == 1 ? 16 : 8, NC == 1 ? 32 : 16};
+    const int cl_opts[4] = {1, 2, 4, 8};
+    for (int ti = 0; ti < 2; ++ti) {
+        const int TX = tx_opts[ti];
+        if (want_lines && TX != want_lines) continue;
+        for (int ci = 0; ci < 4; ++ci) {
+            const int CL = cl_opts[ci];
+            if (want_cluster && CL != want_cluster) continue;
+            if (ny % CL) continue;
+            const int R = ny / CL;
+            for (int m0 : kSharedLeafSizes) {
+                if (want_leaf && m0 != want_leaf) continue;
+                if (m0 > R || R % m0 || !is_pow2(R / m0) || R / m0 > 32) continue;
+                SharedConfig c;
+                c.ncomp = NC; c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
+                c.threads = c.leaves * TX;
+                if (c.threads > 512) continue;
+                c.box_rows = R;
+                while (c.box_rows > 256) c.box_rows /= 2;
+                if (R % c.box_rows) continue;
+                c.slots = 0;
+                for (int na = want_slots ? want_slots : 4; na >= (want_slots ? want_slots : 2); --na) {
+                    c.smem = shared_smem_bytes(TX, R, c.leaves, CL, na, NC);
+                    if (c.smem <= max_smem) { c.slots = na; break; }
+                }
+                if (!c.slots) continue;
+                // as for the general kernel: long leaves (fewer tree levels) first, then 256 threads
+                // per CTA (255 registers each), 128-byte segments, a deep ring, small clusters
+                const double score = 10000.0 * m0 + (c.threads == 256 ? 4000.0 : (c.threads > 256 ? 1000.0 : 2000.0 + c.threads)) +
+                                     (ti == 0 ? 500.0 : 0.0) + 100.0 * c.slots - 50.0 * CL;
+                if (score > best_score) { best_score = score; best = c; }
+            }
+        }
+    }
+    if (best_score < 0) {
+        *why = "no (lines, cluster, leaf) tiling with a power-of-two tree of <= 32 leaves of 4, 8 or 16 rows fits";
+        return false;
+    }
+    *out = best;
+    return true;
+}
+
+// d / x as a tensor of doubles (nx * NC, ny, nz), box (TX * NC, box_rows, 1)
+inline bool make_shared_tensor_map(CUtensorMap *tm, const void *base, int nx, int ny, int nz, int NC, int TX, int box_rows)
+{
+    tdma_encode_tiled_fn enc = get_encode_tiled();
+    if (!enc) return false;
+    cuuint64_t gdim[3] = {(cuuint64_t)nx * NC, (cuuint64_t)ny, (cuuint64_t)nz};
+    cuuint64_t gstr[2] = {(cuuint64_t)nx * NC * sizeof(double), (cuuint64_t)nx * NC * ny * sizeof(double)};
+    cuuint32_t box[3] = {(cuuint32_t)(TX * NC), (cuuint32_t)box_rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    const size_t inner = (size_t)TX * NC * sizeof(double);
+    const CUtensorMapL2promotion promo = inner >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), gdim, gstr, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int TX, int M0, bool kCluster, int MAXT, int NC>
+inline cudaError_t launch_shared_inst(SharedConfig &cfg, const CUtensorMap *tm, const SharedParams &prm, cudaStream_t st)
+{
+    auto kern = shared_tma_kernel<TX, M0, kCluster, MAXT, NC>;
+    cudaLaunchConfig_t lc = {};
+    lc.blockDim = dim3((cfg.threads + 31) & ~31);
+    lc.dynamicSmemBytes = cfg.smem;
+    lc.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cfg.cluster; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    lc.attrs = attr;
+    lc.numAttrs = kCluster ? 1 : 0;
+    if (cfg.max_clusters <= 0) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
+        if (e != cudaSuccess) return e;
+        int dev = 0, sms = 0, n = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (kCluster) {
+            lc.gridDim = dim3((unsigned)(cfg.cluster * sms));
+            e = cudaOccupancyMaxActiveClusters(&n, kern, &lc);
+            if (e != cudaSuccess) return e;
+        } else {
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, (int)lc.blockDim.x, cfg.smem);
+            if (e != cudaSuccess) return e;
+            n *= sms;
+        }
+        if (n < 1) return cudaErrorLaunchOutOfResources;
+        cfg.max_clusters = n;
+    }
+    if (prm.ntiles <= 0) return cudaSuccess;
+    const int nc = prm.ntiles < cfg.max_clusters ? prm.ntiles : cfg.max_clusters;
+    lc.gridDim = dim3((unsigned)(nc * cfg.cluster));
+    return cudaLaunchKernelEx(&lc, kern, tm[0], tm[1], prm);
+}
+
+template <int TX, int NC, bool kCluster>
+inline cudaError_t launch_shared_tx(SharedConfig &cfg, const CUtensorMap *tm, const SharedParams &prm, cudaStream_t st)
+{
+    const bool big = cfg.threads > 256;
+    switch (cfg.leaf_rows) {
+    case 16: return big ? launch_shared_inst<TX, 16, kCluster, 512, NC>(cfg, tm, prm, st)
+                        : launch_shared_inst<TX, 16, kCluster, 256, NC>(cfg, tm, prm, st);
+    case 8: return big ? launch_shared_inst<TX, 8, kCluster, 512, NC>(cfg, tm, prm, st)
+                       : launch_shared_inst<TX, 8, kCluster, 256, NC>(cfg, tm, prm, st);
+    case 4: return big ? cudaErrorInvalidValue : launch_shared_inst<TX, 4, kCluster, 256, NC>(cfg, tm, prm, st);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+inline cudaError_t launch_shared_impl(SharedConfig &cfg, const SharedArgs &a, cudaStream_t st)
+{
+    CUtensorMap tm[2];
+    if (a.nzs > 0) {
+        if (!make_shared_tensor_map(&tm[0], a.d, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows) ||
+            !make_shared_tensor_map(&tm[1], a.x, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows))
+            return cudaErrorInvalidValue;
+    }
+    SharedParams prm;
+    prm.a_y = a.a_y; prm.b0_y = a.b0_y; prm.c_y = a.c_y; prm.sx = a.sx; prm.sz = a.sz;
+    prm.pin00 = a.pin00;
+    prm.nx = a.nx; prm.ny = a.ny; prm.nzs = a.nzs;
+    prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves; prm.NS = cfg.slots;
+    prm.xtiles = (a.nx + cfg.lines - 1) / cfg.lines;
+    prm.ntiles = prm.xtiles * a.nzs;
+    prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
+    const bool cl = cfg.cluster > 1;
+    if (cfg.ncomp == 1) {
+        if (cfg.lines == 16) return cl ? launch_shared_tx<16, 1, true>(cfg, tm, prm, st) : launch_shared_tx<16, 1, false>(cfg, tm, prm, st);
+        if (cfg.lines == 32) return cl ? launch_shared_tx<32, 1, true>(cfg, tm, prm, st) : launch_shared_tx<32, 1, false>(cfg, tm, prm, st);
+    } else {
+        if (cfg.lines == 8) return cl ? launch_shared_tx<8, 2, true>(cfg, tm, prm, st) : launch_shared_tx<8, 2, false>(cfg, tm, prm, st);
+        if (cfg.lines == 16) return cl ? launch_shared_tx<16, 2, true>(cfg, tm, prm, st) : launch_shared_tx<16, 2, false>(cfg, tm, prm, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace tdma

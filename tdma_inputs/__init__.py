@@ -212,6 +212,75 @@ def poisson_wavenumber(nx: int, ny: int, nz: int, seed: int, beta: Optional[floa
     return a, b, c, d
 
 
+@dataclass
+class SharedWorkload:
+    """Shared-coefficient form of a Poisson config: line (i,k) has a = a_y,
+    c = c_y, b = b0_y - (sx[i] + sz[k]); d real or complex (nz, ny, nx)."""
+    name: str
+    nx: int
+    ny: int
+    nz: int
+    a_y: torch.Tensor
+    b0_y: torch.Tensor
+    c_y: torch.Tensor
+    sx: torch.Tensor
+    sz: torch.Tensor
+    d: torch.Tensor
+    pin00: bool
+    meta: Dict[str, float] = field(default_factory=dict)
+
+    @property
+    def cells(self) -> int:
+        return self.nx * self.ny * self.nz
+
+    @property
+    def ncomp(self) -> int:
+        return 2 if self.d.is_complex() else 1
+
+
+def poisson_shared(nx: int, ny: int, nz: int, seed: int, beta: Optional[float], cplx: bool, device="cpu",
+                   Lx: float = 2.0 * math.pi, Lz: float = 2.0 * math.pi, k_offset: int = 0,
+                   nz_total: Optional[int] = None):
+    """The coefficients of ``poisson_wavenumber`` as the 1-D arrays they are made of (PAPER.md:286,
+    318): a_y, c_y, b0_y = -(a_y + c_y), sx = kx^2, sz = kz^2; d ~ N(0,1) per component (complex
+    fields: PAPER.md:377; re uses stream 0 -- the bits of the real config -- and im stream 1);
+    mode (0,0) pinned (pin00) with d_0 = 0."""
+    nzt = nz if nz_total is None else nz_total
+    a_y, c_y = poisson_y_coefficients(ny, beta)
+    a_y, c_y = a_y.to(device), c_y.to(device)
+    dx, dz = Lx / nx, Lz / nzt
+    i = torch.arange(nx, dtype=torch.float64, device=device)
+    k = torch.arange(k_offset, k_offset + nz, dtype=torch.float64, device=device)
+    sx = (2.0 * torch.sin(math.pi * i / nx) / dx) ** 2
+    sz = (2.0 * torch.sin(math.pi * k / nzt) / dz) ** 2
+    d = torch.empty((nz, ny, nx), dtype=torch.complex128 if cplx else torch.float64, device=device)
+    dv = torch.view_as_real(d) if cplx else d.unsqueeze(-1)
+    for k0, k1 in _chunks(nz, ny, nx):
+        idx = _cell_index(nx, ny, k_offset + k0, k_offset + k1, device)
+        for q in range(2 if cplx else 1):
+            dv[k0:k1, :, :, q] = normal01(idx, seed, q)
+        del idx
+    if k_offset == 0:
+        d[0, 0, 0] = 0.0
+    return a_y, -(a_y + c_y), c_y, sx, sz, d
+
+
+def make_shared_workload(name: str, cplx: bool, device="cpu", nz: Optional[int] = None, nx: Optional[int] = None,
+                         ny: Optional[int] = None, k_offset: int = 0) -> SharedWorkload:
+    """Shared-coefficient form of a ``poisson`` config (cfg2_poisson, cfg3_weak); ``nz`` / ``k_offset``
+    restrict generation to a z-range with the bits of the full slab."""
+    spec = config_spec(name)
+    if spec["kind"] != "poisson":
+        raise ValueError("shared-coefficient workloads are defined for the Poisson configs")
+    fnx = spec["nx"] if nx is None else nx
+    fny = spec["ny"] if ny is None else ny
+    gnz = spec["nz"] if nz is None else nz
+    a_y, b0_y, c_y, sx, sz, d = poisson_shared(fnx, fny, gnz, spec["seed"], spec["beta"], cplx, device,
+                                               k_offset=k_offset, nz_total=spec["nz"])
+    return SharedWorkload(name + ("_shared_c128" if cplx else "_shared_f64"), fnx, fny, gnz, a_y, b0_y, c_y, sx, sz, d,
+                          pin00=(k_offset == 0), meta={"seed": spec["seed"], "k_offset": k_offset})
+
+
 def adi_alpha(seed: int) -> float:
     """alpha = nu*dt/h^2 ~ U(0.1, 10), one scalar per run (BASELINE cfg 4)."""
     u = uniform01(torch.zeros(1, dtype=torch.int64), seed, 7).item()

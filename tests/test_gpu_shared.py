@@ -1,0 +1,177 @@
+"""shared-coefficient / complex-RHS lines -- the CUDA
+path (tdma_solve_shared through the C ABI) against oracle.solve_y_shared, element by element on
+the same seeded inputs.  Tolerance as for the general path (G9): per line and per component
+E = ||x - x_or||_inf / ||x_or||_inf <= 1e-11, against the long-double oracle on the weakly
+dominant Poisson coefficients of cfg 2 / cfg 3."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import tdma_inputs
+import paper_2509_03933_b200 as tdma
+
+pytestmark = pytest.mark.gpu
+
+TOL_E = 1e-11
+
+
+def dev():
+    return torch.device("cuda:0")
+
+
+def as_lines(x):
+    """(nz, ny, nx) real or complex -> real (nz, ny, nx * ncomp): every component is a line."""
+    x = np.ascontiguousarray(x)
+    if np.iscomplexobj(x):
+        return x.view(np.float64).reshape(x.shape[0], x.shape[1], -1)
+    return x
+
+
+def gpu_solve_shared(w, P=1, x=None, **opts):
+    dv = dev()
+    t = [v.to(dv) for v in (w.a_y, w.b0_y, w.c_y, w.sx, w.sz, w.d)]
+    out = torch.full_like(t[5], float("nan")) if x is None else x
+    with tdma.Plan(w.nx, w.ny, w.nz, P, 0, **opts) as plan:
+        plan.solve_shared(*t[:5], t[5], out, pin00=w.pin00)
+        torch.cuda.synchronize()
+        info = {k: plan.get(getattr(tdma, "TDMA_GET_SHARED_" + k.upper()))
+                for k in ("lines", "cluster", "leaf_rows", "threads", "slots", "fill")}
+    return out, info
+
+
+def oracle_shared(w, precision):
+    arrs = [v.cpu().numpy() for v in (w.a_y, w.b0_y, w.c_y, w.sx, w.sz, w.d)]
+    return oracle.solve_y_shared(*arrs, pin00=w.pin00, precision=precision)
+
+
+def check(w, x, precision="ld"):
+    xn = x.cpu().numpy()
+    assert np.isfinite(as_lines(xn)).all()
+    ref = oracle_shared(w, precision)
+    E = oracle.normwise_error(as_lines(xn), as_lines(ref)).max()
+    assert E <= TOL_E, "normwise error %.3e" % E
+    return E
+
+
+def random_shared(nz, ny, nx, cplx, seed):
+    """Strictly dominant shared-coefficient case (the recipe of the oracle pins): a, c ~ U(-1,1),
+    b0 ~ 2.5 + U(0,1), shifts <= 0 so that b >= 2.5."""
+    g = torch.Generator().manual_seed(seed)
+    u = lambda n, lo, hi: lo + (hi - lo) * torch.rand(n, dtype=torch.float64, generator=g)
+    d = torch.randn((nz, ny, nx), dtype=torch.float64, generator=g)
+    if cplx:
+        d = torch.complex(d, torch.randn((nz, ny, nx), dtype=torch.float64, generator=g))
+    return tdma_inputs.SharedWorkload("random_shared", nx, ny, nz, u(ny, -1, 1), u(ny, 2.5, 3.5), u(ny, -1, 1),
+                                      -u(nx, 0, 2), -u(nz, 0, 2), d, pin00=False)
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+@pytest.mark.parametrize("name,nz", [("cfg2_poisson", 6), ("cfg3_weak", 16)])
+def test_poisson_shared_slab(name, nz, cplx):
+    """z-slab of cfg 2 / cfg 3 at full nx, ny in the automatic tiling (cfg 3: main + fill launch)."""
+    w = tdma_inputs.make_shared_workload(name, cplx, nz=nz)
+    x, info = gpu_solve_shared(w)
+    check(w, x, "ld")
+    assert x.cpu().numpy()[0, 0, 0] == 0.0                     # pinned mean mode: x_0 = d_0 = 0
+    if name == "cfg3_weak":
+        assert info["cluster"] >= 2 and info["leaf_rows"] == 16
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+@pytest.mark.parametrize("ny,opts", [
+    (16, {}), (32, {}), (64, {}), (128, dict(shared_leaf_rows=4)), (128, dict(shared_leaf_rows=8)),
+    (256, dict(shared_cluster=1)), (256, dict(shared_cluster=2)), (256, dict(shared_cluster=4, shared_leaf_rows=8)),
+    (512, dict(shared_cluster=2)), (512, dict(shared_cluster=8, shared_leaf_rows=16)),
+    (1024, dict(shared_cluster=2)), (1024, dict(shared_cluster=4, shared_slots=2)),
+    (1024, dict(shared_cluster=8, shared_leaf_rows=8)),
+])
+def test_tilings_and_ragged_x(ny, opts, cplx):
+    """Every tiling the kernel is instantiated for, nx not a multiple of the tile width (the last
+    x tile is clipped by TMA), several tiles per cluster."""
+    w = random_shared(5, ny, 88, cplx, seed=ny + (7 if cplx else 0))
+    x, info = gpu_solve_shared(w, **opts)
+    check(w, x, "f64")
+    for key, name in (("shared_cluster", "cluster"), ("shared_leaf_rows", "leaf_rows"), ("shared_slots", "slots")):
+        if key in opts:
+            assert info[name] == opts[key]
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+@pytest.mark.parametrize("lines", [0, 1])
+def test_wide_tiles(lines, cplx):
+    """256-byte row segments (32 real / 16 complex cells per tile row)."""
+    w = random_shared(3, 512, 96, cplx, seed=11)
+    x, info = gpu_solve_shared(w, shared_lines=(32 if not cplx else 16) if lines else 0)
+    check(w, x, "f64")
+    assert info["lines"] == ((32 if not cplx else 16) if lines else (16 if not cplx else 8))
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+def test_in_place_and_repeatable(cplx):
+    """x may alias d; repeated solves give the same bits (races show up as differing bits)."""
+    w = random_shared(24, 1024, 64, cplx, seed=3)
+    x1, _ = gpu_solve_shared(w)
+    x2, _ = gpu_solve_shared(w)
+    assert torch.equal(torch.view_as_real(x1) if cplx else x1, torch.view_as_real(x2) if cplx else x2)
+    dcopy = w.d.clone().to(dev())
+    t = [v.to(dev()) for v in (w.a_y, w.b0_y, w.c_y, w.sx, w.sz)]
+    with tdma.Plan(w.nx, w.ny, w.nz, 1, 0) as plan:
+        plan.solve_shared(*t, dcopy, dcopy)
+        torch.cuda.synchronize()
+    assert torch.equal(torch.view_as_real(dcopy) if cplx else dcopy, torch.view_as_real(x1) if cplx else x1)
+    check(w, x1, "f64")
+
+
+def test_complex_components_are_independent_real_solves():
+    """re / im of the complex solve equal, bit for bit, what the REAL shared solve gives for each
+    component in the same tiling family?  No: tilings differ, so compare within tolerance, and
+    check that a purely real d gives an exactly zero imaginary part."""
+    w = random_shared(4, 256, 32, True, seed=5)
+    xc, _ = gpu_solve_shared(w)
+    for part in ("real", "imag"):
+        wr = tdma_inputs.SharedWorkload("part", w.nx, w.ny, w.nz, w.a_y, w.b0_y, w.c_y, w.sx, w.sz,
+                                        getattr(w.d, part).contiguous(), False)
+        xr, _ = gpu_solve_shared(wr)
+        ref = getattr(xc, part).cpu().numpy()
+        assert oracle.normwise_error(xr.cpu().numpy(), ref).max() <= TOL_E
+    wz = tdma_inputs.SharedWorkload("realonly", w.nx, w.ny, w.nz, w.a_y, w.b0_y, w.c_y, w.sx, w.sz,
+                                    torch.complex(w.d.real, torch.zeros_like(w.d.real)), False)
+    xz, _ = gpu_solve_shared(wz)
+    assert float(xz.imag.abs().max()) == 0.0
+
+
+def test_matches_general_path_on_materialised_arrays():
+    """Same systems through tdma_solve with a, b, c materialised (b formed as b0 - (sx + sz))."""
+    w = random_shared(4, 512, 64, False, seed=9)
+    dv = dev()
+    nz, ny, nx = w.nz, w.ny, w.nx
+    a = w.a_y.view(1, ny, 1).expand(nz, ny, nx).contiguous().to(dv)
+    c = w.c_y.view(1, ny, 1).expand(nz, ny, nx).contiguous().to(dv)
+    b = (w.b0_y.view(1, ny, 1) - (w.sx.view(1, 1, nx) + w.sz.view(nz, 1, 1))).contiguous().to(dv)
+    d = w.d.to(dv)
+    xg = torch.empty_like(d)
+    with tdma.Plan(nx, ny, nz, 8, 0) as plan:
+        plan.solve(a, b, c, d, xg)
+        torch.cuda.synchronize()
+    xs, _ = gpu_solve_shared(w)
+    assert oracle.normwise_error(xs.cpu().numpy(), xg.cpu().numpy()).max() <= TOL_E
+
+
+def test_unsupported_shapes_fail_loudly():
+    dv = dev()
+    def attempt(nx, ny, cplx):
+        w = random_shared(2, ny, nx, cplx, seed=1)
+        return gpu_solve_shared(w)
+    with pytest.raises(tdma.TdmaError) as e1:
+        attempt(32, 24, False)                       # 24 rows: no power-of-two tree of 4/8/16-row leaves
+    assert e1.value.status == tdma.TDMA_ERR_UNSUPPORTED
+    with pytest.raises(tdma.TdmaError) as e2:
+        attempt(33, 64, False)                       # odd nx, real: 8-byte global strides
+    assert e2.value.status == tdma.TDMA_ERR_UNSUPPORTED
+    attempt(33, 64, True)                            # complex cells are 16 bytes: fine
+    w = random_shared(2, 64, 32, False, seed=1)
+    t = [v.to(dv) for v in (w.a_y, w.b0_y, w.c_y, w.sx, w.sz, w.d)]
+    with tdma.Plan(32, 64, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, periodic=1) as plan:
+        with pytest.raises(tdma.TdmaError):
+            plan.solve_shared(*t, torch.empty_like(t[5]))
