@@ -312,6 +312,73 @@ def second_workload(torch, tdma, tdma_inputs, name, dev, steps, warmup, barrier,
     return rec
 
 
+def shared_workload(torch, tdma, tdma_inputs, base, cplx, dev, steps, warmup, barrier, peak, nz=None,
+                    cpu_seconds=5.0):
+    """SURVEY 8(f) f3 / the paper's own benchmark form: the Poisson config with
+    its coefficients passed as 1-D arrays and a real or complex right-hand side, through
+    tdma_solve_shared.  Algorithmic bytes: d read + x written = 16 B per real cell, 32 B per complex
+    cell.  Own roofline, parity check (long-double reference on sampled slices) and CPU baseline."""
+    import numpy as np
+    import oracle
+    w = tdma_inputs.make_shared_workload(base, cplx, device=dev, nz=nz)
+    x = torch.empty_like(w.d)
+    stream = torch.cuda.current_stream()
+    args = (w.a_y, w.b0_y, w.c_y, w.sx, w.sz, w.d, x)
+    with tdma.Plan(w.nx, w.ny, w.nz, 1, 0) as plan:
+        for _ in range(warmup):
+            plan.solve_shared(*args, pin00=w.pin00, stream=stream)
+        torch.cuda.synchronize()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            plan.solve_shared(*args, pin00=w.pin00, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        sec = e0.elapsed_time(e1) * 1e-3 / steps
+        tiling = {k: plan.get(getattr(tdma, "TDMA_GET_SHARED_" + k.upper()))
+                  for k in ("lines", "cluster", "leaf_rows", "threads", "slots", "smem", "fill")}
+    bpc = 16.0 * w.ncomp
+    fill = tiling["fill"]
+    main_bytes = bpc * w.nx * w.ny * (w.nz - fill)
+    rec = {"ms_per_step": sec * 1e3, "value": w.cells / sec, "unit": "complex cells/s" if cplx else UNIT, "steps": steps,
+           "dtype": "c128 (f64 arithmetic)" if cplx else "f64", "alg_bytes_per_cell": bpc,
+           "hbm_gbs": bpc * w.cells / sec / 1e9, "frac_of_measured_peak": bpc * w.cells / sec / 1e9 / peak,
+           "hbm_frac_of_8TBs": bpc * w.cells / sec / 8e12,
+           "roofline": {"bound": "hbm", "kernel": "shared_tma_kernel", "achieved": main_bytes / sec / 1e9, "peak": peak,
+                        "unit": "GB/s", "frac": main_bytes / sec / 1e9 / peak, "traffic": None,
+                        "alg_bytes_per_launch": main_bytes, "launch_ms": sec * 1e3},
+           "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nz": w.nz, "ncomp": w.ncomp, "pin00": w.pin00,
+                      "tiling": tiling}}
+    # parity of what was just timed: sampled slices against the long-double reference
+    picks = pick_slices(w.nz, fill)
+    worst = 0.0
+    host = [t.cpu().numpy() for t in (w.a_y, w.b0_y, w.c_y, w.sx)]
+    def lines(v):
+        return v.view(np.float64).reshape(v.shape[0], v.shape[1], -1) if np.iscomplexobj(v) else v
+    for k in picks:
+        dk, xk = w.d[k:k + 1].cpu().numpy(), x[k:k + 1].cpu().numpy()
+        ref = oracle.solve_y_shared(*host, w.sz[k:k + 1].cpu().numpy(), dk, pin00=(w.pin00 and k == 0), precision="ld")
+        worst = max(worst, float(oracle.normwise_error(lines(np.ascontiguousarray(xk)), lines(ref)).max()))
+    rec["parity_check"] = {"slices": picks, "E_max": worst, "tol": 1e-11, "oracle": "ld", "ok": bool(worst <= 1e-11)}
+    # the CPU reference as it stands on a bounded sample (first slices), all host cores
+    nzc = min(w.nz, 16)
+    dh = w.d[:nzc].cpu().numpy()
+    szh = w.sz[:nzc].cpu().numpy()
+    oracle.solve_y_shared(*host, szh, dh, pin00=w.pin00)
+    t0, reps = time.perf_counter(), 0
+    while True:
+        oracle.solve_y_shared(*host, szh, dh, pin00=w.pin00)
+        reps += 1
+        el = time.perf_counter() - t0
+        if el >= cpu_seconds or reps >= 64:
+            break
+    rec["cpu_baseline"] = {"value": w.nx * w.ny * nzc * reps / el, "unit": rec["unit"], "cores": oracle.max_threads(),
+                           "kind": "oracle", "sample": "%d z-slices x %d repeats, %.1f s" % (nzc, reps, el)}
+    return rec
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -332,6 +399,8 @@ def main():
                     help="further workload timed after the headline one at N = 1 ('' = none)")
     ap.add_argument("--no-extras", action="store_true",
                     help="skip sustained / e2e / cpu_baseline / stage / second-workload legs")
+    ap.add_argument("--shared", default="", choices=["", "f64", "c128"],
+                    help="time only the shared-coefficient form of --workload (real / complex RHS) and print its record")
     ap.add_argument("--sweep", action="store_true", help="S7 batch x stream sweep (JSON lines)")
     ap.add_argument("--timeline", action="store_true",
                     help="S6 evidence without nsys: per-launch start/end of the PIPELINED stages of one solve "
@@ -361,6 +430,14 @@ def main():
 
     spec = tdma_inputs.config_spec(args.workload)
     nz = args.nz if args.nz > 0 else spec["nz"]
+    if args.shared:
+        rec = shared_workload(torch, tdma, tdma_inputs, args.workload, args.shared == "c128", dev, args.steps,
+                              max(3, args.warmup), group.barrier, peak, nz=nz,
+                              cpu_seconds=0.0 if args.no_extras else args.cpu_seconds / 2)
+        if rank == 0:
+            print(json.dumps(rec))
+        group.close()
+        return 0
     w = tdma_inputs.make_workload(args.workload, device=dev, nz=nz)
     x = torch.empty_like(w.d)
     batch = spec["batch"] if args.batch < 0 else args.batch
@@ -526,6 +603,17 @@ def main():
                                                                args.steps, warmup, barrier, peak)}
             except Exception as exc:
                 out["workloads"] = {args.also: {"error": repr(exc)}}
+            # NEXT row f3: the headline config in the paper's own form (shared 1-D coefficients,
+            # complex and real right-hand sides), each with its own 32 / 16 B per cell roofline
+            for tag, cplx in (("c128", True), ("f64", False)):
+                torch.cuda.empty_cache()
+                key = "%s_shared_%s" % (args.workload, tag)
+                try:
+                    out["workloads"][key] = shared_workload(torch, tdma, tdma_inputs, args.workload, cplx, dev,
+                                                            args.steps, warmup, barrier, peak,
+                                                            cpu_seconds=args.cpu_seconds / 2)
+                except Exception as exc:
+                    out["workloads"][key] = {"error": repr(exc)}
     if rank == 0:
         print(json.dumps(out))
     group.close()

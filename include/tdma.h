@@ -119,6 +119,8 @@ typedef struct tdma_options {
     int shared_cluster;  /* tdma_solve_shared: CTAs per cluster (1, 2, 4, 8), 0 = auto */
     int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16), 0 = auto */
     int shared_slots;    /* tdma_solve_shared: tiles in the shared-memory ring (2 .. 4), 0 = auto */
+    int shared_ctas;     /* tdma_solve_shared: CTAs per SM: 1, or 2 (the <= 128-register build of the
+                            16-row-leaf kernel, two CTAs co-resident); 0 = auto */
 } tdma_options;
 
 enum { TDMA_AXIS_Y = 0, TDMA_AXIS_X = 1, TDMA_AXIS_Z = 2 };

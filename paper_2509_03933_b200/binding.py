@@ -47,7 +47,7 @@ class tdma_options(ctypes.Structure):
         ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("axis", ctypes.c_int), ("periodic", ctypes.c_int),
         ("timeline", ctypes.c_int), ("fused_slots", ctypes.c_int), ("host_chunk", ctypes.c_int),
         ("shared_lines", ctypes.c_int), ("shared_cluster", ctypes.c_int), ("shared_leaf_rows", ctypes.c_int),
-        ("shared_slots", ctypes.c_int),
+        ("shared_slots", ctypes.c_int), ("shared_ctas", ctypes.c_int),
     ]
 
 
@@ -165,7 +165,7 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
                         fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0,
                         axis: int = 0, periodic: int = 0, timeline: int = 0, fused_slots: int = 0, host_chunk: int = 0,
                         shared_lines: int = 0, shared_cluster: int = 0, shared_leaf_rows: int = 0,
-                        shared_slots: int = 0) -> int:
+                        shared_slots: int = 0, shared_ctas: int = 0) -> int:
     opt = tdma_options()
     opt.struct_size = ctypes.sizeof(tdma_options)
     opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
@@ -174,6 +174,7 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
     opt.fused_fill, opt.axis, opt.periodic, opt.timeline = fused_fill, axis, periodic, timeline
     opt.host_chunk, opt.fused_slots = host_chunk, fused_slots
     opt.shared_lines, opt.shared_cluster, opt.shared_leaf_rows, opt.shared_slots = shared_lines, shared_cluster, shared_leaf_rows, shared_slots
+    opt.shared_ctas = shared_ctas
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
         raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())

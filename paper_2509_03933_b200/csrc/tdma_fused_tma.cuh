@@ -292,10 +292,15 @@ __device__ __forceinline__ void kmerge_fwd(const NodeBuf &nb, int lx, int g, int
             ab = lds2(o); cd = lds2(o + nb.plane); nb_load_d<NC>(nb, o, cd, dn);
         }
         const double nbe = fma(be, b, -(s * ga));
-        const double sc = pow2_unscale(nbe);
 #pragma unroll
-        for (int q = 0; q < NC; ++q) de[q] = fma(be, d[q], -(s * de[q])) * sc;
-        al = -(s * al) * sc; ga = be * c * sc; be = nbe * sc;
+        for (int q = 0; q < NC; ++q) de[q] = fma(be, d[q], -(s * de[q]));
+        al = -(s * al); ga = be * c; be = nbe;
+        if (i == 2 * k - 1 || ((i - 1) & 7) == 0) {          // rescale: last step, and every 8th of a long sweep
+            const double sc = pow2_unscale(be);
+#pragma unroll
+            for (int q = 0; q < NC; ++q) de[q] *= sc;
+            al *= sc; ga *= sc; be *= sc;
+        }
     }
     sts2(o, al, be); sts2(o + nb.plane, ga, de[0]);           // o: the group's last row
     if (NC == 2) sts1(nb_d1(nb, o), de[NC - 1]);
@@ -322,10 +327,15 @@ __device__ __forceinline__ void kmerge_bwd(const NodeBuf &nb, int lx, int g, int
             ab = lds2(o); cd = lds2(o + nb.plane); nb_load_d<NC>(nb, o, cd, dn);
         }
         const double nbe = fma(be, b, -(c * al));
-        const double sc = pow2_unscale(nbe);
 #pragma unroll
-        for (int q = 0; q < NC; ++q) de[q] = fma(be, d[q], -(c * de[q])) * sc;
-        ga = -(c * ga) * sc; al = be * s * sc; be = nbe * sc;
+        for (int q = 0; q < NC; ++q) de[q] = fma(be, d[q], -(c * de[q]));
+        ga = -(c * ga); al = be * s; be = nbe;
+        if (i == 0 || ((2 * k - 2 - i) & 7) == 0) {
+            const double sc = pow2_unscale(be);
+#pragma unroll
+            for (int q = 0; q < NC; ++q) de[q] *= sc;
+            al *= sc; ga *= sc; be *= sc;
+        }
     }
     sts2(o, al, be); sts2(o + nb.plane, ga, de[0]);           // o: the group's first row
     if (NC == 2) sts1(nb_d1(nb, o), de[NC - 1]);
@@ -481,19 +491,30 @@ __device__ __forceinline__ void cluster_solve_two_sided(const NodeBuf &tb, int l
         const bool fw = j < nf, bw = j < nbk;
         if (j + 1 < nf) { of += step; fab = lds2(of); fcd = lds2(of + tb.plane); nb_load_d<NC>(tb, of, fcd, fdn); }
         if (j + 1 < nbk) { ob -= step; bab = lds2(ob); bcd = lds2(ob + tb.plane); nb_load_d<NC>(tb, ob, bcd, bdn); }
+        const bool rs = (j & 7) == 7;                          // rescale every 8th step of a long sweep
         if (fw) {
             const double nbe = fma(be, fb_, -(fs * ga));
-            const double sc = pow2_unscale(nbe);
 #pragma unroll
-            for (int q = 0; q < NC; ++q) de[q] = fma(be, fd_[q], -(fs * de[q])) * sc;
-            ga = be * fc_ * sc; be = nbe * sc;
+            for (int q = 0; q < NC; ++q) de[q] = fma(be, fd_[q], -(fs * de[q]));
+            ga = be * fc_; be = nbe;
+            if (rs) {
+                const double sc = pow2_unscale(be);
+#pragma unroll
+                for (int q = 0; q < NC; ++q) de[q] *= sc;
+                ga *= sc; be *= sc;
+            }
         }
         if (bw) {
             const double nbb = fma(bb, bb_, -(bc_ * al));
-            const double sc = pow2_unscale(nbb);
 #pragma unroll
-            for (int q = 0; q < NC; ++q) dd[q] = fma(bb, bd_[q], -(bc_ * dd[q])) * sc;
-            al = bb * bs * sc; bb = nbb * sc;
+            for (int q = 0; q < NC; ++q) dd[q] = fma(bb, bd_[q], -(bc_ * dd[q]));
+            al = bb * bs; bb = nbb;
+            if (rs) {
+                const double sc = pow2_unscale(bb);
+#pragma unroll
+                for (int q = 0; q < NC; ++q) dd[q] *= sc;
+                al *= sc; bb *= sc;
+            }
         }
     }
     const double inv = rcp_nr(fma(be, bb, -(ga * al)));
@@ -985,8 +1006,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                     // thread per line), so no second exchange is needed (B2C is a local store)
                     double u0[1], u1[1];
                     cluster_solve_two_sided<TX>(tb, lx, NTR, 2 * (int)crank, u0, u1);
-                    sts1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8, u0[0]);
-                    sts1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8, u1[0]);
+                    // into the CTA's own rows of its INBOX, not into the node rows: other warps of
+                    // this CTA may still be reading those for their sends to the peers
+                    sts1(nb_ab<TX>(tb, 2 * (int)crank, lx) + tb.plane + 8, u0[0]);
+                    sts1(nb_ab<TX>(tb, 2 * (int)crank + 1, lx) + tb.plane + 8, u1[0]);
                 } else if (leaf == 0) {
                     ptx::mbar_wait(&bar[NA + par], (unsigned)((it >> 1) & 1));
                     // cyclic lines: merge the CL nodes, resolve the wrap at the root, walk back
@@ -995,8 +1018,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                     solve_root<TX>(tb, lx, NTR - 1, true);
                     kmerge_tails<TX, 0>(tb, lx, 0, 2, CL);
                     const double xf = lds1(nb_ab<TX>(tb, 0, lx) + tb.plane + 8), xl = lds1(nb_ab<TX>(tb, NTR - 1, lx) + tb.plane + 8);
-                    sts1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8, kmerge_value<TX>(tb, lx, 0, 2, CL, 2 * (int)crank, xf, xl));
-                    sts1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8, kmerge_value<TX>(tb, lx, 0, 2, CL, 2 * (int)crank + 1, xf, xl));
+                    const double v0 = kmerge_value<TX>(tb, lx, 0, 2, CL, 2 * (int)crank, xf, xl);
+                    const double v1 = kmerge_value<TX>(tb, lx, 0, 2, CL, 2 * (int)crank + 1, xf, xl);
+                    sts1(nb_ab<TX>(tb, 2 * (int)crank, lx) + tb.plane + 8, v0);
+                    sts1(nb_ab<TX>(tb, 2 * (int)crank + 1, lx) + tb.plane + 8, v1);
                 }
             }
         }
@@ -1009,8 +1034,14 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             // top-down through the tree in registers: every thread row walks from the CTA's node
             // to its own leaf (x_first / x_last of a child from those of its parent and the
             // interior-row form kmerge_tails left), no barrier, nothing written
-            double xf = lds1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8);
-            double xl = lds1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8);
+            double xf, xl;                                      // cluster: stage B left them in the inbox
+            if (kCluster) {
+                xf = lds1(nb_ab<TX>(tb, 2 * (int)crank, lx) + tb.plane + 8);
+                xl = lds1(nb_ab<TX>(tb, 2 * (int)crank + 1, lx) + tb.plane + 8);
+            } else {
+                xf = lds1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8);
+                xl = lds1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8);
+            }
             for (int l = nl - 1; l >= 0; --l) {
                 const int k = level_k(l), S = level_S(l);
                 const int node = leaf >> ((ccode >> (5 * l)) & 31u);        // my ancestor among this level's children

@@ -95,7 +95,7 @@ struct tdma_plan {
     tdma::SharedConfig sh[2], sh_fill[2];
     int sh_state[2] = {0, 0};     // 0 = not configured, 1 = ready, -1 = does not tile
     bool sh_have_fill[2] = {false, false};
-    int sh_opt[4] = {0, 0, 0, 0}; // options.shared_lines / _cluster / _leaf_rows / _slots
+    int sh_opt[5] = {0, 0, 0, 0, 0}; // options.shared_lines / _cluster / _leaf_rows / _slots / _ctas
     int sh_last = -1, sh_fill_last = 0;
     // host staging (tdma_solve_host), allocated on first use
     int hz = 0;  // slices per host chunk
@@ -562,7 +562,7 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     pl->axis = axis; pl->periodic = periodic;
     pl->host_chunk = options ? options->host_chunk : 0;
     pl->fill_opt = options ? options->fused_fill : 0;
-    if (options) { pl->sh_opt[0] = options->shared_lines; pl->sh_opt[1] = options->shared_cluster; pl->sh_opt[2] = options->shared_leaf_rows; pl->sh_opt[3] = options->shared_slots; }
+    if (options) { pl->sh_opt[0] = options->shared_lines; pl->sh_opt[1] = options->shared_cluster; pl->sh_opt[2] = options->shared_leaf_rows; pl->sh_opt[3] = options->shared_slots; pl->sh_opt[4] = options->shared_ctas; }
     pl->rs = axis == TDMA_AXIS_Z ? (long long)nx * nz : (long long)nx;   // z sweep: plan nz = caller ny
     pl->os = axis == TDMA_AXIS_Z ? (long long)nx : (long long)nx * ny;   // x sweep: slices are z-slices
     pl->bz = batch == 0 ? nz : batch;
@@ -624,7 +624,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         CUDA_TRY(cudaGetDeviceProperties(&prop, pl->device));
         const char *why = nullptr;
         if (!tdma::configure_shared(&pl->sh[q], pl->nx, pl->ny, ncomp, pl->sh_opt[0], pl->sh_opt[1], pl->sh_opt[2],
-                                    pl->sh_opt[3], prop, &why)) {
+                                    pl->sh_opt[3], pl->sh_opt[4], prop, &why)) {
             pl->sh_state[q] = -1;
             return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared unavailable for this shape: %s", why ? why : "?");
         }
@@ -633,7 +633,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         if (pl->sh[q].cluster >= 4 && pl->fill_opt >= 0) {
             const char *why2 = nullptr;
             pl->sh_have_fill[q] = tdma::configure_shared(&pl->sh_fill[q], pl->nx, pl->ny, ncomp, 0,
-                                                         pl->ny % 2 == 0 ? 2 : 1, 0, 0, prop, &why2);
+                                                         pl->ny % 2 == 0 ? 2 : 1, 0, 0, 0, prop, &why2);
         }
         pl->sh_state[q] = 1;
     }
@@ -652,7 +652,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         if (e == cudaSuccess) {
             // the fill launch, as for the general kernel (enqueue_fused): clusters of 2 on the SMs
             // the main launch's clusters cannot be placed on, solving the last nzf slices
-            const long per_sm = (long)(pl->sm_smem / (pl->sh[q].smem + 1024));
+            const long per_sm = pl->sh[q].ctas_per_sm;
             const int main_ctas = pl->sh[q].max_clusters * pl->sh[q].cluster;
             const int idle = per_sm == 1 ? pl->sm_count - main_ctas : 0;
             int fc = idle / pl->sh_fill[q].cluster;

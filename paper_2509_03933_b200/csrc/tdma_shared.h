@@ -22,6 +22,7 @@ struct SharedConfig {
     int threads = 0;    // W * TX
     int box_rows = 0;   // rows per TMA box (<= 256), divides R
     int slots = 0;      // NA: ring slots of one d / x tile each (>= 2)
+    int ctas_per_sm = 1;   // 2: the <= 128-register instantiation, two CTAs share an SM
     int max_clusters = 0;  // co-resident clusters (persistent grid), filled at first launch
     size_t smem = 0;
 };
@@ -37,7 +38,7 @@ struct SharedArgs {
 
 // Tiling for ny-row lines: CL x W x M0 with W a power of two.  want_* = 0: auto.
 bool configure_shared(SharedConfig *out, int nx, int ny, int ncomp, int want_lines, int want_cluster,
-                      int want_leaf, int want_slots, const cudaDeviceProp &prop, const char **why);
+                      int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why);
 
 // nzs = 0: prepare only (function attributes, persistent grid size).
 cudaError_t launch_shared(SharedConfig &cfg, const SharedArgs &args, cudaStream_t st);

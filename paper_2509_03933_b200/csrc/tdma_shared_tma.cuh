@@ -189,8 +189,8 @@ __device__ __forceinline__ void leaf_back_sh(const ShLeafRegs<M0, NC> &R, const 
 // Threads: leaf = t / TX, lx = t % TX; the last warp issues the TMA copies and takes no part in
 // the tree (as in fused_tma_kernel).  Ring: tile q of the cluster lives in slot q % NA from its
 // load until the TMA store of its x has read the slot; then tile q + NA is loaded into it.
-template <int TX, int M0, bool kCluster, int MAXT, int NC>
-__global__ void __launch_bounds__(MAXT, 1)
+template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB)
 shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_x,
                   const SharedParams prm)
 {
@@ -284,6 +284,14 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
     const int crit_threads = helper_mode ? cw * 32 : tree_threads;
     const bool crit = tree && leaf < help0, helper = tree && !crit;
 
+    // tile -> (x tile, slice), ring slot and its mbarrier phase, advanced without divisions
+    const int step_x = NC_ % prm.xtiles, step_k = NC_ / prm.xtiles;
+    int xt = g % prm.xtiles, k = g / prm.xtiles, slot = 0, sphase = 0;
+    auto shift_of = [&](int xt_, int k_) {                     // the line's shift
+        const int gi_ = xt_ * TX + lx < prm.nx ? xt_ * TX + lx : prm.nx - 1;   // ragged x tile: lanes past nx solve a copy
+        return prm.sx[gi_] + prm.sz[k_ < prm.nzs ? k_ : prm.nzs - 1];
+    };
+    double s_next = g < prm.ntiles ? shift_of(xt, k) : 0.0;
     int it = 0;
     for (int tile = g; tile < prm.ntiles; tile += NC_, ++it) {
         const int par = it & 1;
@@ -291,13 +299,16 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         tb.ab += (uint32_t)par * inbox_bytes; tb.d1 += (uint32_t)par * inbox_bytes;
         if (kCluster && t == 0)
             ptx::mbar_expect_tx(&bar[NA + par], (unsigned)(NTR * TX * (32 + 8 * (NC - 1))));
-        const int slot = it % NA;
-        const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
-        const int gi = x0 + lx < prm.nx ? x0 + lx : prm.nx - 1;    // ragged x tile: lanes past nx solve a copy
-        const double s = prm.sx[gi] + prm.sz[k];                   // the line's shift
-        const bool pin = prm.pin00 != 0 && first_leaf && gi == 0 && k == 0;
+        const double s = s_next;
+        const bool pin = prm.pin00 != 0 && first_leaf && xt * TX + lx == 0 && k == 0;
         const uint32_t dbase = ptx::smem_u32(raw + (size_t)slot * arr) + leaf_off;
-        ptx::mbar_wait(&bar[slot], (unsigned)((it / NA) & 1));
+        const int cur_slot = slot, cur_phase = sphase;
+        // next tile's coordinates; its shift is fetched now, a whole tile period ahead of its use
+        xt += step_x; k += step_k;
+        if (xt >= prm.xtiles) { xt -= prm.xtiles; ++k; }
+        if (++slot == NA) { slot = 0; sphase ^= 1; }
+        if (tile + NC_ < prm.ntiles) s_next = shift_of(xt, k);
+        ptx::mbar_wait(&bar[cur_slot], (unsigned)cur_phase);
 
         // ---------------- leaves ----------------
         ShLeafRegs<M0, NC> regs;
@@ -386,8 +397,10 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
                     // Stage B: every CTA computes its own two unknowns of the 2 CL-row system
                     double u0[NC], u1[NC];
                     cluster_solve_two_sided<TX, NC>(tb, lx, NTR, 2 * (int)crank, u0, u1);
-                    nb_store_d<NC>(nb, nb_ab<TX>(nb, 0, lx), u0);
-                    nb_store_d<NC>(nb, nb_ab<TX>(nb, 2 * W - 1, lx), u1);
+                    // into the CTA's own rows of its INBOX, not into the node rows: other warps of
+                    // this CTA may still be reading those for their sends to the peers
+                    nb_store_d<NC>(tb, nb_ab<TX>(tb, 2 * (int)crank, lx), u0);
+                    nb_store_d<NC>(tb, nb_ab<TX>(tb, 2 * (int)crank + 1, lx), u1);
                 }
             }
         }
@@ -396,8 +409,13 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         // ---------------- top-down walk + leaf back-substitution, x written in place ----------
         if (act) {
             double xf[NC], xl[NC];
-            nb_load_donly<NC>(nb, nb_ab<TX>(nb, 0, lx), xf);
-            nb_load_donly<NC>(nb, nb_ab<TX>(nb, 2 * W - 1, lx), xl);
+            if (kCluster) {
+                nb_load_donly<NC>(tb, nb_ab<TX>(tb, 2 * (int)crank, lx), xf);
+                nb_load_donly<NC>(tb, nb_ab<TX>(tb, 2 * (int)crank + 1, lx), xl);
+            } else {
+                nb_load_donly<NC>(nb, nb_ab<TX>(nb, 0, lx), xf);
+                nb_load_donly<NC>(nb, nb_ab<TX>(nb, 2 * W - 1, lx), xl);
+            }
             for (int l = nl - 1; l >= 0; --l) {
                 const int kk = level_k(l), S = level_S(l);
                 const int node = leaf >> ((ccode >> (5 * l)) & 31u);
@@ -437,18 +455,18 @@ inline size_t shared_smem_bytes(int TX, int R, int W, int CL, int NA, int NC)
 constexpr int kSharedLeafSizes[] = {16, 8, 4};
 
 inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int want_lines, int want_cluster,
-                                  int want_leaf, int want_slots, const cudaDeviceProp &prop, const char **why)
+                                  int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why)
 {
     if (NC != 1 && NC != 2) { *why = "ncomp must be 1 (real) or 2 (complex)"; return false; }
     if ((nx * NC) % 2) { *why = "TMA path needs an even number of doubles per row (16-byte global strides)"; return false; }
     const size_t max_smem = prop.sharedMemPerBlockOptin;
     SharedConfig best; double best_score = -1.0;
     // lines per tile: 128-byte row segments first (16 real / 8 complex cells), then 256-byte ones
-    const int tx_opts[2] = {NC == 1 ? 16 : 8, NC == 1 ? 32 : 16};
+    const int tx_opts[3] = {NC == 1 ? 16 : 8, NC == 1 ? 32 : 16, NC == 1 ? 8 : 4};
     const int cl_opts[4] = {1, 2, 4, 8};
-    for (int ti = 0; ti < 2; ++ti) {
+    for (int ti = 0; ti < 3; ++ti) {
         const int TX = tx_opts[ti];
-        if (want_lines && TX != want_lines) continue;
+        if (want_lines ? TX != want_lines : ti == 2) continue;      // 64-byte segments only on request
         for (int ci = 0; ci < 4; ++ci) {
             const int CL = cl_opts[ci];
             if (want_cluster && CL != want_cluster) continue;
@@ -470,6 +488,16 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
                     if (c.smem <= max_smem) { c.slots = na; break; }
                 }
                 if (!c.slots) continue;
+                c.ctas_per_sm = 1;
+                if (want_ctas >= 2) {          // co-residency: registers and shared memory shared out
+                    if (c.threads * want_ctas > 512 || m0 != 16) continue;
+                    for (; c.slots >= 2; --c.slots) {
+                        c.smem = shared_smem_bytes(TX, R, c.leaves, CL, c.slots, NC);
+                        if ((size_t)want_ctas * (c.smem + 1024) <= prop.sharedMemPerMultiprocessor) break;
+                    }
+                    if (c.slots < 2) continue;
+                    c.ctas_per_sm = want_ctas;
+                }
                 // as for the general kernel: long leaves (fewer tree levels) first, then 256 threads
                 // per CTA (255 registers each), 128-byte segments, a deep ring, small clusters
                 const double score = 10000.0 * m0 + (c.threads == 256 ? 4000.0 : (c.threads > 256 ? 1000.0 : 2000.0 + c.threads)) +
@@ -502,10 +530,10 @@ inline bool make_shared_tensor_map(CUtensorMap *tm, const void *base, int nx, in
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int TX, int M0, bool kCluster, int MAXT, int NC>
+template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB = 1>
 inline cudaError_t launch_shared_inst(SharedConfig &cfg, const CUtensorMap *tm, const SharedParams &prm, cudaStream_t st)
 {
-    auto kern = shared_tma_kernel<TX, M0, kCluster, MAXT, NC>;
+    auto kern = shared_tma_kernel<TX, M0, kCluster, MAXT, NC, MINB>;
     cudaLaunchConfig_t lc = {};
     lc.blockDim = dim3((cfg.threads + 31) & ~31);
     lc.dynamicSmemBytes = cfg.smem;
@@ -543,6 +571,16 @@ template <int TX, int NC, bool kCluster>
 inline cudaError_t launch_shared_tx(SharedConfig &cfg, const CUtensorMap *tm, const SharedParams &prm, cudaStream_t st)
 {
     const bool big = cfg.threads > 256;
+    // co-resident CTAs: one sweeps while another walks its tree.  128-thread CTAs keep up to 255
+    // (two per SM) or 168 (three) registers per thread, 256-thread CTAs 128
+    if (cfg.ctas_per_sm >= 2 && cfg.leaf_rows == 16 && !big) {
+        if (cfg.threads <= 128) {
+            if (cfg.ctas_per_sm == 2) return launch_shared_inst<TX, 16, kCluster, 128, NC, 2>(cfg, tm, prm, st);
+            if (cfg.ctas_per_sm == 3) return launch_shared_inst<TX, 16, kCluster, 128, NC, 3>(cfg, tm, prm, st);
+            return launch_shared_inst<TX, 16, kCluster, 128, NC, 4>(cfg, tm, prm, st);
+        }
+        return launch_shared_inst<TX, 16, kCluster, 256, NC, 2>(cfg, tm, prm, st);
+    }
     switch (cfg.leaf_rows) {
     case 16: return big ? launch_shared_inst<TX, 16, kCluster, 512, NC>(cfg, tm, prm, st)
                         : launch_shared_inst<TX, 16, kCluster, 256, NC>(cfg, tm, prm, st);
@@ -571,6 +609,7 @@ inline cudaError_t launch_shared_impl(SharedConfig &cfg, const SharedArgs &a, cu
     prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
     const bool cl = cfg.cluster > 1;
     if (cfg.ncomp == 1) {
+        if (cfg.lines == 8) return cl ? launch_shared_tx<8, 1, true>(cfg, tm, prm, st) : launch_shared_tx<8, 1, false>(cfg, tm, prm, st);
         if (cfg.lines == 16) return cl ? launch_shared_tx<16, 1, true>(cfg, tm, prm, st) : launch_shared_tx<16, 1, false>(cfg, tm, prm, st);
         if (cfg.lines == 32) return cl ? launch_shared_tx<32, 1, true>(cfg, tm, prm, st) : launch_shared_tx<32, 1, false>(cfg, tm, prm, st);
     } else {

@@ -175,3 +175,16 @@ def test_unsupported_shapes_fail_loudly():
     with tdma.Plan(32, 64, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, periodic=1) as plan:
         with pytest.raises(tdma.TdmaError):
             plan.solve_shared(*t, torch.empty_like(t[5]))
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+def test_fill_launch_is_repeatable(cplx):
+    """cfg-3 slab in the automatic tiling (main launch + fill launch with 512-thread CTAs), solved
+    repeatedly: every solve must match the reference.  (Regression: stage B once wrote its result
+    over node rows that slower warps of the same CTA were still sending to the peer CTAs.)"""
+    w = tdma_inputs.make_shared_workload("cfg3_weak", cplx, nz=16)
+    ref = as_lines(oracle_shared(w, "ld"))
+    for rep in range(8):
+        x, info = gpu_solve_shared(w)
+        E = oracle.normwise_error(as_lines(x.cpu().numpy()), ref).max()
+        assert E <= TOL_E, "solve %d: normwise error %.3e (fill %d)" % (rep, E, info["fill"])
