@@ -247,6 +247,15 @@ int tdma_plan_autotune(int nx, int ny, int nz, int P, int dtype, int nstreams, c
                        int ncand, const void *a, const void *b, const void *c, const void *d, void *x,
                        int *best_batch, double *est_ms);
 
+/* fp64 ALU probe: measures on the current device and writes to result[0..5]
+ *   [0] DFMA throughput with many independent chains, TFLOP/s (1 DFMA = 2 flop)
+ *   [1] the same as DFMA per SM and cycle at the nominal SM clock
+ *   [2] cycles per DEPENDENT DFMA            [3] cycles per dependent Newton reciprocal + DADD
+ *   [4] cycles per dependent IEEE division + DADD       [5] nominal SM clock, MHz
+ * n = capacity of result (>= 6).  Synchronises; a measurement utility for bench.py's "alu" roofline
+ * of the shared-coefficient form, not part of the solve path. */
+int tdma_probe_fp64(double *result, int n);
+
 int tdma_plan_destroy(tdma_plan *plan);
 const char *tdma_last_error(void); /* thread-local, never NULL */
 int tdma_version(void);            /* 10000*major + 100*minor + patch */

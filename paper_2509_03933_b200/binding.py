@@ -34,7 +34,7 @@ EXPORTED_SYMBOLS = (
     "tdma_plan_create", "tdma_plan_create_ex", "tdma_solve", "tdma_solve_host", "tdma_stage",
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
     "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
-    "tdma_solve_shared",
+    "tdma_solve_shared", "tdma_probe_fp64",
 )
 
 
@@ -91,6 +91,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_solve.restype = ci
     lib.tdma_solve_shared.argtypes = [vp] * 6 + [ci, ci] + [vp] * 3
     lib.tdma_solve_shared.restype = ci
+    lib.tdma_probe_fp64.argtypes = [ctypes.POINTER(ctypes.c_double), ci]
+    lib.tdma_probe_fp64.restype = ci
     lib.tdma_solve_host.argtypes = [vp] * 6
     lib.tdma_solve_host.restype = ci
     lib.tdma_stage.argtypes = [vp, ci, ci] + [vp] * 6
@@ -189,6 +191,15 @@ def tdma_solve(plan: int, a, b, c, d, x, stream=None) -> None:
 def tdma_solve_shared(plan: int, a_y, b0_y, c_y, sx, sz, ncomp: int, pin00: int, d, x, stream=None) -> None:
     _check(load_library().tdma_solve_shared(plan, _ptr(a_y), _ptr(b0_y), _ptr(c_y), _ptr(sx), _ptr(sz),
                                             int(ncomp), int(pin00), _ptr(d), _ptr(x), _stream_handle(stream)))
+
+
+def tdma_probe_fp64() -> dict:
+    """fp64 ALU probe of the current device (include/tdma.h)."""
+    r = (ctypes.c_double * 6)()
+    _check(load_library().tdma_probe_fp64(r, 6))
+    keys = ("dfma_tflops", "dfma_per_sm_cycle", "dfma_latency_cycles", "rcp_nr_latency_cycles",
+            "div_latency_cycles", "sm_clock_mhz")
+    return dict(zip(keys, [float(v) for v in r]))
 
 
 def tdma_solve_host(plan: int, a, b, c, d, x) -> None:

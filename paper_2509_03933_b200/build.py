@@ -18,6 +18,7 @@ _TDMA_H = os.path.join("..", "..", "include", "tdma.h")
 UNITS = {
     "tdma_plan.cu": ["tdma_stage_kernels.cuh", "tdma_fused.cuh", "tdma_fused_tma.cuh", "tdma_shared.h", _TDMA_H],
     "tdma_shared.cu": ["tdma_shared_tma.cuh", "tdma_fused_tma.cuh", "tdma_shared.h"],
+    "tdma_probe.cu": [_TDMA_H],
 }
 OBJ_DIR = os.path.join(CSRC, "build")
 

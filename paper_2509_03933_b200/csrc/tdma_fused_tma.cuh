@@ -905,7 +905,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     const int mrows = helper_mode ? crit_rows : Wt;                  // rows that share the merges of a level
     const int crit_threads = helper_mode ? cw * 32 : tree_threads;
     const bool crit = tree && leaf < help0, helper = tree && !crit;
-    int it = 0;
+    int it = 0, sn = 0, pn = 0;
     for (int tile = g; tile < prm.ntiles; tile += NC, ++it) {
         const int par = it & 1;
         NodeBuf tb = tb0;                                      // this tile's inbox
@@ -913,10 +913,20 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         // arm this tile's inbox: 4 doubles per (node equation, line) from every CTA
         if (kCluster && t == 0) ptx::mbar_expect_tx(&bar[NA + par], (unsigned)(4 * NTR * TX * sizeof(double)));
         const int n0 = 4 * it;
-        const double *__restrict__ sB = raw + (size_t)(n0 % NA) * arr, *__restrict__ sA = raw + (size_t)((n0 + 1) % NA) * arr;
-        const double *__restrict__ sC = raw + (size_t)((n0 + 2) % NA) * arr, *__restrict__ sD = raw + (size_t)((n0 + 3) % NA) * arr;
+        // ring slot / mbarrier phase of the tile's four arrays, advanced without divisions:
+        // (sn, pn) = (n0 % NA, (n0 / NA) & 1); array j sits j slots further (at most one wrap, NA >= 4)
+        int sl[4], ph[4];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) ptx::mbar_wait(&bar[(n0 + j) % NA], (unsigned)(((n0 + j) / NA) & 1));
+        for (int j = 0; j < 4; ++j) {
+            sl[j] = sn + j; ph[j] = pn;
+            if (sl[j] >= NA) { sl[j] -= NA; ph[j] ^= 1; }
+        }
+        sn += 4;
+        if (sn >= NA) { sn -= NA; pn ^= 1; }
+        const double *__restrict__ sB = raw + (size_t)sl[0] * arr, *__restrict__ sA = raw + (size_t)sl[1] * arr;
+        const double *__restrict__ sC = raw + (size_t)sl[2] * arr, *__restrict__ sD = raw + (size_t)sl[3] * arr;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) ptx::mbar_wait(&bar[sl[j]], (unsigned)ph[j]);
 
         // ---------------- leaves ----------------
         LeafRegs<M0> regs;

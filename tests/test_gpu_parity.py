@@ -380,6 +380,34 @@ def test_tma_fused_unaligned_pointers_fall_back():
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("mode", ["up500", "down500", "mixed", "tiny_pivots"])
+def test_row_scaling_extremes(variant, mode):
+    """Numerical edge of the reciprocal path (D2: Newton reciprocal valid for pivots with
+    2^-1021 < |p| < 2^1021, tree rows carried un-normalised).  Scaling row j of a system by 2^e_j
+    leaves x unchanged and is exact in fp64, so the scaled system must still match the reference
+    on the same scaled arrays: all rows x 2^500, all x 2^-500, a different power per row in
+    [-300, 300], and pivots near 2^-1000."""
+    nz, ny, nx = 3, 512, 64
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 77, dev())
+    g = torch.Generator().manual_seed(5)
+    if mode == "up500":
+        e = torch.full((nz, ny, nx), 500.0, dtype=torch.float64)
+    elif mode == "down500":
+        e = torch.full((nz, ny, nx), -500.0, dtype=torch.float64)
+    elif mode == "mixed":
+        e = torch.randint(-300, 301, (nz, ny, nx), generator=g).to(torch.float64)
+    else:
+        e = torch.full((nz, ny, nx), -1001.0, dtype=torch.float64)          # b in [2, 5) -> pivots ~ 2^-1000
+    sc = torch.pow(torch.tensor(2.0, dtype=torch.float64), e).to(dev())
+    a, b, c, d = a * sc, b * sc, c * sc, d * sc
+    x = gpu_solve(a, b, c, d, 16, 0, **variant)
+    an, bn, cn, dn, xn = to_np(a, b, c, d, x)
+    assert np.isfinite(xn).all()
+    ref = oracle.solve_y(an, bn, cn, dn, "f64")
+    assert oracle.normwise_error(xn, ref).max() <= TOL_E
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_identity_and_diagonal(variant):
     for diag in (False, True):
         a, b, c, d = tdma_inputs.identity_system(32, 16, 3, 2, dev(), diagonal_only=diag)
