@@ -247,6 +247,43 @@ int tdma_plan_autotune(int nx, int ny, int nz, int P, int dtype, int nstreams, c
                        int ncand, const void *a, const void *b, const void *c, const void *d, void *x,
                        int *best_batch, double *est_ms);
 
+/* ---------------------------------------------------------------------------------------------
+ * y-slab decomposition over several GPUs -- the paper's own multi-GPU
+ * setting: "the domain is decomposed along the y-direction" (Fig. 1c); rank r owns
+ * rows r*ny_local .. (r+1)*ny_local-1 of every line.  Per batch (Alg. 2):
+ *   stage A  every rank reduces its slab (P_local partitions of ny_local / P_local rows) to two
+ *            boundary equations per partition and writes them, 6 doubles each, into `send`;
+ *   A2B      all-to-all: the Lb = nx * slices lines of the batch are dealt out evenly, Ls = Lb /
+ *            nranks to each rank ("even distribution");
+ *   stage B  every rank solves the 2 * P_local * nranks-row reduced systems of its Ls lines;
+ *   B2C      all-to-all back: the two boundary unknowns of every partition;
+ *   stage C  every rank back-substitutes inside its partitions.
+ * This library provides the rank-local stages; the two all-to-alls are the caller's (yslab.py:
+ * torch.distributed all_to_all_single over NCCL on a communication stream, pipelined over batches
+ * as Alg. 2).  Buffer layouts (doubles, line fastest), P = P_local:
+ *   send  [nranks dest][P][6][Ls]  (fa, fc, fd | pa, pc, pd): reduced rows 2p, 2p+1 (unit diagonal) of
+ *                                  line dest*Ls + j;   recv = the same as [nranks src][P][6][Ls]
+ *   yout  [nranks dest][2P][Ls]    reduced solution rows of rank dest's partitions for MY Ls lines;
+ *   yrecv [nranks src][2P][Ls]     x_first / x_last of MY partitions for the lines rank src solved.
+ * Ls is that of the batch (the last batch of nz % batch slices is shorter).  a, b, c, d, x: DEVICE
+ * pointers to the rank's slab, nx*ny_local*nz doubles, element (i,j,k) at i + nx*(j + ny_local*k);
+ * a at the global row 0 (rank 0) and c at the global last row (rank nranks-1) are ignored.
+ * tdma_slab_create returns NULL on invalid arguments (ny_local % P_local != 0, fewer than 2 rows per
+ * partition, nx*batch or nx*(nz % batch) not divisible by nranks), without a CUDA device, or when
+ * the scratch ring (3 batches of a', c', d' + reduced buffers) cannot be allocated.  Enqueue-only. */
+typedef struct tdma_slab tdma_slab;
+typedef enum tdma_slab_query {
+    TDMA_SLAB_NB = 0, TDMA_SLAB_BATCH = 1, TDMA_SLAB_LINES = 2 /* Lb of a full batch */,
+    TDMA_SLAB_SHARE = 3 /* Ls of a full batch */, TDMA_SLAB_PTOT = 4
+} tdma_slab_query;
+tdma_slab *tdma_slab_create(int nx, int ny_local, int nz, int P_local, int batch, int rank, int nranks);
+int tdma_slab_get(const tdma_slab *slab, int what);
+int tdma_slab_stage_a(tdma_slab *slab, int batch_index, const void *a, const void *b, const void *c,
+                      const void *d, void *send, void *stream);
+int tdma_slab_stage_b(tdma_slab *slab, int batch_index, const void *recv, void *yout, void *stream);
+int tdma_slab_stage_c(tdma_slab *slab, int batch_index, const void *yrecv, void *x, void *stream);
+int tdma_slab_destroy(tdma_slab *slab);
+
 /* fp64 ALU probe: measures on the current device and writes to result[0..5]
  *   [0] DFMA throughput with many independent chains, TFLOP/s (1 DFMA = 2 flop)
  *   [1] the same as DFMA per SM and cycle at the nominal SM clock

@@ -35,7 +35,10 @@ EXPORTED_SYMBOLS = (
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
     "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
     "tdma_solve_shared", "tdma_probe_fp64",
+    "tdma_slab_create", "tdma_slab_get", "tdma_slab_stage_a", "tdma_slab_stage_b", "tdma_slab_stage_c",
+    "tdma_slab_destroy",
 )
+TDMA_SLAB_NB, TDMA_SLAB_BATCH, TDMA_SLAB_LINES, TDMA_SLAB_SHARE, TDMA_SLAB_PTOT = range(5)
 
 
 class tdma_options(ctypes.Structure):
@@ -91,6 +94,18 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_solve.restype = ci
     lib.tdma_solve_shared.argtypes = [vp] * 6 + [ci, ci] + [vp] * 3
     lib.tdma_solve_shared.restype = ci
+    lib.tdma_slab_create.argtypes = [ci] * 7
+    lib.tdma_slab_create.restype = vp
+    lib.tdma_slab_get.argtypes = [vp, ci]
+    lib.tdma_slab_get.restype = ci
+    lib.tdma_slab_stage_a.argtypes = [vp, ci] + [vp] * 6
+    lib.tdma_slab_stage_a.restype = ci
+    lib.tdma_slab_stage_b.argtypes = [vp, ci] + [vp] * 3
+    lib.tdma_slab_stage_b.restype = ci
+    lib.tdma_slab_stage_c.argtypes = [vp, ci] + [vp] * 3
+    lib.tdma_slab_stage_c.restype = ci
+    lib.tdma_slab_destroy.argtypes = [vp]
+    lib.tdma_slab_destroy.restype = ci
     lib.tdma_probe_fp64.argtypes = [ctypes.POINTER(ctypes.c_double), ci]
     lib.tdma_probe_fp64.restype = ci
     lib.tdma_solve_host.argtypes = [vp] * 6
@@ -191,6 +206,38 @@ def tdma_solve(plan: int, a, b, c, d, x, stream=None) -> None:
 def tdma_solve_shared(plan: int, a_y, b0_y, c_y, sx, sz, ncomp: int, pin00: int, d, x, stream=None) -> None:
     _check(load_library().tdma_solve_shared(plan, _ptr(a_y), _ptr(b0_y), _ptr(c_y), _ptr(sx), _ptr(sz),
                                             int(ncomp), int(pin00), _ptr(d), _ptr(x), _stream_handle(stream)))
+
+
+def tdma_slab_create(nx: int, ny_local: int, nz: int, P_local: int, batch: int, rank: int, nranks: int) -> int:
+    h = load_library().tdma_slab_create(nx, ny_local, nz, P_local, batch, rank, nranks)
+    if not h:
+        raise TdmaError(TDMA_ERR_INVALID_ARG, "tdma_slab_create failed (invalid shape for %d ranks, no CUDA device, "
+                                              "or out of memory)" % nranks)
+    return int(h)
+
+
+def tdma_slab_get(slab: int, what: int) -> int:
+    v = int(load_library().tdma_slab_get(slab, what))
+    if v < 0:
+        raise TdmaError(v, "tdma_slab_get(%d)" % what)
+    return v
+
+
+def tdma_slab_stage_a(slab: int, batch_index: int, a, b, c, d, send, stream=None) -> None:
+    _check(load_library().tdma_slab_stage_a(slab, batch_index, _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(send),
+                                            _stream_handle(stream)))
+
+
+def tdma_slab_stage_b(slab: int, batch_index: int, recv, yout, stream=None) -> None:
+    _check(load_library().tdma_slab_stage_b(slab, batch_index, _ptr(recv), _ptr(yout), _stream_handle(stream)))
+
+
+def tdma_slab_stage_c(slab: int, batch_index: int, yrecv, x, stream=None) -> None:
+    _check(load_library().tdma_slab_stage_c(slab, batch_index, _ptr(yrecv), _ptr(x), _stream_handle(stream)))
+
+
+def tdma_slab_destroy(slab: int) -> None:
+    _check(load_library().tdma_slab_destroy(slab))
 
 
 def tdma_probe_fp64() -> dict:

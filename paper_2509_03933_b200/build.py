@@ -19,6 +19,7 @@ UNITS = {
     "tdma_plan.cu": ["tdma_stage_kernels.cuh", "tdma_fused.cuh", "tdma_fused_tma.cuh", "tdma_shared.h", _TDMA_H],
     "tdma_shared.cu": ["tdma_shared_tma.cuh", "tdma_fused_tma.cuh", "tdma_shared.h"],
     "tdma_probe.cu": [_TDMA_H],
+    "tdma_slab.cu": ["tdma_stage_kernels.cuh", _TDMA_H],
 }
 OBJ_DIR = os.path.join(CSRC, "build")
 

@@ -135,6 +135,7 @@ tdma::StageParams batch_params(const tdma_plan *pl, const SlabPtrs &ptr, int nz_
     prm.Lb = (long long)pl->nx * bzn;
     prm.nx = pl->nx; prm.ny = pl->ny; prm.m = pl->m; prm.P = pl->P;
     prm.rs = pl->rs; prm.os = pl->os;
+    prm.pg0 = 0; prm.Ptot = pl->P; prm.Ls = 0;
     return prm;
 }
 
@@ -145,9 +146,9 @@ int launch_stage(const tdma_plan *pl, int stage, const tdma::StageParams &prm, c
     case TDMA_STAGE_A: {
         dim3 grid((Lb + 127) / 128, pl->P);
         if (pl->separate_gather)
-            tdma::stage_a_kernel<kPrefetchRows, true><<<grid, 128, 0, st>>>(prm);
+            tdma::stage_a_kernel<kPrefetchRows, tdma::kOutSendA><<<grid, 128, 0, st>>>(prm);
         else
-            tdma::stage_a_kernel<kPrefetchRows, false><<<grid, 128, 0, st>>>(prm);
+            tdma::stage_a_kernel<kPrefetchRows, tdma::kOutReduced><<<grid, 128, 0, st>>>(prm);
         break;
     }
     case TDMA_STAGE_GATHER: {

@@ -44,12 +44,21 @@ struct StageParams {
     long long rs, os;             // caller arrays: element stride between rows of a line / between
                                   // slices (y sweep: nx, nx*ny; z sweep: nx*ny, nx); scratch is
                                   // always [slice][row][x]
+    // y-slab decomposition (tdma_slab.cu): this launch holds partitions pg0 .. pg0+P-1
+    // of Ptot; the lines of a batch are dealt out evenly, Ls to each rank (single GPU: 0, P, 0)
+    int pg0 = 0, Ptot = 0;
+    long long Ls = 0;
 };
+
+// where stage A's two boundary equations per (line, partition) go
+enum { kOutReduced = 0,   // RA / RC / RD rows 2p, 2p+1 (gather fused into the epilogue)
+       kOutSendA = 1,     // send_A[P][6][Lb] for the separate gather kernel
+       kOutSlab = 2 };    // send[dest rank][P][6][Ls], dest = l / Ls: the all-to-all's send buffer
 
 // ------------------------------------------------------------------------------------------
 // Stage A
 // ------------------------------------------------------------------------------------------
-template <int U, bool kSeparateGather>
+template <int U, int kOut>
 __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
 {
     const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -68,7 +77,7 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
     double *__restrict__ sc = prm.sc + soff0;
     double *__restrict__ sd = prm.sd + soff0;
     const size_t s = (size_t)prm.rs, ss = (size_t)nx;
-    const bool first_part = (p == 0), last_part = (p == prm.P - 1);
+    const bool first_part = (prm.pg0 + p == 0), last_part = (prm.pg0 + p == prm.Ptot - 1);
 
     // first-row equation  fa x_{-1} + fb x_0 + fc x_frontier = fd
     double inv = 1.0 / ld_stream(b);
@@ -131,10 +140,15 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
     // m == 2: first-row equation is already (fa, 1, fc | fd) with frontier x_1 = x_{m-1}
     inv = 1.0 / fb;
     const size_t Lb = (size_t)prm.Lb;
-    if (kSeparateGather) {
+    if (kOut == kOutSendA) {
         double *__restrict__ sp = prm.send + (size_t)p * 6 * Lb + l;
         st_keep(sp, fa * inv); st_keep(sp + Lb, fc * inv); st_keep(sp + 2 * Lb, fd * inv);
         st_keep(sp + 3 * Lb, pa); st_keep(sp + 4 * Lb, pc); st_keep(sp + 5 * Lb, pd);
+    } else if (kOut == kOutSlab) {
+        const size_t Ls = (size_t)prm.Ls, dest = (size_t)l / Ls, j = (size_t)l - dest * Ls;
+        double *__restrict__ sp = prm.send + ((dest * prm.P + p) * 6) * Ls + j;
+        st_keep(sp, fa * inv); st_keep(sp + Ls, fc * inv); st_keep(sp + 2 * Ls, fd * inv);
+        st_keep(sp + 3 * Ls, pa); st_keep(sp + 4 * Ls, pc); st_keep(sp + 5 * Ls, pd);
     } else {
         const size_t q0 = (size_t)(2 * p) * Lb + l, q1 = q0 + Lb;
         st_keep(prm.ra + q0, fa * inv); st_keep(prm.rc + q0, fc * inv); st_keep(prm.rd + q0, fd * inv);
@@ -144,7 +158,7 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
 
 // Separate A2B gather ("Save data in send_A" / "Get data from recv_B"):
 // send[p][6][Lb] -> RA/RC/RD[2P][Lb].  One thread per (line, partition).
-__global__ void __launch_bounds__(256) gather_kernel(const StageParams prm)
+static __global__ void __launch_bounds__(256) gather_kernel(const StageParams prm)
 {
     const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (l >= prm.Lb) return;
@@ -215,7 +229,9 @@ __global__ void __launch_bounds__(64) stage_b_kernel(const StageParams prm)
 // ------------------------------------------------------------------------------------------
 // Stage C: back-substitution inside each partition, one thread per (line, partition).
 // ------------------------------------------------------------------------------------------
-template <int U>
+// kSlab: x_first / x_last come from the all-to-all's receive buffer yrecv[src rank][2 P][Ls] (prm.y),
+// src = l / Ls (the rank that solved the line's reduced system).
+template <int U, bool kSlab = false>
 __global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
 {
     const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -233,8 +249,15 @@ __global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
     const size_t s = (size_t)prm.rs, ss = (size_t)nx;
     const size_t Lb = (size_t)prm.Lb;
 
-    const double xf = ld_keep(prm.y + (size_t)(2 * p) * Lb + l);
-    const double xl = ld_keep(prm.y + (size_t)(2 * p + 1) * Lb + l);
+    double xf, xl;
+    if (kSlab) {
+        const size_t Ls = (size_t)prm.Ls, src = (size_t)l / Ls, j = (size_t)l - src * Ls;
+        const double *__restrict__ yp = prm.y + (src * 2 * prm.P + 2 * p) * Ls + j;
+        xf = ld_keep(yp); xl = ld_keep(yp + Ls);
+    } else {
+        xf = ld_keep(prm.y + (size_t)(2 * p) * Lb + l);
+        xl = ld_keep(prm.y + (size_t)(2 * p + 1) * Lb + l);
+    }
     st_stream(x, xf);
     st_stream(x + (size_t)(m - 1) * s, xl);
     double xn = xl;
@@ -266,7 +289,7 @@ __global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
 }
 
 // ny == 1 (only possible with P == 1): x = d / b.
-__global__ void __launch_bounds__(256) diagonal_kernel(const double *__restrict__ b,
+static __global__ void __launch_bounds__(256) diagonal_kernel(const double *__restrict__ b,
                                                        const double *__restrict__ d,
                                                        double *__restrict__ x, size_t n)
 {

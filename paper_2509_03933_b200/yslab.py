@@ -1,0 +1,182 @@
+"""y-slab decomposition over several GPUs: the paper's own multi-GPU
+setting ("the domain is decomposed along the y-direction"; PAPER.md:106 the
+all-to-all with even distribution; Alg. 2, the batch pipeline).
+
+One process per GPU.  Rank r owns rows ``r*ny_local .. (r+1)*ny_local-1`` of every line.  The
+rank-local stages are the library's kernels (``tdma_slab_stage_a / _b / _c`` of include/tdma.h); this
+module is the plumbing around them: buffers, streams and events, and the two exchanges per batch as
+``torch.distributed.all_to_all_single`` (NCCL on GPUs; the transfers are ``48 * P_local * Lb`` bytes
+out and ``16 * P_local * Lb`` bytes back per rank and batch, a few MiB, so the library collective
+on its own stream is the right tool -- no arithmetic happens here).
+
+Schedule (Alg. 2 with events instead of stream synchronisation), iteration n = 0 .. nb+1:
+    A(n) on the A+C stream            -> A2B(n)   on the communication stream
+    B(n-1) on the B stream            -> B2C(n-1) on the communication stream
+    C(n-2) on the A+C stream
+so the reduced solve and both exchanges of a batch run behind the partition stages of its
+neighbours.  Ring of 3 buffer slots ("three batched systems concurrently").
+
+UNMEASURED ON HARDWARE with more than one GPU: this container and its GPU box have one device.
+What is tested: the stages and their buffer layouts on one B200 with the ranks' exchanges emulated
+by tensor permutation (tests/test_gpu_yslab.py), and this driver with two ``gloo`` ranks on the
+CPU against a stand-in for the stages (tests/test_yslab_cpu.py).
+"""
+from __future__ import annotations
+
+from typing import List, Optional, Tuple
+
+import torch
+
+from . import binding as _b
+
+DEPTH = 3
+
+
+class CudaSlabStages:
+    """The rank-local stages through the C ABI (device buffers, CUDA streams)."""
+
+    def __init__(self, nx: int, ny_local: int, nz: int, P_local: int, batch: int, rank: int, nranks: int):
+        self.nx, self.ny, self.nz, self.P, self.rank, self.nranks = nx, ny_local, nz, P_local, rank, nranks
+        self.handle = _b.tdma_slab_create(nx, ny_local, nz, P_local, batch, rank, nranks)
+        self.nb = _b.tdma_slab_get(self.handle, _b.TDMA_SLAB_NB)
+        self.bz = _b.tdma_slab_get(self.handle, _b.TDMA_SLAB_BATCH)
+        self.device = torch.device("cuda", torch.cuda.current_device())
+
+    def batch_lines(self, n: int) -> Tuple[int, int]:
+        """(Lb, Ls) of batch n: its lines and every rank's share of them."""
+        slices = min(self.bz, self.nz - n * self.bz)
+        lb = self.nx * slices
+        return lb, lb // self.nranks
+
+    def stage_a(self, n, a, b, c, d, send, stream=None):
+        _b.tdma_slab_stage_a(self.handle, n, a, b, c, d, send, stream)
+
+    def stage_b(self, n, recv, yout, stream=None):
+        _b.tdma_slab_stage_b(self.handle, n, recv, yout, stream)
+
+    def stage_c(self, n, yrecv, x, stream=None):
+        _b.tdma_slab_stage_c(self.handle, n, yrecv, x, stream)
+
+    def close(self):
+        if self.handle:
+            _b.tdma_slab_destroy(self.handle)
+            self.handle = 0
+
+
+class YSlabSolver:
+    """Pipelined y-slab solve of one rank.  ``stages``: the rank-local stages (default: the CUDA
+    kernels through the C ABI); ``group``: a torch.distributed process group (None = default group;
+    with no initialised process group a single rank runs alone and the exchange is a local copy)."""
+
+    def __init__(self, nx: int, ny_local: int, nz: int, P_local: int = 1, batch: int = 0, group=None,
+                 stages=None):
+        import torch.distributed as dist
+        self.dist = dist if dist.is_available() and dist.is_initialized() else None
+        self.group = group
+        self.rank = self.dist.get_rank(group) if self.dist else 0
+        self.nranks = self.dist.get_world_size(group) if self.dist else 1
+        self.stages = stages if stages is not None else CudaSlabStages(nx, ny_local, nz, P_local, batch,
+                                                                       self.rank, self.nranks)
+        self.P = P_local
+        self.device = self.stages.device
+        self.cuda = self.device.type == "cuda"
+        lb, ls = self.stages.batch_lines(0)
+        mk = lambda n: [torch.empty(n, dtype=torch.float64, device=self.device) for _ in range(DEPTH)]
+        self.send, self.recv = mk(self.nranks * P_local * 6 * ls), mk(self.nranks * P_local * 6 * ls)
+        self.yout, self.yrecv = mk(self.nranks * 2 * P_local * ls), mk(self.nranks * 2 * P_local * ls)
+        self.log: List[Tuple[str, int]] = []          # (operation, batch) in enqueue order of the last solve
+        if self.cuda:
+            self.s_b, self.s_comm = torch.cuda.Stream(), torch.cuda.Stream()
+            ev = lambda: [torch.cuda.Event() for _ in range(DEPTH)]
+            self.ev_a, self.ev_x1, self.ev_b, self.ev_x2, self.ev_c = ev(), ev(), ev(), ev(), ev()
+
+    def exchange_bytes(self, n: int = 0) -> Tuple[int, int]:
+        """Bytes this rank sends in A2B and in B2C of batch n (6 values out, 2 back)."""
+        lb, ls = self.stages.batch_lines(n)
+        return 8 * self.nranks * self.P * 6 * ls, 8 * self.nranks * 2 * self.P * ls
+
+    def _all_to_all(self, out: torch.Tensor, inp: torch.Tensor):
+        if self.dist is None or self.nranks == 1:
+            out.copy_(inp)
+        else:
+            self.dist.all_to_all_single(out, inp, group=self.group)
+
+    def solve(self, a, b, c, d, x):
+        """Enqueue the whole slab solve; on CUDA the caller's current stream sees x when it returns
+        (the internal streams are joined back into it)."""
+        st, nb = self.stages, self.stages.nb
+        self.log = []
+        if self.cuda:
+            s_ac = torch.cuda.current_stream()
+            fork = torch.cuda.Event()
+            fork.record(s_ac)
+            self.s_b.wait_event(fork)
+            self.s_comm.wait_event(fork)
+        for n in range(nb + 2):
+            if n < nb:                                    # stage A(n), then A2B(n)
+                slot = n % DEPTH
+                lb, ls = st.batch_lines(n)
+                n6 = self.nranks * self.P * 6 * ls
+                if self.cuda:
+                    if n >= DEPTH:
+                        s_ac.wait_event(self.ev_x1[slot])      # send[slot] was read by A2B(n - DEPTH)
+                    st.stage_a(n, a, b, c, d, self.send[slot], s_ac)
+                    self.ev_a[slot].record(s_ac)
+                    self.s_comm.wait_event(self.ev_a[slot])
+                    if n >= DEPTH:
+                        self.s_comm.wait_event(self.ev_b[slot])  # recv[slot] was read by B(n - DEPTH)
+                    with torch.cuda.stream(self.s_comm):
+                        self._all_to_all(self.recv[slot][:n6], self.send[slot][:n6])
+                    self.ev_x1[slot].record(self.s_comm)
+                else:
+                    st.stage_a(n, a, b, c, d, self.send[slot])
+                    self._all_to_all(self.recv[slot][:n6], self.send[slot][:n6])
+                self.log += [("A", n), ("A2B", n)]
+            q = n - 1
+            if 0 <= q < nb:                               # stage B(n-1), then B2C(n-1)
+                slot = q % DEPTH
+                lb, ls = st.batch_lines(q)
+                n2 = self.nranks * 2 * self.P * ls
+                if self.cuda:
+                    self.s_b.wait_event(self.ev_x1[slot])
+                    if q >= DEPTH:
+                        self.s_b.wait_event(self.ev_x2[slot])    # yout[slot] was read by B2C(q - DEPTH)
+                    st.stage_b(q, self.recv[slot], self.yout[slot], self.s_b)
+                    self.ev_b[slot].record(self.s_b)
+                    self.s_comm.wait_event(self.ev_b[slot])
+                    if q >= DEPTH:
+                        self.s_comm.wait_event(self.ev_c[slot])  # yrecv[slot] was read by C(q - DEPTH)
+                    with torch.cuda.stream(self.s_comm):
+                        self._all_to_all(self.yrecv[slot][:n2], self.yout[slot][:n2])
+                    self.ev_x2[slot].record(self.s_comm)
+                else:
+                    st.stage_b(q, self.recv[slot], self.yout[slot])
+                    self._all_to_all(self.yrecv[slot][:n2], self.yout[slot][:n2])
+                self.log += [("B", q), ("B2C", q)]
+            q = n - 2
+            if 0 <= q < nb:                               # stage C(n-2)
+                slot = q % DEPTH
+                if self.cuda:
+                    s_ac.wait_event(self.ev_x2[slot])
+                    st.stage_c(q, self.yrecv[slot], x, s_ac)
+                    self.ev_c[slot].record(s_ac)
+                else:
+                    st.stage_c(q, self.yrecv[slot], x)
+                self.log.append(("C", q))
+        if self.cuda:
+            join_b, join_c = torch.cuda.Event(), torch.cuda.Event()
+            join_b.record(self.s_b)
+            join_c.record(self.s_comm)
+            s_ac.wait_event(join_b)
+            s_ac.wait_event(join_c)
+        return x
+
+    def close(self):
+        if hasattr(self.stages, "close"):
+            self.stages.close()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
