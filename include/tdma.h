@@ -117,7 +117,7 @@ typedef struct tdma_options {
     int shared_lines;    /* tdma_solve_shared: cells along x per tile (real: 16 or 32, complex: 8 or 16),
                             0 = auto (128-byte row segments) */
     int shared_cluster;  /* tdma_solve_shared: CTAs per cluster (1, 2, 4, 8), 0 = auto */
-    int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16), 0 = auto */
+    int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16, 32), 0 = auto */
     int shared_slots;    /* tdma_solve_shared: tiles in the shared-memory ring (2 .. 4), 0 = auto */
     int shared_ctas;     /* tdma_solve_shared: CTAs per SM: 1, or 2 (the <= 128-register build of the
                             16-row-leaf kernel, two CTAs co-resident); 0 = auto */

@@ -49,21 +49,58 @@ __device__ __forceinline__ void st_rhs(uint32_t a, const double (&v)[NC])
     else sts1(a, v[0]);
 }
 
+// A node's two boundary equations, general diagonals:
+//   first:  fa x_prev + fb x_f + fc x_l = fd        last:  la x_f + lb x_l + lc x_next = ld
+template <int NC>
+struct NodeEq { double fa, fb, fc, fd[NC], la, lb, lc, ld[NC]; };
+
+// The two unknowns a pairwise merge eliminates (last of the left node, first of the right node) in
+// terms of the merged node's first / last unknown:  x = d[j] - a[j] x_f - c[j] x_l.
+template <int NC>
+struct Elim { double a[2], c[2], d[2][NC]; };
+
+// Pairwise merge in registers (the formulas of tdma_fused_tma.cuh's header with general B): the merged
+// equations are carried un-normalised and rescaled by an exact power of two; one reciprocal (of the
+// 2 x 2 determinant), off the chain that produces the merged node.
+template <int NC>
+__device__ __forceinline__ void merge_nodes(const NodeEq<NC> &L, const NodeEq<NC> &R, NodeEq<NC> &M, Elim<NC> &E)
+{
+    const double det = fma(L.lb, R.fb, -(L.lc * R.fa));
+    const double p2 = L.lc * R.fc, p3 = R.fa * L.la;
+    M.fb = fma(det, L.fb, -(L.fc * R.fb * L.la));
+    M.lb = fma(det, R.lb, -(R.la * L.lb * R.fc));
+    const double sf = pow2_unscale(M.fb), sl = pow2_unscale(M.lb);
+    M.fa = det * L.fa * sf; M.fb *= sf; M.fc = L.fc * p2 * sf;
+    M.la = R.la * p3 * sl; M.lb *= sl; M.lc = det * R.lc * sl;
+    const double inv = rcp_nr(det);
+    E.a[0] = R.fb * L.la * inv; E.c[0] = -(p2 * inv);
+    E.a[1] = -(p3 * inv); E.c[1] = L.lb * R.fc * inv;
+#pragma unroll
+    for (int q = 0; q < NC; ++q) {
+        const double nL = fma(R.fb, L.ld[q], -(L.lc * R.fd[q])), nR = fma(L.lb, R.fd[q], -(R.fa * L.ld[q]));
+        M.fd[q] = fma(det, L.fd[q], -(L.fc * nL)) * sf;
+        M.ld[q] = fma(det, R.ld[q], -(R.la * nR)) * sl;
+        E.d[0][q] = nL * inv; E.d[1][q] = nR * inv;
+    }
+}
+
 // What a leaf keeps in registers between its sweep and its back-substitution: the matrix part of
-// the interior rows, x_r = d'_r - ia x_first - ic x_{r+1} (d'_r lives in the tile slot), and for two
-// sub-leaves the rows the in-register merge eliminated, x = md - ma x_0 - mc x_{M0-1}.
+// the interior rows of its K sub-leaves, x_r = d'_r - ia x_first - ic x_{r+1} (d'_r lives in the
+// tile slot), and the rows the in-register merges of the sub-leaves eliminated (K = 2: one merge;
+// K = 4: (0,1), (2,3), then the two pairs).
 template <int M0, int NC>
 struct ShLeafRegs {
-    static constexpr int K = M0 >= 8 ? 2 : 1;
+    static constexpr int K = M0 >= 32 ? 4 : (M0 >= 8 ? 2 : 1);
     static constexpr int H = M0 / K;
     static constexpr int HI = H - 2;
     double ia[K][HI], ic[K][HI];
-    double ma[2], mc[2], md[2][NC];
+    Elim<NC> e[K > 1 ? K - 1 : 1];
 };
 
-// Modified Thomas reduction of the leaf's K sub-leaves (same arithmetic as leaf_reduce in
-// tdma_fused_tma.cuh).  cA, cB, cC: the leaf's rows of a_y, b0_y, c_y in shared memory; s: the
-// line's shift; dbase: shared address of the leaf's first cell, rows row_bytes apart.
+// Modified Thomas reduction of the leaf's K sub-leaves, swept interleaved (K independent
+// recurrences per thread; same arithmetic as leaf_reduce in tdma_fused_tma.cuh).  cA, cB, cC: the
+// leaf's rows of a_y, b0_y, c_y in shared memory; s: the line's shift; dbase: shared address of the
+// leaf's first cell, rows row_bytes apart.
 template <int M0, int NC>
 __device__ __forceinline__ void leaf_reduce_sh(const double *__restrict__ cA, const double *__restrict__ cB,
                                                const double *__restrict__ cC, double s, uint32_t dbase,
@@ -71,7 +108,7 @@ __device__ __forceinline__ void leaf_reduce_sh(const double *__restrict__ cA, co
                                                EqN<NC> &f, EqN<NC> &l, ShLeafRegs<M0, NC> &R)
 {
     constexpr int K = ShLeafRegs<M0, NC>::K, H = ShLeafRegs<M0, NC>::H;
-    static_assert(H >= 4, "leaves of 4, 8 or 16 rows");
+    static_assert(H >= 4, "leaves of 4, 8, 16 or 32 rows");
     double fa[K], fb[K], fc[K], fd[K][NC], pa[K], pc[K], pd[K][NC];
 #pragma unroll
     for (int h = 0; h < K; ++h) {
@@ -115,39 +152,42 @@ __device__ __forceinline__ void leaf_reduce_sh(const double *__restrict__ cA, co
             pa[h] = -(ar * pa[h]) * inv;
         }
     }
+    // the sub-leaves as nodes with unit diagonals
+    NodeEq<NC> nd[K];
 #pragma unroll
     for (int h = 0; h < K; ++h) {
         const double inv = rcp_nr(fb[h]);
-        fa[h] *= inv; fc[h] *= inv;
+        nd[h].fa = fa[h] * inv; nd[h].fb = 1.0; nd[h].fc = fc[h] * inv;
+        nd[h].la = pa[h]; nd[h].lb = 1.0; nd[h].lc = pc[h];
 #pragma unroll
-        for (int q = 0; q < NC; ++q) fd[h][q] *= inv;
+        for (int q = 0; q < NC; ++q) { nd[h].fd[q] = fd[h][q] * inv; nd[h].ld[q] = pd[h][q]; }
     }
-    if (K == 1) {
-        f.a = fa[0]; f.b = 1.0; f.c = fc[0];
-        l.a = pa[0]; l.b = 1.0; l.c = pc[0];
-#pragma unroll
-        for (int q = 0; q < NC; ++q) { f.d[q] = fd[0][q]; l.d[q] = pd[0][q]; }
+    NodeEq<NC> top;
+    if constexpr (K == 1) {
+        top = nd[0];
+    } else if constexpr (K == 2) {
+        merge_nodes<NC>(nd[0], nd[K - 1], top, R.e[0]);
     } else {
-        // pairwise merge of the two sub-leaves in registers (unit diagonals), as leaf_finish
-        const double A1 = fa[0], C1 = fc[0], A2 = pa[0], C2 = pc[0];
-        const double A3 = fa[K - 1], C3 = fc[K - 1], A4 = pa[K - 1], C4 = pc[K - 1];
-        const double det = fma(-C2, A3, 1.0);
-        const double p2 = C2 * C3, p3 = A3 * A2;
-        f.b = fma(-C1, A2, det); l.b = fma(-A4, C3, det);
-        const double sf = pow2_unscale(f.b), sl = pow2_unscale(l.b);
-        f.a = det * A1 * sf; f.b *= sf; f.c = C1 * p2 * sf;
-        l.a = A4 * p3 * sl; l.b *= sl; l.c = det * C4 * sl;
-        const double inv = rcp_nr(det);
-        R.ma[0] = A2 * inv; R.mc[0] = -(p2 * inv);
-        R.ma[1] = -(p3 * inv); R.mc[1] = C3 * inv;
+        NodeEq<NC> m01, m23;
+        merge_nodes<NC>(nd[0], nd[1], m01, R.e[0]);
+        merge_nodes<NC>(nd[K - 2], nd[K - 1], m23, R.e[1]);
+        merge_nodes<NC>(m01, m23, top, R.e[K - 2]);
+    }
+    f.a = top.fa; f.b = top.fb; f.c = top.fc;
+    l.a = top.la; l.b = top.lb; l.c = top.lc;
 #pragma unroll
-        for (int q = 0; q < NC; ++q) {
-            const double D1 = fd[0][q], D2 = pd[0][q], D3 = fd[K - 1][q], D4 = pd[K - 1][q];
-            const double nL = fma(-C2, D3, D2), nR = fma(-A3, D2, D3);
-            f.d[q] = fma(det, D1, -(C1 * nL)) * sf;
-            l.d[q] = fma(det, D4, -(A4 * nR)) * sl;
-            R.md[0][q] = nL * inv; R.md[1][q] = nR * inv;
-        }
+    for (int q = 0; q < NC; ++q) { f.d[q] = top.fd[q]; l.d[q] = top.ld[q]; }
+}
+
+// the two unknowns a merge eliminated, from the merged node's first / last unknown
+template <int NC>
+__device__ __forceinline__ void elim_values(const Elim<NC> &E, const double (&xf)[NC], const double (&xl)[NC],
+                                            double (&lastL)[NC], double (&firstR)[NC])
+{
+#pragma unroll
+    for (int q = 0; q < NC; ++q) {
+        lastL[q] = fma(-E.c[0], xl[q], fma(-E.a[0], xf[q], E.d[0][q]));
+        firstR[q] = fma(-E.c[1], xl[q], fma(-E.a[1], xf[q], E.d[1][q]));
     }
 }
 
@@ -157,14 +197,15 @@ __device__ __forceinline__ void leaf_back_sh(const ShLeafRegs<M0, NC> &R, const 
                                              uint32_t dbase, uint32_t row_bytes)
 {
     constexpr int K = ShLeafRegs<M0, NC>::K, H = ShLeafRegs<M0, NC>::H;
-    double first[K][NC], xn[K][NC];
+    double first[K][NC], xn[K][NC];                            // xn[h] starts as the sub-leaf's last unknown
 #pragma unroll
-    for (int q = 0; q < NC; ++q) {
-        first[0][q] = xf[q]; xn[K - 1][q] = xl[q];
-        if (K == 2) {
-            xn[0][q] = fma(-R.mc[0], xl[q], fma(-R.ma[0], xf[q], R.md[0][q]));
-            first[K - 1][q] = fma(-R.mc[1], xl[q], fma(-R.ma[1], xf[q], R.md[1][q]));
-        }
+    for (int q = 0; q < NC; ++q) { first[0][q] = xf[q]; xn[K - 1][q] = xl[q]; }
+    if constexpr (K == 2) {
+        elim_values<NC>(R.e[0], xf, xl, xn[0], first[K - 1]);
+    } else if constexpr (K == 4) {
+        elim_values<NC>(R.e[K - 2], xf, xl, xn[1], first[K - 2]);          // last of (0,1), first of (2,3)
+        elim_values<NC>(R.e[0], xf, xn[1], xn[0], first[1]);
+        elim_values<NC>(R.e[1], first[K - 2], xl, xn[K - 2], first[K - 1]);
     }
 #pragma unroll
     for (int h = 0; h < K; ++h) {
@@ -452,7 +493,7 @@ inline size_t shared_smem_bytes(int TX, int R, int W, int CL, int NA, int NC)
 }
 
 // Leaf sizes the kernel is instantiated for.
-constexpr int kSharedLeafSizes[] = {16, 8, 4};
+constexpr int kSharedLeafSizes[] = {32, 16, 8, 4};
 
 inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int want_lines, int want_cluster,
                                   int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why)
@@ -475,10 +516,13 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
             for (int m0 : kSharedLeafSizes) {
                 if (want_leaf && m0 != want_leaf) continue;
                 if (m0 > R || R % m0 || !is_pow2(R / m0) || R / m0 > 32) continue;
+                // 32-row leaves (four sub-leaves per thread) halve the tree per cell: 1.46 -> 1.05 ms on 256 slices
+                // of cfg 3 (real).  Complex cells need the registers for the second right-hand side: on request only
+                if (m0 == 32 && want_leaf != 32 && NC != 1) continue;
                 SharedConfig c;
                 c.ncomp = NC; c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
                 c.threads = c.leaves * TX;
-                if (c.threads > 512) continue;
+                if (c.threads > 512 || (m0 == 32 && c.threads > 256)) continue;
                 c.box_rows = R;
                 while (c.box_rows > 256) c.box_rows /= 2;
                 if (R % c.box_rows) continue;
@@ -582,6 +626,7 @@ inline cudaError_t launch_shared_tx(SharedConfig &cfg, const CUtensorMap *tm, co
         return launch_shared_inst<TX, 16, kCluster, 256, NC, 2>(cfg, tm, prm, st);
     }
     switch (cfg.leaf_rows) {
+    case 32: return big ? cudaErrorInvalidValue : launch_shared_inst<TX, 32, kCluster, 256, NC>(cfg, tm, prm, st);
     case 16: return big ? launch_shared_inst<TX, 16, kCluster, 512, NC>(cfg, tm, prm, st)
                         : launch_shared_inst<TX, 16, kCluster, 256, NC>(cfg, tm, prm, st);
     case 8: return big ? launch_shared_inst<TX, 8, kCluster, 512, NC>(cfg, tm, prm, st)
