@@ -386,7 +386,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3_weak")
-    ap.add_argument("--variant", default="auto", choices=["auto", "fused", "pipelined"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "fused", "pipelined", "staged"])
     ap.add_argument("--batch", type=int, default=-1, help="z-slices per batch (-1: workload default)")
     ap.add_argument("--nstreams", type=int, default=0)
     ap.add_argument("--nz", type=int, default=0, help="restrict the slab to the first NZ slices")
@@ -442,7 +442,8 @@ def main():
     x = torch.empty_like(w.d)
     batch = spec["batch"] if args.batch < 0 else args.batch
     cells = w.cells
-    vmap = {"fused": tdma.TDMA_VARIANT_FUSED, "pipelined": tdma.TDMA_VARIANT_PIPELINED}
+    vmap = {"fused": tdma.TDMA_VARIANT_FUSED, "pipelined": tdma.TDMA_VARIANT_PIPELINED,
+            "staged": tdma.TDMA_VARIANT_STAGED}
     warmup = max(3, args.warmup)
 
     if args.sweep:
@@ -453,7 +454,7 @@ def main():
         return timeline(torch, tdma, w, x, args, batch, rank)
 
     # ---- candidate variants: the headline is the faster one; both are reported ---------------
-    names = ["fused", "pipelined"] if args.variant == "auto" else [args.variant]
+    names = ["fused", "pipelined", "staged"] if args.variant == "auto" else [args.variant]
     results = {}
     for name in names:
         opts = dict(variant=vmap[name])
@@ -543,12 +544,16 @@ def main():
                            "alg_bytes_per_launch": alg_bytes, "launch_ms": dur * 1e3, "peak_source": peak_src,
                            "whole_step_frac": ALG_BYTES_PER_CELL * cells / sec / 1e9 / peak}
     # the paper's pipeline (S6): stage times and the hidden share of stage B, whichever variant won
-    if "pipelined" in ok and not args.no_extras:
-        pplan = ok["pipelined"]["plan"]
-        psec = sec if best == "pipelined" else ok["pipelined"]["quick_s"]
+    # (PIPELINED: a', c', d' through HBM, 88 B/cell; STAGED: TMA-staged stage A / C, 72 B/cell)
+    for pname in ("pipelined", "staged"):
+        if pname not in ok or args.no_extras:
+            continue
+        pplan = ok[pname]["plan"]
+        psec = sec if best == pname else ok[pname]["quick_s"]
         rep, st = pipelined_report(torch, tdma, pplan, w, x, psec)
-        out["variants"]["pipelined"].update(rep)
-        if best == "pipelined":
+        out["variants"][pname].update(rep)
+        out["variants"][pname]["hbm_bytes_per_cell"] = 88.0 if pname == "pipelined" else 72.0
+        if best == "pipelined" and pname == "pipelined":
             bz = ok[best]["batch"]
             bcells = w.nx * w.ny * bz
             alg_bytes = (32.0 + 24.0) * bcells + 48.0 * w.P * w.nx * bz   # read a,b,c,d; write a',c',d' + reduced rows
@@ -557,6 +562,16 @@ def main():
                                "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                                "alg_bytes_per_launch": alg_bytes, "launch_ms": st["A"] * 1e3,
                                "peak_source": peak_src}
+            out["stage_ms_per_batch"] = rep["stage_ms_per_batch"]
+            out["stage_b_hidden_frac"] = rep["stage_b_hidden_frac"]
+        if best == "staged" and pname == "staged":
+            bz = ok[best]["batch"]
+            bcells = w.nx * w.ny * bz
+            alg_bytes = 40.0 * bcells                   # stage C: read a, b, c, d again, write x
+            achieved = alg_bytes / st["C"] / 1e9
+            out["roofline"] = {"bound": "hbm", "kernel": "fused_tma_kernel<kStage = 2> (stage C)", "achieved": achieved,
+                               "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                               "alg_bytes_per_launch": alg_bytes, "launch_ms": st["C"] * 1e3, "peak_source": peak_src}
             out["stage_ms_per_batch"] = rep["stage_ms_per_batch"]
             out["stage_b_hidden_frac"] = rep["stage_b_hidden_frac"]
 

@@ -65,7 +65,17 @@ typedef enum tdma_variant {
      * live in the shared memory of the cluster's CTAs (the paper's ranks), the reduced system is
      * exchanged through distributed shared memory (the paper's MPI_Alltoall) and
      * solved inside the cluster, so HBM sees a, b, c, d once and x once (40 B/cell). */
-    TDMA_VARIANT_FUSED = 2
+    TDMA_VARIANT_FUSED = 2,
+    /* The paper's three stages as separate kernels on the Alg. 2 stream pipeline, like PIPELINED,
+     * but stage A and stage C fetch their partition segments by TMA into shared memory and keep
+     * the modified coefficients a', c', d' ON CHIP (north_star): stage A writes
+     * only the partitions' boundary equations (reads 32 B/cell), stage C fetches the segment
+     * again, re-reduces it and back-substitutes with the boundary unknowns stage B computed
+     * (reads 32, writes 8 B/cell).  72 B/cell instead of PIPELINED's 88, no scratch ring.  The
+     * exchanged level of the recursion is the highest whose nodes are no longer than ny/P rows
+     * (TDMA_GET_REDUCED_PARTITIONS of them per line; D1).  y / z sweeps of plain lines,
+     * 16-byte aligned arrays, shapes the TMA kernel tiles. */
+    TDMA_VARIANT_STAGED = 3
 } tdma_variant;
 
 /* Optional tuning knobs for tdma_plan_create_ex.  Zero-initialise, set struct_size =
@@ -206,12 +216,14 @@ typedef enum tdma_query {
     /* tiling of the last tdma_solve_shared (0 before the first one) */
     TDMA_GET_SHARED_LINES = 17, TDMA_GET_SHARED_CLUSTER = 18, TDMA_GET_SHARED_LEAF_ROWS = 19,
     TDMA_GET_SHARED_THREADS = 20, TDMA_GET_SHARED_SMEM = 21, TDMA_GET_SHARED_SLOTS = 22,
-    TDMA_GET_SHARED_FILL = 23      /* z-slices its fill launch took */
+    TDMA_GET_SHARED_FILL = 23,     /* z-slices its fill launch took */
+    TDMA_GET_REDUCED_PARTITIONS = 24 /* partitions per line in the reduced buffers (P; STAGED: see there) */
 } tdma_query;
 int tdma_plan_get(const tdma_plan *plan, int what); /* < 0 on error */
 size_t tdma_plan_workspace_bytes(const tdma_plan *plan); /* device bytes the plan owns */
 
-/* Device pointer + size of a plan-owned buffer of ring slot `slot` (tests only; PIPELINED).
+/* Device pointer + size of a plan-owned buffer of ring slot `slot` (tests only; PIPELINED, and the
+ * reduced-system buffers of STAGED with P = TDMA_GET_REDUCED_PARTITIONS).
  * Reduced-system buffers are [2P][Lb] doubles, line fastest (Lb = nx * batch lines), unit
  * diagonal implicit; row 2p is partition p's first-row equation, row 2p+1 its last-row
  * equation.  Scratch buffers have the slab layout restricted to the batch. */

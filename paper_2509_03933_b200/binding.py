@@ -19,7 +19,7 @@ from . import build as _build
 # enums of include/tdma.h
 TDMA_F64 = 0
 TDMA_OK, TDMA_ERR_INVALID_ARG, TDMA_ERR_UNSUPPORTED, TDMA_ERR_ALLOC, TDMA_ERR_CUDA = 0, -1, -2, -3, -4
-TDMA_VARIANT_AUTO, TDMA_VARIANT_PIPELINED, TDMA_VARIANT_FUSED = 0, 1, 2
+TDMA_VARIANT_AUTO, TDMA_VARIANT_PIPELINED, TDMA_VARIANT_FUSED, TDMA_VARIANT_STAGED = 0, 1, 2, 3
 TDMA_AXIS_Y, TDMA_AXIS_X, TDMA_AXIS_Z = 0, 1, 2
 TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
 (TDMA_GET_NB, TDMA_GET_M, TDMA_GET_BATCH, TDMA_GET_NSTREAMS, TDMA_GET_DEPTH, TDMA_GET_VARIANT,
@@ -27,7 +27,7 @@ TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
  TDMA_GET_FUSED_LEAF_ROWS, TDMA_GET_FUSED_TOP, TDMA_GET_FUSED_THREADS, TDMA_GET_FUSED_SMEM,
  TDMA_GET_FUSED_TOP_ROWS, TDMA_GET_FUSED_IMPL, TDMA_GET_FUSED_FILL, TDMA_GET_SHARED_LINES,
  TDMA_GET_SHARED_CLUSTER, TDMA_GET_SHARED_LEAF_ROWS, TDMA_GET_SHARED_THREADS, TDMA_GET_SHARED_SMEM,
- TDMA_GET_SHARED_SLOTS, TDMA_GET_SHARED_FILL) = range(24)
+ TDMA_GET_SHARED_SLOTS, TDMA_GET_SHARED_FILL, TDMA_GET_REDUCED_PARTITIONS) = range(25)
 (TDMA_BUF_RA, TDMA_BUF_RC, TDMA_BUF_RD, TDMA_BUF_Y, TDMA_BUF_SA, TDMA_BUF_SC, TDMA_BUF_SD) = range(7)
 
 EXPORTED_SYMBOLS = (

@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libtdma.so")
 # translation unit -> the headers it includes (a unit is recompiled when any of them is newer)
 _TDMA_H = os.path.join("..", "..", "include", "tdma.h")
 UNITS = {
-    "tdma_plan.cu": ["tdma_stage_kernels.cuh", "tdma_fused.cuh", "tdma_fused_tma.cuh", "tdma_shared.h", _TDMA_H],
+    "tdma_plan.cu": ["tdma_stage_kernels.cuh", "tdma_fused.cuh", "tdma_fused_tma.cuh", "tdma_shared.h", "tdma_staged.h", _TDMA_H],
+    "tdma_staged.cu": ["tdma_fused_tma.cuh", "tdma_staged.h"],
     "tdma_shared.cu": ["tdma_shared_tma.cuh", "tdma_fused_tma.cuh", "tdma_shared.h"],
     "tdma_probe.cu": [_TDMA_H],
     "tdma_slab.cu": ["tdma_stage_kernels.cuh", _TDMA_H],

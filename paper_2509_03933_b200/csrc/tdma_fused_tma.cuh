@@ -79,6 +79,13 @@ struct TmaFusedParams {
     int CL, R, W, NS;
     int xtiles, ntiles;
     int box_rows, nbox;
+    // STAGED variant (kStage 1 / 2, tdma_staged.cu): reduced system of the batch in HBM, [2 Pe][Lb]
+    // doubles, line fastest, unit diagonal; lp = tree levels run inside the CTA (the nodes of that
+    // level are the partitions whose boundary equations are exchanged), lp_shift = log2(leaves per node)
+    double *red_a = nullptr, *red_c = nullptr, *red_d = nullptr;
+    const double *red_y = nullptr;
+    long long Lb = 0;
+    int lp = 0, lp_shift = 0;
 };
 
 // Dynamic shared memory of one CTA: NA ring slots of one raw array [R][TX] each, the x staging
@@ -786,13 +793,23 @@ __device__ __forceinline__ void named_sync(int id, int nthreads)
 // the last warp hands it to the TMA engine (one tensor store per box) after the NEXT tile's
 // sweep -- an SM retires plain global stores at about a sector per cycle, which would block the
 // load/store unit the sweep reads the raw tile with for > 1000 cycles per tile.
-template <int TX, int M0, bool kCluster, int MAXT, bool kX>
+// kStage (STAGED variant: the paper's three stages as separate kernels with the
+// partition segments staged on chip, nothing spilled):
+//   0  the fused solve described above;
+//   1  stage A: sweep + tree up to the partition level, the partitions' boundary equations
+//      (unit diagonal) go to the reduced buffers in HBM; no back-substitution, x untouched;
+//   2  stage C: the tile is fetched and reduced AGAIN (a', c', d' never leave the chip), the
+//      partitions' boundary unknowns come from the reduced solution Y, then walk-down and leaf
+//      back-substitution as in the fused solve.
+//   kStage != 0: CTAs are independent (no cluster, no DSMEM): CL consecutive CTAs share a line tile.
+template <int TX, int M0, bool kCluster, int MAXT, bool kX, int kStage = 0>
 __global__ void __launch_bounds__(MAXT, 1)
 fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant__ CUtensorMap tm_b,
                  const __grid_constant__ CUtensorMap tm_c, const __grid_constant__ CUtensorMap tm_d,
                  const __grid_constant__ CUtensorMap tm_x, const TmaFusedParams prm)
 {
     static_assert(!kX || M0 == 16, "x sweeps use 16-row (128-byte) leaves");
+    static_assert(kStage == 0 || (!kCluster && !kX), "staged kernels: independent CTAs, y / z sweeps");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     const int R = prm.R, CL = prm.CL, W = prm.W, NA = prm.NS;
     const int arr = R * TX;
@@ -818,6 +835,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     const unsigned tmask = __ballot_sync(0xffffffffu, tree);
     unsigned crank = 0;
     if (kCluster) crank = cg::this_cluster().block_rank();
+    if (kStage != 0) crank = blockIdx.x % CL;
     const int g = blockIdx.x / CL, NC = gridDim.x / CL;        // cluster index / number of clusters
     const int y0 = (int)crank * R;
 
@@ -925,6 +943,19 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         if (sn >= NA) { sn -= NA; pn ^= 1; }
         const double *__restrict__ sB = raw + (size_t)sl[0] * arr, *__restrict__ sA = raw + (size_t)sl[1] * arr;
         const double *__restrict__ sC = raw + (size_t)sl[2] * arr, *__restrict__ sD = raw + (size_t)sl[3] * arr;
+        // staged kernels: where this thread's partition sits in the reduced buffers; stage C fetches its
+        // two boundary unknowns now, a whole sweep ahead of their use
+        long long red_l = -1;
+        double y_first = 0.0, y_last = 0.0;
+        if (kStage != 0) {
+            const int xt_ = tile % prm.xtiles, k_ = tile / prm.xtiles;
+            if (xt_ * TX + lx < prm.nx) red_l = (long long)k_ * prm.nx + xt_ * TX + lx;
+            if (kStage == 2 && act && red_l >= 0) {
+                const long long pg = (long long)crank * (W >> prm.lp_shift) + (leaf >> prm.lp_shift);
+                y_first = __ldcg(prm.red_y + 2 * pg * prm.Lb + red_l);
+                y_last = __ldcg(prm.red_y + (2 * pg + 1) * prm.Lb + red_l);
+            }
+        }
 #pragma unroll
         for (int j = 0; j < 4; ++j) ptx::mbar_wait(&bar[sl[j]], (unsigned)ph[j]);
 
@@ -946,7 +977,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         __syncthreads();                // raw slots consumed, leaf equations visible
         if (issue_lane >= 0) {
             for (int j = 0; j < 4; ++j) issue_array(n0 + NA + j);     // refill the four slots
-            if (it > 0) store_x(tile - NC);                            // x of the previous tile
+            if (kStage != 1 && it > 0) store_x(tile - NC);             // x of the previous tile
         }
         if (kCluster && it == 0) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 
@@ -954,10 +985,11 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         // The warp that issues the copies (the last one) takes no part in the tree, so the
         // 150-200 cycles per copy stay off the serial chain; everybody meets again before the
         // back-substitution.
-        if (helper) {
+        const int nlr = kStage != 0 ? prm.lp : nl;              // levels run inside the CTA
+        if (helper && kStage != 1) {                            // stage A never walks down: no interior forms
             const int h = leaf - help0;
             int cum = 0;                                        // interior-row jobs of the levels below
-            for (int l = 0; l < nl; ++l) {
+            for (int l = 0; l < nlr; ++l) {
                 const int k = level_k(l), S = level_S(l), groups = level_groups(l);
                 int gq = (h - cum) % nhelp;
                 if (gq < 0) gq += nhelp;
@@ -978,15 +1010,15 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             }
         }
         if (crit) {
-            for (int l = 0; l < nl; ++l) {
+            for (int l = 0; l < nlr; ++l) {
                 const int k = level_k(l), S = level_S(l), groups = level_groups(l);
                 for (int q = leaf; q < 2 * groups; q += mrows) {  // q < groups: forward, else backward sweep
                     if (q < groups) { if (k == 4) kmerge_fwd<TX, 4>(nb, lx, q, S, 4); else kmerge_fwd<TX, 2>(nb, lx, q, S, 2); }
                     else { if (k == 4) kmerge_bwd<TX, 4>(nb, lx, q - groups, S, 4); else kmerge_bwd<TX, 2>(nb, lx, q - groups, S, 2); }
                 }
-                if (helper_mode) named_arrive(2 + l, tree_threads);
+                if (helper_mode && kStage != 1) named_arrive(2 + l, tree_threads);
                 tree_sync(crit_threads, tmask);
-                if (!helper_mode) {                             // nobody reads the interior rows any more
+                if (!helper_mode && kStage != 1) {              // nobody reads the interior rows any more
                     for (int q = mrows - 1 - leaf; q < groups; q += mrows) {    // last rows first: row 0 goes on
                         if (k == 4) kmerge_tails<TX, 4>(nb, lx, q, S, 4); else kmerge_tails<TX, 2>(nb, lx, q, S, 2);
                     }
@@ -995,7 +1027,9 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
 
             // ---------------- cluster level ----------------
             // the CTA's node: first equation in node row 0, last equation in node row 2W-1
-            if (!kCluster) {
+            if (kStage != 0) {
+                // staged kernels: the exchange and the reduced solve are stage B's, through HBM
+            } else if (!kCluster) {
                 if (leaf == 0) solve_root<TX>(nb, lx, 2 * W - 1, prm.periodic != 0);
             } else {
                 // A2B as an all-gather (the paper's MPI_Alltoall, with every rank
@@ -1038,6 +1072,23 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         // the TMA engine must have read the previous tile's x out of the staging tile
         if (issue_lane >= 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
         __syncthreads();
+        if (kStage == 1) {
+            // stage A's output: the two boundary equations of every partition (node of level lp),
+            // normalised to unit diagonal, as rows 2 pg, 2 pg + 1 of the reduced system (the paper's
+            // A2B gather, fused into the epilogue)
+            const int Wp = W >> prm.lp_shift, S = 2 << prm.lp_shift;
+            if (t < Wp * TX && red_l >= 0) {
+                const long long pg = (long long)crank * Wp + leaf;      // leaf = t / TX: the node index here
+                const uint32_t oF = nb_ab<TX>(nb, leaf * S, lx), oL = nb_ab<TX>(nb, leaf * S + S - 1, lx);
+                const double2 abf = lds2(oF), cdf = lds2(oF + nb.plane), abl = lds2(oL), cdl = lds2(oL + nb.plane);
+                const double invf = 1.0 / abf.y, invl = 1.0 / abl.y;
+                const long long q0 = 2 * pg * prm.Lb + red_l, q1 = q0 + prm.Lb;
+                __stcg(prm.red_a + q0, abf.x * invf); __stcg(prm.red_c + q0, cdf.x * invf); __stcg(prm.red_d + q0, cdf.y * invf);
+                __stcg(prm.red_a + q1, abl.x * invl); __stcg(prm.red_c + q1, cdl.x * invl); __stcg(prm.red_d + q1, cdl.y * invl);
+            }
+            __syncthreads();            // the node rows are read before the next sweep rewrites them
+            continue;
+        }
 
         // ---------------- leaves: back-substitution from registers into the staging tile --------
         if (act) {
@@ -1045,14 +1096,16 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             // to its own leaf (x_first / x_last of a child from those of its parent and the
             // interior-row form kmerge_tails left), no barrier, nothing written
             double xf, xl;                                      // cluster: stage B left them in the inbox
-            if (kCluster) {
+            if (kStage == 2) {
+                xf = y_first; xl = y_last;                      // of this leaf's partition, from stage B's Y
+            } else if (kCluster) {
                 xf = lds1(nb_ab<TX>(tb, 2 * (int)crank, lx) + tb.plane + 8);
                 xl = lds1(nb_ab<TX>(tb, 2 * (int)crank + 1, lx) + tb.plane + 8);
             } else {
                 xf = lds1(nb_ab<TX>(nb, 0, lx) + nb.plane + 8);
                 xl = lds1(nb_ab<TX>(nb, 2 * W - 1, lx) + nb.plane + 8);
             }
-            for (int l = nl - 1; l >= 0; --l) {
+            for (int l = nlr - 1; l >= 0; --l) {
                 const int k = level_k(l), S = level_S(l);
                 const int node = leaf >> ((ccode >> (5 * l)) & 31u);        // my ancestor among this level's children
                 const int gq = node >> ((kcode >> (2 * l)) & 3u), j = node & (k - 1);
@@ -1068,7 +1121,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         }
     }
     // x of the last tile; the staging tile must outlive the store
-    if (it > 0) {
+    if (kStage != 1 && it > 0) {
         __syncthreads();
         if (issue_lane >= 0) {
             store_x(g + (it - 1) * NC);
@@ -1229,11 +1282,11 @@ inline bool make_xsweep_tensor_map(CUtensorMap *tm, const void *base, int nrows,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int TX, int M0, bool kCluster, int MAXT, bool kX = false>
+template <int TX, int M0, bool kCluster, int MAXT, bool kX = false, int kStage = 0>
 inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                    cudaStream_t st)
 {
-    auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, kX>;
+    auto kern = fused_tma_kernel<TX, M0, kCluster, MAXT, kX, kStage>;
     const size_t smem_bytes = cfg.smem;
     cudaLaunchConfig_t lc = {};
     lc.blockDim = dim3((cfg.threads + 31) & ~31);
@@ -1262,6 +1315,7 @@ inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, c
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, (int)lc.blockDim.x, smem_bytes);
             if (e != cudaSuccess) return e;
             n *= sms;
+            if (kStage != 0) n /= cfg.cluster;          // groups of `cluster` independent CTAs per line tile
         }
         if (n < 1) return cudaErrorLaunchOutOfResources;
         cfg.max_clusters = n;
@@ -1272,6 +1326,9 @@ inline cudaError_t launch_tma_inst(TmaFusedConfig &cfg, const CUtensorMap *tm, c
     return cudaLaunchKernelEx(&lc, kern, tm[0], tm[1], tm[2], tm[3], tm[4], prm);
 }
 
+// The dispatch over every instantiation of the fused solve: only the plan's translation unit wants
+// them compiled (the other units instantiate their own kernels from the template above).
+#ifdef TDMA_FUSED_TMA_DISPATCH
 template <int TX, int M0, bool kCluster>
 inline cudaError_t launch_tma_m0(TmaFusedConfig &cfg, const CUtensorMap *tm, const TmaFusedParams &prm,
                                  cudaStream_t st)
@@ -1329,5 +1386,7 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
     default: return cudaErrorInvalidValue;
     }
 }
+
+#endif  // TDMA_FUSED_TMA_DISPATCH
 
 }  // namespace tdma

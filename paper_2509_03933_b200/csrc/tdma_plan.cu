@@ -14,8 +14,10 @@
 
 #include "tdma_stage_kernels.cuh"
 #include "tdma_fused.cuh"
+#define TDMA_FUSED_TMA_DISPATCH
 #include "tdma_fused_tma.cuh"
 #include "tdma_shared.h"
+#include "tdma_staged.h"
 
 #define TDMA_VERSION_NUM 10200
 
@@ -91,6 +93,9 @@ struct tdma_plan {
     bool have_fill = false;
     int fill_opt = 0, fill_last = 0, sm_count = 0;
     size_t sm_smem = 0;
+    // STAGED: stage A / C as TMA-staged kernels, reduced system of Pred partitions in HBM
+    tdma::StagedConfig staged;
+    int Pred = 0;       // partitions in the reduced buffers (P; STAGED: staged.Pe)
     // shared-coefficient mode (tdma_solve_shared), configured at the first call per ncomp
     tdma::SharedConfig sh[2], sh_fill[2];
     int sh_state[2] = {0, 0};     // 0 = not configured, 1 = ready, -1 = does not tile
@@ -114,7 +119,7 @@ double *slot_scratch(const tdma_plan *pl, int slot, int which)
 }
 double *slot_red(const tdma_plan *pl, int slot, int which)
 {
-    const size_t per = (size_t)2 * pl->P * pl->Lb_max;
+    const size_t per = (size_t)2 * pl->Pred * pl->Lb_max;
     return pl->red + ((size_t)slot * 5 + which) * per;
 }
 
@@ -139,9 +144,22 @@ tdma::StageParams batch_params(const tdma_plan *pl, const SlabPtrs &ptr, int nz_
     return prm;
 }
 
-int launch_stage(const tdma_plan *pl, int stage, const tdma::StageParams &prm, cudaStream_t st)
+int launch_stage(tdma_plan *pl, int stage, const tdma::StageParams &prm_in, cudaStream_t st)
 {
+    tdma::StageParams prm = prm_in;
     const unsigned Lb = (unsigned)prm.Lb;
+    if (pl->variant == TDMA_VARIANT_STAGED) {
+        if (stage == TDMA_STAGE_A || stage == TDMA_STAGE_C) {
+            const int nzs = (int)(prm.Lb / pl->nx);
+            cudaError_t e = tdma::launch_staged(pl->staged, stage == TDMA_STAGE_A ? 1 : 2, prm.a, prm.b, prm.c, prm.d, prm.x,
+                                                prm.ra, prm.rc, prm.rd, prm.y, pl->nx, pl->ny, nzs, pl->rs, pl->os,
+                                                pl->axis == TDMA_AXIS_Z, st);
+            if (e != cudaSuccess) return set_err(TDMA_ERR_CUDA, "staged launch failed: %s", cudaGetErrorString(e));
+            return TDMA_OK;
+        }
+        if (stage == TDMA_STAGE_GATHER) return set_err(TDMA_ERR_INVALID_ARG, "STAGED plans have no separate gather stage");
+        prm.P = pl->Pred;               // stage B: 2 Pred rows
+    }
     switch (stage) {
     case TDMA_STAGE_A: {
         dim3 grid((Lb + 127) / 128, pl->P);
@@ -386,6 +404,7 @@ void free_plan(tdma_plan *pl)
     for (auto &g : pl->graphs) cudaGraphExecDestroy(g.exec);
     for (auto ev : pl->tl_ev) cudaEventDestroy(ev);
     cudaFree(pl->scratch); cudaFree(pl->red); cudaFree(pl->send);
+    if (pl->staged.impl) tdma::free_staged(&pl->staged);
     for (int s = 0; s < 2; ++s)
         for (int i = 0; i < 5; ++i) cudaFree(pl->stage_dev[s][i]);
     auto ds = [](cudaStream_t s) { if (s) cudaStreamDestroy(s); };
@@ -428,13 +447,16 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
             pl->bz = pl->nz; pl->nb = 1; pl->Lb_max = (size_t)pl->nx * pl->bz;
         }
     }
-    if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED)
+    if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED && variant != TDMA_VARIANT_STAGED)
         return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
+    if (variant == TDMA_VARIANT_STAGED && (pl->axis == TDMA_AXIS_X || pl->periodic || pl->ny < 2))
+        return set_err(TDMA_ERR_UNSUPPORTED, "the STAGED variant does y / z sweeps of plain lines with >= 2 rows");
     if (pl->axis == TDMA_AXIS_X && variant != TDMA_VARIANT_FUSED)
         return set_err(TDMA_ERR_UNSUPPORTED, "x sweeps need the FUSED variant (TMA kernel)");
     if (pl->periodic && (variant != TDMA_VARIANT_FUSED || pl->ny < 2))
         return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need the FUSED variant (TMA kernel) and >= 2 rows");
     pl->variant = variant;
+    pl->Pred = pl->P;
     pl->use_graph = (opt && opt->use_graph < 0) ? 0 : 1;
     pl->timeline = (opt && opt->timeline > 0) ? 1 : 0;
     if (pl->timeline) pl->use_graph = 0;
@@ -456,6 +478,19 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
     for (int i = 0; i < pl->nlanes; ++i) CUDA_TRY(mk(&pl->evLaneJoin[i]));
     for (int i = 0; i < pl->depth; ++i) { CUDA_TRY(mk(&pl->evA[i])); CUDA_TRY(mk(&pl->evB[i])); CUDA_TRY(mk(&pl->evC[i])); }
 
+    if (variant == TDMA_VARIANT_STAGED) {
+        const char *why = nullptr;
+        if (!tdma::configure_staged(&pl->staged, pl->nx, pl->ny, pl->P, pl->axis == TDMA_AXIS_Z, prop, &why))
+            return set_err(TDMA_ERR_UNSUPPORTED, "STAGED variant unavailable: %s", why ? why : "?");
+        pl->Pred = pl->staged.Pe;
+        if (opt && opt->separate_gather > 0) return set_err(TDMA_ERR_UNSUPPORTED, "STAGED plans fuse the gather into stage A");
+        const size_t rbytes = (size_t)pl->depth * 5 * 2 * pl->Pred * pl->Lb_max * sizeof(double);
+        if (cudaMalloc(&pl->red, rbytes) != cudaSuccess) {
+            cudaGetLastError();
+            return set_err(TDMA_ERR_ALLOC, "cannot allocate %zu bytes of reduced-system ring", rbytes);
+        }
+        pl->workspace = rbytes;
+    }
     if (variant == TDMA_VARIANT_PIPELINED && pl->ny > 1) {
         const size_t sbytes = (size_t)pl->depth * 3 * pl->bz * pl->slice * sizeof(double);
         const size_t rbytes = (size_t)pl->depth * 5 * 2 * pl->P * pl->Lb_max * sizeof(double);
@@ -593,8 +628,8 @@ int tdma_stage(tdma_plan *plan, int stage, int batch_index, const void *a, const
 {
     int rc = check_ptrs(plan, a, b, c, d, x);
     if (rc != TDMA_OK) return rc;
-    if (plan->variant != TDMA_VARIANT_PIPELINED || plan->ny == 1)
-        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_stage needs a PIPELINED plan with ny > 1");
+    if ((plan->variant != TDMA_VARIANT_PIPELINED && plan->variant != TDMA_VARIANT_STAGED) || plan->ny == 1)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_stage needs a PIPELINED or STAGED plan with ny > 1");
     if (batch_index < 0 || batch_index >= plan->nb)
         return set_err(TDMA_ERR_INVALID_ARG, "batch_index %d outside [0, %d)", batch_index, plan->nb);
     if (stage == TDMA_STAGE_GATHER && !plan->separate_gather)
@@ -704,7 +739,7 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
         // those of tdma_solve; FUSED: `batch` only chunks launches, so the target alone decides.
         const size_t target = (size_t)1 << 24;
         long long hz = pl->host_chunk > 0 ? pl->host_chunk : (long long)std::max<size_t>(1, target / pl->slice);
-        if (pl->variant == TDMA_VARIANT_PIPELINED) hz = std::max<long long>(pl->bz, hz / pl->bz * pl->bz);
+        if (pl->variant != TDMA_VARIANT_FUSED) hz = std::max<long long>(pl->bz, hz / pl->bz * pl->bz);
         pl->hz = (int)std::min<long long>(hz, pl->nz);
         const size_t bytes = (size_t)pl->hz * pl->slice * sizeof(double);
         for (int s = 0; s < 2; ++s)
@@ -887,6 +922,7 @@ int tdma_plan_get(const tdma_plan *plan, int what)
     case TDMA_GET_SHARED_THREADS: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].threads;
     case TDMA_GET_SHARED_SMEM: return plan->sh_last < 0 ? 0 : (int)plan->sh[plan->sh_last].smem;
     case TDMA_GET_SHARED_SLOTS: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].slots;
+    case TDMA_GET_REDUCED_PARTITIONS: return plan->Pred;
     case TDMA_GET_SHARED_FILL: return plan->sh_last < 0 ? 0 : plan->sh_fill_last;
     default: return set_err(TDMA_ERR_INVALID_ARG, "unknown query %d", what);
     }
@@ -897,17 +933,17 @@ size_t tdma_plan_workspace_bytes(const tdma_plan *plan) { return plan ? plan->wo
 int tdma_plan_buffer(const tdma_plan *plan, int which, int slot, void **device_ptr, size_t *bytes)
 {
     if (!plan || !device_ptr || !bytes) return set_err(TDMA_ERR_INVALID_ARG, "NULL argument");
-    if (plan->variant != TDMA_VARIANT_PIPELINED || !plan->scratch)
-        return set_err(TDMA_ERR_UNSUPPORTED, "plan has no stage buffers");
+    if (!plan->red || (which >= TDMA_BUF_SA && !plan->scratch))
+        return set_err(TDMA_ERR_UNSUPPORTED, "plan has no such stage buffer");
     if (slot < 0 || slot >= plan->depth) return set_err(TDMA_ERR_INVALID_ARG, "slot %d outside [0, %d)", slot, plan->depth);
     switch (which) {
     case TDMA_BUF_RA: case TDMA_BUF_RC: case TDMA_BUF_RD:
         *device_ptr = slot_red(plan, slot, which - TDMA_BUF_RA);
-        *bytes = (size_t)2 * plan->P * plan->Lb_max * sizeof(double);
+        *bytes = (size_t)2 * plan->Pred * plan->Lb_max * sizeof(double);
         return TDMA_OK;
     case TDMA_BUF_Y:
         *device_ptr = slot_red(plan, slot, 4);
-        *bytes = (size_t)2 * plan->P * plan->Lb_max * sizeof(double);
+        *bytes = (size_t)2 * plan->Pred * plan->Lb_max * sizeof(double);
         return TDMA_OK;
     case TDMA_BUF_SA: case TDMA_BUF_SC: case TDMA_BUF_SD:
         *device_ptr = slot_scratch(plan, slot, which - TDMA_BUF_SA);

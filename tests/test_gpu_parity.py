@@ -23,12 +23,14 @@ pytestmark = pytest.mark.gpu
 
 TOL_E = 1e-11
 TOL_RES = 1e-12
-# the three code paths behind tdma_solve: stage kernels + stream pipeline, the register-staged
-# fused kernel, and FUSED with fused_impl = auto (the TMA kernel wherever it is eligible)
+# the code paths behind tdma_solve: stage kernels + stream pipeline, the register-staged fused
+# kernel, FUSED with fused_impl = auto (the TMA kernel wherever it is eligible), and the stage
+# pipeline with TMA-staged stage A / C kernels (STAGED)
 VARIANT_OPTS = [dict(variant=tdma.TDMA_VARIANT_PIPELINED),
                 dict(variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1),
-                dict(variant=tdma.TDMA_VARIANT_FUSED)]
-VARIANTS = [pytest.param(o, id=i) for o, i in zip(VARIANT_OPTS, ("pipelined", "fused_reg", "fused_tma"))]
+                dict(variant=tdma.TDMA_VARIANT_FUSED),
+                dict(variant=tdma.TDMA_VARIANT_STAGED)]
+VARIANTS = [pytest.param(o, id=i) for o, i in zip(VARIANT_OPTS, ("pipelined", "fused_reg", "fused_tma", "staged"))]
 TMA = dict(variant=tdma.TDMA_VARIANT_FUSED, fused_impl=2)
 
 
@@ -287,6 +289,8 @@ def test_shapes(variant, shape, P, batch):
     except tdma.TdmaError as exc:
         if variant["variant"] == tdma.TDMA_VARIANT_FUSED and "fused variant unavailable" in str(exc):
             pytest.skip(str(exc))
+        if variant["variant"] == tdma.TDMA_VARIANT_STAGED and "STAGED variant unavailable" in str(exc):
+            pytest.skip(str(exc))       # shapes the TMA kernel cannot tile (30 rows: no power-of-two tree)
         raise
     check_against_oracle(a, b, c, d, x, True)
 
@@ -525,6 +529,58 @@ def test_stage_level_reduced_system_and_forward_rows():
             j = p * m + r
             lhs = SA[:, j, :] * x0 + ref[:, j, :] + SC[:, j, :] * ref[:, j + 1, :]
             assert np.max(np.abs(lhs - SD[:, j, :])) <= 1e-14
+
+
+@pytest.mark.parametrize("P,want_pe", [(4, 4), (16, 16), (32, 16)])
+def test_staged_stage_level_reduced_system(P, want_pe):
+    """STAGED (TMA-staged stage A / C, nothing spilled): the reduced rows stage A leaves in HBM hold
+    for the oracle solution, stage B's Y equals the oracle at the ends of the exchanged nodes, and
+    the stage-isolated calls reproduce the whole solve bit for bit.  256 rows: 16 leaves of 16
+    rows; P = 4 exchanges the nodes of one 4-ary level (64 rows = the paper's partition), P = 16 the
+    leaves, P = 32 (8-row partitions, shorter than a leaf) the leaves as well (D1)."""
+    nx, ny, nz = 96, 256, 5
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 61, dev())
+    an, bn, cn, dn = to_np(a, b, c, d)
+    ref = oracle.solve_y(an, bn, cn, dn)
+    x = torch.full_like(d, float("nan"))
+    with tdma.Plan(nx, ny, nz, P, 0, variant=tdma.TDMA_VARIANT_STAGED) as plan:
+        pe = plan.get(tdma.TDMA_GET_REDUCED_PARTITIONS)
+        assert pe == want_pe
+        for st in (tdma.TDMA_STAGE_A, tdma.TDMA_STAGE_B, tdma.TDMA_STAGE_C):
+            plan.stage(st, 0, a, b, c, d, x)
+        torch.cuda.synchronize()
+        Lb, m = nx * nz, ny // pe
+        bufs = {}
+        for name, which in (("RA", tdma.TDMA_BUF_RA), ("RC", tdma.TDMA_BUF_RC), ("RD", tdma.TDMA_BUF_RD), ("Y", tdma.TDMA_BUF_Y)):
+            ptr, nbytes = plan.buffer(which, 0)
+            bufs[name] = _view(ptr, nbytes, (2 * pe, Lb)).clone().cpu().numpy()
+        with pytest.raises(tdma.TdmaError):
+            plan.buffer(tdma.TDMA_BUF_SA, 0)                       # there is no scratch ring
+        assert plan.workspace_bytes == 3 * 5 * 2 * pe * Lb * 8     # reduced buffers only
+        x_full = torch.empty_like(d)
+        plan.solve(a, b, c, d, x_full)
+        torch.cuda.synchronize()
+    assert torch.equal(x, x_full)
+    check_against_oracle(a, b, c, d, x, True)
+    RA, RC, RD, Y = bufs["RA"], bufs["RC"], bufs["RD"], bufs["Y"]
+    assert (RA[0] == 0).all() and (RC[2 * pe - 1] == 0).all()
+    ref_lines = ref.transpose(1, 0, 2).reshape(ny, Lb)
+    for p in range(pe):
+        xf, xl = ref_lines[p * m], ref_lines[p * m + m - 1]
+        assert np.max(np.abs(Y[2 * p] - xf)) <= 1e-13 and np.max(np.abs(Y[2 * p + 1] - xl)) <= 1e-13
+        xprev = ref_lines[p * m - 1] if p > 0 else 0 * xf
+        xnext = ref_lines[p * m + m] if p < pe - 1 else 0 * xf
+        assert np.max(np.abs(RA[2 * p] * xprev + xf + RC[2 * p] * xl - RD[2 * p])) <= 1e-13
+        assert np.max(np.abs(RA[2 * p + 1] * xf + xl + RC[2 * p + 1] * xnext - RD[2 * p + 1])) <= 1e-13
+
+
+def test_staged_schedule_invariance():
+    """STAGED: x does not depend on batching, stream count or graph capture (G13)."""
+    w = tdma_inputs.make_workload("cfg1_tiny", device=dev())
+    base = gpu_solve(w.a, w.b, w.c, w.d, w.P, 0, variant=tdma.TDMA_VARIANT_STAGED)
+    for batch, opts in [(1, {}), (7, dict(nstreams=3)), (16, dict(nstreams=1)), (24, dict(use_graph=-1)), (5, dict(nstreams=4))]:
+        x = gpu_solve(w.a, w.b, w.c, w.d, w.P, batch, variant=tdma.TDMA_VARIANT_STAGED, **opts)
+        assert torch.equal(x, base), (batch, opts)
 
 
 # ---------------------------------------------------------------------------------------------
