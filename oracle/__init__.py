@@ -9,6 +9,8 @@ Plain CPU definition of the batched y-direction tridiagonal solve, used by ``tes
   * ``residual_y`` / ``apply_y``                   -- long-double residual and d = A x.
   * ``solve_y_shared``                             -- SURVEY 8(f) f3: 1-D coefficients shared by all
     lines, diagonal shifted per line, real or complex right-hand sides.
+  * ``reduced_rows_y`` / ``solve_y_pdd``           -- SURVEY 8(f) f4: the 2P-row reduced system by its
+    definition (Schur complement), and the PDD approximation (Sun 1995) step by step.
   * ``thomas_line``                                -- the same recurrence as a pure-Python loop
     for one small line (brute-force cross-checks).
 
@@ -219,4 +221,96 @@ def solve_y_shared(a_y, b0_y, c_y, sx, sz, d, pin00: bool = False, precision: st
                                        {"f64": 0, "ld": 1}[precision])
     if rc != 0:
         raise RuntimeError("oracle_solve_y_shared failed (%d)" % rc)
+    return x
+
+
+# ---------------------------------------------------------------------------------------------
+# SURVEY 8(f) f4, PDD variant ("Parallel Diagonally Dominant (PDD) method [37] ...
+# designed for diagonally dominant TDM systems"; SURVEY: "PDD = drop the reduced solve's far
+# coupling when spikes decay")
+# ---------------------------------------------------------------------------------------------
+def reduced_rows_y(a, b, c, d, P: int, precision: str = "f64"):
+    """The 2P-row reduced system of the P-partition split, BY DEFINITION (Schur complement of the
+    interior rows of every partition), unit diagonal:
+        row 2p  :  fa x_last(p-1) + x_first(p) + fc x_last(p)  = fd
+        row 2p+1:  pa x_first(p) + x_last(p)  + pc x_first(p+1) = pd
+    Returned as arrays of shape (P, nz, nx): fa, fc, fd, pa, pc, pd.  The interior solves are plain
+    Thomas solves (solve_y) of rows 1 .. m-2 of a partition with three right-hand sides."""
+    a, b, c, d = map(_as3, (a, b, c, d))
+    nz, ny, nx = a.shape
+    if ny % P or ny // P < 2:
+        raise ValueError("ny must split into P partitions of >= 2 rows")
+    m = ny // P
+    out = [np.zeros((P, nz, nx)) for _ in range(6)]
+    for p in range(P):
+        r0 = p * m
+        A, B, C, D = [np.array(t[:, r0:r0 + m, :], dtype=np.float64) for t in (a, b, c, d)]
+        if p == 0:
+            A[:, 0, :] = 0.0
+        if p == P - 1:
+            C[:, m - 1, :] = 0.0
+        if m == 2:
+            g0 = gl = u0 = ul = v0 = vl = None
+            out[0][p], out[1][p], out[2][p] = A[:, 0] / B[:, 0], C[:, 0] / B[:, 0], D[:, 0] / B[:, 0]
+            out[3][p], out[4][p], out[5][p] = A[:, 1] / B[:, 1], C[:, 1] / B[:, 1], D[:, 1] / B[:, 1]
+            continue
+        ai, bi, ci = [np.ascontiguousarray(t[:, 1:m - 1, :]) for t in (A, B, C)]
+        ef, el = np.zeros_like(bi), np.zeros_like(bi)
+        ef[:, 0, :] = A[:, 1, :]                  # a_1 x_0 moved to the right-hand side
+        el[:, -1, :] = C[:, m - 2, :]             # c_{m-2} x_{m-1}
+        g = solve_y(ai, bi, ci, np.ascontiguousarray(D[:, 1:m - 1, :]), precision)
+        u = solve_y(ai, bi, ci, ef, precision)
+        v = solve_y(ai, bi, ci, el, precision)    # x_int = g - u x_0 - v x_{m-1}
+        diag = B[:, 0] - C[:, 0] * u[:, 0]
+        out[0][p], out[1][p], out[2][p] = A[:, 0] / diag, -C[:, 0] * v[:, 0] / diag, (D[:, 0] - C[:, 0] * g[:, 0]) / diag
+        diag = B[:, m - 1] - A[:, m - 1] * v[:, -1]
+        out[3][p], out[4][p] = -A[:, m - 1] * u[:, -1] / diag, C[:, m - 1] / diag
+        out[5][p] = (D[:, m - 1] - A[:, m - 1] * g[:, -1]) / diag
+    return tuple(out)
+
+
+def solve_y_pdd(a, b, c, d, P: int, precision: str = "f64") -> np.ndarray:
+    """The Parallel Diagonally Dominant algorithm (Sun, Parallel Computing 21 (1995), the paper's
+    [37]), step by step, for the P-partition split of every line (m = ny / P rows
+    per partition, block p = rows p m .. p m + m - 1, A_p its tridiagonal block):
+      1. three Thomas solves per block:  A_p xt = d_p,   A_p v = a_first e_0,   A_p w = c_last e_{m-1}
+         (a_first = the block's coupling to the row above it, c_last = to the row below it; the
+         spikes v, w decay away from the block end they start at);
+      2. the exact solution is  x_p = xt - v y_l(p-1) - w y_f(p+1)  with the interface unknowns
+         y_l(p) = x_last(p), y_f(p) = x_first(p); PDD DROPS the far ends of the spikes, w_0 and
+         v_{m-1}, which leaves one 2 x 2 system per interface:
+              y_l(p) + w^p_{m-1} y_f(p+1) = xt^p_{m-1} ,    v^{p+1}_0 y_l(p) + y_f(p+1) = xt^{p+1}_0 ;
+      3. x_p = xt - v y_l(p-1) - w y_f(p+1)  with those y (y_l(-1) = y_f(P) = 0).
+    Exact when the blocks do not couple; otherwise the error is of the order of the dropped
+    entries, which decay geometrically with m for strictly dominant systems (pinned in
+    tests/test_oracle_pins.py)."""
+    a, b, c, d = map(_as3, (a, b, c, d))
+    nz, ny, nx = a.shape
+    if ny % P or ny // P < 2:
+        raise ValueError("ny must split into P partitions of >= 2 rows")
+    m = ny // P
+    xt, v, w = np.empty_like(d), np.zeros_like(d), np.zeros_like(d)
+    for p in range(P):
+        r = slice(p * m, (p + 1) * m)
+        blk = [np.ascontiguousarray(t[:, r, :]) for t in (a, b, c)]
+        xt[:, r, :] = solve_y(*blk, np.ascontiguousarray(d[:, r, :]), precision)
+        if p > 0:
+            e = np.zeros((nz, m, nx)); e[:, 0, :] = a[:, p * m, :]
+            v[:, r, :] = solve_y(*blk, e, precision)
+        if p < P - 1:
+            e = np.zeros((nz, m, nx)); e[:, m - 1, :] = c[:, p * m + m - 1, :]
+            w[:, r, :] = solve_y(*blk, e, precision)
+    yl = np.zeros((P + 1, nz, nx)); yf = np.zeros((P + 1, nz, nx))     # yl[p] = y_l(p-1), yf[p] = y_f(p)
+    for p in range(P - 1):
+        wl, v0 = w[:, p * m + m - 1, :], v[:, (p + 1) * m, :]
+        tl, t0 = xt[:, p * m + m - 1, :], xt[:, (p + 1) * m, :]
+        det = 1.0 - wl * v0
+        yl[p + 1] = (tl - wl * t0) / det
+        yf[p + 1] = (t0 - v0 * tl) / det
+    x = np.empty_like(d)
+    for p in range(P):
+        r = slice(p * m, (p + 1) * m)
+        y_prev = yl[p][:, None, :]
+        y_next = (yf[p + 1] if p < P - 1 else np.zeros((nz, nx)))[:, None, :]
+        x[:, r, :] = xt[:, r, :] - v[:, r, :] * y_prev - w[:, r, :] * y_next
     return x

@@ -474,3 +474,88 @@ def test_f3_shared_toeplitz_eigenform_with_shift(alpha, n):
             ref[k, :, i] = z * mode / (lam - (sx[i] + sz[k]))
     x = oracle.solve_y_shared(np.full(n, -alpha), np.full(n, 1 + 2 * alpha), np.full(n, -alpha), sx, sz, d)
     assert np.max(np.abs(x - ref)) <= (1 + 4 * alpha) * 4e-15 * np.max(np.abs(ref))
+
+
+# ----------------------------------------------------------------------------------------------
+# SURVEY 8(f) f4, PDD variant
+# ----------------------------------------------------------------------------------------------
+def _dominant(rng, nz, ny, nx, margin=1.0):
+    a, c = rng.uniform(-1, 1, (nz, ny, nx)), rng.uniform(-1, 1, (nz, ny, nx))
+    b = margin + np.abs(a) + np.abs(c) + rng.uniform(0, 1, (nz, ny, nx))
+    return a, b, c, rng.uniform(-1, 1, (nz, ny, nx))
+
+
+@pytest.mark.parametrize("P,ny", [(2, 12), (4, 24), (3, 6)])
+def test_reduced_rows_hold_for_the_exact_solution(P, ny):
+    """The reduced system by definition: both rows of every partition are satisfied by the Thomas
+    solution of the whole line (a wrong sign or index in the Schur complement fails here)."""
+    rng = np.random.default_rng(P * 100 + ny)
+    a, b, c, d = _dominant(rng, 2, ny, 3)
+    x = oracle.solve_y(a, b, c, d)
+    fa, fc, fd, pa, pc, pd = oracle.reduced_rows_y(a, b, c, d, P)
+    m = ny // P
+    for p in range(P):
+        xf, xl = x[:, p * m, :], x[:, p * m + m - 1, :]
+        xp = x[:, p * m - 1, :] if p > 0 else 0.0
+        xn = x[:, p * m + m, :] if p < P - 1 else 0.0
+        assert np.max(np.abs(fa[p] * xp + xf + fc[p] * xl - fd[p])) <= 1e-13
+        assert np.max(np.abs(pa[p] * xf + xl + pc[p] * xn - pd[p])) <= 1e-13
+    assert np.all(fa[0] == 0) and np.all(pc[P - 1] == 0)
+
+
+def test_pdd_is_exact_when_partitions_do_not_couple_and_for_one_partition():
+    rng = np.random.default_rng(7)
+    a, b, c, d = _dominant(rng, 2, 32, 3)
+    assert np.array_equal(oracle.solve_y_pdd(a, b, c, d, 1), oracle.solve_y(a, b, c, d))
+    a2, c2 = a.copy(), c.copy()
+    for p in range(1, 4):                        # cut the couplings between the 4 partitions
+        a2[:, p * 8, :] = 0.0
+        c2[:, p * 8 - 1, :] = 0.0
+    exact = oracle.solve_y(a2, b, c2, d)
+    assert np.max(np.abs(oracle.solve_y_pdd(a2, b, c2, d, 4) - exact)) <= 1e-14
+
+
+def test_pdd_two_partitions_against_dense_truncation():
+    """P = 2 spelled out with dense LAPACK solves: spikes from np.linalg.solve, one 2 x 2 interface
+    system with the far spike ends dropped (a transposed spike or a swapped interface row fails)."""
+    rng = np.random.default_rng(13)
+    n, m = 12, 6
+    a, b, c, d = [t[0, :, 0] for t in _dominant(rng, 1, n, 1)]
+    def block(lo):
+        T = np.zeros((m, m))
+        for r in range(m):
+            T[r, r] = b[lo + r]
+            if r > 0: T[r, r - 1] = a[lo + r]
+            if r < m - 1: T[r, r + 1] = c[lo + r]
+        return T
+    T0, T1 = block(0), block(m)
+    xt0, xt1 = np.linalg.solve(T0, d[:m]), np.linalg.solve(T1, d[m:])
+    e = np.zeros(m); e[m - 1] = c[m - 1]
+    w0 = np.linalg.solve(T0, e)
+    e = np.zeros(m); e[0] = a[m]
+    v1 = np.linalg.solve(T1, e)
+    yl, yf = np.linalg.solve(np.array([[1.0, w0[m - 1]], [v1[0], 1.0]]), np.array([xt0[m - 1], xt1[0]]))
+    ref = np.concatenate([xt0 - w0 * yf, xt1 - v1 * yl])
+    got = oracle.solve_y_pdd(a[None, :, None], b[None, :, None], c[None, :, None], d[None, :, None], 2)[0, :, 0]
+    assert np.max(np.abs(got - ref)) <= 1e-14
+
+
+@pytest.mark.parametrize("alpha", [0.1, 1.0, 10.0])
+def test_pdd_error_decays_like_the_spikes(alpha):
+    """Toeplitz ADI lines (a = c = -alpha, b = 1 + 2 alpha; BASELINE cfg 4): the dropped couplings are
+    ~ r^(m-1) with r the root < 1 of alpha r^2 - (1 + 2 alpha) r + alpha = 0, so the error against the
+    exact solve is bounded by a small multiple of r^(m-1) and shrinks geometrically with m."""
+    rng = np.random.default_rng(11)
+    r = ((1 + 2 * alpha) - np.sqrt(1 + 4 * alpha)) / (2 * alpha)
+    prev = None
+    for m in (4, 8, 16, 32):
+        P, nz, nx = 4, 2, 3
+        ny = P * m
+        a = np.full((nz, ny, nx), -alpha); c = a.copy(); b = np.full((nz, ny, nx), 1 + 2 * alpha)
+        d = rng.uniform(-1, 1, (nz, ny, nx))
+        exact = oracle.solve_y(a, b, c, d)
+        err = np.max(np.abs(oracle.solve_y_pdd(a, b, c, d, P) - exact)) / np.max(np.abs(exact))
+        assert err <= 4.0 * r ** (m - 1) + 1e-15, (m, err, r ** (m - 1))
+        if prev is not None and prev > 1e-13:
+            assert err < prev
+        prev = err
