@@ -129,6 +129,13 @@ typedef struct tdma_options {
     int shared_cluster;  /* tdma_solve_shared: CTAs per cluster (1, 2, 4, 8), 0 = auto */
     int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16, 32), 0 = auto */
     int shared_slots;    /* tdma_solve_shared: tiles in the shared-memory ring (2 .. 4), 0 = auto */
+    int pdd;             /* PIPELINED / STAGED: 1 = stage B is the Parallel Diagonally Dominant variant
+                            (Sun 1995): the far ends of the partitions' spikes are
+                            dropped, which leaves one 2 x 2 system per partition interface instead of
+                            the 2P-row chain.  An APPROXIMATION: exact when partitions do not couple,
+                            error of the order of the dropped entries otherwise (they decay
+                            geometrically with ny/P for strictly dominant systems, e.g. below 1e-11
+                            for the ADI sweeps of BASELINE cfg 4 with alpha <= 1 at 64 rows per partition) */
     int shared_ctas;     /* tdma_solve_shared: CTAs per SM: 1, or 2 (the <= 128-register build of the
                             16-row-leaf kernel, two CTAs co-resident); 0 = auto */
 } tdma_options;
@@ -293,6 +300,8 @@ int tdma_slab_get(const tdma_slab *slab, int what);
 int tdma_slab_stage_a(tdma_slab *slab, int batch_index, const void *a, const void *b, const void *c,
                       const void *d, void *send, void *stream);
 int tdma_slab_stage_b(tdma_slab *slab, int batch_index, const void *recv, void *yout, void *stream);
+/* the same with the PDD reduced solve (tdma_options.pdd): independent 2 x 2 interface systems */
+int tdma_slab_stage_b_pdd(tdma_slab *slab, int batch_index, const void *recv, void *yout, void *stream);
 int tdma_slab_stage_c(tdma_slab *slab, int batch_index, const void *yrecv, void *x, void *stream);
 int tdma_slab_destroy(tdma_slab *slab);
 

@@ -35,7 +35,7 @@ EXPORTED_SYMBOLS = (
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
     "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
     "tdma_solve_shared", "tdma_probe_fp64",
-    "tdma_slab_create", "tdma_slab_get", "tdma_slab_stage_a", "tdma_slab_stage_b", "tdma_slab_stage_c",
+    "tdma_slab_create", "tdma_slab_get", "tdma_slab_stage_a", "tdma_slab_stage_b", "tdma_slab_stage_b_pdd", "tdma_slab_stage_c",
     "tdma_slab_destroy",
 )
 TDMA_SLAB_NB, TDMA_SLAB_BATCH, TDMA_SLAB_LINES, TDMA_SLAB_SHARE, TDMA_SLAB_PTOT = range(5)
@@ -50,7 +50,7 @@ class tdma_options(ctypes.Structure):
         ("fused_impl", ctypes.c_int), ("fused_fill", ctypes.c_int), ("axis", ctypes.c_int), ("periodic", ctypes.c_int),
         ("timeline", ctypes.c_int), ("fused_slots", ctypes.c_int), ("host_chunk", ctypes.c_int),
         ("shared_lines", ctypes.c_int), ("shared_cluster", ctypes.c_int), ("shared_leaf_rows", ctypes.c_int),
-        ("shared_slots", ctypes.c_int), ("shared_ctas", ctypes.c_int),
+        ("shared_slots", ctypes.c_int), ("pdd", ctypes.c_int), ("shared_ctas", ctypes.c_int),
     ]
 
 
@@ -102,6 +102,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_slab_stage_a.restype = ci
     lib.tdma_slab_stage_b.argtypes = [vp, ci] + [vp] * 3
     lib.tdma_slab_stage_b.restype = ci
+    lib.tdma_slab_stage_b_pdd.argtypes = [vp, ci] + [vp] * 3
+    lib.tdma_slab_stage_b_pdd.restype = ci
     lib.tdma_slab_stage_c.argtypes = [vp, ci] + [vp] * 3
     lib.tdma_slab_stage_c.restype = ci
     lib.tdma_slab_destroy.argtypes = [vp]
@@ -182,7 +184,7 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
                         fused_leaf_rows: int = 0, fused_top: int = 0, fused_impl: int = 0, fused_fill: int = 0,
                         axis: int = 0, periodic: int = 0, timeline: int = 0, fused_slots: int = 0, host_chunk: int = 0,
                         shared_lines: int = 0, shared_cluster: int = 0, shared_leaf_rows: int = 0,
-                        shared_slots: int = 0, shared_ctas: int = 0) -> int:
+                        shared_slots: int = 0, shared_ctas: int = 0, pdd: int = 0) -> int:
     opt = tdma_options()
     opt.struct_size = ctypes.sizeof(tdma_options)
     opt.variant, opt.nstreams, opt.use_graph = variant, nstreams, use_graph
@@ -191,7 +193,7 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
     opt.fused_fill, opt.axis, opt.periodic, opt.timeline = fused_fill, axis, periodic, timeline
     opt.host_chunk, opt.fused_slots = host_chunk, fused_slots
     opt.shared_lines, opt.shared_cluster, opt.shared_leaf_rows, opt.shared_slots = shared_lines, shared_cluster, shared_leaf_rows, shared_slots
-    opt.shared_ctas = shared_ctas
+    opt.shared_ctas, opt.pdd = shared_ctas, pdd
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
         raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())
@@ -230,6 +232,10 @@ def tdma_slab_stage_a(slab: int, batch_index: int, a, b, c, d, send, stream=None
 
 def tdma_slab_stage_b(slab: int, batch_index: int, recv, yout, stream=None) -> None:
     _check(load_library().tdma_slab_stage_b(slab, batch_index, _ptr(recv), _ptr(yout), _stream_handle(stream)))
+
+
+def tdma_slab_stage_b_pdd(slab: int, batch_index: int, recv, yout, stream=None) -> None:
+    _check(load_library().tdma_slab_stage_b_pdd(slab, batch_index, _ptr(recv), _ptr(yout), _stream_handle(stream)))
 
 
 def tdma_slab_stage_c(slab: int, batch_index: int, yrecv, x, stream=None) -> None:

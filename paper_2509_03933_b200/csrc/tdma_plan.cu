@@ -64,6 +64,7 @@ struct tdma_plan {
     int nx = 0, ny = 0, nz = 0, P = 0, m = 0, bz = 0, nb = 0;
     int variant = TDMA_VARIANT_PIPELINED, nstreams = 2, nlanes = 1, depth = 3;
     int use_graph = 1, separate_gather = 0;
+    int pdd = 0;                           // stage B = PDD (far spike ends dropped, 2 x 2 interface systems)
     int timeline = 0;                      // timing events around every stage launch
     std::vector<cudaEvent_t> tl_ev;        // 2 per launch, reused across solves
     std::vector<int> tl_tag;               // stage * 2^20 + batch, per launch of the last solve
@@ -175,7 +176,12 @@ int launch_stage(tdma_plan *pl, int stage, const tdma::StageParams &prm_in, cuda
         break;
     }
     case TDMA_STAGE_B:
-        tdma::stage_b_kernel<kPrefetchRows><<<(Lb + 63) / 64, 64, 0, st>>>(prm);
+        if (pl->pdd) {
+            dim3 grid((Lb + 127) / 128, prm.P);
+            tdma::stage_b_pdd_kernel<<<grid, 128, 0, st>>>(prm);
+        } else {
+            tdma::stage_b_kernel<kPrefetchRows><<<(Lb + 63) / 64, 64, 0, st>>>(prm);
+        }
         break;
     case TDMA_STAGE_C: {
         dim3 grid((Lb + 127) / 128, pl->P);
@@ -461,6 +467,9 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
     pl->timeline = (opt && opt->timeline > 0) ? 1 : 0;
     if (pl->timeline) pl->use_graph = 0;
     pl->separate_gather = (opt && opt->separate_gather > 0) ? 1 : 0;
+    pl->pdd = (opt && opt->pdd > 0) ? 1 : 0;
+    if (pl->pdd && variant == TDMA_VARIANT_FUSED)
+        return set_err(TDMA_ERR_UNSUPPORTED, "pdd replaces stage B of the PIPELINED / STAGED variants; FUSED has no separate stage B");
     pl->nstreams = (opt && opt->nstreams > 0) ? opt->nstreams : 2;
     if (pl->nstreams > kMaxLanes + 1)
         return set_err(TDMA_ERR_INVALID_ARG, "nstreams %d > %d", pl->nstreams, kMaxLanes + 1);

@@ -133,7 +133,7 @@ int tdma_slab_stage_a(tdma_slab *s, int batch_index, const void *a, const void *
     return cudaGetLastError() == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
 }
 
-int tdma_slab_stage_b(tdma_slab *s, int batch_index, const void *recv, void *yout, void *stream)
+static int slab_stage_b(tdma_slab *s, int batch_index, const void *recv, void *yout, void *stream, bool pdd)
 {
     int k0, bzn;
     if (!s || !recv || !yout || !batch_range(s, batch_index, &k0, &bzn)) return slab_err(TDMA_ERR_INVALID_ARG);
@@ -146,8 +146,23 @@ int tdma_slab_stage_b(tdma_slab *s, int batch_index, const void *recv, void *you
     const unsigned Ls = (unsigned)prm.Ls;
     dim3 grid((Ls + 255) / 256, prm.Ptot);
     tdma::gather_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(prm);
-    tdma::stage_b_kernel<kU><<<(Ls + 63) / 64, 64, 0, (cudaStream_t)stream>>>(prm);
+    if (pdd) {
+        dim3 gb((Ls + 127) / 128, prm.Ptot);
+        tdma::stage_b_pdd_kernel<<<gb, 128, 0, (cudaStream_t)stream>>>(prm);
+    } else {
+        tdma::stage_b_kernel<kU><<<(Ls + 63) / 64, 64, 0, (cudaStream_t)stream>>>(prm);
+    }
     return cudaGetLastError() == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
+}
+
+int tdma_slab_stage_b(tdma_slab *s, int batch_index, const void *recv, void *yout, void *stream)
+{
+    return slab_stage_b(s, batch_index, recv, yout, stream, false);
+}
+
+int tdma_slab_stage_b_pdd(tdma_slab *s, int batch_index, const void *recv, void *yout, void *stream)
+{
+    return slab_stage_b(s, batch_index, recv, yout, stream, true);
 }
 
 int tdma_slab_stage_c(tdma_slab *s, int batch_index, const void *yrecv, void *x, void *stream)

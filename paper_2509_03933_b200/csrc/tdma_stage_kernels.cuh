@@ -227,6 +227,54 @@ __global__ void __launch_bounds__(64) stage_b_kernel(const StageParams prm)
 }
 
 // ------------------------------------------------------------------------------------------
+// Stage B, PDD variant (Sun 1995): no chain over the 2P rows.  The reduced rows
+//      fa y_l(p-1) + x_f + fc x_l = fd ,      pa x_f + x_l + pc y_f(p+1) = pd
+// of partition p are first solved for (x_f, x_l) as functions of the NEIGHBOURS' interface
+// unknowns (the partition's own 2 x 2 block, det = 1 - fc pa):
+//      x_f = xt0 - v0 y_l(p-1) - w0 y_f(p+1) ,   x_l = xtl - vl y_l(p-1) - wl y_f(p+1)
+// -- xt, v, w are the first / last entries of Sun's block solution and spikes.  PDD drops the far
+// spike ends w0 and vl, which leaves one 2 x 2 system per interface,
+//      y_l(p) + wl(p) y_f(p+1) = xtl(p) ,     v0(p+1) y_l(p) + y_f(p+1) = xt0(p+1) ,
+// and then evaluates x_f, x_l with all four spike ends.  One thread per (line, partition): it
+// rebuilds the spike ends of its two neighbours from their rows (18 coalesced loads, no
+// dependence on any other thread).  Exact when partitions do not couple; error of the order of
+// the dropped entries otherwise (strictly dominant systems: geometric in ny/P).
+// ------------------------------------------------------------------------------------------
+struct SpikeEnds { double xt0, v0, w0, xtl, vl, wl; };
+
+__device__ __forceinline__ SpikeEnds spike_ends(const double *__restrict__ ra, const double *__restrict__ rc,
+                                                const double *__restrict__ rd, size_t q0, size_t Lb)
+{
+    const double fa = ld_keep(ra + q0), fc = ld_keep(rc + q0), fd = ld_keep(rd + q0);
+    const double pa = ld_keep(ra + q0 + Lb), pc = ld_keep(rc + q0 + Lb), pd = ld_keep(rd + q0 + Lb);
+    const double inv = 1.0 / fma(-fc, pa, 1.0);
+    SpikeEnds s;
+    s.xt0 = fma(-fc, pd, fd) * inv; s.v0 = fa * inv; s.w0 = -(fc * pc) * inv;
+    s.xtl = fma(-pa, fd, pd) * inv; s.vl = -(pa * fa) * inv; s.wl = pc * inv;
+    return s;
+}
+
+static __global__ void __launch_bounds__(128) stage_b_pdd_kernel(const StageParams prm)
+{
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= prm.Lb) return;
+    const int p = blockIdx.y, P = prm.P;
+    const size_t Lb = (size_t)prm.Lb;
+    const SpikeEnds me = spike_ends(prm.ra, prm.rc, prm.rd, (size_t)(2 * p) * Lb + l, Lb);
+    double y_prev = 0.0, y_next = 0.0;        // y_l(p-1), y_f(p+1)
+    if (p > 0) {
+        const SpikeEnds lo = spike_ends(prm.ra, prm.rc, prm.rd, (size_t)(2 * p - 2) * Lb + l, Lb);
+        y_prev = fma(-lo.wl, me.xt0, lo.xtl) / fma(-lo.wl, me.v0, 1.0);
+    }
+    if (p < P - 1) {
+        const SpikeEnds hi = spike_ends(prm.ra, prm.rc, prm.rd, (size_t)(2 * p + 2) * Lb + l, Lb);
+        y_next = fma(-hi.v0, me.xtl, hi.xt0) / fma(-me.wl, hi.v0, 1.0);
+    }
+    st_keep(prm.y + (size_t)(2 * p) * Lb + l, fma(-me.w0, y_next, fma(-me.v0, y_prev, me.xt0)));
+    st_keep(prm.y + (size_t)(2 * p + 1) * Lb + l, fma(-me.wl, y_next, fma(-me.vl, y_prev, me.xtl)));
+}
+
+// ------------------------------------------------------------------------------------------
 // Stage C: back-substitution inside each partition, one thread per (line, partition).
 // ------------------------------------------------------------------------------------------
 // kSlab: x_first / x_last come from the all-to-all's receive buffer yrecv[src rank][2 P][Ls] (prm.y),

@@ -35,7 +35,9 @@ DEPTH = 3
 class CudaSlabStages:
     """The rank-local stages through the C ABI (device buffers, CUDA streams)."""
 
-    def __init__(self, nx: int, ny_local: int, nz: int, P_local: int, batch: int, rank: int, nranks: int):
+    def __init__(self, nx: int, ny_local: int, nz: int, P_local: int, batch: int, rank: int, nranks: int,
+                 pdd: bool = False):
+        self.pdd = pdd      # stage B = PDD (PAPER.md:280, 326): 2 x 2 interface systems, an approximation
         self.nx, self.ny, self.nz, self.P, self.rank, self.nranks = nx, ny_local, nz, P_local, rank, nranks
         self.handle = _b.tdma_slab_create(nx, ny_local, nz, P_local, batch, rank, nranks)
         self.nb = _b.tdma_slab_get(self.handle, _b.TDMA_SLAB_NB)
@@ -52,7 +54,7 @@ class CudaSlabStages:
         _b.tdma_slab_stage_a(self.handle, n, a, b, c, d, send, stream)
 
     def stage_b(self, n, recv, yout, stream=None):
-        _b.tdma_slab_stage_b(self.handle, n, recv, yout, stream)
+        (_b.tdma_slab_stage_b_pdd if self.pdd else _b.tdma_slab_stage_b)(self.handle, n, recv, yout, stream)
 
     def stage_c(self, n, yrecv, x, stream=None):
         _b.tdma_slab_stage_c(self.handle, n, yrecv, x, stream)
@@ -69,14 +71,14 @@ class YSlabSolver:
     with no initialised process group a single rank runs alone and the exchange is a local copy)."""
 
     def __init__(self, nx: int, ny_local: int, nz: int, P_local: int = 1, batch: int = 0, group=None,
-                 stages=None):
+                 stages=None, pdd: bool = False):
         import torch.distributed as dist
         self.dist = dist if dist.is_available() and dist.is_initialized() else None
         self.group = group
         self.rank = self.dist.get_rank(group) if self.dist else 0
         self.nranks = self.dist.get_world_size(group) if self.dist else 1
         self.stages = stages if stages is not None else CudaSlabStages(nx, ny_local, nz, P_local, batch,
-                                                                       self.rank, self.nranks)
+                                                                       self.rank, self.nranks, pdd=pdd)
         self.P = P_local
         self.device = self.stages.device
         self.cuda = self.device.type == "cuda"

@@ -35,7 +35,7 @@ def test_options_struct_matches_header():
     body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
     fields = re.findall(r"int\s+([a-z_]+)(\[\d+\])?;", body)
     assert [f[0] for f in fields] == [f[0] for f in tdma.tdma_options._fields_]
-    assert ctypes.sizeof(tdma.tdma_options) == 4 * len(tdma.tdma_options._fields_) == 4 * 21
+    assert ctypes.sizeof(tdma.tdma_options) == 4 * len(tdma.tdma_options._fields_) == 4 * 22
 
 
 def test_version():

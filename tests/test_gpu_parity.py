@@ -584,6 +584,38 @@ def test_staged_schedule_invariance():
 
 
 # ---------------------------------------------------------------------------------------------
+# PDD variant of stage B
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [tdma.TDMA_VARIANT_PIPELINED, tdma.TDMA_VARIANT_STAGED], ids=["pipelined", "staged"])
+@pytest.mark.parametrize("kind", ["random", "adi_0.3", "adi_8"])
+def test_pdd_stage_b_matches_the_pdd_reference(variant, kind):
+    """options.pdd: stage B solves the 2 x 2 interface systems of Sun's PDD.  An approximation, so
+    the reference is oracle.solve_y_pdd for the same partition count (element-wise parity at 1e-11:
+    both sides drop the same entries), and the distance to the EXACT solve is checked against the
+    size of what was dropped (alpha = 8: r = 0.70, 64-row partitions -> ~1e-10 relative)."""
+    nx, ny, nz, P = 64, 256, 4, 4
+    if kind == "random":
+        a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 71, dev())
+    else:
+        a, b, c, d, _ = tdma_inputs.adi_toeplitz(nx, ny, nz, 72, dev(), alpha=float(kind.split("_")[1]))
+    x = torch.full_like(d, float("nan"))
+    with tdma.Plan(nx, ny, nz, P, 2, variant=variant, pdd=1) as plan:
+        pe = plan.get(tdma.TDMA_GET_REDUCED_PARTITIONS)
+        plan.solve(a, b, c, d, x)
+        torch.cuda.synchronize()
+    an, bn, cn, dn, xn = to_np(a, b, c, d, x)
+    ref = oracle.solve_y_pdd(an, bn, cn, dn, pe)
+    assert oracle.normwise_error(xn, ref).max() <= TOL_E
+    exact = oracle.solve_y(an, bn, cn, dn)
+    gap, own = oracle.normwise_error(xn, exact).max(), oracle.normwise_error(ref, exact).max()
+    assert gap <= 2 * own + 1e-13                      # the GPU is as far from exact as the reference is
+    if kind == "adi_0.3":
+        assert gap <= 1e-13                            # r = 0.22: r^63 is far below rounding
+    with pytest.raises(tdma.TdmaError):
+        tdma.Plan(nx, ny, nz, P, 0, variant=tdma.TDMA_VARIANT_FUSED, pdd=1)
+
+
+# ---------------------------------------------------------------------------------------------
 # Host-buffer entry point
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("variant", VARIANTS)

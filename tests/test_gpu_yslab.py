@@ -23,13 +23,13 @@ def dev():
     return torch.device("cuda:0")
 
 
-def emulate(a, b, c, d, nranks, P_local, batch, keep=None):
+def emulate(a, b, c, d, nranks, P_local, batch, keep=None, pdd=False):
     """All ranks' stages in sequence; returns x of the undivided slab."""
     nz, ny, nx = a.shape
     nyl = ny // nranks
     loc = [[t[:, r * nyl:(r + 1) * nyl, :].contiguous() for t in (a, b, c, d)] for r in range(nranks)]
     xs = [torch.full_like(loc[r][3], float("nan")) for r in range(nranks)]
-    st = [CudaSlabStages(nx, nyl, nz, P_local, batch, r, nranks) for r in range(nranks)]
+    st = [CudaSlabStages(nx, nyl, nz, P_local, batch, r, nranks, pdd=pdd) for r in range(nranks)]
     try:
         for n in range(st[0].nb):
             lb, ls = st[0].batch_lines(n)
@@ -68,6 +68,19 @@ def test_poisson_slab_over_four_emulated_ranks():
     x = emulate(w.a, w.b, w.c, w.d, 4, 2, 4)
     an, bn, cn, dn, xn = [t.cpu().numpy() for t in (w.a, w.b, w.c, w.d, x)]
     assert oracle.normwise_error(xn, oracle.solve_y(an, bn, cn, dn, "ld")).max() <= TOL_E
+
+
+@pytest.mark.parametrize("nranks,P_local", [(4, 1), (2, 2)])
+def test_pdd_over_emulated_ranks(nranks, P_local):
+    """PDD reduced solve across emulated ranks: parity with oracle.solve_y_pdd for
+    nranks * P_local partitions (both drop the far spike ends), and -- 64-row partitions of a
+    strictly dominant system -- agreement with the exact solve far below the tolerance."""
+    nx, ny, nz = 32, 256, 4
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 53, dev())
+    x = emulate(a, b, c, d, nranks, P_local, 2, pdd=True)
+    an, bn, cn, dn, xn = [t.cpu().numpy() for t in (a, b, c, d, x)]
+    assert oracle.normwise_error(xn, oracle.solve_y_pdd(an, bn, cn, dn, nranks * P_local)).max() <= TOL_E
+    assert oracle.normwise_error(xn, oracle.solve_y(an, bn, cn, dn)).max() <= TOL_E
 
 
 def test_exchange_buffers_hold_the_schur_complement_rows():
