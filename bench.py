@@ -526,15 +526,19 @@ def main():
 
     # ---- roofline of the dominant kernel -----------------------------------------------------
     if best == "fused":
-        # One persistent launch does the whole step.  When clusters of >= 4 CTAs leave SMs empty, a
-        # concurrent fill launch (clusters of 2) solves the last `fill` z-slices on them; the
-        # dominant kernel is the main launch, which spans the whole step (CUDA events around the
-        # step on the launching stream) and processes nz - fill slices.
+        # Persistent launches back to back do the whole step.  When clusters of >= 4 CTAs leave SMs
+        # empty, a concurrent fill launch (clusters of 2) solves the last `fill` z-slices of each
+        # launch's range on them; the dominant kernel is the main launch: together the main launches
+        # span the step (CUDA events around the step on the launching stream).
+        # the slab is solved in nb_f persistent launches of bz_f slices (default: ~2^27 cells each),
+        # every one with its own fill launch over its last `fill` slices
         nb_f = max(1, plan.get(tdma.TDMA_GET_NB))
-        alg_bytes = ALG_BYTES_PER_CELL * w.nx * w.ny * (w.nz - fill) / nb_f
-        dur = sec / nb_f
+        bz_f = plan.get(tdma.TDMA_GET_BATCH)
+        alg_bytes = ALG_BYTES_PER_CELL * w.nx * w.ny * (bz_f - fill)
+        dur = sec * bz_f / w.nz
         achieved = alg_bytes / dur / 1e9
         out["config"]["fill_slices"] = fill
+        out["config"]["launches_per_step"] = ok[best]["launches"]
         fcfg = fused_config(tdma, plan)
         out["config"]["fused"] = fcfg
         traffic, tsrc = ncu_traffic(alg_bytes, fcfg)
@@ -743,11 +747,12 @@ def sweep(torch, tdma, w, x, args, barrier, rank):
     nz = w.nz
     batches = [b for b in (1, 2, 4, 8, 16, 32, 64, 128) if b <= nz]
     points = []
-    for variant, streams_list in (("pipelined", (1, 2, 3, 4)), ("fused", (1,))):
+    vm = {"fused": tdma.TDMA_VARIANT_FUSED, "pipelined": tdma.TDMA_VARIANT_PIPELINED, "staged": tdma.TDMA_VARIANT_STAGED}
+    for variant, streams_list in (("pipelined", (1, 2, 3, 4)), ("staged", (1, 2, 3, 4)), ("fused", (1,))):
         for ns in streams_list:
             for bz in batches + ([0] if variant == "fused" else []):
-                opts = dict(variant={"fused": tdma.TDMA_VARIANT_FUSED, "pipelined": tdma.TDMA_VARIANT_PIPELINED}[variant])
-                if variant == "pipelined":
+                opts = dict(variant=vm[variant])
+                if variant != "fused":
                     opts["nstreams"] = ns
                 try:
                     with tdma.Plan(w.nx, w.ny, nz, w.P, bz, **opts) as plan:

@@ -53,8 +53,9 @@ typedef enum tdma_status {
 /* How the three compute stages of the divide-and-conquer solve (Fig. 5) are
  * mapped onto the GPU. */
 typedef enum tdma_variant {
-    /* The fastest variant that can run the plan: FUSED (TMA kernel, one persistent launch, `batch`
-     * ignored) when the shape tiles, else PIPELINED.  This is what tdma_plan_create uses. */
+    /* The fastest variant that can run the plan: FUSED (TMA kernel, `batch` ignored: persistent
+     * launches of about 2^27 cells each) when the shape tiles, else PIPELINED.  This is what
+     * tdma_plan_create uses. */
     TDMA_VARIANT_AUTO = 0,
     /* Stage A (partition reduce, fused gather) / Stage B (reduced 2P-row solve) / Stage C
      * (back-substitution) as separate kernels, z-batches pipelined over CUDA streams with events
@@ -64,7 +65,8 @@ typedef enum tdma_variant {
     /* One persistent kernel: a thread-block cluster owns whole lines, the partitions of a line
      * live in the shared memory of the cluster's CTAs (the paper's ranks), the reduced system is
      * exchanged through distributed shared memory (the paper's MPI_Alltoall) and
-     * solved inside the cluster, so HBM sees a, b, c, d once and x once (40 B/cell). */
+     * solved inside the cluster, so HBM sees a, b, c, d once and x once (40 B/cell).  `batch` only
+     * chunks the z range into launches (0 = about 2^27 cells per launch). */
     TDMA_VARIANT_FUSED = 2,
     /* The paper's three stages as separate kernels on the Alg. 2 stream pipeline, like PIPELINED,
      * but stage A and stage C fetch their partition segments by TMA into shared memory and keep

@@ -135,6 +135,17 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, in
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
         ::"r"(smem_u32(dst)), "l"(tm), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *tm, int c0, int c1, int c2, int c3, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap *tm, int c0, int c1, int c2, int c3, const void *src)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(src)) : "memory");
+}
 __device__ __forceinline__ void tma_store_3d(const CUtensorMap *tm, int x, int y, int z, const void *src)
 {
     asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];"
@@ -860,10 +871,11 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         double *const dst = raw + (size_t)s * arr;
         const CUtensorMap *const tm = j == 0 ? &tm_b : (j == 1 ? &tm_a : (j == 2 ? &tm_c : &tm_d));
         if (issue_lane == 0) ptx::mbar_expect_tx(&bar[s], arr_bytes);
-        if (kX) {                   // one (16 x, TX lines) box per leaf; x0 = first line (y)
-            __syncwarp();
-            for (int w = issue_lane; w < W; w += 32)
-                ptx::tma_load_3d(dst + w * 16 * TX, tm, y0 + 16 * w, x0, k, &bar[s]);
+        if (kX) {
+            // x sweep: the line axis is viewed as (16 x, leaf) -- tensor (16, lanes, nrows / 16, slices)
+            // -- so ONE copy of box (16, TX, W, 1) brings the CTA's W leaves of all TX lines, laid out
+            // [leaf][line][16 x] with the 128-byte swizzle keyed by the line; x0 = first line
+            if (issue_lane == 0) ptx::tma_load_4d(dst, tm, 0, x0, y0 >> 4, k, &bar[s]);
         } else if (issue_lane == 0) {
             for (int q = 0; q < prm.nbox; ++q) {
                 const int yy = y0 + q * prm.box_rows;
@@ -875,7 +887,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     auto store_x = [&](int tile) {
         const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
         if (kX) {
-            for (int w = issue_lane; w < W; w += 32) ptx::tma_store_3d(&tm_x, y0 + 16 * w, x0, k, sX + w * 16 * TX);
+            if (issue_lane == 0) ptx::tma_store_4d(&tm_x, 0, x0, y0 >> 4, k, sX);
         } else if (issue_lane == 0) {
             for (int q = 0; q < prm.nbox; ++q) {
                 const int yy = y0 + q * prm.box_rows;
@@ -1267,17 +1279,19 @@ inline bool make_slab_tensor_map(CUtensorMap *tm, const void *base, int nx, int 
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// x sweep: contiguous fp64 slab (rows = x fastest, lanes = y, slices); box (16 x, TX lanes, 1)
-// with the 128-byte swizzle.
-inline bool make_xsweep_tensor_map(CUtensorMap *tm, const void *base, int nrows, int nlanes, int nslices, int TX)
+// x sweep: contiguous fp64 slab (rows = x fastest, lanes = y, slices) viewed as the 4-D tensor
+// (16 x, lanes, nrows / 16 leaves, slices); box (16, TX, W, 1) with the 128-byte swizzle: one copy per
+// array and tile, landing as [leaf][line][16 x].  (The leaf dimension has the SMALLER stride, 128 B,
+// than the lane dimension before it; tensor maps do not require ordered strides.)
+inline bool make_xsweep_tensor_map(CUtensorMap *tm, const void *base, int nrows, int nlanes, int nslices, int TX, int W)
 {
     tdma_encode_tiled_fn enc = get_encode_tiled();
-    if (!enc) return false;
-    cuuint64_t gdim[3] = {(cuuint64_t)nrows, (cuuint64_t)nlanes, (cuuint64_t)nslices};
-    cuuint64_t gstr[2] = {(cuuint64_t)nrows * sizeof(double), (cuuint64_t)nrows * nlanes * sizeof(double)};
-    cuuint32_t box[3] = {16, (cuuint32_t)TX, 1};
-    cuuint32_t estr[3] = {1, 1, 1};
-    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), gdim, gstr, box, estr,
+    if (!enc || nrows % 16) return false;
+    cuuint64_t gdim[4] = {16, (cuuint64_t)nlanes, (cuuint64_t)(nrows / 16), (cuuint64_t)nslices};
+    cuuint64_t gstr[3] = {(cuuint64_t)nrows * sizeof(double), 128, (cuuint64_t)nrows * nlanes * sizeof(double)};
+    cuuint32_t box[4] = {16, (cuuint32_t)TX, (cuuint32_t)W, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<void *>(base), gdim, gstr, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -1363,7 +1377,7 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
     CUtensorMap tm[5];
     const void *ptr[5] = {a, b, c, d, x};
     for (int i = 0; i < 5 && nzs > 0; ++i) {
-        if (cfg.xaxis ? !make_xsweep_tensor_map(&tm[i], ptr[i], ny, nx, nzs, cfg.lines)
+        if (cfg.xaxis ? !make_xsweep_tensor_map(&tm[i], ptr[i], ny, nx, nzs, cfg.lines, cfg.leaves)
                       : !make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows))
             return cudaErrorInvalidValue;
     }

@@ -63,6 +63,7 @@ struct GraphEntry {
 struct tdma_plan {
     int nx = 0, ny = 0, nz = 0, P = 0, m = 0, bz = 0, nb = 0;
     int variant = TDMA_VARIANT_PIPELINED, nstreams = 2, nlanes = 1, depth = 3;
+    int batch_arg = 0;                     // `batch` as passed to tdma_plan_create
     int use_graph = 1, separate_gather = 0;
     int pdd = 0;                           // stage B = PDD (far spike ends dropped, 2 x 2 interface systems)
     int timeline = 0;                      // timing events around every stage launch
@@ -449,9 +450,17 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
                                                       prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z,
                                                       opt ? opt->fused_slots : 0);
         variant = (tma_ok || pl->axis == TDMA_AXIS_X || pl->periodic) ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
-        if (variant == TDMA_VARIANT_FUSED) {
-            pl->bz = pl->nz; pl->nb = 1; pl->Lb_max = (size_t)pl->nx * pl->bz;
-        }
+        if (variant == TDMA_VARIANT_FUSED) pl->batch_arg = 0;   // batch is a hint for the stage pipelines only
+    }
+    if (variant == TDMA_VARIANT_FUSED && pl->batch_arg == 0) {
+        // FUSED default: launches of about 2^27 cells (128 slices of 1024 x 1024).  The clusters of a
+        // persistent launch drift apart over a long run and DRAM row locality between neighbouring
+        // x tiles goes with it; a fresh launch every ~0.9 ms re-aligns them (measured on cfg 3:
+        // 7.25 ms as one launch, 7.02 ms in chunks of 128-256 slices; cfg 5: 7.38 -> 7.22 ms)
+        const long long chunk = std::max<long long>(1, ((long long)1 << 27) / (long long)pl->slice);
+        pl->bz = (int)std::min<long long>(pl->nz, chunk);
+        pl->nb = (pl->nz + pl->bz - 1) / pl->bz;
+        pl->Lb_max = (size_t)pl->nx * pl->bz;
     }
     if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED && variant != TDMA_VARIANT_STAGED)
         return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
@@ -610,6 +619,7 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     if (options) { pl->sh_opt[0] = options->shared_lines; pl->sh_opt[1] = options->shared_cluster; pl->sh_opt[2] = options->shared_leaf_rows; pl->sh_opt[3] = options->shared_slots; pl->sh_opt[4] = options->shared_ctas; }
     pl->rs = axis == TDMA_AXIS_Z ? (long long)nx * nz : (long long)nx;   // z sweep: plan nz = caller ny
     pl->os = axis == TDMA_AXIS_Z ? (long long)nx : (long long)nx * ny;   // x sweep: slices are z-slices
+    pl->batch_arg = batch;
     pl->bz = batch == 0 ? nz : batch;
     pl->nb = (nz + pl->bz - 1) / pl->bz;
     pl->slice = (size_t)nx * ny;

@@ -176,7 +176,7 @@ def test_auto_variant_and_host_buffers_on_x_sweep():
     it does not; tdma_solve_host works for x sweeps (z-chunks are contiguous) and refuses z sweeps."""
     with tdma.Plan(64, 64, 8, 4, 2) as plan:
         assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_FUSED
-        assert plan.get(tdma.TDMA_GET_NB) == 1          # batch is a hint for the pipelined variant only
+        assert plan.get(tdma.TDMA_GET_NB) == 1          # batch is a hint for the stage pipelines only
     with tdma.Plan(45, 30, 8, 5, 2) as plan:            # odd nx, m = 6: no power-of-two tree
         assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_PIPELINED
         assert plan.get(tdma.TDMA_GET_NB) == 4

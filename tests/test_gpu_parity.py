@@ -158,11 +158,11 @@ def test_cfg5_full_size_sampled(variant):
 @pytest.mark.parametrize("name,slices,strictly", [("cfg3_weak", [0, 1, 2, 257, 513, 900], False),
                                                   ("cfg5_stress", [0, 1, 300, 777], True)])
 def test_full_size_in_the_bench_launch_configuration(name, slices, strictly):
-    """Exactly what bench.py times: FUSED, batch = 0, i.e. ONE persistent launch over the slab
-    (~1900 tiles per cluster on cfg 3) plus, where clusters of 4 leave SMs empty, the concurrent
-    fill launch; slices of both ranges against the oracle."""
+    """Exactly what bench.py times: FUSED, batch = 0, i.e. persistent launches of 2^27 cells (128
+    slices, ~250 tiles per cluster on cfg 3), each with its concurrent fill launch where clusters
+    of 4 leave SMs empty; slices of main and fill ranges of several launches against the oracle."""
     worst, fill, launches = _sampled_full(name, dict(variant=tdma.TDMA_VARIANT_FUSED), 0, slices, strictly)
-    assert launches == (2 if fill > 0 else 1)
+    assert launches == 8 * (2 if fill > 0 else 1)
 
 
 # ---------------------------------------------------------------------------------------------
