@@ -306,9 +306,10 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
                 int fc = idle / pl->tfill.cluster;
                 if (fc > pl->tfill.max_clusters) fc = pl->tfill.max_clusters;
                 if (fc > 0) {
-                    // measured on cfg 3: an SM of the fill launch (64 B row segments, clusters far
-                    // apart in x) sustains about 0.55 of a main SM
-                    const double w = 0.55 * fc * pl->tfill.cluster;
+                    // measured: an SM of the fill launch sustains about 0.55 of a main SM when its
+                    // tiling has 64-byte row segments (cfg 3: 8 lines per tile) and about as much as a
+                    // main SM with 128-byte segments (cfg 4 z sweeps: best share 0.11 = 16 / 148 SMs)
+                    const double w = (pl->tfill.lines >= 16 ? 1.0 : 0.55) * fc * pl->tfill.cluster;
                     double share = pl->fill_opt > 0 ? pl->fill_opt * 1e-3 : w / (w + main_ctas);
                     nzf = (int)(bzn * share + 0.5);
                     if (nzf >= bzn) nzf = bzn - 1;
