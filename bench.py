@@ -557,6 +557,11 @@ def main():
         rep, st = pipelined_report(torch, tdma, pplan, w, x, psec)
         out["variants"][pname].update(rep)
         out["variants"][pname]["hbm_bytes_per_cell"] = 88.0 if pname == "pipelined" else 72.0
+        try:        # the overlap itself, from per-launch events on the plan's streams (one untimed solve)
+            tl, _ = timeline_overlap(torch, tdma, w, x, vmap[pname], ok[pname]["batch"], ok[pname]["nstreams"])
+            out["variants"][pname]["timeline"] = tl
+        except tdma.TdmaError as exc:
+            out["variants"][pname]["timeline"] = {"error": str(exc)}
         if best == "pipelined" and pname == "pipelined":
             bz = ok[best]["batch"]
             bcells = w.nx * w.ny * bz
@@ -639,12 +644,11 @@ def main():
     return 0
 
 
-def timeline(torch, tdma, w, x, args, batch, rank):
-    """Stream-overlap timeline of the PIPELINED variant (Alg. 2): how much of stage B's time runs
-    while a stage A or C kernel of another batch is running.  Plain stream launches (no graph)."""
-    ns = args.nstreams or 2
-    with tdma.Plan(w.nx, w.ny, w.nz, w.P, batch, variant=tdma.TDMA_VARIANT_PIPELINED, nstreams=ns, timeline=1) as plan:
-        for _ in range(max(3, args.warmup)):
+def timeline_overlap(torch, tdma, w, x, variant, batch, ns, warmup=3):
+    """One solve of a stage-pipeline plan with per-launch timing events (options.timeline): how much
+    of stage B's time lies inside the union of the stage A / C intervals of other batches."""
+    with tdma.Plan(w.nx, w.ny, w.nz, w.P, batch, variant=variant, nstreams=ns, timeline=1) as plan:
+        for _ in range(warmup):
             plan.solve(w.a, w.b, w.c, w.d, x)
         torch.cuda.synchronize()
         plan.solve(w.a, w.b, w.c, w.d, x)
@@ -652,10 +656,10 @@ def timeline(torch, tdma, w, x, args, batch, rank):
     names = {0: "A", 1: "G", 2: "B", 3: "C"}
     t0 = min(r[2] for r in recs)
     recs = sorted(((names[r[0]], r[1], r[2] - t0, r[3] - t0) for r in recs), key=lambda r: r[2])
-    ac = [(r[2], r[3]) for r in recs if r[0] in "AC"]
+    ac = sorted((r[2], r[3]) for r in recs if r[0] in "AC")
     def covered(lo, hi):                       # length of [lo, hi] covered by the union of A/C intervals
         tot, cur = 0.0, lo
-        for s0, s1 in sorted(ac):
+        for s0, s1 in ac:
             s0, s1 = max(s0, cur), min(s1, hi)
             if s1 > s0:
                 tot += s1 - s0
@@ -663,10 +667,19 @@ def timeline(torch, tdma, w, x, args, batch, rank):
         return tot
     tb = sum(r[3] - r[2] for r in recs if r[0] == "B")
     tb_hidden = sum(covered(r[2], r[3]) for r in recs if r[0] == "B")
-    span = max(r[3] for r in recs)
-    rec = {"timeline": True, "workload": args.workload, "batch": batch, "nstreams": ns, "launches": len(recs),
-           "span_ms": span, "sum_ms": {k: sum(r[3] - r[2] for r in recs if r[0] == k) for k in "ABC"},
-           "stage_b_overlapped_frac": tb_hidden / tb if tb > 0 else None,
+    return {"launches": len(recs), "span_ms": max(r[3] for r in recs),
+            "sum_ms": {k: sum(r[3] - r[2] for r in recs if r[0] == k) for k in "ABC"},
+            "stage_b_overlapped_frac": tb_hidden / tb if tb > 0 else None}, recs
+
+
+def timeline(torch, tdma, w, x, args, batch, rank):
+    """Stream-overlap timeline of a stage pipeline (Alg. 2): how much of stage B's time runs while a
+    stage A or C kernel of another batch is running.  Plain stream launches (no graph)."""
+    ns = args.nstreams or 2
+    var = tdma.TDMA_VARIANT_STAGED if args.variant == "staged" else tdma.TDMA_VARIANT_PIPELINED
+    stats, recs = timeline_overlap(torch, tdma, w, x, var, batch, ns, max(3, args.warmup))
+    rec = {"timeline": True, "workload": args.workload, "variant": "staged" if var == tdma.TDMA_VARIANT_STAGED else "pipelined",
+           "batch": batch, "nstreams": ns, **stats,
            "note": "events bracket each launch on its stream: an interval includes the time the kernel "
                    "waits for SM slots, so overlapped_frac is an upper bound of true co-execution"}
     if rank == 0:
