@@ -82,6 +82,8 @@ struct TmaFusedParams {
     // STAGED variant (kStage 1 / 2, tdma_staged.cu): reduced system of the batch in HBM, [2 Pe][Lb]
     // doubles, line fastest, unit diagonal; lp = tree levels run inside the CTA (the nodes of that
     // level are the partitions whose boundary equations are exchanged), lp_shift = log2(leaves per node)
+    int pair = 0;       // 1: a cluster takes two ADJACENT x tiles one after the other (64-byte row segments:
+                        // the pair shares 128-byte lines, fetched whole by the first tile's copies)
     double *red_a = nullptr, *red_c = nullptr, *red_d = nullptr;
     const double *red_y = nullptr;
     long long Lb = 0;
@@ -863,8 +865,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     // TMA copies of one raw array, by the lanes of the last warp
     const int issue_lane = t - ((int)blockDim.x - 32 > 0 ? (int)blockDim.x - 32 : 0);   // >= 0: issuing warp
     const uint32_t arr_bytes = (uint32_t)(arr * sizeof(double));
+    // the cluster's q-th tile
+    auto tile_of = [&](int q) { return prm.pair ? (((q >> 1) * NC + g) << 1) + (q & 1) : g + q * NC; };
     auto issue_array = [&](int n) {
-        const int tile = g + (n >> 2) * NC, j = n & 3;
+        const int tile = tile_of(n >> 2), j = n & 3;
         if (tile >= prm.ntiles) return;
         const int s = n % NA;
         const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
@@ -936,7 +940,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     const int crit_threads = helper_mode ? cw * 32 : tree_threads;
     const bool crit = tree && leaf < help0, helper = tree && !crit;
     int it = 0, sn = 0, pn = 0;
-    for (int tile = g; tile < prm.ntiles; tile += NC, ++it) {
+    for (int tile = tile_of(0); tile < prm.ntiles; tile = tile_of(++it)) {
         const int par = it & 1;
         NodeBuf tb = tb0;                                      // this tile's inbox
         tb.ab += (uint32_t)par * inbox_bytes;
@@ -989,7 +993,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
         __syncthreads();                // raw slots consumed, leaf equations visible
         if (issue_lane >= 0) {
             for (int j = 0; j < 4; ++j) issue_array(n0 + NA + j);     // refill the four slots
-            if (kStage != 1 && it > 0) store_x(tile - NC);             // x of the previous tile
+            if (kStage != 1 && it > 0) store_x(tile_of(it - 1));       // x of the previous tile
         }
         if (kCluster && it == 0) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 
@@ -1136,7 +1140,7 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     if (kStage != 1 && it > 0) {
         __syncthreads();
         if (issue_lane >= 0) {
-            store_x(g + (it - 1) * NC);
+            store_x(tile_of(it - 1));
             asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
         }
     }
@@ -1262,7 +1266,7 @@ inline tdma_encode_tiled_fn get_encode_tiled()
 // y sweep: tensor (nx, rows, slices), box (TX, box_rows, 1); z sweep: tensor (nx, slices, rows),
 // box (TX, 1, box_rows) -- either way the box lands in shared memory as [box_rows][TX].
 inline bool make_slab_tensor_map(CUtensorMap *tm, const void *base, int nx, int nrows, int nslices,
-                                 long long rs, long long os, bool axis_z, int TX, int box_rows)
+                                 long long rs, long long os, bool axis_z, int TX, int box_rows, bool pair = false)
 {
     tdma_encode_tiled_fn enc = get_encode_tiled();
     if (!enc) return false;
@@ -1272,7 +1276,7 @@ inline bool make_slab_tensor_map(CUtensorMap *tm, const void *base, int nx, int 
     cuuint32_t estr[3] = {1, 1, 1};
     const size_t inner = (size_t)TX * sizeof(double);   // one L2 request per row segment, no over-fetch
     const CUtensorMapL2promotion promo = inner >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B
-                                       : inner >= 128 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                                       : (inner >= 128 || pair) ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
                                                       : CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
     return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<void *>(base), gdim, gstr, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
@@ -1376,9 +1380,12 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
 {
     CUtensorMap tm[5];
     const void *ptr[5] = {a, b, c, d, x};
+    const int xtiles = (nx + cfg.lines - 1) / cfg.lines;
+    // 64-byte row segments: neighbouring x tiles share 128-byte lines -> a cluster takes them in pairs
+    const bool pair = !cfg.xaxis && cfg.lines * sizeof(double) < 128 && xtiles % 2 == 0;
     for (int i = 0; i < 5 && nzs > 0; ++i) {
         if (cfg.xaxis ? !make_xsweep_tensor_map(&tm[i], ptr[i], ny, nx, nzs, cfg.lines, cfg.leaves)
-                      : !make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows))
+                      : !make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows, pair))
             return cudaErrorInvalidValue;
     }
     TmaFusedParams prm;
@@ -1386,8 +1393,9 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
     prm.x = x;
     prm.rs = rs; prm.os = os; prm.axis_z = axis_z ? 1 : 0; prm.periodic = periodic ? 1 : 0;
     prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves; prm.NS = cfg.slots;
-    prm.xtiles = (nx + cfg.lines - 1) / cfg.lines;
+    prm.xtiles = xtiles;
     prm.ntiles = prm.xtiles * nzs;
+    prm.pair = pair ? 1 : 0;
     prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
     const bool cl = cfg.cluster > 1;
     if (cfg.xaxis)

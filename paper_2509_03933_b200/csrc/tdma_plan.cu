@@ -306,9 +306,11 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
                 int fc = idle / pl->tfill.cluster;
                 if (fc > pl->tfill.max_clusters) fc = pl->tfill.max_clusters;
                 if (fc > 0) {
-                    // measured: an SM of the fill launch sustains about 0.55 of a main SM when its
-                    // tiling has 64-byte row segments (cfg 3: 8 lines per tile) and about as much as a
-                    // main SM with 128-byte segments (cfg 4 z sweeps: best share 0.11 = 16 / 148 SMs)
+                    // measured: with 64-byte row segments in the fill tiling (cfg 3: 8 lines per tile,
+                    // neighbouring x tiles taken in pairs) the step time is flat for shares of 8-12 of
+                    // 128 slices (6.97-7.04 ms); the smallest of them, weight 0.55, leaves the most to
+                    // the main launch.  With 128-byte segments a fill SM does as much as a main SM
+                    // (cfg 4 z sweeps: best share 0.11 = 16 / 148 SMs)
                     const double w = (pl->tfill.lines >= 16 ? 1.0 : 0.55) * fc * pl->tfill.cluster;
                     double share = pl->fill_opt > 0 ? pl->fill_opt * 1e-3 : w / (w + main_ctas);
                     nzf = (int)(bzn * share + 0.5);
