@@ -36,6 +36,7 @@ import torch
 __all__ = [
     "Workload", "CONFIGS", "config_spec", "make_workload", "uniform01", "normal01",
     "dominant_random", "poisson_wavenumber", "adi_toeplitz", "identity_system",
+    "SharedWorkload", "poisson_shared", "make_shared_workload",
 ]
 
 _MASK64 = (1 << 64) - 1

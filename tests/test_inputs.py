@@ -99,3 +99,27 @@ def test_identity_system():
     assert torch.all(a == 0) and torch.all(c == 0) and torch.all(b == 1)
     a, b, c, d = ti.identity_system(4, 8, 2, 0, diagonal_only=True)
     assert float(b.min()) >= 1 and float(b.max()) < 2
+
+
+def test_shared_form_of_the_poisson_configs():
+    """make_shared_workload: the 1-D arrays the materialised Poisson config is made of (f3).  a, c and
+    the real part of d are bit-identical to the materialised arrays; b agrees to rounding (the
+    shared form subtracts sx + sz in one step); slices of a taller slab carry the bits of the full one."""
+    import numpy as np
+    w = ti.make_workload("cfg2_poisson", nz=3, nx=16, ny=32)
+    for cplx in (False, True):
+        s = ti.make_shared_workload("cfg2_poisson", cplx, nz=3, nx=16, ny=32)
+        assert s.ncomp == (2 if cplx else 1) and s.pin00 and s.d.shape == (3, 32, 16)
+        assert torch.equal(s.a_y, w.a[1, :, 5]) and torch.equal(s.c_y, w.c[2, :, 7])
+        assert torch.equal(s.d.real if cplx else s.d, w.d)
+        b = s.b0_y.view(1, -1, 1) - (s.sx.view(1, 1, -1) + s.sz.view(-1, 1, 1))
+        b[0, 0, 0] = 1.0
+        assert torch.allclose(b, w.b, rtol=1e-14, atol=0)
+        assert s.d[0, 0, 0] == 0
+        if cplx:
+            assert float(s.d.imag.abs().max()) > 0 and not torch.equal(s.d.imag, s.d.real)
+    full = ti.make_shared_workload("cfg2_poisson", True, nz=6, nx=16, ny=32)
+    part = ti.make_shared_workload("cfg2_poisson", True, nz=2, nx=16, ny=32, k_offset=3)
+    assert torch.equal(part.d, full.d[3:5]) and torch.equal(part.sz, full.sz[3:5]) and not part.pin00
+    with pytest.raises(ValueError):
+        ti.make_shared_workload("cfg1_tiny", False)
