@@ -405,6 +405,8 @@ def main():
     ap.add_argument("--timeline", action="store_true",
                     help="S6 evidence without nsys: per-launch start/end of the PIPELINED stages of one solve "
                          "(CUDA events on the plan's streams), overlap statistics as one JSON line")
+    ap.add_argument("--yslab", type=int, default=0,
+                    help="NEXT row f4: time the rank-local stages of an N-rank y-slab job on this GPU (one JSON line)")
     ap.add_argument("--adi", action="store_true",
                     help="NEXT row f1 / BASELINE cfg 4: three successive FUSED solves along x (periodic), "
                          "y (Dirichlet) and z (periodic); use with --workload cfg4_adi_y")
@@ -450,6 +452,8 @@ def main():
         return sweep(torch, tdma, w, x, args, barrier, rank)
     if args.adi:
         return adi(torch, tdma, w, x, args, barrier, rank, peak)
+    if args.yslab:
+        return yslab(torch, tdma, w, args, rank, peak)
     if args.timeline:
         return timeline(torch, tdma, w, x, args, batch, rank)
 
@@ -685,6 +689,58 @@ def timeline(torch, tdma, w, x, args, batch, rank):
     if rank == 0:
         rec["first_launches"] = [{"stage": r[0], "batch": r[1], "start_ms": round(r[2], 4), "end_ms": round(r[3], 4)}
                                  for r in recs[:60]]
+        print(json.dumps(rec))
+    return 0
+
+
+def yslab(torch, tdma, w, args, rank, peak):
+    """SURVEY 8(f) f4, what ONE B200 can measure of it: the rank-local stages of the y-slab
+    decomposition (tdma_slab_stage_a / _b / _c) for one interior rank of an --yslab N job whose
+    global slab is the workload (rank-local slab: nx x ny/N x nz), timed stage by stage, plus the
+    per-batch exchange sizes and what they would take at the profiling guide's 770 GB/s peer-copy
+    rate.  The all-to-alls themselves are NOT measured (one GPU): the record says so."""
+    from paper_2509_03933_b200.yslab import CudaSlabStages
+    n, r = args.yslab, args.yslab // 2
+    nyl = w.ny // n
+    batch = 32 if args.batch < 0 else args.batch
+    loc = [t[:, r * nyl:(r + 1) * nyl, :].contiguous() for t in (w.a, w.b, w.c, w.d)]
+    x = torch.empty_like(loc[3])
+    st = CudaSlabStages(w.nx, nyl, w.nz, 1, batch, r, n)
+    lb, ls = st.batch_lines(0)
+    send = torch.zeros((n, 1, 6, ls), dtype=torch.float64, device=loc[0].device)
+    yout = torch.zeros((n, 2, ls), dtype=torch.float64, device=loc[0].device)
+    stream = torch.cuda.current_stream()
+    nbf = w.nz // st.bz                                  # full batches only
+    def timed(fn):
+        for q in range(min(nbf, 3)):
+            fn(q)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            for q in range(nbf):
+                fn(q)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / (args.steps * nbf)
+    t_a = timed(lambda q: st.stage_a(q, *loc, send, stream))
+    # a stand-in for the exchange, so that stage B sees a consistent system: every source rank
+    # contributes this rank's rows for the receiver's share of the lines
+    recv = send[r].unsqueeze(0).expand(n, 1, 6, ls).contiguous()
+    t_b = timed(lambda q: st.stage_b(q, recv, yout, stream))
+    yrecv = yout[r].unsqueeze(0).expand(n, 2, ls).contiguous()
+    t_c = timed(lambda q: st.stage_c(q, yrecv, x, stream))
+    st.close()
+    cells = w.nx * nyl * st.bz
+    out_b, back_b = 48 * lb, 16 * lb
+    rec = {"yslab": True, "workload": args.workload, "nranks": n, "rank_timed": r, "nx": w.nx, "ny_local": nyl, "nz": w.nz,
+           "batch": st.bz, "stage_ms_per_batch": {"A": t_a, "B": t_b, "C": t_c},
+           "stage_gbs": {"A": 56.0 * cells / t_a / 1e6, "C": 32.0 * cells / t_c / 1e6},
+           "exchange_bytes_per_batch": {"A2B": out_b, "B2C": back_b},
+           "exchange_ms_at_770GBs": {"A2B": out_b / 770e6, "B2C": back_b / 770e6},
+           "rank_cells_per_s_if_exchange_hidden": w.nx * nyl * w.nz / ((t_a + t_c) * (w.nz / st.bz) * 1e-3),
+           "measured": "rank-local stages on one B200; the two all-to-alls per batch are unmeasured (one GPU)"}
+    if rank == 0:
         print(json.dumps(rec))
     return 0
 
