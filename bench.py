@@ -706,9 +706,10 @@ def yslab(torch, tdma, w, args, rank, peak):
     loc = [t[:, r * nyl:(r + 1) * nyl, :].contiguous() for t in (w.a, w.b, w.c, w.d)]
     x = torch.empty_like(loc[3])
     st = CudaSlabStages(w.nx, nyl, w.nz, 1, batch, r, n)
+    tma, pl = st.tma, st.P
     lb, ls = st.batch_lines(0)
-    send = torch.zeros((n, 1, 6, ls), dtype=torch.float64, device=loc[0].device)
-    yout = torch.zeros((n, 2, ls), dtype=torch.float64, device=loc[0].device)
+    send = torch.zeros((n, pl, 6, ls), dtype=torch.float64, device=loc[0].device)
+    yout = torch.zeros((n, 2 * pl, ls), dtype=torch.float64, device=loc[0].device)
     stream = torch.cuda.current_stream()
     nbf = w.nz // st.bz                                  # full batches only
     def timed(fn):
@@ -726,16 +727,18 @@ def yslab(torch, tdma, w, args, rank, peak):
     t_a = timed(lambda q: st.stage_a(q, *loc, send, stream))
     # a stand-in for the exchange, so that stage B sees a consistent system: every source rank
     # contributes this rank's rows for the receiver's share of the lines
-    recv = send[r].unsqueeze(0).expand(n, 1, 6, ls).contiguous()
+    recv = send[r].unsqueeze(0).expand(n, pl, 6, ls).contiguous()
     t_b = timed(lambda q: st.stage_b(q, recv, yout, stream))
-    yrecv = yout[r].unsqueeze(0).expand(n, 2, ls).contiguous()
+    yrecv = yout[r].unsqueeze(0).expand(n, 2 * pl, ls).contiguous()
     t_c = timed(lambda q: st.stage_c(q, yrecv, x, stream))
     st.close()
     cells = w.nx * nyl * st.bz
-    out_b, back_b = 48 * lb, 16 * lb
+    out_b, back_b = 48 * pl * lb, 16 * pl * lb
     rec = {"yslab": True, "workload": args.workload, "nranks": n, "rank_timed": r, "nx": w.nx, "ny_local": nyl, "nz": w.nz,
            "batch": st.bz, "stage_ms_per_batch": {"A": t_a, "B": t_b, "C": t_c},
-           "stage_gbs": {"A": 56.0 * cells / t_a / 1e6, "C": 32.0 * cells / t_c / 1e6},
+           "stage_kernels": "tma-staged (stage A 32 B/cell, stage C 40 B/cell, nothing spilled)" if tma else
+                            "one thread per (line, partition) (stage A 56 B/cell, stage C 32 B/cell, a', c', d' through HBM)",
+           "stage_gbs": {"A": (32.0 if tma else 56.0) * cells / t_a / 1e6, "C": (40.0 if tma else 32.0) * cells / t_c / 1e6},
            "exchange_bytes_per_batch": {"A2B": out_b, "B2C": back_b},
            "exchange_ms_at_770GBs": {"A2B": out_b / 770e6, "B2C": back_b / 770e6},
            "rank_cells_per_s_if_exchange_hidden": w.nx * nyl * w.nz / ((t_a + t_c) * (w.nz / st.bz) * 1e-3),

@@ -289,13 +289,21 @@ int tdma_plan_autotune(int nx, int ny, int nz, int P, int dtype, int nstreams, c
  * Ls is that of the batch (the last batch of nz % batch slices is shorter).  a, b, c, d, x: DEVICE
  * pointers to the rank's slab, nx*ny_local*nz doubles, element (i,j,k) at i + nx*(j + ny_local*k);
  * a at the global row 0 (rank 0) and c at the global last row (rank nranks-1) are ignored.
+ * When the slab tiles for the TMA kernel (even nx, 16-byte aligned arrays, ny_local = CTAs x 2^k
+ * leaves), stage A and stage C are the TMA-staged kernels of TDMA_VARIANT_STAGED: nothing is spilled,
+ * stage C fetches a, b, c, d of the batch AGAIN (the pointers stage A of that batch was given: they
+ * must still be valid and unchanged), and the exchanged level of the recursion -- P in the layouts
+ * above -- is tdma_slab_get(TDMA_SLAB_PLOCAL), which may differ from the P_local asked for
+ * (D1).  Otherwise the one-thread-per-(line, partition) kernels of PIPELINED are used.
  * tdma_slab_create returns NULL on invalid arguments (ny_local % P_local != 0, fewer than 2 rows per
  * partition, nx*batch or nx*(nz % batch) not divisible by nranks), without a CUDA device, or when
  * the scratch ring (3 batches of a', c', d' + reduced buffers) cannot be allocated.  Enqueue-only. */
 typedef struct tdma_slab tdma_slab;
 typedef enum tdma_slab_query {
     TDMA_SLAB_NB = 0, TDMA_SLAB_BATCH = 1, TDMA_SLAB_LINES = 2 /* Lb of a full batch */,
-    TDMA_SLAB_SHARE = 3 /* Ls of a full batch */, TDMA_SLAB_PTOT = 4
+    TDMA_SLAB_SHARE = 3 /* Ls of a full batch */, TDMA_SLAB_PTOT = 4,
+    TDMA_SLAB_PLOCAL = 5 /* partitions per rank actually exchanged: size the buffers with THIS P */,
+    TDMA_SLAB_TMA = 6    /* 1: stage A / C are the TMA-staged kernels (72 B/cell, no scratch ring) */
 } tdma_slab_query;
 tdma_slab *tdma_slab_create(int nx, int ny_local, int nz, int P_local, int batch, int rank, int nranks);
 int tdma_slab_get(const tdma_slab *slab, int what);

@@ -38,7 +38,8 @@ EXPORTED_SYMBOLS = (
     "tdma_slab_create", "tdma_slab_get", "tdma_slab_stage_a", "tdma_slab_stage_b", "tdma_slab_stage_b_pdd", "tdma_slab_stage_c",
     "tdma_slab_destroy",
 )
-TDMA_SLAB_NB, TDMA_SLAB_BATCH, TDMA_SLAB_LINES, TDMA_SLAB_SHARE, TDMA_SLAB_PTOT = range(5)
+(TDMA_SLAB_NB, TDMA_SLAB_BATCH, TDMA_SLAB_LINES, TDMA_SLAB_SHARE, TDMA_SLAB_PTOT, TDMA_SLAB_PLOCAL,
+ TDMA_SLAB_TMA) = range(7)
 
 
 class tdma_options(ctypes.Structure):

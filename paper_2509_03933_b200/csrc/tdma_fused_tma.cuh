@@ -88,6 +88,12 @@ struct TmaFusedParams {
     const double *red_y = nullptr;
     long long Lb = 0;
     int lp = 0, lp_shift = 0;
+    // y-slab decomposition (tdma_slab.cu): this launch holds rows row0 .. row0 + ny - 1 of lines of
+    // ny_total rows (0: the launch holds whole lines); Ls > 0: the reduced rows go to / the boundary
+    // unknowns come from the all-to-all buffers send[dest][Pl][6][Ls] (red_a) / yrecv[src][2 Pl][Ls]
+    // (red_y), dest = src = line / Ls, Pl = exchanged partitions of this rank
+    int row0 = 0, ny_total = 0, Pl = 0;
+    long long Ls = 0;
 };
 
 // Dynamic shared memory of one CTA: NA ring slots of one raw array [R][TX] each, the x staging
@@ -903,8 +909,10 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
     if (issue_lane >= 0) for (int n = 0; n < NA; ++n) issue_array(n);
 
     const int lx = t % TX, leaf = t / TX;
-    const bool first_leaf = !prm.periodic && (y0 + leaf * M0 == 0);
-    const bool last_leaf = !prm.periodic && (y0 + leaf * M0 + M0 == prm.ny);
+    const int ny_line = (kStage != 0 && prm.ny_total > 0) ? prm.ny_total : prm.ny;      // rows of the whole line
+    const int row_g = (kStage != 0 ? prm.row0 : 0) + y0 + leaf * M0;                     // global row of the leaf
+    const bool first_leaf = !prm.periodic && row_g == 0;
+    const bool last_leaf = !prm.periodic && row_g + M0 == ny_line;
     const int o0 = leaf * M0 * TX + lx;
     // levels above the leaves: 4-ary merges (2-ary when the node count is not a multiple of 4)
     // level l merges k = 2^lkb nodes of S = 2 << cum rows (cum = sum of the lkb below); packed into
@@ -968,8 +976,14 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
             if (xt_ * TX + lx < prm.nx) red_l = (long long)k_ * prm.nx + xt_ * TX + lx;
             if (kStage == 2 && act && red_l >= 0) {
                 const long long pg = (long long)crank * (W >> prm.lp_shift) + (leaf >> prm.lp_shift);
-                y_first = __ldcg(prm.red_y + 2 * pg * prm.Lb + red_l);
-                y_last = __ldcg(prm.red_y + (2 * pg + 1) * prm.Lb + red_l);
+                if (prm.Ls > 0) {       // y-slab: yrecv[src][2 Pl][Ls]
+                    const long long src = red_l / prm.Ls, j = red_l - src * prm.Ls;
+                    const double *yp = prm.red_y + ((src * 2 * prm.Pl + 2 * pg) * prm.Ls + j);
+                    y_first = __ldcg(yp); y_last = __ldcg(yp + prm.Ls);
+                } else {
+                    y_first = __ldcg(prm.red_y + 2 * pg * prm.Lb + red_l);
+                    y_last = __ldcg(prm.red_y + (2 * pg + 1) * prm.Lb + red_l);
+                }
             }
         }
 #pragma unroll
@@ -1098,9 +1112,16 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                 const uint32_t oF = nb_ab<TX>(nb, leaf * S, lx), oL = nb_ab<TX>(nb, leaf * S + S - 1, lx);
                 const double2 abf = lds2(oF), cdf = lds2(oF + nb.plane), abl = lds2(oL), cdl = lds2(oL + nb.plane);
                 const double invf = 1.0 / abf.y, invl = 1.0 / abl.y;
-                const long long q0 = 2 * pg * prm.Lb + red_l, q1 = q0 + prm.Lb;
-                __stcg(prm.red_a + q0, abf.x * invf); __stcg(prm.red_c + q0, cdf.x * invf); __stcg(prm.red_d + q0, cdf.y * invf);
-                __stcg(prm.red_a + q1, abl.x * invl); __stcg(prm.red_c + q1, cdl.x * invl); __stcg(prm.red_d + q1, cdl.y * invl);
+                if (prm.Ls > 0) {       // y-slab: send[dest][Pl][6][Ls] = (fa, fc, fd | pa, pc, pd)
+                    const long long dest = red_l / prm.Ls, j = red_l - dest * prm.Ls;
+                    double *sp = prm.red_a + ((dest * prm.Pl + pg) * 6 * prm.Ls + j);
+                    __stcg(sp, abf.x * invf); __stcg(sp + prm.Ls, cdf.x * invf); __stcg(sp + 2 * prm.Ls, cdf.y * invf);
+                    __stcg(sp + 3 * prm.Ls, abl.x * invl); __stcg(sp + 4 * prm.Ls, cdl.x * invl); __stcg(sp + 5 * prm.Ls, cdl.y * invl);
+                } else {
+                    const long long q0 = 2 * pg * prm.Lb + red_l, q1 = q0 + prm.Lb;
+                    __stcg(prm.red_a + q0, abf.x * invf); __stcg(prm.red_c + q0, cdf.x * invf); __stcg(prm.red_d + q0, cdf.y * invf);
+                    __stcg(prm.red_a + q1, abl.x * invl); __stcg(prm.red_c + q1, cdl.x * invl); __stcg(prm.red_d + q1, cdl.y * invl);
+                }
             }
             __syncthreads();            // the node rows are read before the next sweep rewrites them
             continue;

@@ -20,10 +20,12 @@
 
 #include <cuda_runtime.h>
 
+#include <cstdint>
 #include <cstdio>
 #include <new>
 
 #include "tdma_stage_kernels.cuh"
+#include "tdma_staged.h"
 
 namespace {
 constexpr int kU = 4;
@@ -33,7 +35,12 @@ constexpr int kSlabDepth = 3;   // batches in flight: A(n), B(n-1), C(n-2)  (PAP
 struct tdma_slab {
     int nx = 0, ny = 0, nz = 0, P = 0, m = 0, rank = 0, nranks = 0, bz = 0, nb = 0;
     long long Lb = 0, Ls = 0;
-    double *scratch = nullptr;   // depth x {a', c', d'} x [bz][ny][nx]
+    // stage A / C: the TMA-staged kernels of the STAGED variant (nothing spilled, stage C re-reads the
+    // inputs stage A was given) when the slab tiles; else the one-thread-per-(line, partition) kernels
+    bool tma = false;
+    tdma::StagedConfig staged;
+    const double *in[kSlabDepth][4] = {};   // a, b, c, d of the batch in each ring slot (tma: for stage C)
+    double *scratch = nullptr;   // depth x {a', c', d'} x [bz][ny][nx]   (not with tma)
     double *red = nullptr;       // depth x {RA, RC, RD, CP} x [2 Ptot][Ls]
     size_t workspace = 0;
 };
@@ -93,9 +100,21 @@ tdma_slab *tdma_slab_create(int nx, int ny_local, int nz, int P_local, int batch
     s->nx = nx; s->ny = ny_local; s->nz = nz; s->P = P_local; s->m = ny_local / P_local;
     s->rank = rank; s->nranks = nranks; s->bz = bz; s->nb = (nz + bz - 1) / bz;
     s->Lb = (long long)nx * bz; s->Ls = s->Lb / nranks;
-    const size_t sbytes = (size_t)kSlabDepth * 3 * bz * ny_local * nx * sizeof(double);
+    {
+        int dev = 0;
+        cudaDeviceProp prop;
+        const char *why = nullptr;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&prop, dev) == cudaSuccess && prop.major >= 10 &&
+            tdma::configure_staged(&s->staged, nx, ny_local, P_local, false, prop, &why)) {
+            s->tma = true;
+            s->P = s->staged.Pe;            // the exchanged level of the recursion (D1): >= 1 per CTA
+            s->m = ny_local / s->P;
+        }
+    }
+    P_local = s->P;
+    const size_t sbytes = s->tma ? 0 : (size_t)kSlabDepth * 3 * bz * ny_local * nx * sizeof(double);
     const size_t rbytes = (size_t)kSlabDepth * 4 * 2 * P_local * nranks * (size_t)s->Ls * sizeof(double);
-    if (cudaMalloc(&s->scratch, sbytes) != cudaSuccess || cudaMalloc(&s->red, rbytes) != cudaSuccess) {
+    if ((sbytes && cudaMalloc(&s->scratch, sbytes) != cudaSuccess) || cudaMalloc(&s->red, rbytes) != cudaSuccess) {
         cudaGetLastError();
         cudaFree(s->scratch); cudaFree(s->red);
         delete s;
@@ -114,6 +133,8 @@ int tdma_slab_get(const tdma_slab *s, int what)
     case TDMA_SLAB_LINES: return (int)s->Lb;
     case TDMA_SLAB_SHARE: return (int)s->Ls;
     case TDMA_SLAB_PTOT: return s->P * s->nranks;
+    case TDMA_SLAB_PLOCAL: return s->P;
+    case TDMA_SLAB_TMA: return s->tma ? 1 : 0;
     default: return TDMA_ERR_INVALID_ARG;
     }
 }
@@ -128,6 +149,14 @@ int tdma_slab_stage_a(tdma_slab *s, int batch_index, const void *a, const void *
     prm.a = (const double *)a + off; prm.b = (const double *)b + off;
     prm.c = (const double *)c + off; prm.d = (const double *)d + off;
     prm.send = (double *)send;
+    if (s->tma) {
+        if ((((uintptr_t)a | (uintptr_t)b | (uintptr_t)c | (uintptr_t)d) & 15) != 0) return TDMA_ERR_UNSUPPORTED;
+        const int slot = batch_index % kSlabDepth;
+        s->in[slot][0] = prm.a; s->in[slot][1] = prm.b; s->in[slot][2] = prm.c; s->in[slot][3] = prm.d;
+        cudaError_t e = tdma::launch_staged_slab(s->staged, 1, prm.a, prm.b, prm.c, prm.d, nullptr, prm.send, nullptr, s->nx,
+                                                 s->ny, bzn, s->rank * s->ny, s->ny * s->nranks, prm.Ls, (cudaStream_t)stream);
+        return e == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
+    }
     dim3 grid((unsigned)((prm.Lb + 127) / 128), s->P);
     tdma::stage_a_kernel<kU, tdma::kOutSlab><<<grid, 128, 0, (cudaStream_t)stream>>>(prm);
     return cudaGetLastError() == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
@@ -172,6 +201,14 @@ int tdma_slab_stage_c(tdma_slab *s, int batch_index, const void *yrecv, void *x,
     tdma::StageParams prm = slab_params(s, batch_index, k0, bzn);
     prm.x = (double *)x + (size_t)k0 * (size_t)prm.os;
     prm.y = (double *)const_cast<void *>(yrecv);
+    if (s->tma) {
+        const int slot = batch_index % kSlabDepth;
+        if (!s->in[slot][0] || ((uintptr_t)x & 15) != 0) return TDMA_ERR_INVALID_ARG;     // stage A of this batch first
+        cudaError_t e = tdma::launch_staged_slab(s->staged, 2, s->in[slot][0], s->in[slot][1], s->in[slot][2], s->in[slot][3],
+                                                 prm.x, nullptr, prm.y, s->nx, s->ny, bzn, s->rank * s->ny,
+                                                 s->ny * s->nranks, prm.Ls, (cudaStream_t)stream);
+        return e == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
+    }
     dim3 grid((unsigned)((prm.Lb + 127) / 128), s->P);
     tdma::stage_c_kernel<kU, true><<<grid, 128, 0, (cudaStream_t)stream>>>(prm);
     return cudaGetLastError() == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
@@ -182,6 +219,7 @@ int tdma_slab_destroy(tdma_slab *s)
     if (!s) return TDMA_ERR_INVALID_ARG;
     cudaError_t e = cudaDeviceSynchronize();
     cudaFree(s->scratch); cudaFree(s->red);
+    if (s->staged.impl) tdma::free_staged(&s->staged);
     delete s;
     return e == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
 }

@@ -54,14 +54,15 @@ static cudaError_t launch_staged_tx(TmaFusedConfig &t, const CUtensorMap *tm, co
     }
 }
 
-cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
-                          const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
-                          int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st)
+static cudaError_t launch_staged_any(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
+                                     const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
+                                     int nx, int ny, int nzs, long long rs, long long os, bool axis_z, int row0,
+                                     int ny_total, long long Ls, cudaStream_t st)
 {
     if (stage != 1 && stage != 2) return cudaErrorInvalidValue;
     TmaFusedConfig &t = static_cast<TmaFusedConfig *>(cfg.impl)[stage - 1];
     CUtensorMap tm[5];
-    const void *ptr[5] = {a, b, c, d, x};
+    const void *ptr[5] = {a, b, c, d, x ? (const void *)x : (const void *)d};   // stage A never touches x
     for (int i = 0; i < 5 && nzs > 0; ++i)
         if (!make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, t.lines, t.box_rows)) return cudaErrorInvalidValue;
     TmaFusedParams prm;
@@ -75,6 +76,7 @@ cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const d
     prm.red_a = ra; prm.red_c = rc; prm.red_d = rd; prm.red_y = y;
     prm.Lb = (long long)nx * nzs;
     prm.lp = cfg.lp; prm.lp_shift = cfg.lp_shift;
+    prm.row0 = row0; prm.ny_total = ny_total; prm.Ls = Ls; prm.Pl = cfg.Pe;
     cudaError_t e;
     if (stage == 1) {
         switch (t.lines) {
@@ -92,6 +94,21 @@ cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const d
         }
     }
     return e;
+}
+
+cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
+                          const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
+                          int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st)
+{
+    return launch_staged_any(cfg, stage, a, b, c, d, x, ra, rc, rd, y, nx, ny, nzs, rs, os, axis_z, 0, 0, 0, st);
+}
+
+cudaError_t launch_staged_slab(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
+                               const double *d, double *x, double *send, const double *yrecv, int nx, int ny,
+                               int nzs, int row0, int ny_total, long long Ls, cudaStream_t st)
+{
+    return launch_staged_any(cfg, stage, a, b, c, d, x, send, nullptr, nullptr, yrecv, nx, ny, nzs, (long long)nx,
+                             (long long)nx * ny, false, row0, ny_total, Ls, st);
 }
 
 }  // namespace tdma

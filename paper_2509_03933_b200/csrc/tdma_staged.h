@@ -25,4 +25,10 @@ cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const d
                           const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
                           int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st);
 
+// y-slab decomposition (tdma_slab.cu): the launch holds rows row0 .. row0 + ny - 1 of lines of ny_total
+// rows; stage 1 writes send[dest][Pe][6][Ls], stage 2 reads yrecv[src][2 Pe][Ls] (Ls = nx * nzs / ranks).
+cudaError_t launch_staged_slab(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
+                               const double *d, double *x, double *send, const double *yrecv, int nx, int ny,
+                               int nzs, int row0, int ny_total, long long Ls, cudaStream_t st);
+
 }  // namespace tdma

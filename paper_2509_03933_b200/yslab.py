@@ -40,6 +40,8 @@ class CudaSlabStages:
         self.pdd = pdd      # stage B = PDD: 2 x 2 interface systems, an approximation
         self.nx, self.ny, self.nz, self.P, self.rank, self.nranks = nx, ny_local, nz, P_local, rank, nranks
         self.handle = _b.tdma_slab_create(nx, ny_local, nz, P_local, batch, rank, nranks)
+        self.P = _b.tdma_slab_get(self.handle, _b.TDMA_SLAB_PLOCAL)     # the partitions actually exchanged
+        self.tma = bool(_b.tdma_slab_get(self.handle, _b.TDMA_SLAB_TMA))
         self.nb = _b.tdma_slab_get(self.handle, _b.TDMA_SLAB_NB)
         self.bz = _b.tdma_slab_get(self.handle, _b.TDMA_SLAB_BATCH)
         self.device = torch.device("cuda", torch.cuda.current_device())
@@ -79,7 +81,7 @@ class YSlabSolver:
         self.nranks = self.dist.get_world_size(group) if self.dist else 1
         self.stages = stages if stages is not None else CudaSlabStages(nx, ny_local, nz, P_local, batch,
                                                                        self.rank, self.nranks, pdd=pdd)
-        self.P = P_local
+        self.P = P_local = getattr(self.stages, "P", P_local)
         self.device = self.stages.device
         self.cuda = self.device.type == "cuda"
         lb, ls = self.stages.batch_lines(0)

@@ -23,13 +23,17 @@ def dev():
     return torch.device("cuda:0")
 
 
-def emulate(a, b, c, d, nranks, P_local, batch, keep=None, pdd=False):
+def emulate(a, b, c, d, nranks, P_local, batch, keep=None, pdd=False, info=None):
     """All ranks' stages in sequence; returns x of the undivided slab."""
     nz, ny, nx = a.shape
     nyl = ny // nranks
     loc = [[t[:, r * nyl:(r + 1) * nyl, :].contiguous() for t in (a, b, c, d)] for r in range(nranks)]
     xs = [torch.full_like(loc[r][3], float("nan")) for r in range(nranks)]
     st = [CudaSlabStages(nx, nyl, nz, P_local, batch, r, nranks, pdd=pdd) for r in range(nranks)]
+    P_local = st[0].P                   # the partitions per rank actually exchanged (TMA stages: the tiling's)
+    assert all(s.P == P_local for s in st)
+    if info is not None:
+        info.update(P=P_local, tma=st[0].tma)
     try:
         for n in range(st[0].nb):
             lb, ls = st[0].batch_lines(n)
@@ -45,7 +49,7 @@ def emulate(a, b, c, d, nranks, P_local, batch, keep=None, pdd=False):
                 st[r].stage_c(n, yrecv[r], xs[r])
             torch.cuda.synchronize()
             if keep is not None:
-                keep.append((n, send.cpu().numpy(), yout.cpu().numpy()))
+                keep.append((n, send.cpu().numpy(), yout.cpu().numpy(), P_local))
     finally:
         for s in st:
             s.close()
@@ -77,9 +81,24 @@ def test_pdd_over_emulated_ranks(nranks, P_local):
     strictly dominant system -- agreement with the exact solve far below the tolerance."""
     nx, ny, nz = 32, 256, 4
     a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 53, dev())
-    x = emulate(a, b, c, d, nranks, P_local, 2, pdd=True)
+    info = {}
+    x = emulate(a, b, c, d, nranks, P_local, 2, pdd=True, info=info)
     an, bn, cn, dn, xn = [t.cpu().numpy() for t in (a, b, c, d, x)]
-    assert oracle.normwise_error(xn, oracle.solve_y_pdd(an, bn, cn, dn, nranks * P_local)).max() <= TOL_E
+    assert oracle.normwise_error(xn, oracle.solve_y_pdd(an, bn, cn, dn, nranks * info["P"])).max() <= TOL_E
+    assert oracle.normwise_error(xn, oracle.solve_y(an, bn, cn, dn)).max() <= TOL_E
+
+
+@pytest.mark.parametrize("nx,ny,want_tma", [(64, 256, True), (64, 1024, True), (63, 256, False), (64, 120, False)])
+def test_tma_staged_stages_are_used_when_the_slab_tiles(nx, ny, want_tma):
+    """4 ranks: slabs of 64 / 256 rows tile for the TMA kernel (stage A / C staged on chip, no scratch
+    ring); odd nx or 30 rows per rank fall back to the one-thread-per-(line, partition) kernels.  Same
+    result either way."""
+    nz = 4
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 59, dev())
+    info = {}
+    x = emulate(a, b, c, d, 4, 2, 4, info=info)
+    assert info["tma"] == want_tma
+    an, bn, cn, dn, xn = [t.cpu().numpy() for t in (a, b, c, d, x)]
     assert oracle.normwise_error(xn, oracle.solve_y(an, bn, cn, dn)).max() <= TOL_E
 
 
@@ -92,9 +111,9 @@ def test_exchange_buffers_hold_the_schur_complement_rows():
     emulate(a, b, c, d, nranks, P_local, 2, keep)
     an, bn, cn, dn = [t.cpu().numpy() for t in (a, b, c, d)]
     ref = oracle.solve_y(an, bn, cn, dn)
-    nyl, m = ny // nranks, ny // nranks // P_local
     bz = 2
-    for n, send, yout in keep:
+    for n, send, yout, P_local in keep:
+        m = ny // nranks // P_local
         ls = send.shape[-1]
         lb = ls * nranks
         for l in range(0, lb, 5):
