@@ -23,6 +23,11 @@
  * and joins them back, so work enqueued later on `stream` sees x.  No host synchronisation
  * inside.  One solve in flight per plan; concurrent solves need separate plans.
  *
+ * ALSO HERE, each documented at its declaration: tdma_solve_shared (1-D coefficient arrays, real or
+ * complex right-hand sides: the form the paper benchmarks), the tdma_slab_* calls (rank-local stages
+ * of the multi-GPU y-slab decomposition), stage-isolated launches, the batch-size optimiser, the
+ * stream timeline and an fp64 ALU probe.
+ *
  * ERRORS.  tdma_plan_create* return NULL on failure; the int-returning calls return TDMA_OK (0)
  * or a negative tdma_status; a message for the calling thread is in tdma_last_error().
  * There is no CPU fallback: without a CUDA device every compute call fails with TDMA_ERR_CUDA.

@@ -2,8 +2,8 @@
 
 Same names as the C entry points: ``tdma_plan_create``, ``tdma_plan_create_ex``, ``tdma_solve``,
 ``tdma_solve_host``, ``tdma_stage``, ``tdma_plan_get``, ``tdma_plan_workspace_bytes``,
-``tdma_plan_buffer``, ``tdma_plan_destroy``, ``tdma_last_error``, ``tdma_version`` -- plus a small
-``Plan`` convenience class.  Every step of the path runs inside ``libtdma.so``'s kernels; PyTorch
+``tdma_plan_buffer``, ``tdma_plan_destroy``, ``tdma_last_error``, ``tdma_version``, ``tdma_solve_shared``,
+``tdma_slab_*``, ``tdma_probe_fp64``, ... (``EXPORTED_SYMBOLS``) -- plus a small ``Plan`` convenience class.  Every step of the path runs inside ``libtdma.so``'s kernels; PyTorch
 is used by callers only for device memory and streams.  There is no CPU fallback: if the shared
 library is missing (and cannot be built) importing a compute entry point raises.
 """
