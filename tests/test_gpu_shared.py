@@ -191,3 +191,34 @@ def test_fill_launch_is_repeatable(cplx):
         assert info["fill"] > 0
         E = oracle.normwise_error(as_lines(x.cpu().numpy()), ref).max()
         assert E <= TOL_E, "solve %d: normwise error %.3e (fill %d)" % (rep, E, info["fill"])
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+def test_cfg3_shared_full_size_sampled(cplx):
+    """The launch configuration bench.py times for the shared-coefficient workloads: cfg 3 at FULL
+    size (1024^3 cells, complex: 2 x 16 GiB), one persistent launch (plus the fill launch where the
+    tiling has one), sampled z-slices against the long-double reference slice by slice."""
+    free, _ = torch.cuda.mem_get_info()
+    need = 1024 ** 3 * 8 * (2 if cplx else 1) * 2 * 1.15
+    if free < need:
+        pytest.skip("needs %.0f GB of device memory" % (need / 1e9))
+    dv = dev()
+    w = tdma_inputs.make_shared_workload("cfg3_weak", cplx, device=dv)
+    x = torch.full_like(w.d, float("nan"))
+    with tdma.Plan(w.nx, w.ny, w.nz, 1, 0) as plan:
+        plan.solve_shared(w.a_y, w.b0_y, w.c_y, w.sx, w.sz, w.d, x, pin00=True)
+        torch.cuda.synchronize()
+        fill = plan.get(tdma.TDMA_GET_SHARED_FILL)
+    picks = {0, 1, 511, 777, w.nz - 1}
+    if fill > 0:
+        picks |= {w.nz - fill - 1, w.nz - fill, w.nz - fill // 2 - 1}
+    host = [t.cpu().numpy() for t in (w.a_y, w.b0_y, w.c_y, w.sx)]
+    for k in sorted(picks):
+        ref = oracle.solve_y_shared(*host, w.sz[k:k + 1].cpu().numpy(), w.d[k:k + 1].cpu().numpy(),
+                                    pin00=(k == 0), precision="ld")
+        xk = x[k:k + 1].cpu().numpy()
+        assert np.isfinite(as_lines(xk)).all()
+        E = oracle.normwise_error(as_lines(xk), as_lines(ref)).max()
+        assert E <= TOL_E, "slice %d: normwise error %.3e" % (k, E)
+    del w, x
+    torch.cuda.empty_cache()
