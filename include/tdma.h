@@ -300,6 +300,8 @@ int tdma_plan_autotune(int nx, int ny, int nz, int P, int dtype, int nstreams, c
  * must still be valid and unchanged), and the exchanged level of the recursion -- P in the layouts
  * above -- is tdma_slab_get(TDMA_SLAB_PLOCAL), which may differ from the P_local asked for
  * (D1).  Otherwise the one-thread-per-(line, partition) kernels of PIPELINED are used.
+ * Either way the slab keeps a ring of 3 batches: stage C of batch n must be enqueued before stage A
+ * of batch n + 3 (Alg. 2's order A(n), B(n-1), C(n-2) does that).
  * tdma_slab_create returns NULL on invalid arguments (ny_local % P_local != 0, fewer than 2 rows per
  * partition, nx*batch or nx*(nz % batch) not divisible by nranks), without a CUDA device, or when
  * the scratch ring (3 batches of a', c', d' + reduced buffers) cannot be allocated.  Enqueue-only. */

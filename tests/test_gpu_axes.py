@@ -34,8 +34,8 @@ def check(a, b, c, d, x, axis, periodic):
     assert err.max() <= TOL_E, err.max()
 
 
-@pytest.mark.parametrize("opts", [dict(variant=tdma.TDMA_VARIANT_PIPELINED), dict(variant=tdma.TDMA_VARIANT_FUSED)],
-                         ids=["pipelined", "fused_tma"])
+@pytest.mark.parametrize("opts", [dict(variant=tdma.TDMA_VARIANT_PIPELINED), dict(variant=tdma.TDMA_VARIANT_FUSED),
+                                  dict(variant=tdma.TDMA_VARIANT_STAGED)], ids=["pipelined", "fused_tma", "staged"])
 @pytest.mark.parametrize("shape,P,batch", [((64, 48, 32), 4, 0), ((256, 20, 64), 8, 7), ((32, 3, 46), 16, 2),
                                            ((512, 6, 128), 8, 4)])
 def test_z_sweep(opts, shape, P, batch):
