@@ -67,6 +67,12 @@ struct TmaFusedConfig {
     int max_clusters = 0;  // co-resident clusters (persistent grid size), filled at first launch
     bool xaxis = false;    // x sweep: 16-row leaves, swizzled boxes, staging tile for x
     size_t smem = 0;
+    // the tensor maps of the last launches, keyed by the five base pointers and the slice count: plain
+    // stream launches (no CUDA graph) of the same slab do not encode 5 maps per launch again
+    struct MapSet { const void *ptr[5]; int nzs; CUtensorMap tm[5]; };
+    static constexpr int kMapSets = 16;
+    MapSet maps[kMapSets];
+    int nmaps = 0, next_map = 0;
 };
 
 struct TmaFusedParams {
@@ -1399,15 +1405,34 @@ inline cudaError_t launch_tma_fused(TmaFusedConfig &cfg, const double *a, const 
                                     int nzs, long long rs, long long os, bool axis_z, bool periodic,
                                     cudaStream_t st)
 {
-    CUtensorMap tm[5];
     const void *ptr[5] = {a, b, c, d, x};
     const int xtiles = (nx + cfg.lines - 1) / cfg.lines;
     // 64-byte row segments: neighbouring x tiles share 128-byte lines -> a cluster takes them in pairs
     const bool pair = !cfg.xaxis && cfg.lines * sizeof(double) < 128 && xtiles % 2 == 0;
-    for (int i = 0; i < 5 && nzs > 0; ++i) {
-        if (cfg.xaxis ? !make_xsweep_tensor_map(&tm[i], ptr[i], ny, nx, nzs, cfg.lines, cfg.leaves)
-                      : !make_slab_tensor_map(&tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows, pair))
-            return cudaErrorInvalidValue;
+    CUtensorMap dummy[5];
+    const CUtensorMap *tm = dummy;
+    if (nzs > 0) {              // everything else a map depends on is fixed per plan
+        TmaFusedConfig::MapSet *hit = nullptr;
+        for (int i = 0; i < cfg.nmaps && !hit; ++i) {
+            TmaFusedConfig::MapSet &m = cfg.maps[i];
+            if (m.nzs == nzs && m.ptr[0] == a && m.ptr[1] == b && m.ptr[2] == c && m.ptr[3] == d && m.ptr[4] == x) hit = &m;
+        }
+        if (!hit) {
+            TmaFusedConfig::MapSet &m = cfg.maps[cfg.next_map];
+            for (int i = 0; i < 5; ++i) {
+                if (cfg.xaxis ? !make_xsweep_tensor_map(&m.tm[i], ptr[i], ny, nx, nzs, cfg.lines, cfg.leaves)
+                              : !make_slab_tensor_map(&m.tm[i], ptr[i], nx, ny, nzs, rs, os, axis_z, cfg.lines, cfg.box_rows, pair)) {
+                    m.nzs = -1;
+                    return cudaErrorInvalidValue;
+                }
+                m.ptr[i] = ptr[i];
+            }
+            m.nzs = nzs;
+            cfg.next_map = (cfg.next_map + 1) % TmaFusedConfig::kMapSets;
+            if (cfg.nmaps < TmaFusedConfig::kMapSets) ++cfg.nmaps;
+            hit = &m;
+        }
+        tm = hit->tm;
     }
     TmaFusedParams prm;
     prm.nx = nx; prm.ny = ny; prm.nzs = nzs;
