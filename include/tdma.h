@@ -179,9 +179,12 @@ int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, con
  * (0,0) is replaced by b = 1, c = 0 (the singular mean mode of the Poisson problem pinned to
  * x_0 = d_0, BASELINE cfg 2/3).  d, x: DEVICE pointers, 16-byte aligned; x may alias d exactly.
  * HBM traffic: d read once, x written once (16 B per real cell, 32 B per complex cell); the
- * matrix is rebuilt on chip.  Any plan with lines along y and no cyclic coupling can be used
- * (nx, ny, nz are the plan's; P and batch are not used: the line is cut into the kernel's own
- * leaves, D1); one persistent launch (plus the fill launch, see fused_fill) per call.
+ * matrix is rebuilt on chip.  The plan gives the shape and the sweep: lines along y, or along z
+ * (options.axis = TDMA_AXIS_Z: a_y, b0_y, c_y then hold nz entries along z, sz holds ny shifts, one
+ * per y-slice) -- the momentum sweeps of the paper's ADI scheme share their matrix in the same way
+ * -- plain or cyclic (options.periodic, without pin00); x sweeps are not offered.
+ * P and batch are not used: the line is cut into the kernel's own leaves (D1); one
+ * persistent launch (plus the fill launch, see fused_fill) per call.
  * TDMA_ERR_UNSUPPORTED when ny does not tile (ny = CL * W * M0, CL in 1,2,4,8, W a power of two
  * <= 32, M0 in 4,8,16) or nx*ncomp is odd.  Enqueue-only. */
 int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const void *c_y,

@@ -319,6 +319,7 @@ class Plan:
     def __init__(self, nx: int, ny: int, nz: int, P: int, batch: int = 0, **options):
         self.shape = (nz, ny, nx)
         self.P = P
+        self.axis = options.get("axis", TDMA_AXIS_Y)
         self.handle = (tdma_plan_create_ex(nx, ny, nz, P, batch, TDMA_F64, **options)
                        if options else tdma_plan_create(nx, ny, nz, P, batch, TDMA_F64))
 
@@ -338,9 +339,10 @@ class Plan:
         """Shared-coefficient solve; d, x real (nz, ny, nx) fp64 or complex128 tensors."""
         nz, ny, nx = self.shape
         ncomp = 2 if (hasattr(d, "is_complex") and d.is_complex()) else 1
-        for t, n in ((a_y, ny), (b0_y, ny), (c_y, ny), (sx, nx), (sz, nz)):
+        nline, nslice = (nz, ny) if self.axis == TDMA_AXIS_Z else (ny, nz)       # z sweep: lines along z, y-slices
+        for t, n in ((a_y, nline), (b0_y, nline), (c_y, nline), (sx, nx), (sz, nslice)):
             if t.numel() != n or not t.is_contiguous() or t.element_size() != 8:
-                raise ValueError("coefficient arrays must be contiguous fp64 of lengths ny, ny, ny, nx, nz")
+                raise ValueError("coefficient arrays must be contiguous fp64 of lengths n, n, n (line length), nx, slices")
         for t in (d, x):
             if t.numel() != nz * ny * nx or not t.is_contiguous() or t.element_size() != 8 * ncomp:
                 raise ValueError("d, x must be contiguous with nz*ny*nx cells of %d bytes" % (8 * ncomp))

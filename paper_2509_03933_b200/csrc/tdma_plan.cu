@@ -670,8 +670,10 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
     if (!sx || !sz) return set_err(TDMA_ERR_INVALID_ARG, "NULL shift array");
     if (ncomp != 1 && ncomp != 2) return set_err(TDMA_ERR_INVALID_ARG, "ncomp = %d must be 1 (real) or 2 (complex)", ncomp);
     tdma_plan *pl = plan;
-    if (pl->axis != TDMA_AXIS_Y || pl->periodic)
-        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: lines along y without cyclic coupling only");
+    if (pl->axis == TDMA_AXIS_X)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: lines along y or z (x sweeps take tdma_solve)");
+    if (pl->periodic && pin00)
+        return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: pin00 is for plain lines");
     if ((((uintptr_t)d | (uintptr_t)x) & 15) != 0)
         return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared needs 16-byte aligned d and x (tensor maps)");
     const int q = ncomp - 1;
@@ -703,6 +705,8 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
     args.d = (const double *)d; args.x = (double *)x;
     args.pin00 = pin00 ? 1 : 0;
     args.nx = pl->nx; args.ny = pl->ny; args.nzs = 0;
+    args.rs = pl->rs; args.os = pl->os;
+    args.axis_z = pl->axis == TDMA_AXIS_Z ? 1 : 0; args.periodic = pl->periodic ? 1 : 0;
     cudaError_t e = tdma::launch_shared(pl->sh[q], args, origin);          // prepare: attributes, grid size
     int nzf = 0;
     if (e == cudaSuccess && pl->sh_have_fill[q]) {
@@ -734,7 +738,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
     e = tdma::launch_shared(pl->sh[q], args, origin);
     if (e == cudaSuccess && nzf > 0) {
         tdma::SharedArgs fa = args;
-        const size_t off = (size_t)(pl->nz - nzf) * pl->slice * (size_t)ncomp;
+        const size_t off = (size_t)(pl->nz - nzf) * (size_t)pl->os * (size_t)ncomp;
         fa.d = args.d + off; fa.x = args.x + off; fa.sz = args.sz + (pl->nz - nzf);
         fa.pin00 = 0;                    // line (0,0) lies in slice 0, which the main launch owns
         fa.nzs = nzf;

@@ -33,7 +33,9 @@ struct SharedArgs {
     const double *d;                  // slice 0 of the launch
     double *x;
     int pin00;                        // row 0 of line (0, 0) of THIS launch's slice 0 is b = 1, c = 0
-    int nx, ny, nzs;
+    int nx, ny, nzs;                  // lanes, rows per line, slices of the launch
+    long long rs = 0, os = 0;         // cells between rows of a line / between slices of d and x
+    int axis_z = 0, periodic = 0;     // z sweep (rows are the slow axis); cyclic lines
 };
 
 // Tiling for ny-row lines: CL x W x M0 with W a power of two.  want_* = 0: auto.

@@ -26,6 +26,8 @@ namespace tdma {
 struct SharedParams {
     const double *a_y, *b0_y, *c_y, *sx, *sz;
     int pin00;
+    int axis_z;         // 1: lines along z (rows = tensor dim 2, slices = dim 1), as in fused_tma_kernel
+    int periodic;       // cyclic lines: the wrap is resolved at the root of the recursion
     int nx, ny, nzs;
     int CL, R, W, NS;
     int xtiles, ntiles;
@@ -283,7 +285,10 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         double *const dst = raw + (size_t)s * arr;
         ptx::mbar_expect_tx(&bar[s], arr_bytes);
         for (int b = 0; b < prm.nbox; ++b)
-            ptx::tma_load_3d(dst + b * prm.box_rows * TXD, &tm_d, x0 * NC, y0 + b * prm.box_rows, k, &bar[s]);
+        {
+            const int yy = y0 + b * prm.box_rows;
+            ptx::tma_load_3d(dst + b * prm.box_rows * TXD, &tm_d, x0 * NC, prm.axis_z ? k : yy, prm.axis_z ? yy : k, &bar[s]);
+        }
     };
     auto store_tile = [&](int q) {                             // x of the q-th tile (TMA clips a ragged x tile)
         const int tile = g + q * NC_;
@@ -291,15 +296,18 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
             const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
             const double *const src = raw + (size_t)(q % NA) * arr;
             for (int b = 0; b < prm.nbox; ++b)
-                ptx::tma_store_3d(&tm_x, x0 * NC, y0 + b * prm.box_rows, k, src + b * prm.box_rows * TXD);
+            {
+                const int yy = y0 + b * prm.box_rows;
+                ptx::tma_store_3d(&tm_x, x0 * NC, prm.axis_z ? k : yy, prm.axis_z ? yy : k, src + b * prm.box_rows * TXD);
+            }
         }
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     };
     if (issue_lane >= 0) for (int q = 0; q < NA; ++q) issue_tile(q);
 
     const int lx = t % TX, leaf = t / TX;
-    const bool first_leaf = y0 + leaf * M0 == 0;
-    const bool last_leaf = y0 + leaf * M0 + M0 == prm.ny;
+    const bool first_leaf = !prm.periodic && y0 + leaf * M0 == 0;          // cyclic lines use a_0 and c_{n-1}
+    const bool last_leaf = !prm.periodic && y0 + leaf * M0 + M0 == prm.ny;
     const uint32_t row_bytes = TXD * 8u;
     const uint32_t leaf_off = (uint32_t)(leaf * M0 * TXD + lx * NC) * 8u;
     // K-ary tree levels, packed as in fused_tma_kernel
@@ -341,7 +349,7 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         if (kCluster && t == 0)
             ptx::mbar_expect_tx(&bar[NA + par], (unsigned)(NTR * TX * (32 + 8 * (NC - 1))));
         const double s = s_next;
-        const bool pin = prm.pin00 != 0 && first_leaf && xt * TX + lx == 0 && k == 0;
+        const bool pin = prm.pin00 != 0 && y0 + leaf * M0 == 0 && xt * TX + lx == 0 && k == 0;
         const uint32_t dbase = ptx::smem_u32(raw + (size_t)slot * arr) + leaf_off;
         const int cur_slot = slot, cur_phase = sphase;
         // next tile's coordinates; its shift is fetched now, a whole tile period ahead of its use
@@ -411,7 +419,7 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
             }
             // ---------------- cluster level ----------------
             if (!kCluster) {
-                if (leaf == 0) solve_root<TX, NC>(nb, lx, 2 * W - 1, false);
+                if (leaf == 0) solve_root<TX, NC>(nb, lx, 2 * W - 1, prm.periodic != 0);
             } else {
                 // all-gather of the CTA's node (the paper's MPI_Alltoall)
                 const uint32_t bar_s = ptx::smem_u32(&bar[NA + par]);
@@ -437,7 +445,20 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
                     ptx::mbar_wait(&bar[NA + par], (unsigned)((it >> 1) & 1));
                     // Stage B: every CTA computes its own two unknowns of the 2 CL-row system
                     double u0[NC], u1[NC];
-                    cluster_solve_two_sided<TX, NC>(tb, lx, NTR, 2 * (int)crank, u0, u1);
+                    if (!prm.periodic) {
+                        cluster_solve_two_sided<TX, NC>(tb, lx, NTR, 2 * (int)crank, u0, u1);
+                    } else {
+                        // cyclic lines: merge the CL nodes, resolve the wrap at the root, walk back
+                        kmerge_fwd<TX, 0, NC>(tb, lx, 0, 2, CL);
+                        kmerge_bwd<TX, 0, NC>(tb, lx, 0, 2, CL);
+                        solve_root<TX, NC>(tb, lx, NTR - 1, true);
+                        kmerge_tails<TX, 0, NC>(tb, lx, 0, 2, CL);
+                        double rf[NC], rl[NC];
+                        nb_load_donly<NC>(tb, nb_ab<TX>(tb, 0, lx), rf);
+                        nb_load_donly<NC>(tb, nb_ab<TX>(tb, NTR - 1, lx), rl);
+                        kmerge_value_n<TX, NC>(tb, lx, 0, 2, CL, 2 * (int)crank, rf, rl, u0);
+                        kmerge_value_n<TX, NC>(tb, lx, 0, 2, CL, 2 * (int)crank + 1, rf, rl, u1);
+                    }
                     // into the CTA's own rows of its INBOX, not into the node rows: other warps of
                     // this CTA may still be reading those for their sends to the peers
                     nb_store_d<NC>(tb, nb_ab<TX>(tb, 2 * (int)crank, lx), u0);
@@ -559,13 +580,15 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
 }
 
 // d / x as a tensor of doubles (nx * NC, ny, nz), box (TX * NC, box_rows, 1)
-inline bool make_shared_tensor_map(CUtensorMap *tm, const void *base, int nx, int ny, int nz, int NC, int TX, int box_rows)
+inline bool make_shared_tensor_map(CUtensorMap *tm, const void *base, int nx, int ny, int nz, int NC, int TX, int box_rows,
+                                   long long rs, long long os, bool axis_z)
 {
     tdma_encode_tiled_fn enc = get_encode_tiled();
     if (!enc) return false;
-    cuuint64_t gdim[3] = {(cuuint64_t)nx * NC, (cuuint64_t)ny, (cuuint64_t)nz};
-    cuuint64_t gstr[2] = {(cuuint64_t)nx * NC * sizeof(double), (cuuint64_t)nx * NC * ny * sizeof(double)};
-    cuuint32_t box[3] = {(cuuint32_t)(TX * NC), (cuuint32_t)box_rows, 1};
+    // rs / os: cells between rows of a line / between slices (y sweep: nx, nx * ny; z sweep: nx * slices, nx)
+    cuuint64_t gdim[3] = {(cuuint64_t)nx * NC, (cuuint64_t)(axis_z ? nz : ny), (cuuint64_t)(axis_z ? ny : nz)};
+    cuuint64_t gstr[2] = {(cuuint64_t)(axis_z ? os : rs) * NC * sizeof(double), (cuuint64_t)(axis_z ? rs : os) * NC * sizeof(double)};
+    cuuint32_t box[3] = {(cuuint32_t)(TX * NC), (cuuint32_t)(axis_z ? 1 : box_rows), (cuuint32_t)(axis_z ? box_rows : 1)};
     cuuint32_t estr[3] = {1, 1, 1};
     const size_t inner = (size_t)TX * NC * sizeof(double);
     const CUtensorMapL2promotion promo = inner >= 256 ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B;
@@ -640,13 +663,14 @@ inline cudaError_t launch_shared_impl(SharedConfig &cfg, const SharedArgs &a, cu
 {
     CUtensorMap tm[2];
     if (a.nzs > 0) {
-        if (!make_shared_tensor_map(&tm[0], a.d, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows) ||
-            !make_shared_tensor_map(&tm[1], a.x, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows))
+        if (!make_shared_tensor_map(&tm[0], a.d, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows, a.rs, a.os, a.axis_z != 0) ||
+            !make_shared_tensor_map(&tm[1], a.x, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows, a.rs, a.os, a.axis_z != 0))
             return cudaErrorInvalidValue;
     }
     SharedParams prm;
     prm.a_y = a.a_y; prm.b0_y = a.b0_y; prm.c_y = a.c_y; prm.sx = a.sx; prm.sz = a.sz;
     prm.pin00 = a.pin00;
+    prm.axis_z = a.axis_z; prm.periodic = a.periodic;
     prm.nx = a.nx; prm.ny = a.ny; prm.nzs = a.nzs;
     prm.CL = cfg.cluster; prm.R = cfg.rows; prm.W = cfg.leaves; prm.NS = cfg.slots;
     prm.xtiles = (a.nx + cfg.lines - 1) / cfg.lines;

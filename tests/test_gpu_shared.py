@@ -175,8 +175,12 @@ def test_unsupported_shapes_fail_loudly():
     w = random_shared(2, 64, 32, False, seed=1)
     t = [v.to(dv) for v in (w.a_y, w.b0_y, w.c_y, w.sx, w.sz, w.d)]
     with tdma.Plan(32, 64, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, periodic=1) as plan:
-        with pytest.raises(tdma.TdmaError):
-            plan.solve_shared(*t, torch.empty_like(t[5]))
+        with pytest.raises(tdma.TdmaError):               # the pinned mean mode belongs to plain lines
+            plan.solve_shared(*t, torch.empty_like(t[5]), pin00=True)
+    with tdma.Plan(64, 32, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X) as plan:
+        with pytest.raises(tdma.TdmaError) as e3:         # x sweeps are not offered in this form
+            tdma.tdma_solve_shared(plan.handle, *t[:5], 1, 0, t[5], torch.empty_like(t[5]))
+        assert e3.value.status == tdma.TDMA_ERR_UNSUPPORTED
 
 
 @pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
@@ -222,3 +226,43 @@ def test_cfg3_shared_full_size_sampled(cplx):
         assert E <= TOL_E, "slice %d: normwise error %.3e" % (k, E)
     del w, x
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+@pytest.mark.parametrize("axis,periodic,shape", [
+    ("y", True, (5, 256, 48)), ("y", True, (3, 1024, 40)), ("z", False, (256, 6, 48)),
+    ("z", True, (512, 5, 40)), ("z", True, (64, 7, 32)), ("z", False, (1024, 3, 64)),
+])
+def test_shared_z_sweeps_and_cyclic_lines(axis, periodic, shape, cplx):
+    """Shared coefficients along z and / or with the cyclic coupling (the matrix-sharing momentum sweeps
+    of the ADI scheme): against oracle.solve_axis on the materialised arrays, whose
+    diagonal is formed exactly as the kernel forms it, b0 - (sx + s_slice)."""
+    nz, ny, nx = shape
+    n, nsl = (nz, ny) if axis == "z" else (ny, nz)            # line length, slices
+    g = torch.Generator().manual_seed(1000 + n + nsl)
+    u = lambda k, lo, hi: lo + (hi - lo) * torch.rand(k, dtype=torch.float64, generator=g)
+    a1, c1, b01 = u(n, -1, 1), u(n, -1, 1), u(n, 2.5, 3.5)
+    sx, ss = -u(nx, 0, 2), -u(nsl, 0, 2)
+    d = torch.randn((nz, ny, nx), dtype=torch.float64, generator=g)
+    if cplx:
+        d = torch.complex(d, torch.randn((nz, ny, nx), dtype=torch.float64, generator=g))
+    dv = dev()
+    x = torch.full_like(d, float("nan")).to(dv)
+    opts = dict(axis=tdma.TDMA_AXIS_Z if axis == "z" else tdma.TDMA_AXIS_Y, periodic=1 if periodic else 0)
+    with tdma.Plan(nx, ny, nz, 1, 0, **opts) as plan:
+        plan.solve_shared(*[t.to(dv) for t in (a1, b01, c1, sx, ss)], d.to(dv), x)
+        torch.cuda.synchronize()
+    # materialise: the line axis is z (dim 0) or y (dim 1) of the (nz, ny, nx) arrays
+    line = (n, 1, 1) if axis == "z" else (1, n, 1)
+    sl = (1, nsl, 1) if axis == "z" else (nsl, 1, 1)
+    a = a1.view(line).expand(nz, ny, nx).contiguous().numpy()
+    c = c1.view(line).expand(nz, ny, nx).contiguous().numpy()
+    b = (b01.view(line) - (sx.view(1, 1, nx) + ss.view(sl))).expand(nz, ny, nx).contiguous().numpy()
+    xn = x.cpu().numpy()
+    ax = 0 if axis == "z" else 1
+    for part in (("real", "imag") if cplx else (None,)):
+        dn = getattr(d, part).contiguous().numpy() if part else d.numpy()
+        xp = getattr(xn, part) if part else xn
+        ref = oracle.solve_axis(a, b, c, dn, axis, periodic)
+        err = (np.max(np.abs(xp - ref), axis=ax) / np.max(np.abs(ref), axis=ax)).max()
+        assert np.isfinite(xp).all() and err <= TOL_E, err
