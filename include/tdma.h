@@ -182,7 +182,10 @@ int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, con
  * matrix is rebuilt on chip.  The plan gives the shape and the sweep: lines along y, or along z
  * (options.axis = TDMA_AXIS_Z: a_y, b0_y, c_y then hold nz entries along z, sz holds ny shifts, one
  * per y-slice) -- the momentum sweeps of the paper's ADI scheme share their matrix in the same way
- * -- plain or cyclic (options.periodic, without pin00); x sweeps are not offered.
+ * -- or along x (options.axis = TDMA_AXIS_X, ncomp = 1 only, nx a multiple of 16:
+ * a_y, b0_y, c_y hold nx entries along x, sx holds NY shifts, one per line of a slice, sz the nz
+ * shifts of the slices: line (j,k) has the shift sx[j] + sz[k]) -- plain or cyclic
+ * (options.periodic, without pin00).
  * P and batch are not used: the line is cut into the kernel's own leaves (D1); one
  * persistent launch (plus the fill launch, see fused_fill) per call.
  * TDMA_ERR_UNSUPPORTED when ny does not tile (ny = CL * W * M0, CL in 1,2,4,8, W a power of two

@@ -339,10 +339,12 @@ class Plan:
         """Shared-coefficient solve; d, x real (nz, ny, nx) fp64 or complex128 tensors."""
         nz, ny, nx = self.shape
         ncomp = 2 if (hasattr(d, "is_complex") and d.is_complex()) else 1
-        nline, nslice = (nz, ny) if self.axis == TDMA_AXIS_Z else (ny, nz)       # z sweep: lines along z, y-slices
-        for t, n in ((a_y, nline), (b0_y, nline), (c_y, nline), (sx, nx), (sz, nslice)):
+        # (line length, lines side by side, slices): z sweep: lines along z, y-slices; x sweep: lines along x,
+        # ny of them per z-slice
+        nline, nlane, nslice = {TDMA_AXIS_Z: (nz, nx, ny), TDMA_AXIS_X: (nx, ny, nz)}.get(self.axis, (ny, nx, nz))
+        for t, n in ((a_y, nline), (b0_y, nline), (c_y, nline), (sx, nlane), (sz, nslice)):
             if t.numel() != n or not t.is_contiguous() or t.element_size() != 8:
-                raise ValueError("coefficient arrays must be contiguous fp64 of lengths n, n, n (line length), nx, slices")
+                raise ValueError("coefficient arrays must be contiguous fp64 of lengths n, n, n (line length), lanes, slices")
         for t in (d, x):
             if t.numel() != nz * ny * nx or not t.is_contiguous() or t.element_size() != 8 * ncomp:
                 raise ValueError("d, x must be contiguous with nz*ny*nx cells of %d bytes" % (8 * ncomp))

@@ -670,8 +670,9 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
     if (!sx || !sz) return set_err(TDMA_ERR_INVALID_ARG, "NULL shift array");
     if (ncomp != 1 && ncomp != 2) return set_err(TDMA_ERR_INVALID_ARG, "ncomp = %d must be 1 (real) or 2 (complex)", ncomp);
     tdma_plan *pl = plan;
-    if (pl->axis == TDMA_AXIS_X)
-        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: lines along y or z (x sweeps take tdma_solve)");
+    const bool xsw = pl->axis == TDMA_AXIS_X;
+    if (xsw && ncomp != 1)
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: x sweeps take real right-hand sides (ncomp = 1)");
     if (pl->periodic && pin00)
         return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: pin00 is for plain lines");
     if ((((uintptr_t)d | (uintptr_t)x) & 15) != 0)
@@ -684,7 +685,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         CUDA_TRY(cudaGetDeviceProperties(&prop, pl->device));
         const char *why = nullptr;
         if (!tdma::configure_shared(&pl->sh[q], pl->nx, pl->ny, ncomp, pl->sh_opt[0], pl->sh_opt[1], pl->sh_opt[2],
-                                    pl->sh_opt[3], pl->sh_opt[4], prop, &why)) {
+                                    pl->sh_opt[3], pl->sh_opt[4], prop, &why, xsw)) {
             pl->sh_state[q] = -1;
             return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared unavailable for this shape: %s", why ? why : "?");
         }
@@ -693,7 +694,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         if (pl->sh[q].cluster >= 4 && pl->fill_opt >= 0) {
             const char *why2 = nullptr;
             pl->sh_have_fill[q] = tdma::configure_shared(&pl->sh_fill[q], pl->nx, pl->ny, ncomp, 0,
-                                                         pl->ny % 2 == 0 ? 2 : 1, 0, 0, 0, prop, &why2);
+                                                         pl->ny % 2 == 0 ? 2 : 1, 0, 0, 0, prop, &why2, xsw);
         }
         pl->sh_state[q] = 1;
     }

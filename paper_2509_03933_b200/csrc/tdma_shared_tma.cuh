@@ -99,6 +99,42 @@ struct ShLeafRegs {
     Elim<NC> e[K > 1 ? K - 1 : 1];
 };
 
+// The K swept sub-leaves as nodes with unit diagonals, merged pairwise in registers into the leaf's
+// two boundary equations.
+template <int M0, int NC>
+__device__ __forceinline__ void leaf_finish_sh(const double (&fa)[ShLeafRegs<M0, NC>::K], const double (&fb)[ShLeafRegs<M0, NC>::K],
+                                               const double (&fc)[ShLeafRegs<M0, NC>::K], const double (&fd)[ShLeafRegs<M0, NC>::K][NC],
+                                               const double (&pa)[ShLeafRegs<M0, NC>::K], const double (&pc)[ShLeafRegs<M0, NC>::K],
+                                               const double (&pd)[ShLeafRegs<M0, NC>::K][NC],
+                                               EqN<NC> &f, EqN<NC> &l, ShLeafRegs<M0, NC> &R)
+{
+    constexpr int K = ShLeafRegs<M0, NC>::K;
+    NodeEq<NC> nd[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const double inv = rcp_nr(fb[h]);
+        nd[h].fa = fa[h] * inv; nd[h].fb = 1.0; nd[h].fc = fc[h] * inv;
+        nd[h].la = pa[h]; nd[h].lb = 1.0; nd[h].lc = pc[h];
+#pragma unroll
+        for (int q = 0; q < NC; ++q) { nd[h].fd[q] = fd[h][q] * inv; nd[h].ld[q] = pd[h][q]; }
+    }
+    NodeEq<NC> top;
+    if constexpr (K == 1) {
+        top = nd[0];
+    } else if constexpr (K == 2) {
+        merge_nodes<NC>(nd[0], nd[K - 1], top, R.e[0]);
+    } else {
+        NodeEq<NC> m01, m23;
+        merge_nodes<NC>(nd[0], nd[1], m01, R.e[0]);
+        merge_nodes<NC>(nd[K - 2], nd[K - 1], m23, R.e[1]);
+        merge_nodes<NC>(m01, m23, top, R.e[K - 2]);
+    }
+    f.a = top.fa; f.b = top.fb; f.c = top.fc;
+    l.a = top.la; l.b = top.lb; l.c = top.lc;
+#pragma unroll
+    for (int q = 0; q < NC; ++q) { f.d[q] = top.fd[q]; l.d[q] = top.ld[q]; }
+}
+
 // Modified Thomas reduction of the leaf's K sub-leaves, swept interleaved (K independent
 // recurrences per thread; same arithmetic as leaf_reduce in tdma_fused_tma.cuh).  cA, cB, cC: the
 // leaf's rows of a_y, b0_y, c_y in shared memory; s: the line's shift; dbase: shared address of the
@@ -154,31 +190,7 @@ __device__ __forceinline__ void leaf_reduce_sh(const double *__restrict__ cA, co
             pa[h] = -(ar * pa[h]) * inv;
         }
     }
-    // the sub-leaves as nodes with unit diagonals
-    NodeEq<NC> nd[K];
-#pragma unroll
-    for (int h = 0; h < K; ++h) {
-        const double inv = rcp_nr(fb[h]);
-        nd[h].fa = fa[h] * inv; nd[h].fb = 1.0; nd[h].fc = fc[h] * inv;
-        nd[h].la = pa[h]; nd[h].lb = 1.0; nd[h].lc = pc[h];
-#pragma unroll
-        for (int q = 0; q < NC; ++q) { nd[h].fd[q] = fd[h][q] * inv; nd[h].ld[q] = pd[h][q]; }
-    }
-    NodeEq<NC> top;
-    if constexpr (K == 1) {
-        top = nd[0];
-    } else if constexpr (K == 2) {
-        merge_nodes<NC>(nd[0], nd[K - 1], top, R.e[0]);
-    } else {
-        NodeEq<NC> m01, m23;
-        merge_nodes<NC>(nd[0], nd[1], m01, R.e[0]);
-        merge_nodes<NC>(nd[K - 2], nd[K - 1], m23, R.e[1]);
-        merge_nodes<NC>(m01, m23, top, R.e[K - 2]);
-    }
-    f.a = top.fa; f.b = top.fb; f.c = top.fc;
-    l.a = top.la; l.b = top.lb; l.c = top.lc;
-#pragma unroll
-    for (int q = 0; q < NC; ++q) { f.d[q] = top.fd[q]; l.d[q] = top.ld[q]; }
+    leaf_finish_sh<M0, NC>(fa, fb, fc, fd, pa, pc, pd, f, l, R);
 }
 
 // the two unknowns a merge eliminated, from the merged node's first / last unknown
@@ -229,14 +241,114 @@ __device__ __forceinline__ void leaf_back_sh(const ShLeafRegs<M0, NC> &R, const 
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// x sweeps (lines along the contiguous axis; real right-hand sides, 16- or 32-row leaves).  As in
+// fused_tma_kernel 16 consecutive x of one line are one 128-byte row of the box
+// [leaf][line][16 x], 128-byte swizzle keyed by the line (xs_addr).  The thread reads and writes
+// its row in 16-byte pairs (conflict-free per quarter warp): d' of rows 2p, 2p+1 goes back as one
+// store once both are known, x likewise.  Same arithmetic, in the same order, as leaf_reduce_sh /
+// leaf_back_sh<16, 1>.
+// ------------------------------------------------------------------------------------------
+// sub-leaf h of a leaf: 8 x = pairs 4 (h & 1) .. + 3 of the 128-byte row in 16-row box h >> 1
+template <int TX>
+__device__ __forceinline__ uint32_t xs_sub(uint32_t box, int l, int h, int p)
+{
+    return xs_addr(box + (uint32_t)(h >> 1) * (uint32_t)(TX * 128), l, 4 * (h & 1) + p);
+}
+
+template <int TX, int M0>
+__device__ __forceinline__ void leaf_reduce_sh_x(const double *__restrict__ cA, const double *__restrict__ cB,
+                                                 const double *__restrict__ cC, double s, uint32_t box, int l,
+                                                 bool first_leaf, bool last_leaf, bool pin,
+                                                 EqN<1> &f, EqN<1> &le, ShLeafRegs<M0, 1> &R)
+{
+    constexpr int K = ShLeafRegs<M0, 1>::K, H = ShLeafRegs<M0, 1>::H;
+    static_assert(H == 8 && K >= 2, "x sweeps: 16- or 32-row leaves of 8-row sub-leaves");
+    double fa[K], fb[K], fc[K], fd[K][1], pa[K], pc[K], pd[K][1], hold[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const int o = h * H;
+        double b0 = cB[o] - s, c0 = cC[o];
+        if (h == 0 && pin) { b0 = 1.0; c0 = 0.0; }
+        double inv = rcp_nr(b0);
+        const double2 d2 = lds2(xs_sub<TX>(box, l, h, 0));
+        fa[h] = (h == 0 && first_leaf) ? 0.0 : cA[o] * inv;
+        fc[h] = c0 * inv; fb[h] = 1.0; fd[h][0] = d2.x * inv;
+        inv = rcp_nr(cB[o + 1] - s);
+        pa[h] = cA[o + 1] * inv; pc[h] = cC[o + 1] * inv; pd[h][0] = d2.y * inv;
+        hold[h] = 0.0;                                   // row 0 of the sub-leaf: overwritten by x_first
+    }
+#pragma unroll
+    for (int p = 1; p < H / 2; ++p) {
+        double2 d2[K];
+#pragma unroll
+        for (int h = 0; h < K; ++h) d2[h] = lds2(xs_sub<TX>(box, l, h, p));
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int r = 2 * p + e;
+#pragma unroll
+            for (int h = 0; h < K; ++h) {
+                const int o = h * H + r;
+                const double ar = cA[o], br = cB[o] - s, dr = e ? d2[h].y : d2[h].x;
+                double cr = cC[o];
+                if (r == H - 1 && h == K - 1 && last_leaf) cr = 0.0;
+                fb[h] = fma(-fc[h], pa[h], fb[h]);
+                fd[h][0] = fma(-fc[h], pd[h][0], fd[h][0]);
+                fc[h] = -fc[h] * pc[h];
+                R.ia[h][r - 2] = pa[h]; R.ic[h][r - 2] = pc[h];
+                if (e == 0) sts2(xs_sub<TX>(box, l, h, p - 1), hold[h], pd[h][0]);   // d' of rows r-2, r-1, in place
+                else hold[h] = pd[h][0];
+                const double inv = rcp_nr(fma(-ar, pc[h], br));
+                pd[h][0] = fma(-ar, pd[h][0], dr) * inv;
+                pc[h] = cr * inv;
+                pa[h] = -(ar * pa[h]) * inv;
+            }
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < K; ++h) sts2(xs_sub<TX>(box, l, h, 3), hold[h], 0.0);         // d' of row H-2; row H-1 becomes x_last
+    leaf_finish_sh<M0, 1>(fa, fb, fc, fd, pa, pc, pd, f, le, R);
+}
+
+template <int TX, int M0>
+__device__ __forceinline__ void leaf_back_sh_x(const ShLeafRegs<M0, 1> &R, const double (&xf)[1], const double (&xl)[1],
+                                               uint32_t box, int l)
+{
+    constexpr int K = ShLeafRegs<M0, 1>::K, H = ShLeafRegs<M0, 1>::H;
+    double first[K][1], xn[K][1];
+    first[0][0] = xf[0]; xn[K - 1][0] = xl[0];
+    if constexpr (K == 2) {
+        elim_values<1>(R.e[0], xf, xl, xn[0], first[K - 1]);
+    } else {
+        elim_values<1>(R.e[K - 2], xf, xl, xn[1], first[K - 2]);
+        elim_values<1>(R.e[0], xf, xn[1], xn[0], first[1]);
+        elim_values<1>(R.e[1], first[K - 2], xl, xn[K - 2], first[K - 1]);
+    }
+#pragma unroll
+    for (int p = H / 2 - 1; p >= 0; --p) {
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            const uint32_t o = xs_sub<TX>(box, l, h, p);
+            const double2 dp = lds2(o);
+            double hi = xn[h][0];                                   // x of row 2p+1 (p = 3: the sub-leaf's last unknown)
+            if (p < H / 2 - 1) hi = fma(-R.ic[h][2 * p], xn[h][0], fma(-R.ia[h][2 * p], first[h][0], dp.y));
+            double lo = first[h][0];                                // x of row 2p (p = 0: the sub-leaf's first unknown)
+            if (p > 0) lo = fma(-R.ic[h][2 * p - 1], hi, fma(-R.ia[h][2 * p - 1], first[h][0], dp.x));
+            sts2(o, lo, hi);
+            xn[h][0] = lo;
+        }
+    }
+}
+
 // Threads: leaf = t / TX, lx = t % TX; the last warp issues the TMA copies and takes no part in
 // the tree (as in fused_tma_kernel).  Ring: tile q of the cluster lives in slot q % NA from its
 // load until the TMA store of its x has read the slot; then tile q + NA is loaded into it.
-template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB>
+template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB, bool kX = false>
 __global__ void __launch_bounds__(MAXT, MINB)
 shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_x,
                   const SharedParams prm)
 {
+    static_assert(!kX || ((M0 == 16 || M0 == 32) && NC == 1 && TX % 8 == 0), "x sweeps: real right-hand sides, leaves of whole 128-byte rows");
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     constexpr int TXD = TX * NC;                                      // doubles per tile row
     const int R = prm.R, CL = prm.CL, W = prm.W, NA = prm.NS;
@@ -284,6 +396,10 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
         double *const dst = raw + (size_t)s * arr;
         ptx::mbar_expect_tx(&bar[s], arr_bytes);
+        if (kX) {                                              // one box (16 x, TX lines, W leaves, 1): [leaf][line][16 x]
+            ptx::tma_load_4d(dst, &tm_d, 0, x0, y0 >> 4, k, &bar[s]);
+            return;
+        }
         for (int b = 0; b < prm.nbox; ++b)
         {
             const int yy = y0 + b * prm.box_rows;
@@ -295,7 +411,8 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         if (issue_lane == 0) {
             const int x0 = (tile % prm.xtiles) * TX, k = tile / prm.xtiles;
             const double *const src = raw + (size_t)(q % NA) * arr;
-            for (int b = 0; b < prm.nbox; ++b)
+            if (kX) ptx::tma_store_4d(&tm_x, 0, x0, y0 >> 4, k, src);
+            else for (int b = 0; b < prm.nbox; ++b)
             {
                 const int yy = y0 + b * prm.box_rows;
                 ptx::tma_store_3d(&tm_x, x0 * NC, prm.axis_z ? k : yy, prm.axis_z ? yy : k, src + b * prm.box_rows * TXD);
@@ -309,7 +426,8 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
     const bool first_leaf = !prm.periodic && y0 + leaf * M0 == 0;          // cyclic lines use a_0 and c_{n-1}
     const bool last_leaf = !prm.periodic && y0 + leaf * M0 + M0 == prm.ny;
     const uint32_t row_bytes = TXD * 8u;
-    const uint32_t leaf_off = (uint32_t)(leaf * M0 * TXD + lx * NC) * 8u;
+    // x sweep: the leaf's box of TX 128-byte rows, addressed through xs_addr(box, lx, pair)
+    const uint32_t leaf_off = kX ? (uint32_t)(leaf * M0 * TX) * 8u : (uint32_t)(leaf * M0 * TXD + lx * NC) * 8u;
     // K-ary tree levels, packed as in fused_tma_kernel
     unsigned kcode = 0, ccode = 0;
     int nl = 0;
@@ -363,8 +481,11 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         ShLeafRegs<M0, NC> regs;
         if (act) {
             EqN<NC> f, l;
-            leaf_reduce_sh<M0, NC>(cA + leaf * M0, cB + leaf * M0, cC + leaf * M0, s, dbase, row_bytes,
-                                   first_leaf, last_leaf, pin, f, l, regs);
+            if constexpr (kX)
+                leaf_reduce_sh_x<TX, M0>(cA + leaf * M0, cB + leaf * M0, cC + leaf * M0, s, dbase, lx, first_leaf, last_leaf, pin, f, l, regs);
+            else
+                leaf_reduce_sh<M0, NC>(cA + leaf * M0, cB + leaf * M0, cC + leaf * M0, s, dbase, row_bytes,
+                                       first_leaf, last_leaf, pin, f, l, regs);
             const uint32_t of = nb_ab<TX>(nb, 2 * leaf, lx), ol = of + TX * 16u;
             sts2(of, f.a, f.b); sts2(of + nb.plane, f.c, f.d[0]);
             sts2(ol, l.a, l.b); sts2(ol + nb.plane, l.c, l.d[0]);
@@ -488,7 +609,8 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
 #pragma unroll
                 for (int q = 0; q < NC; ++q) { xf[q] = nf[q]; xl[q] = nla[q]; }
             }
-            leaf_back_sh<M0, NC>(regs, xf, xl, dbase, row_bytes);
+            if constexpr (kX) leaf_back_sh_x<TX, M0>(regs, xf, xl, dbase, lx);
+            else leaf_back_sh<M0, NC>(regs, xf, xl, dbase, row_bytes);
             ptx::fence_proxy_async_smem();      // x in the slot -> visible to the TMA store
         }
     }
@@ -517,10 +639,12 @@ inline size_t shared_smem_bytes(int TX, int R, int W, int CL, int NA, int NC)
 constexpr int kSharedLeafSizes[] = {32, 16, 8, 4};
 
 inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int want_lines, int want_cluster,
-                                  int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why)
+                                  int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why,
+                                  bool xsweep = false)
 {
     if (NC != 1 && NC != 2) { *why = "ncomp must be 1 (real) or 2 (complex)"; return false; }
-    if ((nx * NC) % 2) { *why = "TMA path needs an even number of doubles per row (16-byte global strides)"; return false; }
+    if (xsweep && (NC != 1 || ny % 16)) { *why = "x sweeps: real right-hand sides, line length a multiple of 16"; return false; }
+    if (!xsweep && (nx * NC) % 2) { *why = "TMA path needs an even number of doubles per row (16-byte global strides)"; return false; }
     const size_t max_smem = prop.sharedMemPerBlockOptin;
     SharedConfig best; double best_score = -1.0;
     // lines per tile: 128-byte row segments first (16 real / 8 complex cells), then 256-byte ones
@@ -529,6 +653,7 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
     for (int ti = 0; ti < 3; ++ti) {
         const int TX = tx_opts[ti];
         if (want_lines ? TX != want_lines : ti == 2) continue;      // 64-byte segments only on request
+        if (xsweep && TX != 16) continue;                           // x sweeps: 16 lines of 128-byte leaf rows
         for (int ci = 0; ci < 4; ++ci) {
             const int CL = cl_opts[ci];
             if (want_cluster && CL != want_cluster) continue;
@@ -536,13 +661,14 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
             const int R = ny / CL;
             for (int m0 : kSharedLeafSizes) {
                 if (want_leaf && m0 != want_leaf) continue;
+                if (xsweep && m0 != 16 && m0 != 32) continue;
                 if (m0 > R || R % m0 || !is_pow2(R / m0) || R / m0 > 32) continue;
                 // 32-row leaves (four sub-leaves per thread) halve the tree per cell: 1.46 -> 1.05 ms on 256 slices
                 // of cfg 3 (real).  Complex cells need the registers for the second right-hand side: on request only
                 if (m0 == 32 && want_leaf != 32 && NC != 1) continue;
                 SharedConfig c;
                 c.ncomp = NC; c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
-                c.threads = c.leaves * TX;
+                c.threads = c.leaves * TX; c.xsweep = xsweep ? 1 : 0;
                 if (c.threads > 512 || (m0 == 32 && c.threads > 256)) continue;
                 c.box_rows = R;
                 while (c.box_rows > 256) c.box_rows /= 2;
@@ -554,7 +680,7 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
                 }
                 if (!c.slots) continue;
                 c.ctas_per_sm = 1;
-                if (want_ctas >= 2) {          // co-residency: registers and shared memory shared out
+                if (want_ctas >= 2 && !xsweep) {          // co-residency: registers and shared memory shared out
                     if (c.threads * want_ctas > 512 || m0 != 16) continue;
                     for (; c.slots >= 2; --c.slots) {
                         c.smem = shared_smem_bytes(TX, R, c.leaves, CL, c.slots, NC);
@@ -597,10 +723,10 @@ inline bool make_shared_tensor_map(CUtensorMap *tm, const void *base, int nx, in
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB = 1>
+template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB = 1, bool kX = false>
 inline cudaError_t launch_shared_inst(SharedConfig &cfg, const CUtensorMap *tm, const SharedParams &prm, cudaStream_t st)
 {
-    auto kern = shared_tma_kernel<TX, M0, kCluster, MAXT, NC, MINB>;
+    auto kern = shared_tma_kernel<TX, M0, kCluster, MAXT, NC, MINB, kX>;
     cudaLaunchConfig_t lc = {};
     lc.blockDim = dim3((cfg.threads + 31) & ~31);
     lc.dynamicSmemBytes = cfg.smem;
@@ -662,7 +788,11 @@ inline cudaError_t launch_shared_tx(SharedConfig &cfg, const CUtensorMap *tm, co
 inline cudaError_t launch_shared_impl(SharedConfig &cfg, const SharedArgs &a, cudaStream_t st)
 {
     CUtensorMap tm[2];
-    if (a.nzs > 0) {
+    if (a.nzs > 0 && cfg.xsweep) {
+        if (!make_xsweep_tensor_map(&tm[0], a.d, a.ny, a.nx, a.nzs, cfg.lines, cfg.rows / 16) ||
+            !make_xsweep_tensor_map(&tm[1], a.x, a.ny, a.nx, a.nzs, cfg.lines, cfg.rows / 16))
+            return cudaErrorInvalidValue;
+    } else if (a.nzs > 0) {
         if (!make_shared_tensor_map(&tm[0], a.d, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows, a.rs, a.os, a.axis_z != 0) ||
             !make_shared_tensor_map(&tm[1], a.x, a.nx, a.ny, a.nzs, cfg.ncomp, cfg.lines, cfg.box_rows, a.rs, a.os, a.axis_z != 0))
             return cudaErrorInvalidValue;
@@ -677,6 +807,14 @@ inline cudaError_t launch_shared_impl(SharedConfig &cfg, const SharedArgs &a, cu
     prm.ntiles = prm.xtiles * a.nzs;
     prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
     const bool cl = cfg.cluster > 1;
+    if (cfg.xsweep) {
+        if (cfg.ncomp != 1 || cfg.lines != 16 || (cfg.leaf_rows != 16 && cfg.leaf_rows != 32)) return cudaErrorInvalidValue;
+        if (cfg.leaf_rows == 32)
+            return cl ? launch_shared_inst<16, 32, true, 256, 1, 1, true>(cfg, tm, prm, st) : launch_shared_inst<16, 32, false, 256, 1, 1, true>(cfg, tm, prm, st);
+        if (cfg.threads > 256)
+            return cl ? launch_shared_inst<16, 16, true, 512, 1, 1, true>(cfg, tm, prm, st) : launch_shared_inst<16, 16, false, 512, 1, 1, true>(cfg, tm, prm, st);
+        return cl ? launch_shared_inst<16, 16, true, 256, 1, 1, true>(cfg, tm, prm, st) : launch_shared_inst<16, 16, false, 256, 1, 1, true>(cfg, tm, prm, st);
+    }
     if (cfg.ncomp == 1) {
         if (cfg.lines == 8) return cl ? launch_shared_tx<8, 1, true>(cfg, tm, prm, st) : launch_shared_tx<8, 1, false>(cfg, tm, prm, st);
         if (cfg.lines == 16) return cl ? launch_shared_tx<16, 1, true>(cfg, tm, prm, st) : launch_shared_tx<16, 1, false>(cfg, tm, prm, st);

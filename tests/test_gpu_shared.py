@@ -178,9 +178,11 @@ def test_unsupported_shapes_fail_loudly():
         with pytest.raises(tdma.TdmaError):               # the pinned mean mode belongs to plain lines
             plan.solve_shared(*t, torch.empty_like(t[5]), pin00=True)
     with tdma.Plan(64, 32, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X) as plan:
-        with pytest.raises(tdma.TdmaError) as e3:         # x sweeps are not offered in this form
-            tdma.tdma_solve_shared(plan.handle, *t[:5], 1, 0, t[5], torch.empty_like(t[5]))
+        with pytest.raises(tdma.TdmaError) as e3:         # x sweeps take real right-hand sides only
+            tdma.tdma_solve_shared(plan.handle, *t[:5], 2, 0, t[5], torch.empty_like(t[5]))
         assert e3.value.status == tdma.TDMA_ERR_UNSUPPORTED
+    with pytest.raises(tdma.TdmaError):                   # x lines of 40 cells: not whole 16-cell leaves (no such plan)
+        tdma.Plan(40, 32, 2, 1, 0, axis=tdma.TDMA_AXIS_X)
 
 
 @pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
@@ -266,3 +268,58 @@ def test_shared_z_sweeps_and_cyclic_lines(axis, periodic, shape, cplx):
         ref = oracle.solve_axis(a, b, c, dn, axis, periodic)
         err = (np.max(np.abs(xp - ref), axis=ax) / np.max(np.abs(ref), axis=ax)).max()
         assert np.isfinite(xp).all() and err <= TOL_E, err
+
+
+@pytest.mark.parametrize("periodic", [False, True], ids=["plain", "cyclic"])
+@pytest.mark.parametrize("leaf", [0, 16], ids=["auto", "leaf16"])
+@pytest.mark.parametrize("shape", [(3, 40, 256), (2, 37, 512), (5, 16, 64), (2, 130, 1024), (4, 9, 16), (2, 24, 2048)])
+def test_shared_x_sweeps(shape, periodic, leaf):
+    """Shared coefficients along x (lines along the contiguous axis: the third momentum sweep of the ADI
+    scheme), real right-hand sides: a_y, b0_y, c_y hold nx entries, sx one shift per
+    line of a slice (ny), sz one per slice.  Ragged line tiles (ny not a multiple of 16), one to
+    several CTAs per line, the fill tiling at 1024 cells.  Against oracle.solve_axis on the
+    materialised arrays."""
+    nz, ny, nx = shape
+    g = torch.Generator().manual_seed(2000 + nx + ny)
+    u = lambda k, lo, hi: lo + (hi - lo) * torch.rand(k, dtype=torch.float64, generator=g)
+    a1, c1, b01 = u(nx, -1, 1), u(nx, -1, 1), u(nx, 2.5, 3.5)
+    sy, sz = -u(ny, 0, 2), -u(nz, 0, 2)
+    d = torch.randn((nz, ny, nx), dtype=torch.float64, generator=g)
+    dv = dev()
+    x = torch.full_like(d, float("nan")).to(dv)
+    with tdma.Plan(nx, ny, nz, 1, 0, axis=tdma.TDMA_AXIS_X, periodic=1 if periodic else 0, shared_leaf_rows=leaf) as plan:
+        for _ in range(2):
+            plan.solve_shared(*[t.to(dv) for t in (a1, b01, c1, sy, sz)], d.to(dv), x)
+        torch.cuda.synchronize()
+        assert plan.get(tdma.TDMA_GET_SHARED_LEAF_ROWS) == (leaf if leaf else (32 if nx >= 32 else 16))
+    a = a1.view(1, 1, nx).expand(nz, ny, nx).contiguous().numpy()
+    c = c1.view(1, 1, nx).expand(nz, ny, nx).contiguous().numpy()
+    b = (b01.view(1, 1, nx) - (sy.view(1, ny, 1) + sz.view(nz, 1, 1))).expand(nz, ny, nx).contiguous().numpy()
+    xn = x.cpu().numpy()
+    ref = oracle.solve_axis(a, b, c, d.numpy(), "x", periodic)
+    err = (np.max(np.abs(xn - ref), axis=2) / np.max(np.abs(ref), axis=2)).max()
+    assert np.isfinite(xn).all() and err <= TOL_E, err
+
+
+def test_shared_x_sweep_in_place_and_pinned():
+    """x = d in place, and the pinned row 0 of line (0, 0) in an x sweep."""
+    nz, ny, nx = 3, 20, 128
+    g = torch.Generator().manual_seed(77)
+    u = lambda k, lo, hi: lo + (hi - lo) * torch.rand(k, dtype=torch.float64, generator=g)
+    a1, c1, b01 = u(nx, -1, 1), u(nx, -1, 1), u(nx, 2.5, 3.5)
+    sy, sz = -u(ny, 0, 2), -u(nz, 0, 2)
+    d = torch.randn((nz, ny, nx), dtype=torch.float64, generator=g)
+    dv = dev()
+    x = d.clone().to(dv)
+    with tdma.Plan(nx, ny, nz, 1, 0, axis=tdma.TDMA_AXIS_X) as plan:
+        plan.solve_shared(*[t.to(dv) for t in (a1, b01, c1, sy, sz)], x, x, pin00=True)
+        torch.cuda.synchronize()
+    a = a1.view(1, 1, nx).expand(nz, ny, nx).contiguous().numpy()
+    c = c1.view(1, 1, nx).expand(nz, ny, nx).contiguous().numpy()
+    b = (b01.view(1, 1, nx) - (sy.view(1, ny, 1) + sz.view(nz, 1, 1))).expand(nz, ny, nx).contiguous().numpy()
+    b[0, 0, 0] = 1.0
+    c[0, 0, 0] = 0.0
+    ref = oracle.solve_axis(a, b, c, d.numpy(), "x", False)
+    xn = x.cpu().numpy()
+    err = (np.max(np.abs(xn - ref), axis=2) / np.max(np.abs(ref), axis=2)).max()
+    assert np.isfinite(xn).all() and err <= TOL_E, err
