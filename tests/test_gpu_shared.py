@@ -323,3 +323,37 @@ def test_shared_x_sweep_in_place_and_pinned():
     xn = x.cpu().numpy()
     err = (np.max(np.abs(xn - ref), axis=2) / np.max(np.abs(ref), axis=2)).max()
     assert np.isfinite(xn).all() and err <= TOL_E, err
+
+
+def test_cfg4_adi_full_size_in_shared_form_sampled():
+    """BASELINE cfg 4 at FULL size (512^3) in the matrix-sharing form `bench.py --adi` times
+    (PAPER.md:318): x periodic -> y Dirichlet -> z periodic with a = c = -alpha, b = 1 + 2 alpha as 1-D
+    arrays and zero shifts; every sweep against oracle.solve_axis on sampled z-slices / y-planes."""
+    w = tdma_inputs.make_workload("cfg4_adi_y", device=dev())
+    dv = dev()
+    alpha = float(w.meta["alpha"])
+    coef = lambda n: (torch.full((n,), -alpha, dtype=torch.float64, device=dv),
+                      torch.full((n,), 1.0 + 2.0 * alpha, dtype=torch.float64, device=dv),
+                      torch.full((n,), -alpha, dtype=torch.float64, device=dv))
+    zero = lambda n: torch.zeros(n, dtype=torch.float64, device=dv)
+    src = w.d
+    for axis, name, periodic, n, lanes, nsl in ((tdma.TDMA_AXIS_X, "x", 1, w.nx, w.ny, w.nz),
+                                                (tdma.TDMA_AXIS_Y, "y", 0, w.ny, w.nx, w.nz),
+                                                (tdma.TDMA_AXIS_Z, "z", 1, w.nz, w.nx, w.ny)):
+        dst = torch.full_like(w.d, float("nan"))
+        with tdma.Plan(w.nx, w.ny, w.nz, 1, 0, axis=axis, periodic=periodic) as plan:
+            plan.solve_shared(*coef(n), zero(lanes), zero(nsl), src, dst)
+            torch.cuda.synchronize()
+            fill = plan.get(tdma.TDMA_GET_SHARED_FILL)
+        assert bool(torch.isfinite(dst).all())
+        picks = {0, 1, nsl // 2 + 1, nsl - 1}
+        if fill > 0:
+            picks |= {nsl - fill, nsl - fill - 1}
+        ax = {"y": 1, "z": 0, "x": 2}[name]
+        for q in sorted(picks):
+            sl = (slice(None), slice(q, q + 1)) if name == "z" else (slice(q, q + 1),)
+            an, bn, cn, dn, xn = [t[sl].cpu().numpy() for t in (w.a, w.b, w.c, src, dst)]
+            ref = oracle.solve_axis(an, bn, cn, dn, name, bool(periodic))
+            err = (np.max(np.abs(xn - ref), axis=ax) / np.max(np.abs(ref), axis=ax)).max()
+            assert err <= TOL_E, (name, q, err)
+        src = dst
