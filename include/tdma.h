@@ -326,6 +326,23 @@ int tdma_slab_stage_b(tdma_slab *slab, int batch_index, const void *recv, void *
 /* the same with the PDD reduced solve (tdma_options.pdd): independent 2 x 2 interface systems */
 int tdma_slab_stage_b_pdd(tdma_slab *slab, int batch_index, const void *recv, void *yout, void *stream);
 int tdma_slab_stage_c(tdma_slab *slab, int batch_index, const void *yrecv, void *x, void *stream);
+/* Stages fused with their all-to-all: instead of filling a send / yout buffer that a
+ * collective then redistributes, the kernels store block `dest` of it straight into rank dest's
+ * receive buffer -- peer memory mapped into this process (NVLink P2P / symmetric memory), or any
+ * device pointer -- at the place the all-to-all would have put it: block [src = rank] of
+ * recv[src][P][6][Ls] / yrecv[src][2P][Ls].  The transfer then overlaps the stage tile by tile; what is
+ * left of the exchange is ordering: the CALLER makes every rank's stage A (B) of batch n complete
+ * and visible before any rank's stage B (C) of that batch reads its buffer (a cross-rank barrier
+ * on the stream), and keeps a receive buffer unwritten by batch n + 3 until its reader is done.
+ * tdma_slab_set_peers(slab, slot, recv_of_rank, yrecv_of_rank): HOST arrays of nranks DEVICE
+ * pointers, rank q's recv and yrecv buffer of ring slot `slot` (0..2; batch n uses slot n % 3);
+ * copied to the device synchronously -- call it once per slot before the first batch.
+ * _stage_a_peer / _stage_b_peer (pdd != 0: the PDD reduced solve) = _stage_a / _stage_b with the
+ * output redirected; TDMA_ERR_INVALID_ARG before set_peers for the batch's slot. */
+int tdma_slab_set_peers(tdma_slab *slab, int slot, const void *const *recv_of_rank, const void *const *yrecv_of_rank);
+int tdma_slab_stage_a_peer(tdma_slab *slab, int batch_index, const void *a, const void *b, const void *c,
+                           const void *d, void *stream);
+int tdma_slab_stage_b_peer(tdma_slab *slab, int batch_index, const void *recv, int pdd, void *stream);
 int tdma_slab_destroy(tdma_slab *slab);
 
 /* fp64 ALU probe: measures on the current device and writes to result[0..5]

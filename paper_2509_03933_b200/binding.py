@@ -36,7 +36,7 @@ EXPORTED_SYMBOLS = (
     "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
     "tdma_solve_shared", "tdma_probe_fp64",
     "tdma_slab_create", "tdma_slab_get", "tdma_slab_stage_a", "tdma_slab_stage_b", "tdma_slab_stage_b_pdd", "tdma_slab_stage_c",
-    "tdma_slab_destroy",
+    "tdma_slab_set_peers", "tdma_slab_stage_a_peer", "tdma_slab_stage_b_peer", "tdma_slab_destroy",
 )
 (TDMA_SLAB_NB, TDMA_SLAB_BATCH, TDMA_SLAB_LINES, TDMA_SLAB_SHARE, TDMA_SLAB_PTOT, TDMA_SLAB_PLOCAL,
  TDMA_SLAB_TMA) = range(7)
@@ -107,6 +107,12 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_slab_stage_b_pdd.restype = ci
     lib.tdma_slab_stage_c.argtypes = [vp, ci] + [vp] * 3
     lib.tdma_slab_stage_c.restype = ci
+    lib.tdma_slab_set_peers.argtypes = [vp, ci, ctypes.POINTER(vp), ctypes.POINTER(vp)]
+    lib.tdma_slab_set_peers.restype = ci
+    lib.tdma_slab_stage_a_peer.argtypes = [vp, ci] + [vp] * 5
+    lib.tdma_slab_stage_a_peer.restype = ci
+    lib.tdma_slab_stage_b_peer.argtypes = [vp, ci, vp, ci, vp]
+    lib.tdma_slab_stage_b_peer.restype = ci
     lib.tdma_slab_destroy.argtypes = [vp]
     lib.tdma_slab_destroy.restype = ci
     lib.tdma_probe_fp64.argtypes = [ctypes.POINTER(ctypes.c_double), ci]
@@ -241,6 +247,26 @@ def tdma_slab_stage_b_pdd(slab: int, batch_index: int, recv, yout, stream=None) 
 
 def tdma_slab_stage_c(slab: int, batch_index: int, yrecv, x, stream=None) -> None:
     _check(load_library().tdma_slab_stage_c(slab, batch_index, _ptr(yrecv), _ptr(x), _stream_handle(stream)))
+
+
+def tdma_slab_set_peers(slab: int, slot: int, recv_of_rank, yrecv_of_rank) -> None:
+    """recv_of_rank / yrecv_of_rank: per rank, a tensor or an integer device address."""
+    addr = lambda t: int(t) if isinstance(t, int) else int(t.data_ptr())
+    n = len(recv_of_rank)
+    if len(yrecv_of_rank) != n:
+        raise ValueError("one recv and one yrecv buffer per rank")
+    r = (ctypes.c_void_p * n)(*[addr(t) for t in recv_of_rank])
+    y = (ctypes.c_void_p * n)(*[addr(t) for t in yrecv_of_rank])
+    _check(load_library().tdma_slab_set_peers(slab, slot, r, y))
+
+
+def tdma_slab_stage_a_peer(slab: int, batch_index: int, a, b, c, d, stream=None) -> None:
+    _check(load_library().tdma_slab_stage_a_peer(slab, batch_index, _ptr(a), _ptr(b), _ptr(c), _ptr(d),
+                                                 _stream_handle(stream)))
+
+
+def tdma_slab_stage_b_peer(slab: int, batch_index: int, recv, pdd: bool = False, stream=None) -> None:
+    _check(load_library().tdma_slab_stage_b_peer(slab, batch_index, _ptr(recv), 1 if pdd else 0, _stream_handle(stream)))
 
 
 def tdma_slab_destroy(slab: int) -> None:

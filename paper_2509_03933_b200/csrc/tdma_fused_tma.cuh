@@ -100,6 +100,10 @@ struct TmaFusedParams {
     // (red_y), dest = src = line / Ls, Pl = exchanged partitions of this rank
     int row0 = 0, ny_total = 0, Pl = 0;
     long long Ls = 0;
+    // peer stores (tdma_slab_stage_a_peer): block `dest` of the send buffer is written straight into
+    // rank dest's receive buffer, red_peer[dest] + red_peer_off (device table of nranks pointers)
+    double *const *red_peer = nullptr;
+    long long red_peer_off = 0;
 };
 
 // Dynamic shared memory of one CTA: NA ring slots of one raw array [R][TX] each, the x staging
@@ -1120,7 +1124,8 @@ fused_tma_kernel(const __grid_constant__ CUtensorMap tm_a, const __grid_constant
                 const double invf = 1.0 / abf.y, invl = 1.0 / abl.y;
                 if (prm.Ls > 0) {       // y-slab: send[dest][Pl][6][Ls] = (fa, fc, fd | pa, pc, pd)
                     const long long dest = red_l / prm.Ls, j = red_l - dest * prm.Ls;
-                    double *sp = prm.red_a + ((dest * prm.Pl + pg) * 6 * prm.Ls + j);
+                    double *sp = prm.red_peer ? prm.red_peer[dest] + (prm.red_peer_off + (long long)pg * 6 * prm.Ls + j)
+                                              : prm.red_a + ((dest * prm.Pl + pg) * 6 * prm.Ls + j);
                     __stcg(sp, abf.x * invf); __stcg(sp + prm.Ls, cdf.x * invf); __stcg(sp + 2 * prm.Ls, cdf.y * invf);
                     __stcg(sp + 3 * prm.Ls, abl.x * invl); __stcg(sp + 4 * prm.Ls, cdl.x * invl); __stcg(sp + 5 * prm.Ls, cdl.y * invl);
                 } else {

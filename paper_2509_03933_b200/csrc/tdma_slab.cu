@@ -4,8 +4,11 @@
 // every rank solves a share of the reduced systems (stage B; "even distribution", PAPER.md:106,
 // Alg. 2 :179-203), a second all-to-all returns the two boundary unknowns per partition and the
 // ranks back-substitute (stage C).  This unit holds the rank-local stages; the exchange itself is
-// the caller's (torch.distributed all_to_all_single over NCCL in yslab.py: the transfers are a few
-// MiB per batch, so the library collective on its own stream is the right tool).
+// the caller's: either a library all-to-all between the stages (torch.distributed
+// all_to_all_single over NCCL in yslab.py), or -- tdma_slab_set_peers + the _peer entry points --
+// NO separate exchange at all: stage A and stage B store every block of their output straight
+// into the destination rank's receive buffer (peer memory over NVLink, or the same device), so
+// the transfer overlaps the stage tile by tile and only a cross-rank barrier remains.
 //
 // Buffers of one batch (Lb = nx * slices lines, Ls = Lb / nranks lines per rank, P = local
 // partitions per rank, Ptot = P * nranks; all doubles, line fastest):
@@ -42,6 +45,8 @@ struct tdma_slab {
     const double *in[kSlabDepth][4] = {};   // a, b, c, d of the batch in each ring slot (tma: for stage C)
     double *scratch = nullptr;   // depth x {a', c', d'} x [bz][ny][nx]   (not with tma)
     double *red = nullptr;       // depth x {RA, RC, RD, CP} x [2 Ptot][Ls]
+    double **peer_tab = nullptr; // device: depth x {recv, yrecv} x [nranks] pointers (tdma_slab_set_peers)
+    bool have_peers[kSlabDepth] = {};
     size_t workspace = 0;
 };
 
@@ -139,12 +144,36 @@ int tdma_slab_get(const tdma_slab *s, int what)
     }
 }
 
-int tdma_slab_stage_a(tdma_slab *s, int batch_index, const void *a, const void *b, const void *c,
-                      const void *d, void *send, void *stream)
+int tdma_slab_set_peers(tdma_slab *s, int slot, const void *const *recv_of_rank, const void *const *yrecv_of_rank)
+{
+    if (!s || slot < 0 || slot >= kSlabDepth || !recv_of_rank || !yrecv_of_rank) return slab_err(TDMA_ERR_INVALID_ARG);
+    for (int q = 0; q < s->nranks; ++q)
+        if (!recv_of_rank[q] || !yrecv_of_rank[q] || (((uintptr_t)recv_of_rank[q] | (uintptr_t)yrecv_of_rank[q]) & 7) != 0)
+            return slab_err(TDMA_ERR_INVALID_ARG);
+    if (!s->peer_tab && cudaMalloc(&s->peer_tab, (size_t)kSlabDepth * 2 * s->nranks * sizeof(double *)) != cudaSuccess) {
+        cudaGetLastError();
+        return slab_err(TDMA_ERR_ALLOC);
+    }
+    double **row = s->peer_tab + (size_t)slot * 2 * s->nranks;
+    // synchronous copies: the table is set up once, before the first batch
+    if (cudaMemcpy(row, recv_of_rank, (size_t)s->nranks * sizeof(double *), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(row + s->nranks, yrecv_of_rank, (size_t)s->nranks * sizeof(double *), cudaMemcpyHostToDevice) != cudaSuccess)
+        return slab_err(TDMA_ERR_CUDA);
+    s->have_peers[slot] = true;
+    return TDMA_OK;
+}
+
+static int slab_stage_a(tdma_slab *s, int batch_index, const void *a, const void *b, const void *c,
+                        const void *d, void *send, void *stream, bool peer)
 {
     int k0, bzn;
-    if (!s || !a || !b || !c || !d || !send || !batch_range(s, batch_index, &k0, &bzn)) return slab_err(TDMA_ERR_INVALID_ARG);
+    if (!s || !a || !b || !c || !d || (!send && !peer) || !batch_range(s, batch_index, &k0, &bzn)) return slab_err(TDMA_ERR_INVALID_ARG);
+    if (peer && !s->have_peers[batch_index % kSlabDepth]) return slab_err(TDMA_ERR_INVALID_ARG);
     tdma::StageParams prm = slab_params(s, batch_index, k0, bzn);
+    if (peer) {     // my block [src = rank] of every receiver's recv[src][P][6][Ls]
+        prm.peer = s->peer_tab + (size_t)(batch_index % kSlabDepth) * 2 * s->nranks;
+        prm.peer_off = (long long)s->rank * s->P * 6 * prm.Ls;
+    }
     const size_t off = (size_t)k0 * (size_t)prm.os;
     prm.a = (const double *)a + off; prm.b = (const double *)b + off;
     prm.c = (const double *)c + off; prm.d = (const double *)d + off;
@@ -154,7 +183,8 @@ int tdma_slab_stage_a(tdma_slab *s, int batch_index, const void *a, const void *
         const int slot = batch_index % kSlabDepth;
         s->in[slot][0] = prm.a; s->in[slot][1] = prm.b; s->in[slot][2] = prm.c; s->in[slot][3] = prm.d;
         cudaError_t e = tdma::launch_staged_slab(s->staged, 1, prm.a, prm.b, prm.c, prm.d, nullptr, prm.send, nullptr, s->nx,
-                                                 s->ny, bzn, s->rank * s->ny, s->ny * s->nranks, prm.Ls, (cudaStream_t)stream);
+                                                 s->ny, bzn, s->rank * s->ny, s->ny * s->nranks, prm.Ls, (cudaStream_t)stream,
+                                                 prm.peer, prm.peer_off);
         return e == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
     }
     dim3 grid((unsigned)((prm.Lb + 127) / 128), s->P);
@@ -162,11 +192,29 @@ int tdma_slab_stage_a(tdma_slab *s, int batch_index, const void *a, const void *
     return cudaGetLastError() == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;
 }
 
-static int slab_stage_b(tdma_slab *s, int batch_index, const void *recv, void *yout, void *stream, bool pdd)
+int tdma_slab_stage_a(tdma_slab *s, int batch_index, const void *a, const void *b, const void *c,
+                      const void *d, void *send, void *stream)
+{
+    return slab_stage_a(s, batch_index, a, b, c, d, send, stream, false);
+}
+
+int tdma_slab_stage_a_peer(tdma_slab *s, int batch_index, const void *a, const void *b, const void *c,
+                           const void *d, void *stream)
+{
+    return slab_stage_a(s, batch_index, a, b, c, d, nullptr, stream, true);
+}
+
+static int slab_stage_b(tdma_slab *s, int batch_index, const void *recv, void *yout, void *stream, bool pdd, bool peer = false)
 {
     int k0, bzn;
-    if (!s || !recv || !yout || !batch_range(s, batch_index, &k0, &bzn)) return slab_err(TDMA_ERR_INVALID_ARG);
+    if (!s || !recv || (!yout && !peer) || !batch_range(s, batch_index, &k0, &bzn)) return slab_err(TDMA_ERR_INVALID_ARG);
+    if (peer && !s->have_peers[batch_index % kSlabDepth]) return slab_err(TDMA_ERR_INVALID_ARG);
     tdma::StageParams prm = slab_params(s, batch_index, k0, bzn);
+    if (peer) {     // my block [src = rank] of every receiver's yrecv[src][2 P][Ls]
+        prm.peer = s->peer_tab + ((size_t)(batch_index % kSlabDepth) * 2 + 1) * s->nranks;
+        prm.peer_off = (long long)s->rank * 2 * s->P * prm.Ls;
+        prm.peer_rows = 2 * s->P;
+    }
     // the reduced systems of MY share: Ls lines of 2 Ptot rows; recv is send_A[Ptot][6][Ls]
     prm.send = (double *)const_cast<void *>(recv);
     prm.y = (double *)yout;
@@ -194,6 +242,11 @@ int tdma_slab_stage_b_pdd(tdma_slab *s, int batch_index, const void *recv, void 
     return slab_stage_b(s, batch_index, recv, yout, stream, true);
 }
 
+int tdma_slab_stage_b_peer(tdma_slab *s, int batch_index, const void *recv, int pdd, void *stream)
+{
+    return slab_stage_b(s, batch_index, recv, nullptr, stream, pdd != 0, true);
+}
+
 int tdma_slab_stage_c(tdma_slab *s, int batch_index, const void *yrecv, void *x, void *stream)
 {
     int k0, bzn;
@@ -218,7 +271,7 @@ int tdma_slab_destroy(tdma_slab *s)
 {
     if (!s) return TDMA_ERR_INVALID_ARG;
     cudaError_t e = cudaDeviceSynchronize();
-    cudaFree(s->scratch); cudaFree(s->red);
+    cudaFree(s->scratch); cudaFree(s->red); cudaFree(s->peer_tab);
     if (s->staged.impl) tdma::free_staged(&s->staged);
     delete s;
     return e == cudaSuccess ? TDMA_OK : TDMA_ERR_CUDA;

@@ -48,7 +48,24 @@ struct StageParams {
     // of Ptot; the lines of a batch are dealt out evenly, Ls to each rank (single GPU: 0, P, 0)
     int pg0 = 0, Ptot = 0;
     long long Ls = 0;
+    // peer stores (tdma_slab_stage_a_peer / _b_peer): the block of the send / yout buffer meant for
+    // rank q is written straight into rank q's receive buffer, peer[q] + peer_off (device table of
+    // nranks pointers; peer_off = this rank's block in the receiver's [src] layout); peer_rows =
+    // rows of Ls doubles per block of yout (2 P_local)
+    double *const *peer = nullptr;
+    long long peer_off = 0;
+    int peer_rows = 0;
 };
+
+// row q of stage B's solution for line l (slab: yout[dest][2 P_local][Ls], or the peer's yrecv block)
+__device__ __forceinline__ double *y_row(const StageParams &prm, int q, long long l)
+{
+    if (prm.peer) {
+        const int dest = q / prm.peer_rows;
+        return prm.peer[dest] + (prm.peer_off + (long long)(q - dest * prm.peer_rows) * prm.Lb + l);
+    }
+    return prm.y + (size_t)q * (size_t)prm.Lb + l;
+}
 
 // where stage A's two boundary equations per (line, partition) go
 enum { kOutReduced = 0,   // RA / RC / RD rows 2p, 2p+1 (gather fused into the epilogue)
@@ -146,7 +163,8 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
         st_keep(sp + 3 * Lb, pa); st_keep(sp + 4 * Lb, pc); st_keep(sp + 5 * Lb, pd);
     } else if (kOut == kOutSlab) {
         const size_t Ls = (size_t)prm.Ls, dest = (size_t)l / Ls, j = (size_t)l - dest * Ls;
-        double *__restrict__ sp = prm.send + ((dest * prm.P + p) * 6) * Ls + j;
+        double *__restrict__ sp = prm.peer ? prm.peer[dest] + ((size_t)prm.peer_off + (size_t)p * 6 * Ls + j)
+                                           : prm.send + ((dest * prm.P + p) * 6) * Ls + j;
         st_keep(sp, fa * inv); st_keep(sp + Ls, fc * inv); st_keep(sp + 2 * Ls, fd * inv);
         st_keep(sp + 3 * Ls, pa); st_keep(sp + 4 * Ls, pc); st_keep(sp + 5 * Ls, pd);
     } else {
@@ -185,12 +203,14 @@ __global__ void __launch_bounds__(64) stage_b_kernel(const StageParams prm)
     const int Q = 2 * prm.P;
     const double *__restrict__ ra = prm.ra + l;
     const double *__restrict__ rc = prm.rc + l;
-    const double *__restrict__ rd = prm.rd + l;
+    const double *rd = prm.rd + l;
     double *__restrict__ cpb = prm.cp + l;
-    double *__restrict__ y = prm.y + l;
+    // the forward-eliminated right-hand side d' is parked in y; with peer stores y is remote memory
+    // that is written once, and d' overwrites RD in place (row q is stored after it was loaded)
+    double *tmp = prm.peer ? prm.rd + l : prm.y + l;
 
     double cp = ld_keep(rc), dp = ld_keep(rd);          // row 0: sub-diagonal is 0
-    st_keep(cpb, cp); st_keep(y, dp);
+    st_keep(cpb, cp); st_keep(tmp, dp);
     double na[U], nc[U], nd[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
@@ -214,15 +234,16 @@ __global__ void __launch_bounds__(64) stage_b_kernel(const StageParams prm)
                 dp = fma(-ca[u], dp, cd[u]) * inv;
                 cp = cc[u] * inv;
                 st_keep(cpb + q * Lb, cp);
-                st_keep(y + q * Lb, dp);
+                st_keep(tmp + q * Lb, dp);
             }
         }
     }
     // back substitution; the last row's cp is 0 by construction (c_{ny-1} := 0)
     double xq = dp;
+    st_keep(y_row(prm, Q - 1, l), xq);
     for (int q = Q - 2; q >= 0; --q) {
-        xq = fma(-ld_keep(cpb + q * Lb), xq, ld_keep(y + q * Lb));
-        st_keep(y + q * Lb, xq);
+        xq = fma(-ld_keep(cpb + q * Lb), xq, ld_keep(tmp + q * Lb));
+        st_keep(y_row(prm, q, l), xq);
     }
 }
 
@@ -270,8 +291,8 @@ static __global__ void __launch_bounds__(128) stage_b_pdd_kernel(const StagePara
         const SpikeEnds hi = spike_ends(prm.ra, prm.rc, prm.rd, (size_t)(2 * p + 2) * Lb + l, Lb);
         y_next = fma(-hi.v0, me.xtl, hi.xt0) / fma(-me.wl, hi.v0, 1.0);
     }
-    st_keep(prm.y + (size_t)(2 * p) * Lb + l, fma(-me.w0, y_next, fma(-me.v0, y_prev, me.xt0)));
-    st_keep(prm.y + (size_t)(2 * p + 1) * Lb + l, fma(-me.wl, y_next, fma(-me.vl, y_prev, me.xtl)));
+    st_keep(y_row(prm, 2 * p, l), fma(-me.w0, y_next, fma(-me.v0, y_prev, me.xt0)));
+    st_keep(y_row(prm, 2 * p + 1, l), fma(-me.wl, y_next, fma(-me.vl, y_prev, me.xtl)));
 }
 
 // ------------------------------------------------------------------------------------------

@@ -57,7 +57,7 @@ static cudaError_t launch_staged_tx(TmaFusedConfig &t, const CUtensorMap *tm, co
 static cudaError_t launch_staged_any(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
                                      const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
                                      int nx, int ny, int nzs, long long rs, long long os, bool axis_z, int row0,
-                                     int ny_total, long long Ls, cudaStream_t st)
+                                     int ny_total, long long Ls, double *const *peer, long long peer_off, cudaStream_t st)
 {
     if (stage != 1 && stage != 2) return cudaErrorInvalidValue;
     TmaFusedConfig &t = static_cast<TmaFusedConfig *>(cfg.impl)[stage - 1];
@@ -77,6 +77,7 @@ static cudaError_t launch_staged_any(StagedConfig &cfg, int stage, const double 
     prm.Lb = (long long)nx * nzs;
     prm.lp = cfg.lp; prm.lp_shift = cfg.lp_shift;
     prm.row0 = row0; prm.ny_total = ny_total; prm.Ls = Ls; prm.Pl = cfg.Pe;
+    prm.red_peer = peer; prm.red_peer_off = peer_off;
     cudaError_t e;
     if (stage == 1) {
         switch (t.lines) {
@@ -100,15 +101,16 @@ cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const d
                           const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
                           int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st)
 {
-    return launch_staged_any(cfg, stage, a, b, c, d, x, ra, rc, rd, y, nx, ny, nzs, rs, os, axis_z, 0, 0, 0, st);
+    return launch_staged_any(cfg, stage, a, b, c, d, x, ra, rc, rd, y, nx, ny, nzs, rs, os, axis_z, 0, 0, 0, nullptr, 0, st);
 }
 
 cudaError_t launch_staged_slab(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
                                const double *d, double *x, double *send, const double *yrecv, int nx, int ny,
-                               int nzs, int row0, int ny_total, long long Ls, cudaStream_t st)
+                               int nzs, int row0, int ny_total, long long Ls, cudaStream_t st, double *const *peer,
+                               long long peer_off)
 {
     return launch_staged_any(cfg, stage, a, b, c, d, x, send, nullptr, nullptr, yrecv, nx, ny, nzs, (long long)nx,
-                             (long long)nx * ny, false, row0, ny_total, Ls, st);
+                             (long long)nx * ny, false, row0, ny_total, Ls, peer, peer_off, st);
 }
 
 }  // namespace tdma

@@ -29,6 +29,7 @@ cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const d
 // rows; stage 1 writes send[dest][Pe][6][Ls], stage 2 reads yrecv[src][2 Pe][Ls] (Ls = nx * nzs / ranks).
 cudaError_t launch_staged_slab(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
                                const double *d, double *x, double *send, const double *yrecv, int nx, int ny,
-                               int nzs, int row0, int ny_total, long long Ls, cudaStream_t st);
+                               int nzs, int row0, int ny_total, long long Ls, cudaStream_t st,
+                               double *const *peer = nullptr, long long peer_off = 0);
 
 }  // namespace tdma

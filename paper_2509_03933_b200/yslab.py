@@ -61,6 +61,16 @@ class CudaSlabStages:
     def stage_c(self, n, yrecv, x, stream=None):
         _b.tdma_slab_stage_c(self.handle, n, yrecv, x, stream)
 
+    # stages fused with their exchange: the output goes straight into the receivers' buffers
+    def set_peers(self, slot, recv_of_rank, yrecv_of_rank):
+        _b.tdma_slab_set_peers(self.handle, slot, recv_of_rank, yrecv_of_rank)
+
+    def stage_a_peer(self, n, a, b, c, d, stream=None):
+        _b.tdma_slab_stage_a_peer(self.handle, n, a, b, c, d, stream)
+
+    def stage_b_peer(self, n, recv, stream=None):
+        _b.tdma_slab_stage_b_peer(self.handle, n, recv, self.pdd, stream)
+
     def close(self):
         if self.handle:
             _b.tdma_slab_destroy(self.handle)

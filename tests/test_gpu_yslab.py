@@ -153,3 +153,79 @@ def test_slab_create_rejects_bad_shapes():
                  (16, 32, 4, 1, 0, 2, 2)]:     # rank out of range
         with pytest.raises(tdma.TdmaError):
             tdma.tdma_slab_create(*args)
+
+
+def emulate_peer(a, b, c, d, nranks, P_local, batch, pdd=False):
+    """The same job with the stages storing straight into the receivers' buffers
+    (tdma_slab_set_peers + _stage_a_peer / _stage_b_peer): no send / yout buffer, no permutation.  All
+    "ranks" live on this GPU, so the peer pointers are plain device pointers.  Returns x and, per batch,
+    every rank's recv and yrecv buffer."""
+    nz, ny, nx = a.shape
+    nyl = ny // nranks
+    loc = [[t[:, r * nyl:(r + 1) * nyl, :].contiguous() for t in (a, b, c, d)] for r in range(nranks)]
+    xs = [torch.full_like(loc[r][3], float("nan")) for r in range(nranks)]
+    st = [CudaSlabStages(nx, nyl, nz, P_local, batch, r, nranks, pdd=pdd) for r in range(nranks)]
+    P = st[0].P
+    lb0, ls0 = st[0].batch_lines(0)
+    mk = lambda rows: [[torch.full((nranks * rows * ls0,), float("nan"), dtype=torch.float64, device=a.device)
+                        for _ in range(nranks)] for _ in range(3)]
+    recv, yrecv = mk(P * 6), mk(2 * P)                      # [slot][rank]
+    kept = []
+    try:
+        for slot in range(3):
+            for s in st:
+                s.set_peers(slot, recv[slot], yrecv[slot])
+        for n in range(st[0].nb):
+            slot = n % 3
+            lb, ls = st[0].batch_lines(n)
+            for r in range(nranks):
+                st[r].stage_a_peer(n, *loc[r])
+            for q in range(nranks):
+                st[q].stage_b_peer(n, recv[slot][q])
+            for r in range(nranks):
+                st[r].stage_c(n, yrecv[slot][r], xs[r])
+            torch.cuda.synchronize()
+            kept.append((n, ls, [t[:nranks * P * 6 * ls].clone() for t in recv[slot]],
+                         [t[:nranks * 2 * P * ls].clone() for t in yrecv[slot]]))
+    finally:
+        for s in st:
+            s.close()
+    return torch.cat(xs, dim=1), kept, P
+
+
+@pytest.mark.parametrize("pdd", [False, True], ids=["thomas", "pdd"])
+@pytest.mark.parametrize("nx,ny,nranks,P_local,batch", [(64, 256, 4, 2, 3), (64, 256, 2, 4, 0), (27, 90, 3, 3, 4),
+                                                        (64, 512, 8, 1, 2)])
+def test_peer_stores_equal_the_all_to_all(nx, ny, nranks, P_local, batch, pdd):
+    """Stage A / B fused with their exchange: every rank's recv / yrecv buffer and x are BITWISE what
+    the buffered stages followed by the all-to-all (tensor permutation) produce, for the TMA-staged
+    and the thread-per-line kernels, a ragged last batch included; x against the oracle."""
+    nz = 7
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 61, dev())
+    keep = []
+    x_ref = emulate(a, b, c, d, nranks, P_local, batch, keep, pdd=pdd)
+    x, kept, P = emulate_peer(a, b, c, d, nranks, P_local, batch, pdd=pdd)
+    assert torch.equal(x, x_ref)
+    assert len(kept) == len(keep)
+    for (n, send, yout, P_ref), (n2, ls, recv, yrecv) in zip(keep, kept):
+        assert n == n2 and P == P_ref
+        for q in range(nranks):
+            want_recv = np.ascontiguousarray(send[:, q]).reshape(-1)        # recv[q][src] = send[src][dest = q]
+            want_y = np.ascontiguousarray(yout[:, q]).reshape(-1)
+            assert np.array_equal(recv[q].cpu().numpy(), want_recv)
+            assert np.array_equal(yrecv[q].cpu().numpy(), want_y)
+    an, bn, cn, dn, xn = [t.cpu().numpy() for t in (a, b, c, d, x)]
+    ref = oracle.solve_y_pdd(an, bn, cn, dn, nranks * P) if pdd else oracle.solve_y(an, bn, cn, dn)
+    assert oracle.normwise_error(xn, ref).max() <= TOL_E
+
+
+def test_peer_stages_need_their_table():
+    s = CudaSlabStages(32, 64, 2, 2, 0, 0, 2)
+    try:
+        t = torch.zeros(32 * 64 * 2, dtype=torch.float64, device=dev())
+        with pytest.raises(tdma.TdmaError):
+            s.stage_a_peer(0, t, t, t, t)
+        with pytest.raises(tdma.TdmaError):
+            s.set_peers(3, [t, t], [t, t])                   # slots 0..2
+    finally:
+        s.close()
