@@ -731,11 +731,23 @@ def yslab(torch, tdma, w, args, rank, peak):
     t_b = timed(lambda q: st.stage_b(q, recv, yout, stream))
     yrecv = yout[r].unsqueeze(0).expand(n, 2 * pl, ls).contiguous()
     t_c = timed(lambda q: st.stage_c(q, yrecv, x, stream))
+    # the stages fused with their exchange (peer stores): every block goes straight into a receiver's
+    # ring -- here n separate buffers on this GPU standing in for the n ranks' memory
+    rings = [[torch.zeros(n * pl * 6 * ls, dtype=torch.float64, device=loc[0].device) for _ in range(n)] for _ in range(3)]
+    yrings = [[torch.zeros(n * 2 * pl * ls, dtype=torch.float64, device=loc[0].device) for _ in range(n)] for _ in range(3)]
+    for slot in range(3):
+        st.set_peers(slot, rings[slot], yrings[slot])
+    t_ap = timed(lambda q: st.stage_a_peer(q, *loc, stream))
+    t_bp = timed(lambda q: st.stage_b_peer(q, recv, stream))
     st.close()
     cells = w.nx * nyl * st.bz
     out_b, back_b = 48 * pl * lb, 16 * pl * lb
     rec = {"yslab": True, "workload": args.workload, "nranks": n, "rank_timed": r, "nx": w.nx, "ny_local": nyl, "nz": w.nz,
            "batch": st.bz, "stage_ms_per_batch": {"A": t_a, "B": t_b, "C": t_c},
+           "peer_store_stage_ms_per_batch": {"A": t_ap, "B": t_bp,
+                                             "note": "stage A / B storing straight into n receive rings (all on this GPU): "
+                                                     "no send / yout buffer and no all-to-all; what a real job adds is "
+                                                     "NVLink store latency and one barrier per exchange"},
            "stage_kernels": "tma-staged (stage A 32 B/cell, stage C 40 B/cell, nothing spilled)" if tma else
                             "one thread per (line, partition) (stage A 56 B/cell, stage C 32 B/cell, a', c', d' through HBM)",
            "stage_gbs": {"A": (32.0 if tma else 56.0) * cells / t_a / 1e6, "C": (40.0 if tma else 32.0) * cells / t_c / 1e6},

@@ -16,6 +16,15 @@ Schedule (Alg. 2 with events instead of stream synchronisation), iteration n = 0
 so the reduced solve and both exchanges of a batch run behind the partition stages of its
 neighbours.  Ring of 3 buffer slots ("three batched systems concurrently").
 
+Peer mode (``exchange=``): no all-to-all at all.  The receive buffers live in memory every rank can
+store into (``SymmMemExchange``: torch symmetric memory, NVLink peer mappings), stage A and stage B
+write every block of their output straight into its receiver's buffer (``tdma_slab_stage_a_peer`` /
+``_b_peer``), so the transfer overlaps the stage tile by tile, and each exchange shrinks to one
+cross-rank barrier on the communication stream.  Ring hazards need no extra edges: A(n) follows
+C(n-3) on its stream, C(n-3) waited for the barrier behind every rank's B(n-3), so recv[slot] is
+free on every rank when A(n) stores into it; likewise every rank's A(n) follows its C(n-3), and
+B(n) waits for the barrier behind all A(n), so yrecv[slot] is free when B(n) stores into it.
+
 UNMEASURED ON HARDWARE with more than one GPU: this container and its GPU box have one device.
 What is tested: the stages and their buffer layouts on one B200 with the ranks' exchanges emulated
 by tensor permutation (tests/test_gpu_yslab.py), and this driver with two ``gloo`` ranks on the
@@ -77,13 +86,59 @@ class CudaSlabStages:
             self.handle = 0
 
 
+class LocalExchange:
+    """Peer-mode plumbing of a single rank: its own buffers, nothing to wait for."""
+
+    def __init__(self, device):
+        self.device = device
+
+    def alloc(self, n: int) -> torch.Tensor:
+        return torch.empty(n, dtype=torch.float64, device=self.device)
+
+    def peers(self, t: torch.Tensor):
+        return [t]
+
+    def barrier(self):
+        pass
+
+
+class SymmMemExchange:
+    """Peer-mode plumbing over torch symmetric memory (one process per GPU, NVLink peer mappings):
+    ``alloc`` is collective and returns this rank's buffer, ``peers`` the device addresses of every
+    rank's copy, ``barrier`` a device-side barrier over all ranks on the current stream.
+    UNMEASURED: needs more than one GPU."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        import torch.distributed._symmetric_memory as symm
+        self.symm, self.group = symm, group if group is not None else dist.group.WORLD
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        self.handles = {}
+        self.first = None
+
+    def alloc(self, n: int) -> torch.Tensor:
+        t = self.symm.empty(n, dtype=torch.float64, device=self.device)
+        h = self.symm.rendezvous(t, self.group)
+        self.handles[t.data_ptr()] = h
+        self.first = self.first or h
+        return t
+
+    def peers(self, t: torch.Tensor):
+        return [int(p) for p in self.handles[t.data_ptr()].buffer_ptrs]
+
+    def barrier(self):
+        self.first.barrier(channel=0)
+
+
 class YSlabSolver:
     """Pipelined y-slab solve of one rank.  ``stages``: the rank-local stages (default: the CUDA
     kernels through the C ABI); ``group``: a torch.distributed process group (None = default group;
-    with no initialised process group a single rank runs alone and the exchange is a local copy)."""
+    with no initialised process group a single rank runs alone and the exchange is a local copy);
+    ``exchange``: None = the two all-to-alls per batch; an object with ``alloc / peers / barrier``
+    (``SymmMemExchange``, ``LocalExchange``) = peer mode, see the module docstring."""
 
     def __init__(self, nx: int, ny_local: int, nz: int, P_local: int = 1, batch: int = 0, group=None,
-                 stages=None, pdd: bool = False):
+                 stages=None, pdd: bool = False, exchange=None):
         import torch.distributed as dist
         self.dist = dist if dist.is_available() and dist.is_initialized() else None
         self.group = group
@@ -96,8 +151,16 @@ class YSlabSolver:
         self.cuda = self.device.type == "cuda"
         lb, ls = self.stages.batch_lines(0)
         mk = lambda n: [torch.empty(n, dtype=torch.float64, device=self.device) for _ in range(DEPTH)]
-        self.send, self.recv = mk(self.nranks * P_local * 6 * ls), mk(self.nranks * P_local * 6 * ls)
-        self.yout, self.yrecv = mk(self.nranks * 2 * P_local * ls), mk(self.nranks * 2 * P_local * ls)
+        self.exchange = exchange
+        if exchange is None:
+            self.send, self.recv = mk(self.nranks * P_local * 6 * ls), mk(self.nranks * P_local * 6 * ls)
+            self.yout, self.yrecv = mk(self.nranks * 2 * P_local * ls), mk(self.nranks * 2 * P_local * ls)
+        else:       # receive rings only, in memory the other ranks store into (same allocation order on every rank)
+            self.recv = [exchange.alloc(self.nranks * P_local * 6 * ls) for _ in range(DEPTH)]
+            self.yrecv = [exchange.alloc(self.nranks * 2 * P_local * ls) for _ in range(DEPTH)]
+            for slot in range(DEPTH):
+                self.stages.set_peers(slot, exchange.peers(self.recv[slot]), exchange.peers(self.yrecv[slot]))
+            exchange.barrier()      # every rank's table is set before anyone stores
         self.log: List[Tuple[str, int]] = []          # (operation, batch) in enqueue order of the last solve
         if self.cuda:
             self.s_b, self.s_comm = torch.cuda.Stream(), torch.cuda.Stream()
@@ -131,7 +194,18 @@ class YSlabSolver:
                 slot = n % DEPTH
                 lb, ls = st.batch_lines(n)
                 n6 = self.nranks * self.P * 6 * ls
-                if self.cuda:
+                if self.exchange is not None:             # stage A stores into the receivers: A2B = a barrier
+                    if self.cuda:
+                        st.stage_a_peer(n, a, b, c, d, s_ac)
+                        self.ev_a[slot].record(s_ac)
+                        self.s_comm.wait_event(self.ev_a[slot])
+                        with torch.cuda.stream(self.s_comm):
+                            self.exchange.barrier()
+                        self.ev_x1[slot].record(self.s_comm)
+                    else:
+                        st.stage_a_peer(n, a, b, c, d)
+                        self.exchange.barrier()
+                elif self.cuda:
                     if n >= DEPTH:
                         s_ac.wait_event(self.ev_x1[slot])      # send[slot] was read by A2B(n - DEPTH)
                     st.stage_a(n, a, b, c, d, self.send[slot], s_ac)
@@ -151,7 +225,19 @@ class YSlabSolver:
                 slot = q % DEPTH
                 lb, ls = st.batch_lines(q)
                 n2 = self.nranks * 2 * self.P * ls
-                if self.cuda:
+                if self.exchange is not None:             # stage B stores into the receivers: B2C = a barrier
+                    if self.cuda:
+                        self.s_b.wait_event(self.ev_x1[slot])
+                        st.stage_b_peer(q, self.recv[slot], self.s_b)
+                        self.ev_b[slot].record(self.s_b)
+                        self.s_comm.wait_event(self.ev_b[slot])
+                        with torch.cuda.stream(self.s_comm):
+                            self.exchange.barrier()
+                        self.ev_x2[slot].record(self.s_comm)
+                    else:
+                        st.stage_b_peer(q, self.recv[slot])
+                        self.exchange.barrier()
+                elif self.cuda:
                     self.s_b.wait_event(self.ev_x1[slot])
                     if q >= DEPTH:
                         self.s_b.wait_event(self.ev_x2[slot])    # yout[slot] was read by B2C(q - DEPTH)

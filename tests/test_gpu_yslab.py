@@ -12,7 +12,7 @@ import torch
 import oracle
 import tdma_inputs
 import paper_2509_03933_b200 as tdma
-from paper_2509_03933_b200.yslab import YSlabSolver, CudaSlabStages
+from paper_2509_03933_b200.yslab import YSlabSolver, CudaSlabStages, LocalExchange
 from yslab_standin import reduced_rows
 
 pytestmark = pytest.mark.gpu
@@ -131,14 +131,16 @@ def test_exchange_buffers_hold_the_schur_complement_rows():
                     assert abs(yout[l // ls, r, 2 * p + 1, l % ls] - ref[k, (pg + 1) * m - 1, i]) <= 1e-12
 
 
+@pytest.mark.parametrize("peer", [False, True], ids=["all_to_all", "peer_stores"])
 @pytest.mark.parametrize("batch", [0, 2])
-def test_driver_single_rank_streams_and_events(batch):
-    """YSlabSolver as one rank (the exchange degenerates to a copy): its three streams, the event
-    ring and the join back into the caller's stream, on hardware; x read right after solve()."""
+def test_driver_single_rank_streams_and_events(batch, peer):
+    """YSlabSolver as one rank (the exchange degenerates to a copy; in peer mode the stages store into
+    the rank's own receive ring): its three streams, the event ring and the join back into the
+    caller's stream, on hardware; x read right after solve()."""
     nx, ny, nz = 128, 128, 9
     a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 47, dev())
     x = torch.full_like(d, float("nan"))
-    with YSlabSolver(nx, ny, nz, P_local=4, batch=batch) as solver:
+    with YSlabSolver(nx, ny, nz, P_local=4, batch=batch, exchange=LocalExchange(dev()) if peer else None) as solver:
         for _ in range(2):
             solver.solve(a, b, c, d, x)
         xn = x.cpu().numpy()                      # same stream as the caller's: ordered after the join

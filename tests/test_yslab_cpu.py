@@ -32,7 +32,29 @@ loc = [t[:, sl, :].contiguous() for t in (a, b, c, d)]
 x = torch.full_like(loc[3], float("nan"))
 st = NumpySlabStages(nx, nyl, nz, P_local, batch, rank, world)
 st.bind_inputs(*loc)
-solver = YSlabSolver(nx, nyl, nz, P_local, batch, stages=st)
+
+class FileExchange:
+    # peer-mode plumbing for CPU ranks: every rank's buffer is a file mapped by all ranks
+    def __init__(self, folder):
+        self.folder, self.count, self.bufs, self.key = folder, 0, {}, {}
+    def alloc(self, n):
+        idx, self.count = self.count, self.count + 1
+        path = lambda q: os.path.join(self.folder, "buf%%d_rank%%d" %% (idx, q))
+        own = np.memmap(path(rank), dtype=np.float64, mode="w+", shape=(n,))
+        own[:] = np.nan
+        own.flush()
+        dist.barrier()
+        self.bufs[idx] = [torch.from_numpy(np.memmap(path(q), dtype=np.float64, mode="r+", shape=(n,))) for q in range(world)]
+        t = self.bufs[idx][rank]
+        self.key[t.data_ptr()] = idx
+        return t
+    def peers(self, t):
+        return self.bufs[self.key[t.data_ptr()]]
+    def barrier(self):
+        dist.barrier()
+
+exchange = FileExchange(%(peer_dir)r) if %(peer_dir)r else None
+solver = YSlabSolver(nx, nyl, nz, P_local, batch, stages=st, exchange=exchange)
 solver.solve(*loc, x)
 ref = oracle.solve_y(*[t.numpy() for t in (a, b, c, d)])[:, sl, :]
 err = float(oracle.normwise_error(np.ascontiguousarray(x.numpy()), np.ascontiguousarray(ref)).max())
@@ -50,9 +72,9 @@ def _free_port():
     return p
 
 
-def _run(world, **kw):
+def _run(world, peer_dir="", **kw):
     port = _free_port()
-    code = WORKER % dict(root=ROOT, **kw)
+    code = WORKER % dict(root=ROOT, peer_dir=peer_dir, **kw)
     procs = []
     for r in range(world):
         env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(world),
@@ -66,10 +88,13 @@ def _run(world, **kw):
 
 
 @pytest.mark.timeout(400)
+@pytest.mark.parametrize("peer", [False, True], ids=["all_to_all", "peer_stores"])
 @pytest.mark.parametrize("P_local,batch", [(1, 2), (2, 0), (4, 3)])
-def test_yslab_driver_two_gloo_ranks_matches_whole_line_thomas(P_local, batch):
+def test_yslab_driver_two_gloo_ranks_matches_whole_line_thomas(P_local, batch, peer, tmp_path):
+    """peer_stores: the driver's peer mode -- no all-to-all, the stages store into the other rank's
+    receive ring (files mapped by both ranks), one barrier per exchange; same result, same order."""
     nx, ny, nz = 6, 32, 7
-    recs = _run(2, nx=nx, ny=ny, nz=nz, P=P_local, batch=batch)
+    recs = _run(2, nx=nx, ny=ny, nz=nz, P=P_local, batch=batch, peer_dir=str(tmp_path) if peer else "")
     bz = nz if batch == 0 else batch
     nb = (nz + bz - 1) // bz
     for r in recs:

@@ -117,6 +117,29 @@ class NumpySlabStages:
                     rhs[nn - 1] -= C[k, r0 + m - 2, i] * xl
                     X[k, r0 + 1:r0 + m - 1, i] = np.linalg.solve(T, rhs)
 
+    # peer mode (tdma_slab_set_peers / _stage_a_peer / _stage_b_peer): the block meant for rank q goes
+    # straight into rank q's receive buffer, at the place the all-to-all would have put it
+    def set_peers(self, slot, recv_of_rank, yrecv_of_rank):
+        if not hasattr(self, "_peers"):
+            self._peers = {}
+        self._peers[slot] = (list(recv_of_rank), list(yrecv_of_rank))
+
+    def stage_a_peer(self, n, a, b, c, d, stream=None):
+        lb, ls = self.batch_lines(n)
+        blk = self.P * 6 * ls
+        send = torch.empty(self.nranks * blk, dtype=torch.float64)
+        self.stage_a(n, a, b, c, d, send)
+        for q in range(self.nranks):
+            self._peers[n % 3][0][q][self.rank * blk:(self.rank + 1) * blk] = send[q * blk:(q + 1) * blk]
+
+    def stage_b_peer(self, n, recv, stream=None):
+        lb, ls = self.batch_lines(n)
+        blk = 2 * self.P * ls
+        yout = torch.empty(self.nranks * blk, dtype=torch.float64)
+        self.stage_b(n, recv, yout)
+        for q in range(self.nranks):
+            self._peers[n % 3][1][q][self.rank * blk:(self.rank + 1) * blk] = yout[q * blk:(q + 1) * blk]
+
     def bind_inputs(self, a, b, c, d):
         """stage C of the real library reads its own scratch; the stand-in re-reads the inputs."""
         self._abcd = [t.numpy() for t in (a, b, c, d)]
