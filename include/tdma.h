@@ -25,7 +25,8 @@
  *
  * ALSO HERE, each documented at its declaration: tdma_solve_shared (1-D coefficient arrays, real or
  * complex right-hand sides: the form the paper benchmarks), the tdma_slab_* calls (rank-local stages
- * of the multi-GPU y-slab decomposition), stage-isolated launches, the batch-size optimiser, the
+ * of the multi-GPU y-slab decomposition, with buffered output or storing straight into the peers'
+ * receive buffers), stage-isolated launches, the batch-size optimiser, the
  * stream timeline and an fp64 ALU probe.
  *
  * ERRORS.  tdma_plan_create* return NULL on failure; the int-returning calls return TDMA_OK (0)
