@@ -27,7 +27,7 @@
  * complex right-hand sides: the form the paper benchmarks), the tdma_slab_* calls (rank-local stages
  * of the multi-GPU y-slab decomposition, with buffered output or storing straight into the peers'
  * receive buffers), stage-isolated launches, the batch-size optimiser, the
- * stream timeline and an fp64 ALU probe.
+ * stream timeline, an allocation-free solve (tdma_solve_static) and an fp64 ALU probe.
  *
  * ERRORS.  tdma_plan_create* return NULL on failure; the int-returning calls return TDMA_OK (0)
  * or a negative tdma_status; a message for the calling thread is in tdma_last_error().
@@ -345,6 +345,27 @@ int tdma_slab_stage_a_peer(tdma_slab *slab, int batch_index, const void *a, cons
                            const void *d, void *stream);
 int tdma_slab_stage_b_peer(tdma_slab *slab, int batch_index, const void *recv, int pdd, void *stream);
 int tdma_slab_destroy(tdma_slab *slab);
+
+/* Allocation-free solve, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Solves the same nx*ny*nz systems as tdma_solve
+ * (layout and meaning of a, b, c, d, x as at the top of this file; DEVICE pointers, 8-byte aligned;
+ * y split into P partitions, ny % P == 0, ny / P >= 2) with the PIPELINED variant's three stage
+ * kernels run in Alg. 1 order on `stream`, batch after batch.  No plan: the
+ * scratch (a', c', d' of a batch and its reduced system) is a file-scope __device__ array of
+ * TDMA_STATIC_SCRATCH_BYTES that every GPU loading the library holds until the process exits, and
+ * the call performs no cudaMalloc / cudaFree and no allocating library call.  The z range is cut
+ * into the largest batches that fit; TDMA_ERR_UNSUPPORTED (message in tdma_last_error()) when a
+ * single z-slice does not:  8 * nx * (3 ny + 10 P) bytes (+ rounding) must not exceed the maximum
+ * -- e.g. 1024 x 1024 slices with P = 16 fit (25.3 MiB), 2048 x 1024 do not.
+ * The array is SHARED by every call and keeps the last call's contents; nothing in it needs to be
+ * zero at entry (every element read is written earlier in the same call) and nothing is cleared.
+ * Calls that OVERLAP on the GPU -- different streams, independent graph branches, several host
+ * threads -- race on it: order them.  The first call on a device resolves the array's device
+ * address (cudaGetSymbolAddress) and, with lazy module loading, loads the kernels: make it
+ * outside stream capture.  Not a fast path: use a plan when allocation is possible.  Enqueue-only. */
+#define TDMA_STATIC_SCRATCH_BYTES (32u << 20)
+int tdma_solve_static(int nx, int ny, int nz, int P, const void *a, const void *b, const void *c,
+                      const void *d, void *x, void *stream);
 
 /* fp64 ALU probe: measures on the current device and writes to result[0..5]
  *   [0] DFMA throughput with many independent chains, TFLOP/s (1 DFMA = 2 flop)

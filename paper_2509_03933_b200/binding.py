@@ -34,7 +34,7 @@ EXPORTED_SYMBOLS = (
     "tdma_plan_create", "tdma_plan_create_ex", "tdma_solve", "tdma_solve_host", "tdma_stage",
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
     "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
-    "tdma_solve_shared", "tdma_probe_fp64",
+    "tdma_solve_shared", "tdma_probe_fp64", "tdma_solve_static",
     "tdma_slab_create", "tdma_slab_get", "tdma_slab_stage_a", "tdma_slab_stage_b", "tdma_slab_stage_b_pdd", "tdma_slab_stage_c",
     "tdma_slab_set_peers", "tdma_slab_stage_a_peer", "tdma_slab_stage_b_peer", "tdma_slab_destroy",
 )
@@ -115,6 +115,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_slab_stage_b_peer.restype = ci
     lib.tdma_slab_destroy.argtypes = [vp]
     lib.tdma_slab_destroy.restype = ci
+    lib.tdma_solve_static.argtypes = [ci] * 4 + [vp] * 6
+    lib.tdma_solve_static.restype = ci
     lib.tdma_probe_fp64.argtypes = [ctypes.POINTER(ctypes.c_double), ci]
     lib.tdma_probe_fp64.restype = ci
     lib.tdma_solve_host.argtypes = [vp] * 6
@@ -271,6 +273,15 @@ def tdma_slab_stage_b_peer(slab: int, batch_index: int, recv, pdd: bool = False,
 
 def tdma_slab_destroy(slab: int) -> None:
     _check(load_library().tdma_slab_destroy(slab))
+
+
+TDMA_STATIC_SCRATCH_BYTES = 32 << 20
+
+
+def tdma_solve_static(nx: int, ny: int, nz: int, P: int, a, b, c, d, x, stream=None) -> None:
+    """Allocation-free solve (include/tdma.h): scratch in a static device array of TDMA_STATIC_SCRATCH_BYTES."""
+    _check(load_library().tdma_solve_static(nx, ny, nz, P, _ptr(a), _ptr(b), _ptr(c), _ptr(d), _ptr(x),
+                                            _stream_handle(stream)))
 
 
 def tdma_probe_fp64() -> dict:

@@ -21,6 +21,7 @@ UNITS = {
     "tdma_shared.cu": ["tdma_shared_tma.cuh", "tdma_fused_tma.cuh", "tdma_shared.h"],
     "tdma_probe.cu": [_TDMA_H],
     "tdma_slab.cu": ["tdma_stage_kernels.cuh", "tdma_staged.h", _TDMA_H],
+    "tdma_static.cu": ["tdma_stage_kernels.cuh", _TDMA_H],
 }
 OBJ_DIR = os.path.join(CSRC, "build")
 

@@ -593,6 +593,11 @@ int check_ptrs(const tdma_plan *plan, const void *a, const void *b, const void *
 
 }  // namespace
 
+namespace tdma {
+// for the library's other translation units: sets the calling thread's tdma_last_error() message
+int report_error(int code, const char *msg) { return set_err(code, "%s", msg); }
+}  // namespace tdma
+
 extern "C" {
 
 tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dtype,
