@@ -187,6 +187,12 @@ int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, con
  * a_y, b0_y, c_y hold nx entries along x, sx holds NY shifts, one per line of a slice, sz the nz
  * shifts of the slices: line (j,k) has the shift sx[j] + sz[k]) -- plain or cyclic
  * (options.periodic, without pin00).
+ * UNIFORM MATRIX: sx = sz = NULL (both) means every line has the same matrix a_y, b0_y, c_y -- the
+ * ADI momentum sweeps, "all systems in the batch share the same matrix A"; pin00 must
+ * be 0.  For real cells on shapes a 16-line tile with 16- or 32-row leaves covers, everything that
+ * depends on the matrix alone (every reciprocal below the tree) is then computed once per launch
+ * instead of once per line (x agrees with zero shift arrays to rounding); other shapes and complex
+ * cells run the general form with plan-owned zero shifts (allocated at the first such call).
  * P and batch are not used: the line is cut into the kernel's own leaves (D1); one
  * persistent launch (plus the fill launch, see fused_fill) per call.
  * TDMA_ERR_UNSUPPORTED when ny does not tile (ny = CL * W * M0, CL in 1,2,4,8, W a power of two

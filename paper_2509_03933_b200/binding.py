@@ -373,19 +373,23 @@ class Plan:
         return x
 
     def solve_shared(self, a_y, b0_y, c_y, sx, sz, d, x, pin00: bool = False, stream=None):
-        """Shared-coefficient solve; d, x real (nz, ny, nx) fp64 or complex128 tensors."""
+        """Shared-coefficient solve; d, x real (nz, ny, nx) fp64 or complex128 tensors.  sx = sz = None:
+        the same matrix for every line (uniform matrix, include/tdma.h)."""
         nz, ny, nx = self.shape
         ncomp = 2 if (hasattr(d, "is_complex") and d.is_complex()) else 1
         # (line length, lines side by side, slices): z sweep: lines along z, y-slices; x sweep: lines along x,
         # ny of them per z-slice
         nline, nlane, nslice = {TDMA_AXIS_Z: (nz, nx, ny), TDMA_AXIS_X: (nx, ny, nz)}.get(self.axis, (ny, nx, nz))
-        for t, n in ((a_y, nline), (b0_y, nline), (c_y, nline), (sx, nlane), (sz, nslice)):
+        if (sx is None) != (sz is None):
+            raise ValueError("pass both shift arrays, or None for both (uniform matrix)")
+        for t, n in ((a_y, nline), (b0_y, nline), (c_y, nline)) + (((sx, nlane), (sz, nslice)) if sx is not None else ()):
             if t.numel() != n or not t.is_contiguous() or t.element_size() != 8:
                 raise ValueError("coefficient arrays must be contiguous fp64 of lengths n, n, n (line length), lanes, slices")
         for t in (d, x):
             if t.numel() != nz * ny * nx or not t.is_contiguous() or t.element_size() != 8 * ncomp:
                 raise ValueError("d, x must be contiguous with nz*ny*nx cells of %d bytes" % (8 * ncomp))
-        tdma_solve_shared(self.handle, a_y, b0_y, c_y, sx, sz, ncomp, 1 if pin00 else 0, d, x, stream)
+        tdma_solve_shared(self.handle, a_y, b0_y, c_y, 0 if sx is None else sx, 0 if sz is None else sz, ncomp,
+                          1 if pin00 else 0, d, x, stream)
         return x
 
     def solve_host(self, a, b, c, d, x):

@@ -99,9 +99,10 @@ struct tdma_plan {
     tdma::StagedConfig staged;
     int Pred = 0;       // partitions in the reduced buffers (P; STAGED: staged.Pe)
     // shared-coefficient mode (tdma_solve_shared), configured at the first call per ncomp
-    tdma::SharedConfig sh[2], sh_fill[2];
-    int sh_state[2] = {0, 0};     // 0 = not configured, 1 = ready, -1 = does not tile
-    bool sh_have_fill[2] = {false, false};
+    tdma::SharedConfig sh[3], sh_fill[3];   // real, complex, real with a uniform matrix (no shift arrays)
+    int sh_state[3] = {0, 0, 0};  // 0 = not configured, 1 = ready, -1 = does not tile
+    bool sh_have_fill[3] = {false, false, false};
+    double *sh_zero = nullptr;    // zero shifts, for uniform-matrix calls on shapes the uniform tiling does not cover
     int sh_opt[5] = {0, 0, 0, 0, 0}; // options.shared_lines / _cluster / _leaf_rows / _slots / _ctas
     int sh_last = -1, sh_fill_last = 0;
     // host staging (tdma_solve_host), allocated on first use
@@ -413,7 +414,7 @@ void free_plan(tdma_plan *pl)
     if (!pl) return;
     for (auto &g : pl->graphs) cudaGraphExecDestroy(g.exec);
     for (auto ev : pl->tl_ev) cudaEventDestroy(ev);
-    cudaFree(pl->scratch); cudaFree(pl->red); cudaFree(pl->send);
+    cudaFree(pl->scratch); cudaFree(pl->red); cudaFree(pl->send); cudaFree(pl->sh_zero);
     if (pl->staged.impl) tdma::free_staged(&pl->staged);
     for (int s = 0; s < 2; ++s)
         for (int i = 0; i < 5; ++i) cudaFree(pl->stage_dev[s][i]);
@@ -672,9 +673,11 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
 {
     int rc = check_ptrs(plan, a_y, b0_y, c_y, d, x);
     if (rc != TDMA_OK) return rc;
-    if (!sx || !sz) return set_err(TDMA_ERR_INVALID_ARG, "NULL shift array");
     if (ncomp != 1 && ncomp != 2) return set_err(TDMA_ERR_INVALID_ARG, "ncomp = %d must be 1 (real) or 2 (complex)", ncomp);
     tdma_plan *pl = plan;
+    bool uniform = !sx && !sz;                 // the same matrix for every line
+    if (!uniform && (!sx || !sz)) return set_err(TDMA_ERR_INVALID_ARG, "NULL shift array (pass both as NULL for a uniform matrix)");
+    if (uniform && pin00) return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: pin00 changes one line's matrix; pass shift arrays");
     const bool xsw = pl->axis == TDMA_AXIS_X;
     if (xsw && ncomp != 1)
         return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: x sweeps take real right-hand sides (ncomp = 1)");
@@ -682,9 +685,38 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: pin00 is for plain lines");
     if ((((uintptr_t)d | (uintptr_t)x) & 15) != 0)
         return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared needs 16-byte aligned d and x (tensor maps)");
-    const int q = ncomp - 1;
     cudaStream_t origin = (cudaStream_t)stream;
     if (pl->ny == 1) return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared needs ny >= 4");
+    if (uniform && ncomp == 1 && pl->sh_state[2] == 0) {
+        // the uniform-matrix build covers 16-line tiles with 16- / 32-row leaves and up to 256 threads
+        cudaDeviceProp prop;
+        CUDA_TRY(cudaGetDeviceProperties(&prop, pl->device));
+        const char *why = nullptr;
+        const bool ok = tdma::configure_shared(&pl->sh[2], pl->nx, pl->ny, 1, pl->sh_opt[0], pl->sh_opt[1], pl->sh_opt[2],
+                                               pl->sh_opt[3], 0, prop, &why, xsw, true);
+        pl->sh_state[2] = ok ? 1 : -1;
+        pl->sm_count = prop.multiProcessorCount;
+        pl->sm_smem = prop.sharedMemPerMultiprocessor;
+        if (ok && pl->sh[2].cluster >= 4 && pl->fill_opt >= 0) {
+            const char *why2 = nullptr;
+            pl->sh_have_fill[2] = tdma::configure_shared(&pl->sh_fill[2], pl->nx, pl->ny, 1, 0, pl->ny % 2 == 0 ? 2 : 1,
+                                                         0, 0, 0, prop, &why2, xsw, true);
+        }
+    }
+    if (uniform && (ncomp != 1 || pl->sh_state[2] < 0)) {
+        // no uniform-matrix build for this shape / complex cells: the general form with zero shifts
+        const size_t nzero = (size_t)std::max(std::max(pl->nx, pl->ny), pl->nz);
+        if (!pl->sh_zero) {
+            if (cudaMalloc(&pl->sh_zero, nzero * sizeof(double)) != cudaSuccess) {
+                cudaGetLastError();
+                return set_err(TDMA_ERR_ALLOC, "tdma_solve_shared: no memory for %zu zero shifts", nzero);
+            }
+            CUDA_TRY(cudaMemset(pl->sh_zero, 0, nzero * sizeof(double)));
+        }
+        sx = sz = pl->sh_zero;
+        uniform = false;
+    }
+    const int q = uniform ? 2 : ncomp - 1;
     if (pl->sh_state[q] == 0) {
         cudaDeviceProp prop;
         CUDA_TRY(cudaGetDeviceProperties(&prop, pl->device));
@@ -713,6 +745,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
     args.nx = pl->nx; args.ny = pl->ny; args.nzs = 0;
     args.rs = pl->rs; args.os = pl->os;
     args.axis_z = pl->axis == TDMA_AXIS_Z ? 1 : 0; args.periodic = pl->periodic ? 1 : 0;
+    args.uniform = uniform ? 1 : 0;
     cudaError_t e = tdma::launch_shared(pl->sh[q], args, origin);          // prepare: attributes, grid size
     int nzf = 0;
     if (e == cudaSuccess && pl->sh_have_fill[q]) {
@@ -745,7 +778,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
     if (e == cudaSuccess && nzf > 0) {
         tdma::SharedArgs fa = args;
         const size_t off = (size_t)(pl->nz - nzf) * (size_t)pl->os * (size_t)ncomp;
-        fa.d = args.d + off; fa.x = args.x + off; fa.sz = args.sz + (pl->nz - nzf);
+        fa.d = args.d + off; fa.x = args.x + off; fa.sz = uniform ? nullptr : args.sz + (pl->nz - nzf);
         fa.pin00 = 0;                    // line (0,0) lies in slice 0, which the main launch owns
         fa.nzs = nzf;
         e = tdma::launch_shared(pl->sh_fill[q], fa, pl->sB);

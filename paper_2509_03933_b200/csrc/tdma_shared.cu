@@ -5,10 +5,10 @@
 namespace tdma {
 
 bool configure_shared(SharedConfig *out, int nx, int ny, int ncomp, int want_lines, int want_cluster,
-                      int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why, bool xsweep)
+                      int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why, bool xsweep, bool uniform)
 {
     if (!get_encode_tiled()) { *why = "cuTensorMapEncodeTiled not found"; return false; }
-    return configure_shared_impl(out, nx, ny, ncomp, want_lines, want_cluster, want_leaf, want_slots, want_ctas, prop, why, xsweep);
+    return configure_shared_impl(out, nx, ny, ncomp, want_lines, want_cluster, want_leaf, want_slots, want_ctas, prop, why, xsweep, uniform);
 }
 
 cudaError_t launch_shared(SharedConfig &cfg, const SharedArgs &args, cudaStream_t st)

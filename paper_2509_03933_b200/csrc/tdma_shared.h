@@ -22,6 +22,7 @@ struct SharedConfig {
     int threads = 0;    // W * TX
     int box_rows = 0;   // rows per TMA box (<= 256), divides R
     int slots = 0;      // NA: ring slots of one d / x tile each (>= 2)
+    int uniform = 0;    // uniform matrix (no shift arrays): matrix work hoisted out of the tile loop
     int xsweep = 0;     // lines along the contiguous axis: 4-D tensor map, [leaf][line][16 x] slots
     int ctas_per_sm = 1;   // 2: the <= 128-register instantiation, two CTAs share an SM
     int max_clusters = 0;  // co-resident clusters (persistent grid), filled at first launch
@@ -36,6 +37,7 @@ struct SharedArgs {
     int pin00;                        // row 0 of line (0, 0) of THIS launch's slice 0 is b = 1, c = 0
     int nx, ny, nzs;                  // lanes, rows per line, slices of the launch
     long long rs = 0, os = 0;         // cells between rows of a line / between slices of d and x
+    int uniform = 0;                  // sx = sz = NULL: the same matrix for every line (needs SharedConfig::uniform)
     int axis_z = 0, periodic = 0;     // z sweep (rows are the slow axis); cyclic lines
                                       // x sweep: SharedConfig::xsweep; nx = lanes (caller's ny), ny = rows (caller's nx)
 };
@@ -43,7 +45,7 @@ struct SharedArgs {
 // Tiling for ny-row lines: CL x W x M0 with W a power of two.  want_* = 0: auto.
 bool configure_shared(SharedConfig *out, int nx, int ny, int ncomp, int want_lines, int want_cluster,
                       int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why,
-                      bool xsweep = false);
+                      bool xsweep = false, bool uniform = false);
 
 // nzs = 0: prepare only (function attributes, persistent grid size).
 cudaError_t launch_shared(SharedConfig &cfg, const SharedArgs &args, cudaStream_t st);

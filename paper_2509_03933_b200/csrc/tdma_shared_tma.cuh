@@ -340,10 +340,223 @@ __device__ __forceinline__ void leaf_back_sh_x(const ShLeafRegs<M0, 1> &R, const
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// Uniform matrix (sx = sz = NULL: every line of the launch has the SAME matrix -- the ADI momentum
+// sweeps, "all systems in the batch share the same matrix A").  A thread sweeps the same
+// leaf rows for every tile, so everything that depends on the matrix alone is computed ONCE per
+// launch: per row the multipliers of the right-hand-side recurrences go to a shared-memory table
+// (read by broadcast), per leaf the multipliers of the in-register merges go to a small record,
+// and the back-substitution coefficients (ia, ic), the merges' Elim::a / ::c and the matrix part
+// of the leaf's two boundary equations stay in registers across tiles.  Per tile and row that
+// leaves 2 multiply-adds + 1 multiply forward and 2 multiply-adds backward: no reciprocal in the
+// tile loop below the tree.  The formulas and their order are those of leaf_reduce_sh / merge_nodes
+// with s = 0; x agrees with the shifted kernel for zero shifts to rounding (the compiler contracts
+// the two forms differently), not bit for bit.
+// ------------------------------------------------------------------------------------------
+struct MergeRhs { double Rfb, Llc, Llb, Rfa, det, Lfc, sf, Rla, sl, inv; };   // what merge_nodes needs for d
+constexpr int kMergeRhsDoubles = 10;
+
+template <int M0>
+struct UniLeaf {
+    static constexpr int K = ShLeafRegs<M0, 1>::K;
+    static constexpr int kRec = K + kMergeRhsDoubles * (K - 1);   // doubles per leaf record: invfb[K], MergeRhs[K-1]
+    static constexpr int kStride = M0 + 1;                       // table rows per leaf (+1: two leaves of a warp hit different banks)
+};
+
+// matrix part of merge_nodes
+__device__ __forceinline__ void merge_matrix(const NodeEq<1> &L, const NodeEq<1> &R, NodeEq<1> &M, Elim<1> &E, MergeRhs &q)
+{
+    const double det = fma(L.lb, R.fb, -(L.lc * R.fa));
+    const double p2 = L.lc * R.fc, p3 = R.fa * L.la;
+    M.fb = fma(det, L.fb, -(L.fc * R.fb * L.la));
+    M.lb = fma(det, R.lb, -(R.la * L.lb * R.fc));
+    const double sf = pow2_unscale(M.fb), sl = pow2_unscale(M.lb);
+    M.fa = det * L.fa * sf; M.fb *= sf; M.fc = L.fc * p2 * sf;
+    M.la = R.la * p3 * sl; M.lb *= sl; M.lc = det * R.lc * sl;
+    const double inv = rcp_nr(det);
+    E.a[0] = R.fb * L.la * inv; E.c[0] = -(p2 * inv);
+    E.a[1] = -(p3 * inv); E.c[1] = L.lb * R.fc * inv;
+    q.Rfb = R.fb; q.Llc = L.lc; q.Llb = L.lb; q.Rfa = R.fa; q.det = det; q.Lfc = L.fc; q.sf = sf; q.Rla = R.la; q.sl = sl; q.inv = inv;
+}
+
+// right-hand-side part of merge_nodes; q: the record's 10 doubles.  kUnit: both nodes have unit
+// diagonals (merges of swept sub-leaves), as the compiler also knows in merge_nodes
+template <bool kUnit>
+__device__ __forceinline__ void merge_rhs(const double *__restrict__ q, double Lfd, double Lld, double Rfd, double Rld,
+                                          double &Mfd, double &Mld, Elim<1> &E)
+{
+    const double Rfb = kUnit ? 1.0 : q[0], Llb = kUnit ? 1.0 : q[2];
+    const double Llc = q[1], Rfa = q[3], det = q[4], Lfc = q[5], sf = q[6], Rla = q[7], sl = q[8], inv = q[9];
+    const double nL = fma(Rfb, Lld, -(Llc * Rfd)), nR = fma(Llb, Rfd, -(Rfa * Lld));
+    Mfd = fma(det, Lfd, -(Lfc * nL)) * sf;
+    Mld = fma(det, Rld, -(Rla * nR)) * sl;
+    E.d[0][0] = nL * inv; E.d[1][0] = nR * inv;
+}
+
+// Once per launch.  tA, tB, tC: the leaf's rows (kStride apart per leaf) holding a, b0, c on entry;
+// write = true (ONE thread per leaf, after every thread has read the coefficients): they become the
+// table (a_r, 1 / pivot_r, running fc_r), and rec the leaf's record.  Every thread keeps R.ia, R.ic,
+// Elim::a / ::c and the matrix part of f, l.
+template <int M0>
+__device__ __forceinline__ void leaf_matrix_uni(double *tA, double *tB, double *tC, bool first_leaf, bool last_leaf,
+                                                bool write, double *rec, EqN<1> &f, EqN<1> &l, ShLeafRegs<M0, 1> &R)
+{
+    constexpr int K = ShLeafRegs<M0, 1>::K, H = ShLeafRegs<M0, 1>::H;
+    double fa[K], fb[K], fc[K], pa[K], pc[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const int o = h * H;
+        double inv = rcp_nr(tB[o]);
+        fa[h] = (h == 0 && first_leaf) ? 0.0 : tA[o] * inv;
+        fc[h] = tC[o] * inv; fb[h] = 1.0;
+        if (write) tB[o] = inv;
+        inv = rcp_nr(tB[o + 1]);
+        pa[h] = tA[o + 1] * inv; pc[h] = tC[o + 1] * inv;
+        if (write) tB[o + 1] = inv;
+    }
+#pragma unroll
+    for (int r = 2; r < H; ++r) {
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            const int o = h * H + r;
+            const double ar = tA[o], br = tB[o];
+            double cr = tC[o];
+            if (r == H - 1 && h == K - 1 && last_leaf) cr = 0.0;
+            fb[h] = fma(-fc[h], pa[h], fb[h]);
+            if (write) tC[o] = fc[h];                               // the fc that folds d'_{r-1} into the first equation
+            fc[h] = -fc[h] * pc[h];
+            R.ia[h][r - 2] = pa[h]; R.ic[h][r - 2] = pc[h];
+            const double inv = rcp_nr(fma(-ar, pc[h], br));
+            if (write) tB[o] = inv;
+            pc[h] = cr * inv;
+            pa[h] = -(ar * pa[h]) * inv;
+        }
+    }
+    NodeEq<1> nd[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const double inv = rcp_nr(fb[h]);
+        nd[h].fa = fa[h] * inv; nd[h].fb = 1.0; nd[h].fc = fc[h] * inv;
+        nd[h].la = pa[h]; nd[h].lb = 1.0; nd[h].lc = pc[h];
+        nd[h].fd[0] = 0.0; nd[h].ld[0] = 0.0;
+        if (write) rec[h] = inv;
+    }
+    NodeEq<1> top;
+    MergeRhs q[K > 1 ? K - 1 : 1];
+    if constexpr (K == 1) {
+        top = nd[0];
+    } else if constexpr (K == 2) {
+        merge_matrix(nd[0], nd[K - 1], top, R.e[0], q[0]);
+    } else {
+        NodeEq<1> m01, m23;
+        merge_matrix(nd[0], nd[1], m01, R.e[0], q[0]);
+        merge_matrix(nd[K - 2], nd[K - 1], m23, R.e[1], q[1]);
+        merge_matrix(m01, m23, top, R.e[K - 2], q[K - 2]);
+    }
+    if (write) {
+#pragma unroll
+        for (int j = 0; j < K - 1; ++j) {
+            double *w = rec + K + kMergeRhsDoubles * j;
+            w[0] = q[j].Rfb; w[1] = q[j].Llc; w[2] = q[j].Llb; w[3] = q[j].Rfa; w[4] = q[j].det;
+            w[5] = q[j].Lfc; w[6] = q[j].sf; w[7] = q[j].Rla; w[8] = q[j].sl; w[9] = q[j].inv;
+        }
+    }
+    f.a = top.fa; f.b = top.fb; f.c = top.fc; l.a = top.la; l.b = top.lb; l.c = top.lc;
+}
+
+// the K sub-leaves' right-hand sides (fd, pd after the sweep) -> the leaf's f.d, l.d and Elim::d
+template <int M0>
+__device__ __forceinline__ void leaf_finish_uni(const double *__restrict__ rec, const double (&fd)[ShLeafRegs<M0, 1>::K],
+                                                const double (&pd)[ShLeafRegs<M0, 1>::K], EqN<1> &f, EqN<1> &l, ShLeafRegs<M0, 1> &R)
+{
+    constexpr int K = ShLeafRegs<M0, 1>::K;
+    double nfd[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) nfd[h] = fd[h] * rec[h];
+    if constexpr (K == 1) {
+        f.d[0] = nfd[0]; l.d[0] = pd[0];
+    } else if constexpr (K == 2) {
+        merge_rhs<true>(rec + K, nfd[0], pd[0], nfd[K - 1], pd[K - 1], f.d[0], l.d[0], R.e[0]);
+    } else {
+        double fd01, ld01, fd23, ld23;
+        merge_rhs<true>(rec + K, nfd[0], pd[0], nfd[1], pd[1], fd01, ld01, R.e[0]);
+        merge_rhs<true>(rec + K + kMergeRhsDoubles, nfd[K - 2], pd[K - 2], nfd[K - 1], pd[K - 1], fd23, ld23, R.e[1]);
+        merge_rhs<false>(rec + K + kMergeRhsDoubles * (K - 2), fd01, ld01, fd23, ld23, f.d[0], l.d[0], R.e[K - 2]);
+    }
+}
+
+// Per tile: the right-hand-side recurrences of leaf_reduce_sh with the table's multipliers.
+template <int M0>
+__device__ __forceinline__ void leaf_rhs_uni(const double *__restrict__ tA, const double *__restrict__ tB,
+                                             const double *__restrict__ tC, const double *__restrict__ rec, uint32_t dbase,
+                                             uint32_t row_bytes, EqN<1> &f, EqN<1> &l, ShLeafRegs<M0, 1> &R)
+{
+    constexpr int K = ShLeafRegs<M0, 1>::K, H = ShLeafRegs<M0, 1>::H;
+    double fd[K], pd[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const int o = h * H;
+        fd[h] = lds1(dbase + (uint32_t)o * row_bytes) * tB[o];
+        pd[h] = lds1(dbase + (uint32_t)(o + 1) * row_bytes) * tB[o + 1];
+    }
+#pragma unroll
+    for (int r = 2; r < H; ++r) {
+#pragma unroll
+        for (int h = 0; h < K; ++h) {
+            const int o = h * H + r;
+            const double dr = lds1(dbase + (uint32_t)o * row_bytes);
+            fd[h] = fma(-tC[o], pd[h], fd[h]);
+            sts1(dbase + (uint32_t)(o - 1) * row_bytes, pd[h]);     // d' of row r-1, in place
+            pd[h] = fma(-tA[o], pd[h], dr) * tB[o];
+        }
+    }
+    leaf_finish_uni<M0>(rec, fd, pd, f, l, R);
+}
+
+// the same for x sweeps (16-byte pairs through the swizzled boxes, as leaf_reduce_sh_x)
+template <int TX, int M0>
+__device__ __forceinline__ void leaf_rhs_uni_x(const double *__restrict__ tA, const double *__restrict__ tB,
+                                               const double *__restrict__ tC, const double *__restrict__ rec, uint32_t box, int l_,
+                                               EqN<1> &f, EqN<1> &l, ShLeafRegs<M0, 1> &R)
+{
+    constexpr int K = ShLeafRegs<M0, 1>::K, H = ShLeafRegs<M0, 1>::H;
+    static_assert(H == 8 && K >= 2, "x sweeps: 16- or 32-row leaves of 8-row sub-leaves");
+    double fd[K], pd[K], hold[K];
+#pragma unroll
+    for (int h = 0; h < K; ++h) {
+        const int o = h * H;
+        const double2 d2 = lds2(xs_sub<TX>(box, l_, h, 0));
+        fd[h] = d2.x * tB[o]; pd[h] = d2.y * tB[o + 1];
+        hold[h] = 0.0;
+    }
+#pragma unroll
+    for (int p = 1; p < H / 2; ++p) {
+        double2 d2[K];
+#pragma unroll
+        for (int h = 0; h < K; ++h) d2[h] = lds2(xs_sub<TX>(box, l_, h, p));
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int r = 2 * p + e;
+#pragma unroll
+            for (int h = 0; h < K; ++h) {
+                const int o = h * H + r;
+                const double dr = e ? d2[h].y : d2[h].x;
+                fd[h] = fma(-tC[o], pd[h], fd[h]);
+                if (e == 0) sts2(xs_sub<TX>(box, l_, h, p - 1), hold[h], pd[h]);
+                else hold[h] = pd[h];
+                pd[h] = fma(-tA[o], pd[h], dr) * tB[o];
+            }
+        }
+    }
+#pragma unroll
+    for (int h = 0; h < K; ++h) sts2(xs_sub<TX>(box, l_, h, 3), hold[h], 0.0);
+    leaf_finish_uni<M0>(rec, fd, pd, f, l, R);
+}
+
 // Threads: leaf = t / TX, lx = t % TX; the last warp issues the TMA copies and takes no part in
 // the tree (as in fused_tma_kernel).  Ring: tile q of the cluster lives in slot q % NA from its
 // load until the TMA store of its x has read the slot; then tile q + NA is loaded into it.
-template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB, bool kX = false>
+template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB, bool kX = false, bool kUni = false>
 __global__ void __launch_bounds__(MAXT, MINB)
 shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constant__ CUtensorMap tm_x,
                   const SharedParams prm)
@@ -354,9 +567,16 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
     const int R = prm.R, CL = prm.CL, W = prm.W, NA = prm.NS;
     const int arr = R * TXD;
     double *const raw = reinterpret_cast<double *>(smem_raw);         // NA slots of [R][TX][NC]
-    double *const cA = raw + (size_t)NA * arr, *const cB = cA + R, *const cC = cB + R;
+    static_assert(!kUni || (NC == 1 && M0 >= 8), "uniform matrix: real right-hand sides, leaves of 8 rows or more");
+    // coefficient rows of the CTA; uniform matrix: one spare row per leaf (bank spread), then the
+    // leaves' records (shared_coef_doubles on the host side is the same sum)
+    constexpr int kRec = UniLeaf<M0 >= 8 ? M0 : 8>::kRec;
+    const int LS = kUni ? M0 + 1 : M0, CR = kUni ? R + W : R;
+    double *const cA = raw + (size_t)NA * arr, *const cB = cA + CR, *const cC = cB + CR;
+    double *const rec0 = cC + CR;
+    const int coef_doubles = kUni ? ((3 * CR + W * kRec + 1) & ~1) : 3 * R;
     NodeBuf nb;                                                       // node buffer: [2W][TX] per plane
-    nb.ab = ptx::smem_u32(cC + R); nb.plane = (uint32_t)(2 * W * TX) * 16u; nb.d1 = nb.ab + 2u * nb.plane;
+    nb.ab = ptx::smem_u32(cA + coef_doubles); nb.plane = (uint32_t)(2 * W * TX) * 16u; nb.d1 = nb.ab + 2u * nb.plane;
     const uint32_t nb_bytes = 2u * nb.plane + (NC == 2 ? (uint32_t)(2 * W * TX) * 8u : 0u);
     const int NTR = 2 * CL;                                           // rows of the cluster-level system
     NodeBuf tb0;                                                      // inbox of parity 0: [NTR][TX] per plane
@@ -382,7 +602,8 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         ptx::fence_mbar_init();
     }
     for (int r = t; r < R; r += (int)blockDim.x) {             // this CTA's rows of the 1-D coefficients
-        cA[r] = prm.a_y[y0 + r]; cB[r] = prm.b0_y[y0 + r]; cC[r] = prm.c_y[y0 + r];
+        const int pr = kUni ? r + r / M0 : r;
+        cA[pr] = prm.a_y[y0 + r]; cB[pr] = prm.b0_y[y0 + r]; cC[pr] = prm.c_y[y0 + r];
     }
     __syncthreads();
     if (kCluster) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
@@ -458,7 +679,17 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         const int gi_ = xt_ * TX + lx < prm.nx ? xt_ * TX + lx : prm.nx - 1;   // ragged x tile: lanes past nx solve a copy
         return prm.sx[gi_] + prm.sz[k_ < prm.nzs ? k_ : prm.nzs - 1];
     };
-    double s_next = g < prm.ntiles ? shift_of(xt, k) : 0.0;
+    double s_next = (!kUni && g < prm.ntiles) ? shift_of(xt, k) : 0.0;     // uniform matrix: no shift arrays
+    // uniform matrix: everything that depends on the matrix alone, once per launch
+    ShLeafRegs<M0, NC> uregs;
+    EqN<NC> uf, ul;
+    if constexpr (kUni) {
+        double *const tA = cA + leaf * LS, *const tB = cB + leaf * LS, *const tC = cC + leaf * LS;
+        if (act) leaf_matrix_uni<M0>(tA, tB, tC, first_leaf, last_leaf, false, nullptr, uf, ul, uregs);
+        __syncthreads();                // every thread has read the coefficients: one thread per leaf turns them into the table
+        if (act && lx == 0) leaf_matrix_uni<M0>(tA, tB, tC, first_leaf, last_leaf, true, rec0 + leaf * kRec, uf, ul, uregs);
+        __syncthreads();
+    }
     int it = 0;
     for (int tile = g; tile < prm.ntiles; tile += NC_, ++it) {
         const int par = it & 1;
@@ -474,14 +705,19 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
         xt += step_x; k += step_k;
         if (xt >= prm.xtiles) { xt -= prm.xtiles; ++k; }
         if (++slot == NA) { slot = 0; sphase ^= 1; }
-        if (tile + NC_ < prm.ntiles) s_next = shift_of(xt, k);
+        if (!kUni && tile + NC_ < prm.ntiles) s_next = shift_of(xt, k);
         ptx::mbar_wait(&bar[cur_slot], (unsigned)cur_phase);
 
         // ---------------- leaves ----------------
         ShLeafRegs<M0, NC> regs;
         if (act) {
             EqN<NC> f, l;
-            if constexpr (kX)
+            if constexpr (kUni) {
+                f = uf; l = ul;
+                const double *const tA = cA + leaf * LS, *const tB = cB + leaf * LS, *const tC = cC + leaf * LS;
+                if constexpr (kX) leaf_rhs_uni_x<TX, M0>(tA, tB, tC, rec0 + leaf * kRec, dbase, lx, f, l, uregs);
+                else leaf_rhs_uni<M0>(tA, tB, tC, rec0 + leaf * kRec, dbase, row_bytes, f, l, uregs);
+            } else if constexpr (kX)
                 leaf_reduce_sh_x<TX, M0>(cA + leaf * M0, cB + leaf * M0, cC + leaf * M0, s, dbase, lx, first_leaf, last_leaf, pin, f, l, regs);
             else
                 leaf_reduce_sh<M0, NC>(cA + leaf * M0, cB + leaf * M0, cC + leaf * M0, s, dbase, row_bytes,
@@ -609,8 +845,8 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
 #pragma unroll
                 for (int q = 0; q < NC; ++q) { xf[q] = nf[q]; xl[q] = nla[q]; }
             }
-            if constexpr (kX) leaf_back_sh_x<TX, M0>(regs, xf, xl, dbase, lx);
-            else leaf_back_sh<M0, NC>(regs, xf, xl, dbase, row_bytes);
+            if constexpr (kX) leaf_back_sh_x<TX, M0>(kUni ? uregs : regs, xf, xl, dbase, lx);
+            else leaf_back_sh<M0, NC>(kUni ? uregs : regs, xf, xl, dbase, row_bytes);
             ptx::fence_proxy_async_smem();      // x in the slot -> visible to the TMA store
         }
     }
@@ -626,10 +862,12 @@ shared_tma_kernel(const __grid_constant__ CUtensorMap tm_d, const __grid_constan
 // ------------------------------------------------------------------------------------------
 // Host side
 // ------------------------------------------------------------------------------------------
-inline size_t shared_smem_bytes(int TX, int R, int W, int CL, int NA, int NC)
+inline size_t shared_smem_bytes(int TX, int R, int W, int CL, int NA, int NC, int uni_leaf = 0)
 {
     const size_t slots = (size_t)NA * R * TX * NC * sizeof(double);
-    const size_t coef = (size_t)3 * R * sizeof(double);
+    // uniform matrix (uni_leaf = its leaf size): padded table rows + the leaves' records, as in the kernel
+    const int rec = uni_leaf >= 32 ? UniLeaf<32>::kRec : UniLeaf<16>::kRec;
+    const size_t coef = (uni_leaf ? (size_t)((3 * (R + W) + W * rec + 1) & ~1) : (size_t)3 * R) * sizeof(double);
     const size_t node = (size_t)2 * W * TX * (32 + 8 * (NC - 1));
     const size_t inbox = CL > 1 ? (size_t)2 * 2 * CL * TX * (32 + 8 * (NC - 1)) : 0;
     return slots + coef + node + inbox + 128;
@@ -640,8 +878,9 @@ constexpr int kSharedLeafSizes[] = {32, 16, 8, 4};
 
 inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int want_lines, int want_cluster,
                                   int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why,
-                                  bool xsweep = false)
+                                  bool xsweep = false, bool uniform = false)
 {
+    if (uniform && NC != 1) { *why = "uniform matrix: real right-hand sides"; return false; }
     if (NC != 1 && NC != 2) { *why = "ncomp must be 1 (real) or 2 (complex)"; return false; }
     if (xsweep && (NC != 1 || ny % 16)) { *why = "x sweeps: real right-hand sides, line length a multiple of 16"; return false; }
     if (!xsweep && (nx * NC) % 2) { *why = "TMA path needs an even number of doubles per row (16-byte global strides)"; return false; }
@@ -653,7 +892,7 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
     for (int ti = 0; ti < 3; ++ti) {
         const int TX = tx_opts[ti];
         if (want_lines ? TX != want_lines : ti == 2) continue;      // 64-byte segments only on request
-        if (xsweep && TX != 16) continue;                           // x sweeps: 16 lines of 128-byte leaf rows
+        if ((xsweep || uniform) && TX != 16) continue;              // x sweeps: 16 lines of 128-byte leaf rows
         for (int ci = 0; ci < 4; ++ci) {
             const int CL = cl_opts[ci];
             if (want_cluster && CL != want_cluster) continue;
@@ -661,26 +900,27 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
             const int R = ny / CL;
             for (int m0 : kSharedLeafSizes) {
                 if (want_leaf && m0 != want_leaf) continue;
-                if (xsweep && m0 != 16 && m0 != 32) continue;
+                if ((xsweep || uniform) && m0 != 16 && m0 != 32) continue;
                 if (m0 > R || R % m0 || !is_pow2(R / m0) || R / m0 > 32) continue;
                 // 32-row leaves (four sub-leaves per thread) halve the tree per cell: 1.46 -> 1.05 ms on 256 slices
                 // of cfg 3 (real).  Complex cells need the registers for the second right-hand side: on request only
                 if (m0 == 32 && want_leaf != 32 && NC != 1) continue;
                 SharedConfig c;
                 c.ncomp = NC; c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
-                c.threads = c.leaves * TX; c.xsweep = xsweep ? 1 : 0;
+                c.threads = c.leaves * TX; c.xsweep = xsweep ? 1 : 0; c.uniform = uniform ? 1 : 0;
+                if (uniform && c.threads > 256) continue;
                 if (c.threads > 512 || (m0 == 32 && c.threads > 256)) continue;
                 c.box_rows = R;
                 while (c.box_rows > 256) c.box_rows /= 2;
                 if (R % c.box_rows) continue;
                 c.slots = 0;
                 for (int na = want_slots ? want_slots : 4; na >= (want_slots ? want_slots : 2); --na) {
-                    c.smem = shared_smem_bytes(TX, R, c.leaves, CL, na, NC);
+                    c.smem = shared_smem_bytes(TX, R, c.leaves, CL, na, NC, uniform ? m0 : 0);
                     if (c.smem <= max_smem) { c.slots = na; break; }
                 }
                 if (!c.slots) continue;
                 c.ctas_per_sm = 1;
-                if (want_ctas >= 2 && !xsweep) {          // co-residency: registers and shared memory shared out
+                if (want_ctas >= 2 && !xsweep && !uniform) {          // co-residency: registers and shared memory shared out
                     if (c.threads * want_ctas > 512 || m0 != 16) continue;
                     for (; c.slots >= 2; --c.slots) {
                         c.smem = shared_smem_bytes(TX, R, c.leaves, CL, c.slots, NC);
@@ -723,10 +963,10 @@ inline bool make_shared_tensor_map(CUtensorMap *tm, const void *base, int nx, in
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB = 1, bool kX = false>
+template <int TX, int M0, bool kCluster, int MAXT, int NC, int MINB = 1, bool kX = false, bool kUni = false>
 inline cudaError_t launch_shared_inst(SharedConfig &cfg, const CUtensorMap *tm, const SharedParams &prm, cudaStream_t st)
 {
-    auto kern = shared_tma_kernel<TX, M0, kCluster, MAXT, NC, MINB, kX>;
+    auto kern = shared_tma_kernel<TX, M0, kCluster, MAXT, NC, MINB, kX, kUni>;
     cudaLaunchConfig_t lc = {};
     lc.blockDim = dim3((cfg.threads + 31) & ~31);
     lc.dynamicSmemBytes = cfg.smem;
@@ -807,6 +1047,20 @@ inline cudaError_t launch_shared_impl(SharedConfig &cfg, const SharedArgs &a, cu
     prm.ntiles = prm.xtiles * a.nzs;
     prm.box_rows = cfg.box_rows; prm.nbox = cfg.rows / cfg.box_rows;
     const bool cl = cfg.cluster > 1;
+    if (cfg.uniform) {
+        if (cfg.ncomp != 1 || cfg.lines != 16 || cfg.threads > 256 || !a.uniform) return cudaErrorInvalidValue;
+        const bool xs = cfg.xsweep != 0;
+        if (cfg.leaf_rows == 32) {
+            if (xs) return cl ? launch_shared_inst<16, 32, true, 256, 1, 1, true, true>(cfg, tm, prm, st) : launch_shared_inst<16, 32, false, 256, 1, 1, true, true>(cfg, tm, prm, st);
+            return cl ? launch_shared_inst<16, 32, true, 256, 1, 1, false, true>(cfg, tm, prm, st) : launch_shared_inst<16, 32, false, 256, 1, 1, false, true>(cfg, tm, prm, st);
+        }
+        if (cfg.leaf_rows == 16) {
+            if (xs) return cl ? launch_shared_inst<16, 16, true, 256, 1, 1, true, true>(cfg, tm, prm, st) : launch_shared_inst<16, 16, false, 256, 1, 1, true, true>(cfg, tm, prm, st);
+            return cl ? launch_shared_inst<16, 16, true, 256, 1, 1, false, true>(cfg, tm, prm, st) : launch_shared_inst<16, 16, false, 256, 1, 1, false, true>(cfg, tm, prm, st);
+        }
+        return cudaErrorInvalidValue;
+    }
+    if (a.uniform) return cudaErrorInvalidValue;           // NULL shift arrays need the uniform-matrix tiling
     if (cfg.xsweep) {
         if (cfg.ncomp != 1 || cfg.lines != 16 || (cfg.leaf_rows != 16 && cfg.leaf_rows != 32)) return cudaErrorInvalidValue;
         if (cfg.leaf_rows == 32)

@@ -357,3 +357,81 @@ def test_cfg4_adi_full_size_in_shared_form_sampled():
             err = (np.max(np.abs(xn - ref), axis=ax) / np.max(np.abs(ref), axis=ax)).max()
             assert err <= TOL_E, (name, q, err)
         src = dst
+
+
+@pytest.mark.parametrize("periodic", [False, True], ids=["plain", "cyclic"])
+@pytest.mark.parametrize("axis,shape,leaf", [
+    ("y", (5, 512, 48), 0), ("y", (3, 1024, 40), 0), ("y", (6, 256, 64), 16), ("y", (4, 64, 32), 0),
+    ("z", (512, 5, 48), 0), ("z", (1024, 3, 64), 16), ("x", (3, 40, 512), 0), ("x", (2, 37, 1024), 0),
+    ("x", (4, 20, 256), 16), ("y", (2, 2048, 32), 0),
+])
+def test_uniform_matrix_equals_zero_shifts(axis, shape, leaf, periodic):
+    """sx = sz = NULL (the same matrix for every line: the ADI momentum sweeps): the
+    matrix work is hoisted out of the tile loop; x must agree with what zero shift arrays give to
+    rounding (same formulas, contracted differently), and with oracle.solve_axis within the tolerance.  One to several CTAs per line, both
+    leaf sizes, ragged line tiles, the fill launch at 1024 rows."""
+    nz, ny, nx = shape
+    n, lanes, nsl = {"y": (ny, nx, nz), "z": (nz, nx, ny), "x": (nx, ny, nz)}[axis]
+    g = torch.Generator().manual_seed(3000 + n + nsl)
+    u = lambda k, lo, hi: lo + (hi - lo) * torch.rand(k, dtype=torch.float64, generator=g)
+    a1, c1, b01 = u(n, -1, 1), u(n, -1, 1), u(n, 2.5, 3.5)
+    d = torch.randn((nz, ny, nx), dtype=torch.float64, generator=g)
+    dv = dev()
+    ax = {"y": tdma.TDMA_AXIS_Y, "z": tdma.TDMA_AXIS_Z, "x": tdma.TDMA_AXIS_X}[axis]
+    coef = [t.to(dv) for t in (a1, b01, c1)]
+    zl, zs = torch.zeros(lanes, dtype=torch.float64, device=dv), torch.zeros(nsl, dtype=torch.float64, device=dv)
+    xu, xz = [torch.full_like(d, float("nan")).to(dv) for _ in range(2)]
+    with tdma.Plan(nx, ny, nz, 1, 0, axis=ax, periodic=1 if periodic else 0, shared_lines=16,
+                   shared_leaf_rows=leaf) as plan:
+        for _ in range(2):
+            plan.solve_shared(*coef, None, None, d.to(dv), xu)
+        torch.cuda.synchronize()
+        cfg_u = [plan.get(q) for q in (tdma.TDMA_GET_SHARED_LINES, tdma.TDMA_GET_SHARED_CLUSTER, tdma.TDMA_GET_SHARED_LEAF_ROWS)]
+        plan.solve_shared(*coef, zl, zs, d.to(dv), xz)
+        torch.cuda.synchronize()
+        cfg_z = [plan.get(q) for q in (tdma.TDMA_GET_SHARED_LINES, tdma.TDMA_GET_SHARED_CLUSTER, tdma.TDMA_GET_SHARED_LEAF_ROWS)]
+    line = {"y": (1, n, 1), "z": (n, 1, 1), "x": (1, 1, n)}[axis]
+    a = a1.view(line).expand(nz, ny, nx).contiguous().numpy()
+    b = b01.view(line).expand(nz, ny, nx).contiguous().numpy()
+    c = c1.view(line).expand(nz, ny, nx).contiguous().numpy()
+    ref = oracle.solve_axis(a, b, c, d.numpy(), axis, periodic)
+    xn = xu.cpu().numpy()
+    dim = {"y": 1, "z": 0, "x": 2}[axis]
+    err = (np.max(np.abs(xn - ref), axis=dim) / np.max(np.abs(ref), axis=dim)).max()
+    assert np.isfinite(xn).all() and err <= TOL_E, err
+    assert cfg_u[0] == 16 and cfg_u[2] in (16, 32)
+    tol = 1e-13 if cfg_u == cfg_z else TOL_E        # same tiling: the same formulas in the same order
+    assert (np.max(np.abs(xn - xz.cpu().numpy()), axis=dim) / np.max(np.abs(ref), axis=dim)).max() <= tol
+
+
+def test_uniform_matrix_fallback_and_errors():
+    """Complex cells and shapes outside the uniform-matrix build run the general form with plan-owned
+    zero shifts; pin00 and a single NULL shift array are refused."""
+    dv = dev()
+    nz, ny, nx = 3, 128, 24
+    g = torch.Generator().manual_seed(5)
+    u = lambda k, lo, hi: lo + (hi - lo) * torch.rand(k, dtype=torch.float64, generator=g)
+    a1, c1, b01 = u(ny, -1, 1), u(ny, -1, 1), u(ny, 2.5, 3.5)
+    d = torch.complex(torch.randn((nz, ny, nx), dtype=torch.float64, generator=g),
+                      torch.randn((nz, ny, nx), dtype=torch.float64, generator=g))
+    coef = [t.to(dv) for t in (a1, b01, c1)]
+    zx, zz = torch.zeros(nx, dtype=torch.float64, device=dv), torch.zeros(nz, dtype=torch.float64, device=dv)
+    x1, x2 = [torch.full_like(d, float("nan")).to(dv) for _ in range(2)]
+    with tdma.Plan(nx, ny, nz, 1, 0) as plan:
+        plan.solve_shared(*coef, None, None, d.to(dv), x1)          # complex: general form, zero shifts
+        plan.solve_shared(*coef, zx, zz, d.to(dv), x2)
+        torch.cuda.synchronize()
+        assert torch.equal(x1, x2)
+        with pytest.raises(tdma.TdmaError):
+            tdma.tdma_solve_shared(plan.handle, *coef, zx, 0, 1, 0, x1.real.contiguous(), x2.real.contiguous())
+        with pytest.raises(tdma.TdmaError):
+            tdma.tdma_solve_shared(plan.handle, *coef, 0, 0, 1, 1, x1.real.contiguous(), x2.real.contiguous())
+    # real cells, 8-row leaves forced: outside the uniform build (16- / 32-row leaves) -> general form
+    dr = d.real.contiguous().to(dv)
+    y1, y2 = [torch.full_like(dr, float("nan")) for _ in range(2)]
+    with tdma.Plan(nx, ny, nz, 1, 0, shared_leaf_rows=8) as plan:
+        plan.solve_shared(*coef, None, None, dr, y1)
+        plan.solve_shared(*coef, zx, zz, dr, y2)
+        torch.cuda.synchronize()
+        assert plan.get(tdma.TDMA_GET_SHARED_LEAF_ROWS) == 8
+    assert torch.equal(y1, y2)
