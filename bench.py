@@ -642,6 +642,17 @@ def main():
                                                             cpu_seconds=args.cpu_seconds / 2)
                 except Exception as exc:
                     out["workloads"][key] = {"error": repr(exc)}
+            # NEXT row f1: BASELINE cfg 4, the ADI step (x periodic, y Dirichlet, z periodic) in the general
+            # form, the matrix-sharing form and the uniform-matrix form, each sweep checked against the oracle
+            torch.cuda.empty_cache()
+            try:
+                w4 = tdma_inputs.make_workload("cfg4_adi_y", device=dev)
+                x4 = torch.empty_like(w4.d)
+                a4 = argparse.Namespace(steps=args.steps, warmup=warmup, workload="cfg4_adi_y")
+                out["workloads"]["cfg4_adi"] = adi(torch, tdma, w4, x4, a4, barrier, rank, peak, emit=False)
+                del w4, x4
+            except Exception as exc:
+                out["workloads"]["cfg4_adi"] = {"error": repr(exc)}
     if rank == 0:
         print(json.dumps(out))
     group.close()
@@ -760,10 +771,11 @@ def yslab(torch, tdma, w, args, rank, peak):
     return 0
 
 
-def adi(torch, tdma, w, x, args, barrier, rank, peak):
+def adi(torch, tdma, w, x, args, barrier, rank, peak, emit=True):
     """BASELINE cfg 4: ADI implicit viscous sweeps, three batched solves per step (x and z periodic,
     y Dirichlet with P partitions), each a FUSED plan of its own; x1 -> x2 -> x3 chained as in an
-    ADI step.  One JSON line: time per sweep and for the whole step."""
+    ADI step.  One JSON line: time per sweep and for the whole step (emit = False: the record is
+    returned instead, for the default line's `workloads`)."""
     F = tdma.TDMA_VARIANT_FUSED
     plans = [("x", tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=F, axis=tdma.TDMA_AXIS_X, periodic=1)),
              ("y", tdma.Plan(w.nx, w.ny, w.nz, w.P, 0, variant=F)),
@@ -871,10 +883,11 @@ def adi(torch, tdma, w, x, args, barrier, rank, peak):
         rec["uniform_matrix_form"] = shared_leg(True)
         sxp.close()
         sy.close(); sz_.close()
-        print(json.dumps(rec))
+        if emit:
+            print(json.dumps(rec))
     for _, plan in plans:
         plan.close()
-    return 0
+    return 0 if emit else rec
 
 
 def sweep(torch, tdma, w, x, args, barrier, rank):
