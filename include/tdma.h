@@ -121,9 +121,12 @@ typedef struct tdma_options {
                             z-slices; FUSED TMA kernel only, nx a multiple of 16, 16-byte aligned
                             arrays including x) */
     int periodic;        /* 1 = cyclic lines: row 0 couples to row n-1 through a_0 and row n-1 to
-                            row 0 through c_{n-1} (both entries are then USED).  The cyclic
-                            coupling is resolved at the root of the recursion, so only the FUSED
-                            TMA kernel supports it */
+                            row 0 through c_{n-1} (both entries are then USED).  The wrap is
+                            resolved at the top of the recursion: at the root of the tree in the
+                            FUSED TMA kernel, in stage B's reduced system (then a cyclic 2P-row
+                            system) in the PIPELINED variant, which takes any nx and line length
+                            along y or z.  AUTO picks FUSED when the shape tiles, else PIPELINED;
+                            STAGED, pdd and the register-staged fused kernel do plain lines only */
     int timeline;        /* PIPELINED, 1 = record a timing event before and after every stage launch
                             (forces plain stream launches); read back with tdma_plan_timeline */
     int fused_slots;     /* FUSED, TMA kernel: ring slots of one raw array tile each: 4 = the next tile is
@@ -384,6 +387,9 @@ int tdma_probe_fp64(double *result, int n);
 
 int tdma_plan_destroy(tdma_plan *plan);
 const char *tdma_last_error(void); /* thread-local, never NULL */
+int tdma_last_status(void);        /* thread-local: the tdma_status that came with tdma_last_error()'s message
+                                      (what a failed tdma_plan_create*, which returns NULL, would have returned);
+                                      TDMA_OK before the first failure */
 int tdma_version(void);            /* 10000*major + 100*minor + patch */
 
 #ifdef __cplusplus

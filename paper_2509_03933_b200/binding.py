@@ -33,7 +33,7 @@ TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
 EXPORTED_SYMBOLS = (
     "tdma_plan_create", "tdma_plan_create_ex", "tdma_solve", "tdma_solve_host", "tdma_stage",
     "tdma_plan_get", "tdma_plan_workspace_bytes", "tdma_plan_buffer", "tdma_plan_destroy",
-    "tdma_last_error", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
+    "tdma_last_error", "tdma_last_status", "tdma_version", "tdma_pipeline_model", "tdma_plan_autotune", "tdma_plan_timeline",
     "tdma_solve_shared", "tdma_probe_fp64", "tdma_solve_static",
     "tdma_slab_create", "tdma_slab_get", "tdma_slab_stage_a", "tdma_slab_stage_b", "tdma_slab_stage_b_pdd", "tdma_slab_stage_c",
     "tdma_slab_set_peers", "tdma_slab_stage_a_peer", "tdma_slab_stage_b_peer", "tdma_slab_destroy",
@@ -133,6 +133,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
     lib.tdma_plan_destroy.restype = ci
     lib.tdma_last_error.argtypes = []
     lib.tdma_last_error.restype = ctypes.c_char_p
+    lib.tdma_last_status.argtypes = []
+    lib.tdma_last_status.restype = ctypes.c_int
     lib.tdma_version.argtypes = []
     lib.tdma_version.restype = ci
     lib.tdma_plan_timeline.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ci]
@@ -148,6 +150,10 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
 
 def tdma_last_error() -> str:
     return load_library().tdma_last_error().decode("utf-8", "replace")
+
+
+def tdma_last_status() -> int:
+    return int(load_library().tdma_last_status())
 
 
 def tdma_version() -> int:
@@ -183,7 +189,7 @@ def _stream_handle(stream) -> int:
 def tdma_plan_create(nx: int, ny: int, nz: int, P: int, batch: int, dtype: int = TDMA_F64) -> int:
     h = load_library().tdma_plan_create(nx, ny, nz, P, batch, dtype)
     if not h:
-        raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())
+        raise TdmaError(tdma_last_status() or TDMA_ERR_INVALID_ARG, tdma_last_error())
     return int(h)
 
 
@@ -205,7 +211,7 @@ def tdma_plan_create_ex(nx: int, ny: int, nz: int, P: int, batch: int, dtype: in
     opt.shared_ctas, opt.pdd = shared_ctas, pdd
     h = load_library().tdma_plan_create_ex(nx, ny, nz, P, batch, dtype, ctypes.byref(opt))
     if not h:
-        raise TdmaError(TDMA_ERR_INVALID_ARG, tdma_last_error())
+        raise TdmaError(tdma_last_status() or TDMA_ERR_INVALID_ARG, tdma_last_error())
     return int(h)
 
 

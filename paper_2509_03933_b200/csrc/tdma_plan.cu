@@ -24,9 +24,11 @@
 namespace {
 
 thread_local char g_err[512] = "";
+thread_local int g_err_code = TDMA_OK;
 
 int set_err(int code, const char *fmt, ...)
 {
+    g_err_code = code;
     va_list ap;
     va_start(ap, fmt);
     vsnprintf(g_err, sizeof(g_err), fmt, ap);
@@ -144,6 +146,7 @@ tdma::StageParams batch_params(const tdma_plan *pl, const SlabPtrs &ptr, int nz_
     prm.nx = pl->nx; prm.ny = pl->ny; prm.m = pl->m; prm.P = pl->P;
     prm.rs = pl->rs; prm.os = pl->os;
     prm.pg0 = 0; prm.Ptot = pl->P; prm.Ls = 0;
+    prm.cyclic = pl->periodic ? 1 : 0;
     return prm;
 }
 
@@ -181,6 +184,8 @@ int launch_stage(tdma_plan *pl, int stage, const tdma::StageParams &prm_in, cuda
         if (pl->pdd) {
             dim3 grid((Lb + 127) / 128, prm.P);
             tdma::stage_b_pdd_kernel<<<grid, 128, 0, st>>>(prm);
+        } else if (pl->periodic) {
+            tdma::stage_b_cyclic_kernel<<<(Lb + 63) / 64, 64, 0, st>>>(prm);
         } else {
             tdma::stage_b_kernel<kPrefetchRows><<<(Lb + 63) / 64, 64, 0, st>>>(prm);
         }
@@ -340,7 +345,7 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
                                    ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
         else
             return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel needs 16-byte aligned arrays%s",
-                           plain_y ? "" : " (x / z sweeps and cyclic lines have no other kernel)");
+                           plain_y ? "" : " (z sweeps and cyclic lines of such arrays: TDMA_VARIANT_PIPELINED; x sweeps have no other kernel)");
         if (e != cudaSuccess)
             return set_err(TDMA_ERR_CUDA, "fused launch failed: %s", cudaGetErrorString(e));
     }
@@ -453,7 +458,7 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
                                                       opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
                                                       prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z,
                                                       opt ? opt->fused_slots : 0);
-        variant = (tma_ok || pl->axis == TDMA_AXIS_X || pl->periodic) ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
+        variant = (tma_ok || pl->axis == TDMA_AXIS_X) ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
         if (variant == TDMA_VARIANT_FUSED) pl->batch_arg = 0;   // batch is a hint for the stage pipelines only
     }
     if (variant == TDMA_VARIANT_FUSED && pl->batch_arg == 0) {
@@ -472,8 +477,10 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         return set_err(TDMA_ERR_UNSUPPORTED, "the STAGED variant does y / z sweeps of plain lines with >= 2 rows");
     if (pl->axis == TDMA_AXIS_X && variant != TDMA_VARIANT_FUSED)
         return set_err(TDMA_ERR_UNSUPPORTED, "x sweeps need the FUSED variant (TMA kernel)");
-    if (pl->periodic && (variant != TDMA_VARIANT_FUSED || pl->ny < 2))
-        return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need the FUSED variant (TMA kernel) and >= 2 rows");
+    if (pl->periodic && pl->ny < 2)
+        return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need >= 2 rows");
+    if (pl->periodic && opt && opt->pdd > 0)
+        return set_err(TDMA_ERR_UNSUPPORTED, "pdd is defined for plain lines only");
     pl->variant = variant;
     pl->Pred = pl->P;
     pl->use_graph = (opt && opt->use_graph < 0) ? 0 : 1;
@@ -1028,6 +1035,7 @@ int tdma_plan_destroy(tdma_plan *plan)
 }
 
 const char *tdma_last_error(void) { return g_err; }
+int tdma_last_status(void) { return g_err_code; }
 int tdma_version(void) { return TDMA_VERSION_NUM; }
 
 }  // extern "C"

@@ -55,6 +55,9 @@ struct StageParams {
     double *const *peer = nullptr;
     long long peer_off = 0;
     int peer_rows = 0;
+    // cyclic lines (options.periodic): a_0 couples x_{n-1} and c_{n-1} couples x_0; stage A keeps both
+    // entries, which makes the reduced system cyclic (stage_b_cyclic_kernel); stage C is unchanged
+    int cyclic = 0;
 };
 
 // row q of stage B's solution for line l (slab: yout[dest][2 P_local][Ls], or the peer's yrecv block)
@@ -94,7 +97,7 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
     double *__restrict__ sc = prm.sc + soff0;
     double *__restrict__ sd = prm.sd + soff0;
     const size_t s = (size_t)prm.rs, ss = (size_t)nx;
-    const bool first_part = (prm.pg0 + p == 0), last_part = (prm.pg0 + p == prm.Ptot - 1);
+    const bool first_part = !prm.cyclic && (prm.pg0 + p == 0), last_part = !prm.cyclic && (prm.pg0 + p == prm.Ptot - 1);
 
     // first-row equation  fa x_{-1} + fb x_0 + fc x_frontier = fd
     double inv = 1.0 / ld_stream(b);
@@ -245,6 +248,58 @@ __global__ void __launch_bounds__(64) stage_b_kernel(const StageParams prm)
         xq = fma(-ld_keep(cpb + q * Lb), xq, ld_keep(tmp + q * Lb));
         st_keep(y_row(prm, q, l), xq);
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// Stage B for CYCLIC lines (options.periodic; the periodic sweeps of BASELINE cfg 4).
+// Stage A then leaves a_0 and c_{n-1} in place, so row 0 of the reduced system couples y_{Q-1}
+// through ra_0 and row Q-1 couples y_0 through rc_{Q-1}: a cyclic tridiagonal system with unit
+// diagonal -- the wrap is resolved here, at the level of the paper's reduced system, and nothing
+// else changes (no Sherman-Morrison pass over the full lines).  Condensation on the last unknown:
+// rows 0 .. Q-2 are a plain tridiagonal system T in y_0 .. y_{Q-2} with y_{Q-1} as a parameter,
+//     T y = rd - y_{Q-1} h0 ,    h0 = ra_0 e_0 + rc_{Q-2} e_{Q-2} ,
+// one forward elimination of T carries both right-hand sides (g' for rd, h' for h0), the back
+// substitution gives y_i = g_i - h_i y_{Q-1}, and row Q-1 fixes
+//     y_{Q-1} = (rd_{Q-1} - ra_{Q-1} g_{Q-2} - rc_{Q-1} g_0) / (1 - ra_{Q-1} h_{Q-2} - rc_{Q-1} h_0).
+// h' / h overwrite RA in place (a row is stored after it was loaded), g' / g sit where stage B parks d'.
+// ------------------------------------------------------------------------------------------
+static __global__ void __launch_bounds__(64) stage_b_cyclic_kernel(const StageParams prm)
+{
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= prm.Lb) return;
+    const size_t Lb = (size_t)prm.Lb;
+    const int Q = 2 * prm.P, n = Q - 1;                  // T has n >= 1 rows
+    double *ra = prm.ra + l;
+    const double *__restrict__ rc = prm.rc + l;
+    const double *rd = prm.rd + l;
+    double *__restrict__ cpb = prm.cp + l;
+    double *tmp = prm.peer ? prm.rd + l : prm.y + l;
+
+    double cp = ld_keep(rc), gp = ld_keep(rd), hp = ld_keep(ra);
+    if (n == 1) hp += cp;                                // Q = 2: both neighbours of y_0 are y_1
+    st_keep(cpb, cp); st_keep(tmp, gp); st_keep(ra, hp);
+    for (int q = 1; q < n; ++q) {
+        const double aq = ld_keep(ra + q * Lb), cq = ld_keep(rc + q * Lb), dq = ld_keep(rd + q * Lb);
+        const double inv = 1.0 / fma(-aq, cp, 1.0);
+        gp = fma(-aq, gp, dq) * inv;
+        hp = fma(-aq, hp, q == n - 1 ? cq : 0.0) * inv;
+        cp = cq * inv;
+        st_keep(cpb + q * Lb, cp); st_keep(tmp + q * Lb, gp); st_keep(ra + q * Lb, hp);
+    }
+    double g = gp, h = hp;                               // row n-1 of T
+    const double g_last = g, h_last = h;
+    for (int q = n - 2; q >= 0; --q) {
+        const double cq = ld_keep(cpb + q * Lb);
+        g = fma(-cq, g, ld_keep(tmp + q * Lb));
+        h = fma(-cq, h, ld_keep(ra + q * Lb));
+        st_keep(tmp + q * Lb, g); st_keep(ra + q * Lb, h);
+    }
+    // g, h: row 0.  Row Q-1 of the reduced system was not touched above.
+    const double aL = ld_keep(ra + (size_t)n * Lb), cL = ld_keep(rc + (size_t)n * Lb), dL = ld_keep(rd + (size_t)n * Lb);
+    const double yl = fma(-cL, g, fma(-aL, g_last, dL)) / fma(-cL, h, fma(-aL, h_last, 1.0));
+    st_keep(y_row(prm, Q - 1, l), yl);
+    for (int q = 0; q < n; ++q)
+        st_keep(y_row(prm, q, l), fma(-ld_keep(ra + q * Lb), yl, ld_keep(tmp + q * Lb)));
 }
 
 // ------------------------------------------------------------------------------------------

@@ -60,6 +60,15 @@ def test_unknown_dtype_rejected():
     with pytest.raises(tdma.TdmaError) as ei:
         tdma.tdma_plan_create(8, 8, 8, 2, 0, 1)
     assert "TDMA_F64" in str(ei.value)
+    # a failed tdma_plan_create returns NULL; its status travels through tdma_last_status()
+    assert ei.value.status == tdma.TDMA_ERR_UNSUPPORTED == tdma.tdma_last_status()
+
+
+def test_last_status_follows_the_last_error():
+    with pytest.raises(tdma.TdmaError) as ei:
+        tdma.tdma_plan_create(0, 8, 8, 1, 0)
+    assert ei.value.status == tdma.TDMA_ERR_INVALID_ARG == tdma.tdma_last_status()
+    assert tdma.load_library().tdma_plan_destroy(None) == tdma.tdma_last_status() < 0
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful without a GPU")

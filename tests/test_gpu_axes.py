@@ -126,9 +126,56 @@ def test_cfg4_adi_full_size_three_sweeps_sampled():
         src = dst
 
 
+@pytest.mark.parametrize("axis", ["y", "z"])
+@pytest.mark.parametrize("n,P,lanes,other,batch,nstreams", [
+    (113, 1, 31, 5, 0, 2), (12, 6, 43, 27, 26, 2), (177, 59, 1022, 3, 2, 3), (64, 4, 64, 6, 0, 1), (3, 1, 7, 4, 1, 2),
+    (768, 16, 77, 4, 3, 2), (2048, 256, 31, 2, 0, 2), (1024, 16, 256, 3, 2, 4)])
+def test_cyclic_lines_on_the_stage_pipeline(axis, n, P, lanes, other, batch, nstreams):
+    """Cyclic lines in the PIPELINED variant: stage A keeps a_0 and c_{n-1}, stage B solves the cyclic
+    2P-row reduced system, stage C is unchanged.  Any nx (odd included) and any line length, i.e. the
+    shapes the TMA kernel cannot tile; P = 1 (a two-row reduced system), ragged last batch, 1-4 streams."""
+    shape = (other, n, lanes) if axis == "y" else (n, other, lanes)
+    a, b, c, d = tdma_inputs.dominant_random(shape[2], shape[1], shape[0], 71, dev())
+    x = solve(a, b, c, d, P, batch, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1, nstreams=nstreams,
+              axis=tdma.TDMA_AXIS_Z if axis == "z" else tdma.TDMA_AXIS_Y)
+    check(a, b, c, d, x, axis, True)
+
+
+def test_cyclic_lines_auto_falls_back_to_the_stage_pipeline():
+    """AUTO: cyclic lines go to the fused TMA kernel when the shape tiles, else to PIPELINED; both against
+    the oracle, and against each other to rounding on a shape both can run."""
+    a, b, c, d = tdma_inputs.dominant_random(45, 30, 8, 73, dev())             # odd nx
+    x = torch.full_like(d, float("nan"))
+    with tdma.Plan(45, 30, 8, 5, 2, periodic=1) as plan:
+        assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_PIPELINED
+        plan.solve(a, b, c, d, x)
+        torch.cuda.synchronize()
+    check(a, b, c, d, x, "y", True)
+    a, b, c, d = tdma_inputs.dominant_random(64, 256, 6, 74, dev())
+    with tdma.Plan(64, 256, 6, 8, 0, periodic=1) as plan:
+        assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_FUSED
+    xf = solve(a, b, c, d, 8, 0, variant=tdma.TDMA_VARIANT_FUSED, periodic=1)
+    xp = solve(a, b, c, d, 8, 2, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1)
+    check(a, b, c, d, xp, "y", True)
+    assert float((xf - xp).abs().max() / xf.abs().max()) <= 1e-13
+
+
+def test_cyclic_pipelined_circulant_closed_form():
+    """cfg 4's periodic z sweep (a = c = -alpha, b = 1 + 2 alpha) through the PIPELINED variant against
+    the circulant closed form x = IFFT(FFT(d) / lambda), lambda_q = 1 + 2 alpha - 2 alpha cos(2 pi q / n)."""
+    w = tdma_inputs.make_workload("cfg4_adi_y", device=dev(), nx=48, ny=20, nz=200, P=8)
+    alpha = w.meta["alpha"]
+    x = solve(w.a, w.b, w.c, w.d, w.P, 7, variant=tdma.TDMA_VARIANT_PIPELINED, axis=tdma.TDMA_AXIS_Z, periodic=1)
+    lam = 1 + 2 * alpha - 2 * alpha * np.cos(2 * np.pi * np.arange(w.nz) / w.nz)
+    ref = np.fft.ifft(np.fft.fft(w.d.cpu().numpy(), axis=0) / lam[:, None, None], axis=0).real
+    assert np.max(np.abs(x.cpu().numpy() - ref)) <= (1 + 4 * alpha) * 1e-13 * np.max(np.abs(ref))
+
+
 def test_unsupported_combinations_fail_loudly():
+    with pytest.raises(tdma.TdmaError):            # cyclic lines: FUSED TMA kernel or PIPELINED
+        tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_STAGED, periodic=1)
     with pytest.raises(tdma.TdmaError):
-        tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1)
+        tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1, pdd=1)
     with pytest.raises(tdma.TdmaError):
         tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1, axis=tdma.TDMA_AXIS_Z)
     with pytest.raises(tdma.TdmaError):            # x sweeps: FUSED only
