@@ -118,8 +118,9 @@ typedef struct tdma_options {
                             z-slices) or TDMA_AXIS_Z = 2 (lines along z, stride nx*ny, z split into
                             P partitions, `batch` counts y-slices) or TDMA_AXIS_X = 1 (lines along
                             x, the contiguous axis, x split into P partitions, `batch` counts
-                            z-slices; FUSED TMA kernel only, nx a multiple of 16, 16-byte aligned
-                            arrays including x) */
+                            z-slices; FUSED TMA kernel: nx a multiple of 16, 16-byte aligned
+                            arrays including x; PIPELINED: any nx, with strided accesses -- the
+                            fallback AUTO takes when the TMA kernel cannot tile the lines) */
     int periodic;        /* 1 = cyclic lines: row 0 couples to row n-1 through a_0 and row n-1 to
                             row 0 through c_{n-1} (both entries are then USED).  The wrap is
                             resolved at the top of the recursion: at the root of the tree in the

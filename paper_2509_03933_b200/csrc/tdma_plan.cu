@@ -145,6 +145,7 @@ tdma::StageParams batch_params(const tdma_plan *pl, const SlabPtrs &ptr, int nz_
     prm.Lb = (long long)pl->nx * bzn;
     prm.nx = pl->nx; prm.ny = pl->ny; prm.m = pl->m; prm.P = pl->P;
     prm.rs = pl->rs; prm.os = pl->os;
+    if (pl->axis == TDMA_AXIS_X) { prm.rs = 1; prm.ls = pl->ny; }   // lines along the contiguous axis
     prm.pg0 = 0; prm.Ptot = pl->P; prm.Ls = 0;
     prm.cyclic = pl->periodic ? 1 : 0;
     return prm;
@@ -345,7 +346,7 @@ int enqueue_fused(tdma_plan *pl, const SlabPtrs &ptr, int nz_count, cudaStream_t
                                    ptr.d + off, ptr.x + off, pl->nx, pl->ny, bzn, origin);
         else
             return set_err(TDMA_ERR_UNSUPPORTED, "fused TMA kernel needs 16-byte aligned arrays%s",
-                           plain_y ? "" : " (z sweeps and cyclic lines of such arrays: TDMA_VARIANT_PIPELINED; x sweeps have no other kernel)");
+                           plain_y ? "" : " (x / z sweeps and cyclic lines of such arrays: TDMA_VARIANT_PIPELINED)");
         if (e != cudaSuccess)
             return set_err(TDMA_ERR_CUDA, "fused launch failed: %s", cudaGetErrorString(e));
     }
@@ -458,7 +459,7 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
                                                       opt ? opt->fused_cluster : 0, opt ? opt->fused_leaf_rows : 0,
                                                       prop, &why, pl->axis == TDMA_AXIS_X, pl->axis == TDMA_AXIS_Z,
                                                       opt ? opt->fused_slots : 0);
-        variant = (tma_ok || pl->axis == TDMA_AXIS_X) ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
+        variant = tma_ok ? TDMA_VARIANT_FUSED : TDMA_VARIANT_PIPELINED;
         if (variant == TDMA_VARIANT_FUSED) pl->batch_arg = 0;   // batch is a hint for the stage pipelines only
     }
     if (variant == TDMA_VARIANT_FUSED && pl->batch_arg == 0) {
@@ -475,8 +476,6 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
     if (variant == TDMA_VARIANT_STAGED && (pl->axis == TDMA_AXIS_X || pl->periodic || pl->ny < 2))
         return set_err(TDMA_ERR_UNSUPPORTED, "the STAGED variant does y / z sweeps of plain lines with >= 2 rows");
-    if (pl->axis == TDMA_AXIS_X && variant != TDMA_VARIANT_FUSED)
-        return set_err(TDMA_ERR_UNSUPPORTED, "x sweeps need the FUSED variant (TMA kernel)");
     if (pl->periodic && pl->ny < 2)
         return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need >= 2 rows");
     if (pl->periodic && opt && opt->pdd > 0)

@@ -44,6 +44,10 @@ struct StageParams {
     long long rs, os;             // caller arrays: element stride between rows of a line / between
                                   // slices (y sweep: nx, nx*ny; z sweep: nx*ny, nx); scratch is
                                   // always [slice][row][x]
+    long long ls = 1;             // ... and between neighbouring lines of a slice: 1, except for x sweeps
+                                  // (lines along the contiguous axis: rs = 1, ls = line length; the
+                                  // accesses of a warp are then strided -- the fallback for x sweeps
+                                  // the TMA kernel cannot tile)
     // y-slab decomposition (tdma_slab.cu): this launch holds partitions pg0 .. pg0+P-1
     // of Ptot; the lines of a batch are dealt out evenly, Ls to each rank (single GPU: 0, P, 0)
     int pg0 = 0, Ptot = 0;
@@ -87,7 +91,7 @@ __global__ void __launch_bounds__(128) stage_a_kernel(const StageParams prm)
     const int nx = prm.nx, m = prm.m;
     const long long kk = l / nx;
     const int i = (int)(l - kk * nx);
-    const size_t off0 = (size_t)kk * (size_t)prm.os + i + (size_t)p * m * (size_t)prm.rs;
+    const size_t off0 = (size_t)kk * (size_t)prm.os + (size_t)i * (size_t)prm.ls + (size_t)p * m * (size_t)prm.rs;
     const size_t soff0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
     const double *__restrict__ a = prm.a + off0;
     const double *__restrict__ b = prm.b + off0;
@@ -364,7 +368,7 @@ __global__ void __launch_bounds__(128) stage_c_kernel(const StageParams prm)
     const int nx = prm.nx, m = prm.m;
     const long long kk = l / nx;
     const int i = (int)(l - kk * nx);
-    const size_t off0 = (size_t)kk * (size_t)prm.os + i + (size_t)p * m * (size_t)prm.rs;
+    const size_t off0 = (size_t)kk * (size_t)prm.os + (size_t)i * (size_t)prm.ls + (size_t)p * m * (size_t)prm.rs;
     const size_t soff0 = (size_t)kk * (size_t)prm.ny * nx + i + (size_t)p * m * (size_t)nx;
     const double *__restrict__ sa = prm.sa + soff0;
     const double *__restrict__ sc = prm.sc + soff0;

@@ -141,6 +141,22 @@ def test_cyclic_lines_on_the_stage_pipeline(axis, n, P, lanes, other, batch, nst
     check(a, b, c, d, x, axis, True)
 
 
+@pytest.mark.parametrize("periodic", [0, 1])
+@pytest.mark.parametrize("shape,P,batch", [((3, 40, 115), 5, 2), ((2, 16, 49), 7, 0), ((4, 37, 18), 1, 3), ((1, 5, 3), 1, 0),
+                                           ((5, 33, 192), 3, 4), ((2, 70, 1024), 16, 1)])
+def test_x_sweep_on_the_stage_pipeline(periodic, shape, P, batch):
+    """Lines along the contiguous axis in the PIPELINED variant (one thread per (line, partition), strided
+    accesses): the fallback for line lengths the TMA kernel cannot tile -- odd nx, nx not a multiple of 16 --
+    and what AUTO resolves to for them."""
+    nz, ny, nx = shape
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 43, dev())
+    x = solve(a, b, c, d, P, batch, variant=tdma.TDMA_VARIANT_PIPELINED, axis=tdma.TDMA_AXIS_X, periodic=periodic)
+    check(a, b, c, d, x, "x", bool(periodic))
+    if nx % 16:
+        with tdma.Plan(nx, ny, nz, P, batch, axis=tdma.TDMA_AXIS_X, periodic=periodic) as plan:
+            assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_PIPELINED
+
+
 def test_cyclic_lines_auto_falls_back_to_the_stage_pipeline():
     """AUTO: cyclic lines go to the fused TMA kernel when the shape tiles, else to PIPELINED; both against
     the oracle, and against each other to rounding on a shape both can run."""
@@ -178,8 +194,8 @@ def test_unsupported_combinations_fail_loudly():
         tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1, pdd=1)
     with pytest.raises(tdma.TdmaError):
         tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1, axis=tdma.TDMA_AXIS_Z)
-    with pytest.raises(tdma.TdmaError):            # x sweeps: FUSED only
-        tdma.Plan(32, 32, 32, 2, 0, variant=tdma.TDMA_VARIANT_PIPELINED, axis=tdma.TDMA_AXIS_X)
+    with pytest.raises(tdma.TdmaError):            # x sweeps: FUSED (TMA kernel) or PIPELINED
+        tdma.Plan(32, 32, 32, 2, 0, variant=tdma.TDMA_VARIANT_STAGED, axis=tdma.TDMA_AXIS_X)
     with pytest.raises(tdma.TdmaError):            # x sweeps: 16-row leaves must tile the partitions
         tdma.Plan(24, 32, 32, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X)
     with pytest.raises(tdma.TdmaError):

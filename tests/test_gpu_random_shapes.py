@@ -1,7 +1,7 @@
 """Seeded random sweep over shapes and options of tdma_solve / tdma_solve_shared (through the C ABI)
 against the oracle: every case either solves within the 1e-11 tolerance of G9 or is refused at plan
-creation / solve with TDMA_ERR_UNSUPPORTED -- never a wrong x, never a non-finite one, and a plain y or
-z sweep under the AUTO variant is never refused (PIPELINED takes what the TMA kernels cannot tile).
+creation / solve with TDMA_ERR_UNSUPPORTED -- never a wrong x, never a non-finite one, and under the AUTO
+and PIPELINED variants nothing is refused (the stage pipeline takes what the TMA kernels cannot tile).
 The shapes mix the line lengths the kernels tile (2^k, 3 * 2^k, 5 * 2^k), lengths they cannot, odd and
 ragged nx, one-row partitions' neighbours (m = 2), ragged last batches, cyclic lines, all sweep axes."""
 import numpy as np
@@ -67,7 +67,7 @@ def test_random_shapes_general_form(seed):
                 torch.cuda.synchronize()
         except tdma.TdmaError as e:
             assert e.status == tdma.TDMA_ERR_UNSUPPORTED, tag + ": " + str(e)
-            assert not (vname in ("auto", "pipelined") and axis != "x"), tag + " refused: " + str(e)
+            assert vname not in ("auto", "pipelined"), tag + " refused: " + str(e)
             refused += 1
             continue
         an, bn, cn, dn, xn = [t.cpu().numpy() for t in (a, b, c, d, x)]

@@ -181,8 +181,16 @@ def test_unsupported_shapes_fail_loudly():
         with pytest.raises(tdma.TdmaError) as e3:         # x sweeps take real right-hand sides only
             tdma.tdma_solve_shared(plan.handle, *t[:5], 2, 0, t[5], torch.empty_like(t[5]))
         assert e3.value.status == tdma.TDMA_ERR_UNSUPPORTED
-    with pytest.raises(tdma.TdmaError):                   # x lines of 40 cells: not whole 16-cell leaves (no such plan)
-        tdma.Plan(40, 32, 2, 1, 0, axis=tdma.TDMA_AXIS_X)
+    # x lines of 40 cells are not whole 16-cell leaves: tdma_solve takes the stage pipeline for them
+    # (AUTO), the shared form has no kernel for them
+    g = torch.Generator().manual_seed(3)
+    rnd = lambda *shape: torch.rand(*shape, dtype=torch.float64, generator=g).to(dv)
+    with tdma.Plan(40, 32, 2, 1, 0, axis=tdma.TDMA_AXIS_X) as plan:
+        assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_PIPELINED
+        with pytest.raises(tdma.TdmaError) as e4:
+            plan.solve_shared(rnd(40) - 0.5, rnd(40) + 3.0, rnd(40) - 0.5, -rnd(32), -rnd(2), rnd(2, 32, 40),
+                              torch.empty(2, 32, 40, dtype=torch.float64, device=dv))
+        assert e4.value.status == tdma.TDMA_ERR_UNSUPPORTED
 
 
 @pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
