@@ -199,8 +199,14 @@ int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, con
  * cells run the general form with plan-owned zero shifts (allocated at the first such call).
  * P and batch are not used: the line is cut into the kernel's own leaves (D1); one
  * persistent launch (plus the fill launch, see fused_fill) per call.
- * TDMA_ERR_UNSUPPORTED when ny does not tile (ny = CL * W * M0, CL in 1,2,4,8, W a power of two
- * <= 32, M0 in 4,8,16) or nx*ncomp is odd.  Enqueue-only. */
+ * GENERAL SHAPES.  The tiled kernel needs ny = CL * W * M0 (CL in 1,2,4,8, W a power of two <= 32, M0 in
+ * 4,8,16,32), an even nx*ncomp, real cells for x sweeps and 16-byte aligned d, x.  Everything else (any
+ * ny >= 1, odd nx, complex cells along x, 8-byte aligned arrays) runs a one-thread-per-line Thomas kernel
+ * with the matrix rebuilt on the fly: correct for every shape, not fast (48 instead of 16 B per real cell:
+ * c' travels through a plan-owned scratch array of at most 256 MiB, allocated at the first such call, and
+ * d' through x; x sweeps strided) -- unless a tiling was requested through the shared_* options, in which
+ * case the call fails with TDMA_ERR_UNSUPPORTED.  TDMA_GET_SHARED_LINE_KERNEL tells which one ran.
+ * Enqueue-only. */
 int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const void *c_y,
                       const void *sx, const void *sz, int ncomp, int pin00, const void *d, void *x,
                       void *stream);
@@ -248,7 +254,9 @@ typedef enum tdma_query {
     TDMA_GET_SHARED_LINES = 17, TDMA_GET_SHARED_CLUSTER = 18, TDMA_GET_SHARED_LEAF_ROWS = 19,
     TDMA_GET_SHARED_THREADS = 20, TDMA_GET_SHARED_SMEM = 21, TDMA_GET_SHARED_SLOTS = 22,
     TDMA_GET_SHARED_FILL = 23,     /* z-slices its fill launch took */
-    TDMA_GET_REDUCED_PARTITIONS = 24 /* partitions per line in the reduced buffers (P; STAGED: see there) */
+    TDMA_GET_REDUCED_PARTITIONS = 24, /* partitions per line in the reduced buffers (P; STAGED: see there) */
+    TDMA_GET_SHARED_LINE_KERNEL = 25  /* 1: the last tdma_solve_shared ran the one-thread-per-line kernel (a shape or
+                                         alignment the tiled kernel does not take; TDMA_GET_SHARED_* are then 0) */
 } tdma_query;
 int tdma_plan_get(const tdma_plan *plan, int what); /* < 0 on error */
 size_t tdma_plan_workspace_bytes(const tdma_plan *plan); /* device bytes the plan owns */

@@ -27,7 +27,7 @@ TDMA_STAGE_A, TDMA_STAGE_GATHER, TDMA_STAGE_B, TDMA_STAGE_C = 0, 1, 2, 3
  TDMA_GET_FUSED_LEAF_ROWS, TDMA_GET_FUSED_TOP, TDMA_GET_FUSED_THREADS, TDMA_GET_FUSED_SMEM,
  TDMA_GET_FUSED_TOP_ROWS, TDMA_GET_FUSED_IMPL, TDMA_GET_FUSED_FILL, TDMA_GET_SHARED_LINES,
  TDMA_GET_SHARED_CLUSTER, TDMA_GET_SHARED_LEAF_ROWS, TDMA_GET_SHARED_THREADS, TDMA_GET_SHARED_SMEM,
- TDMA_GET_SHARED_SLOTS, TDMA_GET_SHARED_FILL, TDMA_GET_REDUCED_PARTITIONS) = range(25)
+ TDMA_GET_SHARED_SLOTS, TDMA_GET_SHARED_FILL, TDMA_GET_REDUCED_PARTITIONS, TDMA_GET_SHARED_LINE_KERNEL) = range(26)
 (TDMA_BUF_RA, TDMA_BUF_RC, TDMA_BUF_RD, TDMA_BUF_Y, TDMA_BUF_SA, TDMA_BUF_SC, TDMA_BUF_SD) = range(7)
 
 EXPORTED_SYMBOLS = (

@@ -19,6 +19,7 @@ UNITS = {
     "tdma_plan.cu": ["tdma_stage_kernels.cuh", "tdma_fused.cuh", "tdma_fused_tma.cuh", "tdma_shared.h", "tdma_staged.h", _TDMA_H],
     "tdma_staged.cu": ["tdma_fused_tma.cuh", "tdma_staged.h"],
     "tdma_shared.cu": ["tdma_shared_tma.cuh", "tdma_fused_tma.cuh", "tdma_shared.h"],
+    "tdma_shared_lines.cu": ["tdma_shared.h"],
     "tdma_probe.cu": [_TDMA_H],
     "tdma_slab.cu": ["tdma_stage_kernels.cuh", "tdma_staged.h", _TDMA_H],
     "tdma_static.cu": ["tdma_stage_kernels.cuh", _TDMA_H],

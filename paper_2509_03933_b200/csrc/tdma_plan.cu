@@ -107,6 +107,9 @@ struct tdma_plan {
     double *sh_zero = nullptr;    // zero shifts, for uniform-matrix calls on shapes the uniform tiling does not cover
     int sh_opt[5] = {0, 0, 0, 0, 0}; // options.shared_lines / _cluster / _leaf_rows / _slots / _ctas
     int sh_last = -1, sh_fill_last = 0;
+    double *sh_lines = nullptr;        // scratch of the general-shape shared kernel (c', h' of a chunk of slices)
+    size_t sh_lines_doubles = 0;
+    int sh_lines_last = 0;             // 1: the last tdma_solve_shared ran the general-shape kernel
     // host staging (tdma_solve_host), allocated on first use
     int hz = 0;  // slices per host chunk
     int host_chunk = 0;  // options.host_chunk (0 = auto)
@@ -420,7 +423,7 @@ void free_plan(tdma_plan *pl)
     if (!pl) return;
     for (auto &g : pl->graphs) cudaGraphExecDestroy(g.exec);
     for (auto ev : pl->tl_ev) cudaEventDestroy(ev);
-    cudaFree(pl->scratch); cudaFree(pl->red); cudaFree(pl->send); cudaFree(pl->sh_zero);
+    cudaFree(pl->scratch); cudaFree(pl->red); cudaFree(pl->send); cudaFree(pl->sh_zero); cudaFree(pl->sh_lines);
     if (pl->staged.impl) tdma::free_staged(&pl->staged);
     for (int s = 0; s < 2; ++s)
         for (int i = 0; i < 5; ++i) cudaFree(pl->stage_dev[s][i]);
@@ -600,6 +603,51 @@ int check_ptrs(const tdma_plan *plan, const void *a, const void *b, const void *
 
 }  // namespace
 
+namespace {
+
+// tdma_solve_shared on shapes / alignments the tiled TMA kernel does not take: one thread per line
+// (tdma_shared_lines.cu), the z range in chunks whose c' (and h' for cyclic lines) fit a plan-owned
+// scratch array of at most 256 MiB (one slice, if a slice alone needs more), allocated at the first such call.
+int shared_lines_solve(tdma_plan *pl, const void *a_y, const void *b0_y, const void *c_y, const void *sx, const void *sz,
+                       int ncomp, int pin00, const void *d, void *x, cudaStream_t st)
+{
+    if (pl->periodic && pl->ny < 2) return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: cyclic lines need >= 2 rows");
+    const size_t per_slice = (size_t)pl->ny * (size_t)pl->nx * (pl->periodic ? 2 : 1);   // doubles of scratch
+    const size_t budget = (size_t)32 << 20;
+    long long sl = (long long)std::max<size_t>(1, budget / per_slice);
+    if (sl > pl->nz) sl = pl->nz;
+    const size_t need = per_slice * (size_t)sl;
+    if (need > pl->sh_lines_doubles) {
+        cudaFree(pl->sh_lines);
+        pl->sh_lines = nullptr; pl->sh_lines_doubles = 0;
+        if (cudaMalloc(&pl->sh_lines, need * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            return set_err(TDMA_ERR_ALLOC, "tdma_solve_shared: cannot allocate %zu bytes of line scratch", need * sizeof(double));
+        }
+        pl->sh_lines_doubles = need;
+    }
+    tdma::SharedLineArgs args;
+    args.a_y = (const double *)a_y; args.b0_y = (const double *)b0_y; args.c_y = (const double *)c_y;
+    args.sx = (const double *)sx; args.sz = (const double *)sz;
+    args.n = pl->ny; args.lanes = pl->nx;
+    args.ncomp = ncomp; args.pin00 = pin00 ? 1 : 0; args.periodic = pl->periodic ? 1 : 0;
+    if (pl->axis == TDMA_AXIS_X) { args.rs = 1; args.ls = pl->ny; args.os = (long long)pl->nx * pl->ny; }
+    else { args.rs = pl->rs; args.ls = 1; args.os = pl->os; }
+    for (long long k0 = 0; k0 < pl->nz; k0 += sl) {
+        const long long n = std::min<long long>(sl, pl->nz - k0);
+        const size_t off = (size_t)k0 * (size_t)args.os * (size_t)ncomp;
+        args.d = (const double *)d + off; args.x = (double *)x + off;
+        args.k0 = (int)k0; args.slices = (int)n;
+        args.cs = pl->sh_lines; args.hs = pl->sh_lines + (size_t)pl->ny * (size_t)pl->nx * (size_t)n;
+        const cudaError_t e = tdma::launch_shared_lines(args, st);
+        if (e != cudaSuccess) return set_err(TDMA_ERR_CUDA, "shared line-kernel launch failed: %s", cudaGetErrorString(e));
+    }
+    pl->sh_last = -1; pl->sh_fill_last = 0; pl->sh_lines_last = 1;
+    return TDMA_OK;
+}
+
+}  // namespace
+
 namespace tdma {
 // for the library's other translation units: sets the calling thread's tdma_last_error() message
 int report_error(int code, const char *msg) { return set_err(code, "%s", msg); }
@@ -685,14 +733,29 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
     if (!uniform && (!sx || !sz)) return set_err(TDMA_ERR_INVALID_ARG, "NULL shift array (pass both as NULL for a uniform matrix)");
     if (uniform && pin00) return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: pin00 changes one line's matrix; pass shift arrays");
     const bool xsw = pl->axis == TDMA_AXIS_X;
-    if (xsw && ncomp != 1)
-        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: x sweeps take real right-hand sides (ncomp = 1)");
+    cudaStream_t origin = (cudaStream_t)stream;
     if (pl->periodic && pin00)
         return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: pin00 is for plain lines");
-    if ((((uintptr_t)d | (uintptr_t)x) & 15) != 0)
-        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared needs 16-byte aligned d and x (tensor maps)");
-    cudaStream_t origin = (cudaStream_t)stream;
-    if (pl->ny == 1) return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared needs ny >= 4");
+    if ((((uintptr_t)d | (uintptr_t)x) & 7) != 0)
+        return set_err(TDMA_ERR_INVALID_ARG, "tdma_solve_shared: d and x must be 8-byte aligned");
+    // What the tiled TMA kernel does not take goes to the one-thread-per-line kernel, unless the caller
+    // asked for a particular tiling (then the refusal is the answer).
+    const bool asked = pl->sh_opt[0] || pl->sh_opt[1] || pl->sh_opt[2] || pl->sh_opt[3] || pl->sh_opt[4];
+    const void *sx_in = sx, *sz_in = sz;
+    auto line_kernel = [&]() { return shared_lines_solve(pl, a_y, b0_y, c_y, sx_in, sz_in, ncomp, pin00, d, x, origin); };
+    pl->sh_lines_last = 0;
+    if (xsw && ncomp != 1) {
+        if (!asked) return line_kernel();
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: the tiled x sweep takes real right-hand sides (ncomp = 1)");
+    }
+    if ((((uintptr_t)d | (uintptr_t)x) & 15) != 0) {
+        if (!asked) return line_kernel();
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: the tiled kernel needs 16-byte aligned d and x (tensor maps)");
+    }
+    if (pl->ny == 1) {
+        if (!asked) return line_kernel();
+        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared: the tiled kernel needs ny >= 4");
+    }
     if (uniform && ncomp == 1 && pl->sh_state[2] == 0) {
         // the uniform-matrix build covers 16-line tiles with 16- / 32-row leaves and up to 256 threads
         cudaDeviceProp prop;
@@ -730,6 +793,7 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         if (!tdma::configure_shared(&pl->sh[q], pl->nx, pl->ny, ncomp, pl->sh_opt[0], pl->sh_opt[1], pl->sh_opt[2],
                                     pl->sh_opt[3], pl->sh_opt[4], prop, &why, xsw)) {
             pl->sh_state[q] = -1;
+            if (!asked) return line_kernel();
             return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared unavailable for this shape: %s", why ? why : "?");
         }
         pl->sm_count = prop.multiProcessorCount;
@@ -741,8 +805,10 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
         }
         pl->sh_state[q] = 1;
     }
-    if (pl->sh_state[q] < 0)
+    if (pl->sh_state[q] < 0) {
+        if (!asked) return line_kernel();
         return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_shared unavailable for this shape (see the first call)");
+    }
     tdma::SharedArgs args;
     args.a_y = (const double *)a_y; args.b0_y = (const double *)b0_y; args.c_y = (const double *)c_y;
     args.sx = (const double *)sx; args.sz = (const double *)sz;
@@ -994,6 +1060,7 @@ int tdma_plan_get(const tdma_plan *plan, int what)
     case TDMA_GET_SHARED_SMEM: return plan->sh_last < 0 ? 0 : (int)plan->sh[plan->sh_last].smem;
     case TDMA_GET_SHARED_SLOTS: return plan->sh_last < 0 ? 0 : plan->sh[plan->sh_last].slots;
     case TDMA_GET_REDUCED_PARTITIONS: return plan->Pred;
+    case TDMA_GET_SHARED_LINE_KERNEL: return plan->sh_lines_last;
     case TDMA_GET_SHARED_FILL: return plan->sh_last < 0 ? 0 : plan->sh_fill_last;
     default: return set_err(TDMA_ERR_INVALID_ARG, "unknown query %d", what);
     }

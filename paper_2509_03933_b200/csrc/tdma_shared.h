@@ -50,4 +50,17 @@ bool configure_shared(SharedConfig *out, int nx, int ny, int ncomp, int want_lin
 // nzs = 0: prepare only (function attributes, persistent grid size).
 cudaError_t launch_shared(SharedConfig &cfg, const SharedArgs &args, cudaStream_t st);
 
+// General-shape kernel (tdma_shared_lines.cu): one thread per line, plain Thomas over the whole line.
+struct SharedLineArgs {
+    const double *a_y, *b0_y, *c_y;   // [n] device
+    const double *sx, *sz;            // [lanes], [all slices] device, or both NULL (uniform matrix)
+    const double *d;                  // slice k0
+    double *x;
+    double *cs, *hs;                  // scratch [n][lanes * slices] each; hs for cyclic lines only
+    int n, lanes, slices, k0;         // rows per line, lines side by side, slices of this launch, its first slice
+    long long rs, ls, os;             // CELLS between rows of a line / neighbouring lines / slices
+    int ncomp, pin00, periodic;
+};
+cudaError_t launch_shared_lines(const SharedLineArgs &args, cudaStream_t st);
+
 }  // namespace tdma

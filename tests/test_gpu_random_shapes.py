@@ -90,16 +90,17 @@ def as_lines(x):
 @pytest.mark.parametrize("seed", [11, 22, 33])
 def test_random_shapes_shared_form(seed):
     """tdma_solve_shared along y: real / complex cells, per-line shifts or a uniform matrix, plain or cyclic
-    lines, in place or not; ny that the kernel tiles and ny it must refuse; odd, ragged and tiny nx."""
+    lines, in place or not; ny that the tiled kernel takes and ny that go to the one-thread-per-line kernel;
+    odd, ragged and tiny nx.  Nothing is refused."""
     rng = np.random.RandomState(seed)
     pool_n = [4, 8, 16, 32, 48, 64, 96, 128, 192, 256, 384, 512, 640, 768, 1024, 2048, 4096]
-    solved = refused = 0
+    tiled = lines = 0
     for it in range(50):
         ny = int(rng.choice(pool_n)) if rng.rand() < 0.85 else int(rng.randint(2, 300))
         nx = int(rng.choice(POOL_L)) if rng.rand() < 0.7 else int(rng.randint(1, 80))
         nz = int(rng.randint(1, max(1, min(40, (1 << 19) // (ny * nx))) + 1))
         cplx, uniform = bool(rng.rand() < 0.4), bool(rng.rand() < 0.3)
-        periodic, inplace = int(rng.rand() < 0.25), bool(rng.rand() < 0.3)
+        periodic, inplace = int(rng.rand() < 0.25) if ny >= 3 else 0, bool(rng.rand() < 0.3)
         tag = "seed %d case %d: shape %s cplx %d uniform %d periodic %d inplace %d" % (seed, it, (nz, ny, nx), cplx,
                                                                                      uniform, periodic, inplace)
         g = torch.Generator().manual_seed(100 * seed + it)
@@ -113,15 +114,14 @@ def test_random_shapes_shared_form(seed):
             sx, sz = torch.zeros(nx, dtype=torch.float64), torch.zeros(nz, dtype=torch.float64)
         dd = d.to(dev())
         x = dd.clone() if inplace else torch.full_like(dd, float("nan"))
-        try:
-            with tdma.Plan(nx, ny, nz, 1, 0, **(dict(periodic=1) if periodic else {})) as plan:
-                plan.solve_shared(a_y.to(dev()), b0_y.to(dev()), c_y.to(dev()), None if uniform else sx.to(dev()),
-                                  None if uniform else sz.to(dev()), x if inplace else dd, x)
-                torch.cuda.synchronize()
-        except tdma.TdmaError as e:
-            assert e.status == tdma.TDMA_ERR_UNSUPPORTED, tag + ": " + str(e)
-            refused += 1
-            continue
+        with tdma.Plan(nx, ny, nz, 1, 0, **(dict(periodic=1) if periodic else {})) as plan:
+            plan.solve_shared(a_y.to(dev()), b0_y.to(dev()), c_y.to(dev()), None if uniform else sx.to(dev()),
+                              None if uniform else sz.to(dev()), x if inplace else dd, x)
+            torch.cuda.synchronize()
+            if plan.get(tdma.TDMA_GET_SHARED_LINE_KERNEL):
+                lines += 1
+            else:
+                tiled += 1
         xn = x.cpu().numpy()
         assert np.isfinite(as_lines(xn)).all(), tag
         if periodic:                                        # the materialised cyclic lines, one component at a time
@@ -137,5 +137,4 @@ def test_random_shapes_shared_form(seed):
                                         pin00=False, precision="f64")
         E = oracle.normwise_error(as_lines(xn), as_lines(ref)).max()
         assert E <= TOL_E, tag + ": E = %.3e" % E
-        solved += 1
-    assert solved >= 15 and solved + refused == 50
+    assert tiled >= 10 and lines >= 10 and tiled + lines == 50

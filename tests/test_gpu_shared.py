@@ -160,37 +160,135 @@ def test_matches_general_path_on_materialised_arrays():
     assert oracle.normwise_error(xs.cpu().numpy(), xg.cpu().numpy()).max() <= TOL_E
 
 
-def test_unsupported_shapes_fail_loudly():
+def test_requested_tilings_that_do_not_fit_fail_loudly():
+    """A tiling asked for through the shared_* options is never replaced by another kernel: shapes it does
+    not fit are refused (without such a request the one-thread-per-line kernel takes them, see
+    test_line_kernel_takes_every_shape)."""
     dv = dev()
-    def attempt(nx, ny, cplx):
+    def attempt(nx, ny, cplx, **opts):
         w = random_shared(2, ny, nx, cplx, seed=1)
-        return gpu_solve_shared(w)
+        return gpu_solve_shared(w, **opts)
     with pytest.raises(tdma.TdmaError) as e1:
-        attempt(32, 24, False)                       # 24 rows: no power-of-two tree of 4/8/16-row leaves
+        attempt(32, 24, False, shared_leaf_rows=8)   # 24 rows: no power-of-two tree of 8-row leaves
     assert e1.value.status == tdma.TDMA_ERR_UNSUPPORTED
     with pytest.raises(tdma.TdmaError) as e2:
-        attempt(33, 64, False)                       # odd nx, real: 8-byte global strides
+        attempt(33, 64, False, shared_cluster=1)     # odd nx, real: 8-byte global strides
     assert e2.value.status == tdma.TDMA_ERR_UNSUPPORTED
-    attempt(33, 64, True)                            # complex cells are 16 bytes: fine
+    attempt(33, 64, True, shared_cluster=1)          # complex cells are 16 bytes: fine
     w = random_shared(2, 64, 32, False, seed=1)
     t = [v.to(dv) for v in (w.a_y, w.b0_y, w.c_y, w.sx, w.sz, w.d)]
     with tdma.Plan(32, 64, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, periodic=1) as plan:
         with pytest.raises(tdma.TdmaError):               # the pinned mean mode belongs to plain lines
             plan.solve_shared(*t, torch.empty_like(t[5]), pin00=True)
-    with tdma.Plan(64, 32, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X) as plan:
-        with pytest.raises(tdma.TdmaError) as e3:         # x sweeps take real right-hand sides only
+    with tdma.Plan(64, 32, 2, 1, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X, shared_leaf_rows=16) as plan:
+        with pytest.raises(tdma.TdmaError) as e3:         # the tiled x sweep takes real right-hand sides only
             tdma.tdma_solve_shared(plan.handle, *t[:5], 2, 0, t[5], torch.empty_like(t[5]))
         assert e3.value.status == tdma.TDMA_ERR_UNSUPPORTED
-    # x lines of 40 cells are not whole 16-cell leaves: tdma_solve takes the stage pipeline for them
-    # (AUTO), the shared form has no kernel for them
+    # x lines of 40 cells are not whole 16-cell leaves
     g = torch.Generator().manual_seed(3)
     rnd = lambda *shape: torch.rand(*shape, dtype=torch.float64, generator=g).to(dv)
-    with tdma.Plan(40, 32, 2, 1, 0, axis=tdma.TDMA_AXIS_X) as plan:
+    with tdma.Plan(40, 32, 2, 1, 0, axis=tdma.TDMA_AXIS_X, shared_leaf_rows=16) as plan:
         assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_PIPELINED
         with pytest.raises(tdma.TdmaError) as e4:
             plan.solve_shared(rnd(40) - 0.5, rnd(40) + 3.0, rnd(40) - 0.5, -rnd(32), -rnd(2), rnd(2, 32, 40),
                               torch.empty(2, 32, 40, dtype=torch.float64, device=dv))
         assert e4.value.status == tdma.TDMA_ERR_UNSUPPORTED
+
+
+def shared_case(axis, shape, cplx, seed):
+    """1-D coefficients, shifts and d of a strictly dominant shared-coefficient case along `axis`, and the
+    materialised (a, b, c) with the diagonal formed as the kernels form it, b0 - (s_lane + s_slice)."""
+    nz, ny, nx = shape
+    n, lanes, nsl = {"y": (ny, nx, nz), "z": (nz, nx, ny), "x": (nx, ny, nz)}[axis]
+    g = torch.Generator().manual_seed(seed)
+    u = lambda k, lo, hi: lo + (hi - lo) * torch.rand(k, dtype=torch.float64, generator=g)
+    a1, c1, b01 = u(n, -1, 1), u(n, -1, 1), u(n, 2.5, 3.5)
+    s_lane, s_slice = -u(lanes, 0, 2), -u(nsl, 0, 2)
+    d = torch.randn(shape, dtype=torch.float64, generator=g)
+    if cplx:
+        d = torch.complex(d, torch.randn(shape, dtype=torch.float64, generator=g))
+    line = {"y": (1, n, 1), "z": (n, 1, 1), "x": (1, 1, n)}[axis]
+    lane = {"y": (1, 1, lanes), "z": (1, 1, lanes), "x": (1, lanes, 1)}[axis]
+    slc = {"y": (nsl, 1, 1), "z": (1, nsl, 1), "x": (nsl, 1, 1)}[axis]
+    def materialise(uniform):
+        shift = torch.zeros(shape, dtype=torch.float64) if uniform else (s_lane.view(lane) + s_slice.view(slc)).expand(shape)
+        a = a1.view(line).expand(shape).contiguous().numpy()
+        c = c1.view(line).expand(shape).contiguous().numpy()
+        b = (b01.view(line) - shift).contiguous().numpy()
+        return a, b, c
+    return (a1, b01, c1, s_lane, s_slice, d), materialise
+
+
+def check_axis(a, b, c, d, x, axis, periodic):
+    xn = x.cpu().numpy()
+    ax = {"y": 1, "z": 0, "x": 2}[axis]
+    for part in (("real", "imag") if np.iscomplexobj(xn) else (None,)):
+        dn = np.ascontiguousarray(getattr(d.numpy(), part)) if part else d.numpy()
+        xp = getattr(xn, part) if part else xn
+        if periodic and a.shape[ax] == 2:
+            # two-row ring, by Cramer's rule: [[b_0, a_0 + c_0], [a_1 + c_1, b_1]] x = d  (the oracle's
+            # Sherman-Morrison form needs n >= 3)
+            t = lambda v, r: np.take(v, r, axis=ax)
+            m01, m10 = t(a, 0) + t(c, 0), t(a, 1) + t(c, 1)
+            det = t(b, 0) * t(b, 1) - m01 * m10
+            ref = np.stack([(t(dn, 0) * t(b, 1) - m01 * t(dn, 1)) / det, (t(b, 0) * t(dn, 1) - m10 * t(dn, 0)) / det], axis=ax)
+        else:
+            ref = oracle.solve_axis(a, b, c, dn, axis, periodic)
+        err = (np.max(np.abs(xp - ref), axis=ax) / np.max(np.abs(ref), axis=ax)).max()
+        assert np.isfinite(xp).all() and err <= TOL_E, err
+
+
+@pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
+@pytest.mark.parametrize("periodic", [False, True], ids=["plain", "cyclic"])
+@pytest.mark.parametrize("axis,shape", [
+    ("y", (3, 24, 32)), ("y", (4, 100, 33)), ("y", (2, 200, 7)), ("y", (5, 2, 9)), ("y", (3, 3, 1)), ("y", (2, 1000, 64)),
+    ("z", (100, 3, 33)), ("z", (37, 5, 16)), ("x", (3, 9, 40)), ("x", (2, 5, 115)), ("x", (2, 3, 64))])
+def test_line_kernel_takes_every_shape(axis, shape, periodic, cplx):
+    """tdma_solve_shared on what the tiled TMA kernel refuses -- line lengths without a power-of-two tree of
+    4- .. 32-row leaves, odd nx with real cells, complex cells along x: the one-thread-per-line kernel,
+    y / z / x sweeps, plain and cyclic lines, per-line shifts and the uniform matrix, in place."""
+    if axis == "x" and shape[2] % 16 == 0 and not cplx:
+        pytest.skip("the tiled x-sweep kernel takes this one")
+    (a1, b01, c1, s_lane, s_slice, d), materialise = shared_case(axis, shape, cplx, seed=sum(shape))
+    nz, ny, nx = shape
+    dv = dev()
+    opts = dict(periodic=1 if periodic else 0)
+    if axis != "y":
+        opts["axis"] = {"z": tdma.TDMA_AXIS_Z, "x": tdma.TDMA_AXIS_X}[axis]
+    coef = [t.to(dv) for t in (a1, b01, c1)]
+    x = torch.full_like(d, float("nan")).to(dv)
+    xu = d.clone().to(dv)                                     # the uniform-matrix solve runs in place
+    with tdma.Plan(nx, ny, nz, 1, 0, **opts) as plan:
+        plan.solve_shared(*coef, s_lane.to(dv), s_slice.to(dv), d.to(dv), x)
+        assert plan.get(tdma.TDMA_GET_SHARED_LINE_KERNEL) == 1 and plan.get(tdma.TDMA_GET_SHARED_THREADS) == 0
+        plan.solve_shared(*coef, None, None, xu, xu)
+        torch.cuda.synchronize()
+    check_axis(*materialise(False), d, x, axis, periodic)
+    check_axis(*materialise(True), d, xu, axis, periodic)
+
+
+def test_line_kernel_pinned_row_and_unaligned_arrays():
+    """pin00 on the line kernel (ny = 100), and d / x that are only 8-byte aligned on a shape the tiled kernel
+    would take (ny = 64): the same systems through both kernels agree to rounding."""
+    w = random_shared(3, 100, 18, False, seed=8)
+    w.pin00 = True
+    x, _ = gpu_solve_shared(w)
+    check(w, x, "f64")
+    w = random_shared(4, 64, 32, True, seed=9)
+    dv = dev()
+    t = [v.to(dv) for v in (w.a_y, w.b0_y, w.c_y, w.sx, w.sz)]
+    x_tiled, _ = gpu_solve_shared(w)
+    n = w.nz * w.ny * w.nx
+    buf_d = torch.empty(2 * n + 1, dtype=torch.float64, device=dv)
+    buf_x = torch.full((2 * n + 1,), float("nan"), dtype=torch.float64, device=dv)
+    buf_d[1:].copy_(torch.view_as_real(w.d.to(dv)).reshape(-1))
+    with tdma.Plan(w.nx, w.ny, w.nz, 1, 0) as plan:
+        tdma.tdma_solve_shared(plan.handle, *t, 2, 0, buf_d[1:], buf_x[1:])
+        torch.cuda.synchronize()
+        assert plan.get(tdma.TDMA_GET_SHARED_LINE_KERNEL) == 1
+    xl = torch.view_as_complex(buf_x[1:].reshape(w.nz, w.ny, w.nx, 2).clone())
+    check(w, xl, "f64")
+    assert oracle.normwise_error(as_lines(xl.cpu().numpy()), as_lines(x_tiled.cpu().numpy())).max() <= 1e-13
 
 
 @pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
