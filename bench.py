@@ -211,22 +211,27 @@ def run_reference(args):
     return 0
 
 
-def time_solve(torch, plan, w, x, steps, warmup, barrier):
-    """Returns seconds per step (device time, CUDA events on the launching stream)."""
+def time_solve(torch, plan, w, x, steps, warmup, barrier, per_step=None):
+    """Returns seconds per step (device time, CUDA events on the launching stream).  per_step: a list
+    that receives every step's own duration in ms (an event between consecutive steps; SURVEY 8(d):
+    "report median and best")."""
     stream = torch.cuda.current_stream()
     for _ in range(warmup):
         plan.solve(w.a, w.b, w.c, w.d, x, stream)
     torch.cuda.synchronize()
     barrier()
-    e0 = torch.cuda.Event(enable_timing=True)
-    e1 = torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(steps):
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1 if per_step is not None else 2)]
+    marks[0].record(stream)
+    for i in range(steps):
         plan.solve(w.a, w.b, w.c, w.d, x, stream)
-    e1.record(stream)
+        if per_step is not None and i + 1 < steps:
+            marks[i + 1].record(stream)
+    marks[-1].record(stream)
     torch.cuda.synchronize()
     barrier()
-    return e0.elapsed_time(e1) * 1e-3 / steps
+    if per_step is not None:
+        per_step.extend(marks[i].elapsed_time(marks[i + 1]) for i in range(steps))
+    return marks[0].elapsed_time(marks[-1]) * 1e-3 / steps
 
 
 def stage_times(torch, tdma, plan, w, x, reps=3):
@@ -486,7 +491,8 @@ def main():
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    sec = time_solve(torch, plan, w, x, args.steps, warmup, barrier)
+    step_ms = []
+    sec = time_solve(torch, plan, w, x, args.steps, warmup, barrier, per_step=step_ms)
     clocks = sampler.stop() if rank == 0 else None
     sec = max_over_ranks(sec)
     value = group.aggregate(cells, sec)
@@ -505,6 +511,8 @@ def main():
     }
     if clocks is not None:
         out["clocks"] = clocks
+    out["step_ms"] = {"median": sorted(step_ms)[len(step_ms) // 2], "best": min(step_ms), "worst": max(step_ms),
+                      "note": "rank 0, per-step CUDA events inside the timed region"}
     out["variants"] = {k: ({"ms_per_step": v["quick_s"] * 1e3, "batch": v["batch"], "launches": v["launches"]}
                            if "plan" in v else v) for k, v in results.items()}
 
