@@ -35,43 +35,104 @@ __global__ void __launch_bounds__(128) shared_lines_kernel(const SharedLineArgs 
     const size_t LL = (size_t)L;
     const int n = p.n, nt = kCyclic ? n - 1 : n;                    // rows of the plain system swept below
 
+    // Rows are handled U at a time with the next U rows' loads issued first (the recurrences are serial
+    // per thread; bandwidth comes from loads kept in flight, as in the stage kernels).  x may alias d
+    // exactly: a row of d is always loaded before that row of x is stored.
+    constexpr int U = 8;
+
     // forward elimination of rows 0 .. nt-1: c' -> cs, d' (g') -> x, h' -> hs
     double inv = 1.0 / (pin ? 1.0 : b0[0] - s);
     double cp = pin ? 0.0 : c[0] * inv, dp[NC], hp = 0.0;
 #pragma unroll
     for (int q = 0; q < NC; ++q) dp[q] = d[q] * inv;
     if (kCyclic) hp = (a[0] + (nt == 1 ? c[0] : 0.0)) * inv;       // n = 2: both neighbours of x_0 are x_1
+    double nd[U][NC];
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+        if (1 + u < nt) {
+#pragma unroll
+            for (int q = 0; q < NC; ++q) nd[u][q] = d[(size_t)(1 + u) * rs + q];
+        }
 #pragma unroll
     for (int q = 0; q < NC; ++q) x[q] = dp[q];
     cs[0] = cp;
     if (kCyclic) hs[0] = hp;
-    for (int j = 1; j < nt; ++j) {
-        const double aj = a[j];
-        inv = 1.0 / fma(-aj, cp, b0[j] - s);
+    for (int j0 = 1; j0 < nt; j0 += U) {
+        double cd[U][NC];
 #pragma unroll
-        for (int q = 0; q < NC; ++q) {
-            dp[q] = fma(-aj, dp[q], d[j * rs + q]) * inv;
-            x[j * rs + q] = dp[q];
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int q = 0; q < NC; ++q) cd[u][q] = nd[u][q];
         }
-        if (kCyclic) { hp = fma(-aj, hp, j == nt - 1 ? c[j] : 0.0) * inv; hs[j * LL] = hp; }
-        cp = c[j] * inv;
-        cs[j * LL] = cp;
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (j0 + U + u < nt) {
+#pragma unroll
+                for (int q = 0; q < NC; ++q) nd[u][q] = d[(size_t)(j0 + U + u) * rs + q];
+            }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int j = j0 + u;
+            if (j < nt) {
+                const double aj = a[j];
+                inv = 1.0 / fma(-aj, cp, b0[j] - s);
+#pragma unroll
+                for (int q = 0; q < NC; ++q) {
+                    dp[q] = fma(-aj, dp[q], cd[u][q]) * inv;
+                    x[(size_t)j * rs + q] = dp[q];
+                }
+                if (kCyclic) { hp = fma(-aj, hp, j == nt - 1 ? c[j] : 0.0) * inv; hs[(size_t)j * LL] = hp; }
+                cp = c[j] * inv;
+                cs[(size_t)j * LL] = cp;
+            }
+        }
     }
     // back substitution of rows nt-2 .. 0 (row nt-1 is final already)
-    double xv[NC], hv = hp;
+    double xv[NC], hv = hp, g_last[NC];
+    const double h_last = hp;
 #pragma unroll
-    for (int q = 0; q < NC; ++q) xv[q] = dp[q];
-    double g_last[NC], h_last = hp;
+    for (int q = 0; q < NC; ++q) xv[q] = g_last[q] = dp[q];
+    double nc_[U], nh[U], nx_[U][NC];
 #pragma unroll
-    for (int q = 0; q < NC; ++q) g_last[q] = dp[q];
-    for (int j = nt - 2; j >= 0; --j) {
-        const double cj = cs[j * LL];
+    for (int u = 0; u < U; ++u) {
+        const int j = nt - 2 - u;
+        if (j >= 0) {
+            nc_[u] = cs[(size_t)j * LL];
+            if (kCyclic) nh[u] = hs[(size_t)j * LL];
 #pragma unroll
-        for (int q = 0; q < NC; ++q) {
-            xv[q] = fma(-cj, xv[q], x[j * rs + q]);
-            x[j * rs + q] = xv[q];
+            for (int q = 0; q < NC; ++q) nx_[u][q] = x[(size_t)j * rs + q];
         }
-        if (kCyclic) { hv = fma(-cj, hv, hs[j * LL]); hs[j * LL] = hv; }
+    }
+    for (int j0 = nt - 2; j0 >= 0; j0 -= U) {
+        double cc[U], ch[U], cx[U][NC];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            cc[u] = nc_[u]; ch[u] = nh[u];
+#pragma unroll
+            for (int q = 0; q < NC; ++q) cx[u][q] = nx_[u][q];
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int j = j0 - U - u;
+            if (j >= 0) {
+                nc_[u] = cs[(size_t)j * LL];
+                if (kCyclic) nh[u] = hs[(size_t)j * LL];
+#pragma unroll
+                for (int q = 0; q < NC; ++q) nx_[u][q] = x[(size_t)j * rs + q];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int j = j0 - u;
+            if (j >= 0) {
+#pragma unroll
+                for (int q = 0; q < NC; ++q) {
+                    xv[q] = fma(-cc[u], xv[q], cx[u][q]);
+                    x[(size_t)j * rs + q] = xv[q];
+                }
+                if (kCyclic) { hv = fma(-cc[u], hv, ch[u]); hs[(size_t)j * LL] = hv; }
+            }
+        }
     }
     if (!kCyclic) return;
     // xv, hv: row 0.  Row n-1 closes the ring.
@@ -80,13 +141,24 @@ __global__ void __launch_bounds__(128) shared_lines_kernel(const SharedLineArgs 
     double xl[NC];
 #pragma unroll
     for (int q = 0; q < NC; ++q) {
-        xl[q] = fma(-c[l], xv[q], fma(-a[l], g_last[q], d[l * rs + q])) * den;
-        x[l * rs + q] = xl[q];
+        xl[q] = fma(-c[l], xv[q], fma(-a[l], g_last[q], d[(size_t)l * rs + q])) * den;
+        x[(size_t)l * rs + q] = xl[q];
     }
-    for (int j = 0; j < nt; ++j) {
-        const double hj = hs[j * LL];
+    for (int j0 = 0; j0 < nt; j0 += U) {
+        double ch[U], cx[U][NC];
 #pragma unroll
-        for (int q = 0; q < NC; ++q) x[j * rs + q] = fma(-hj, xl[q], x[j * rs + q]);
+        for (int u = 0; u < U; ++u)
+            if (j0 + u < nt) {
+                ch[u] = hs[(size_t)(j0 + u) * LL];
+#pragma unroll
+                for (int q = 0; q < NC; ++q) cx[u][q] = x[(size_t)(j0 + u) * rs + q];
+            }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (j0 + u < nt) {
+#pragma unroll
+                for (int q = 0; q < NC; ++q) x[(size_t)(j0 + u) * rs + q] = fma(-ch[u], xl[q], cx[u][q]);
+            }
     }
 }
 
