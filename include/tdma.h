@@ -212,7 +212,9 @@ int tdma_solve_shared(tdma_plan *plan, const void *a_y, const void *b0_y, const 
                       void *stream);
 
 /* Same solve with HOST buffers: the slab is streamed through plan-owned device staging buffers
- * in z-chunks (H2D copy of chunk n+1 and D2H copy of chunk n-1 overlap the solve of chunk n).
+ * in z-chunks (H2D copy of chunk n+1 and D2H copy of chunk n-1 overlap the solve of chunk n); a z
+ * sweep is streamed in chunks of y-slices (strided 2-D copies; every chunk is a slab of its own and
+ * runs on a plan of its own, created with the same options at the first call).
  * Blocks until x is complete on the host.  Pinned host memory gives asynchronous copies;
  * pageable memory works but serialises. */
 int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c, const void *d,

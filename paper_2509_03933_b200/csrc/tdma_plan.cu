@@ -112,6 +112,8 @@ struct tdma_plan {
     int sh_lines_last = 0;             // 1: the last tdma_solve_shared ran the general-shape kernel
     // host staging (tdma_solve_host), allocated on first use
     int hz = 0;  // slices per host chunk
+    tdma_options opt_saved = {};       // the options the plan was created with (struct_size = 0: none)
+    tdma_plan *zchild[2] = {};         // tdma_solve_host of a z sweep: plans for a chunk of hz y-slices / the last, shorter chunk
     int host_chunk = 0;  // options.host_chunk (0 = auto)
     double *stage_dev[2][5] = {};
     cudaStream_t sH2D = nullptr, sD2H = nullptr;
@@ -427,6 +429,7 @@ void free_plan(tdma_plan *pl)
     if (pl->staged.impl) tdma::free_staged(&pl->staged);
     for (int s = 0; s < 2; ++s)
         for (int i = 0; i < 5; ++i) cudaFree(pl->stage_dev[s][i]);
+    free_plan(pl->zchild[0]); free_plan(pl->zchild[1]);
     auto ds = [](cudaStream_t s) { if (s) cudaStreamDestroy(s); };
     auto de = [](cudaEvent_t e) { if (e) cudaEventDestroy(e); };
     ds(pl->sMain); ds(pl->sB); ds(pl->sH2D); ds(pl->sD2H);
@@ -677,6 +680,7 @@ tdma_plan *tdma_plan_create_ex(int nx, int ny, int nz, int P, int batch, int dty
     if (!pl) { set_err(TDMA_ERR_ALLOC, "out of host memory"); return nullptr; }
     pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->P = P; pl->m = ny / P;   // ny, nz already mapped
     pl->axis = axis; pl->periodic = periodic;
+    if (options) pl->opt_saved = *options;
     pl->host_chunk = options ? options->host_chunk : 0;
     pl->fill_opt = options ? options->fused_fill : 0;
     if (options) { pl->sh_opt[0] = options->shared_lines; pl->sh_opt[1] = options->shared_cluster; pl->sh_opt[2] = options->shared_leaf_rows; pl->sh_opt[3] = options->shared_slots; pl->sh_opt[4] = options->shared_ctas; }
@@ -868,8 +872,7 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
     int rc = check_ptrs(plan, a, b, c, d, x);
     if (rc != TDMA_OK) return rc;
     tdma_plan *pl = plan;
-    if (pl->axis == TDMA_AXIS_Z)
-        return set_err(TDMA_ERR_UNSUPPORTED, "tdma_solve_host streams z-chunks: x and y sweeps only");
+    const bool zsw = pl->axis == TDMA_AXIS_Z;      // chunks of y-slices: strided in the caller's arrays
     if (!pl->sH2D) {  // first use: staging buffers, copy streams
         // chunk = about 16 Mi cells (128 MiB per array), or options.host_chunk slices.  PIPELINED:
         // rounded to whole batches so that the batch boundaries (and with them the bits of x) are
@@ -879,6 +882,20 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
         if (pl->variant != TDMA_VARIANT_FUSED) hz = std::max<long long>(pl->bz, hz / pl->bz * pl->bz);
         pl->hz = (int)std::min<long long>(hz, pl->nz);
         const size_t bytes = (size_t)pl->hz * pl->slice * sizeof(double);
+        if (zsw) {
+            // A chunk of hz y-slices of a z sweep is a slab of its own, (nx, hz, line length), with its own
+            // row stride: it gets its own plan (same options), and so does the last, shorter chunk.
+            tdma_options o = pl->opt_saved;
+            o.struct_size = (int)sizeof(o); o.axis = TDMA_AXIS_Z; o.periodic = pl->periodic; o.variant = pl->variant;
+            const int tail = pl->nz % pl->hz;
+            for (int t = 0; t < (tail ? 2 : 1); ++t) {
+                const int hzc = t == 0 ? pl->hz : tail;
+                const int bzc = pl->variant == TDMA_VARIANT_FUSED ? 0 : std::min(pl->bz, hzc);
+                free_plan(pl->zchild[t]);
+                pl->zchild[t] = tdma_plan_create_ex(pl->nx, hzc, pl->ny, pl->P, bzc, TDMA_F64, &o);
+                if (!pl->zchild[t]) return g_err_code;       // message set by the failed creation
+            }
+        }
         for (int s = 0; s < 2; ++s)
             for (int i = 0; i < 5; ++i)
                 if (cudaMalloc(&pl->stage_dev[s][i], bytes) != cudaSuccess) {
@@ -907,16 +924,29 @@ int tdma_solve_host(tdma_plan *plan, const void *a, const void *b, const void *c
             CUDA_TRY(cudaStreamWaitEvent(pl->sH2D, pl->evDone[s], 0));
             CUDA_TRY(cudaStreamWaitEvent(pl->sH2D, pl->evD2H[s], 0));
         }
-        for (int i = 0; i < 4; ++i)
-            CUDA_TRY(cudaMemcpyAsync(pl->stage_dev[s][i], h[i] + off, bytes, cudaMemcpyHostToDevice, pl->sH2D));
+        // z sweep: rows of the line are caller z-slices, a chunk is nx * nzc contiguous doubles of each
+        const size_t zoff = (size_t)k0 * pl->nx, zrow = (size_t)pl->nx * nzc * sizeof(double),
+                     zpitch = (size_t)pl->nx * pl->nz * sizeof(double);
+        for (int i = 0; i < 4; ++i) {
+            if (zsw)
+                CUDA_TRY(cudaMemcpy2DAsync(pl->stage_dev[s][i], zrow, h[i] + zoff, zpitch, zrow, (size_t)pl->ny,
+                                           cudaMemcpyHostToDevice, pl->sH2D));
+            else
+                CUDA_TRY(cudaMemcpyAsync(pl->stage_dev[s][i], h[i] + off, bytes, cudaMemcpyHostToDevice, pl->sH2D));
+        }
         CUDA_TRY(cudaEventRecord(pl->evH2D[s], pl->sH2D));
         CUDA_TRY(cudaStreamWaitEvent(pl->sMain, pl->evH2D[s], 0));
         const SlabPtrs ptr{pl->stage_dev[s][0], pl->stage_dev[s][1], pl->stage_dev[s][2],
                            pl->stage_dev[s][3], pl->stage_dev[s][4]};
-        if ((rc = run_solve(pl, ptr, nzc, pl->sMain)) != TDMA_OK) return rc;
+        tdma_plan *solver = zsw ? pl->zchild[nzc == pl->hz ? 0 : 1] : pl;
+        if ((rc = run_solve(solver, ptr, nzc, pl->sMain)) != TDMA_OK) return rc;
         CUDA_TRY(cudaEventRecord(pl->evDone[s], pl->sMain));
         CUDA_TRY(cudaStreamWaitEvent(pl->sD2H, pl->evDone[s], 0));
-        CUDA_TRY(cudaMemcpyAsync(hx + off, pl->stage_dev[s][4], bytes, cudaMemcpyDeviceToHost, pl->sD2H));
+        if (zsw)
+            CUDA_TRY(cudaMemcpy2DAsync(hx + zoff, zpitch, pl->stage_dev[s][4], zrow, zrow, (size_t)pl->ny,
+                                       cudaMemcpyDeviceToHost, pl->sD2H));
+        else
+            CUDA_TRY(cudaMemcpyAsync(hx + off, pl->stage_dev[s][4], bytes, cudaMemcpyDeviceToHost, pl->sD2H));
         CUDA_TRY(cudaEventRecord(pl->evD2H[s], pl->sD2H));
     }
     CUDA_TRY(cudaStreamSynchronize(pl->sD2H));

@@ -236,7 +236,7 @@ def test_fused_tma_is_bitwise_reproducible(shape, opts):
 
 def test_auto_variant_and_host_buffers_on_x_sweep():
     """tdma_plan_create (variant AUTO) resolves to FUSED when the shape tiles and to PIPELINED when
-    it does not; tdma_solve_host works for x sweeps (z-chunks are contiguous) and refuses z sweeps."""
+    it does not; tdma_solve_host works for x sweeps (z-chunks are contiguous)."""
     with tdma.Plan(64, 64, 8, 4, 2) as plan:
         assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_FUSED
         assert plan.get(tdma.TDMA_GET_NB) == 1          # batch is a hint for the stage pipelines only
@@ -249,6 +249,25 @@ def test_auto_variant_and_host_buffers_on_x_sweep():
     with tdma.Plan(128, 24, 6, 2, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_X, periodic=1) as plan:
         plan.solve_host(*host, xh)
     check(a, b, c, d, xh, "x", True)
-    with tdma.Plan(32, 24, 16, 2, 0, variant=tdma.TDMA_VARIANT_FUSED, axis=tdma.TDMA_AXIS_Z) as plan:
-        with pytest.raises(tdma.TdmaError):
-            plan.solve_host(*[torch.zeros(16, 24, 32, dtype=torch.float64) for _ in range(5)])
+
+
+@pytest.mark.parametrize("opts,periodic", [(dict(variant=tdma.TDMA_VARIANT_FUSED), 1), (dict(variant=tdma.TDMA_VARIANT_PIPELINED), 0),
+                                           (dict(variant=tdma.TDMA_VARIANT_PIPELINED), 1), (dict(variant=tdma.TDMA_VARIANT_STAGED), 0),
+                                           (dict(), 0)], ids=["fused_cyclic", "pipelined", "pipelined_cyclic", "staged", "auto"])
+@pytest.mark.parametrize("chunk", [0, 5])
+def test_solve_host_on_z_sweeps(opts, periodic, chunk):
+    """tdma_solve_host of a z sweep: chunks of y-slices (strided copies), each solved by a plan of its own;
+    host_chunk = 5 gives 4 chunks with a ragged last one (17 = 3 * 5 + 2).  Against the oracle and, to
+    rounding, against the device solve."""
+    nz, ny, nx = 64, 17, 48
+    a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 63, "cpu")
+    host = [t.pin_memory() for t in (a, b, c, d)]
+    xh = torch.full_like(d, float("nan")).pin_memory()
+    with tdma.Plan(nx, ny, nz, 4, 2, axis=tdma.TDMA_AXIS_Z, periodic=periodic, host_chunk=chunk, **opts) as plan:
+        plan.solve_host(*host, xh)
+        plan.solve_host(*host, xh)                       # second call: staging and chunk plans are reused
+        xd = torch.full_like(d, float("nan"), device=dev())
+        plan.solve(*[t.to(dev()) for t in (a, b, c, d)], xd)
+        torch.cuda.synchronize()
+    check(a, b, c, d, xh, "z", bool(periodic))
+    assert float((xh - xd.cpu()).abs().max() / xh.abs().max()) <= 1e-13
