@@ -81,7 +81,7 @@ typedef enum tdma_variant {
      * again, re-reduces it and back-substitutes with the boundary unknowns stage B computed
      * (reads 32, writes 8 B/cell).  72 B/cell instead of PIPELINED's 88, no scratch ring.  The
      * exchanged level of the recursion is the highest whose nodes are no longer than ny/P rows
-     * (TDMA_GET_REDUCED_PARTITIONS of them per line; D1).  y / z sweeps of plain lines,
+     * (TDMA_GET_REDUCED_PARTITIONS of them per line; D1).  y / z sweeps, plain or cyclic lines,
      * 16-byte aligned arrays, shapes the TMA kernel tiles. */
     TDMA_VARIANT_STAGED = 3
 } tdma_variant;
@@ -126,8 +126,8 @@ typedef struct tdma_options {
                             resolved at the top of the recursion: at the root of the tree in the
                             FUSED TMA kernel, in stage B's reduced system (then a cyclic 2P-row
                             system) in the PIPELINED variant, which takes any nx and line length
-                            along y or z.  AUTO picks FUSED when the shape tiles, else PIPELINED;
-                            STAGED, pdd and the register-staged fused kernel do plain lines only */
+                            along x, y or z, and in STAGED.  AUTO picks FUSED when the shape tiles,
+                            else PIPELINED; pdd and the register-staged fused kernel do plain lines only */
     int timeline;        /* PIPELINED, 1 = record a timing event before and after every stage launch
                             (forces plain stream launches); read back with tdma_plan_timeline */
     int fused_slots;     /* FUSED, TMA kernel: ring slots of one raw array tile each: 4 = the next tile is

@@ -165,7 +165,7 @@ int launch_stage(tdma_plan *pl, int stage, const tdma::StageParams &prm_in, cuda
             const int nzs = (int)(prm.Lb / pl->nx);
             cudaError_t e = tdma::launch_staged(pl->staged, stage == TDMA_STAGE_A ? 1 : 2, prm.a, prm.b, prm.c, prm.d, prm.x,
                                                 prm.ra, prm.rc, prm.rd, prm.y, pl->nx, pl->ny, nzs, pl->rs, pl->os,
-                                                pl->axis == TDMA_AXIS_Z, st);
+                                                pl->axis == TDMA_AXIS_Z, st, pl->periodic != 0);
             if (e != cudaSuccess) return set_err(TDMA_ERR_CUDA, "staged launch failed: %s", cudaGetErrorString(e));
             return TDMA_OK;
         }
@@ -480,8 +480,8 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
     }
     if (variant != TDMA_VARIANT_PIPELINED && variant != TDMA_VARIANT_FUSED && variant != TDMA_VARIANT_STAGED)
         return set_err(TDMA_ERR_INVALID_ARG, "unknown variant %d", variant);
-    if (variant == TDMA_VARIANT_STAGED && (pl->axis == TDMA_AXIS_X || pl->periodic || pl->ny < 2))
-        return set_err(TDMA_ERR_UNSUPPORTED, "the STAGED variant does y / z sweeps of plain lines with >= 2 rows");
+    if (variant == TDMA_VARIANT_STAGED && (pl->axis == TDMA_AXIS_X || pl->ny < 2))
+        return set_err(TDMA_ERR_UNSUPPORTED, "the STAGED variant does y / z sweeps of lines with >= 2 rows");
     if (pl->periodic && pl->ny < 2)
         return set_err(TDMA_ERR_UNSUPPORTED, "cyclic lines need >= 2 rows");
     if (pl->periodic && opt && opt->pdd > 0)

@@ -57,7 +57,8 @@ static cudaError_t launch_staged_tx(TmaFusedConfig &t, const CUtensorMap *tm, co
 static cudaError_t launch_staged_any(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
                                      const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
                                      int nx, int ny, int nzs, long long rs, long long os, bool axis_z, int row0,
-                                     int ny_total, long long Ls, double *const *peer, long long peer_off, cudaStream_t st)
+                                     int ny_total, long long Ls, double *const *peer, long long peer_off, cudaStream_t st,
+                                     bool periodic = false)
 {
     if (stage != 1 && stage != 2) return cudaErrorInvalidValue;
     TmaFusedConfig &t = static_cast<TmaFusedConfig *>(cfg.impl)[stage - 1];
@@ -68,7 +69,7 @@ static cudaError_t launch_staged_any(StagedConfig &cfg, int stage, const double 
     TmaFusedParams prm;
     prm.nx = nx; prm.ny = ny; prm.nzs = nzs;
     prm.x = x;
-    prm.rs = rs; prm.os = os; prm.axis_z = axis_z ? 1 : 0; prm.periodic = 0;
+    prm.rs = rs; prm.os = os; prm.axis_z = axis_z ? 1 : 0; prm.periodic = periodic ? 1 : 0;
     prm.CL = t.cluster; prm.R = t.rows; prm.W = t.leaves; prm.NS = t.slots;
     prm.xtiles = (nx + t.lines - 1) / t.lines;
     prm.ntiles = prm.xtiles * nzs;
@@ -99,9 +100,11 @@ static cudaError_t launch_staged_any(StagedConfig &cfg, int stage, const double 
 
 cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
                           const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
-                          int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st)
+                          int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st,
+                          bool periodic)
 {
-    return launch_staged_any(cfg, stage, a, b, c, d, x, ra, rc, rd, y, nx, ny, nzs, rs, os, axis_z, 0, 0, 0, nullptr, 0, st);
+    return launch_staged_any(cfg, stage, a, b, c, d, x, ra, rc, rd, y, nx, ny, nzs, rs, os, axis_z, 0, 0, 0, nullptr, 0, st,
+                             periodic);
 }
 
 cudaError_t launch_staged_slab(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,

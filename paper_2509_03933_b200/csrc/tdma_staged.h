@@ -20,10 +20,12 @@ bool configure_staged(StagedConfig *out, int nx, int ny, int P, bool axis_z, con
 void free_staged(StagedConfig *cfg);
 
 // stage = 1 (A: reduce, writes ra / rc / rd [2 Pe][Lb]) or 2 (C: re-reduce + back-substitute, reads y).
-// a, b, c, d, x: slice 0 of the batch; Lb = nx * nzs lines.
+// a, b, c, d, x: slice 0 of the batch; Lb = nx * nzs lines.  periodic: cyclic lines -- a_0 and c_{n-1} are
+// kept, so rows 0 and 2 Pe - 1 of the reduced system couple each other (stage_b_cyclic_kernel).
 cudaError_t launch_staged(StagedConfig &cfg, int stage, const double *a, const double *b, const double *c,
                           const double *d, double *x, double *ra, double *rc, double *rd, const double *y,
-                          int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st);
+                          int nx, int ny, int nzs, long long rs, long long os, bool axis_z, cudaStream_t st,
+                          bool periodic = false);
 
 // y-slab decomposition (tdma_slab.cu): the launch holds rows row0 .. row0 + ny - 1 of lines of ny_total
 // rows; stage 1 writes send[dest][Pe][6][Ls], stage 2 reads yrecv[src][2 Pe][Ls] (Ls = nx * nzs / ranks).

@@ -157,6 +157,19 @@ def test_x_sweep_on_the_stage_pipeline(periodic, shape, P, batch):
             assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_PIPELINED
 
 
+@pytest.mark.parametrize("axis", ["y", "z"])
+@pytest.mark.parametrize("n,P,batch", [(64, 4, 0), (256, 8, 2), (1024, 16, 3), (768, 16, 0), (32, 16, 1)])
+def test_cyclic_lines_staged(axis, n, P, batch):
+    """Cyclic lines in the STAGED variant: the TMA-staged stage A / C kernels keep a_0 and c_{n-1}, stage B
+    is the cyclic reduced solve."""
+    other, nx = 5, 96
+    shape = (other, n, nx) if axis == "y" else (n, other, nx)
+    a, b, c, d = tdma_inputs.dominant_random(shape[2], shape[1], shape[0], 75, dev())
+    x = solve(a, b, c, d, P, batch, variant=tdma.TDMA_VARIANT_STAGED, periodic=1,
+              axis=tdma.TDMA_AXIS_Z if axis == "z" else tdma.TDMA_AXIS_Y)
+    check(a, b, c, d, x, axis, True)
+
+
 def test_cyclic_lines_auto_falls_back_to_the_stage_pipeline():
     """AUTO: cyclic lines go to the fused TMA kernel when the shape tiles, else to PIPELINED; both against
     the oracle, and against each other to rounding on a shape both can run."""
@@ -188,8 +201,8 @@ def test_cyclic_pipelined_circulant_closed_form():
 
 
 def test_unsupported_combinations_fail_loudly():
-    with pytest.raises(tdma.TdmaError):            # cyclic lines: FUSED TMA kernel or PIPELINED
-        tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_STAGED, periodic=1)
+    with pytest.raises(tdma.TdmaError):            # cyclic lines: not in the register-staged fused kernel
+        tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_FUSED, fused_impl=1, periodic=1)
     with pytest.raises(tdma.TdmaError):
         tdma.Plan(32, 32, 32, 4, 0, variant=tdma.TDMA_VARIANT_PIPELINED, periodic=1, pdd=1)
     with pytest.raises(tdma.TdmaError):
