@@ -384,6 +384,85 @@ def shared_workload(torch, tdma, tdma_inputs, base, cplx, dev, steps, warmup, ba
     return rec
 
 
+def general_shapes(torch, tdma, tdma_inputs, dev, steps, warmup):
+    """The general-shape paths next to the tiled kernels on neighbouring shapes (not headline numbers: they
+    exist so that every nx, line length, axis and wrap is solved).  Every timed solve is checked against the
+    oracle on two sampled slices, outside the timed region."""
+    import numpy as np
+    import oracle
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / steps
+
+    def err_axis(a, b, c, d, x, axis, periodic, slices):
+        ax = {"y": 1, "z": 0, "x": 2}[axis]
+        worst = 0.0
+        for k in slices:
+            sl = (slice(None), slice(k, k + 1)) if axis == "z" else (slice(k, k + 1),)
+            arrs = [t[sl].cpu().numpy() for t in (a, b, c, d, x)]
+            ref = oracle.solve_axis(*arrs[:4], axis, bool(periodic))
+            worst = max(worst, float((np.max(np.abs(arrs[4] - ref), axis=ax) / np.max(np.abs(ref), axis=ax)).max()))
+        return worst
+
+    out = {"general_shapes": True, "steps": steps, "tol": 1e-11, "records": []}
+    V = {"pipelined": tdma.TDMA_VARIANT_PIPELINED, "staged": tdma.TDMA_VARIANT_STAGED, "fused": tdma.TDMA_VARIANT_FUSED}
+    # general form: cyclic y lines on all three variants, x sweeps on the TMA kernel and on the stage pipeline
+    for name, (nz, ny, nx), P, batch, opts, axis in [
+            ("y cyclic, fused", (64, 1024, 1024), 16, 0, dict(variant=V["fused"], periodic=1), "y"),
+            ("y cyclic, pipelined", (64, 1024, 1024), 16, 16, dict(variant=V["pipelined"], periodic=1), "y"),
+            ("y plain, pipelined", (64, 1024, 1024), 16, 16, dict(variant=V["pipelined"]), "y"),
+            ("y cyclic, staged", (64, 1024, 1024), 16, 16, dict(variant=V["staged"], periodic=1), "y"),
+            ("y cyclic, 1000 rows x 1023 (auto -> pipelined)", (64, 1000, 1023), 8, 16, dict(periodic=1), "y"),
+            ("x sweep, nx = 1024 (auto -> fused)", (64, 512, 1024), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x"),
+            ("x sweep, nx = 1000 (auto -> pipelined)", (64, 512, 1000), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x")]:
+        a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 7, dev)
+        x = torch.full_like(d, float("nan"))
+        with tdma.Plan(nx, ny, nz, P, batch, **opts) as plan:
+            ms = timed(lambda: plan.solve(a, b, c, d, x))
+            variant = plan.get(tdma.TDMA_GET_VARIANT)
+        E = err_axis(a, b, c, d, x, axis, opts.get("periodic", 0), [0, nz - 1])
+        out["records"].append({"case": name, "shape": [nz, ny, nx], "variant": {1: "pipelined", 2: "fused", 3: "staged"}[variant],
+                               "ms": ms, "gbs_40B": 40.0 * nz * ny * nx / ms / 1e6, "E_max": E, "ok": bool(E <= 1e-11)})
+        del a, b, c, d, x
+    # shared form: the tiled kernel and the one-thread-per-line kernel on neighbouring shapes
+    g = torch.Generator().manual_seed(5)
+    u = lambda n, lo, hi: (lo + (hi - lo) * torch.rand(n, dtype=torch.float64, generator=g)).to(dev)
+    for name, (nz, ny, nx), cplx in [("shared, ny = 1024", (128, 1024, 1024), False), ("shared, ny = 1000", (128, 1000, 1024), False),
+                                     ("shared, nx = 1023", (128, 1024, 1023), False), ("shared complex, ny = 1000", (128, 1000, 1024), True)]:
+        a_y, b0_y, c_y, sx, sz = u(ny, -1, 1), u(ny, 2.5, 3.5), u(ny, -1, 1), -u(nx, 0, 2), -u(nz, 0, 2)
+        d = torch.randn((nz, ny, nx), dtype=torch.float64, device=dev)
+        if cplx:
+            d = torch.complex(d, torch.randn((nz, ny, nx), dtype=torch.float64, device=dev))
+        x = torch.full_like(d, float("nan"))
+        with tdma.Plan(nx, ny, nz, 1, 0) as plan:
+            ms = timed(lambda: plan.solve_shared(a_y, b0_y, c_y, sx, sz, d, x))
+            line_kernel = plan.get(tdma.TDMA_GET_SHARED_LINE_KERNEL)
+        worst = 0.0
+        for k in (0, nz - 1):
+            ref = oracle.solve_y_shared(*[t.cpu().numpy() for t in (a_y, b0_y, c_y, sx)], sz[k:k + 1].cpu().numpy(),
+                                        d[k:k + 1].cpu().numpy(), pin00=False, precision="f64")
+            xr, rr = x[k:k + 1].cpu().numpy(), ref
+            if cplx:
+                xr, rr = xr.view(np.float64).reshape(1, ny, -1), np.ascontiguousarray(rr).view(np.float64).reshape(1, ny, -1)
+            worst = max(worst, float(oracle.normwise_error(xr, rr).max()))
+        bpc = 32.0 if cplx else 16.0
+        out["records"].append({"case": name, "shape": [nz, ny, nx], "kernel": "one thread per line" if line_kernel else "tiled TMA",
+                               "ms": ms, "gbs_alg": bpc * nz * ny * nx / ms / 1e6, "alg_bytes_per_cell": bpc, "E_max": worst,
+                               "ok": bool(worst <= 1e-11)})
+        del d, x
+    out["ok"] = all(r["ok"] for r in out["records"])
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -415,6 +494,10 @@ def main():
     ap.add_argument("--adi", action="store_true",
                     help="NEXT row f1 / BASELINE cfg 4: three successive FUSED solves along x (periodic), "
                          "y (Dirichlet) and z (periodic); use with --workload cfg4_adi_y")
+    ap.add_argument("--general-shapes", action="store_true",
+                    help="time the paths that take what the TMA kernels cannot tile (cyclic lines / x sweeps on the "
+                         "stage pipeline, the one-thread-per-line kernel of the shared form), each checked against "
+                         "the oracle on sampled slices; one JSON line")
     args = ap.parse_args()
 
     if args.impl == "reference":
@@ -435,6 +518,12 @@ def main():
     barrier, max_over_ranks = group.barrier, group.max
     peak, peak_src = measured_peak()
 
+    if args.general_shapes:
+        rec = general_shapes(torch, tdma, tdma_inputs, dev, args.steps, max(3, args.warmup))
+        if rank == 0:
+            print(json.dumps(rec))
+        group.close()
+        return 0
     spec = tdma_inputs.config_spec(args.workload)
     nz = args.nz if args.nz > 0 else spec["nz"]
     if args.shared:
