@@ -436,7 +436,10 @@ def general_shapes(torch, tdma, tdma_inputs, dev, steps, warmup):
     # shared form: the tiled kernel and the one-thread-per-line kernel on neighbouring shapes
     g = torch.Generator().manual_seed(5)
     u = lambda n, lo, hi: (lo + (hi - lo) * torch.rand(n, dtype=torch.float64, generator=g)).to(dev)
-    for name, (nz, ny, nx), cplx in [("shared, ny = 1024", (128, 1024, 1024), False), ("shared, ny = 1000", (128, 1000, 1024), False),
+    for name, (nz, ny, nx), cplx in [("shared, ny = 1024", (128, 1024, 1024), False), ("shared, ny = 768 (24-row leaves)", (128, 768, 1024), False),
+                                     ("shared, ny = 640 (20-row leaves)", (128, 640, 1024), False),
+                                     ("shared complex, ny = 768 (12-row leaves)", (128, 768, 1024), True),
+                                     ("shared, ny = 1000", (128, 1000, 1024), False),
                                      ("shared, nx = 1023", (128, 1024, 1023), False), ("shared complex, ny = 1000", (128, 1000, 1024), True)]:
         a_y, b0_y, c_y, sx, sz = u(ny, -1, 1), u(ny, 2.5, 3.5), u(ny, -1, 1), -u(nx, 0, 2), -u(nz, 0, 2)
         d = torch.randn((nz, ny, nx), dtype=torch.float64, device=dev)

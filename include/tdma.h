@@ -139,7 +139,7 @@ typedef struct tdma_options {
     int shared_lines;    /* tdma_solve_shared: cells along x per tile (real: 16 or 32, complex: 8 or 16),
                             0 = auto (128-byte row segments) */
     int shared_cluster;  /* tdma_solve_shared: CTAs per cluster (1, 2, 4, 8), 0 = auto */
-    int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16, 32), 0 = auto */
+    int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16, 32; 10, 12, 20, 24), 0 = auto */
     int shared_slots;    /* tdma_solve_shared: tiles in the shared-memory ring (2 .. 4), 0 = auto */
     int pdd;             /* PIPELINED / STAGED: 1 = stage B is the Parallel Diagonally Dominant variant
                             (Sun 1995): the far ends of the partitions' spikes are
@@ -200,7 +200,7 @@ int tdma_solve(tdma_plan *plan, const void *a, const void *b, const void *c, con
  * P and batch are not used: the line is cut into the kernel's own leaves (D1); one
  * persistent launch (plus the fill launch, see fused_fill) per call.
  * GENERAL SHAPES.  The tiled kernel needs ny = CL * W * M0 (CL in 1,2,4,8, W a power of two <= 32, M0 in
- * 4,8,16,32), an even nx*ncomp, real cells for x sweeps and 16-byte aligned d, x.  Everything else (any
+ * 4,8,16,32 or, for 3 * 2^k and 5 * 2^k lengths, 12,24 / 10,20), an even nx*ncomp, real cells for x sweeps and 16-byte aligned d, x.  Everything else (any
  * ny >= 1, odd nx, complex cells along x, 8-byte aligned arrays) runs a one-thread-per-line Thomas kernel
  * with the matrix rebuilt on the fly: correct for every shape, not fast (48 instead of 16 B per real cell:
  * c' travels through a plan-owned scratch array of at most 256 MiB, allocated at the first such call, and

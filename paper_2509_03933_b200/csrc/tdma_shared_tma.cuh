@@ -874,7 +874,10 @@ inline size_t shared_smem_bytes(int TX, int R, int W, int CL, int NA, int NC, in
 }
 
 // Leaf sizes the kernel is instantiated for.
-constexpr int kSharedLeafSizes[] = {32, 16, 8, 4};
+// 24 / 12 and 20 / 10 rows (two sub-leaves of 12, 6, 10, 5) tile 3 * 2^k and 5 * 2^k line lengths (96, 192, 384, 768,
+// 160, 320, 640 ...) with the same power-of-two tree; built for the default tile width only.
+constexpr int kSharedLeafSizes[] = {32, 24, 20, 16, 12, 10, 8, 4};
+inline bool shared_odd_leaf(int m0) { return m0 == 24 || m0 == 20 || m0 == 12 || m0 == 10; }
 
 inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int want_lines, int want_cluster,
                                   int want_leaf, int want_slots, int want_ctas, const cudaDeviceProp &prop, const char **why,
@@ -902,6 +905,7 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
                 if (want_leaf && m0 != want_leaf) continue;
                 if ((xsweep || uniform) && m0 != 16 && m0 != 32) continue;
                 if (m0 > R || R % m0 || !is_pow2(R / m0) || R / m0 > 32) continue;
+                if (shared_odd_leaf(m0) && (ti != 0 || want_ctas >= 2 || (m0 >= 20 && NC != 1))) continue;
                 // 32-row leaves (four sub-leaves per thread) halve the tree per cell: 1.46 -> 1.05 ms on 256 slices
                 // of cfg 3 (real).  Complex cells need the registers for the second right-hand side: on request only
                 if (m0 == 32 && want_leaf != 32 && NC != 1) continue;
@@ -909,7 +913,7 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
                 c.ncomp = NC; c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
                 c.threads = c.leaves * TX; c.xsweep = xsweep ? 1 : 0; c.uniform = uniform ? 1 : 0;
                 if (uniform && c.threads > 256) continue;
-                if (c.threads > 512 || (m0 == 32 && c.threads > 256)) continue;
+                if (c.threads > 512 || ((m0 == 32 || shared_odd_leaf(m0)) && c.threads > 256)) continue;
                 c.box_rows = R;
                 while (c.box_rows > 256) c.box_rows /= 2;
                 if (R % c.box_rows) continue;
@@ -1013,6 +1017,14 @@ inline cudaError_t launch_shared_tx(SharedConfig &cfg, const CUtensorMap *tm, co
             return launch_shared_inst<TX, 16, kCluster, 128, NC, 4>(cfg, tm, prm, st);
         }
         return launch_shared_inst<TX, 16, kCluster, 256, NC, 2>(cfg, tm, prm, st);
+    }
+    if constexpr ((NC == 1 && TX == 16) || (NC == 2 && TX == 8)) {        // 3 * 2^k and 5 * 2^k line lengths
+        if (!big && cfg.leaf_rows == 12) return launch_shared_inst<TX, 12, kCluster, 256, NC>(cfg, tm, prm, st);
+        if (!big && cfg.leaf_rows == 10) return launch_shared_inst<TX, 10, kCluster, 256, NC>(cfg, tm, prm, st);
+        if constexpr (NC == 1) {
+            if (!big && cfg.leaf_rows == 24) return launch_shared_inst<TX, 24, kCluster, 256, NC>(cfg, tm, prm, st);
+            if (!big && cfg.leaf_rows == 20) return launch_shared_inst<TX, 20, kCluster, 256, NC>(cfg, tm, prm, st);
+        }
     }
     switch (cfg.leaf_rows) {
     case 32: return big ? cudaErrorInvalidValue : launch_shared_inst<TX, 32, kCluster, 256, NC>(cfg, tm, prm, st);

@@ -137,4 +137,4 @@ def test_random_shapes_shared_form(seed):
                                         pin00=False, precision="f64")
         E = oracle.normwise_error(as_lines(xn), as_lines(ref)).max()
         assert E <= TOL_E, tag + ": E = %.3e" % E
-    assert tiled >= 10 and lines >= 10 and tiled + lines == 50
+    assert tiled >= 10 and lines >= 5 and tiled + lines == 50

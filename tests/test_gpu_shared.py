@@ -87,6 +87,10 @@ def test_poisson_shared_slab(name, nz, cplx):
     (1024, dict(shared_cluster=8, shared_leaf_rows=8)),
     (256, dict(shared_leaf_rows=32)), (512, dict(shared_cluster=1, shared_leaf_rows=32)),
     (1024, dict(shared_cluster=2, shared_leaf_rows=32)), (1024, dict(shared_cluster=4, shared_leaf_rows=32)),
+    # 3 * 2^k and 5 * 2^k line lengths: leaves of 12 / 24 and 10 / 20 rows
+    (24, {}), (48, {}), (96, {}), (192, {}), (384, {}), (768, {}), (1536, {}), (3072, {}), (40, {}), (160, {}), (320, {}),
+    (640, {}), (1280, {}), (768, dict(shared_leaf_rows=12)), (640, dict(shared_leaf_rows=10)),
+    (768, dict(shared_cluster=8)), (1280, dict(shared_cluster=4)),
 ])
 def test_tilings_and_ragged_x(ny, opts, cplx):
     """Every tiling the kernel is instantiated for, nx not a multiple of the tile width (the last
@@ -94,9 +98,14 @@ def test_tilings_and_ragged_x(ny, opts, cplx):
     w = random_shared(5, ny, 88, cplx, seed=ny + (7 if cplx else 0))
     x, info = gpu_solve_shared(w, **opts)
     check(w, x, "f64")
+    assert info["threads"] > 0                               # the tiled kernel, not the one-thread-per-line kernel
     for key, name in (("shared_cluster", "cluster"), ("shared_leaf_rows", "leaf_rows"), ("shared_slots", "slots")):
         if key in opts:
             assert info[name] == opts[key]
+    if ny % 3 == 0:
+        assert info["leaf_rows"] in (12, 24)
+    if ny % 5 == 0:
+        assert info["leaf_rows"] in (10, 20)
 
 
 @pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
@@ -241,7 +250,7 @@ def check_axis(a, b, c, d, x, axis, periodic):
 @pytest.mark.parametrize("cplx", [False, True], ids=["f64", "c128"])
 @pytest.mark.parametrize("periodic", [False, True], ids=["plain", "cyclic"])
 @pytest.mark.parametrize("axis,shape", [
-    ("y", (3, 24, 32)), ("y", (4, 100, 33)), ("y", (2, 200, 7)), ("y", (5, 2, 9)), ("y", (3, 3, 1)), ("y", (2, 1000, 64)),
+    ("y", (3, 28, 32)), ("y", (4, 100, 33)), ("y", (2, 200, 7)), ("y", (5, 2, 9)), ("y", (3, 3, 1)), ("y", (2, 1000, 64)),
     ("z", (100, 3, 33)), ("z", (37, 5, 16)), ("x", (3, 9, 40)), ("x", (2, 5, 115)), ("x", (2, 3, 64))])
 def test_line_kernel_takes_every_shape(axis, shape, periodic, cplx):
     """tdma_solve_shared on what the tiled TMA kernel refuses -- line lengths without a power-of-two tree of
