@@ -423,6 +423,7 @@ def general_shapes(torch, tdma, tdma_inputs, dev, steps, warmup):
             ("y cyclic, staged", (64, 1024, 1024), 16, 16, dict(variant=V["staged"], periodic=1), "y"),
             ("y cyclic, 1000 rows x 1023 (auto -> pipelined)", (64, 1000, 1023), 8, 16, dict(periodic=1), "y"),
             ("x sweep, nx = 1024 (auto -> fused)", (64, 512, 1024), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x"),
+            ("x sweep, nx = 768 (auto -> fused, clusters of 3)", (64, 512, 768), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x"),
             ("x sweep, nx = 1000 (auto -> pipelined)", (64, 512, 1000), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x")]:
         a, b, c, d = tdma_inputs.dominant_random(nx, ny, nz, 7, dev)
         x = torch.full_like(d, float("nan"))

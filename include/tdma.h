@@ -100,7 +100,7 @@ typedef struct tdma_options {
                             assembles the reduced system (the paper's A2B);
                             default 0 = gather fused into stage A's epilogue */
     int fused_lines;     /* FUSED: lines (x extent) per cluster tile (8, 16, 32), 0 = auto */
-    int fused_cluster;   /* FUSED: CTAs per cluster (1, 2, 4, 8, 16), 0 = auto */
+    int fused_cluster;   /* FUSED: CTAs per cluster (1, 2, 4, 8, 16; x sweeps also 3, 5, 6), 0 = auto */
     int fused_leaf_rows; /* FUSED: rows per thread-level leaf (a divisor of ny/P, >= 2), 0 = auto */
     int fused_top;       /* FUSED: 1 = the cluster exchanges / solves the 2P-row reduced system as
                             is; 2 = every CTA first reduces its 2P/cluster rows to two (same
@@ -138,7 +138,7 @@ typedef struct tdma_options {
                             PIPELINED plans round it to whole batches) */
     int shared_lines;    /* tdma_solve_shared: cells along x per tile (real: 16 or 32, complex: 8 or 16),
                             0 = auto (128-byte row segments) */
-    int shared_cluster;  /* tdma_solve_shared: CTAs per cluster (1, 2, 4, 8), 0 = auto */
+    int shared_cluster;  /* tdma_solve_shared: CTAs per cluster (1, 2, 4, 8; x sweeps also 3, 5, 6), 0 = auto */
     int shared_leaf_rows;/* tdma_solve_shared: rows per thread-level leaf (4, 8, 16, 32; 10, 12, 20, 24), 0 = auto */
     int shared_slots;    /* tdma_solve_shared: tiles in the shared-memory ring (2 .. 4), 0 = auto */
     int pdd;             /* PIPELINED / STAGED: 1 = stage B is the Parallel Diagonally Dominant variant

@@ -1210,15 +1210,18 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
     const size_t sm_smem = prop.sharedMemPerMultiprocessor;
     TmaFusedConfig best; double best_score = -1.0;
     const int tx_opts[3] = {16, 32, 8};
-    const int cl_opts[5] = {1, 2, 4, 8, 16};
+    // clusters of 3 / 6 / 5: x sweeps of 3 * 2^k and 5 * 2^k cells (their leaves are whole 128-byte rows of 16 x,
+    // so the odd factor cannot go into the leaf as it does for y / z sweeps)
+    const int cl_opts[8] = {1, 2, 4, 8, 16, 3, 6, 5};
     for (int ti = 0; ti < 3; ++ti) {
         const int TX = tx_opts[ti];
         if (want_lines && TX != want_lines) continue;
         if (!want_lines && TX > 8 && nx < TX) continue;
-        for (int ci = 0; ci < 5; ++ci) {
+        for (int ci = 0; ci < 8; ++ci) {
             const int CL = cl_opts[ci];
             if (want_cluster && CL != want_cluster) continue;
             if (CL > 8 && !want_cluster) continue;
+            if ((CL == 3 || CL == 6 || CL == 5) && !xaxis) continue;
             if (ny % CL) continue;
             const int R = ny / CL;
             for (int m0 : kLeafSizes) {

@@ -891,14 +891,15 @@ inline bool configure_shared_impl(SharedConfig *out, int nx, int ny, int NC, int
     SharedConfig best; double best_score = -1.0;
     // lines per tile: 128-byte row segments first (16 real / 8 complex cells), then 256-byte ones
     const int tx_opts[3] = {NC == 1 ? 16 : 8, NC == 1 ? 32 : 16, NC == 1 ? 8 : 4};
-    const int cl_opts[4] = {1, 2, 4, 8};
+    const int cl_opts[7] = {1, 2, 4, 8, 3, 6, 5};                    // 3, 6, 5: x sweeps of 3 * 2^k / 5 * 2^k cells
     for (int ti = 0; ti < 3; ++ti) {
         const int TX = tx_opts[ti];
         if (want_lines ? TX != want_lines : ti == 2) continue;      // 64-byte segments only on request
         if ((xsweep || uniform) && TX != 16) continue;              // x sweeps: 16 lines of 128-byte leaf rows
-        for (int ci = 0; ci < 4; ++ci) {
+        for (int ci = 0; ci < 7; ++ci) {
             const int CL = cl_opts[ci];
             if (want_cluster && CL != want_cluster) continue;
+            if ((CL == 3 || CL == 6 || CL == 5) && !xsweep) continue;
             if (ny % CL) continue;
             const int R = ny / CL;
             for (int m0 : kSharedLeafSizes) {
