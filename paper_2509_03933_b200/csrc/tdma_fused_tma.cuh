@@ -1221,7 +1221,7 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
             const int CL = cl_opts[ci];
             if (want_cluster && CL != want_cluster) continue;
             if (CL > 8 && !want_cluster) continue;
-            if ((CL == 3 || CL == 6 || CL == 5) && !xaxis) continue;
+            const bool odd_cl = CL == 3 || CL == 6 || CL == 5;
             if (ny % CL) continue;
             const int R = ny / CL;
             for (int m0 : kLeafSizes) {
@@ -1231,6 +1231,11 @@ inline bool configure_tma_fused(TmaFusedConfig *out, int nx, int ny, int P, int 
                 c.lines = TX; c.cluster = CL; c.rows = R; c.leaf_rows = m0; c.leaves = R / m0;
                 c.threads = c.leaves * TX;
                 if (c.threads > 512 || (xaxis && c.threads > 256)) continue;
+                // y / z sweeps of 3 * 2^k and 5 * 2^k rows: a cluster of 3, 6 or 5 that leaves 256 threads with
+                // 16-row leaves (the tiling of the power-of-two lengths) beats leaves of 12 / 10 rows under a
+                // power-of-two cluster (ny = 768: 6.12 against 5.24 TB/s, 1280: 5.48 against 3.79, 384: 6.26
+                // against 5.53, 1536: 5.14 against 4.34); smaller CTAs do not (ny = 640, 128 threads: 3.1 against 4.7)
+                if (odd_cl && !xaxis && want_cluster != CL && !(m0 == 16 && c.threads == 256)) continue;
                 c.nlev = 0;
                 while ((1 << c.nlev) < c.leaves) ++c.nlev;
                 c.box_rows = R;

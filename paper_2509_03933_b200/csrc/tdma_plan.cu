@@ -581,7 +581,10 @@ int init_plan(tdma_plan *pl, const tdma_options *opt)
         pl->sm_count = prop.multiProcessorCount;
         pl->sm_smem = prop.sharedMemPerMultiprocessor;
         pl->fill_opt = opt ? opt->fused_fill : 0;
-        if (have_tma && pl->tfused.cluster >= 4 && pl->fill_opt >= 0) {
+        // clusters of 5 / 6 (3 * 2^k, 5 * 2^k lines): no automatic fill launch -- the cluster-of-2 tiling of
+        // such lengths is slow enough to finish last (ny = 640: 5.08 TB/s without it, 3.39 with it)
+        const bool pow2_cluster = (pl->tfused.cluster & (pl->tfused.cluster - 1)) == 0;
+        if (have_tma && pl->tfused.cluster >= 4 && pl->fill_opt >= 0 && (pow2_cluster || pl->fill_opt > 0)) {
             const char *why2 = nullptr;
             pl->have_fill = tdma::configure_tma_fused(&pl->tfill, pl->nx, pl->ny, pl->P, 0,
                                                       pl->ny % 2 == 0 ? 2 : 1, 0, prop, &why2,

@@ -369,6 +369,32 @@ def test_tma_fused_shapes(shape, P, cluster, lines):
     check_against_oracle(a, b, c, d, x, True)
 
 
+@pytest.mark.parametrize("axis", ["y", "z"])
+@pytest.mark.parametrize("n,P,cluster", [(768, 16, (3, 6)), (384, 8, (3,)), (640, 16, (5,)), (1280, 16, (5,)), (1536, 16, (6,))])
+def test_odd_clusters_for_3_2k_and_5_2k_lines(axis, n, P, cluster):
+    """AUTO on 3 * 2^k / 5 * 2^k line lengths: clusters of 3, 5 or 6 CTAs with 16-row leaves (256 threads), no
+    fill launch; many tiles per cluster, repeated solves with equal bits, parity on the first and last slices."""
+    lanes, nsl = 96, 40
+    shape = (nsl, n, lanes) if axis == "y" else (n, nsl, lanes)
+    a, b, c, d = tdma_inputs.dominant_random(shape[2], shape[1], shape[0], 17, dev())
+    xs = []
+    with tdma.Plan(shape[2], shape[1], shape[0], P, 0, axis=tdma.TDMA_AXIS_Z if axis == "z" else tdma.TDMA_AXIS_Y) as plan:
+        assert plan.get(tdma.TDMA_GET_VARIANT) == tdma.TDMA_VARIANT_FUSED
+        assert plan.get(tdma.TDMA_GET_FUSED_CLUSTER) in cluster and plan.get(tdma.TDMA_GET_FUSED_LEAF_ROWS) == 16
+        for _ in range(4):
+            x = torch.full_like(d, float("nan"))
+            plan.solve(a, b, c, d, x)
+            xs.append(x)
+        torch.cuda.synchronize()
+        assert plan.get(tdma.TDMA_GET_FUSED_FILL) == 0
+    assert all(torch.equal(xs[0], t) for t in xs[1:])
+    an, bn, cn, dn, xn = to_np(a, b, c, d, xs[0])
+    ref = oracle.solve_axis(an, bn, cn, dn, axis, False)
+    ax = 1 if axis == "y" else 0
+    err = (np.max(np.abs(xn - ref), axis=ax) / np.max(np.abs(ref), axis=ax)).max()
+    assert np.isfinite(xn).all() and err <= TOL_E, err
+
+
 def test_tma_fused_unaligned_pointers_fall_back():
     """Arrays that are only 8-byte aligned cannot be described by a tensor map: the plan routes
     the solve to the register-staged kernel instead of failing."""
