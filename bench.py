@@ -422,6 +422,12 @@ def general_shapes(torch, tdma, tdma_inputs, dev, steps, warmup):
             ("y plain, pipelined", (64, 1024, 1024), 16, 16, dict(variant=V["pipelined"]), "y"),
             ("y cyclic, staged", (64, 1024, 1024), 16, 16, dict(variant=V["staged"], periodic=1), "y"),
             ("y cyclic, 1000 rows x 1023 (auto -> pipelined)", (64, 1000, 1023), 8, 16, dict(periodic=1), "y"),
+            ("y sweep, ny = 768 (auto: clusters of 3, 16-row leaves)", (256, 768, 1024), 16, 0, dict(variant=V["fused"]), "y"),
+            ("y sweep, ny = 768, clusters of 4, 12-row leaves", (256, 768, 1024), 16, 0, dict(variant=V["fused"], fused_cluster=4), "y"),
+            ("y sweep, ny = 1280 (auto: clusters of 5, 16-row leaves)", (128, 1280, 1024), 16, 0, dict(variant=V["fused"]), "y"),
+            ("y sweep, ny = 1280, clusters of 8, 10-row leaves", (128, 1280, 1024), 16, 0, dict(variant=V["fused"], fused_cluster=8), "y"),
+            ("z sweep, nz = 640 (auto: clusters of 5)", (640, 256, 1024), 16, 0, dict(variant=V["fused"], axis=tdma.TDMA_AXIS_Z), "z"),
+            ("z sweep, nz = 640, clusters of 4, 10-row leaves", (640, 256, 1024), 16, 0, dict(variant=V["fused"], axis=tdma.TDMA_AXIS_Z, fused_cluster=4), "z"),
             ("x sweep, nx = 1024 (auto -> fused)", (64, 512, 1024), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x"),
             ("x sweep, nx = 768 (auto -> fused, clusters of 3)", (64, 512, 768), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x"),
             ("x sweep, nx = 1000 (auto -> pipelined)", (64, 512, 1000), 8, 8, dict(axis=tdma.TDMA_AXIS_X), "x")]:
@@ -430,7 +436,7 @@ def general_shapes(torch, tdma, tdma_inputs, dev, steps, warmup):
         with tdma.Plan(nx, ny, nz, P, batch, **opts) as plan:
             ms = timed(lambda: plan.solve(a, b, c, d, x))
             variant = plan.get(tdma.TDMA_GET_VARIANT)
-        E = err_axis(a, b, c, d, x, axis, opts.get("periodic", 0), [0, nz - 1])
+        E = err_axis(a, b, c, d, x, axis, opts.get("periodic", 0), [0, (ny if axis == "z" else nz) - 1])
         out["records"].append({"case": name, "shape": [nz, ny, nx], "variant": {1: "pipelined", 2: "fused", 3: "staged"}[variant],
                                "ms": ms, "gbs_40B": 40.0 * nz * ny * nx / ms / 1e6, "E_max": E, "ok": bool(E <= 1e-11)})
         del a, b, c, d, x
